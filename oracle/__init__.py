@@ -1,0 +1,227 @@
+"""CPU oracle of the SSS-GS forward relighting render path -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It shares no code with the CUDA path and never imports it.
+The arithmetic lives in sssgs_oracle.cpp (plain C++, cited against PAPER.md); this file
+only builds it (g++) and marshals numpy arrays.  Scene objects are duck-typed
+(attributes as produced by paper_2408_12282_b200.scenes), nothing is imported from there.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from types import SimpleNamespace
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sssgs_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+GBUF_CH = 16
+CXXFLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-mfma", "-fopenmp", "-shared", "-fPIC"]
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so if missing or older than its source."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", *CXXFLAGS, "-o", _LIB, _SRC])
+    return _LIB
+
+
+class OrcCamera(ctypes.Structure):
+    _fields_ = [("R", ctypes.c_float * 9), ("t", ctypes.c_float * 3),
+                ("fx", ctypes.c_float), ("fy", ctypes.c_float), ("cx", ctypes.c_float),
+                ("cy", ctypes.c_float), ("tan_half_fovx", ctypes.c_float),
+                ("tan_half_fovy", ctypes.c_float), ("width", ctypes.c_int),
+                ("height", ctypes.c_int), ("znear", ctypes.c_float), ("bg", ctypes.c_float * 3)]
+
+
+def _cam(cam) -> OrcCamera:
+    c = OrcCamera()
+    c.R[:] = [float(v) for v in np.asarray(cam.R, np.float32).ravel()]
+    c.t[:] = [float(v) for v in np.asarray(cam.t, np.float32).ravel()]
+    c.fx, c.fy, c.cx, c.cy = cam.fx, cam.fy, cam.cx, cam.cy
+    c.tan_half_fovx, c.tan_half_fovy = cam.tan_half_fovx, cam.tan_half_fovy
+    c.width, c.height, c.znear = int(cam.width), int(cam.height), cam.znear
+    c.bg[:] = [float(v) for v in np.asarray(cam.bg, np.float32).ravel()]
+    return c
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.orc_build_lists.restype = ctypes.c_int64
+        _lib.orc_num_threads.restype = ctypes.c_int
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def mlp_inputs(scene, cam, light_pos) -> np.ndarray:
+    """Step 1: [n, 40+F] float64."""
+    n = int(scene.n)
+    F = int(scene.feat.shape[1]) if scene.feat is not None and scene.feat.ndim == 2 else 0
+    x = np.empty((n, 40 + F), np.float64)
+    feat = _f32(scene.feat) if F else np.zeros((1,), np.float32)
+    lp = _f32(light_pos)
+    c = _cam(cam)
+    lib().orc_mlp_inputs(ctypes.c_int64(n), _p(_f32(scene.means)), _p(_f32(scene.normals)),
+                         _p(_f32(scene.rotations)), _p(_f32(scene.scales)), _p(_f32(scene.vis_sh)),
+                         ctypes.c_int(scene.vis_sh_degree), _p(feat), ctypes.c_int(F),
+                         ctypes.byref(c), _p(lp), _p(x))
+    return x
+
+
+def mlp_forward(x, mlp, mode: int = 0) -> np.ndarray:
+    """Step 2: x [n, in_dim] float64 -> [n, 4] float64.
+    mode 0 = double reference, 1 = bf16-emulating."""
+    x = np.ascontiguousarray(x, np.float64)
+    n = x.shape[0]
+    assert x.shape[1] == mlp.in_dim
+    out = np.empty((n, 4), np.float64)
+    tw = np.asarray(mlp.trunk_width, np.int32)
+    iw = np.asarray(list(mlp.inc_hidden_width) + [0], np.int32)
+    params = _f32(mlp.params)
+    lib().orc_mlp_forward(ctypes.c_int64(n), _p(x), ctypes.c_int(mlp.in_dim),
+                          ctypes.c_int(len(mlp.trunk_width)), _p(tw),
+                          ctypes.c_int(len(mlp.inc_hidden_width)), _p(iw),
+                          ctypes.c_int(mlp.activation), ctypes.c_double(mlp.leaky_slope),
+                          _p(params), ctypes.c_int(mode), _p(out))
+    return out
+
+
+def project(scene, cam, tile=16):
+    """Step 3 (Eq. 2), canonical fp32."""
+    n = int(scene.n)
+    o = SimpleNamespace(
+        visible=np.zeros(n, np.int32), pix=np.zeros((n, 2), np.float32),
+        depth=np.zeros(n, np.float32), conic=np.zeros((n, 3), np.float32),
+        radius=np.zeros(n, np.float32), rect=np.zeros((n, 4), np.int32),
+        touched=np.zeros(n, np.int32))
+    c = _cam(cam)
+    lib().orc_project(ctypes.c_int64(n), _p(_f32(scene.means)), _p(_f32(scene.scales)),
+                      _p(_f32(scene.rotations)), ctypes.byref(c), ctypes.c_int(tile),
+                      ctypes.c_int(tile), _p(o.visible), _p(o.pix), _p(o.depth), _p(o.conic),
+                      _p(o.radius), _p(o.rect), _p(o.touched))
+    o.tiles_x = (cam.width + tile - 1) // tile
+    o.tiles_y = (cam.height + tile - 1) // tile
+    return o
+
+
+def project_f64(scene, cam):
+    n = int(scene.n)
+    cov = np.zeros((n, 3), np.float64)
+    pix = np.zeros((n, 2), np.float64)
+    depth = np.zeros(n, np.float64)
+    c = _cam(cam)
+    lib().orc_project_f64(ctypes.c_int64(n), _p(_f32(scene.means)), _p(_f32(scene.scales)),
+                          _p(_f32(scene.rotations)), ctypes.byref(c), _p(cov), _p(pix), _p(depth))
+    return cov, pix, depth
+
+
+def build_lists(proj):
+    """Step 4: (keys u64 [I], vals u32 [I], ranges u32 [tiles, 2])."""
+    n = proj.touched.shape[0]
+    args = (ctypes.c_int64(n), _p(proj.rect), _p(proj.depth), _p(proj.touched),
+            ctypes.c_int(proj.tiles_x), ctypes.c_int(proj.tiles_y))
+    total = int(lib().orc_build_lists(*args, None, None, None))
+    keys = np.zeros(max(total, 1), np.uint64)
+    vals = np.zeros(max(total, 1), np.uint32)
+    ranges = np.zeros((proj.tiles_x * proj.tiles_y, 2), np.uint32)
+    lib().orc_build_lists(*args, _p(keys), _p(vals), _p(ranges))
+    return keys[:total], vals[:total], ranges
+
+
+def channels(scene, proj, mlp_out) -> np.ndarray:
+    """Per-Gaussian channel values [n, 14] in G-buffer order (channels 0..13)."""
+    n = int(scene.n)
+    ch = np.zeros((n, 14), np.float64)
+    ch[:, 0] = proj.depth
+    ch[:, 1:4] = scene.normals
+    ch[:, 4:7] = scene.base_color
+    ch[:, 7] = scene.roughness
+    ch[:, 8] = scene.metallic
+    ch[:, 9] = scene.subsurface
+    ch[:, 10:14] = mlp_out
+    return ch
+
+
+def composite(scene, cam, proj, ch, order, ranges, tile=16):
+    """Step 5 (tiled: ranges given) or step 7 (brute force: ranges None); Eq. 3 L68-72."""
+    W, H = int(cam.width), int(cam.height)
+    gbuf = np.zeros((H, W, GBUF_CH), np.float64)
+    unstable = np.zeros((H, W), np.uint8)
+    counters = np.zeros(4, np.int64)
+    contrib = np.zeros(max(int(scene.n), 1), np.uint8)
+    order = np.ascontiguousarray(order, np.uint32)
+    rg = np.ascontiguousarray(ranges, np.uint32) if ranges is not None else None
+    lib().orc_composite(ctypes.c_int(W), ctypes.c_int(H), ctypes.c_int(tile), ctypes.c_int(tile),
+                        _p(proj.pix), _p(proj.conic), _p(_f32(scene.opacities)),
+                        _p(np.ascontiguousarray(ch, np.float64)), _p(order),
+                        ctypes.c_int64(order.shape[0]), _p(rg), _p(gbuf), _p(unstable),
+                        _p(counters), _p(contrib))
+    return SimpleNamespace(gbuf=gbuf, unstable=unstable.astype(bool), p_eval=int(counters[0]),
+                           p_blend=int(counters[1]), n_unstable=int(counters[2]),
+                           contrib=contrib[:int(scene.n)].astype(bool))
+
+
+def brute_order(proj) -> np.ndarray:
+    """All visible Gaussians sorted by (depth bits, index) -- the order of step 7."""
+    vis = np.nonzero(proj.visible)[0]
+    bits = proj.depth.view(np.uint32)[vis].astype(np.uint64)
+    key = (bits << np.uint64(32)) | vis.astype(np.uint64)
+    return vis[np.argsort(key, kind="stable")].astype(np.uint32)
+
+
+def shade(cam, light, gbuf, f32: bool = False):
+    """Step 6 (Eq. 4, Eq. 7).  Returns (rgb, aov_diffuse, aov_specular)."""
+    H, W = gbuf.shape[:2]
+    dt = np.float32 if f32 else np.float64
+    rgb = np.zeros((H, W, 3), dt)
+    ad = np.zeros((H, W, 3), dt)
+    as_ = np.zeros((H, W, 3), dt)
+    fn = lib().orc_shade_f32 if f32 else lib().orc_shade
+    c = _cam(cam)
+    fn(ctypes.c_int(W), ctypes.c_int(H), ctypes.byref(c), _p(_f32(light.position)),
+       _p(_f32(light.intensity)), _p(np.ascontiguousarray(gbuf, np.float64)), _p(rgb), _p(ad), _p(as_))
+    return rgb, ad, as_
+
+
+def render_frame(scene, view: int = 0, light: int = 0, mlp_mode: int = 0, mlp_out=None, tile=16,
+                 geometry=None):
+    """Whole path for one (view, light) frame; returns every intermediate.
+    `geometry` = a previous result for the same view (re-uses projection and lists)."""
+    cam = scene.cameras[view]
+    lt = scene.lights[view][light]
+    r = SimpleNamespace()
+    if geometry is None:
+        r.proj = project(scene, cam, tile)
+        r.keys, r.vals, r.ranges = build_lists(r.proj)
+    else:
+        r.proj, r.keys, r.vals, r.ranges = geometry.proj, geometry.keys, geometry.vals, geometry.ranges
+    if mlp_out is None:
+        r.x = mlp_inputs(scene, cam, lt.position)
+        mlp_out = mlp_forward(r.x, scene.mlp, mlp_mode)
+    r.mlp_out = np.asarray(mlp_out, np.float64)
+    r.ch = channels(scene, r.proj, r.mlp_out)
+    r.comp = composite(scene, cam, r.proj, r.ch, r.vals, r.ranges, tile)
+    r.gbuf = r.comp.gbuf
+    r.rgb, r.aov_diffuse, r.aov_specular = shade(cam, lt, r.gbuf)
+    r.n_vis = int(r.proj.visible.sum())
+    r.n_instances = int(r.keys.shape[0])
+    return r

@@ -1,0 +1,160 @@
+"""Pins of the oracle's MLP input assembly and MLP (steps 1-2; Eq. 6,
+L347) against direct formulas, routing weights, a library special case (torch linear
+chain in float64) and the bf16 quantisation bound.  CPU only."""
+import numpy as np
+import torch
+
+import oracle
+from paper_2408_12282_b200 import scenes
+from util import custom_scene, with_mlp_params
+
+
+def _direct_inputs(s, cam, lp):
+    """MLP input row written independently from the formulas of SURVEY 8(c) step 1."""
+    mu = s.means.astype(np.float64)
+    pc = -(cam.R.astype(np.float64).T @ cam.t.astype(np.float64))
+    wi = np.asarray(lp, np.float64)[None] - mu
+    d = np.linalg.norm(wi, axis=1)
+    wi = wi / d[:, None]
+    wo = pc[None] - mu
+    wo = wo / np.linalg.norm(wo, axis=1, keepdims=True)
+    q = s.rotations.astype(np.float64)
+    q = q * np.where(q[:, :1] < 0, -1.0, 1.0)
+    sh = s.vis_sh.astype(np.float64)
+    v = 0.2820948 * sh[:, 0] + 0.4886025 * (sh[:, 1] * wi[:, 1] + sh[:, 2] * wi[:, 2] + sh[:, 3] * wi[:, 0])
+    v = np.clip(v, 0, 1)
+    cols = [s.normals.astype(np.float64), q[:, :2], s.scales.astype(np.float64), wi, wo, d[:, None], v[:, None]]
+    for k in range(4):
+        cols.append(np.sin((2.0 ** k) * np.pi * mu))
+        cols.append(np.cos((2.0 ** k) * np.pi * mu))
+    cols.append(s.feat.astype(np.float64))
+    return np.concatenate(cols, axis=1)
+
+
+def test_input_row_vs_direct_formulas():
+    s = scenes.make_scene(1, n=300)
+    cam, lt = s.cameras[0], s.lights[0][0]
+    x = oracle.mlp_inputs(s, cam, lt.position)
+    assert x.shape == (300, 56)
+    ref = _direct_inputs(s, cam, lt.position)
+    np.testing.assert_allclose(x, ref, rtol=0, atol=1e-12)
+    # unit directions, Fourier identity sin^2+cos^2 = 1
+    np.testing.assert_allclose(np.linalg.norm(x[:, 8:11], axis=1), 1, atol=1e-12)
+    np.testing.assert_allclose(np.linalg.norm(x[:, 11:14], axis=1), 1, atol=1e-12)
+    for k in range(4):
+        np.testing.assert_allclose(x[:, 16 + 6 * k:19 + 6 * k] ** 2 + x[:, 19 + 6 * k:22 + 6 * k] ** 2, 1, atol=1e-12)
+
+
+def test_visibility_closed_form():
+    # c0 = 0.5/Y00, c1 = 0.5 n / 0.4886 gives v = 0.5 + 0.5 n.w_in
+    rng = np.random.default_rng(0)
+    n = 64
+    nr = rng.standard_normal((n, 3))
+    nr /= np.linalg.norm(nr, axis=1, keepdims=True)
+    s = custom_scene(rng.uniform(-1, 1, (n, 3)), 0.05, normals=nr)
+    lp = np.float32([0.3, -2.0, 1.5])
+    x = oracle.mlp_inputs(s, s.cameras[0], lp)
+    wi = lp[None].astype(np.float64) - s.means
+    wi /= np.linalg.norm(wi, axis=1, keepdims=True)
+    np.testing.assert_allclose(x[:, 15], 0.5 + 0.5 * (s.normals.astype(np.float64) * wi).sum(1), atol=2e-7)
+
+
+def test_quaternion_sign_canonical():
+    s = custom_scene([[0, 0, 0], [0, 0, 0]], 0.05, rotations=[[0.5, 0.5, 0.5, 0.5], [-0.5, -0.5, -0.5, -0.5]])
+    x = oracle.mlp_inputs(s, s.cameras[0], np.float32([0, -3, 1]))
+    np.testing.assert_array_equal(x[0, 3:5], x[1, 3:5])
+    np.testing.assert_array_equal(x[0, 3:5], [0.5, 0.5])
+
+
+def test_zero_weights_give_bias_activations():
+    s = scenes.make_scene(1, n=10)
+    layers = s.mlp.unpack()
+    p = np.zeros_like(s.mlp.params)
+    s0 = with_mlp_params(s, p)
+    off = 0
+    bias_sss = np.array([0.3, -0.7, 1.1], np.float32)
+    for (W, b, kind) in layers:
+        off += W.size
+        if kind == "sss":
+            p[off:off + 3] = bias_sss
+        if kind == "inc_out":
+            p[off] = 0.25
+        off += b.size
+    x = oracle.mlp_inputs(s0, s0.cameras[0], s0.lights[0][0].position)
+    for mode in (0, 1):
+        y = oracle.mlp_forward(x, s0.mlp, mode)
+        np.testing.assert_allclose(y[:, :3], np.broadcast_to(1 / (1 + np.exp(-bias_sss.astype(np.float64))), (10, 3)), atol=1e-12)
+        np.testing.assert_allclose(y[:, 3], 0.25, atol=1e-12)
+    p[off - 1] = -0.25  # negative incident bias -> ReLU clamps to 0
+    assert (oracle.mlp_forward(x, s0.mlp, 0)[:, 3] == 0).all()
+
+
+def test_routing_weights_expose_each_input():
+    # 1 trunk layer of width = in_dim with identity weights routes x through a ReLU;
+    # the incident head then picks one coordinate: relu(x_j) is observable for every j.
+    s = custom_scene(np.random.default_rng(1).uniform(-0.8, 0.8, (50, 3)), 0.05, feat_dim=4, trunk=(44,))
+    cam, lp = s.cameras[0], s.lights[0][0].position
+    x = oracle.mlp_inputs(s, cam, lp)
+    ref = _direct_inputs(s, cam, lp)
+    D = 44
+    for j in range(D):
+        for sign in (1.0, -1.0):
+            W0 = sign * np.eye(D, dtype=np.float32)
+            p = np.concatenate([W0.ravel(), np.zeros(D, np.float32),          # trunk
+                                np.zeros(3 * D + 3, np.float32),               # sss head
+                                np.eye(D, dtype=np.float32)[j], np.zeros(1, np.float32)])  # inc out
+            y = oracle.mlp_forward(x, with_mlp_params(s, p).mlp, 0)
+            np.testing.assert_allclose(y[:, 3], np.maximum(sign * ref[:, j], 0), atol=1e-12)
+            np.testing.assert_allclose(y[:, :3], 0.5, atol=1e-12)
+
+
+def _torch_chain(x, mlp):
+    h = torch.from_numpy(x)
+    layers = [(torch.from_numpy(W.astype(np.float64)), torch.from_numpy(b.astype(np.float64)), k) for W, b, k in mlp.unpack()]
+    act = (lambda t: torch.nn.functional.leaky_relu(t, mlp.leaky_slope)) if mlp.activation == scenes.ACT_LEAKY_RELU else torch.relu
+    hi = None
+    for W, b, kind in layers:
+        if kind == "trunk":
+            h = act(torch.nn.functional.linear(h, W, b))
+        elif kind == "sss":
+            sss = torch.sigmoid(torch.nn.functional.linear(h, W, b))
+            hi = h
+        elif kind == "inc_hidden":
+            hi = act(torch.nn.functional.linear(hi, W, b))
+        else:
+            inc = torch.relu(torch.nn.functional.linear(hi, W, b))
+    return torch.cat([sss, inc], 1).numpy()
+
+
+def test_mlp_equals_torch_linear_chain_float64():
+    for cfg in (1, 2, 6):
+        s = scenes.make_scene(cfg, n=400)
+        x = oracle.mlp_inputs(s, s.cameras[0], s.lights[0][0].position)
+        y = oracle.mlp_forward(x, s.mlp, 0)
+        np.testing.assert_allclose(y, _torch_chain(x, s.mlp), rtol=1e-12, atol=1e-12)
+        assert (y[:, 3] > 0).any() and (y[:, :3] > 0).all() and (y[:, :3] < 1).all()
+
+
+def test_bf16_mode_quantisation_bound():
+    # bf16-emulating mode: inputs of every layer rounded to bf16 (8 bits of mantissa); the
+    # SSS outputs (sigmoid) stay within 1e-2 of the reference (BASELINE north_star), the
+    # unbounded incident output within a few 1e-2 (SURVEY 8(c) measured note).
+    for cfg in (2, 3, 6):
+        s = scenes.make_scene(cfg, n=4000)
+        x = oracle.mlp_inputs(s, s.cameras[0], s.lights[0][0].position)
+        y0 = oracle.mlp_forward(x, s.mlp, 0)
+        y1 = oracle.mlp_forward(x, s.mlp, 1)
+        err = np.abs(y1 - y0)
+        assert err[:, :3].max() < 1e-2
+        assert err[:, 3].max() < 6e-2
+        assert err.max() > 1e-6  # the mode really rounds
+    # rounding helper: exactly representable values pass through unchanged
+    xs = np.float64([[1.0, -0.5, 0.00390625, 3.0] + [0.0] * 36])
+    s = custom_scene([[0, 0, 0]], 0.05, trunk=(40,))
+    p = np.concatenate([np.eye(40, dtype=np.float32).ravel(), np.zeros(40, np.float32), np.zeros(123, np.float32),
+                        np.eye(40, dtype=np.float32)[3], np.zeros(1, np.float32)])
+    assert oracle.mlp_forward(xs, with_mlp_params(s, p).mlp, 1)[0, 3] == 3.0
+    xs[0, 3] = 1.0 + 2.0 ** -9  # half a bf16 ulp above 1: ties-to-even rounds to 1
+    assert oracle.mlp_forward(xs, with_mlp_params(s, p).mlp, 1)[0, 3] == 1.0
+    xs[0, 3] = 1.0 + 3 * 2.0 ** -9  # 1.5 ulp: ties-to-even rounds up to 1 + 2 ulp
+    assert oracle.mlp_forward(xs, with_mlp_params(s, p).mlp, 1)[0, 3] == 1.0 + 2.0 ** -7
