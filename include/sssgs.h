@@ -1,0 +1,195 @@
+/* sssgs.h -- C ABI of libsssgs: the forward relighting render path of SSS-GS
+ * ("Subsurface Scattering for 3D Gaussian Splatting", arXiv 2408.12282) on one B200.
+ *
+ * Citations "L<n>" are line numbers of the paper text; "S<k>" are the readings
+ * of points the paper leaves open, listed in DESIGN.md.
+ *
+ * The path (Fig. 2, L87-116):
+ *   1. per Gaussian and per (view, light): the joint MLP
+ *        (L_SSS, L_in) = f_Theta(mu, Sigma, n, w_in, w_out, v)            (Eq. 6; L347)
+ *   2. EWA projection Sigma' = J W Sigma W^T J^T (Eq. 2), tile binning, depth sort,
+ *      front-to-back alpha compositing C = sum_i prod_{j<i}(1-alpha_j) alpha_i c_i (Eq. 3,
+ *      L68-72) of a 16-channel G-buffer (L55, L114)
+ *   3. per-pixel deferred shading (L114): Cook-Torrance/GGX + diffuse (Eq. 4) times the
+ *      learned incident light, blended with the SSS residual (Eq. 7).
+ *
+ * Conventions
+ *   - Every pointer inside sssgs_gaussians / sssgs_mlp / sssgs_out is a DEVICE pointer for
+ *     sssgs_render and a HOST pointer for sssgs_render_host.  cams / lights are HOST arrays.
+ *   - All memory reachable through the argument structs is caller-owned: the library never
+ *     frees it and never keeps a pointer to it after the call's work has finished.
+ *   - Device pointers must be 16-byte aligned; arrays are dense, row-major, fp32 unless noted.
+ *   - Work is enqueued on the given CUDA stream; sssgs_render never synchronises and is
+ *     CUDA-graph-capture safe.  Results are valid once the caller has synchronised the stream.
+ *   - Every function returns 0 (SSSGS_OK) or a negative sssgs_status; no exceptions or aborts
+ *     cross the ABI.  sssgs_last_error() returns a human-readable description.
+ *   - There is no CPU fallback: without an sm_100 device sssgs_create fails (SSSGS_EARCH).
+ */
+#ifndef SSSGS_H_
+#define SSSGS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SSSGS_OK = 0,
+  SSSGS_EINVAL = -1,    /* bad argument (NULL, dimension mismatch, misaligned pointer, ...)   */
+  SSSGS_ECAPACITY = -2, /* a size exceeds what the context was created for                    */
+  SSSGS_ECUDA = -3,     /* a CUDA runtime call failed                                         */
+  SSSGS_EARCH = -4,     /* device is not compute capability 10.x                              */
+  SSSGS_EOVERFLOW = -5  /* (sssgs_render_host only) tile-instance buffer overflowed           */
+} sssgs_status;
+
+enum { SSSGS_ACT_RELU = 0, SSSGS_ACT_LEAKY_RELU = 1 };
+enum { SSSGS_F32 = 0, SSSGS_BF16 = 1 };
+
+/* flags of sssgs_render */
+enum {
+  SSSGS_LIGHTS_PER_CAMERA = 1u /* lights is [n_cam][n_light] (camera c uses its own n_light
+                                  lights) instead of one shared [n_light] list            */
+};
+
+/* indices into sssgs_out.counters (int64 each, per camera: counters[cam*SSSGS_NCOUNTERS + k]) */
+enum {
+  SSSGS_CNT_NVIS = 0,      /* Gaussians that survive projection/culling                       */
+  SSSGS_CNT_INSTANCES = 1, /* I = sum of tiles touched (tile list length, before clamping)   */
+  SSSGS_CNT_OVERFLOW = 2,  /* 1 if I > max_instances: the frame content is then undefined    */
+  SSSGS_CNT_SORT_ERROR = 3,/* non-zero if a look-back wait exceeded its spin bound (bug trap) */
+  SSSGS_NCOUNTERS = 8
+};
+
+#define SSSGS_TILE 16            /* tiles are 16x16 pixels; part of the tile-list contract   */
+#define SSSGS_GBUF_CHANNELS 16   /* see sssgs_out.gbuffer                                    */
+#define SSSGS_MAX_TRUNK 8
+#define SSSGS_MAX_INC_HIDDEN 2
+
+typedef struct sssgs_ctx sssgs_ctx; /* opaque; owns only scratch memory */
+
+typedef struct {
+  int device;             /* CUDA device ordinal                                              */
+  int64_t max_gaussians;  /* largest n of any later call                                      */
+  int max_width, max_height;
+  int64_t max_instances;  /* capacity of the tile-instance list (sum of tiles touched); if it
+                             is exceeded the overflow counter is set, nothing is written out
+                             of bounds, and the frame is undefined (no host sync happens)     */
+  int max_lights_per_pass;/* lights composited per list walk: 1, 4 or 8 (0 -> 8)              */
+  void* workspace;        /* optional caller-allocated device scratch (>= sssgs_workspace_bytes,
+                             256-byte aligned); NULL -> the context allocates its own         */
+  size_t workspace_bytes;
+  uint32_t flags;         /* reserved, must be 0                                              */
+} sssgs_config;
+
+/* Scene: 3D Gaussians {mu, q, s, o} (L59-72) + PBR attributes {b, r, m, n} (L76) +
+ * subsurfaceness (L102) + visibility SH (L110-112) + optional extra MLP feature (S2).       */
+typedef struct {
+  int64_t n;
+  const float* means;      /* [n,3] world space                                               */
+  const float* scales;     /* [n,3] ACTIVATED (exp already applied)                    (L72)  */
+  const float* rotations;  /* [n,4] unit quaternion (w,x,y,z), caller-normalised       (L72)  */
+  const float* opacities;  /* [n]   ACTIVATED, in [0,1]                                (L64)  */
+  const float* normals;    /* [n,3] unit                                               (L76)  */
+  const float* base_color; /* [n,3]                                                    (L76)  */
+  const float* roughness;  /* [n]                                                      (L76)  */
+  const float* metallic;   /* [n]                                                      (L76)  */
+  const float* subsurface; /* [n]   sss in [0,1]                                       (L102) */
+  const float* vis_sh;     /* [n,(deg+1)^2] visibility SH coefficients, real basis
+                              Y00 = .2820948, Y1{-1,0,1} = .4886025 {y,z,x}            (L112) */
+  int vis_sh_degree;       /* 0 or 1                                                          */
+  const float* feat;       /* [n,feat_dim] extra per-Gaussian MLP input, may be NULL if 0     */
+  int feat_dim;            /* 0..88, multiple of 4 (row = 16-byte aligned)                    */
+} sssgs_gaussians;
+
+/* The global MLP Theta (L98-100, L347).  Input row (in_dim = 40 + feat_dim):
+ *   [ n(3) | rot(2) = (q_w,q_x), sign-canonical q_w>=0 | scale(3) | w_in(3) | w_out(3) | d(1) |
+ *     v(1) | gamma(mu)(24) = for k=0..3 [sin(2^k pi mu_xyz), cos(2^k pi mu_xyz)] | feat(F) ]
+ * params: packed fp32 (or bf16), per layer W[out][in] row-major then b[out]; order = trunk
+ * layers, SSS head (3 outputs, sigmoid), incident-head hidden layers, incident output (1,
+ * ReLU).  Hidden layers use `activation`.  Compute is bf16 x bf16 -> fp32 on the tensor cores:
+ * weights and every layer input are rounded to bf16 (RNE); biases stay fp32.
+ * All widths must be multiples of 16 and <= 128.
+ * precomputed_out: if non-NULL the MLP is skipped and these values are used instead
+ * ([n_cam][n_light][n][4], = (L_SSS rgb, L_in)); lets a caller edit the residual (L169) and
+ * lets tests feed the rasteriser reference values.                                           */
+typedef struct {
+  int in_dim;
+  int n_trunk;
+  int trunk_width[SSSGS_MAX_TRUNK];
+  int n_inc_hidden;
+  int inc_hidden_width[SSSGS_MAX_INC_HIDDEN];
+  int activation;    /* SSSGS_ACT_RELU | SSSGS_ACT_LEAKY_RELU */
+  float leaky_slope; /* paper is silent; 0.01 is customary (S14) */
+  int dtype;         /* SSSGS_F32 | SSSGS_BF16: storage type of params */
+  const void* params;
+  size_t params_bytes;
+  const float* precomputed_out;
+} sssgs_mlp;
+
+/* Pinhole camera.  World -> camera: p_c = R p + t (R row-major); the camera looks down +z,
+ * x right, y down; pixel k is centred at integer coordinate k.  Everything is precomputed by
+ * the caller so that no transcendental is evaluated upstream of a sort key.                  */
+typedef struct {
+  float R[9], t[3];
+  float fx, fy, cx, cy, tan_half_fovx, tan_half_fovy;
+  int width, height;
+  float znear;
+  float bg[3];
+} sssgs_camera;
+
+/* Point light at a known position (L110); RGB intensity multiplier (S16). */
+typedef struct {
+  float position[3];
+  float intensity[3];
+} sssgs_light;
+
+/* Outputs; NULL = not wanted.  F = n_cam * n_light frames, frame f = cam * n_light + light.
+ * gbuffer pixel (16 fp32, UN-normalised accumulations of Eq. 3):
+ *   [0] depth [1-3] normal [4-6] base colour [7] roughness [8] metallic [9] sss
+ *   [10-12] L_SSS [13] L_in [14] A = sum of weights [15] final transmittance T.               */
+typedef struct {
+  float* rgb;            /* [F][H][W][3] linear radiance, no tone mapping (S17)               */
+  float* gbuffer;        /* [F][H][W][16]                                                     */
+  float* aov_diffuse;    /* [F][H][W][3] diffuse illumination before base colour      (L320) */
+  float* aov_specular;   /* [F][H][W][3] specular illumination                         (L320) */
+  float* mlp_out;        /* [F][n][4] (L_SSS rgb, L_in) per Gaussian                          */
+  uint64_t* sorted_keys; /* [n_cam][max_instances] tile<<32 | bits(depth), sorted             */
+  uint32_t* sorted_vals; /* [n_cam][max_instances] Gaussian index of each list entry          */
+  uint32_t* tile_ranges; /* [n_cam][tiles_y*tiles_x][2] = [begin,end) of each tile's entries  */
+  int64_t* counters;     /* [n_cam][SSSGS_NCOUNTERS]                                          */
+} sssgs_out;
+
+/* Scratch bytes a context with this configuration needs (0 on invalid configuration). */
+size_t sssgs_workspace_bytes(const sssgs_config* cfg);
+
+/* Create / destroy a context.  destroy is NULL-safe and never frees caller memory. */
+int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out);
+void sssgs_destroy(sssgs_ctx* ctx);
+
+/* Render F = n_cam x n_light frames.  Geometry (projection, sort, tile lists) runs once per
+ * camera; the MLP and the light-dependent channels once per (camera, light); up to
+ * max_lights_per_pass lights share one walk of the tile lists (OLAT sweeps).
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).                                */
+int sssgs_render(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
+                 const sssgs_camera* cams, int n_cam, const sssgs_light* lights, int n_light,
+                 const sssgs_out* out, uint32_t flags, void* cuda_stream);
+
+/* Same call with HOST buffers: copies the scene and parameters to the device, renders, copies
+ * every requested output back and synchronises.  Returns SSSGS_EOVERFLOW if the instance list
+ * overflowed.  (The end-to-end entry point: one host->device crossing per call.)             */
+int sssgs_render_host(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
+                      const sssgs_camera* cams, int n_cam, const sssgs_light* lights, int n_light,
+                      const sssgs_out* out, uint32_t flags);
+
+/* Number of kernels the last sssgs_render / sssgs_render_host call launched. */
+int64_t sssgs_last_launch_count(const sssgs_ctx* ctx);
+
+/* Description of the last error on this context (or of the last failed create if ctx = NULL). */
+const char* sssgs_last_error(const sssgs_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SSSGS_H_ */

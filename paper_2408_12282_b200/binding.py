@@ -1,0 +1,337 @@
+"""Thin ctypes binding of libsssgs (include/sssgs.h): argument marshalling only.
+
+Every step of the render path runs in the CUDA kernels behind the C ABI.  The functions
+keep the ABI's names (`sssgs_create`, `sssgs_render`, `sssgs_render_host`, `sssgs_destroy`);
+`Renderer` is a convenience wrapper that allocates device memory through torch (plumbing) and
+hands raw pointers + the current CUDA stream to `sssgs_render`.
+
+Loading fails loudly if libsssgs.so is missing: there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsssgs.so")
+
+SSSGS_TILE = 16
+SSSGS_GBUF_CHANNELS = 16
+SSSGS_NCOUNTERS = 8
+SSSGS_MAX_TRUNK = 8
+SSSGS_MAX_INC_HIDDEN = 2
+SSSGS_LIGHTS_PER_CAMERA = 1
+SSSGS_F32, SSSGS_BF16 = 0, 1
+(SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
+CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR = 0, 1, 2, 3
+
+EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
+           "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error"]
+
+_f = ctypes.c_float
+_vp = ctypes.c_void_p
+
+
+class sssgs_config(ctypes.Structure):
+    _fields_ = [("device", ctypes.c_int), ("max_gaussians", ctypes.c_int64),
+                ("max_width", ctypes.c_int), ("max_height", ctypes.c_int),
+                ("max_instances", ctypes.c_int64), ("max_lights_per_pass", ctypes.c_int),
+                ("workspace", _vp), ("workspace_bytes", ctypes.c_size_t), ("flags", ctypes.c_uint32)]
+
+
+class sssgs_gaussians(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int64), ("means", _vp), ("scales", _vp), ("rotations", _vp),
+                ("opacities", _vp), ("normals", _vp), ("base_color", _vp), ("roughness", _vp),
+                ("metallic", _vp), ("subsurface", _vp), ("vis_sh", _vp),
+                ("vis_sh_degree", ctypes.c_int), ("feat", _vp), ("feat_dim", ctypes.c_int)]
+
+
+class sssgs_mlp(ctypes.Structure):
+    _fields_ = [("in_dim", ctypes.c_int), ("n_trunk", ctypes.c_int),
+                ("trunk_width", ctypes.c_int * SSSGS_MAX_TRUNK), ("n_inc_hidden", ctypes.c_int),
+                ("inc_hidden_width", ctypes.c_int * SSSGS_MAX_INC_HIDDEN),
+                ("activation", ctypes.c_int), ("leaky_slope", _f), ("dtype", ctypes.c_int),
+                ("params", _vp), ("params_bytes", ctypes.c_size_t), ("precomputed_out", _vp)]
+
+
+class sssgs_camera(ctypes.Structure):
+    _fields_ = [("R", _f * 9), ("t", _f * 3), ("fx", _f), ("fy", _f), ("cx", _f), ("cy", _f),
+                ("tan_half_fovx", _f), ("tan_half_fovy", _f), ("width", ctypes.c_int),
+                ("height", ctypes.c_int), ("znear", _f), ("bg", _f * 3)]
+
+
+class sssgs_light(ctypes.Structure):
+    _fields_ = [("position", _f * 3), ("intensity", _f * 3)]
+
+
+class sssgs_out(ctypes.Structure):
+    _fields_ = [("rgb", _vp), ("gbuffer", _vp), ("aov_diffuse", _vp), ("aov_specular", _vp),
+                ("mlp_out", _vp), ("sorted_keys", _vp), ("sorted_vals", _vp), ("tile_ranges", _vp),
+                ("counters", _vp)]
+
+
+class SssgsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libsssgs error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsssgs.so (never falls back to anything else)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2408_12282_b200.build` "
+                              "(libsssgs has no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.sssgs_workspace_bytes.restype = ctypes.c_size_t
+        L.sssgs_workspace_bytes.argtypes = [ctypes.POINTER(sssgs_config)]
+        L.sssgs_create.restype = ctypes.c_int
+        L.sssgs_create.argtypes = [ctypes.POINTER(sssgs_config), ctypes.POINTER(_vp)]
+        L.sssgs_destroy.restype = None
+        L.sssgs_destroy.argtypes = [_vp]
+        render_args = [_vp, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_mlp),
+                       ctypes.POINTER(sssgs_camera), ctypes.c_int, ctypes.POINTER(sssgs_light),
+                       ctypes.c_int, ctypes.POINTER(sssgs_out), ctypes.c_uint32]
+        L.sssgs_render.restype = ctypes.c_int
+        L.sssgs_render.argtypes = render_args + [_vp]
+        L.sssgs_render_host.restype = ctypes.c_int
+        L.sssgs_render_host.argtypes = render_args
+        L.sssgs_last_launch_count.restype = ctypes.c_int64
+        L.sssgs_last_launch_count.argtypes = [_vp]
+        L.sssgs_last_error.restype = ctypes.c_char_p
+        L.sssgs_last_error.argtypes = [_vp]
+        _lib = L
+    return _lib
+
+
+# ---- the ABI calls, same names --------------------------------------------------------------
+def sssgs_workspace_bytes(cfg: sssgs_config) -> int:
+    return int(lib().sssgs_workspace_bytes(ctypes.byref(cfg)))
+
+
+def sssgs_create(cfg: sssgs_config) -> _vp:
+    h = _vp()
+    rc = lib().sssgs_create(ctypes.byref(cfg), ctypes.byref(h))
+    if rc != SSSGS_OK:
+        raise SssgsError(rc, (lib().sssgs_last_error(None) or b"").decode())
+    return h
+
+
+def sssgs_destroy(ctx) -> None:
+    lib().sssgs_destroy(ctx)
+
+
+def _check(ctx, rc):
+    if rc != SSSGS_OK:
+        raise SssgsError(rc, (lib().sssgs_last_error(ctx) or b"").decode())
+
+
+def sssgs_render(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0, stream=None) -> None:
+    _check(ctx, lib().sssgs_render(ctx, ctypes.byref(g), ctypes.byref(mlp), cams, n_cam, lights, n_light,
+                                   ctypes.byref(out), flags, _vp(stream or 0)))
+
+
+def sssgs_render_host(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0) -> None:
+    _check(ctx, lib().sssgs_render_host(ctx, ctypes.byref(g), ctypes.byref(mlp), cams, n_cam, lights,
+                                        n_light, ctypes.byref(out), flags))
+
+
+def sssgs_last_launch_count(ctx) -> int:
+    return int(lib().sssgs_last_launch_count(ctx))
+
+
+# ---- marshalling helpers ------------------------------------------------------------------------
+def make_camera(cam) -> sssgs_camera:
+    c = sssgs_camera()
+    c.R[:] = [float(v) for v in np.asarray(cam.R, np.float32).ravel()]
+    c.t[:] = [float(v) for v in np.asarray(cam.t, np.float32).ravel()]
+    c.fx, c.fy, c.cx, c.cy = cam.fx, cam.fy, cam.cx, cam.cy
+    c.tan_half_fovx, c.tan_half_fovy = cam.tan_half_fovx, cam.tan_half_fovy
+    c.width, c.height, c.znear = int(cam.width), int(cam.height), cam.znear
+    c.bg[:] = [float(v) for v in np.asarray(cam.bg, np.float32).ravel()]
+    return c
+
+
+def make_light(light) -> sssgs_light:
+    l = sssgs_light()
+    l.position[:] = [float(v) for v in np.asarray(light.position, np.float32)]
+    l.intensity[:] = [float(v) for v in np.asarray(light.intensity, np.float32)]
+    return l
+
+
+def make_mlp(spec, params_ptr, params_bytes, dtype=SSSGS_F32, precomputed_ptr=None) -> sssgs_mlp:
+    m = sssgs_mlp()
+    m.in_dim = spec.in_dim
+    m.n_trunk = len(spec.trunk_width)
+    for i, w in enumerate(spec.trunk_width):
+        m.trunk_width[i] = w
+    m.n_inc_hidden = len(spec.inc_hidden_width)
+    for i, w in enumerate(spec.inc_hidden_width):
+        m.inc_hidden_width[i] = w
+    m.activation = spec.activation
+    m.leaky_slope = spec.leaky_slope
+    m.dtype = dtype
+    m.params = params_ptr
+    m.params_bytes = params_bytes
+    m.precomputed_out = precomputed_ptr
+    return m
+
+
+_FIELDS = ("means", "scales", "rotations", "opacities", "normals", "base_color", "roughness",
+           "metallic", "subsurface", "vis_sh", "feat")
+
+
+def make_gaussians(n, ptrs: dict, vis_sh_degree: int, feat_dim: int) -> sssgs_gaussians:
+    g = sssgs_gaussians()
+    g.n = n
+    for f in _FIELDS:
+        setattr(g, f, ptrs.get(f))
+    g.vis_sh_degree = vis_sh_degree
+    g.feat_dim = feat_dim
+    return g
+
+
+class Renderer:
+    """Device-resident scene + context.  torch is used for memory and streams only."""
+
+    def __init__(self, scene, max_instances: Optional[int] = None, max_lights_per_pass: int = 0,
+                 device: int = 0, max_width: Optional[int] = None, max_height: Optional[int] = None):
+        import torch
+        self.torch = torch
+        self.scene = scene
+        self.device = torch.device("cuda", device)
+        self.n = int(scene.n)
+        W = max_width or max(c.width for c in scene.cameras)
+        H = max_height or max(c.height for c in scene.cameras)
+        self.cfg = sssgs_config()
+        self.cfg.device = device
+        self.cfg.max_gaussians = max(self.n, 1)
+        self.cfg.max_width, self.cfg.max_height = W, H
+        self.cfg.max_instances = int(max_instances if max_instances is not None else max(16 * self.n, 1 << 16))
+        self.cfg.max_lights_per_pass = max_lights_per_pass
+        self.ctx = sssgs_create(self.cfg)
+        self.t = {}
+        for f in _FIELDS:
+            a = np.ascontiguousarray(getattr(scene, f), dtype=np.float32)
+            if a.size == 0:
+                a = np.zeros(4, np.float32)
+            self.t[f] = torch.from_numpy(a).to(self.device)
+        self.params = torch.from_numpy(np.ascontiguousarray(scene.mlp.params, np.float32)).to(self.device)
+        self.feat_dim = int(scene.feat.shape[1]) if scene.feat.ndim == 2 else 0
+        self.g = make_gaussians(self.n, {f: self.t[f].data_ptr() for f in _FIELDS}, scene.vis_sh_degree,
+                                self.feat_dim)
+
+    def close(self):
+        if self.ctx is not None:
+            sssgs_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def alloc_outputs(self, n_cam, n_light, W, H, want: Sequence[str]):
+        torch = self.torch
+        F = n_cam * n_light
+        tiles = ((W + 15) // 16) * ((H + 15) // 16)
+        cap = int(self.cfg.max_instances)
+        shapes = {"rgb": ((F, H, W, 3), torch.float32), "gbuffer": ((F, H, W, 16), torch.float32),
+                  "aov_diffuse": ((F, H, W, 3), torch.float32), "aov_specular": ((F, H, W, 3), torch.float32),
+                  "mlp_out": ((F, max(self.n, 1), 4), torch.float32),
+                  "sorted_keys": ((n_cam, cap), torch.int64), "sorted_vals": ((n_cam, cap), torch.int32),
+                  "tile_ranges": ((n_cam, tiles, 2), torch.int32),
+                  "counters": ((n_cam, SSSGS_NCOUNTERS), torch.int64)}
+        return {k: torch.zeros(shapes[k][0], dtype=shapes[k][1], device=self.device) for k in want}
+
+    def render(self, cams=None, lights=None, want=("rgb",), outputs=None, precomputed=None,
+               lights_per_camera=False, stream=None):
+        """Enqueue one sssgs_render on the current torch stream.  cams: list of scene cameras;
+        lights: list of lights (or list per camera with lights_per_camera).  Returns the dict of
+        output tensors (device)."""
+        torch = self.torch
+        cams = list(cams if cams is not None else self.scene.cameras)
+        if lights is None:
+            lights = self.scene.lights[0]
+        flat = [l for per in lights for l in per] if lights_per_camera else list(lights)
+        n_cam = len(cams)
+        n_light = (len(lights[0]) if lights else 0) if lights_per_camera else len(flat)
+        W, H = cams[0].width, cams[0].height
+        if outputs is None:
+            outputs = self.alloc_outputs(n_cam, n_light, W, H, want)
+        o = sssgs_out()
+        for k, v in outputs.items():
+            setattr(o, k, v.data_ptr())
+        carr = (sssgs_camera * max(n_cam, 1))(*[make_camera(c) for c in cams])
+        larr = (sssgs_light * max(len(flat), 1))(*[make_light(l) for l in flat])
+        pre_ptr = None
+        if precomputed is not None:
+            self._pre = torch.as_tensor(np.ascontiguousarray(precomputed, np.float32)).to(self.device) \
+                if not torch.is_tensor(precomputed) else precomputed
+            pre_ptr = self._pre.data_ptr()
+        m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr)
+        st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
+        sssgs_render(self.ctx, self.g, m, carr, n_cam, larr, n_light, o,
+                     SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0, st)
+        return outputs
+
+    def launch_count(self) -> int:
+        return sssgs_last_launch_count(self.ctx)
+
+
+def render_host(scene, cams=None, lights=None, want=("rgb",), max_instances=None, ctx_holder=None):
+    """sssgs_render_host with numpy (host) buffers; returns dict of numpy outputs.
+    ctx_holder: optional dict to cache the context between calls."""
+    cams = list(cams if cams is not None else scene.cameras)
+    lights = list(lights if lights is not None else scene.lights[0])
+    n = int(scene.n)
+    W, H = cams[0].width, cams[0].height
+    n_cam, n_light = len(cams), len(lights)
+    key = (n, W, H, max_instances)
+    if ctx_holder is not None and ctx_holder.get("key") == key:
+        ctx, cfg = ctx_holder["ctx"], ctx_holder["cfg"]
+    else:
+        cfg = sssgs_config()
+        cfg.device = 0
+        cfg.max_gaussians = max(n, 1)
+        cfg.max_width, cfg.max_height = W, H
+        cfg.max_instances = int(max_instances if max_instances is not None else max(16 * n, 1 << 16))
+        ctx = sssgs_create(cfg)
+        if ctx_holder is not None:
+            if ctx_holder.get("ctx") is not None:
+                sssgs_destroy(ctx_holder["ctx"])
+            ctx_holder.update(key=key, ctx=ctx, cfg=cfg)
+    arrs = {f: np.ascontiguousarray(getattr(scene, f), dtype=np.float32) for f in _FIELDS}
+    feat_dim = int(scene.feat.shape[1]) if scene.feat.ndim == 2 else 0
+    g = make_gaussians(n, {f: arrs[f].ctypes.data if arrs[f].size else None for f in _FIELDS},
+                       scene.vis_sh_degree, feat_dim)
+    params = np.ascontiguousarray(scene.mlp.params, np.float32)
+    m = make_mlp(scene.mlp, params.ctypes.data, params.nbytes)
+    F = n_cam * n_light
+    tiles = ((W + 15) // 16) * ((H + 15) // 16)
+    cap = int(cfg.max_instances)
+    shapes = {"rgb": ((F, H, W, 3), np.float32), "gbuffer": ((F, H, W, 16), np.float32),
+              "aov_diffuse": ((F, H, W, 3), np.float32), "aov_specular": ((F, H, W, 3), np.float32),
+              "mlp_out": ((F, max(n, 1), 4), np.float32), "sorted_keys": ((n_cam, cap), np.uint64),
+              "sorted_vals": ((n_cam, cap), np.uint32), "tile_ranges": ((n_cam, tiles, 2), np.uint32),
+              "counters": ((n_cam, SSSGS_NCOUNTERS), np.int64)}
+    outs = {k: np.zeros(shapes[k][0], shapes[k][1]) for k in want}
+    o = sssgs_out()
+    for k, v in outs.items():
+        setattr(o, k, v.ctypes.data)
+    carr = (sssgs_camera * max(n_cam, 1))(*[make_camera(c) for c in cams])
+    larr = (sssgs_light * max(n_light, 1))(*[make_light(l) for l in lights])
+    try:
+        sssgs_render_host(ctx, g, m, carr, n_cam, larr, n_light, o, 0)
+    finally:
+        if ctx_holder is None:
+            sssgs_destroy(ctx)
+    return outs

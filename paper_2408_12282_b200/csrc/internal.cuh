@@ -1,0 +1,141 @@
+// Internal declarations shared by the kernels of libsssgs (never installed; not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sssgs.h"
+
+namespace sssgs {
+
+// ---- constants of the method (S4) -----------------------------------
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kAlphaMax = 0.99f;
+constexpr float kTMin = 1e-4f;
+constexpr float kLowPass = 0.3f;
+constexpr float kFrustumClamp = 1.3f;
+constexpr float kDiscFloor = 0.1f;
+constexpr float kRadiusSigma = 3.33f;
+constexpr int kTile = SSSGS_TILE;
+
+// ---- radix sort geometry --------------------------------------------------------------------
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 15;
+constexpr int kSortTile = kSortThreads * kSortItems;  // keys per ticket
+constexpr int kRadixMax = 256;
+constexpr uint32_t kFlagAgg = 1u << 30;  // look-back status: aggregate of this tile only
+constexpr uint32_t kFlagInc = 2u << 30;  // inclusive prefix up to and including this tile
+constexpr uint32_t kFlagMask = 3u << 30;
+constexpr uint32_t kValMask = ~kFlagMask;
+constexpr int kSpinLimit = 1 << 24;  // bug trap for look-back waits (sets SSSGS_CNT_SORT_ERROR)
+
+// ---- emit (scan + expand) geometry ----------------------------------------------------------
+constexpr int kEmitThreads = 256;
+constexpr int kEmitItems = 4;
+constexpr int kEmitChunk = kEmitThreads * kEmitItems;  // Gaussians per ticket
+
+struct CamParams {   // device copy of sssgs_camera plus derived values
+  float R[9], t[3];
+  float fx, fy, cx, cy, tanx, tany;
+  int width, height;
+  float znear;
+  float bg[3];
+  float pos[3];      // camera position in world space = -R^T t
+  int tiles_x, tiles_y;
+};
+
+struct LightParams {
+  float pos[3];
+  float intensity[3];
+};
+
+constexpr int kMaxLightsPerPass = 8;
+struct LightBatch {
+  LightParams l[kMaxLightsPerPass];
+};
+
+// Device counters (uint32 each), zeroed once per camera.
+enum {
+  DC_NVIS = 0,
+  DC_INSTANCES = 1,   // total I (unclamped)
+  DC_OVERFLOW = 2,
+  DC_SORT_ERROR = 3,
+  DC_TICKET_BASE = 8, // tickets: one per ticketed kernel launch
+  DC_WORDS = 32
+};
+
+// Geometry buffers of one camera view.
+struct GeomBuffers {
+  float4* rec_a;      // [n] (pix_x, pix_y, depth, radius)
+  float4* rec_b;      // [n] (conic a, conic b, conic c, opacity)
+  uint2* rect;        // [n] packed tile rect: x = x0 | x1<<16, y = y0 | y1<<16
+  uint32_t* touched;  // [n]
+  uint32_t* dkeys[2]; // [n] depth keys ping/pong
+  uint32_t* dvals[2]; // [n] Gaussian index ping/pong
+  uint32_t* ikeys[2]; // [cap] tile id of each instance ping/pong
+  uint32_t* ivals[2]; // [cap] Gaussian index of each instance ping/pong
+  uint2* ranges;      // [tiles]
+  uint32_t* hist;     // [6][256] digit histograms: 4 depth passes + 2 tile passes
+  uint32_t* status;   // look-back status words, carved per pass
+  uint32_t* counters; // [DC_WORDS]
+};
+
+// ---- MLP description on the device ----------------------------------------------------------
+constexpr int kMlpMaxStages = SSSGS_MAX_TRUNK + SSSGS_MAX_INC_HIDDEN + 1;
+enum { ST_HIDDEN = 0, ST_HEAD_JOINT = 1, ST_HEAD_SPLIT_A = 2, ST_HEAD_SPLIT_B = 3 };
+struct MlpStage {
+  int k_pad;        // padded input width (multiple of 16)
+  int n_pad;        // padded output width (multiple of 16)
+  int n_act;        // outputs that go through the hidden activation and feed the next stage
+  int type;
+  int w_off;        // byte offset of this stage's packed bf16 weights in the blob
+  int b_off;        // float offset of this stage's bias vector (n_pad floats) in the bias block
+  // where the rows come from in the caller's packed parameter array (element offsets):
+  // rows [0, src_rows[0]) from source 0, rows [src_rows[0], src_rows[0]+src_rows[1]) from source 1
+  int src_w[2], src_b[2], src_rows[2];
+  int src_k;        // un-padded input width (row length of the source matrices)
+};
+struct MlpPlan {
+  int n_stages;
+  int in_dim, in_pad;
+  int feat_dim;
+  int activation;
+  float leaky_slope;
+  int blob_bytes;   // packed weights (all stages), multiple of 1024
+  int bias_floats;
+  int max_n;        // widest n_pad
+  int max_k_bytes;  // bytes of the largest A tile (128 rows)
+  MlpStage st[kMlpMaxStages];
+};
+
+// ---- launchers (each enqueues on `s`, returns the number of kernels launched) ---------------
+int launch_pack_attr(const sssgs_gaussians& g, float4* attr, cudaStream_t s);
+int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb,
+                   cudaStream_t s);
+int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t* keys_out,
+                     uint32_t* vals_out, const uint32_t* count_ptr, uint32_t count_cap, int shift,
+                     int bits, const uint32_t* hist, uint32_t* status, uint32_t* ticket,
+                     uint32_t* err, int max_blocks, cudaStream_t s);
+int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_idx,
+                uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
+                uint32_t* status, uint32_t* ticket, cudaStream_t s);
+int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
+                  uint32_t cap, uint2* ranges_user, cudaStream_t s);
+int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_vals,
+                        const GeomBuffers& gb, uint32_t cap, uint64_t* keys_out, uint32_t* vals_out,
+                        int64_t* counters_out, cudaStream_t s);
+int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
+                    cudaStream_t s);
+int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
+               const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
+               float4* out_internal, float* out_user, int64_t user_light_stride, int num_sms,
+               cudaStream_t s);
+int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,
+                              float4* out_internal, cudaStream_t s);
+int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
+                  const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
+                  const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
+                  int64_t frame_stride_px, cudaStream_t s);
+
+int mlp_smem_bytes(const MlpPlan& plan);
+
+}  // namespace sssgs

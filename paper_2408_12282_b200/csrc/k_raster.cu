@@ -1,0 +1,282 @@
+// Tile rasteriser fused with deferred shading (hot-path steps a7 + a8).
+//
+// Front-to-back alpha compositing of every property channel (Eq. 3; "we
+// accumulate and rasterize each property on the image plane in a deferred shading pipeline",
+// L55), then per-pixel shading from the accumulators still in registers (L114): back-project the
+// pixel, Cook-Torrance/GGX + diffuse (Eq. 4) times the learned incident light, blended
+// with the SSS residual (Eq. 7).  Up to LB lights share one walk of the tile list:
+// the compositing weights T_i alpha_i do not depend on the light, only the four MLP channels
+// do (OLAT sweeps, L301).
+//
+// One CTA per 16x16 tile, one thread per pixel (a warp covers an 8x4 pixel block).  List
+// entries are staged in shared memory in batches of 128 as component-major float4 arrays
+// (gathered with 128-bit loads, all threads sharing the work), and every lane reads them back
+// as broadcasts.  Outputs are written once: RGB, and on request the 16-channel G-buffer
+// (4 x 128-bit stores per pixel) and the diffuse / specular AOVs (L320).  Nothing else goes
+// to HBM: the G-buffer round trip of a separate shading pass is avoided.
+#include "internal.cuh"
+
+namespace sssgs {
+
+namespace {
+
+constexpr int kBatch = 128;
+constexpr int kRasterThreads = 256;
+constexpr float kPi = 3.14159265358979323846f;
+
+struct ShadeIn {
+  float depth, nx, ny, nz, br, bg, bb, rough, metal, sss;  // already divided by coverage A
+};
+
+// Deferred shading of one pixel for one light.  fp32 restatement of DESIGN.md "Shading".
+__device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3], float lin,
+                                            float A, int px, int py, const CamParams& cam,
+                                            const LightParams& lt, float rgb[3], float dif[3],
+                                            float spc[3]) {
+  // back-projection of the pixel at depth q.depth, camera -> world: x = R^T (x_c - t)
+  const float xc0 = ((float)px - cam.cx) / cam.fx * q.depth - cam.t[0];
+  const float xc1 = ((float)py - cam.cy) / cam.fy * q.depth - cam.t[1];
+  const float xc2 = q.depth - cam.t[2];
+  float xw[3], l[3], v[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    xw[k] = cam.R[0 + k] * xc0 + cam.R[3 + k] * xc1 + cam.R[6 + k] * xc2;
+    l[k] = lt.pos[k] - xw[k];
+    v[k] = cam.pos[k] - xw[k];
+  }
+  const float il = rsqrtf(l[0] * l[0] + l[1] * l[1] + l[2] * l[2]);
+  const float iv = rsqrtf(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    l[k] *= il;
+    v[k] *= iv;
+  }
+  float brdf[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+  for (int c = 0; c < 3; ++c) dif[c] = spc[c] = 0.f;
+  const float nn2 = q.nx * q.nx + q.ny * q.ny + q.nz * q.nz;
+  if (nn2 >= 1e-16f) {
+    const float in = rsqrtf(nn2);
+    const float n[3] = {q.nx * in, q.ny * in, q.nz * in};
+    float h[3] = {l[0] + v[0], l[1] + v[1], l[2] + v[2]};
+    const float hl2 = h[0] * h[0] + h[1] * h[1] + h[2] * h[2];
+    if (hl2 >= 1e-16f) {
+      const float ih = rsqrtf(hl2);
+      h[0] *= ih; h[1] *= ih; h[2] *= ih;
+    } else {
+      h[0] = n[0]; h[1] = n[1]; h[2] = n[2];
+    }
+    const float nl = fmaxf(0.f, n[0] * l[0] + n[1] * l[1] + n[2] * l[2]);
+    const float nv = fmaxf(1e-4f, n[0] * v[0] + n[1] * v[1] + n[2] * v[2]);
+    const float nh = fminf(1.f, fmaxf(0.f, n[0] * h[0] + n[1] * h[1] + n[2] * h[2]));
+    const float vh = fminf(1.f, fmaxf(0.f, v[0] * h[0] + v[1] * h[1] + v[2] * h[2]));
+    const float ar = fmaxf(1e-3f, q.rough * q.rough);
+    const float a2 = ar * ar;
+    // cancellation-free GGX: 1 - nh^2 = |n x h|^2
+    const float cx = n[1] * h[2] - n[2] * h[1], cy = n[2] * h[0] - n[0] * h[2],
+                cz = n[0] * h[1] - n[1] * h[0];
+    const float s2 = cx * cx + cy * cy + cz * cz;
+    const float dd = a2 * nh * nh + s2;
+    const float D = a2 / (kPi * dd * dd);
+    const float k = 0.5f * ar;
+    const float V = 1.f / (4.f * (nl * (1.f - k) + k) * (nv * (1.f - k) + k));
+    const float om = 1.f - vh;
+    const float om2 = om * om;
+    const float om5 = om2 * om2 * om;
+    const float base[3] = {q.br, q.bg, q.bb};
+    const float lnl = lin * nl;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float F0 = 0.04f * (1.f - q.metal) + base[c] * q.metal;
+      const float F = F0 + (1.f - F0) * om5;
+      const float fs = D * F * V;
+      const float fd = (1.f - q.metal) * base[c] / kPi;
+      brdf[c] = (fs + fd) * lnl;
+      spc[c] = (1.f - q.sss) * fs * lnl;
+      dif[c] = (1.f - q.sss) * (1.f - q.metal) / kPi * lnl;
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const float lout = q.sss * lsss[c] + (1.f - q.sss) * brdf[c];
+    rgb[c] = lt.intensity[c] * A * lout + (1.f - A) * cam.bg[c];
+  }
+}
+
+template <int LB>
+__global__ void __launch_bounds__(kRasterThreads)
+raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
+                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ sorted_vals,
+                    const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
+                    const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
+                    float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
+                    float* __restrict__ aovd_out, float* __restrict__ aovs_out,
+                    int64_t frame_stride_px) {
+  constexpr int NC = 5 + LB;  // float4 components per list entry
+  __shared__ float4 s_c[NC][kBatch];
+  __shared__ uint32_t s_id[kBatch];
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tile = blockIdx.x;
+  const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
+  // warp -> 8x4 pixel block of the 16x16 tile; lane -> pixel inside the block
+  const int px = tx * kTile + (warp & 1) * 8 + (lane & 7);
+  const int py = ty * kTile + (warp >> 1) * 4 + (lane >> 3);
+  const bool inside = px < cam.width && py < cam.height;
+  const float fpx = (float)px, fpy = (float)py;
+
+  const uint2 range = ranges[tile];
+  float T = 1.f, A = 0.f;
+  float acc[10];
+  float accl[LB][4];
+#pragma unroll
+  for (int c = 0; c < 10; ++c) acc[c] = 0.f;
+#pragma unroll
+  for (int l = 0; l < LB; ++l)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) accl[l][c] = 0.f;
+  bool done = !inside;
+
+  for (uint32_t base = range.x; base < range.y; base += kBatch) {
+    if (__syncthreads_and(done)) break;  // also: previous batch fully consumed
+    const int cnt = min((uint32_t)kBatch, range.y - base);
+    if (tid < cnt) s_id[tid] = sorted_vals[base + tid];
+    __syncthreads();
+    for (int q = tid; q < NC * kBatch; q += kRasterThreads) {
+      const int comp = q / kBatch, e = q % kBatch;
+      if (e < cnt) {
+        const uint32_t g = s_id[e];
+        float4 v;
+        if (comp == 0) v = rec_a[g];
+        else if (comp == 1) v = rec_b[g];
+        else if (comp < 5) v = attr[3 * (size_t)g + (comp - 2)];
+        else v = (comp - 5 < n_lights) ? mlp_out[(size_t)g * n_lights + (comp - 5)]
+                                       : make_float4(0.f, 0.f, 0.f, 0.f);
+        s_c[comp][e] = v;
+      }
+    }
+    __syncthreads();
+    if (!done) {
+      for (int j = 0; j < cnt; ++j) {
+        const float4 ra = s_c[0][j];
+        const float4 rb = s_c[1][j];
+        const float dx = fpx - ra.x, dy = fpy - ra.y;
+        const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
+        if (power > 0.f) continue;
+        const float alpha = fminf(kAlphaMax, rb.w * __expf(power));
+        if (alpha < kAlphaMin) continue;
+        const float Tn = T * (1.f - alpha);
+        if (Tn < kTMin) {
+          done = true;
+          break;
+        }
+        const float w = alpha * T;
+        const float4 a0 = s_c[2][j], a1 = s_c[3][j], a2 = s_c[4][j];
+        acc[0] = fmaf(w, ra.z, acc[0]);
+        acc[1] = fmaf(w, a0.x, acc[1]);
+        acc[2] = fmaf(w, a0.y, acc[2]);
+        acc[3] = fmaf(w, a0.z, acc[3]);
+        acc[4] = fmaf(w, a1.x, acc[4]);
+        acc[5] = fmaf(w, a1.y, acc[5]);
+        acc[6] = fmaf(w, a1.z, acc[6]);
+        acc[7] = fmaf(w, a0.w, acc[7]);
+        acc[8] = fmaf(w, a1.w, acc[8]);
+        acc[9] = fmaf(w, a2.x, acc[9]);
+#pragma unroll
+        for (int l = 0; l < LB; ++l) {
+          const float4 m = s_c[5 + l][j];
+          accl[l][0] = fmaf(w, m.x, accl[l][0]);
+          accl[l][1] = fmaf(w, m.y, accl[l][1]);
+          accl[l][2] = fmaf(w, m.z, accl[l][2]);
+          accl[l][3] = fmaf(w, m.w, accl[l][3]);
+        }
+        A += w;
+        T = Tn;
+      }
+    }
+  }
+
+  if (!inside) return;
+  // ---- epilogue: G-buffer stores + deferred shading, per light ---------------------------------
+  const int64_t pidx = (int64_t)py * cam.width + px;
+  ShadeIn q;
+  const bool covered = A >= 1e-6f;
+  const float iA = covered ? 1.f / A : 0.f;
+  q.depth = acc[0] * iA; q.nx = acc[1] * iA; q.ny = acc[2] * iA; q.nz = acc[3] * iA;
+  q.br = acc[4] * iA; q.bg = acc[5] * iA; q.bb = acc[6] * iA;
+  q.rough = acc[7] * iA; q.metal = acc[8] * iA; q.sss = acc[9] * iA;
+#pragma unroll
+  for (int l = 0; l < LB; ++l) {
+    if (l >= n_lights) break;
+    const int64_t fp = (int64_t)l * frame_stride_px + pidx;
+    if (gbuf_out) {
+      float4* gp = reinterpret_cast<float4*>(gbuf_out + fp * SSSGS_GBUF_CHANNELS);
+      gp[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      gp[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      gp[2] = make_float4(acc[8], acc[9], accl[l][0], accl[l][1]);
+      gp[3] = make_float4(accl[l][2], accl[l][3], A, T);
+    }
+    float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
+    if (covered) {
+      const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
+      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc);
+    } else {
+      rgb[0] = cam.bg[0]; rgb[1] = cam.bg[1]; rgb[2] = cam.bg[2];
+    }
+    if (rgb_out) {
+      float* o = rgb_out + fp * 3;
+      o[0] = rgb[0]; o[1] = rgb[1]; o[2] = rgb[2];
+    }
+    if (aovd_out) {
+      float* o = aovd_out + fp * 3;
+      o[0] = dif[0]; o[1] = dif[1]; o[2] = dif[2];
+    }
+    if (aovs_out) {
+      float* o = aovs_out + fp * 3;
+      o[0] = spc[0]; o[1] = spc[1]; o[2] = spc[2];
+    }
+  }
+}
+
+// Copies caller-supplied MLP outputs ([n_light][n][4], light stride given) into the internal
+// [n][n_lights] float4 layout the rasteriser gathers from.
+__global__ void __launch_bounds__(256)
+gather_precomputed_kernel(const float4* __restrict__ pre, int64_t n, int n_lights,
+                          int64_t light_stride_f4, float4* __restrict__ out) {
+  const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n * n_lights) return;
+  const int64_t g = i / n_lights;
+  const int l = (int)(i % n_lights);
+  out[i] = pre[(int64_t)l * light_stride_f4 + g];
+}
+
+}  // namespace
+
+int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,
+                              float4* out_internal, cudaStream_t s) {
+  if (n == 0) return 0;
+  const int64_t total = n * n_lights;
+  gather_precomputed_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(
+      reinterpret_cast<const float4*>(pre), n, n_lights, light_stride / 4, out_internal);
+  return 1;
+}
+
+int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
+                  const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
+                  const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
+                  int64_t frame_stride_px, cudaStream_t s) {
+  const int tiles = cam.tiles_x * cam.tiles_y;
+  if (tiles == 0) return 0;
+#define SSSGS_RASTER(LB)                                                                        \
+  raster_shade_kernel<LB><<<tiles, kRasterThreads, 0, s>>>(cam, lights, n_lights, gb.ranges,    \
+                                                           sorted_vals, gb.rec_a, gb.rec_b, attr, \
+                                                           mlp_out, rgb, gbuf, aov_d, aov_s,     \
+                                                           frame_stride_px)
+  if (n_lights <= 1) SSSGS_RASTER(1);
+  else if (n_lights <= 4) SSSGS_RASTER(4);
+  else SSSGS_RASTER(8);
+#undef SSSGS_RASTER
+  return 1;
+}
+
+}  // namespace sssgs

@@ -1,0 +1,506 @@
+// Host side of libsssgs: context, argument validation, workspace carving, MLP plan, and the
+// orchestration of one sssgs_render call (hot-path step a9: geometry once per camera, MLP +
+// light channels + shading per light batch; PAPER.md L301 OLAT sweeps).  No CPU fallback exists:
+// every step of the path runs in the kernels of this directory.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "internal.cuh"
+
+using namespace sssgs;
+
+struct sssgs_ctx {
+  sssgs_config cfg;
+  int num_sms = 0;
+  int max_lb = 8;
+  uint8_t* ws = nullptr;       // workspace base
+  bool owns_ws = false;
+  size_t ws_bytes = 0;
+  // carved pointers
+  float4* attr = nullptr;
+  GeomBuffers gb{};
+  uint8_t* control = nullptr;  // zeroed once per camera
+  size_t control_bytes = 0;
+  uint32_t* status_depth[4] = {};
+  uint32_t* status_tile[2] = {};
+  uint32_t* status_emit = nullptr;
+  float4* mlp_out = nullptr;
+  uint8_t* mlp_blob = nullptr;
+  float* mlp_bias = nullptr;
+  int64_t launches = 0;
+  // device staging of sssgs_render_host (grown on demand, owned)
+  std::vector<std::pair<void*, size_t>> staging;
+  std::string err;
+};
+
+namespace {
+
+std::string g_create_err;
+
+constexpr size_t kMaxBlobBytes = 512 * 1024;
+constexpr size_t kMaxBiasFloats = 4096;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int fail(sssgs_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf; else g_create_err = buf;
+  return code;
+}
+
+bool config_ok(const sssgs_config* cfg) {
+  if (!cfg) return false;
+  if (cfg->max_gaussians < 0 || cfg->max_gaussians > (int64_t)1 << 30) return false;
+  if (cfg->max_width <= 0 || cfg->max_height <= 0) return false;
+  if (cfg->max_width > 65535 * kTile || cfg->max_height > 65535 * kTile) return false;
+  const int64_t tiles = (int64_t)((cfg->max_width + kTile - 1) / kTile) * ((cfg->max_height + kTile - 1) / kTile);
+  if (tiles > 65536) return false;  // tile ids are sorted with at most two 8-bit digits
+  if (cfg->max_instances < 0 || cfg->max_instances >= (int64_t)1 << 30) return false;
+  const int lb = cfg->max_lights_per_pass;
+  if (!(lb == 0 || lb == 1 || lb == 4 || lb == 8)) return false;
+  if (cfg->flags != 0) return false;
+  return true;
+}
+
+// Carves the workspace; with base == nullptr only computes the size.
+size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> uint8_t* {
+    uint8_t* p = base ? base + off : nullptr;
+    off += align_up(bytes ? bytes : 16, 256);
+    return p;
+  };
+  const size_t n = (size_t)cfg.max_gaussians, cap = (size_t)cfg.max_instances;
+  const size_t tiles = (size_t)((cfg.max_width + kTile - 1) / kTile) * ((cfg.max_height + kTile - 1) / kTile);
+  const int lb = cfg.max_lights_per_pass ? cfg.max_lights_per_pass : 8;
+  uint8_t* p;
+  p = take(n * 48); if (c) c->attr = (float4*)p;
+  p = take(n * 16); if (c) c->gb.rec_a = (float4*)p;
+  p = take(n * 16); if (c) c->gb.rec_b = (float4*)p;
+  p = take(n * 8);  if (c) c->gb.rect = (uint2*)p;
+  p = take(n * 4);  if (c) c->gb.touched = (uint32_t*)p;
+  for (int k = 0; k < 2; ++k) { p = take(n * 4); if (c) c->gb.dkeys[k] = (uint32_t*)p; }
+  for (int k = 0; k < 2; ++k) { p = take(n * 4); if (c) c->gb.dvals[k] = (uint32_t*)p; }
+  for (int k = 0; k < 2; ++k) { p = take(cap * 4); if (c) c->gb.ikeys[k] = (uint32_t*)p; }
+  for (int k = 0; k < 2; ++k) { p = take(cap * 4); if (c) c->gb.ivals[k] = (uint32_t*)p; }
+  p = take(tiles * 8); if (c) c->gb.ranges = (uint2*)p;
+  p = take(n * (size_t)lb * 16); if (c) c->mlp_out = (float4*)p;
+  p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
+  p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
+  // control block: everything that must be zero at the start of a camera
+  const size_t ctrl_begin = off;
+  if (c) c->control = base ? base + off : nullptr;
+  p = take(6 * 256 * 4); if (c) c->gb.hist = (uint32_t*)p;
+  p = take(DC_WORDS * 4); if (c) c->gb.counters = (uint32_t*)p;
+  const size_t nblk_d = (n + kSortTile - 1) / kSortTile, nblk_i = (cap + kSortTile - 1) / kSortTile;
+  for (int k = 0; k < 4; ++k) { p = take(nblk_d * kRadixMax * 4); if (c) c->status_depth[k] = (uint32_t*)p; }
+  for (int k = 0; k < 2; ++k) { p = take(nblk_i * kRadixMax * 4); if (c) c->status_tile[k] = (uint32_t*)p; }
+  p = take(((n + kEmitChunk - 1) / kEmitChunk) * 4); if (c) c->status_emit = (uint32_t*)p;
+  if (c) c->control_bytes = off - ctrl_begin;
+  return off;
+}
+
+bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+// Builds the tensor-core stage list of the MLP.
+int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
+  if (m.in_dim != 40 + feat_dim) return fail(c, SSSGS_EINVAL, "mlp.in_dim %d != 40 + feat_dim %d", m.in_dim, feat_dim);
+  if (m.n_trunk < 1 || m.n_trunk > SSSGS_MAX_TRUNK) return fail(c, SSSGS_EINVAL, "mlp.n_trunk out of range");
+  if (m.n_inc_hidden < 0 || m.n_inc_hidden > SSSGS_MAX_INC_HIDDEN) return fail(c, SSSGS_EINVAL, "mlp.n_inc_hidden out of range");
+  if (m.activation != SSSGS_ACT_RELU && m.activation != SSSGS_ACT_LEAKY_RELU) return fail(c, SSSGS_EINVAL, "mlp.activation");
+  if (m.dtype != SSSGS_F32 && m.dtype != SSSGS_BF16) return fail(c, SSSGS_EINVAL, "mlp.dtype");
+  for (int l = 0; l < m.n_trunk; ++l)
+    if (m.trunk_width[l] < 16 || m.trunk_width[l] > 128 || m.trunk_width[l] % 16) return fail(c, SSSGS_EINVAL, "trunk width must be a multiple of 16 in [16,128]");
+  for (int l = 0; l < m.n_inc_hidden; ++l)
+    if (m.inc_hidden_width[l] < 16 || m.inc_hidden_width[l] > 128 || m.inc_hidden_width[l] % 16) return fail(c, SSSGS_EINVAL, "incident hidden width must be a multiple of 16 in [16,128]");
+  memset(plan, 0, sizeof *plan);
+  plan->in_dim = m.in_dim;
+  plan->in_pad = (m.in_dim + 15) / 16 * 16;
+  plan->feat_dim = feat_dim;
+  plan->activation = m.activation;
+  plan->leaky_slope = m.leaky_slope;
+  int off = 0;       // element offset into params
+  int d = m.in_dim;  // current un-padded input width
+  int ns = 0, w_off = 0, b_off = 0, max_kb = 0, max_n = 0;
+  auto add = [&](int type, int k, int n_pad, int n_act) -> MlpStage& {
+    MlpStage& st = plan->st[ns++];
+    st.type = type;
+    st.k_pad = (k + 15) / 16 * 16;
+    st.n_pad = n_pad;
+    st.n_act = n_act;
+    st.src_k = k;
+    st.w_off = w_off;
+    st.b_off = b_off;
+    const int kblocks = (st.k_pad + 63) / 64;
+    w_off += kblocks * n_pad * 128;
+    b_off += n_pad;
+    if (kblocks > max_kb) max_kb = kblocks;
+    if (n_pad > max_n) max_n = n_pad;
+    st.src_w[0] = st.src_w[1] = st.src_b[0] = st.src_b[1] = 0;
+    st.src_rows[0] = st.src_rows[1] = 0;
+    return st;
+  };
+  for (int l = 0; l < m.n_trunk; ++l) {
+    const int o = m.trunk_width[l];
+    MlpStage& st = add(ST_HIDDEN, d, o, o);
+    st.src_w[0] = off; st.src_b[0] = off + o * d; st.src_rows[0] = o;
+    off += o * d + o;
+    d = o;
+  }
+  const int sss_w = off, sss_b = off + 3 * d;
+  off += 3 * d + 3;
+  if (m.n_inc_hidden == 0) {
+    MlpStage& st = add(ST_HEAD_JOINT, d, 16, 0);
+    st.src_w[0] = sss_w; st.src_b[0] = sss_b; st.src_rows[0] = 3;
+    st.src_w[1] = off; st.src_b[1] = off + d; st.src_rows[1] = 1;
+    off += d + 1;
+  } else {
+    int di = d;
+    for (int l = 0; l < m.n_inc_hidden; ++l) {
+      const int o = m.inc_hidden_width[l];
+      if (l == 0) {
+        MlpStage& st = add(ST_HEAD_SPLIT_A, di, o + 16, o);
+        st.src_w[0] = off; st.src_b[0] = off + o * di; st.src_rows[0] = o;
+        st.src_w[1] = sss_w; st.src_b[1] = sss_b; st.src_rows[1] = 3;
+      } else {
+        MlpStage& st = add(ST_HIDDEN, di, o, o);
+        st.src_w[0] = off; st.src_b[0] = off + o * di; st.src_rows[0] = o;
+      }
+      off += o * di + o;
+      di = o;
+    }
+    MlpStage& st = add(ST_HEAD_SPLIT_B, di, 16, 0);
+    st.src_w[0] = off; st.src_b[0] = off + di; st.src_rows[0] = 1;
+    off += di + 1;
+  }
+  plan->n_stages = ns;
+  plan->blob_bytes = (int)align_up((size_t)w_off, 1024);
+  plan->bias_floats = b_off;
+  plan->max_n = max_n;
+  plan->max_k_bytes = max_kb * 128 * 128;
+  const size_t elem = m.dtype == SSSGS_BF16 ? 2 : 4;
+  if (m.params_bytes != (size_t)off * elem)
+    return fail(c, SSSGS_EINVAL, "mlp.params_bytes %zu != expected %zu", m.params_bytes, (size_t)off * elem);
+  if ((size_t)plan->blob_bytes > kMaxBlobBytes || (size_t)b_off > kMaxBiasFloats || max_n > 256)
+    return fail(c, SSSGS_ECAPACITY, "MLP too large for the context");
+  if (mlp_smem_bytes(*plan) > 227 * 1024)
+    return fail(c, SSSGS_ECAPACITY, "MLP weights (%d B) + activations do not fit in shared memory", plan->blob_bytes);
+  return SSSGS_OK;
+}
+
+CamParams make_cam(const sssgs_camera& s) {
+  CamParams c;
+  memcpy(c.R, s.R, sizeof c.R);
+  memcpy(c.t, s.t, sizeof c.t);
+  c.fx = s.fx; c.fy = s.fy; c.cx = s.cx; c.cy = s.cy;
+  c.tanx = s.tan_half_fovx; c.tany = s.tan_half_fovy;
+  c.width = s.width; c.height = s.height; c.znear = s.znear;
+  memcpy(c.bg, s.bg, sizeof c.bg);
+  for (int k = 0; k < 3; ++k) c.pos[k] = -(s.R[0 + k] * s.t[0] + s.R[3 + k] * s.t[1] + s.R[6 + k] * s.t[2]);
+  c.tiles_x = (s.width + kTile - 1) / kTile;
+  c.tiles_y = (s.height + kTile - 1) / kTile;
+  return c;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t sssgs_workspace_bytes(const sssgs_config* cfg) {
+  if (!config_ok(cfg)) return 0;
+  return carve(nullptr, *cfg, nullptr);
+}
+
+int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
+  if (!out) return fail(nullptr, SSSGS_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!config_ok(cfg)) return fail(nullptr, SSSGS_EINVAL, "invalid sssgs_config");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev)
+    return fail(nullptr, SSSGS_ECUDA, "no CUDA device %d (libsssgs has no CPU fallback)", cfg->device);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "cudaGetDeviceProperties failed");
+  if (prop.major != 10) return fail(nullptr, SSSGS_EARCH, "device is sm_%d%d; libsssgs is built for sm_100a only", prop.major, prop.minor);
+  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "cudaSetDevice failed");
+  sssgs_ctx* c = new (std::nothrow) sssgs_ctx();
+  if (!c) return fail(nullptr, SSSGS_ECUDA, "out of host memory");
+  c->cfg = *cfg;
+  c->num_sms = prop.multiProcessorCount;
+  c->max_lb = cfg->max_lights_per_pass ? cfg->max_lights_per_pass : 8;
+  c->ws_bytes = carve(nullptr, *cfg, nullptr);
+  if (cfg->workspace) {
+    if (cfg->workspace_bytes < c->ws_bytes || ((uintptr_t)cfg->workspace & 255u)) {
+      delete c;
+      return fail(nullptr, SSSGS_EINVAL, "workspace too small or not 256-byte aligned");
+    }
+    c->ws = (uint8_t*)cfg->workspace;
+  } else {
+    if (cudaMalloc(&c->ws, c->ws_bytes) != cudaSuccess) {
+      delete c;
+      return fail(nullptr, SSSGS_ECUDA, "cudaMalloc of %zu workspace bytes failed", c->ws_bytes);
+    }
+    c->owns_ws = true;
+  }
+  carve(c, *cfg, c->ws);
+  *out = c;
+  return SSSGS_OK;
+}
+
+void sssgs_destroy(sssgs_ctx* c) {
+  if (!c) return;
+  for (auto& s : c->staging)
+    if (s.first) cudaFree(s.first);
+  if (c->owns_ws && c->ws) cudaFree(c->ws);
+  delete c;
+}
+
+const char* sssgs_last_error(const sssgs_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+int64_t sssgs_last_launch_count(const sssgs_ctx* c) { return c ? c->launches : 0; }
+
+int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, const sssgs_camera* cams,
+                 int n_cam, const sssgs_light* lights, int n_light, const sssgs_out* out,
+                 uint32_t flags, void* cuda_stream) {
+  if (!c) return SSSGS_EINVAL;
+  if (!g || !mlp || !out || (n_cam > 0 && !cams) || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
+  if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
+  if (flags & ~(uint32_t)SSSGS_LIGHTS_PER_CAMERA) return fail(c, SSSGS_EINVAL, "unknown flags");
+  if (g->n < 0) return fail(c, SSSGS_EINVAL, "n < 0");
+  if (g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n %lld > max_gaussians %lld", (long long)g->n, (long long)c->cfg.max_gaussians);
+  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(c, SSSGS_EINVAL, "vis_sh_degree must be 0 or 1");
+  if (g->feat_dim < 0 || g->feat_dim > 88 || g->feat_dim % 4) return fail(c, SSSGS_EINVAL, "feat_dim must be a multiple of 4 in [0,88]");
+  if (g->n > 0) {
+    const void* req[] = {g->means, g->scales, g->rotations, g->opacities, g->normals, g->base_color,
+                         g->roughness, g->metallic, g->subsurface, g->vis_sh};
+    for (const void* p : req)
+      if (!p || !aligned16(p)) return fail(c, SSSGS_EINVAL, "a Gaussian attribute pointer is NULL or not 16-byte aligned");
+    if (g->feat_dim > 0 && (!g->feat || !aligned16(g->feat))) return fail(c, SSSGS_EINVAL, "feat is NULL or misaligned");
+  }
+  const void* outs[] = {out->rgb, out->gbuffer, out->aov_diffuse, out->aov_specular, out->mlp_out,
+                        out->sorted_keys, out->sorted_vals, out->tile_ranges, out->counters};
+  for (const void* p : outs)
+    if (p && !aligned16(p)) return fail(c, SSSGS_EINVAL, "an output pointer is not 16-byte aligned");
+  MlpPlan plan;
+  const bool run_mlp = mlp->precomputed_out == nullptr;
+  if (run_mlp) {
+    if (!mlp->params || !aligned16(mlp->params)) return fail(c, SSSGS_EINVAL, "mlp.params is NULL or misaligned");
+    const int rc = build_plan(c, *mlp, g->feat_dim, &plan);
+    if (rc != SSSGS_OK) return rc;
+  } else if (!aligned16(mlp->precomputed_out)) {
+    return fail(c, SSSGS_EINVAL, "mlp.precomputed_out misaligned");
+  }
+  for (int v = 0; v < n_cam; ++v) {
+    const sssgs_camera& cm = cams[v];
+    if (cm.width <= 0 || cm.height <= 0) return fail(c, SSSGS_EINVAL, "camera %d: empty image", v);
+    if (cm.width > c->cfg.max_width || cm.height > c->cfg.max_height)
+      return fail(c, SSSGS_ECAPACITY, "camera %d: %dx%d exceeds the context's %dx%d", v, cm.width, cm.height, c->cfg.max_width, c->cfg.max_height);
+    if (!(cm.fx > 0.f) || !(cm.fy > 0.f) || !(cm.znear > 0.f)) return fail(c, SSSGS_EINVAL, "camera %d: fx, fy, znear must be > 0", v);
+  }
+
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const uint32_t cap = (uint32_t)c->cfg.max_instances;
+  const int max_blocks = c->num_sms * 4;
+  int64_t launches = 0;
+  auto add = [&](int k) { if (k > 0) launches += k; return k; };
+
+  if (add(launch_pack_attr(*g, c->attr, s)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
+  if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, s));
+
+  const int64_t npix_max = 0;
+  (void)npix_max;
+  for (int v = 0; v < n_cam; ++v) {
+    const CamParams cam = make_cam(cams[v]);
+    const int tiles = cam.tiles_x * cam.tiles_y;
+    const int64_t npix = (int64_t)cam.width * cam.height;
+    if (cudaMemsetAsync(c->control, 0, c->control_bytes, s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "memset failed");
+    uint32_t* cnt = c->gb.counters;
+    // ---- a3: projection ------------------------------------------------------------------------
+    add(launch_project(*g, cam, c->gb, s));
+    // ---- a5 (1/2): all Gaussians by depth, 4 x 8 bits, stable ------------------------------------
+    const uint32_t n32 = (uint32_t)g->n;
+    for (int p = 0; p < 4; ++p) {
+      const int src = p & 1, dst = src ^ 1;
+      add(launch_sort_pass(c->gb.dkeys[src], p == 0 ? nullptr : c->gb.dvals[src],
+                           p == 3 ? nullptr : c->gb.dkeys[dst], c->gb.dvals[dst], nullptr, n32, 8 * p, 8,
+                           c->gb.hist + p * 256, c->status_depth[p], cnt + DC_TICKET_BASE + p,
+                           cnt + DC_SORT_ERROR, max_blocks, s));
+    }
+    const uint32_t* sorted_idx = c->gb.dvals[0];
+    // ---- a4: scan + expansion into (tile, Gaussian) instances, in depth order ---------------------
+    int tb = 1;
+    while ((1 << tb) < tiles) ++tb;
+    const int npass = tb > 8 ? 2 : 1;
+    const int bits0 = npass == 2 ? (tb + 1) / 2 : tb, bits1 = npass == 2 ? tb - bits0 : 0;
+    add(launch_emit(g->n, cam, c->gb, sorted_idx, cap, 0, bits0, bits0, bits1, c->status_emit,
+                    cnt + DC_TICKET_BASE + 4, s));
+    // ---- a5 (2/2): instances by tile id, stable -> per tile (depth, index) order -------------------
+    add(launch_sort_pass(c->gb.ikeys[0], c->gb.ivals[0], c->gb.ikeys[1], c->gb.ivals[1], cnt + DC_INSTANCES,
+                         cap, 0, bits0, c->gb.hist + 4 * 256, c->status_tile[0], cnt + DC_TICKET_BASE + 5,
+                         cnt + DC_SORT_ERROR, max_blocks, s));
+    if (npass == 2)
+      add(launch_sort_pass(c->gb.ikeys[1], c->gb.ivals[1], c->gb.ikeys[0], c->gb.ivals[0], cnt + DC_INSTANCES,
+                           cap, bits0, bits1, c->gb.hist + 5 * 256, c->status_tile[1],
+                           cnt + DC_TICKET_BASE + 6, cnt + DC_SORT_ERROR, max_blocks, s));
+    const int fi = npass & 1;
+    const uint32_t* sorted_tiles = c->gb.ikeys[fi];
+    const uint32_t* sorted_vals = c->gb.ivals[fi];
+    // ---- a6: tile ranges ---------------------------------------------------------------------------
+    add(launch_ranges(sorted_tiles, cam, c->gb, cap,
+                      out->tile_ranges ? (uint2*)(out->tile_ranges + (size_t)v * tiles * 2) : nullptr, s));
+    if (out->sorted_keys || out->sorted_vals || out->counters)
+      add(launch_export_lists(sorted_tiles, sorted_vals, c->gb, cap,
+                              out->sorted_keys ? out->sorted_keys + (size_t)v * cap : nullptr,
+                              out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr,
+                              out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr, s));
+    // ---- per light batch: a1+a2 MLP, a7+a8 raster + shade -------------------------------------------
+    for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
+      const int nl = n_light - l0 < c->max_lb ? n_light - l0 : c->max_lb;
+      LightBatch lb;
+      memset(&lb, 0, sizeof lb);
+      for (int l = 0; l < nl; ++l) {
+        const sssgs_light& L = lights[(flags & SSSGS_LIGHTS_PER_CAMERA) ? (size_t)v * n_light + l0 + l : (size_t)(l0 + l)];
+        memcpy(lb.l[l].pos, L.position, 12);
+        memcpy(lb.l[l].intensity, L.intensity, 12);
+      }
+      const int64_t frame0 = (int64_t)v * n_light + l0;
+      if (run_mlp) {
+        const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, c->mlp_out,
+                                 out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
+                                 c->num_sms, s);
+        if (k < 0) return fail(c, SSSGS_ECUDA, "MLP kernel configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
+        add(k);
+      } else {
+        add(launch_gather_precomputed(mlp->precomputed_out + frame0 * g->n * 4, g->n, nl, g->n * 4, c->mlp_out, s));
+        if (out->mlp_out && g->n > 0)
+          if (cudaMemcpyAsync(out->mlp_out + frame0 * g->n * 4, mlp->precomputed_out + frame0 * g->n * 4,
+                              (size_t)nl * g->n * 16, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+            return fail(c, SSSGS_ECUDA, "memcpy failed");
+      }
+      add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, c->mlp_out,
+                        out->rgb ? out->rgb + frame0 * npix * 3 : nullptr,
+                        out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr,
+                        out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr,
+                        out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix, s));
+    }
+  }
+  c->launches = launches;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, SSSGS_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
+  return SSSGS_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Host-buffer entry point: one host->device crossing per call, results copied back.
+// ---------------------------------------------------------------------------------------------
+namespace {
+void* stage_buf(sssgs_ctx* c, size_t idx, size_t bytes) {
+  if (c->staging.size() <= idx) c->staging.resize(idx + 1, {nullptr, 0});
+  auto& s = c->staging[idx];
+  if (s.second < bytes || !s.first) {
+    if (s.first) cudaFree(s.first);
+    s.first = nullptr;
+    s.second = 0;
+    if (cudaMalloc(&s.first, bytes ? bytes : 16) != cudaSuccess) return nullptr;
+    s.second = bytes ? bytes : 16;
+  }
+  return s.first;
+}
+}  // namespace
+
+extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp,
+                                 const sssgs_camera* cams, int n_cam, const sssgs_light* lights,
+                                 int n_light, const sssgs_out* out, uint32_t flags) {
+  if (!c) return SSSGS_EINVAL;
+  if (!g || !mlp || !out) return fail(c, SSSGS_EINVAL, "NULL argument");
+  if (g->n < 0 || g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n out of range");
+  if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
+  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1 || g->feat_dim < 0) return fail(c, SSSGS_EINVAL, "bad Gaussian description");
+  cudaStream_t s = 0;
+  const size_t n = (size_t)g->n;
+  const size_t ncoef = (size_t)(g->vis_sh_degree + 1) * (g->vis_sh_degree + 1);
+  size_t idx = 0;
+  bool ok = true;
+  auto up = [&](const void* host, size_t bytes) -> void* {
+    void* d = stage_buf(c, idx++, bytes);
+    if (!d) { ok = false; return nullptr; }
+    if (host && bytes && cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) ok = false;
+    return d;
+  };
+  sssgs_gaussians dg = *g;
+  dg.means = (const float*)up(g->means, n * 12);
+  dg.scales = (const float*)up(g->scales, n * 12);
+  dg.rotations = (const float*)up(g->rotations, n * 16);
+  dg.opacities = (const float*)up(g->opacities, n * 4);
+  dg.normals = (const float*)up(g->normals, n * 12);
+  dg.base_color = (const float*)up(g->base_color, n * 12);
+  dg.roughness = (const float*)up(g->roughness, n * 4);
+  dg.metallic = (const float*)up(g->metallic, n * 4);
+  dg.subsurface = (const float*)up(g->subsurface, n * 4);
+  dg.vis_sh = (const float*)up(g->vis_sh, n * ncoef * 4);
+  dg.feat = (const float*)up(g->feat_dim ? g->feat : nullptr, n * (size_t)g->feat_dim * 4);
+  sssgs_mlp dm = *mlp;
+  dm.params = up(mlp->params, mlp->params ? mlp->params_bytes : 0);
+  const size_t frames = (size_t)n_cam * n_light;
+  dm.precomputed_out = mlp->precomputed_out ? (const float*)up(mlp->precomputed_out, frames * n * 16) : nullptr;
+  if (!mlp->precomputed_out) idx++;
+
+  size_t npix = 0, tiles = 0;  // all cameras of one call share the frame size of the first
+  if (n_cam > 0 && cams) {
+    npix = (size_t)cams[0].width * cams[0].height;
+    tiles = (size_t)((cams[0].width + kTile - 1) / kTile) * ((cams[0].height + kTile - 1) / kTile);
+    for (int v = 1; v < n_cam; ++v)
+      if (cams[v].width != cams[0].width || cams[v].height != cams[0].height)
+        return fail(c, SSSGS_EINVAL, "sssgs_render_host: all cameras of a call must share one image size");
+  }
+  const size_t cap = (size_t)c->cfg.max_instances;
+  struct Back { void* host; void* dev; size_t bytes; };
+  std::vector<Back> back;
+  auto down = [&](void* host, size_t bytes) -> void* {
+    if (!host) { idx++; return nullptr; }
+    void* d = stage_buf(c, idx++, bytes);
+    if (!d) { ok = false; return nullptr; }
+    back.push_back({host, d, bytes});
+    return d;
+  };
+  sssgs_out dout;
+  dout.rgb = (float*)down(out->rgb, frames * npix * 12);
+  dout.gbuffer = (float*)down(out->gbuffer, frames * npix * 64);
+  dout.aov_diffuse = (float*)down(out->aov_diffuse, frames * npix * 12);
+  dout.aov_specular = (float*)down(out->aov_specular, frames * npix * 12);
+  dout.mlp_out = (float*)down(out->mlp_out, frames * n * 16);
+  dout.sorted_keys = (uint64_t*)down(out->sorted_keys, (size_t)n_cam * cap * 8);
+  dout.sorted_vals = (uint32_t*)down(out->sorted_vals, (size_t)n_cam * cap * 4);
+  dout.tile_ranges = (uint32_t*)down(out->tile_ranges, (size_t)n_cam * tiles * 8);
+  // counters are always fetched: they carry the overflow flag
+  std::vector<int64_t> cnt_host((size_t)(n_cam > 0 ? n_cam : 1) * SSSGS_NCOUNTERS, 0);
+  dout.counters = (int64_t*)stage_buf(c, idx++, cnt_host.size() * 8);
+  if (!dout.counters) ok = false;
+  if (!ok) return fail(c, SSSGS_ECUDA, "device staging allocation or upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+
+  const int rc = sssgs_render(c, &dg, &dm, cams, n_cam, lights, n_light, &dout, flags, s);
+  if (rc != SSSGS_OK) return rc;
+  for (const Back& b : back)
+    if (b.bytes && cudaMemcpyAsync(b.host, b.dev, b.bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+      return fail(c, SSSGS_ECUDA, "download failed");
+  if (n_cam > 0 && cudaMemcpyAsync(cnt_host.data(), dout.counters, (size_t)n_cam * SSSGS_NCOUNTERS * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+    return fail(c, SSSGS_ECUDA, "download failed");
+  const cudaError_t e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail(c, SSSGS_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
+  for (int v = 0; v < n_cam; ++v) {
+    if (out->counters) memcpy(out->counters + (size_t)v * SSSGS_NCOUNTERS, cnt_host.data() + (size_t)v * SSSGS_NCOUNTERS, SSSGS_NCOUNTERS * 8);
+    if (cnt_host[(size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_SORT_ERROR]) return fail(c, SSSGS_ECUDA, "internal: look-back wait exceeded its bound (camera %d)", v);
+    if (cnt_host[(size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_OVERFLOW])
+      return fail(c, SSSGS_EOVERFLOW, "camera %d: %lld tile instances exceed max_instances %lld", v,
+                  (long long)cnt_host[(size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_INSTANCES], (long long)cap);
+  }
+  return SSSGS_OK;
+}
