@@ -183,6 +183,25 @@ int sssgs_render_host(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp*
                       const sssgs_camera* cams, int n_cam, const sssgs_light* lights, int n_light,
                       const sssgs_out* out, uint32_t flags);
 
+/* Per-stage device timing (measurement aid, off by default).  When enabled, sssgs_render
+ * records CUDA events around each stage on the caller's stream (not capture-safe while on);
+ * sssgs_profile_read synchronises those events and writes the milliseconds each stage of the
+ * LAST call took, summed over cameras and light batches, and the number of kernels per stage. */
+enum {
+  SSSGS_STAGE_PACK = 0,       /* attribute + weight packing                    */
+  SSSGS_STAGE_PROJECT = 1,    /* a3                                            */
+  SSSGS_STAGE_DEPTH_SORT = 2, /* a5, Gaussians by depth                        */
+  SSSGS_STAGE_EMIT = 3,       /* a4                                            */
+  SSSGS_STAGE_TILE_SORT = 4,  /* a5, instances by tile                         */
+  SSSGS_STAGE_RANGES = 5,     /* a6 (+ optional list export)                   */
+  SSSGS_STAGE_MLP = 6,        /* a1 + a2                                       */
+  SSSGS_STAGE_RASTER = 7,     /* a7 + a8                                       */
+  SSSGS_NSTAGES = 8
+};
+int sssgs_profile_enable(sssgs_ctx* ctx, int enable);
+int sssgs_profile_read(sssgs_ctx* ctx, float* stage_ms /* [SSSGS_NSTAGES] */,
+                       int* stage_launches /* [SSSGS_NSTAGES], may be NULL */);
+
 /* Number of kernels the last sssgs_render / sssgs_render_host call launched. */
 int64_t sssgs_last_launch_count(const sssgs_ctx* ctx);
 

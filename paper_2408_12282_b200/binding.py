@@ -29,7 +29,9 @@ SSSGS_F32, SSSGS_BF16 = 0, 1
 CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR = 0, 1, 2, 3
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
-           "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error"]
+           "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
+           "sssgs_profile_enable", "sssgs_profile_read"]
+STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster"]
 
 _f = ctypes.c_float
 _vp = ctypes.c_void_p
@@ -105,6 +107,10 @@ def lib() -> ctypes.CDLL:
         L.sssgs_render_host.argtypes = render_args
         L.sssgs_last_launch_count.restype = ctypes.c_int64
         L.sssgs_last_launch_count.argtypes = [_vp]
+        L.sssgs_profile_enable.restype = ctypes.c_int
+        L.sssgs_profile_enable.argtypes = [_vp, ctypes.c_int]
+        L.sssgs_profile_read.restype = ctypes.c_int
+        L.sssgs_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
         L.sssgs_last_error.restype = ctypes.c_char_p
         L.sssgs_last_error.argtypes = [_vp]
         _lib = L
@@ -145,6 +151,18 @@ def sssgs_render_host(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0) -
 
 def sssgs_last_launch_count(ctx) -> int:
     return int(lib().sssgs_last_launch_count(ctx))
+
+
+def sssgs_profile_enable(ctx, enable: bool) -> None:
+    _check(ctx, lib().sssgs_profile_enable(ctx, 1 if enable else 0))
+
+
+def sssgs_profile_read(ctx):
+    """-> ({stage: ms}, {stage: kernel launches}) of the last sssgs_render call."""
+    ms = (ctypes.c_float * len(STAGES))()
+    nl = (ctypes.c_int * len(STAGES))()
+    _check(ctx, lib().sssgs_profile_read(ctx, ms, nl))
+    return {k: float(ms[i]) for i, k in enumerate(STAGES)}, {k: int(nl[i]) for i, k in enumerate(STAGES)}
 
 
 # ---- marshalling helpers ------------------------------------------------------------------------

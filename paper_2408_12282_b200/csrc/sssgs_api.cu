@@ -32,6 +32,12 @@ struct sssgs_ctx {
   uint8_t* mlp_blob = nullptr;
   float* mlp_bias = nullptr;
   int64_t launches = 0;
+  // optional per-stage timing
+  bool profile = false;
+  struct Span { int stage; cudaEvent_t a, b; };
+  std::vector<Span> spans;        // spans of the last call
+  std::vector<cudaEvent_t> pool;  // recycled events
+  int stage_launches[SSSGS_NSTAGES] = {};
   // device staging of sssgs_render_host (grown on demand, owned)
   std::vector<std::pair<void*, size_t>> staging;
   std::string err;
@@ -258,8 +264,30 @@ void sssgs_destroy(sssgs_ctx* c) {
   if (!c) return;
   for (auto& s : c->staging)
     if (s.first) cudaFree(s.first);
+  for (auto& sp : c->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+  for (auto& e : c->pool) cudaEventDestroy(e);
   if (c->owns_ws && c->ws) cudaFree(c->ws);
   delete c;
+}
+
+int sssgs_profile_enable(sssgs_ctx* c, int enable) {
+  if (!c) return SSSGS_EINVAL;
+  c->profile = enable != 0;
+  return SSSGS_OK;
+}
+
+int sssgs_profile_read(sssgs_ctx* c, float* stage_ms, int* stage_launches) {
+  if (!c || !stage_ms) return SSSGS_EINVAL;
+  for (int k = 0; k < SSSGS_NSTAGES; ++k) stage_ms[k] = 0.f;
+  for (auto& sp : c->spans) {
+    if (cudaEventSynchronize(sp.b) != cudaSuccess) return fail(c, SSSGS_ECUDA, "event sync failed");
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, sp.a, sp.b) != cudaSuccess) return fail(c, SSSGS_ECUDA, "event elapsed failed");
+    stage_ms[sp.stage] += ms;
+  }
+  if (stage_launches)
+    for (int k = 0; k < SSSGS_NSTAGES; ++k) stage_launches[k] = c->stage_launches[k];
+  return SSSGS_OK;
 }
 
 const char* sssgs_last_error(const sssgs_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
@@ -308,10 +336,42 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   const uint32_t cap = (uint32_t)c->cfg.max_instances;
   const int max_blocks = c->num_sms * 4;
   int64_t launches = 0;
-  auto add = [&](int k) { if (k > 0) launches += k; return k; };
+  int cur_stage = -1;
+  auto add = [&](int k) {
+    if (k > 0) {
+      launches += k;
+      if (cur_stage >= 0) c->stage_launches[cur_stage] += k;
+    }
+    return k;
+  };
+  auto new_event = [&]() {
+    cudaEvent_t e = nullptr;
+    if (!c->pool.empty()) { e = c->pool.back(); c->pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+  };
+  if (c->profile) {
+    for (auto& sp : c->spans) { c->pool.push_back(sp.a); c->pool.push_back(sp.b); }
+    c->spans.clear();
+  }
+  memset(c->stage_launches, 0, sizeof c->stage_launches);
+  auto begin = [&](int stage) {
+    cur_stage = stage;
+    if (c->profile) {
+      sssgs_ctx::Span sp{stage, new_event(), new_event()};
+      cudaEventRecord(sp.a, s);
+      c->spans.push_back(sp);
+    }
+  };
+  auto end = [&]() {
+    if (c->profile && !c->spans.empty()) cudaEventRecord(c->spans.back().b, s);
+    cur_stage = -1;
+  };
 
+  begin(SSSGS_STAGE_PACK);
   if (add(launch_pack_attr(*g, c->attr, s)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
   if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, s));
+  end();
 
   const int64_t npix_max = 0;
   (void)npix_max;
@@ -322,7 +382,10 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     if (cudaMemsetAsync(c->control, 0, c->control_bytes, s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "memset failed");
     uint32_t* cnt = c->gb.counters;
     // ---- a3: projection ------------------------------------------------------------------------
+    begin(SSSGS_STAGE_PROJECT);
     add(launch_project(*g, cam, c->gb, s));
+    end();
+    begin(SSSGS_STAGE_DEPTH_SORT);
     // ---- a5 (1/2): all Gaussians by depth, 4 x 8 bits, stable ------------------------------------
     const uint32_t n32 = (uint32_t)g->n;
     for (int p = 0; p < 4; ++p) {
@@ -332,14 +395,18 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                            c->gb.hist + p * 256, c->status_depth[p], cnt + DC_TICKET_BASE + p,
                            cnt + DC_SORT_ERROR, max_blocks, s));
     }
+    end();
     const uint32_t* sorted_idx = c->gb.dvals[0];
     // ---- a4: scan + expansion into (tile, Gaussian) instances, in depth order ---------------------
     int tb = 1;
     while ((1 << tb) < tiles) ++tb;
     const int npass = tb > 8 ? 2 : 1;
     const int bits0 = npass == 2 ? (tb + 1) / 2 : tb, bits1 = npass == 2 ? tb - bits0 : 0;
+    begin(SSSGS_STAGE_EMIT);
     add(launch_emit(g->n, cam, c->gb, sorted_idx, cap, 0, bits0, bits0, bits1, c->status_emit,
                     cnt + DC_TICKET_BASE + 4, s));
+    end();
+    begin(SSSGS_STAGE_TILE_SORT);
     // ---- a5 (2/2): instances by tile id, stable -> per tile (depth, index) order -------------------
     add(launch_sort_pass(c->gb.ikeys[0], c->gb.ivals[0], c->gb.ikeys[1], c->gb.ivals[1], cnt + DC_INSTANCES,
                          cap, 0, bits0, c->gb.hist + 4 * 256, c->status_tile[0], cnt + DC_TICKET_BASE + 5,
@@ -348,10 +415,12 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       add(launch_sort_pass(c->gb.ikeys[1], c->gb.ivals[1], c->gb.ikeys[0], c->gb.ivals[0], cnt + DC_INSTANCES,
                            cap, bits0, bits1, c->gb.hist + 5 * 256, c->status_tile[1],
                            cnt + DC_TICKET_BASE + 6, cnt + DC_SORT_ERROR, max_blocks, s));
+    end();
     const int fi = npass & 1;
     const uint32_t* sorted_tiles = c->gb.ikeys[fi];
     const uint32_t* sorted_vals = c->gb.ivals[fi];
     // ---- a6: tile ranges ---------------------------------------------------------------------------
+    begin(SSSGS_STAGE_RANGES);
     add(launch_ranges(sorted_tiles, cam, c->gb, cap,
                       out->tile_ranges ? (uint2*)(out->tile_ranges + (size_t)v * tiles * 2) : nullptr, s));
     if (out->sorted_keys || out->sorted_vals || out->counters)
@@ -359,6 +428,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                               out->sorted_keys ? out->sorted_keys + (size_t)v * cap : nullptr,
                               out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr,
                               out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr, s));
+    end();
     // ---- per light batch: a1+a2 MLP, a7+a8 raster + shade -------------------------------------------
     for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
       const int nl = n_light - l0 < c->max_lb ? n_light - l0 : c->max_lb;
@@ -370,6 +440,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         memcpy(lb.l[l].intensity, L.intensity, 12);
       }
       const int64_t frame0 = (int64_t)v * n_light + l0;
+      begin(SSSGS_STAGE_MLP);
       if (run_mlp) {
         const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, c->mlp_out,
                                  out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
@@ -383,11 +454,14 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                               (size_t)nl * g->n * 16, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
             return fail(c, SSSGS_ECUDA, "memcpy failed");
       }
+      end();
+      begin(SSSGS_STAGE_RASTER);
       add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, c->mlp_out,
                         out->rgb ? out->rgb + frame0 * npix * 3 : nullptr,
                         out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr,
                         out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr,
                         out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix, s));
+      end();
     }
   }
   c->launches = launches;
