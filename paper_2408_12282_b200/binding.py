@@ -353,3 +353,59 @@ def render_host(scene, cams=None, lights=None, want=("rgb",), max_instances=None
         if ctx_holder is None:
             sssgs_destroy(ctx)
     return outs
+
+
+class HostRenderer:
+    """sssgs_render_host with PINNED host buffers (torch.pin_memory is used for allocation only).
+    Every call crosses host->device with the whole scene and device->host with the outputs."""
+
+    def __init__(self, scene, max_instances: Optional[int] = None, device: int = 0):
+        import torch
+        self.torch = torch
+        self.scene = scene
+        self.n = int(scene.n)
+        cam = scene.cameras[0]
+        self.cfg = sssgs_config()
+        self.cfg.device = device
+        self.cfg.max_gaussians = max(self.n, 1)
+        self.cfg.max_width = max(c.width for c in scene.cameras)
+        self.cfg.max_height = max(c.height for c in scene.cameras)
+        self.cfg.max_instances = int(max_instances if max_instances is not None else max(16 * self.n, 1 << 16))
+        self.ctx = sssgs_create(self.cfg)
+        self.t = {}
+        for f in _FIELDS:
+            a = np.ascontiguousarray(getattr(scene, f), dtype=np.float32)
+            if a.size == 0:
+                a = np.zeros(4, np.float32)
+            self.t[f] = torch.from_numpy(a).pin_memory()
+        self.params = torch.from_numpy(np.ascontiguousarray(scene.mlp.params, np.float32)).pin_memory()
+        self.feat_dim = int(scene.feat.shape[1]) if scene.feat.ndim == 2 else 0
+        self.g = make_gaussians(self.n, {f: self.t[f].data_ptr() for f in _FIELDS}, scene.vis_sh_degree,
+                                self.feat_dim)
+        self.h2d_bytes = sum(int(getattr(scene, f).nbytes) for f in _FIELDS) + int(scene.mlp.params.nbytes)
+        self.out = {}
+
+    def close(self):
+        if self.ctx is not None:
+            sssgs_destroy(self.ctx)
+            self.ctx = None
+
+    def render(self, cams, lights, want=("rgb",)):
+        torch = self.torch
+        n_cam, n_light = len(cams), len(lights)
+        W, H = cams[0].width, cams[0].height
+        F = n_cam * n_light
+        shapes = {"rgb": (F, H, W, 3), "gbuffer": (F, H, W, 16), "mlp_out": (F, max(self.n, 1), 4)}
+        o = sssgs_out()
+        d2h = n_cam * SSSGS_NCOUNTERS * 8
+        for k in want:
+            if k not in self.out or tuple(self.out[k].shape) != shapes[k]:
+                self.out[k] = torch.zeros(shapes[k], dtype=torch.float32).pin_memory()
+            setattr(o, k, self.out[k].data_ptr())
+            d2h += self.out[k].numel() * 4
+        carr = (sssgs_camera * max(n_cam, 1))(*[make_camera(c) for c in cams])
+        larr = (sssgs_light * max(n_light, 1))(*[make_light(l) for l in lights])
+        m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4)
+        sssgs_render_host(self.ctx, self.g, m, carr, n_cam, larr, n_light, o, 0)
+        self.d2h_bytes = d2h
+        return {k: self.out[k] for k in want}
