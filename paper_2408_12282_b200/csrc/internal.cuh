@@ -60,12 +60,14 @@ enum {
   DC_OVERFLOW = 2,
   DC_SORT_ERROR = 3,
   DC_TICKET_BASE = 8, // tickets: one per ticketed kernel launch
-  DC_WORDS = 32
+  DC_RANGES_DONE = 24,   // blocks of ranges_kernel that have finished
+  DC_BUCKET_BASE = 32,   // 32 counters: tiles per list-length bucket (floor(log2(len+1)))
+  DC_WORDS = 64
 };
 
 // Geometry buffers of one camera view.
 struct GeomBuffers {
-  float4* rec_a;      // [n] (pix_x, pix_y, depth, radius)
+  float4* rec_a;      // [n] (pix_x, pix_y, depth, half2 support half-extents ex|ey)
   float4* rec_b;      // [n] (conic a, conic b, conic c, opacity)
   uint2* rect;        // [n] packed tile rect: x = x0 | x1<<16, y = y0 | y1<<16
   uint32_t* touched;  // [n]
@@ -74,6 +76,8 @@ struct GeomBuffers {
   uint32_t* ikeys[2]; // [cap] tile id of each instance ping/pong
   uint32_t* ivals[2]; // [cap] Gaussian index of each instance ping/pong
   uint2* ranges;      // [tiles]
+  uint32_t* tile_order; // [tiles] tile ids, longest lists first (raster work order)
+  uint32_t* tile_slot;  // [tiles] scratch: bucket << 20 | rank inside the bucket
   uint32_t* hist;     // [6][256] digit histograms: 4 depth passes + 2 tile passes
   uint32_t* status;   // look-back status words, carved per pass
   uint32_t* counters; // [DC_WORDS]

@@ -168,26 +168,53 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
   if (bits1 && s_hist[1][tid]) atomicAdd(&hist1[tid], s_hist[1][tid]);
 }
 
-// ranges[t] = [lower_bound(t), lower_bound(t+1)) over the sorted tile ids (one thread per tile)
+// ranges[t] = [lower_bound(t), lower_bound(t+1)) over the sorted tile ids (one thread per tile).
+// The last block to finish also builds the rasteriser's work order: tile ids bucketed by
+// floor(log2(list length)) and laid out longest first, so that the longest lists start first and
+// the tail of the raster kernel is short (order inside a bucket is arbitrary; it only schedules).
 __global__ void __launch_bounds__(256)
-ranges_kernel(const uint32_t* __restrict__ sorted_tiles, const uint32_t* __restrict__ counters,
-              uint32_t cap, int tiles, uint2* __restrict__ ranges, uint2* __restrict__ ranges_user) {
+ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ counters,
+              uint32_t cap, int tiles, uint2* __restrict__ ranges, uint2* __restrict__ ranges_user,
+              uint32_t* __restrict__ tile_slot, uint32_t* __restrict__ tile_order) {
+  __shared__ uint32_t s_start[32];
+  __shared__ bool s_last;
   const int t = blockIdx.x * 256 + threadIdx.x;
-  if (t >= tiles) return;
-  const uint32_t n = min(counters[DC_INSTANCES], cap);
-  uint32_t res[2];
+  if (t < tiles) {
+    const uint32_t n = min(counters[DC_INSTANCES], cap);
+    uint32_t res[2];
 #pragma unroll
-  for (int q = 0; q < 2; ++q) {
-    const uint32_t target = (uint32_t)t + q;
-    uint32_t lo = 0, hi = n;  // first index with key >= target
-    while (lo < hi) {
-      const uint32_t mid = lo + ((hi - lo) >> 1);
-      if (sorted_tiles[mid] < target) lo = mid + 1; else hi = mid;
+    for (int q = 0; q < 2; ++q) {
+      const uint32_t target = (uint32_t)t + q;
+      uint32_t lo = 0, hi = n;  // first index with key >= target
+      while (lo < hi) {
+        const uint32_t mid = lo + ((hi - lo) >> 1);
+        if (sorted_tiles[mid] < target) lo = mid + 1; else hi = mid;
+      }
+      res[q] = lo;
     }
-    res[q] = lo;
+    ranges[t] = make_uint2(res[0], res[1]);
+    if (ranges_user) ranges_user[t] = make_uint2(res[0], res[1]);
+    const uint32_t len = res[1] - res[0];
+    const uint32_t bucket = 32u - __clz(len);  // 0 for empty lists, else floor(log2(len)) + 1
+    const uint32_t rank = atomicAdd(&counters[DC_BUCKET_BASE + bucket], 1u);
+    tile_slot[t] = (bucket << 20) | rank;
   }
-  ranges[t] = make_uint2(res[0], res[1]);
-  if (ranges_user) ranges_user[t] = make_uint2(res[0], res[1]);
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) s_last = atomicAdd(&counters[DC_RANGES_DONE], 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (threadIdx.x < 32) {
+    uint32_t start = 0;
+    for (int b = 31; b > (int)threadIdx.x; --b) start += atomicAdd(&counters[DC_BUCKET_BASE + b], 0u);
+    s_start[threadIdx.x] = start;
+  }
+  __syncthreads();
+  for (int u = threadIdx.x; u < tiles; u += 256) {
+    const uint32_t slot = __ldcg(&tile_slot[u]);
+    tile_order[s_start[slot >> 20] + (slot & 0xFFFFFu)] = (uint32_t)u;
+  }
 }
 
 // Optional export in the ABI format: key = tile << 32 | bits(depth), value = Gaussian index.
@@ -231,7 +258,7 @@ int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const Geom
                   uint32_t cap, uint2* ranges_user, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   ranges_kernel<<<(tiles + 255) / 256, 256, 0, s>>>(sorted_tiles, gb.counters, cap, tiles, gb.ranges,
-                                                    ranges_user);
+                                                    ranges_user, gb.tile_slot, gb.tile_order);
   return 1;
 }
 

@@ -10,6 +10,8 @@
 // 44 B written (2 x float4 record, packed rect, tiles_touched) + 4 B depth key.
 // The block also accumulates the four 8-bit digit histograms of the depth keys (used by the
 // one-sweep radix sort) with warp-aggregated shared-memory atomics.
+#include <cuda_fp16.h>
+
 #include "internal.cuh"
 
 namespace sssgs {
@@ -134,8 +136,19 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
             vis = true;
             cnt = (uint32_t)c2;
             key = __float_as_uint(z);  // P10
-            ra = make_float4(pix_x, pix_y, z, rad);
-            rb = make_float4(con_a, con_b, con_c, opacities[i]);
+            // Half-extents of the alpha >= 1/255 support along x and y (bounding box of the ellipse
+            // 1/2 d^T Q d <= tau, tau = ln(255 o)): used ONLY by the rasteriser to skip entries per
+            // 8x4 pixel block; never by a key or a rect.  Rounded up (slack 0.1 % + 0.01 px, fp16 rp).
+            const float o = opacities[i];
+            const float tau = logf(255.f * o);
+            float ex = 0.f, ey = 0.f;
+            if (tau > 0.f) {
+              ex = sqrtf(2.f * tau * a) * 1.001f + 0.01f;
+              ey = sqrtf(2.f * tau * c) * 1.001f + 0.01f;
+            }
+            const __half2 ext = __halves2half2(__float2half_ru(fminf(ex, 60000.f)), __float2half_ru(fminf(ey, 60000.f)));
+            ra = make_float4(pix_x, pix_y, z, __uint_as_float(*reinterpret_cast<const uint32_t*>(&ext)));
+            rb = make_float4(con_a, con_b, con_c, o);
             rc = make_uint2((uint32_t)x0 | ((uint32_t)x1 << 16), (uint32_t)y0 | ((uint32_t)y1 << 16));
           }
         }

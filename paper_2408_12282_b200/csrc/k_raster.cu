@@ -14,6 +14,8 @@
 // as broadcasts.  Outputs are written once: RGB, and on request the 16-channel G-buffer
 // (4 x 128-bit stores per pixel) and the diffuse / specular AOVs (L320).  Nothing else goes
 // to HBM: the G-buffer round trip of a separate shading pass is avoided.
+#include <cuda_fp16.h>
+
 #include "internal.cuh"
 
 namespace sssgs {
@@ -103,27 +105,40 @@ __device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3
   }
 }
 
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+constexpr int kGroup = 4;  // list entries evaluated together per warp (instruction-level parallelism)
+
 template <int LB>
 __global__ void __launch_bounds__(kRasterThreads)
 raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
-                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ sorted_vals,
+                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
+                    const uint32_t* __restrict__ sorted_vals,
                     const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
                     const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
                     int64_t frame_stride_px) {
   constexpr int NC = 5 + LB;  // float4 components per list entry
-  __shared__ float4 s_c[NC][kBatch];
-  __shared__ uint32_t s_id[kBatch];
+  extern __shared__ float4 s_dyn[];
+  // two stages of component-major entry data + two stages of entry ids
+  float4 (*s_c)[NC][kBatch] = reinterpret_cast<float4 (*)[NC][kBatch]>(s_dyn);
+  uint32_t (*s_id)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + 2 * NC * kBatch);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = blockIdx.x;
+  const int tile = (int)tile_order[blockIdx.x];  // longest lists first
   const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
   // warp -> 8x4 pixel block of the 16x16 tile; lane -> pixel inside the block
-  const int px = tx * kTile + (warp & 1) * 8 + (lane & 7);
-  const int py = ty * kTile + (warp >> 1) * 4 + (lane >> 3);
+  const int bx = tx * kTile + (warp & 1) * 8, by = ty * kTile + (warp >> 1) * 4;
+  const int px = bx + (lane & 7), py = by + (lane >> 3);
   const bool inside = px < cam.width && py < cam.height;
   const float fpx = (float)px, fpy = (float)py;
+  const float bx0 = (float)bx, bx1 = (float)(bx + 7), by0 = (float)by, by1 = (float)(by + 3);
 
   const uint2 range = ranges[tile];
   float T = 1.f, A = 0.f;
@@ -137,64 +152,118 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     for (int c = 0; c < 4; ++c) accl[l][c] = 0.f;
   bool done = !inside;
 
-  for (uint32_t base = range.x; base < range.y; base += kBatch) {
-    if (__syncthreads_and(done)) break;  // also: previous batch fully consumed
-    const int cnt = min((uint32_t)kBatch, range.y - base);
-    if (tid < cnt) s_id[tid] = sorted_vals[base + tid];
-    __syncthreads();
+  // gathers one batch of entries into stage `st` with 16-byte cp.async (all threads share the work)
+  auto gather = [&](int st, int cnt) {
     for (int q = tid; q < NC * kBatch; q += kRasterThreads) {
       const int comp = q / kBatch, e = q % kBatch;
       if (e < cnt) {
-        const uint32_t g = s_id[e];
-        float4 v;
-        if (comp == 0) v = rec_a[g];
-        else if (comp == 1) v = rec_b[g];
-        else if (comp < 5) v = attr[3 * (size_t)g + (comp - 2)];
-        else v = (comp - 5 < n_lights) ? mlp_out[(size_t)g * n_lights + (comp - 5)]
-                                       : make_float4(0.f, 0.f, 0.f, 0.f);
-        s_c[comp][e] = v;
+        const uint32_t g = s_id[st][e];
+        const float4* src;
+        if (comp == 0) src = rec_a + g;
+        else if (comp == 1) src = rec_b + g;
+        else if (comp < 5) src = attr + 3 * (size_t)g + (comp - 2);
+        else src = mlp_out + (size_t)g * n_lights + min(comp - 5, n_lights - 1);
+        cp_async16(&s_c[st][comp][e], src);
       }
     }
+    cp_async_commit();
+  };
+
+  const uint32_t n_entries = range.y - range.x;
+  const int n_batches = (int)((n_entries + kBatch - 1) / kBatch);
+  if (n_batches > 0) {
+    if (tid < kBatch && (uint32_t)tid < n_entries) s_id[0][tid] = sorted_vals[range.x + tid];
     __syncthreads();
-    if (!done) {
-      for (int j = 0; j < cnt; ++j) {
-        const float4 ra = s_c[0][j];
-        const float4 rb = s_c[1][j];
-        const float dx = fpx - ra.x, dy = fpy - ra.y;
-        const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
-        if (power > 0.f) continue;
-        const float alpha = fminf(kAlphaMax, rb.w * __expf(power));
-        if (alpha < kAlphaMin) continue;
-        const float Tn = T * (1.f - alpha);
-        if (Tn < kTMin) {
-          done = true;
-          break;
-        }
-        const float w = alpha * T;
-        const float4 a0 = s_c[2][j], a1 = s_c[3][j], a2 = s_c[4][j];
-        acc[0] = fmaf(w, ra.z, acc[0]);
-        acc[1] = fmaf(w, a0.x, acc[1]);
-        acc[2] = fmaf(w, a0.y, acc[2]);
-        acc[3] = fmaf(w, a0.z, acc[3]);
-        acc[4] = fmaf(w, a1.x, acc[4]);
-        acc[5] = fmaf(w, a1.y, acc[5]);
-        acc[6] = fmaf(w, a1.z, acc[6]);
-        acc[7] = fmaf(w, a0.w, acc[7]);
-        acc[8] = fmaf(w, a1.w, acc[8]);
-        acc[9] = fmaf(w, a2.x, acc[9]);
+    gather(0, (int)min((uint32_t)kBatch, n_entries));
+    if (n_batches > 1 && tid < kBatch && (uint32_t)(kBatch + tid) < n_entries)
+      s_id[1][tid] = sorted_vals[range.x + kBatch + tid];
+  }
+
+  for (int b = 0; b < n_batches; ++b) {
+    const int st = b & 1;
+    const int cnt = (int)min((uint32_t)kBatch, n_entries - (uint32_t)b * kBatch);
+    cp_async_wait_all();
+    // every thread's copies of batch b have landed; all warps have left batch b-1 (stage st^1)
+    if (__syncthreads_and(done)) break;
+    if (b + 1 < n_batches) {
+      gather(st ^ 1, (int)min((uint32_t)kBatch, n_entries - (uint32_t)(b + 1) * kBatch));
+      const uint32_t nxt = (uint32_t)(b + 2) * kBatch + tid;   // ids of batch b+2 reuse s_id[st]
+      if (tid < kBatch && nxt < n_entries) s_id[st][tid] = sorted_vals[range.x + nxt];
+    }
+    if (__all_sync(0xFFFFFFFFu, done)) continue;  // this warp's 8x4 block is finished
+
+    for (int c0 = 0; c0 < cnt; c0 += 32) {
+      // ---- per-warp cull: lane <-> entry; keep entries whose alpha >= 1/255 support box
+      //      overlaps this warp's 8x4 pixel block --------------------------------------------------
+      bool hit = false;
+      if (c0 + lane < cnt) {
+        const float4 ra = s_c[st][0][c0 + lane];
+        const __half2 ext = *reinterpret_cast<const __half2*>(&ra.w);
+        const float ex = __low2float(ext), ey = __high2float(ext);
+        hit = (ra.x + ex >= bx0) && (ra.x - ex <= bx1) && (ra.y + ey >= by0) && (ra.y - ey <= by1);
+      }
+      unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
+      while (m) {
+        // ---- evaluate up to kGroup entries independently ---------------------------------------
+        int idx[kGroup];
+        float alpha[kGroup];
 #pragma unroll
-        for (int l = 0; l < LB; ++l) {
-          const float4 m = s_c[5 + l][j];
-          accl[l][0] = fmaf(w, m.x, accl[l][0]);
-          accl[l][1] = fmaf(w, m.y, accl[l][1]);
-          accl[l][2] = fmaf(w, m.z, accl[l][2]);
-          accl[l][3] = fmaf(w, m.w, accl[l][3]);
+        for (int k = 0; k < kGroup; ++k) {
+          idx[k] = m ? c0 + __ffs(m) - 1 : -1;
+          m &= m - 1;
         }
-        A += w;
-        T = Tn;
+#pragma unroll
+        for (int k = 0; k < kGroup; ++k) {
+          alpha[k] = 0.f;
+          if (idx[k] >= 0) {
+            const float4 ra = s_c[st][0][idx[k]];
+            const float4 rb = s_c[st][1][idx[k]];
+            const float dx = fpx - ra.x, dy = fpy - ra.y;
+            const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
+            const float al = fminf(kAlphaMax, rb.w * __expf(power));
+            alpha[k] = (power > 0.f || al < kAlphaMin) ? 0.f : al;
+          }
+        }
+        // ---- blend sequentially (front to back) ------------------------------------------------
+#pragma unroll
+        for (int k = 0; k < kGroup; ++k) {
+          if (alpha[k] > 0.f && !done) {
+            const float Tn = T * (1.f - alpha[k]);
+            if (Tn < kTMin) {
+              done = true;
+            } else {
+              const int j = idx[k];
+              const float w = alpha[k] * T;
+              const float4 ra = s_c[st][0][j];
+              const float4 a0 = s_c[st][2][j], a1 = s_c[st][3][j], a2 = s_c[st][4][j];
+              acc[0] = fmaf(w, ra.z, acc[0]);
+              acc[1] = fmaf(w, a0.x, acc[1]);
+              acc[2] = fmaf(w, a0.y, acc[2]);
+              acc[3] = fmaf(w, a0.z, acc[3]);
+              acc[4] = fmaf(w, a1.x, acc[4]);
+              acc[5] = fmaf(w, a1.y, acc[5]);
+              acc[6] = fmaf(w, a1.z, acc[6]);
+              acc[7] = fmaf(w, a0.w, acc[7]);
+              acc[8] = fmaf(w, a1.w, acc[8]);
+              acc[9] = fmaf(w, a2.x, acc[9]);
+#pragma unroll
+              for (int l = 0; l < LB; ++l) {
+                const float4 mo = s_c[st][5 + l][j];
+                accl[l][0] = fmaf(w, mo.x, accl[l][0]);
+                accl[l][1] = fmaf(w, mo.y, accl[l][1]);
+                accl[l][2] = fmaf(w, mo.z, accl[l][2]);
+                accl[l][3] = fmaf(w, mo.w, accl[l][3]);
+              }
+              A += w;
+              T = Tn;
+            }
+          }
+        }
+        if (__all_sync(0xFFFFFFFFu, done)) { m = 0; c0 = cnt; }
       }
     }
   }
+  cp_async_wait_all();
 
   if (!inside) return;
   // ---- epilogue: G-buffer stores + deferred shading, per light ---------------------------------
@@ -267,11 +336,19 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   int64_t frame_stride_px, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
-#define SSSGS_RASTER(LB)                                                                        \
-  raster_shade_kernel<LB><<<tiles, kRasterThreads, 0, s>>>(cam, lights, n_lights, gb.ranges,    \
-                                                           sorted_vals, gb.rec_a, gb.rec_b, attr, \
-                                                           mlp_out, rgb, gbuf, aov_d, aov_s,     \
-                                                           frame_stride_px)
+#define SSSGS_RASTER(LB)                                                                          \
+  do {                                                                                            \
+    constexpr int smem = 2 * (5 + LB) * kBatch * 16 + 2 * kBatch * 4;                             \
+    static bool configured = false;                                                               \
+    if (!configured) {                                                                            \
+      if (cudaFuncSetAttribute(raster_shade_kernel<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                               smem) != cudaSuccess) return -1;                                   \
+      configured = true;                                                                          \
+    }                                                                                             \
+    raster_shade_kernel<LB><<<tiles, kRasterThreads, smem, s>>>(                                  \
+        cam, lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr,   \
+        mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px);                                       \
+  } while (0)
   if (n_lights <= 1) SSSGS_RASTER(1);
   else if (n_lights <= 4) SSSGS_RASTER(4);
   else SSSGS_RASTER(8);

@@ -98,6 +98,8 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   for (int k = 0; k < 2; ++k) { p = take(cap * 4); if (c) c->gb.ikeys[k] = (uint32_t*)p; }
   for (int k = 0; k < 2; ++k) { p = take(cap * 4); if (c) c->gb.ivals[k] = (uint32_t*)p; }
   p = take(tiles * 8); if (c) c->gb.ranges = (uint2*)p;
+  p = take(tiles * 4); if (c) c->gb.tile_order = (uint32_t*)p;
+  p = take(tiles * 4); if (c) c->gb.tile_slot = (uint32_t*)p;
   p = take(n * (size_t)lb * 16); if (c) c->mlp_out = (float4*)p;
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
   p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
