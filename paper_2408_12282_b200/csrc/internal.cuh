@@ -19,8 +19,22 @@ constexpr int kTile = SSSGS_TILE;
 
 // ---- radix sort geometry --------------------------------------------------------------------
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 15;
-constexpr int kSortTile = kSortThreads * kSortItems;  // keys per ticket
+constexpr int kSortItemsMax = 15;
+constexpr int kSortTileMax = kSortThreads * kSortItemsMax;  // keys per ticket, at most
+constexpr uint32_t kSortFill = 148 * 4;                     // tickets that fill the machine
+// keys per thread and ticket, by problem size: the smallest of {3, 7, 15} that needs no more
+// than kSortFill tickets (15 beyond that)
+__host__ __device__ inline int sort_items_for(uint32_t n) {
+  if (n <= kSortFill * (uint32_t)kSortThreads * 3u) return 3;
+  if (n <= kSortFill * (uint32_t)kSortThreads * 7u) return 7;
+  return 15;
+}
+// rows of look-back status a pass over at most `cap` keys can need
+__host__ __device__ inline uint32_t sort_status_rows(uint32_t cap) {
+  const uint32_t per = (uint32_t)kSortThreads * (uint32_t)sort_items_for(cap);
+  const uint32_t rows = (cap + per - 1) / per;
+  return (cap > kSortFill * (uint32_t)kSortThreads * 3u && rows < kSortFill) ? kSortFill : rows;
+}
 constexpr int kRadixMax = 256;
 constexpr uint32_t kFlagAgg = 1u << 30;  // look-back status: aggregate of this tile only
 constexpr uint32_t kFlagInc = 2u << 30;  // inclusive prefix up to and including this tile
@@ -30,8 +44,7 @@ constexpr int kSpinLimit = 1 << 24;  // bug trap for look-back waits (sets SSSGS
 
 // ---- emit (scan + expand) geometry ----------------------------------------------------------
 constexpr int kEmitThreads = 256;
-constexpr int kEmitItems = 4;
-constexpr int kEmitChunk = kEmitThreads * kEmitItems;  // Gaussians per ticket
+constexpr int kEmitChunk = kEmitThreads;  // Gaussians per ticket
 
 struct CamParams {   // device copy of sssgs_camera plus derived values
   float R[9], t[3];
@@ -61,7 +74,6 @@ enum {
   DC_SORT_ERROR = 3,
   DC_TICKET_BASE = 8, // tickets: one per ticketed kernel launch
   DC_RANGES_DONE = 24,   // blocks of ranges_kernel that have finished
-  DC_BUCKET_BASE = 32,   // 32 counters: tiles per list-length bucket (floor(log2(len+1)))
   DC_WORDS = 64
 };
 
@@ -77,7 +89,7 @@ struct GeomBuffers {
   uint32_t* ivals[2]; // [cap] Gaussian index of each instance ping/pong
   uint2* ranges;      // [tiles]
   uint32_t* tile_order; // [tiles] tile ids, longest lists first (raster work order)
-  uint32_t* tile_slot;  // [tiles] scratch: bucket << 20 | rank inside the bucket
+  uint32_t* tile_slot;  // [tiles + 1] scratch: lower bound of every tile id in the sorted instances
   uint32_t* hist;     // [6][256] digit histograms: 4 depth passes + 2 tile passes
   uint32_t* status;   // look-back status words, carved per pass
   uint32_t* counters; // [DC_WORDS]

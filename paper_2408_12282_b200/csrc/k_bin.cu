@@ -2,11 +2,11 @@
 // with the expansion into (tile id, Gaussian) instances, the per-tile ranges, and the optional
 // export of the sorted lists in the ABI's 64-bit key format.
 //
-// emit_kernel: persistent CTAs pull chunks of 1024 depth-sorted Gaussians by ticket.  A chunk
-// is scanned in shared memory, its global base comes from a decoupled look-back over the
-// chunk totals (integer prefix sums: deterministic), and the instances are written by
-// consecutive threads to consecutive addresses (each thread finds its Gaussian by binary
-// search in the chunk's offsets), tile y then x ascending inside a Gaussian.  The CTA also
+// emit_kernel: persistent CTAs pull chunks of 256 depth-sorted Gaussians by ticket.  A chunk is
+// scanned with warp shuffles, its global base comes from a decoupled look-back over the chunk
+// totals (integer prefix sums: deterministic), and each warp expands its 32 Gaussians so that
+// consecutive lanes write consecutive instances (a lane finds its Gaussian by a 5-step shuffle
+// search over the warp's offsets), tile y then x ascending inside a Gaussian.  The CTA also
 // accumulates the digit histograms of the tile ids for the tile sort.
 // Traffic: 4+4+8 B read per Gaussian, 8 B written per instance.
 #include "internal.cuh"
@@ -31,9 +31,6 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
             uint32_t* __restrict__ hist0, uint32_t* __restrict__ hist1, int shift0, int bits0,
             int shift1, int bits1, uint32_t* __restrict__ status, uint32_t* __restrict__ ticket,
             uint32_t* __restrict__ counters) {
-  __shared__ uint32_t s_off[kEmitChunk + 1];
-  __shared__ uint32_t s_g[kEmitChunk];
-  __shared__ uint2 s_rect[kEmitChunk];
   __shared__ uint32_t s_hist[2][kRadixMax];
   __shared__ uint32_t s_wsum[kEmitThreads / 32];
   __shared__ uint32_t s_ticket, s_base;
@@ -51,24 +48,16 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
     const uint32_t t = s_ticket;
     if (t >= nchunks) break;
 
-    // ---- load 4 consecutive sorted positions per thread, scan tiles-touched -----------------
-    uint32_t c[kEmitItems], sum = 0;
-#pragma unroll
-    for (int k = 0; k < kEmitItems; ++k) {
-      const uint32_t j = t * (uint32_t)kEmitChunk + tid * kEmitItems + k;
-      uint32_t g = 0, cnt = 0;
-      uint2 r = make_uint2(0u, 0u);
-      if (j < n) {
-        g = sorted_idx[j];
-        cnt = touched[g];
-        r = rect[g];
-      }
-      s_g[tid * kEmitItems + k] = g;
-      s_rect[tid * kEmitItems + k] = r;
-      c[k] = cnt;
-      sum += cnt;
+    // ---- one depth-sorted Gaussian per thread; scan of tiles-touched over the chunk -----------
+    const uint32_t j = t * (uint32_t)kEmitChunk + tid;
+    uint32_t g = 0, cnt = 0;
+    uint2 r = make_uint2(0u, 0u);
+    if (j < n) {
+      g = sorted_idx[j];
+      cnt = touched[g];
+      r = rect[g];
     }
-    uint32_t inc = sum;
+    uint32_t inc = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, inc, o);
@@ -83,82 +72,89 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
       if ((unsigned)w < warp) wbase += v;
       total += v;
     }
-    uint32_t run = wbase + inc - sum;
-#pragma unroll
-    for (int k = 0; k < kEmitItems; ++k) {
-      s_off[tid * kEmitItems + k] = run;
-      run += c[k];
-    }
-    if (tid == 0) {
-      s_off[kEmitChunk] = total;
-      // ---- decoupled look-back over chunk totals ------------------------------------------
+    if (warp == 0) {
+      // ---- decoupled look-back over chunk totals, one warp looking at 32 earlier chunks at a time --
       uint32_t excl = 0;
       if (t == 0) {
-        st_volatile(status, kFlagInc | total);
+        if (lane == 0) st_volatile(status, kFlagInc | total);
       } else {
-        st_volatile(status + t, kFlagAgg | total);
+        if (lane == 0) st_volatile(status + t, kFlagAgg | total);
         int spins = 0;
-        for (uint32_t tt = t; tt-- > 0;) {
-          uint32_t v = ld_volatile(status + tt);
-          while ((v & kFlagMask) == 0u) {
+        for (int64_t first = (int64_t)t - 1;;) {
+          const int64_t idx = first - lane;
+          const uint32_t v = idx >= 0 ? ld_volatile(status + idx) : kFlagInc;
+          const unsigned inc = __ballot_sync(0xFFFFFFFFu, (v & kFlagMask) == kFlagInc);
+          const unsigned none = __ballot_sync(0xFFFFFFFFu, (v & kFlagMask) == 0u);
+          const int stop = inc ? __ffs(inc) - 1 : 31;            // nearest chunk with an inclusive prefix
+          const unsigned need = stop == 31 ? 0xFFFFFFFFu : ((2u << stop) - 1u);
+          if (none & need) {                                     // a chunk in between is not published yet
             if (++spins > kSpinLimit) {
-              atomicExch(&counters[DC_SORT_ERROR], 2u);
-              v = kFlagInc;
+              if (lane == 0) atomicExch(&counters[DC_SORT_ERROR], 2u);
               break;
             }
-            __nanosleep(32);
-            v = ld_volatile(status + tt);
+            __nanosleep(20);
+            continue;
           }
-          excl += v & kValMask;
-          if (v & kFlagInc) break;
+          uint32_t val = lane <= stop ? (v & kValMask) : 0u;
+#pragma unroll
+          for (int o = 16; o >= 1; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
+          excl += val;
+          if (inc) break;
+          first -= 32;
         }
-        st_volatile(status + t, kFlagInc | ((excl + total) & kValMask));
+        if (lane == 0) st_volatile(status + t, kFlagInc | ((excl + total) & kValMask));
       }
-      s_base = excl;
-      if (t == nchunks - 1) {
-        const uint32_t all = excl + total;
-        counters[DC_INSTANCES] = all;
-        if (all > cap) counters[DC_OVERFLOW] = 1u;
+      if (lane == 0) {
+        s_base = excl;
+        if (t == nchunks - 1) {
+          const uint32_t all = excl + total;
+          counters[DC_INSTANCES] = all;
+          if (all > cap) counters[DC_OVERFLOW] = 1u;
+        }
       }
     }
     __syncthreads();
-    const uint32_t base = s_base;
 
-    // ---- expand: consecutive threads write consecutive instances ----------------------------
-    for (uint32_t ob = 0; ob < total; ob += kEmitThreads) {  // warp-uniform trip count
-      const uint32_t o = ob + tid;
-      bool ok = false;
-      uint32_t tile = 0;
-      if (o < total) {
-        // last e with s_off[e] <= o  (zero-count entries share their successor's start)
-        uint32_t lo = 0, hi = kEmitChunk;  // invariant: s_off[lo] <= o < s_off[hi]
-        while (hi - lo > 1) {
-          const uint32_t mid = (lo + hi) >> 1;
-          if (s_off[mid] <= o) lo = mid; else hi = mid;
-        }
-        const uint32_t k = o - s_off[lo];
-        const uint2 r = s_rect[lo];
-        const uint32_t x0 = r.x & 0xFFFFu, x1 = r.x >> 16, y0 = r.y & 0xFFFFu;
+    // ---- expand, one warp per 32 Gaussians: consecutive lanes write consecutive instances ------
+    const uint32_t woff = inc - cnt;                       // exclusive offset inside the warp
+    const uint32_t wtotal = __shfl_sync(0xFFFFFFFFu, inc, 31);
+    const uint32_t gbase = s_base + wbase;
+    for (uint32_t ob = 0; ob < wtotal; ob += 32) {         // warp-uniform trip count
+      const uint32_t o = ob + lane;
+      // last lane l with woff[l] <= o (zero-count lanes share their successor's start)
+      uint32_t lo = 0;
+#pragma unroll
+      for (int step = 16; step >= 1; step >>= 1) {
+        const uint32_t cand = lo + step;
+        const uint32_t v = __shfl_sync(0xFFFFFFFFu, woff, cand & 31);
+        if (v <= o) lo = cand;
+      }
+      const uint32_t l_off = __shfl_sync(0xFFFFFFFFu, woff, lo);
+      const uint32_t l_rx = __shfl_sync(0xFFFFFFFFu, r.x, lo);
+      const uint32_t l_ry = __shfl_sync(0xFFFFFFFFu, r.y, lo);
+      const uint32_t l_g = __shfl_sync(0xFFFFFFFFu, g, lo);
+      const uint32_t dst = gbase + o;
+      const bool ok = o < wtotal && dst < cap;
+      if (ok) {
+        const uint32_t k = o - l_off;
+        const uint32_t x0 = l_rx & 0xFFFFu, x1 = l_rx >> 16, y0 = l_ry & 0xFFFFu;
         const uint32_t w = x1 - x0;
         const uint32_t ty = y0 + k / w, tx = x0 + k % w;
-        tile = ty * (uint32_t)tiles_x + tx;
-        const uint32_t dst = base + o;
-        ok = dst < cap;
-        if (ok) {
-          ikeys[dst] = tile;
-          ivals[dst] = s_g[lo];
-        }
-      }
-      // warp-aggregated digit histograms
-      const unsigned act = __ballot_sync(0xFFFFFFFFu, ok);
-      if (ok) {
-        const uint32_t d0 = (tile >> shift0) & mask0;
-        unsigned peers = __match_any_sync(act, d0);
-        if ((peers & ((1u << lane) - 1u)) == 0) atomicAdd(&s_hist[0][d0], __popc(peers));
+        const uint32_t tile = ty * (uint32_t)tiles_x + tx;
+        ikeys[dst] = tile;
+        ivals[dst] = l_g;
+        // digit histograms of the tile id for the tile sort: the low digit differs between
+        // neighbouring instances (x ascending), the high digit is mostly warp-uniform
+        atomicAdd(&s_hist[0][(tile >> shift0) & mask0], 1u);
         if (bits1) {
           const uint32_t d1 = (tile >> shift1) & mask1;
-          peers = __match_any_sync(act, d1);
-          if ((peers & ((1u << lane) - 1u)) == 0) atomicAdd(&s_hist[1][d1], __popc(peers));
+          const unsigned act = __activemask();
+          const uint32_t d1_first = __shfl_sync(act, d1, __ffs(act) - 1);
+          if (__all_sync(act, d1 == d1_first)) {
+            if (lane == (unsigned)(__ffs(act) - 1)) atomicAdd(&s_hist[1][d1], __popc(act));
+          } else {
+            atomicAdd(&s_hist[1][d1], 1u);
+          }
         }
       }
     }
@@ -168,36 +164,24 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
   if (bits1 && s_hist[1][tid]) atomicAdd(&hist1[tid], s_hist[1][tid]);
 }
 
-// ranges[t] = [lower_bound(t), lower_bound(t+1)) over the sorted tile ids (one thread per tile).
-// The last block to finish also builds the rasteriser's work order: tile ids bucketed by
-// floor(log2(list length)) and laid out longest first, so that the longest lists start first and
-// the tail of the raster kernel is short (order inside a bucket is arbitrary; it only schedules).
+// ranges[t] = [lower_bound(t), lower_bound(t+1)) over the sorted tile ids.  Every boundary i
+// between two different neighbouring tile ids a < b defines lower_bound(t) = i for all t in
+// (a, b] (the ends count as tile ids -1 and `tiles`), so one coalesced sweep over the sorted ids
+// fills lb[0..tiles].  The last block to finish turns lb into ranges and builds the
+// rasteriser's work order: tile ids bucketed by floor(log2(list length)) and laid out longest
+// first, so that the longest lists start first and the tail of the raster kernel is short
+// (order inside a bucket is arbitrary; it only schedules).
 __global__ void __launch_bounds__(256)
 ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ counters,
               uint32_t cap, int tiles, uint2* __restrict__ ranges, uint2* __restrict__ ranges_user,
-              uint32_t* __restrict__ tile_slot, uint32_t* __restrict__ tile_order) {
-  __shared__ uint32_t s_start[32];
+              uint32_t* __restrict__ lb, uint32_t* __restrict__ tile_order) {
+  __shared__ uint32_t s_cnt[32], s_start[32];
   __shared__ bool s_last;
-  const int t = blockIdx.x * 256 + threadIdx.x;
-  if (t < tiles) {
-    const uint32_t n = min(counters[DC_INSTANCES], cap);
-    uint32_t res[2];
-#pragma unroll
-    for (int q = 0; q < 2; ++q) {
-      const uint32_t target = (uint32_t)t + q;
-      uint32_t lo = 0, hi = n;  // first index with key >= target
-      while (lo < hi) {
-        const uint32_t mid = lo + ((hi - lo) >> 1);
-        if (sorted_tiles[mid] < target) lo = mid + 1; else hi = mid;
-      }
-      res[q] = lo;
-    }
-    ranges[t] = make_uint2(res[0], res[1]);
-    if (ranges_user) ranges_user[t] = make_uint2(res[0], res[1]);
-    const uint32_t len = res[1] - res[0];
-    const uint32_t bucket = 32u - __clz(len);  // 0 for empty lists, else floor(log2(len)) + 1
-    const uint32_t rank = atomicAdd(&counters[DC_BUCKET_BASE + bucket], 1u);
-    tile_slot[t] = (bucket << 20) | rank;
+  const uint32_t n = min(counters[DC_INSTANCES], cap);
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i <= n; i += gridDim.x * 256u) {
+    const int a = i == 0 ? -1 : (int)sorted_tiles[i - 1];
+    const int b = i == n ? tiles : (int)sorted_tiles[i];
+    for (int t = a + 1; t <= b; ++t) lb[t] = i;
   }
   __threadfence();
   __syncthreads();
@@ -205,15 +189,24 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
   __syncthreads();
   if (!s_last) return;
   __threadfence();
+  if (threadIdx.x < 32) s_cnt[threadIdx.x] = 0;
+  __syncthreads();
+  for (int t = threadIdx.x; t < tiles; t += 256) {
+    const uint32_t b0 = __ldcg(&lb[t]), b1 = __ldcg(&lb[t + 1]);
+    ranges[t] = make_uint2(b0, b1);
+    if (ranges_user) ranges_user[t] = make_uint2(b0, b1);
+    atomicAdd(&s_cnt[32u - __clz(b1 - b0)], 1u);  // bucket 0: empty list, else floor(log2(len)) + 1
+  }
+  __syncthreads();
   if (threadIdx.x < 32) {
     uint32_t start = 0;
-    for (int b = 31; b > (int)threadIdx.x; --b) start += atomicAdd(&counters[DC_BUCKET_BASE + b], 0u);
+    for (int k = 31; k > (int)threadIdx.x; --k) start += s_cnt[k];
     s_start[threadIdx.x] = start;
   }
   __syncthreads();
-  for (int u = threadIdx.x; u < tiles; u += 256) {
-    const uint32_t slot = __ldcg(&tile_slot[u]);
-    tile_order[s_start[slot >> 20] + (slot & 0xFFFFFu)] = (uint32_t)u;
+  for (int t = threadIdx.x; t < tiles; t += 256) {
+    const uint32_t len = __ldcg(&lb[t + 1]) - __ldcg(&lb[t]);
+    tile_order[atomicAdd(&s_start[32u - __clz(len)], 1u)] = (uint32_t)t;
   }
 }
 
@@ -257,8 +250,10 @@ int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, const ui
 int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
                   uint32_t cap, uint2* ranges_user, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
-  ranges_kernel<<<(tiles + 255) / 256, 256, 0, s>>>(sorted_tiles, gb.counters, cap, tiles, gb.ranges,
-                                                    ranges_user, gb.tile_slot, gb.tile_order);
+  int64_t blocks = ((int64_t)cap + 1 + 1023) / 1024;
+  if (blocks > 148 * 4) blocks = 148 * 4;
+  ranges_kernel<<<(unsigned)blocks, 256, 0, s>>>(sorted_tiles, gb.counters, cap, tiles, gb.ranges,
+                                                 ranges_user, gb.tile_slot, gb.tile_order);
   return 1;
 }
 

@@ -16,6 +16,8 @@
 // to HBM: the G-buffer round trip of a separate shading pass is avoided.
 #include <cuda_fp16.h>
 
+#include <cstdlib>
+
 #include "internal.cuh"
 
 namespace sssgs {
@@ -23,7 +25,6 @@ namespace sssgs {
 namespace {
 
 constexpr int kBatch = 128;
-constexpr int kRasterThreads = 256;
 constexpr float kPi = 3.14159265358979323846f;
 
 struct ShadeIn {
@@ -112,10 +113,28 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-constexpr int kGroup = 4;  // list entries evaluated together per warp (instruction-level parallelism)
+// Work decomposition of one rasteriser variant.  A warp covers P = 32/E pixels (a PW x PH block)
+// and evaluates E consecutive list entries of that block at once ("entry slots"): lane =
+// slot * P + pixel.  A CTA of WARPS warps covers an RW x RH pixel region of a 16x16 tile, so a
+// tile is rendered by (16/RW) x (16/RH) CTAs that walk the same list.  E = 1, WARPS = 8 is the
+// classic one-thread-per-pixel, one-CTA-per-tile layout; E > 1 shortens the sequential walk of a
+// long list by E (more warps share it) and culls at a finer pixel-block granularity.
+template <int E, int WARPS>
+struct RasterShape {
+  static constexpr int P = 32 / E;
+  static constexpr int PW = (E == 1) ? 8 : (E == 8 ? 2 : 4);
+  static constexpr int PH = P / PW;
+  static constexpr int NPIX = WARPS * P;
+  static constexpr int RW = NPIX >= 128 ? 16 : 8;
+  static constexpr int RH = NPIX / RW;
+  static constexpr int SX = kTile / RW, SY = kTile / RH;
+  static constexpr int SUBS = SX * SY;
+  static constexpr int THREADS = WARPS * 32;
+  static_assert(RH >= PH && RH <= kTile && (RW % PW) == 0 && (RH % PH) == 0, "bad raster shape");
+};
 
-template <int LB>
-__global__ void __launch_bounds__(kRasterThreads)
+template <int LB, int E, int WARPS, int U>
+__global__ void __launch_bounds__(WARPS * 32)
 raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
                     const uint32_t* __restrict__ sorted_vals,
@@ -124,24 +143,31 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
                     int64_t frame_stride_px) {
+  using S = RasterShape<E, WARPS>;
+  constexpr int P = S::P, THREADS = S::THREADS;
   constexpr int NC = 5 + LB;  // float4 components per list entry
+  constexpr unsigned FULL = 0xFFFFFFFFu;
   extern __shared__ float4 s_dyn[];
-  // two stages of component-major entry data + two stages of entry ids
+  // two stages of component-major entry data, two stages of entry ids, one hit queue per warp
   float4 (*s_c)[NC][kBatch] = reinterpret_cast<float4 (*)[NC][kBatch]>(s_dyn);
   uint32_t (*s_id)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + 2 * NC * kBatch);
+  uint8_t (*s_q)[kBatch] = reinterpret_cast<uint8_t (*)[kBatch]>(s_id + 2);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = (int)tile_order[blockIdx.x];  // longest lists first
+  const int slot = lane / P, pix = lane % P;
+  const int tile = (int)tile_order[blockIdx.x / S::SUBS];  // longest lists first
+  const int sub = blockIdx.x % S::SUBS;
   const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
-  // warp -> 8x4 pixel block of the 16x16 tile; lane -> pixel inside the block
-  const int bx = tx * kTile + (warp & 1) * 8, by = ty * kTile + (warp >> 1) * 4;
-  const int px = bx + (lane & 7), py = by + (lane >> 3);
+  constexpr int WPR = S::RW / S::PW;  // warps per region row
+  const int bx = tx * kTile + (sub % S::SX) * S::RW + (warp % WPR) * S::PW;
+  const int by = ty * kTile + (sub / S::SX) * S::RH + (warp / WPR) * S::PH;
+  const int px = bx + pix % S::PW, py = by + pix / S::PW;
   const bool inside = px < cam.width && py < cam.height;
   const float fpx = (float)px, fpy = (float)py;
-  const float bx0 = (float)bx, bx1 = (float)(bx + 7), by0 = (float)by, by1 = (float)(by + 3);
+  const float bx0 = (float)bx, bx1 = (float)(bx + S::PW - 1), by0 = (float)by, by1 = (float)(by + S::PH - 1);
 
   const uint2 range = ranges[tile];
-  float T = 1.f, A = 0.f;
+  float T = 1.f, A = 0.f;  // T is identical in the E lanes of a pixel; A is a per-lane partial sum
   float acc[10];
   float accl[LB][4];
 #pragma unroll
@@ -154,7 +180,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
 
   // gathers one batch of entries into stage `st` with 16-byte cp.async (all threads share the work)
   auto gather = [&](int st, int cnt) {
-    for (int q = tid; q < NC * kBatch; q += kRasterThreads) {
+    for (int q = tid; q < NC * kBatch; q += THREADS) {
       const int comp = q / kBatch, e = q % kBatch;
       if (e < cnt) {
         const uint32_t g = s_id[st][e];
@@ -190,11 +216,12 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
       const uint32_t nxt = (uint32_t)(b + 2) * kBatch + tid;   // ids of batch b+2 reuse s_id[st]
       if (tid < kBatch && nxt < n_entries) s_id[st][tid] = sorted_vals[range.x + nxt];
     }
-    if (__all_sync(0xFFFFFFFFu, done)) continue;  // this warp's 8x4 block is finished
+    if (__all_sync(FULL, done)) continue;  // this warp's pixel block is finished
 
+    // ---- cull: lane <-> entry; queue the entries whose alpha >= 1/255 support box overlaps this
+    //      warp's pixel block, in list order --------------------------------------------------------
+    int nq = 0;
     for (int c0 = 0; c0 < cnt; c0 += 32) {
-      // ---- per-warp cull: lane <-> entry; keep entries whose alpha >= 1/255 support box
-      //      overlaps this warp's 8x4 pixel block --------------------------------------------------
       bool hit = false;
       if (c0 + lane < cnt) {
         const float4 ra = s_c[st][0][c0 + lane];
@@ -202,71 +229,113 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
         const float ex = __low2float(ext), ey = __high2float(ext);
         hit = (ra.x + ex >= bx0) && (ra.x - ex <= bx1) && (ra.y + ey >= by0) && (ra.y - ey <= by1);
       }
-      unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
-      while (m) {
-        // ---- evaluate up to kGroup entries independently ---------------------------------------
-        int idx[kGroup];
-        float alpha[kGroup];
+      const unsigned m = __ballot_sync(FULL, hit);
+      if (hit) s_q[warp][nq + __popc(m & ((1u << lane) - 1u))] = (uint8_t)(c0 + lane);
+      nq += __popc(m);
+    }
+    __syncwarp();
+
+    // ---- walk the queue, U groups of E entries at a time --------------------------------------------
+    for (int q0 = 0; q0 < nq; q0 += E * U) {
+      int j[U];
+      float alpha[U];
 #pragma unroll
-        for (int k = 0; k < kGroup; ++k) {
-          idx[k] = m ? c0 + __ffs(m) - 1 : -1;
-          m &= m - 1;
+      for (int u = 0; u < U; ++u) {
+        const int qi = q0 + u * E + slot;
+        const bool have = qi < nq;
+        j[u] = s_q[warp][have ? qi : q0];
+        const float4 ra = s_c[st][0][j[u]];
+        const float4 rb = s_c[st][1][j[u]];
+        const float dx = fpx - ra.x, dy = fpy - ra.y;
+        const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
+        const float al = fminf(kAlphaMax, rb.w * __expf(power));
+        alpha[u] = (!have || done || power > 0.f || al < kAlphaMin) ? 0.f : al;
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        // front-to-back over the E slots of this group: T_{k+1} = T_k (1 - alpha_k), in list order
+        if (done) alpha[u] = 0.f;  // a stop in an earlier group of this iteration
+        const float om = 1.f - alpha[u];
+        float Tk = T, myT = T;
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+          const float omk = (E == 1) ? om : __shfl_sync(FULL, om, k * P + pix);
+          if (k == slot) myT = Tk;
+          Tk *= omk;
         }
+        float w;
+        if (__any_sync(FULL, Tk < kTMin)) {
+          // some pixel crosses T_min inside this group: apply the stop rule entry by entry
+          // (the entry that would take T below T_min is not blended, nor is anything behind it)
+          float Ts = T;
+          bool stop = done, mine = false;
 #pragma unroll
-        for (int k = 0; k < kGroup; ++k) {
-          alpha[k] = 0.f;
-          if (idx[k] >= 0) {
-            const float4 ra = s_c[st][0][idx[k]];
-            const float4 rb = s_c[st][1][idx[k]];
-            const float dx = fpx - ra.x, dy = fpy - ra.y;
-            const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
-            const float al = fminf(kAlphaMax, rb.w * __expf(power));
-            alpha[k] = (power > 0.f || al < kAlphaMin) ? 0.f : al;
-          }
-        }
-        // ---- blend sequentially (front to back) ------------------------------------------------
-#pragma unroll
-        for (int k = 0; k < kGroup; ++k) {
-          if (alpha[k] > 0.f && !done) {
-            const float Tn = T * (1.f - alpha[k]);
-            if (Tn < kTMin) {
-              done = true;
-            } else {
-              const int j = idx[k];
-              const float w = alpha[k] * T;
-              const float4 ra = s_c[st][0][j];
-              const float4 a0 = s_c[st][2][j], a1 = s_c[st][3][j], a2 = s_c[st][4][j];
-              acc[0] = fmaf(w, ra.z, acc[0]);
-              acc[1] = fmaf(w, a0.x, acc[1]);
-              acc[2] = fmaf(w, a0.y, acc[2]);
-              acc[3] = fmaf(w, a0.z, acc[3]);
-              acc[4] = fmaf(w, a1.x, acc[4]);
-              acc[5] = fmaf(w, a1.y, acc[5]);
-              acc[6] = fmaf(w, a1.z, acc[6]);
-              acc[7] = fmaf(w, a0.w, acc[7]);
-              acc[8] = fmaf(w, a1.w, acc[8]);
-              acc[9] = fmaf(w, a2.x, acc[9]);
-#pragma unroll
-              for (int l = 0; l < LB; ++l) {
-                const float4 mo = s_c[st][5 + l][j];
-                accl[l][0] = fmaf(w, mo.x, accl[l][0]);
-                accl[l][1] = fmaf(w, mo.y, accl[l][1]);
-                accl[l][2] = fmaf(w, mo.z, accl[l][2]);
-                accl[l][3] = fmaf(w, mo.w, accl[l][3]);
+          for (int k = 0; k < E; ++k) {
+            const float omk = (E == 1) ? om : __shfl_sync(FULL, om, k * P + pix);
+            if (!stop && omk < 1.f) {
+              const float Tn = Ts * omk;
+              if (Tn < kTMin) {
+                stop = true;
+              } else {
+                if (k == slot) { myT = Ts; mine = true; }
+                Ts = Tn;
               }
-              A += w;
-              T = Tn;
             }
           }
+          T = Ts;
+          done = stop;
+          w = mine ? alpha[u] * myT : 0.f;
+        } else {
+          T = Tk;
+          w = alpha[u] * myT;
         }
-        if (__all_sync(0xFFFFFFFFu, done)) { m = 0; c0 = cnt; }
+        if (__any_sync(FULL, w > 0.f)) {
+          const int jj = j[u];
+          const float4 ra = s_c[st][0][jj];
+          const float4 a0 = s_c[st][2][jj], a1 = s_c[st][3][jj], a2 = s_c[st][4][jj];
+          acc[0] = fmaf(w, ra.z, acc[0]);
+          acc[1] = fmaf(w, a0.x, acc[1]);
+          acc[2] = fmaf(w, a0.y, acc[2]);
+          acc[3] = fmaf(w, a0.z, acc[3]);
+          acc[4] = fmaf(w, a1.x, acc[4]);
+          acc[5] = fmaf(w, a1.y, acc[5]);
+          acc[6] = fmaf(w, a1.z, acc[6]);
+          acc[7] = fmaf(w, a0.w, acc[7]);
+          acc[8] = fmaf(w, a1.w, acc[8]);
+          acc[9] = fmaf(w, a2.x, acc[9]);
+#pragma unroll
+          for (int l = 0; l < LB; ++l) {
+            const float4 mo = s_c[st][5 + l][jj];
+            accl[l][0] = fmaf(w, mo.x, accl[l][0]);
+            accl[l][1] = fmaf(w, mo.y, accl[l][1]);
+            accl[l][2] = fmaf(w, mo.z, accl[l][2]);
+            accl[l][3] = fmaf(w, mo.w, accl[l][3]);
+          }
+          A += w;
+        }
       }
+      if (__all_sync(FULL, done)) break;
     }
   }
   cp_async_wait_all();
 
+  // ---- combine the E per-slot partial sums of every pixel (all E lanes end up with the total) ----
+  if (E > 1) {
+#pragma unroll
+    for (int o = P; o < 32; o <<= 1) {
+#pragma unroll
+      for (int c = 0; c < 10; ++c) acc[c] += __shfl_xor_sync(FULL, acc[c], o);
+#pragma unroll
+      for (int l = 0; l < LB; ++l)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) accl[l][c] += __shfl_xor_sync(FULL, accl[l][c], o);
+      A += __shfl_xor_sync(FULL, A, o);
+    }
+  }
+
   if (!inside) return;
-  // ---- epilogue: G-buffer stores + deferred shading, per light ---------------------------------
+  // ---- epilogue: G-buffer stores + deferred shading; lights and store quarters are dealt to the
+  //      E lanes of a pixel round-robin ---------------------------------------------------------------
   const int64_t pidx = (int64_t)py * cam.width + px;
   ShadeIn q;
   const bool covered = A >= 1e-6f;
@@ -280,11 +349,12 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     const int64_t fp = (int64_t)l * frame_stride_px + pidx;
     if (gbuf_out) {
       float4* gp = reinterpret_cast<float4*>(gbuf_out + fp * SSSGS_GBUF_CHANNELS);
-      gp[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-      gp[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-      gp[2] = make_float4(acc[8], acc[9], accl[l][0], accl[l][1]);
-      gp[3] = make_float4(accl[l][2], accl[l][3], A, T);
+      if (0 % E == slot) gp[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      if (1 % E == slot) gp[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      if (2 % E == slot) gp[2] = make_float4(acc[8], acc[9], accl[l][0], accl[l][1]);
+      if (3 % E == slot) gp[3] = make_float4(accl[l][2], accl[l][3], A, T);
     }
+    if (l % E != slot) continue;
     float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
     if (covered) {
       const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
@@ -330,30 +400,64 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
   return 1;
 }
 
+// Launches one rasteriser variant: LB lights per walk, E entry slots per warp, WARPS warps per CTA.
+template <int LB, int E, int WARPS, int U>
+static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_lights,
+                          const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
+                          const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
+                          int64_t frame_stride_px, int tiles, cudaStream_t s) {
+  using S = RasterShape<E, WARPS>;
+  constexpr int smem = 2 * (5 + LB) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch;
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U>,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+      return -1;
+    configured = true;
+  }
+  raster_shade_kernel<LB, E, WARPS, U><<<tiles * S::SUBS, S::THREADS, smem, s>>>(
+      cam, lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out,
+      rgb, gbuf, aov_d, aov_s, frame_stride_px);
+  return 1;
+}
+
+// Tuning aid: SSSGS_RASTER_MODE = "<E><W>" digits, e.g. "18" (E=1, 8 warps: one CTA per tile, one
+// thread per pixel), "48" (E=4, 8 warps: four 8x8-pixel CTAs per tile), "416" (E=4, 16 warps).
+static int raster_mode() {
+  static int mode = -1;
+  if (mode < 0) {
+    const char* e = getenv("SSSGS_RASTER_MODE");
+    mode = e ? atoi(e) : 0;
+  }
+  return mode;
+}
+
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                   const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
                   int64_t frame_stride_px, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
-#define SSSGS_RASTER(LB)                                                                          \
-  do {                                                                                            \
-    constexpr int smem = 2 * (5 + LB) * kBatch * 16 + 2 * kBatch * 4;                             \
-    static bool configured = false;                                                               \
-    if (!configured) {                                                                            \
-      if (cudaFuncSetAttribute(raster_shade_kernel<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                               smem) != cudaSuccess) return -1;                                   \
-      configured = true;                                                                          \
-    }                                                                                             \
-    raster_shade_kernel<LB><<<tiles, kRasterThreads, smem, s>>>(                                  \
-        cam, lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr,   \
-        mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px);                                       \
+  int mode = raster_mode();
+  if (mode == 0) mode = 48;
+#define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s
+#define SSSGS_BY_LB(E, W, U)                                                   \
+  do {                                                                         \
+    if (n_lights <= 1) return launch_variant<1, E, W, U>(SSSGS_ARGS);          \
+    if (n_lights <= 4) return launch_variant<4, E, W, U>(SSSGS_ARGS);          \
+    return launch_variant<8, E, W, U>(SSSGS_ARGS);                             \
   } while (0)
-  if (n_lights <= 1) SSSGS_RASTER(1);
-  else if (n_lights <= 4) SSSGS_RASTER(4);
-  else SSSGS_RASTER(8);
-#undef SSSGS_RASTER
-  return 1;
+  switch (mode) {
+    case 18: SSSGS_BY_LB(1, 8, 4);
+    case 28: SSSGS_BY_LB(2, 8, 2);
+    case 216: SSSGS_BY_LB(2, 16, 2);
+    case 48: SSSGS_BY_LB(4, 8, 2);
+    case 416: SSSGS_BY_LB(4, 16, 2);
+    case 88: SSSGS_BY_LB(8, 8, 1);
+    default: SSSGS_BY_LB(4, 8, 2);
+  }
+#undef SSSGS_BY_LB
+#undef SSSGS_ARGS
 }
 
 }  // namespace sssgs

@@ -9,7 +9,7 @@
 //
 // Structure of a pass (persistent CTAs pulling tickets, so a CTA only ever waits on tickets
 // that are already running -> forward progress):
-//   1. load 256 x 15 keys warp-striped (coalesced), rank them per warp with __match_any_sync
+//   1. load 256 x ITEMS keys (ITEMS = 3, 7 or 15 by problem size) warp-striped (coalesced), rank them per warp with __match_any_sync
 //      (stable: item order, then lane order), combine the per-warp digit counts,
 //   2. publish the CTA's digit counts and resolve its global offsets by decoupled look-back
 //      over the status words of earlier tickets (flag and 30-bit count share one word, so no
@@ -52,63 +52,63 @@ __device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* tm
   return wbase + inc - v;
 }
 
-__global__ void __launch_bounds__(kSortThreads)
-radix_pass_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
-                  uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                  const uint32_t* __restrict__ count_ptr, uint32_t count_cap, int shift, int bits,
-                  const uint32_t* __restrict__ hist, uint32_t* __restrict__ status,
-                  uint32_t* __restrict__ ticket, uint32_t* __restrict__ err) {
-  __shared__ uint32_t s_keys[kSortTile];
-  __shared__ uint32_t s_vals[kSortTile];
-  __shared__ uint32_t s_wcnt[kSortThreads / 32][kRadixMax];
-  __shared__ uint32_t s_binstart[kRadixMax];
-  __shared__ uint32_t s_digstart[kRadixMax];
-  __shared__ uint32_t s_gbase[kRadixMax];
-  __shared__ uint32_t s_tmp[8];
-  __shared__ uint32_t s_ticket;
+constexpr int kLookW = 8;  // look-back status words in flight per thread
 
+struct SortSmem {
+  uint32_t keys[kSortTileMax];
+  uint32_t vals[kSortTileMax];
+  uint32_t wcnt[kSortThreads / 32][kRadixMax];
+  uint32_t binstart[kRadixMax];
+  uint32_t digstart[kRadixMax];
+  uint32_t gbase[kRadixMax];
+  uint32_t tmp[8];
+  uint32_t ticket;
+};
+
+// Processes tickets of 256 x ITEMS keys until the ticket counter runs out.
+template <int ITEMS>
+__device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __restrict__ keys_in,
+                                             const uint32_t* __restrict__ vals_in,
+                                             uint32_t* __restrict__ keys_out,
+                                             uint32_t* __restrict__ vals_out, uint32_t n, int shift,
+                                             uint32_t radix, uint32_t mask,
+                                             uint32_t* __restrict__ status,
+                                             uint32_t* __restrict__ ticket, uint32_t* __restrict__ err) {
+  constexpr uint32_t TILE = kSortThreads * ITEMS;
   const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t n = count_ptr ? min(*count_ptr, count_cap) : count_cap;
-  const uint32_t ntiles = (n + kSortTile - 1) / kSortTile;
-  const uint32_t radix = 1u << bits, mask = radix - 1u;
-
-  // start of every digit bin in the output = exclusive scan of the global histogram
-  {
-    const uint32_t h = tid < radix ? hist[tid] : 0u;
-    const uint32_t ex = block_excl_scan_256(h, s_tmp);
-    s_binstart[tid] = ex;
-  }
-
+  const uint32_t ntiles = (n + TILE - 1) / TILE;
   while (true) {
-    __syncthreads();  // also protects s_keys/s_vals/s_wcnt of the previous ticket
-    if (tid == 0) s_ticket = atomicAdd(ticket, 1u);
+    __syncthreads();  // also protects keys/vals/wcnt of the previous ticket
+    if (tid == 0) sm.ticket = atomicAdd(ticket, 1u);
     __syncthreads();
-    const uint32_t t = s_ticket;
+    const uint32_t t = sm.ticket;
     if (t >= ntiles) break;
 
     // ---- 1. load + per-warp stable ranking ------------------------------------------------
-    const uint32_t tile_base = t * (uint32_t)kSortTile;
-    const uint32_t tile_count = min((uint32_t)kSortTile, n - tile_base);
-    uint32_t key[kSortItems], val[kSortItems];
-    uint32_t rank[kSortItems];
-    const uint32_t first = tile_base + warp * (32u * kSortItems) + lane;
+    const uint32_t tile_base = t * TILE;
+    const uint32_t tile_count = min(TILE, n - tile_base);
+    uint32_t key[ITEMS], val[ITEMS], rank[ITEMS];
+    unsigned peers[ITEMS];
+    const uint32_t first = tile_base + warp * (32u * ITEMS) + lane;
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
       const uint32_t idx = first + 32u * i;
       const bool ok = idx < n;
       key[i] = ok ? keys_in[idx] : 0xFFFFFFFFu;
       val[i] = ok ? (vals_in ? vals_in[idx] : idx) : 0u;
     }
-    for (uint32_t d = lane; d < radix; d += 32) s_wcnt[warp][d] = 0;
+    for (uint32_t d = lane; d < radix; d += 32) sm.wcnt[warp][d] = 0;
+    // the matches of all items are independent of each other: issue them back to back
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) peers[i] = __match_any_sync(0xFFFFFFFFu, (key[i] >> shift) & mask);
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
       const uint32_t d = (key[i] >> shift) & mask;
-      const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-      const uint32_t r = __popc(peers & ((1u << lane) - 1u));
-      const uint32_t base = s_wcnt[warp][d];
+      const uint32_t r = __popc(peers[i] & ((1u << lane) - 1u));
+      const uint32_t base = sm.wcnt[warp][d];
       __syncwarp();
-      if (r == 0) s_wcnt[warp][d] = base + __popc(peers);
+      if (r == 0) sm.wcnt[warp][d] = base + __popc(peers[i]);
       __syncwarp();
       rank[i] = base + r;
     }
@@ -119,15 +119,15 @@ radix_pass_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restri
     if (tid < radix) {
 #pragma unroll
       for (int w = 0; w < kSortThreads / 32; ++w) {
-        const uint32_t c = s_wcnt[w][tid];
-        s_wcnt[w][tid] = total;
+        const uint32_t c = sm.wcnt[w][tid];
+        sm.wcnt[w][tid] = total;
         total += c;
       }
       // padding keys (0xFFFFFFFF, only in the last ticket) were ranked last in the last bin
-      if (tid == mask) total -= (uint32_t)kSortTile - tile_count;
+      if (tid == mask) total -= TILE - tile_count;
     }
-    const uint32_t dig_start = block_excl_scan_256(total, s_tmp);
-    if (tid < radix) s_digstart[tid] = dig_start;
+    const uint32_t dig_start = block_excl_scan_256(total, sm.tmp);
+    if (tid < radix) sm.digstart[tid] = dig_start;
 
     // ---- 2. decoupled look-back --------------------------------------------------------------
     if (tid < radix) {
@@ -137,44 +137,82 @@ radix_pass_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restri
         st_volatile(my, kFlagInc | total);
       } else {
         st_volatile(my, kFlagAgg | total);
+        // walk back over earlier tickets, kLookW status words in flight at a time (the loads are
+        // independent; only a word that is not published yet is re-read)
         int spins = 0;
-        for (uint32_t tt = t; tt-- > 0;) {
-          const uint32_t* p = status + (size_t)tt * kRadixMax + tid;
-          uint32_t v = ld_volatile(p);
-          while ((v & kFlagMask) == 0u) {
-            if (++spins > kSpinLimit) {
-              atomicExch(err, 1u);
-              v = kFlagInc;  // give up: result undefined, but no hang
-              break;
+        bool found = false;
+        for (int64_t tt = (int64_t)t - 1; !found; tt -= kLookW) {
+          uint32_t v[kLookW];
+#pragma unroll
+          for (int k = 0; k < kLookW; ++k)
+            v[k] = tt - k >= 0 ? ld_volatile(status + (size_t)(tt - k) * kRadixMax + tid) : kFlagInc;
+#pragma unroll
+          for (int k = 0; k < kLookW; ++k) {
+            if (!found) {
+              while ((v[k] & kFlagMask) == 0u) {
+                if (++spins > kSpinLimit) {
+                  atomicExch(err, 1u);
+                  v[k] = kFlagInc;  // give up: result undefined, but no hang
+                  break;
+                }
+                __nanosleep(20);
+                v[k] = ld_volatile(status + (size_t)(tt - k) * kRadixMax + tid);
+              }
+              excl += v[k] & kValMask;
+              found = (v[k] & kFlagInc) != 0u;
             }
-            __nanosleep(32);
-            v = ld_volatile(p);
           }
-          excl += v & kValMask;
-          if (v & kFlagInc) break;
         }
         st_volatile(my, kFlagInc | ((excl + total) & kValMask));
       }
-      s_gbase[tid] = s_binstart[tid] + excl - dig_start;
+      sm.gbase[tid] = sm.binstart[tid] + excl - dig_start;
     }
     __syncthreads();
 
     // ---- 3. reorder through shared memory, then coalesced scatter ----------------------------
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
+    for (int i = 0; i < ITEMS; ++i) {
       const uint32_t d = (key[i] >> shift) & mask;
-      const uint32_t pos = s_digstart[d] + s_wcnt[warp][d] + rank[i];
-      s_keys[pos] = key[i];
-      s_vals[pos] = val[i];
+      const uint32_t pos = sm.digstart[d] + sm.wcnt[warp][d] + rank[i];
+      sm.keys[pos] = key[i];
+      sm.vals[pos] = val[i];
     }
     __syncthreads();
     for (uint32_t j = tid; j < tile_count; j += kSortThreads) {
-      const uint32_t k = s_keys[j];
-      const uint32_t dst = s_gbase[(k >> shift) & mask] + j;
+      const uint32_t k = sm.keys[j];
+      const uint32_t dst = sm.gbase[(k >> shift) & mask] + j;
       if (keys_out) keys_out[dst] = k;
-      vals_out[dst] = s_vals[j];
+      vals_out[dst] = sm.vals[j];
     }
   }
+}
+
+__global__ void __launch_bounds__(kSortThreads)
+radix_pass_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
+                  uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
+                  const uint32_t* __restrict__ count_ptr, uint32_t count_cap, int shift, int bits,
+                  const uint32_t* __restrict__ hist, uint32_t* __restrict__ status,
+                  uint32_t* __restrict__ ticket, uint32_t* __restrict__ err) {
+  __shared__ SortSmem sm;
+  const unsigned tid = threadIdx.x;
+  const uint32_t n = count_ptr ? min(*count_ptr, count_cap) : count_cap;
+  const uint32_t radix = 1u << bits, mask = radix - 1u;
+
+  // start of every digit bin in the output = exclusive scan of the global histogram
+  {
+    const uint32_t h = tid < radix ? hist[tid] : 0u;
+    const uint32_t ex = block_excl_scan_256(h, sm.tmp);
+    sm.binstart[tid] = ex;
+  }
+  // ticket size by problem size (uniform over the grid): small inputs are split finely so that
+  // every SM gets work, large ones use long tickets that amortise the look-back
+  const int items = sort_items_for(n);
+  if (items == 3)
+    sort_tickets<3>(sm, keys_in, vals_in, keys_out, vals_out, n, shift, radix, mask, status, ticket, err);
+  else if (items == 7)
+    sort_tickets<7>(sm, keys_in, vals_in, keys_out, vals_out, n, shift, radix, mask, status, ticket, err);
+  else
+    sort_tickets<15>(sm, keys_in, vals_in, keys_out, vals_out, n, shift, radix, mask, status, ticket, err);
 }
 
 }  // namespace
@@ -184,7 +222,7 @@ int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t*
                      int bits, const uint32_t* hist, uint32_t* status, uint32_t* ticket,
                      uint32_t* err, int max_blocks, cudaStream_t s) {
   if (count_cap == 0) return 0;
-  int64_t blocks = ((int64_t)count_cap + kSortTile - 1) / kSortTile;
+  int64_t blocks = (int64_t)sort_status_rows(count_cap);
   if (blocks > max_blocks) blocks = max_blocks;
   radix_pass_kernel<<<(unsigned)blocks, kSortThreads, 0, s>>>(
       keys_in, vals_in, keys_out, vals_out, count_ptr, count_cap, shift, bits, hist, status, ticket,

@@ -28,7 +28,9 @@ struct sssgs_ctx {
   uint32_t* status_depth[4] = {};
   uint32_t* status_tile[2] = {};
   uint32_t* status_emit = nullptr;
-  float4* mlp_out = nullptr;
+  float4* mlp_out[2] = {};     // double-buffered: the MLP of batch k+1 overlaps the raster of batch k
+  cudaStream_t side = nullptr; // the MLP runs here, concurrently with the geometry stages
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_mlp[2] = {}, ev_raster[2] = {};
   uint8_t* mlp_blob = nullptr;
   float* mlp_bias = nullptr;
   int64_t launches = 0;
@@ -99,8 +101,8 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   for (int k = 0; k < 2; ++k) { p = take(cap * 4); if (c) c->gb.ivals[k] = (uint32_t*)p; }
   p = take(tiles * 8); if (c) c->gb.ranges = (uint2*)p;
   p = take(tiles * 4); if (c) c->gb.tile_order = (uint32_t*)p;
-  p = take(tiles * 4); if (c) c->gb.tile_slot = (uint32_t*)p;
-  p = take(n * (size_t)lb * 16); if (c) c->mlp_out = (float4*)p;
+  p = take((tiles + 1) * 4); if (c) c->gb.tile_slot = (uint32_t*)p;
+  for (int k = 0; k < 2; ++k) { p = take(n * (size_t)lb * 16); if (c) c->mlp_out[k] = (float4*)p; }
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
   p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
   // control block: everything that must be zero at the start of a camera
@@ -108,7 +110,7 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   if (c) c->control = base ? base + off : nullptr;
   p = take(6 * 256 * 4); if (c) c->gb.hist = (uint32_t*)p;
   p = take(DC_WORDS * 4); if (c) c->gb.counters = (uint32_t*)p;
-  const size_t nblk_d = (n + kSortTile - 1) / kSortTile, nblk_i = (cap + kSortTile - 1) / kSortTile;
+  const size_t nblk_d = sort_status_rows((uint32_t)n), nblk_i = sort_status_rows((uint32_t)cap);
   for (int k = 0; k < 4; ++k) { p = take(nblk_d * kRadixMax * 4); if (c) c->status_depth[k] = (uint32_t*)p; }
   for (int k = 0; k < 2; ++k) { p = take(nblk_i * kRadixMax * 4); if (c) c->status_tile[k] = (uint32_t*)p; }
   p = take(((n + kEmitChunk - 1) / kEmitChunk) * 4); if (c) c->status_emit = (uint32_t*)p;
@@ -258,6 +260,13 @@ int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
     c->owns_ws = true;
   }
   carve(c, *cfg, c->ws);
+  bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess;
+  cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_join, &c->ev_mlp[0], &c->ev_mlp[1], &c->ev_raster[0], &c->ev_raster[1]};
+  for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) {
+    sssgs_destroy(c);
+    return fail(nullptr, SSSGS_ECUDA, "could not create the side stream / events");
+  }
   *out = c;
   return SSSGS_OK;
 }
@@ -268,6 +277,10 @@ void sssgs_destroy(sssgs_ctx* c) {
     if (s.first) cudaFree(s.first);
   for (auto& sp : c->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto& e : c->pool) cudaEventDestroy(e);
+  cudaEvent_t evs[] = {c->ev_fork, c->ev_join, c->ev_mlp[0], c->ev_mlp[1], c->ev_raster[0], c->ev_raster[1]};
+  for (cudaEvent_t e : evs)
+    if (e) cudaEventDestroy(e);
+  if (c->side) cudaStreamDestroy(c->side);
   if (c->owns_ws && c->ws) cudaFree(c->ws);
   delete c;
 }
@@ -369,11 +382,22 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     if (c->profile && !c->spans.empty()) cudaEventRecord(c->spans.back().b, s);
     cur_stage = -1;
   };
+  // The MLP depends on the view and the light but not on the geometry stages, so it runs on the
+  // context's side stream and overlaps projection / sort / binning (and, in a sweep, the raster of
+  // the previous light batch).  With per-stage timing on, everything is serialised on `s` so that
+  // each stage is timed alone.
+  const bool overlap = run_mlp && !c->profile && g->n > 0 && n_light > 0 && n_cam > 0;
+  cudaStream_t sm = overlap ? c->side : s;
+  if (overlap) {
+    if (cudaEventRecord(c->ev_fork, s) != cudaSuccess || cudaStreamWaitEvent(sm, c->ev_fork, 0) != cudaSuccess)
+      return fail(c, SSSGS_ECUDA, "stream fork failed");
+  }
 
   begin(SSSGS_STAGE_PACK);
   if (add(launch_pack_attr(*g, c->attr, s)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
-  if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, s));
+  if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, sm));
   end();
+  int64_t batch_no = 0;
 
   const int64_t npix_max = 0;
   (void)npix_max;
@@ -442,15 +466,22 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         memcpy(lb.l[l].intensity, L.intensity, 12);
       }
       const int64_t frame0 = (int64_t)v * n_light + l0;
+      const int buf = (int)(batch_no & 1);
+      float4* mlp_buf = c->mlp_out[buf];
       begin(SSSGS_STAGE_MLP);
       if (run_mlp) {
-        const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, c->mlp_out,
+        // buffer `buf` was last read by the raster of batch_no - 2
+        if (overlap && batch_no >= 2 && cudaStreamWaitEvent(sm, c->ev_raster[buf], 0) != cudaSuccess)
+          return fail(c, SSSGS_ECUDA, "stream wait failed");
+        const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, mlp_buf,
                                  out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
-                                 c->num_sms, s);
+                                 c->num_sms, sm);
         if (k < 0) return fail(c, SSSGS_ECUDA, "MLP kernel configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
         add(k);
+        if (overlap && (cudaEventRecord(c->ev_mlp[buf], sm) != cudaSuccess || cudaStreamWaitEvent(s, c->ev_mlp[buf], 0) != cudaSuccess))
+          return fail(c, SSSGS_ECUDA, "stream join failed");
       } else {
-        add(launch_gather_precomputed(mlp->precomputed_out + frame0 * g->n * 4, g->n, nl, g->n * 4, c->mlp_out, s));
+        add(launch_gather_precomputed(mlp->precomputed_out + frame0 * g->n * 4, g->n, nl, g->n * 4, mlp_buf, s));
         if (out->mlp_out && g->n > 0)
           if (cudaMemcpyAsync(out->mlp_out + frame0 * g->n * 4, mlp->precomputed_out + frame0 * g->n * 4,
                               (size_t)nl * g->n * 16, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
@@ -458,13 +489,19 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       }
       end();
       begin(SSSGS_STAGE_RASTER);
-      add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, c->mlp_out,
+      add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf,
                         out->rgb ? out->rgb + frame0 * npix * 3 : nullptr,
                         out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr,
                         out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr,
                         out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix, s));
       end();
+      if (overlap && cudaEventRecord(c->ev_raster[buf], s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "event record failed");
+      ++batch_no;
     }
+  }
+  if (overlap) {  // everything on the side stream is ordered before the end of the call on `s`
+    if (cudaEventRecord(c->ev_join, sm) != cudaSuccess || cudaStreamWaitEvent(s, c->ev_join, 0) != cudaSuccess)
+      return fail(c, SSSGS_ECUDA, "stream join failed");
   }
   c->launches = launches;
   const cudaError_t e = cudaGetLastError();
