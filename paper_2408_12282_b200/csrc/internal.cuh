@@ -42,6 +42,26 @@ constexpr uint32_t kFlagMask = 3u << 30;
 constexpr uint32_t kValMask = ~kFlagMask;
 constexpr int kSpinLimit = 1 << 24;  // bug trap for look-back waits (sets SSSGS_CNT_SORT_ERROR)
 
+// Depth-sort passes whose digit is the same for all n keys are identity permutations and are
+// skipped on the device (for an object in front of the camera the exponent byte of the depth
+// usually is).  Counts the passes among [0, upto) that do run: a pass runs if its histogram has
+// no bin holding all n keys; the last pass also runs if nothing ran before it, so that the
+// sorted index array always exists.  Called by all 256 threads of a CTA; hist = 4 x 256 words.
+#ifdef __CUDACC__
+__device__ __forceinline__ int depth_passes_run(const uint32_t* __restrict__ hist, uint32_t n, int upto,
+                                                bool* runs_last) {
+  int ran = 0;
+  bool r = true;
+  for (int q = 0; q < upto; ++q) {
+    const bool trivial = __syncthreads_or(hist[q * 256 + threadIdx.x] == n) != 0;
+    r = !trivial || (q == 3 && ran == 0);
+    ran += r ? 1 : 0;
+  }
+  if (runs_last) *runs_last = r;
+  return ran;
+}
+#endif
+
 // ---- emit (scan + expand) geometry ----------------------------------------------------------
 constexpr int kEmitThreads = 256;
 constexpr int kEmitChunk = kEmitThreads;  // Gaussians per ticket
@@ -80,7 +100,7 @@ enum {
 // Geometry buffers of one camera view.
 struct GeomBuffers {
   float4* rec_a;      // [n] (pix_x, pix_y, depth, half2 support half-extents ex|ey)
-  float4* rec_b;      // [n] (conic a, conic b, conic c, opacity)
+  float4* rec_b;      // [n] (-log2e/2 conic a, -log2e conic b, -log2e/2 conic c, opacity)
   uint2* rect;        // [n] packed tile rect: x = x0 | x1<<16, y = y0 | y1<<16
   uint32_t* touched;  // [n]
   uint32_t* dkeys[2]; // [n] depth keys ping/pong
@@ -131,14 +151,18 @@ int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t*
                      uint32_t* vals_out, const uint32_t* count_ptr, uint32_t count_cap, int shift,
                      int bits, const uint32_t* hist, uint32_t* status, uint32_t* ticket,
                      uint32_t* err, int max_blocks, cudaStream_t s);
-int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_idx,
-                uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
+// depth pass `pass` of 4 over the ping-pong buffers keys[2] / vals[2] (skipped on the device when
+// trivial, see depth_passes_run); hist4 = the 4 x 256 depth-digit histograms
+int launch_depth_pass(uint32_t* const keys[2], uint32_t* const vals[2], uint32_t n, int pass,
+                      const uint32_t* hist4, uint32_t* status, uint32_t* ticket, uint32_t* err,
+                      int max_blocks, cudaStream_t s);
+int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
                 uint32_t* status, uint32_t* ticket, cudaStream_t s);
 int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
-                  uint32_t cap, uint2* ranges_user, cudaStream_t s);
+                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, cudaStream_t s);
 int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_vals,
                         const GeomBuffers& gb, uint32_t cap, uint64_t* keys_out, uint32_t* vals_out,
-                        int64_t* counters_out, cudaStream_t s);
+                        cudaStream_t s);
 int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
                     cudaStream_t s);
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,

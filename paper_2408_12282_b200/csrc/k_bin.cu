@@ -25,8 +25,8 @@ __device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v) {
 }
 
 __global__ void __launch_bounds__(kEmitThreads)
-emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
-            const uint32_t* __restrict__ touched, const uint2* __restrict__ rect, int tiles_x,
+emit_kernel(uint32_t n, const uint32_t* __restrict__ dvals0, const uint32_t* __restrict__ dvals1,
+            const uint32_t* __restrict__ depth_hist, const uint32_t* __restrict__ touched, const uint2* __restrict__ rect, int tiles_x,
             uint32_t cap, uint32_t* __restrict__ ikeys, uint32_t* __restrict__ ivals,
             uint32_t* __restrict__ hist0, uint32_t* __restrict__ hist1, int shift0, int bits0,
             int shift1, int bits1, uint32_t* __restrict__ status, uint32_t* __restrict__ ticket,
@@ -40,6 +40,8 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
   const uint32_t mask0 = (1u << bits0) - 1u, mask1 = bits1 ? (1u << bits1) - 1u : 0u;
   s_hist[0][tid] = 0;
   s_hist[1][tid] = 0;
+  // the depth-sorted index array sits in the buffer the last executed depth pass wrote
+  const uint32_t* __restrict__ sorted_idx = (depth_passes_run(depth_hist, n, 4, nullptr) & 1) ? dvals1 : dvals0;
 
   while (true) {
     __syncthreads();
@@ -139,7 +141,9 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
         const uint32_t k = o - l_off;
         const uint32_t x0 = l_rx & 0xFFFFu, x1 = l_rx >> 16, y0 = l_ry & 0xFFFFu;
         const uint32_t w = x1 - x0;
-        const uint32_t ty = y0 + k / w, tx = x0 + k % w;
+        // k < tiles touched <= 65536 and w <= 4096: the float quotient of (k + 0.5) / w floors exactly
+        const uint32_t row = (uint32_t)__fdividef((float)k + 0.5f, (float)w);
+        const uint32_t ty = y0 + row, tx = x0 + (k - row * w);
         const uint32_t tile = ty * (uint32_t)tiles_x + tx;
         ikeys[dst] = tile;
         ivals[dst] = l_g;
@@ -174,7 +178,8 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ sorted_idx,
 __global__ void __launch_bounds__(256)
 ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ counters,
               uint32_t cap, int tiles, uint2* __restrict__ ranges, uint2* __restrict__ ranges_user,
-              uint32_t* __restrict__ lb, uint32_t* __restrict__ tile_order) {
+              uint32_t* __restrict__ lb, uint32_t* __restrict__ tile_order,
+              int64_t* __restrict__ counters_out) {
   __shared__ uint32_t s_cnt[32], s_start[32];
   __shared__ bool s_last;
   const uint32_t n = min(counters[DC_INSTANCES], cap);
@@ -190,6 +195,14 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
   if (!s_last) return;
   __threadfence();
   if (threadIdx.x < 32) s_cnt[threadIdx.x] = 0;
+  if (counters_out && threadIdx.x < SSSGS_NCOUNTERS) {
+    int64_t v = 0;
+    if (threadIdx.x == SSSGS_CNT_NVIS) v = counters[DC_NVIS];
+    if (threadIdx.x == SSSGS_CNT_INSTANCES) v = counters[DC_INSTANCES];
+    if (threadIdx.x == SSSGS_CNT_OVERFLOW) v = counters[DC_OVERFLOW];
+    if (threadIdx.x == SSSGS_CNT_SORT_ERROR) v = counters[DC_SORT_ERROR];
+    counters_out[threadIdx.x] = v;
+  }
   __syncthreads();
   for (int t = threadIdx.x; t < tiles; t += 256) {
     const uint32_t b0 = __ldcg(&lb[t]), b1 = __ldcg(&lb[t + 1]);
@@ -214,17 +227,8 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
 __global__ void __launch_bounds__(256)
 export_lists_kernel(const uint32_t* __restrict__ sorted_tiles, const uint32_t* __restrict__ sorted_vals,
                     const float4* __restrict__ rec_a, const uint32_t* __restrict__ counters,
-                    uint32_t cap, uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                    int64_t* __restrict__ counters_out) {
+                    uint32_t cap, uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
   const uint32_t n = min(counters[DC_INSTANCES], cap);
-  if (counters_out && blockIdx.x == 0 && threadIdx.x < SSSGS_NCOUNTERS) {
-    int64_t v = 0;
-    if (threadIdx.x == SSSGS_CNT_NVIS) v = counters[DC_NVIS];
-    if (threadIdx.x == SSSGS_CNT_INSTANCES) v = counters[DC_INSTANCES];
-    if (threadIdx.x == SSSGS_CNT_OVERFLOW) v = counters[DC_OVERFLOW];
-    if (threadIdx.x == SSSGS_CNT_SORT_ERROR) v = counters[DC_SORT_ERROR];
-    counters_out[threadIdx.x] = v;
-  }
   for (uint32_t j = blockIdx.x * 256u + threadIdx.x; j < n; j += gridDim.x * 256u) {
     const uint32_t g = sorted_vals[j];
     if (keys_out) keys_out[j] = ((uint64_t)sorted_tiles[j] << 32) | __float_as_uint(rec_a[g].z);
@@ -234,39 +238,36 @@ export_lists_kernel(const uint32_t* __restrict__ sorted_tiles, const uint32_t* _
 
 }  // namespace
 
-int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_idx,
-                uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
+int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
                 uint32_t* status, uint32_t* ticket, cudaStream_t s) {
   if (n == 0) return 0;
   int64_t blocks = (n + kEmitChunk - 1) / kEmitChunk;
   if (blocks > 148 * 4) blocks = 148 * 4;
   emit_kernel<<<(unsigned)blocks, kEmitThreads, 0, s>>>(
-      (uint32_t)n, sorted_idx, gb.touched, gb.rect, cam.tiles_x, cap, gb.ikeys[0], gb.ivals[0],
+      (uint32_t)n, gb.dvals[0], gb.dvals[1], gb.hist, gb.touched, gb.rect, cam.tiles_x, cap, gb.ikeys[0], gb.ivals[0],
       gb.hist + 4 * 256, gb.hist + 5 * 256, tile_shift0, tile_bits0, tile_shift1, tile_bits1, status,
       ticket, gb.counters);
   return 1;
 }
 
 int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
-                  uint32_t cap, uint2* ranges_user, cudaStream_t s) {
+                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   int64_t blocks = ((int64_t)cap + 1 + 1023) / 1024;
   if (blocks > 148 * 4) blocks = 148 * 4;
   ranges_kernel<<<(unsigned)blocks, 256, 0, s>>>(sorted_tiles, gb.counters, cap, tiles, gb.ranges,
-                                                 ranges_user, gb.tile_slot, gb.tile_order);
+                                                 ranges_user, gb.tile_slot, gb.tile_order, counters_out);
   return 1;
 }
 
 int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_vals,
                         const GeomBuffers& gb, uint32_t cap, uint64_t* keys_out, uint32_t* vals_out,
-                        int64_t* counters_out, cudaStream_t s) {
+                        cudaStream_t s) {
   int64_t blocks = ((int64_t)cap + 255) / 256;
   if (blocks > 148 * 8) blocks = 148 * 8;
   if (blocks < 1) blocks = 1;
-  if (!keys_out && !vals_out) blocks = 1;
   export_lists_kernel<<<(unsigned)blocks, 256, 0, s>>>(sorted_tiles, sorted_vals, gb.rec_a,
-                                                       gb.counters, cap, keys_out, vals_out,
-                                                       counters_out);
+                                                       gb.counters, cap, keys_out, vals_out);
   return 1;
 }
 

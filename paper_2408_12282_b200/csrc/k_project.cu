@@ -148,7 +148,10 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
             }
             const __half2 ext = __halves2half2(__float2half_ru(fminf(ex, 60000.f)), __float2half_ru(fminf(ey, 60000.f)));
             ra = make_float4(pix_x, pix_y, z, __uint_as_float(*reinterpret_cast<const uint32_t*>(&ext)));
-            rb = make_float4(con_a, con_b, con_c, o);
+            // the rasteriser evaluates alpha = o * 2^(A' dx^2 + B' dx dy + C' dy^2): conic pre-scaled
+            // by log2(e) (and the -1/2); not part of any key or rect
+            constexpr float kLog2e = 1.4426950408889634f;
+            rb = make_float4(-0.5f * kLog2e * con_a, -kLog2e * con_b, -0.5f * kLog2e * con_c, o);
             rc = make_uint2((uint32_t)x0 | ((uint32_t)x1 << 16), (uint32_t)y0 | ((uint32_t)y1 << 16));
           }
         }

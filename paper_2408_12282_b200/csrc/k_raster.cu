@@ -110,6 +110,12 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
   const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+// 2^x, single MUFU.EX2 (flushes denormal results to zero: alpha is thresholded at 1/255 anyway)
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -164,7 +170,9 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   const int px = bx + pix % S::PW, py = by + pix / S::PW;
   const bool inside = px < cam.width && py < cam.height;
   const float fpx = (float)px, fpy = (float)py;
-  const float bx0 = (float)bx, bx1 = (float)(bx + S::PW - 1), by0 = (float)by, by1 = (float)(by + S::PH - 1);
+  // centre and half-size of this warp's pixel block
+  constexpr float bhw = 0.5f * (S::PW - 1), bhh = 0.5f * (S::PH - 1);
+  const float bcx = (float)bx + bhw, bcy = (float)by + bhh;
 
   const uint2 range = ranges[tile];
   float T = 1.f, A = 0.f;  // T is identical in the E lanes of a pixel; A is a per-lane partial sum
@@ -225,9 +233,9 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
       bool hit = false;
       if (c0 + lane < cnt) {
         const float4 ra = s_c[st][0][c0 + lane];
-        const __half2 ext = *reinterpret_cast<const __half2*>(&ra.w);
-        const float ex = __low2float(ext), ey = __high2float(ext);
-        hit = (ra.x + ex >= bx0) && (ra.x - ex <= bx1) && (ra.y + ey >= by0) && (ra.y - ey <= by1);
+        const float2 ext = __half22float2(*reinterpret_cast<const __half2*>(&ra.w));
+        // support box [pix - ext, pix + ext] against the block [bcx - bhw, bcx + bhw] (same in y)
+        hit = fabsf(ra.x - bcx) <= ext.x + bhw && fabsf(ra.y - bcy) <= ext.y + bhh;
       }
       const unsigned m = __ballot_sync(FULL, hit);
       if (hit) s_q[warp][nq + __popc(m & ((1u << lane) - 1u))] = (uint8_t)(c0 + lane);
@@ -238,18 +246,20 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     // ---- walk the queue, U groups of E entries at a time --------------------------------------------
     for (int q0 = 0; q0 < nq; q0 += E * U) {
       int j[U];
-      float alpha[U];
+      float alpha[U], zed[U];
 #pragma unroll
       for (int u = 0; u < U; ++u) {
         const int qi = q0 + u * E + slot;
-        const bool have = qi < nq;
-        j[u] = s_q[warp][have ? qi : q0];
+        const bool live = qi < nq && !done;
+        j[u] = s_q[warp][qi < nq ? qi : q0];
         const float4 ra = s_c[st][0][j[u]];
-        const float4 rb = s_c[st][1][j[u]];
+        const float4 rb = s_c[st][1][j[u]];  // conic pre-scaled for exp2 (see project_kernel)
         const float dx = fpx - ra.x, dy = fpy - ra.y;
-        const float power = -0.5f * (rb.x * dx * dx + rb.z * dy * dy) - rb.y * dx * dy;
-        const float al = fminf(kAlphaMax, rb.w * __expf(power));
-        alpha[u] = (!have || done || power > 0.f || al < kAlphaMin) ? 0.f : al;
+        // p = log2(e) * (-1/2 d^T Sigma'^-1 d)
+        const float p = fmaf(fmaf(rb.y, dy, rb.x * dx), dx, rb.z * dy * dy);
+        const float al = fminf(kAlphaMax, rb.w * ex2_approx(p));
+        alpha[u] = (live && p <= 0.f && al >= kAlphaMin) ? al : 0.f;
+        zed[u] = ra.z;
       }
 #pragma unroll
       for (int u = 0; u < U; ++u) {
@@ -291,9 +301,8 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
         }
         if (__any_sync(FULL, w > 0.f)) {
           const int jj = j[u];
-          const float4 ra = s_c[st][0][jj];
           const float4 a0 = s_c[st][2][jj], a1 = s_c[st][3][jj], a2 = s_c[st][4][jj];
-          acc[0] = fmaf(w, ra.z, acc[0]);
+          acc[0] = fmaf(w, zed[u], acc[0]);
           acc[1] = fmaf(w, a0.x, acc[1]);
           acc[2] = fmaf(w, a0.y, acc[2]);
           acc[3] = fmaf(w, a0.z, acc[3]);

@@ -77,10 +77,14 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
   constexpr uint32_t TILE = kSortThreads * ITEMS;
   const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t ntiles = (n + TILE - 1) / TILE;
-  while (true) {
+  // the first ticket was drawn at kernel entry (its latency overlaps the histogram scan)
+  for (bool first_ticket = true;; first_ticket = false) {
     __syncthreads();  // also protects keys/vals/wcnt of the previous ticket
-    if (tid == 0) sm.ticket = atomicAdd(ticket, 1u);
-    __syncthreads();
+    if (!first_ticket) {
+      if (ntiles <= gridDim.x) break;  // one ticket per CTA covers everything
+      if (tid == 0) sm.ticket = atomicAdd(ticket, 1u);
+      __syncthreads();
+    }
     const uint32_t t = sm.ticket;
     if (t >= ntiles) break;
 
@@ -187,16 +191,32 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
   }
 }
 
+// depth_pass >= 0: pass `depth_pass` of the 4-pass depth sort over the ping-pong buffers
+// (k0,v0) <-> (k1,v1); `hist` then points at all four histograms and trivial passes are skipped.
+// depth_pass < 0: a plain pass from (k0,v0) to (k1,v1) with its own histogram.
 __global__ void __launch_bounds__(kSortThreads)
-radix_pass_kernel(const uint32_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
-                  uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
-                  const uint32_t* __restrict__ count_ptr, uint32_t count_cap, int shift, int bits,
-                  const uint32_t* __restrict__ hist, uint32_t* __restrict__ status,
-                  uint32_t* __restrict__ ticket, uint32_t* __restrict__ err) {
+radix_pass_kernel(uint32_t* __restrict__ k0, uint32_t* __restrict__ v0, uint32_t* __restrict__ k1,
+                  uint32_t* __restrict__ v1, const uint32_t* __restrict__ count_ptr,
+                  uint32_t count_cap, int shift, int bits, const uint32_t* __restrict__ hist,
+                  uint32_t* __restrict__ status, uint32_t* __restrict__ ticket,
+                  uint32_t* __restrict__ err, int depth_pass) {
   __shared__ SortSmem sm;
   const unsigned tid = threadIdx.x;
+  if (tid == 0) sm.ticket = atomicAdd(ticket, 1u);
   const uint32_t n = count_ptr ? min(*count_ptr, count_cap) : count_cap;
   const uint32_t radix = 1u << bits, mask = radix - 1u;
+  const uint32_t *keys_in = k0, *vals_in = v0;
+  uint32_t *keys_out = k1, *vals_out = v1;
+  if (depth_pass >= 0) {
+    bool runs;
+    const int ran = depth_passes_run(hist, n, depth_pass + 1, &runs);
+    if (!runs) return;
+    const int before = ran - 1;  // passes that ran before this one
+    if (before & 1) { keys_in = k1; vals_in = v1; keys_out = k0; vals_out = v0; }
+    if (before == 0) vals_in = nullptr;      // nothing permuted yet: payload = index
+    if (depth_pass == 3) keys_out = nullptr; // the keys are not needed after the last pass
+    hist += depth_pass * 256;
+  }
 
   // start of every digit bin in the output = exclusive scan of the global histogram
   {
@@ -225,8 +245,20 @@ int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t*
   int64_t blocks = (int64_t)sort_status_rows(count_cap);
   if (blocks > max_blocks) blocks = max_blocks;
   radix_pass_kernel<<<(unsigned)blocks, kSortThreads, 0, s>>>(
-      keys_in, vals_in, keys_out, vals_out, count_ptr, count_cap, shift, bits, hist, status, ticket,
-      err);
+      const_cast<uint32_t*>(keys_in), const_cast<uint32_t*>(vals_in), keys_out, vals_out, count_ptr,
+      count_cap, shift, bits, hist, status, ticket, err, -1);
+  return 1;
+}
+
+int launch_depth_pass(uint32_t* const keys[2], uint32_t* const vals[2], uint32_t n, int pass,
+                      const uint32_t* hist4, uint32_t* status, uint32_t* ticket, uint32_t* err,
+                      int max_blocks, cudaStream_t s) {
+  if (n == 0) return 0;
+  int64_t blocks = (int64_t)sort_status_rows(n);
+  if (blocks > max_blocks) blocks = max_blocks;
+  radix_pass_kernel<<<(unsigned)blocks, kSortThreads, 0, s>>>(keys[0], vals[0], keys[1], vals[1], nullptr,
+                                                              n, 8 * pass, 8, hist4, status, ticket, err,
+                                                              pass);
   return 1;
 }
 

@@ -394,7 +394,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   }
 
   begin(SSSGS_STAGE_PACK);
-  if (add(launch_pack_attr(*g, c->attr, s)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
+  if (add(launch_pack_attr(*g, c->attr, sm)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
   if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, sm));
   end();
   int64_t batch_no = 0;
@@ -414,22 +414,17 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     begin(SSSGS_STAGE_DEPTH_SORT);
     // ---- a5 (1/2): all Gaussians by depth, 4 x 8 bits, stable ------------------------------------
     const uint32_t n32 = (uint32_t)g->n;
-    for (int p = 0; p < 4; ++p) {
-      const int src = p & 1, dst = src ^ 1;
-      add(launch_sort_pass(c->gb.dkeys[src], p == 0 ? nullptr : c->gb.dvals[src],
-                           p == 3 ? nullptr : c->gb.dkeys[dst], c->gb.dvals[dst], nullptr, n32, 8 * p, 8,
-                           c->gb.hist + p * 256, c->status_depth[p], cnt + DC_TICKET_BASE + p,
-                           cnt + DC_SORT_ERROR, max_blocks, s));
-    }
+    for (int p = 0; p < 4; ++p)
+      add(launch_depth_pass(c->gb.dkeys, c->gb.dvals, n32, p, c->gb.hist, c->status_depth[p],
+                            cnt + DC_TICKET_BASE + p, cnt + DC_SORT_ERROR, max_blocks, s));
     end();
-    const uint32_t* sorted_idx = c->gb.dvals[0];
     // ---- a4: scan + expansion into (tile, Gaussian) instances, in depth order ---------------------
     int tb = 1;
     while ((1 << tb) < tiles) ++tb;
     const int npass = tb > 8 ? 2 : 1;
     const int bits0 = npass == 2 ? (tb + 1) / 2 : tb, bits1 = npass == 2 ? tb - bits0 : 0;
     begin(SSSGS_STAGE_EMIT);
-    add(launch_emit(g->n, cam, c->gb, sorted_idx, cap, 0, bits0, bits0, bits1, c->status_emit,
+    add(launch_emit(g->n, cam, c->gb, cap, 0, bits0, bits0, bits1, c->status_emit,
                     cnt + DC_TICKET_BASE + 4, s));
     end();
     begin(SSSGS_STAGE_TILE_SORT);
@@ -448,12 +443,12 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     // ---- a6: tile ranges ---------------------------------------------------------------------------
     begin(SSSGS_STAGE_RANGES);
     add(launch_ranges(sorted_tiles, cam, c->gb, cap,
-                      out->tile_ranges ? (uint2*)(out->tile_ranges + (size_t)v * tiles * 2) : nullptr, s));
-    if (out->sorted_keys || out->sorted_vals || out->counters)
+                      out->tile_ranges ? (uint2*)(out->tile_ranges + (size_t)v * tiles * 2) : nullptr,
+                      out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr, s));
+    if (out->sorted_keys || out->sorted_vals)
       add(launch_export_lists(sorted_tiles, sorted_vals, c->gb, cap,
                               out->sorted_keys ? out->sorted_keys + (size_t)v * cap : nullptr,
-                              out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr,
-                              out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr, s));
+                              out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr, s));
     end();
     // ---- per light batch: a1+a2 MLP, a7+a8 raster + shade -------------------------------------------
     for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
