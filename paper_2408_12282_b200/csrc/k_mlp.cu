@@ -27,9 +27,7 @@ namespace sssgs {
 
 namespace {
 
-constexpr int kMlpThreads = 288;       // 2 x 4 epilogue warps + 1 MMA warp
 constexpr int kRows = 128;             // rows per tile = UMMA M
-constexpr int kSlotCols = 256;         // TMEM columns per slot
 constexpr int kKBlockBytes = kRows * 128;  // one 64-wide K block of an A tile (128 rows x 128 B)
 constexpr float kY00 = 0.2820948f, kY1 = 0.4886025f;
 
@@ -192,209 +190,336 @@ struct MlpArgs {
   float4* out_internal;        // [n][n_lights]
   float* out_user;             // optional: light l at out_user + l*user_light_stride, [n][4]
   int64_t user_light_stride;   // in floats
+  int slots;                   // row tiles in flight per CTA (2..4)
+  int wps;                     // epilogue warps per slot: 4 (one per 32 rows) or 8 (two column halves)
+  int slot_cols;               // TMEM columns per slot
   MlpPlan plan;
 };
+
+constexpr int kKeepChunks = 5;   // 16-byte input chunks a thread keeps in registers across lights
+                                 // (chunk 0 and gamma(mu); the per-Gaussian feature is re-read per light, from L2)
 
 __device__ __forceinline__ float act_fn(float v, int activation, float slope) {
   return v > 0.f ? v : (activation == SSSGS_ACT_LEAKY_RELU ? slope * v : 0.f);
 }
 
-// Step a1: assemble the input row of Gaussian g for one light and store it as bf16 into row r
-// of the A tile.  Row layout (S1/S13/S14):
-//   [ n(3) | rot(2) | scale(3) | w_in(3) | w_out(3) | d | v | gamma(mu)(24) | feat(F) | 0-pad ]
-__device__ __forceinline__ void assemble_row(const MlpArgs& a, int64_t g, const LightParams& lt,
-                                             uint8_t* A, int r) {
-  const float mx = a.means[3 * g], my = a.means[3 * g + 1], mz = a.means[3 * g + 2];
-  const float4 q = reinterpret_cast<const float4*>(a.rotations)[g];
-  const float sgn = q.x < 0.f ? -1.f : 1.f;
-  {
-    const uint4 c0 = make_uint4(pack_bf16(a.normals[3 * g], a.normals[3 * g + 1]),
-                                pack_bf16(a.normals[3 * g + 2], sgn * q.x),
-                                pack_bf16(sgn * q.y, a.scales[3 * g]),
-                                pack_bf16(a.scales[3 * g + 1], a.scales[3 * g + 2]));
-    *reinterpret_cast<uint4*>(A + swz_off(r, 0, kKBlockBytes)) = c0;
-  }
-  {
-    float wix = lt.pos[0] - mx, wiy = lt.pos[1] - my, wiz = lt.pos[2] - mz;
-    const float d = sqrtf(wix * wix + wiy * wiy + wiz * wiz);
-    const float id = 1.f / d;
-    wix *= id; wiy *= id; wiz *= id;
-    float wox = a.cam_pos[0] - mx, woy = a.cam_pos[1] - my, woz = a.cam_pos[2] - mz;
+
+__device__ __forceinline__ uint4 pack8(const float* v) {
+  return make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
+                    pack_bf16(v[6], v[7]));
+}
+
+// Step a1, light-independent part.  Input row layout (S1/S13/S14), in
+// 16-byte chunks of 8 bf16:
+//   chunk 0: n(3) rot(2) scale(3) | chunk 1: w_in(3) w_out(3) d v | chunks 2-4: gamma(mu)(24) |
+//   chunks 5..: feat(F), zero padded to in_pad
+// Fills keep[0], keep[2..4] (when this thread owns them: c_begin == 0), mu and w_out.
+__device__ __forceinline__ void assemble_static(const MlpArgs& a, int64_t g, int c_begin, int c_end,
+                                                uint4* keep, float mu[3], float wout[3]) {
+  mu[0] = a.means[3 * g]; mu[1] = a.means[3 * g + 1]; mu[2] = a.means[3 * g + 2];
+  if (c_begin == 0) {
+    const float4 q = reinterpret_cast<const float4*>(a.rotations)[g];
+    const float sgn = q.x < 0.f ? -1.f : 1.f;
+    keep[0] = make_uint4(pack_bf16(a.normals[3 * g], a.normals[3 * g + 1]),
+                         pack_bf16(a.normals[3 * g + 2], sgn * q.x),
+                         pack_bf16(sgn * q.y, a.scales[3 * g]),
+                         pack_bf16(a.scales[3 * g + 1], a.scales[3 * g + 2]));
+    float wox = a.cam_pos[0] - mu[0], woy = a.cam_pos[1] - mu[1], woz = a.cam_pos[2] - mu[2];
     const float io = 1.f / sqrtf(wox * wox + woy * woy + woz * woz);
-    wox *= io; woy *= io; woz *= io;
-    float v;
-    if (a.sh_coefs == 4) {
-      const float4 sh = reinterpret_cast<const float4*>(a.vis_sh)[g];
-      v = kY00 * sh.x + kY1 * (sh.y * wiy + sh.z * wiz + sh.w * wix);
-    } else {
-      v = kY00 * a.vis_sh[g];
-    }
-    v = fminf(1.f, fmaxf(0.f, v));
-    const uint4 c1 = make_uint4(pack_bf16(wix, wiy), pack_bf16(wiz, wox), pack_bf16(woy, woz),
-                                pack_bf16(d, v));
-    *reinterpret_cast<uint4*>(A + swz_off(r, 1, kKBlockBytes)) = c1;
-  }
-  {
-    // gamma(mu): for k = 0..3: [sin(2^k pi mu_xyz), cos(2^k pi mu_xyz)]; sin(pi x) via sincospif
+    wout[0] = wox * io; wout[1] = woy * io; wout[2] = woz * io;
+    // gamma(mu): for k = 0..3: [sin(2^k pi mu_xyz), cos(2^k pi mu_xyz)]; octave 0 by sincospif,
+    // the next octaves by the double-angle recurrences (error << the bf16 rounding that follows)
     float ga[24];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const float f = (float)(1 << k);
-      sincospif(f * mx, &ga[6 * k + 0], &ga[6 * k + 3]);
-      sincospif(f * my, &ga[6 * k + 1], &ga[6 * k + 4]);
-      sincospif(f * mz, &ga[6 * k + 2], &ga[6 * k + 5]);
-    }
+    for (int ax = 0; ax < 3; ++ax) {
+      float s, c;
+      sincospif(mu[ax], &s, &c);
+      ga[ax] = s; ga[3 + ax] = c;
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      const uint4 cc = make_uint4(pack_bf16(ga[8 * c], ga[8 * c + 1]), pack_bf16(ga[8 * c + 2], ga[8 * c + 3]),
-                                  pack_bf16(ga[8 * c + 4], ga[8 * c + 5]), pack_bf16(ga[8 * c + 6], ga[8 * c + 7]));
-      *reinterpret_cast<uint4*>(A + swz_off(r, 2 + c, kKBlockBytes)) = cc;
+      for (int k = 1; k < 4; ++k) {
+        const float s2 = 2.f * s * c, c2 = 1.f - 2.f * s * s;
+        s = s2; c = c2;
+        ga[6 * k + ax] = s; ga[6 * k + 3 + ax] = c;
+      }
     }
+    keep[2] = pack8(ga);
+    keep[3] = pack8(ga + 8);
+    keep[4] = pack8(ga + 16);
   }
+}
+
+// Light-dependent chunk 1: (w_in, w_out, d, v) for light `lt`.
+__device__ __forceinline__ uint4 assemble_light(const MlpArgs& a, int64_t g, const LightParams& lt,
+                                                const float mu[3], const float wout[3]) {
+  float wix = lt.pos[0] - mu[0], wiy = lt.pos[1] - mu[1], wiz = lt.pos[2] - mu[2];
+  const float d = sqrtf(wix * wix + wiy * wiy + wiz * wiz);
+  const float id = 1.f / d;
+  wix *= id; wiy *= id; wiz *= id;
+  float v;
+  if (a.sh_coefs == 4) {
+    const float4 sh = reinterpret_cast<const float4*>(a.vis_sh)[g];
+    v = kY00 * sh.x + kY1 * (sh.y * wiy + sh.z * wiz + sh.w * wix);
+  } else {
+    v = kY00 * a.vis_sh[g];
+  }
+  v = fminf(1.f, fmaxf(0.f, v));
+  return make_uint4(pack_bf16(wix, wiy), pack_bf16(wiz, wout[0]), pack_bf16(wout[1], wout[2]),
+                    pack_bf16(d, v));
+}
+
+// Writes the chunks [c_begin, c_end) of row r of the layer-0 A tile.
+__device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, uint8_t* A, int r, int c_begin,
+                                          int c_end, const uint4* keep, const uint4& light_chunk) {
+#pragma unroll
+  for (int c = 0; c < kKeepChunks; ++c)
+    if (c >= c_begin && c < c_end)
+      *reinterpret_cast<uint4*>(A + swz_off(r, c, kKBlockBytes)) = (c == 1) ? light_chunk : keep[c];
+  // the per-Gaussian feature (chunks 5..) is read here: it stays L2-resident across the lights
   const int F = a.plan.feat_dim;
-  const int nchunks = a.plan.in_pad >> 3;
-  for (int c = 5; c < nchunks; ++c) {
+  for (int c = max(c_begin, kKeepChunks); c < c_end; ++c) {
     const int j = (c - 5) * 8;
     float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0;
     if (j < F) f0 = *reinterpret_cast<const float4*>(a.feat + g * F + j);
     if (j + 4 < F) f1 = *reinterpret_cast<const float4*>(a.feat + g * F + j + 4);
-    const uint4 cc = make_uint4(pack_bf16(f0.x, f0.y), pack_bf16(f0.z, f0.w), pack_bf16(f1.x, f1.y),
-                                pack_bf16(f1.z, f1.w));
-    *reinterpret_cast<uint4*>(A + swz_off(r, c, kKBlockBytes)) = cc;
+    *reinterpret_cast<uint4*>(A + swz_off(r, c, kKBlockBytes)) =
+        make_uint4(pack_bf16(f0.x, f0.y), pack_bf16(f0.z, f0.w), pack_bf16(f1.x, f1.y), pack_bf16(f1.z, f1.w));
   }
 }
 
-__global__ void __launch_bounds__(kMlpThreads, 1) mlp_kernel(const __grid_constant__ MlpArgs a) {
+// ---- epilogue helpers --------------------------------------------------------------------------
+// 16 accumulator columns of this thread's row, TMEM -> registers, asynchronously: the registers
+// are valid only after tmem_wait16 on the same array (which carries the data dependence).
+__device__ __forceinline__ void tmem_ld16_async(uint32_t taddr, uint32_t* r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
+        "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]),
+        "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_wait16(uint32_t* r) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  // empty volatile asms keep their order after the wait and make every later use of r[i] depend on it
+#pragma unroll
+  for (int i = 0; i < 16; ++i) asm volatile("" : "+r"(r[i]));
+}
+// bf16x2 {lo, hi} = round-to-nearest-even of (max(lo, 0), max(hi, 0)): the ReLU rides on the convert
+__device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
+  uint32_t d;
+  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
+__device__ __forceinline__ void sts128(uint32_t saddr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "r"(x), "r"(y), "r"(z), "r"(w)
+               : "memory");
+}
+
+// bias + activation + bf16 of 16 accumulator columns -> two 16-byte chunks of the next A operand
+// at shared addresses sa0, sa1; bias = 16 floats (16-byte aligned, shared memory).
+template <bool RELU>
+__device__ __forceinline__ void finish16(const uint32_t* r, const float* bias, uint32_t sa0, uint32_t sa1,
+                                         int activation, float slope) {
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    const float4 b0 = *reinterpret_cast<const float4*>(bias + 8 * q);
+    const float4 b1 = *reinterpret_cast<const float4*>(bias + 8 * q + 4);
+    float v[8];
+    v[0] = __uint_as_float(r[8 * q + 0]) + b0.x; v[1] = __uint_as_float(r[8 * q + 1]) + b0.y;
+    v[2] = __uint_as_float(r[8 * q + 2]) + b0.z; v[3] = __uint_as_float(r[8 * q + 3]) + b0.w;
+    v[4] = __uint_as_float(r[8 * q + 4]) + b1.x; v[5] = __uint_as_float(r[8 * q + 5]) + b1.y;
+    v[6] = __uint_as_float(r[8 * q + 6]) + b1.z; v[7] = __uint_as_float(r[8 * q + 7]) + b1.w;
+    const uint32_t sa = q ? sa1 : sa0;
+    if (RELU) {
+      sts128(sa, pack_bf16_relu(v[0], v[1]), pack_bf16_relu(v[2], v[3]), pack_bf16_relu(v[4], v[5]),
+             pack_bf16_relu(v[6], v[7]));
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) v[i] = act_fn(v[i], activation, slope);
+      sts128(sa, pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
+    }
+  }
+}
+
+// Hidden-stage epilogue of one thread: its share of the activated columns [0, n_act), in groups
+// of 16, with the TMEM load of the next group in flight while the current one is finished.
+// WPS = 4: all columns; WPS = 8: the two warps of a row quarter take alternate 32-column blocks.
+// Chunk k (16 bytes = 8 columns) of K block kb of this row sits at rowbase + kb * kKBlockBytes +
+// ((k ^ (row & 7)) << 4); rowbase is 128-byte aligned, so the swizzle is an XOR on the address.
+template <int WPS_, bool RELU>
+__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, const float* bias, int n_act, int half,
+                                                uint32_t rowbase, uint32_t swz, int activation,
+                                                float slope) {
+  constexpr int G = WPS_ == 4 ? 8 : 4;  // groups of 16 columns per thread for 128 columns
+  uint32_t ra[16], rb[16];
+  // group gi covers columns col(gi) .. +15
+  auto col = [&](int gi) { return WPS_ == 4 ? 16 * gi : 32 * half + 64 * (gi >> 1) + 16 * (gi & 1); };
+  auto finish = [&](const uint32_t* regs, int c0) {
+    const uint32_t k0 = (uint32_t)(c0 >> 3);  // first 16-byte chunk of the group
+    const uint32_t base = rowbase + (k0 >> 3) * (uint32_t)kKBlockBytes;
+    finish16<RELU>(regs, bias + c0, base + (((k0 & 7u) << 4) ^ swz), base + ((((k0 & 7u) + 1u) << 4) ^ swz),
+                   activation, slope);
+  };
+  if (col(0) + 16 <= n_act) tmem_ld16_async(taddr + col(0), ra);
+#pragma unroll
+  for (int gp = 0; gp < G / 2; ++gp) {
+    const int c0 = col(2 * gp), c1 = col(2 * gp + 1);
+    if (c0 + 16 > n_act) break;
+    tmem_wait16(ra);
+    if (c1 + 16 <= n_act) tmem_ld16_async(taddr + c1, rb);
+    finish(ra, c0);
+    if (c1 + 16 > n_act) break;
+    tmem_wait16(rb);
+    if (2 * gp + 2 < G) {
+      const int c2 = col(2 * gp + 2);
+      if (c2 + 16 <= n_act) tmem_ld16_async(taddr + c2, ra);
+    }
+    finish(rb, c1);
+  }
+}
+
+constexpr int kMaxSlots = 4;
+constexpr int kMlpThreadsMax = 512;  // up to 16 warps: 4 slots x 4 warps or 2 slots x 8 warps
+
+// Work distribution: a "unit" is a block of 128 Gaussians with all the lights of the batch; slot s of
+// CTA b owns the units (i * slots + s) * gridDim.x + b, i = 0, 1, ...  Within a unit the lights are
+// walked in order so that the light-independent inputs of a row are assembled once.
+template <int WPS, bool RELU>
+__global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_constant__ MlpArgs a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const MlpPlan& plan = a.plan;
   const int a_bytes = plan.max_k_bytes;
+  const int S = a.slots;
   uint8_t* sW = smem;
-  uint8_t* sA[2] = {smem + plan.blob_bytes, smem + plan.blob_bytes + a_bytes};
-  float* sBias = reinterpret_cast<float*>(smem + plan.blob_bytes + 2 * a_bytes);
+  uint8_t* sA0 = smem + plan.blob_bytes;
+  float* sBias = reinterpret_cast<float*>(sA0 + S * a_bytes);
   uint64_t* bars = reinterpret_cast<uint64_t*>(sBias + ((plan.bias_floats + 3) & ~3));
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 4);
-  const uint32_t bar_a[2] = {smem_u32(bars + 0), smem_u32(bars + 1)};
-  const uint32_t bar_d[2] = {smem_u32(bars + 2), smem_u32(bars + 3)};
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kMaxSlots);
+  // bars[s] = a_ready of slot s, bars[kMaxSlots + s] = d_ready of slot s
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int64_t n_gblocks = (a.n + kRows - 1) / kRows;
-  const int64_t total_tiles = n_gblocks * a.n_lights;  // tile = gblock * n_lights + light
+  const int64_t n_units = (a.n + kRows - 1) / kRows;
 
   // ---- prologue: weights + biases to smem, barriers, TMEM -------------------------------------
-  for (int i = tid * 16; i < plan.blob_bytes; i += kMlpThreads * 16)
+  for (int i = tid * 16; i < plan.blob_bytes; i += blockDim.x * 16)
     *reinterpret_cast<uint4*>(sW + i) = *reinterpret_cast<const uint4*>(a.blob + i);
-  for (int i = tid; i < plan.bias_floats; i += kMlpThreads) sBias[i] = a.bias[i];
+  for (int i = tid; i < plan.bias_floats; i += blockDim.x) sBias[i] = a.bias[i];
   if (tid == 0) {
-    mbar_init(bar_a[0], kRows);
-    mbar_init(bar_a[1], kRows);
-    mbar_init(bar_d[0], 1);
-    mbar_init(bar_d[1], 1);
+    for (int s = 0; s < S; ++s) {
+      mbar_init(smem_u32(bars + s), WPS * 32);
+      mbar_init(smem_u32(bars + kMaxSlots + s), 1);
+    }
     fence_barrier_init();
   }
-  if (warp == 8) tmem_alloc(smem_u32(tmem_slot), 2 * kSlotCols);
+  if (warp == 0) tmem_alloc(smem_u32(tmem_slot), 512);
   fence_proxy_async();  // weights were written with generic stores; UMMA reads via the async proxy
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  if (warp == 8) {
-    // ===================== MMA issuer =====================
-    uint32_t pa[2] = {0, 0};
-    for (int64_t jp = 0;; jp += 2) {
-      const bool have0 = blockIdx.x + jp * gridDim.x < total_tiles;
-      const bool have1 = blockIdx.x + (jp + 1) * gridDim.x < total_tiles;
-      if (!have0) break;
-      for (int s = 0; s < plan.n_stages; ++s) {
-        const MlpStage& st = plan.st[s];
+  {
+    // ===================== input assembly + epilogue warps =====================
+    // a warp may only touch the TMEM lanes 32 * (warp % 4) .. +31: WPS is 4 or 8, so warp % 4 is
+    // also the row quarter inside the slot
+    const int slot = warp / WPS, wq = warp % WPS;
+    const int quarter = wq & 3, half = wq >> 2;   // column half (WPS = 8)
+    const int r = quarter * 32 + lane;            // row of the tile = TMEM lane
+    const uint32_t taddr = tmem_base + slot * a.slot_cols + ((uint32_t)(quarter * 32) << 16);
+    uint8_t* A = sA0 + slot * a_bytes;
+    const uint32_t bar_a = smem_u32(bars + slot), bar_d = smem_u32(bars + kMaxSlots + slot);
+    // The first warp of a slot also issues the slot's MMAs: once all rows of the A operand have
+    // arrived (a_ready), one elected lane issues the K steps of the stage and commits them to
+    // d_ready.  A slot's pipeline is serial anyway (A operand -> MMA -> epilogue -> next A operand);
+    // the tensor core is kept busy by the other slots.
+    uint32_t pa = 0;
+    auto issue_stage = [&](int s_idx) {
+      if (wq != 0) return;
+      mbar_wait(bar_a, pa);
+      pa ^= 1u;
+      tc_fence_after();
+      if (lane == 0) {
+        const MlpStage& st = plan.st[s_idx];
         const uint32_t idesc = make_idesc(st.n_pad);
         const uint32_t w_addr = smem_u32(sW + st.w_off);
+        const uint32_t a_addr = smem_u32(A);
+        const uint32_t d_addr = tmem_base + slot * a.slot_cols;
         const int ksteps = st.k_pad >> 4;
-        for (int slot = 0; slot < 2; ++slot) {
-          if (slot == 1 && !have1) continue;
-          mbar_wait(bar_a[slot], pa[slot]);
-          pa[slot] ^= 1u;
-          tc_fence_after();
-          if (lane == 0) {
-            const uint32_t a_addr = smem_u32(sA[slot]);
-            const uint32_t d_addr = tmem_base + slot * kSlotCols;
-            for (int ks = 0; ks < ksteps; ++ks) {
-              const int kb = ks >> 2, kin = ks & 3;
-              const uint64_t da = make_desc(a_addr + kb * kKBlockBytes + kin * 32);
-              const uint64_t db = make_desc(w_addr + kb * (st.n_pad * 128) + kin * 32);
-              umma_bf16(d_addr, da, db, idesc, ks > 0 ? 1u : 0u);
-            }
-            umma_commit(bar_d[slot]);  // arrives when the MMAs above have completed
-          }
-          __syncwarp();
+        for (int ks = 0; ks < ksteps; ++ks) {
+          const int kb = ks >> 2, kin = ks & 3;
+          const uint64_t da = make_desc(a_addr + kb * kKBlockBytes + kin * 32);
+          const uint64_t db = make_desc(w_addr + kb * (st.n_pad * 128) + kin * 32);
+          umma_bf16(d_addr, da, db, idesc, ks > 0 ? 1u : 0u);
         }
+        umma_commit(bar_d);  // arrives when the MMAs above have completed
       }
-    }
-  } else {
-    // ===================== input assembly + epilogue warps =====================
-    const int slot = warp >> 2;                 // warps 0-3 -> slot 0, 4-7 -> slot 1
-    const int r = (warp & 3) * 32 + lane;       // row of the tile = TMEM lane
-    const uint32_t taddr = tmem_base + slot * kSlotCols + ((uint32_t)((warp & 3) * 32) << 16);
-    uint8_t* A = sA[slot];
+      __syncwarp();
+    };
+    // 16-byte input chunks this thread writes
+    const int nchunks = plan.in_pad >> 3;
+    const int c_split = nchunks > 5 ? 5 : nchunks;
+    const int c_begin = (WPS == 8 && half == 1) ? c_split : 0;
+    const int c_end = (WPS == 8 && half == 0) ? c_split : nchunks;
+    const uint32_t rowbase = smem_u32(A) + (uint32_t)(r * 128), swz = (uint32_t)((r & 7) << 4);
     uint32_t pd = 0;
-    for (int64_t j = slot;; j += 2) {
-      const int64_t tile = blockIdx.x + j * gridDim.x;
-      if (tile >= total_tiles) break;
-      const int64_t gblock = tile / a.n_lights;
-      const int light = (int)(tile % a.n_lights);
-      const int64_t g_raw = gblock * kRows + r;
+    for (int64_t u = (int64_t)slot * gridDim.x + blockIdx.x; u < n_units; u += (int64_t)S * gridDim.x) {
+      const int64_t g_raw = u * kRows + r;
       const bool row_ok = g_raw < a.n;
       const int64_t g = row_ok ? g_raw : a.n - 1;
+      uint4 keep[kKeepChunks];
+      float mu[3], wout[3];
+      assemble_static(a, g, c_begin, c_end, keep, mu, wout);
+      for (int light = 0; light < a.n_lights; ++light) {
+        uint4 lc = make_uint4(0u, 0u, 0u, 0u);
+        if (c_begin == 0) lc = assemble_light(a, g, a.lights.l[light], mu, wout);
+        write_row(a, g, A, r, c_begin, c_end, keep, lc);
+        fence_proxy_async();
+        mbar_arrive(bar_a);
+        issue_stage(0);
 
-      assemble_row(a, g, a.lights.l[light], A, r);
-      fence_proxy_async();
-      mbar_arrive(bar_a[slot]);
-
-      float sss_keep[3] = {0.f, 0.f, 0.f};
-      for (int s = 0; s < plan.n_stages; ++s) {
-        const MlpStage& st = plan.st[s];
-        const float* bias = sBias + st.b_off;
-        mbar_wait(bar_d[slot], pd);
-        pd ^= 1u;
-        tc_fence_after();
-        float v[16];
-        if (st.type == ST_HIDDEN || st.type == ST_HEAD_SPLIT_A) {
-          // activated columns [0, n_act) -> bf16 -> next stage's A operand
-          for (int c0 = 0; c0 < st.n_act; c0 += 16) {
-            tmem_ld16(taddr + c0, v);
+        float sss_keep[3] = {0.f, 0.f, 0.f};
+        for (int s = 0; s < plan.n_stages; ++s) {
+          const MlpStage& st = plan.st[s];
+          const float* bias = sBias + st.b_off;
+          mbar_wait(bar_d, pd);
+          pd ^= 1u;
+          tc_fence_after();
+          if (st.type == ST_HIDDEN || st.type == ST_HEAD_SPLIT_A) {
+            // activated columns [0, n_act) -> bf16 -> next stage's A operand
+            hidden_epilogue<WPS, RELU>(taddr, bias, st.n_act, half, rowbase, swz, plan.activation, plan.leaky_slope);
+            if (st.type == ST_HEAD_SPLIT_A && half == 0) {  // SSS logits sit right after the activated columns
+              float v[16];
+              tmem_ld16(taddr + st.n_act, v);
 #pragma unroll
-            for (int i = 0; i < 16; ++i) v[i] = act_fn(v[i] + bias[c0 + i], plan.activation, plan.leaky_slope);
-            const uint4 lo = make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
-            const uint4 hi = make_uint4(pack_bf16(v[8], v[9]), pack_bf16(v[10], v[11]), pack_bf16(v[12], v[13]), pack_bf16(v[14], v[15]));
-            *reinterpret_cast<uint4*>(A + swz_off(r, (c0 >> 3), kKBlockBytes)) = lo;
-            *reinterpret_cast<uint4*>(A + swz_off(r, (c0 >> 3) + 1, kKBlockBytes)) = hi;
+              for (int c = 0; c < 3; ++c) sss_keep[c] = 1.f / (1.f + __expf(-(v[c] + bias[st.n_act + c])));
+            }
+            tc_fence_before();
+            fence_proxy_async();
+            mbar_arrive(bar_a);
+            issue_stage(s + 1);
+          } else {
+            if (half == 0) {
+              float v[16];
+              tmem_ld16(taddr, v);
+              float4 o;
+              if (st.type == ST_HEAD_JOINT) {
+                o.x = 1.f / (1.f + __expf(-(v[0] + bias[0])));
+                o.y = 1.f / (1.f + __expf(-(v[1] + bias[1])));
+                o.z = 1.f / (1.f + __expf(-(v[2] + bias[2])));
+                o.w = fmaxf(0.f, v[3] + bias[3]);
+              } else {  // ST_HEAD_SPLIT_B
+                o = make_float4(sss_keep[0], sss_keep[1], sss_keep[2], fmaxf(0.f, v[0] + bias[0]));
+              }
+              if (row_ok) {
+                a.out_internal[(size_t)g * a.n_lights + light] = o;
+                if (a.out_user)
+                  *reinterpret_cast<float4*>(a.out_user + (int64_t)light * a.user_light_stride + g * 4) = o;
+              }
+            }
+            tc_fence_before();  // TMEM reads are ordered before the next tile's a_ready arrive
           }
-          if (st.type == ST_HEAD_SPLIT_A) {  // SSS logits sit right after the activated columns
-            tmem_ld16(taddr + st.n_act, v);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) sss_keep[c] = 1.f / (1.f + __expf(-(v[c] + bias[st.n_act + c])));
-          }
-          tc_fence_before();
-          fence_proxy_async();
-          mbar_arrive(bar_a[slot]);
-        } else {
-          tmem_ld16(taddr, v);
-          float4 o;
-          if (st.type == ST_HEAD_JOINT) {
-            o.x = 1.f / (1.f + __expf(-(v[0] + bias[0])));
-            o.y = 1.f / (1.f + __expf(-(v[1] + bias[1])));
-            o.z = 1.f / (1.f + __expf(-(v[2] + bias[2])));
-            o.w = fmaxf(0.f, v[3] + bias[3]);
-          } else {  // ST_HEAD_SPLIT_B
-            o = make_float4(sss_keep[0], sss_keep[1], sss_keep[2], fmaxf(0.f, v[0] + bias[0]));
-          }
-          if (row_ok) {
-            a.out_internal[(size_t)g * a.n_lights + light] = o;
-            if (a.out_user)
-              *reinterpret_cast<float4*>(a.out_user + (int64_t)light * a.user_light_stride + g * 4) = o;
-          }
-          tc_fence_before();  // TMEM reads are ordered before the next tile's a_ready arrive
         }
       }
     }
@@ -403,13 +528,28 @@ __global__ void __launch_bounds__(kMlpThreads, 1) mlp_kernel(const __grid_consta
   // ---- teardown ----------------------------------------------------------------------------------
   tc_fence_before();
   __syncthreads();
-  if (warp == 8) tmem_dealloc(tmem_base, 2 * kSlotCols);
+  if (warp == 0) tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace
 
+// Slots (row tiles in flight per CTA), epilogue warps per slot and TMEM columns per slot for a plan.
+static void mlp_shape(const MlpPlan& plan, int* slots, int* wps, int* slot_cols) {
+  const int cols = plan.max_n <= 128 ? 128 : 256;
+  const int fixed = plan.blob_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 2 * kMaxSlots * 8 + 16 + 1024;
+  int s = (227 * 1024 - fixed) / plan.max_k_bytes;
+  if (s > 512 / cols) s = 512 / cols;
+  if (s > kMaxSlots) s = kMaxSlots;
+  if (s < 1) s = 1;
+  *slots = s;
+  *wps = s <= 2 ? 8 : 4;
+  *slot_cols = cols;
+}
+
 int mlp_smem_bytes(const MlpPlan& plan) {
-  return plan.blob_bytes + 2 * plan.max_k_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 4 * 8 + 16 + 1024;
+  int s, w, c;
+  mlp_shape(plan, &s, &w, &c);
+  return plan.blob_bytes + s * plan.max_k_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 2 * kMaxSlots * 8 + 16 + 1024;
 }
 
 int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
@@ -434,17 +574,23 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
   a.blob = blob; a.bias = bias;
   a.out_internal = out_internal; a.out_user = out_user; a.user_light_stride = user_light_stride;
   a.plan = plan;
+  mlp_shape(plan, &a.slots, &a.wps, &a.slot_cols);
   const int smem = mlp_smem_bytes(plan);
-  static int configured_smem = 0;
-  if (smem > configured_smem) {
-    if (cudaFuncSetAttribute(mlp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-      return -1;
-    configured_smem = smem;
-  }
-  const int64_t tiles = ((g.n + kRows - 1) / kRows) * n_lights;
-  const int grid = (int)(tiles < num_sms ? tiles : num_sms);
-  mlp_kernel<<<grid, kMlpThreads, smem, s>>>(a);
-  return 1;
+  const int64_t units = (g.n + kRows - 1) / kRows;
+  const int grid = (int)(units < num_sms ? units : num_sms);
+  const bool relu = plan.activation == SSSGS_ACT_RELU;
+  auto launch = [&](auto kernel, int* configured_smem) -> int {
+    if (smem > *configured_smem) {
+      if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+        return -1;
+      *configured_smem = smem;
+    }
+    kernel<<<grid, a.slots * a.wps * 32, smem, s>>>(a);
+    return 1;
+  };
+  static int cfg_smem[4] = {0, 0, 0, 0};
+  if (a.wps == 4) return relu ? launch(mlp_kernel<4, true>, &cfg_smem[0]) : launch(mlp_kernel<4, false>, &cfg_smem[1]);
+  return relu ? launch(mlp_kernel<8, true>, &cfg_smem[2]) : launch(mlp_kernel<8, false>, &cfg_smem[3]);
 }
 
 }  // namespace sssgs
