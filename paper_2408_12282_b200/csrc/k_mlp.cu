@@ -316,20 +316,40 @@ __device__ __forceinline__ void sts128(uint32_t saddr, uint32_t x, uint32_t y, u
                : "memory");
 }
 
+// (x0, x1) += (y0, y1) as one packed fp32x2 add (sm_100 FADD2)
+__device__ __forceinline__ void add2(float& x0, float& x1, float y0, float y1) {
+  asm("{\n\t.reg .b64 a, b;\n\t"
+      "mov.b64 a, {%0, %1};\n\t"
+      "mov.b64 b, {%2, %3};\n\t"
+      "add.rn.f32x2 a, a, b;\n\t"
+      "mov.b64 {%0, %1}, a;\n\t}"
+      : "+f"(x0), "+f"(x1)
+      : "f"(y0), "f"(y1));
+}
+// 16 bias values from shared memory.  Not volatile: the biases never change during the kernel, so
+// the compiler may schedule these loads ahead of the TMEM wait they are independent of.
+__device__ __forceinline__ void lds_bias16(uint32_t saddr, float4* b) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+        : "=f"(b[q].x), "=f"(b[q].y), "=f"(b[q].z), "=f"(b[q].w)
+        : "r"(saddr + 16u * q));
+}
+
 // bias + activation + bf16 of 16 accumulator columns -> two 16-byte chunks of the next A operand
-// at shared addresses sa0, sa1; bias = 16 floats (16-byte aligned, shared memory).
+// at shared addresses sa0, sa1; b = the 16 biases.
 template <bool RELU>
-__device__ __forceinline__ void finish16(const uint32_t* r, const float* bias, uint32_t sa0, uint32_t sa1,
+__device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, uint32_t sa0, uint32_t sa1,
                                          int activation, float slope) {
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
-    const float4 b0 = *reinterpret_cast<const float4*>(bias + 8 * q);
-    const float4 b1 = *reinterpret_cast<const float4*>(bias + 8 * q + 4);
     float v[8];
-    v[0] = __uint_as_float(r[8 * q + 0]) + b0.x; v[1] = __uint_as_float(r[8 * q + 1]) + b0.y;
-    v[2] = __uint_as_float(r[8 * q + 2]) + b0.z; v[3] = __uint_as_float(r[8 * q + 3]) + b0.w;
-    v[4] = __uint_as_float(r[8 * q + 4]) + b1.x; v[5] = __uint_as_float(r[8 * q + 5]) + b1.y;
-    v[6] = __uint_as_float(r[8 * q + 6]) + b1.z; v[7] = __uint_as_float(r[8 * q + 7]) + b1.w;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[8 * q + i]);
+    add2(v[0], v[1], b[2 * q].x, b[2 * q].y);
+    add2(v[2], v[3], b[2 * q].z, b[2 * q].w);
+    add2(v[4], v[5], b[2 * q + 1].x, b[2 * q + 1].y);
+    add2(v[6], v[7], b[2 * q + 1].z, b[2 * q + 1].w);
     const uint32_t sa = q ? sa1 : sa0;
     if (RELU) {
       sts128(sa, pack_bf16_relu(v[0], v[1]), pack_bf16_relu(v[2], v[3]), pack_bf16_relu(v[4], v[5]),
@@ -348,34 +368,37 @@ __device__ __forceinline__ void finish16(const uint32_t* r, const float* bias, u
 // Chunk k (16 bytes = 8 columns) of K block kb of this row sits at rowbase + kb * kKBlockBytes +
 // ((k ^ (row & 7)) << 4); rowbase is 128-byte aligned, so the swizzle is an XOR on the address.
 template <int WPS_, bool RELU>
-__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, const float* bias, int n_act, int half,
+__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, uint32_t bias_saddr, int n_act, int half,
                                                 uint32_t rowbase, uint32_t swz, int activation,
                                                 float slope) {
   constexpr int G = WPS_ == 4 ? 8 : 4;  // groups of 16 columns per thread for 128 columns
   uint32_t ra[16], rb[16];
   // group gi covers columns col(gi) .. +15
   auto col = [&](int gi) { return WPS_ == 4 ? 16 * gi : 32 * half + 64 * (gi >> 1) + 16 * (gi & 1); };
-  auto finish = [&](const uint32_t* regs, int c0) {
+  auto finish = [&](const uint32_t* regs, const float4* b, int c0) {
     const uint32_t k0 = (uint32_t)(c0 >> 3);  // first 16-byte chunk of the group
     const uint32_t base = rowbase + (k0 >> 3) * (uint32_t)kKBlockBytes;
-    finish16<RELU>(regs, bias + c0, base + (((k0 & 7u) << 4) ^ swz), base + ((((k0 & 7u) + 1u) << 4) ^ swz),
+    finish16<RELU>(regs, b, base + (((k0 & 7u) << 4) ^ swz), base + ((((k0 & 7u) + 1u) << 4) ^ swz),
                    activation, slope);
   };
+  float4 ba[4], bb[4];
   if (col(0) + 16 <= n_act) tmem_ld16_async(taddr + col(0), ra);
 #pragma unroll
   for (int gp = 0; gp < G / 2; ++gp) {
     const int c0 = col(2 * gp), c1 = col(2 * gp + 1);
     if (c0 + 16 > n_act) break;
+    lds_bias16(bias_saddr + 4u * c0, ba);
     tmem_wait16(ra);
     if (c1 + 16 <= n_act) tmem_ld16_async(taddr + c1, rb);
-    finish(ra, c0);
+    finish(ra, ba, c0);
     if (c1 + 16 > n_act) break;
+    lds_bias16(bias_saddr + 4u * c1, bb);
     tmem_wait16(rb);
     if (2 * gp + 2 < G) {
       const int c2 = col(2 * gp + 2);
       if (c2 + 16 <= n_act) tmem_ld16_async(taddr + c2, ra);
     }
-    finish(rb, c1);
+    finish(rb, bb, c1);
   }
 }
 
@@ -488,7 +511,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
           tc_fence_after();
           if (st.type == ST_HIDDEN || st.type == ST_HEAD_SPLIT_A) {
             // activated columns [0, n_act) -> bf16 -> next stage's A operand
-            hidden_epilogue<WPS, RELU>(taddr, bias, st.n_act, half, rowbase, swz, plan.activation, plan.leaky_slope);
+            hidden_epilogue<WPS, RELU>(taddr, smem_u32(bias), st.n_act, half, rowbase, swz, plan.activation, plan.leaky_slope);
             if (st.type == ST_HEAD_SPLIT_A && half == 0) {  // SSS logits sit right after the activated columns
               float v[16];
               tmem_ld16(taddr + st.n_act, v);
