@@ -28,7 +28,7 @@ namespace sssgs {
 namespace {
 
 constexpr int kRows = 128;             // rows per tile = UMMA M
-constexpr int kKBlockBytes = kRows * 128;  // one 64-wide K block of an A tile (128 rows x 128 B)
+constexpr int kKBlockBytes = kRows * 128;  // one 64-wide K block of an smem A tile (128 rows x 128 B)
 constexpr float kY00 = 0.2820948f, kY1 = 0.4886025f;
 
 // ---------------------------------------------------------------------------------------------
@@ -80,16 +80,6 @@ __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
 __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
   asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols)
                : "memory");
-}
-// D[tmem] (+)= A[smem desc] . B[smem desc]^T, kind::f16 (bf16 inputs, fp32 accumulate)
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b,
-                                          uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
-      : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar)
@@ -190,9 +180,11 @@ struct MlpArgs {
   float4* out_internal;        // [n][n_lights]
   float* out_user;             // optional: light l at out_user + l*user_light_stride, [n][4]
   int64_t user_light_stride;   // in floats
-  int slots;                   // row tiles in flight per CTA (2..4)
-  int wps;                     // epilogue warps per slot: 4 (one per 32 rows) or 8 (two column halves)
-  int slot_cols;               // TMEM columns per slot
+  int slots;                   // row tiles in flight per CTA (1..4)
+  int wps;                     // warps per slot: 4 (one per 32 rows) or 8 (two column halves)
+  int slot_cols;               // TMEM columns per slot: accumulator D (then the A operand, TS mode)
+  int a_col;                   // TS mode: column offset of the A operand inside a slot
+  int a_bytes;                 // SS mode: bytes of one slot's A tile in shared memory
   MlpPlan plan;
 };
 
@@ -267,13 +259,98 @@ __device__ __forceinline__ uint4 assemble_light(const MlpArgs& a, int64_t g, con
                     pack_bf16(d, v));
 }
 
-// Writes the chunks [c_begin, c_end) of row r of the layer-0 A tile.
-__device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, uint8_t* A, int r, int c_begin,
+// ---- TMEM helpers ---------------------------------------------------------------------------------
+// The A operand of every layer lives in TMEM (tcgen05.mma with A from tensor memory): row m of the
+// tile is TMEM lane m, and 32-bit column j of the operand holds the bf16 pair (k = 2j, 2j + 1), low
+// half first.  Only the weights are read from shared memory by the tensor core.
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, uint4 v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(v.x),
+               "r"(v.y), "r"(v.z), "r"(v.w)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() {
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+// D[tmem] (+)= A[tmem] . B[smem desc]^T, kind::f16 (bf16 inputs, fp32 accumulate); ACC = false
+// overwrites D.  The predicate is a compile-time constant so that the issuing lane spends no
+// instructions on it: the K steps of a stage are issued back to back by one thread, and every
+// instruction in that loop adds latency between tensor-core dispatches.
+template <bool ACC>
+__device__ __forceinline__ void umma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b,
+                                             uint32_t idesc) {
+  if (ACC) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.eq.u32 p, 1, 1;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.eq.u32 p, 1, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc)
+        : "memory");
+  }
+}
+
+// Same with A from shared memory (K-major, 128-byte swizzle descriptors for both operands).
+template <bool ACC>
+__device__ __forceinline__ void umma_bf16_ss(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b,
+                                             uint32_t idesc) {
+  if (ACC) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.eq.u32 p, 1, 1;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.eq.u32 p, 1, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void sts128(uint32_t saddr, uint4 v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+               : "memory");
+}
+
+// Where one thread writes its row of a slot's A operand.  Two modes (template flag TS):
+//   TS: A in TMEM at `at` (this thread's lane; 16-byte chunk c = columns at + 4c .. 4c + 3)
+//   SS: A in shared memory, K-major with the 128-byte swizzle: chunk c of the row sits at
+//       rowbase + (c / 8) * kKBlockBytes + (((c % 8) << 4) ^ swz), swz = (row % 8) << 4
+struct ARow {
+  uint32_t at, rowbase, swz;
+};
+template <bool TS>
+__device__ __forceinline__ void a_store(const ARow& ar, int c, uint4 v) {
+  if (TS) tmem_st4(ar.at + 4 * c, v);
+  else sts128(ar.rowbase + (uint32_t)(c >> 3) * (uint32_t)kKBlockBytes + ((((uint32_t)c & 7u) << 4) ^ ar.swz), v);
+}
+// Makes this thread's A-operand writes visible to the tensor core before it signals a_ready.
+template <bool TS>
+__device__ __forceinline__ void a_publish() {
+  if (TS) {
+    tmem_wait_st();
+    tc_fence_before();
+  } else {
+    tc_fence_before();
+    fence_proxy_async();
+  }
+}
+
+// Writes the 16-byte chunks [c_begin, c_end) of this thread's row of the layer-0 A operand.
+template <bool TS>
+__device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, const ARow& ar, int c_begin,
                                           int c_end, const uint4* keep, const uint4& light_chunk) {
 #pragma unroll
   for (int c = 0; c < kKeepChunks; ++c)
-    if (c >= c_begin && c < c_end)
-      *reinterpret_cast<uint4*>(A + swz_off(r, c, kKBlockBytes)) = (c == 1) ? light_chunk : keep[c];
+    if (c >= c_begin && c < c_end) a_store<TS>(ar, c, (c == 1) ? light_chunk : keep[c]);
   // the per-Gaussian feature (chunks 5..) is read here: it stays L2-resident across the lights
   const int F = a.plan.feat_dim;
   for (int c = max(c_begin, kKeepChunks); c < c_end; ++c) {
@@ -281,8 +358,8 @@ __device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, uint8_t* 
     float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0;
     if (j < F) f0 = *reinterpret_cast<const float4*>(a.feat + g * F + j);
     if (j + 4 < F) f1 = *reinterpret_cast<const float4*>(a.feat + g * F + j + 4);
-    *reinterpret_cast<uint4*>(A + swz_off(r, c, kKBlockBytes)) =
-        make_uint4(pack_bf16(f0.x, f0.y), pack_bf16(f0.z, f0.w), pack_bf16(f1.x, f1.y), pack_bf16(f1.z, f1.w));
+    a_store<TS>(ar, c, make_uint4(pack_bf16(f0.x, f0.y), pack_bf16(f0.z, f0.w), pack_bf16(f1.x, f1.y),
+                                  pack_bf16(f1.z, f1.w)));
   }
 }
 
@@ -311,11 +388,6 @@ __device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
   asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
-__device__ __forceinline__ void sts128(uint32_t saddr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
-  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(saddr), "r"(x), "r"(y), "r"(z), "r"(w)
-               : "memory");
-}
-
 // (x0, x1) += (y0, y1) as one packed fp32x2 add (sm_100 FADD2)
 __device__ __forceinline__ void add2(float& x0, float& x1, float y0, float y1) {
   asm("{\n\t.reg .b64 a, b;\n\t"
@@ -336,90 +408,96 @@ __device__ __forceinline__ void lds_bias16(uint32_t saddr, float4* b) {
         : "r"(saddr + 16u * q));
 }
 
-// bias + activation + bf16 of 16 accumulator columns -> two 16-byte chunks of the next A operand
-// at shared addresses sa0, sa1; b = the 16 biases.
-template <bool RELU>
-__device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, uint32_t sa0, uint32_t sa1,
+// bias + activation + bf16 of the 16 accumulator columns c0 .. c0 + 15 -> next A operand.
+template <bool RELU, bool TS>
+__device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, const ARow& ar, int c0,
                                          int activation, float slope) {
+  float v[16];
 #pragma unroll
-  for (int q = 0; q < 2; ++q) {
-    float v[8];
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[8 * q + i]);
-    add2(v[0], v[1], b[2 * q].x, b[2 * q].y);
-    add2(v[2], v[3], b[2 * q].z, b[2 * q].w);
-    add2(v[4], v[5], b[2 * q + 1].x, b[2 * q + 1].y);
-    add2(v[6], v[7], b[2 * q + 1].z, b[2 * q + 1].w);
-    const uint32_t sa = q ? sa1 : sa0;
+  for (int q = 0; q < 4; ++q) {
+    add2(v[4 * q], v[4 * q + 1], b[q].x, b[q].y);
+    add2(v[4 * q + 2], v[4 * q + 3], b[q].z, b[q].w);
+  }
+  uint32_t w[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
     if (RELU) {
-      sts128(sa, pack_bf16_relu(v[0], v[1]), pack_bf16_relu(v[2], v[3]), pack_bf16_relu(v[4], v[5]),
-             pack_bf16_relu(v[6], v[7]));
+      w[i] = pack_bf16_relu(v[2 * i], v[2 * i + 1]);
     } else {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) v[i] = act_fn(v[i], activation, slope);
-      sts128(sa, pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]), pack_bf16(v[6], v[7]));
+      w[i] = pack_bf16(act_fn(v[2 * i], activation, slope), act_fn(v[2 * i + 1], activation, slope));
     }
   }
+  a_store<TS>(ar, c0 >> 3, make_uint4(w[0], w[1], w[2], w[3]));
+  a_store<TS>(ar, (c0 >> 3) + 1, make_uint4(w[4], w[5], w[6], w[7]));
 }
 
 // Hidden-stage epilogue of one thread: its share of the activated columns [0, n_act), in groups
 // of 16, with the TMEM load of the next group in flight while the current one is finished.
 // WPS = 4: all columns; WPS = 8: the two warps of a row quarter take alternate 32-column blocks.
-// Chunk k (16 bytes = 8 columns) of K block kb of this row sits at rowbase + kb * kKBlockBytes +
-// ((k ^ (row & 7)) << 4); rowbase is 128-byte aligned, so the swizzle is an XOR on the address.
-template <int WPS_, bool RELU>
-__device__ __forceinline__ void hidden_epilogue(uint32_t taddr, uint32_t bias_saddr, int n_act, int half,
-                                                uint32_t rowbase, uint32_t swz, int activation,
-                                                float slope) {
+// d_taddr: this thread's lane base in the slot's accumulator.
+template <int WPS_, bool RELU, bool TS>
+__device__ __forceinline__ void hidden_epilogue(uint32_t d_taddr, const ARow& ar, uint32_t bias_saddr,
+                                                int n_act, int half, int activation, float slope) {
   constexpr int G = WPS_ == 4 ? 8 : 4;  // groups of 16 columns per thread for 128 columns
   uint32_t ra[16], rb[16];
+  float4 ba[4], bb[4];
   // group gi covers columns col(gi) .. +15
   auto col = [&](int gi) { return WPS_ == 4 ? 16 * gi : 32 * half + 64 * (gi >> 1) + 16 * (gi & 1); };
-  auto finish = [&](const uint32_t* regs, const float4* b, int c0) {
-    const uint32_t k0 = (uint32_t)(c0 >> 3);  // first 16-byte chunk of the group
-    const uint32_t base = rowbase + (k0 >> 3) * (uint32_t)kKBlockBytes;
-    finish16<RELU>(regs, b, base + (((k0 & 7u) << 4) ^ swz), base + ((((k0 & 7u) + 1u) << 4) ^ swz),
-                   activation, slope);
-  };
-  float4 ba[4], bb[4];
-  if (col(0) + 16 <= n_act) tmem_ld16_async(taddr + col(0), ra);
+  if (col(0) + 16 <= n_act) tmem_ld16_async(d_taddr + col(0), ra);
 #pragma unroll
   for (int gp = 0; gp < G / 2; ++gp) {
     const int c0 = col(2 * gp), c1 = col(2 * gp + 1);
     if (c0 + 16 > n_act) break;
     lds_bias16(bias_saddr + 4u * c0, ba);
     tmem_wait16(ra);
-    if (c1 + 16 <= n_act) tmem_ld16_async(taddr + c1, rb);
-    finish(ra, ba, c0);
+    if (c1 + 16 <= n_act) tmem_ld16_async(d_taddr + c1, rb);
+    finish16<RELU, TS>(ra, ba, ar, c0, activation, slope);
     if (c1 + 16 > n_act) break;
     lds_bias16(bias_saddr + 4u * c1, bb);
     tmem_wait16(rb);
     if (2 * gp + 2 < G) {
       const int c2 = col(2 * gp + 2);
-      if (c2 + 16 <= n_act) tmem_ld16_async(taddr + c2, ra);
+      if (c2 + 16 <= n_act) tmem_ld16_async(d_taddr + c2, ra);
     }
-    finish(rb, bb, c1);
+    finish16<RELU, TS>(rb, bb, ar, c1, activation, slope);
   }
 }
 
 constexpr int kMaxSlots = 4;
+
+#ifdef SSSGS_MLP_TIMELINE
+// Debug builds only (-DSSSGS_MLP_TIMELINE): SM-clock stamps of one CTA's slots, read back with
+// sssgs_debug_mlp_timeline().  Not compiled into the product library.
+__device__ long long g_timeline[kMaxSlots][512];
+#define TL_STAMP(code)                                                              \
+  do {                                                                              \
+    if (blockIdx.x == 0 && wq == 0 && lane == 0 && tl_n < 510) {                    \
+      g_timeline[slot][tl_n++] = (clock64() << 4) | (code);                         \
+      g_timeline[slot][511] = tl_n;                                                 \
+    }                                                                               \
+  } while (0)
+#else
+#define TL_STAMP(code) do {} while (0)
+#endif
 constexpr int kMlpThreadsMax = 512;  // up to 16 warps: 4 slots x 4 warps or 2 slots x 8 warps
 
 // Work distribution: a "unit" is a block of 128 Gaussians with all the lights of the batch; slot s of
 // CTA b owns the units (i * slots + s) * gridDim.x + b, i = 0, 1, ...  Within a unit the lights are
 // walked in order so that the light-independent inputs of a row are assembled once.
-template <int WPS, bool RELU>
+template <int WPS, bool RELU, bool TS>
 __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_constant__ MlpArgs a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const MlpPlan& plan = a.plan;
-  const int a_bytes = plan.max_k_bytes;
   const int S = a.slots;
   uint8_t* sW = smem;
-  uint8_t* sA0 = smem + plan.blob_bytes;
-  float* sBias = reinterpret_cast<float*>(sA0 + S * a_bytes);
+  uint8_t* sA0 = smem + plan.blob_bytes;  // SS mode: one A tile per slot (a_bytes = 0 in TS mode)
+  float* sBias = reinterpret_cast<float*>(sA0 + S * a.a_bytes);
   uint64_t* bars = reinterpret_cast<uint64_t*>(sBias + ((plan.bias_floats + 3) & ~3));
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kMaxSlots);
+  uint32_t* issue_lock = tmem_slot + 1;  // serialises the slots' MMA batches (see issue_stage)
   // bars[s] = a_ready of slot s, bars[kMaxSlots + s] = d_ready of slot s
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -434,6 +512,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
       mbar_init(smem_u32(bars + s), WPS * 32);
       mbar_init(smem_u32(bars + kMaxSlots + s), 1);
     }
+    *issue_lock = 0u;
     fence_barrier_init();
   }
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), 512);
@@ -450,42 +529,74 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
     const int slot = warp / WPS, wq = warp % WPS;
     const int quarter = wq & 3, half = wq >> 2;   // column half (WPS = 8)
     const int r = quarter * 32 + lane;            // row of the tile = TMEM lane
+    // this thread's lane base in the slot's accumulator (d) and A operand (at)
     const uint32_t taddr = tmem_base + slot * a.slot_cols + ((uint32_t)(quarter * 32) << 16);
-    uint8_t* A = sA0 + slot * a_bytes;
+    ARow ar;
+    ar.at = taddr + a.a_col;
+    ar.rowbase = smem_u32(sA0 + slot * a.a_bytes) + (uint32_t)(r * 128);
+    ar.swz = (uint32_t)((r & 7) << 4);
     const uint32_t bar_a = smem_u32(bars + slot), bar_d = smem_u32(bars + kMaxSlots + slot);
     // The first warp of a slot also issues the slot's MMAs: once all rows of the A operand have
     // arrived (a_ready), one elected lane issues the K steps of the stage and commits them to
     // d_ready.  A slot's pipeline is serial anyway (A operand -> MMA -> epilogue -> next A operand);
     // the tensor core is kept busy by the other slots.
+    int tl_n = 0;
+    (void)tl_n;
     uint32_t pa = 0;
     auto issue_stage = [&](int s_idx) {
       if (wq != 0) return;
+      TL_STAMP(0);
       mbar_wait(bar_a, pa);
       pa ^= 1u;
       tc_fence_after();
+      TL_STAMP(1);
       if (lane == 0) {
+        // TS mode (two slots): one slot's K steps go to the tensor core as a batch.  If the two slots
+        // interleaved their steps they would finish together and stay in lock-step (both in the
+        // epilogue, then both waiting for the tensor core); batching staggers them so that one
+        // slot's epilogue runs under the other's MMAs.
+        if (TS) {
+          while (atomicCAS(issue_lock, 0u, 1u) != 0u) {
+          }
+        }
+        TL_STAMP(6);
         const MlpStage& st = plan.st[s_idx];
         const uint32_t idesc = make_idesc(st.n_pad);
         const uint32_t w_addr = smem_u32(sW + st.w_off);
-        const uint32_t a_addr = smem_u32(A);
         const uint32_t d_addr = tmem_base + slot * a.slot_cols;
+        const uint32_t a_addr = d_addr + a.a_col;                          // TS: A operand in TMEM
+        const uint32_t a_smem = smem_u32(sA0 + slot * a.a_bytes);          // SS: A tile in smem
+        // one K step = 16 bf16 = 8 TMEM columns of A and 32 bytes inside a 128-byte swizzled row of
+        // the weights (the descriptor's start address advances by 32 >> 4; the second 64-wide K block
+        // starts n_pad * 128 bytes further)
         const int ksteps = st.k_pad >> 4;
-        for (int ks = 0; ks < ksteps; ++ks) {
-          const int kb = ks >> 2, kin = ks & 3;
-          const uint64_t da = make_desc(a_addr + kb * kKBlockBytes + kin * 32);
-          const uint64_t db = make_desc(w_addr + kb * (st.n_pad * 128) + kin * 32);
-          umma_bf16(d_addr, da, db, idesc, ks > 0 ? 1u : 0u);
+        const uint64_t db0 = make_desc(w_addr);
+        const uint64_t db1 = make_desc(w_addr + st.n_pad * 128);
+        if (TS) {
+          umma_bf16_ts<false>(d_addr, a_addr, db0, idesc);
+#pragma unroll
+          for (int ks = 1; ks < 8; ++ks)
+            if (ks < ksteps) umma_bf16_ts<true>(d_addr, a_addr + ks * 8, (ks < 4 ? db0 : db1) + (uint64_t)((ks & 3) * 2), idesc);
+        } else {
+          const uint64_t da0 = make_desc(a_smem), da1 = make_desc(a_smem + kKBlockBytes);
+          umma_bf16_ss<false>(d_addr, da0, db0, idesc);
+#pragma unroll
+          for (int ks = 1; ks < 8; ++ks)
+            if (ks < ksteps)
+              umma_bf16_ss<true>(d_addr, (ks < 4 ? da0 : da1) + (uint64_t)((ks & 3) * 2),
+                                 (ks < 4 ? db0 : db1) + (uint64_t)((ks & 3) * 2), idesc);
         }
         umma_commit(bar_d);  // arrives when the MMAs above have completed
+        if (TS) atomicExch(issue_lock, 0u);
       }
       __syncwarp();
+      TL_STAMP(2);
     };
     // 16-byte input chunks this thread writes
     const int nchunks = plan.in_pad >> 3;
     const int c_split = nchunks > 5 ? 5 : nchunks;
     const int c_begin = (WPS == 8 && half == 1) ? c_split : 0;
     const int c_end = (WPS == 8 && half == 0) ? c_split : nchunks;
-    const uint32_t rowbase = smem_u32(A) + (uint32_t)(r * 128), swz = (uint32_t)((r & 7) << 4);
     uint32_t pd = 0;
     for (int64_t u = (int64_t)slot * gridDim.x + blockIdx.x; u < n_units; u += (int64_t)S * gridDim.x) {
       const int64_t g_raw = u * kRows + r;
@@ -497,8 +608,8 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
       for (int light = 0; light < a.n_lights; ++light) {
         uint4 lc = make_uint4(0u, 0u, 0u, 0u);
         if (c_begin == 0) lc = assemble_light(a, g, a.lights.l[light], mu, wout);
-        write_row(a, g, A, r, c_begin, c_end, keep, lc);
-        fence_proxy_async();
+        write_row<TS>(a, g, ar, c_begin, c_end, keep, lc);
+        a_publish<TS>();
         mbar_arrive(bar_a);
         issue_stage(0);
 
@@ -509,17 +620,18 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
           mbar_wait(bar_d, pd);
           pd ^= 1u;
           tc_fence_after();
+          TL_STAMP(3);
           if (st.type == ST_HIDDEN || st.type == ST_HEAD_SPLIT_A) {
             // activated columns [0, n_act) -> bf16 -> next stage's A operand
-            hidden_epilogue<WPS, RELU>(taddr, smem_u32(bias), st.n_act, half, rowbase, swz, plan.activation, plan.leaky_slope);
+            hidden_epilogue<WPS, RELU, TS>(taddr, ar, smem_u32(bias), st.n_act, half, plan.activation, plan.leaky_slope);
             if (st.type == ST_HEAD_SPLIT_A && half == 0) {  // SSS logits sit right after the activated columns
               float v[16];
               tmem_ld16(taddr + st.n_act, v);
 #pragma unroll
               for (int c = 0; c < 3; ++c) sss_keep[c] = 1.f / (1.f + __expf(-(v[c] + bias[st.n_act + c])));
             }
-            tc_fence_before();
-            fence_proxy_async();
+            TL_STAMP(4);
+            a_publish<TS>();
             mbar_arrive(bar_a);
             issue_stage(s + 1);
           } else {
@@ -541,6 +653,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
                   *reinterpret_cast<float4*>(a.out_user + (int64_t)light * a.user_light_stride + g * 4) = o;
               }
             }
+            TL_STAMP(5);
             tc_fence_before();  // TMEM reads are ordered before the next tile's a_ready arrive
           }
         }
@@ -556,23 +669,40 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
 
 }  // namespace
 
-// Slots (row tiles in flight per CTA), epilogue warps per slot and TMEM columns per slot for a plan.
-static void mlp_shape(const MlpPlan& plan, int* slots, int* wps, int* slot_cols) {
-  const int cols = plan.max_n <= 128 ? 128 : 256;
+// How a plan runs.  A slot (one 128-row tile in flight) needs its fp32 accumulator in TMEM (widest
+// layer, rounded up to 32 columns) and its bf16 A operand either in shared memory (SS mode: one
+// max_k_bytes tile per slot next to the weights) or in TMEM behind the accumulator (TS mode: widest
+// input / 2 columns).  Reading accumulators back is the binding resource (TMEM reads ~64 B/clk per
+// SM), and TS mode adds the A reads to it, so SS mode is used whenever shared memory
+// holds 4 tiles (or more tiles than TMEM would); wide nets whose weights fill shared memory run in
+// TS mode.  At most 4 slots (512 TMEM columns, 16 warps).
+struct MlpShape {
+  int slots, wps, slot_cols, a_col, a_bytes;
+  bool ts;
+};
+static MlpShape mlp_shape(const MlpPlan& plan) {
+  const int d_cols = (plan.max_n + 31) / 32 * 32;
+  const int a_cols = plan.max_k_bytes / (kRows * 128) * 32;  // K blocks of 64 bf16 = 32 columns each
   const int fixed = plan.blob_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 2 * kMaxSlots * 8 + 16 + 1024;
-  int s = (227 * 1024 - fixed) / plan.max_k_bytes;
-  if (s > 512 / cols) s = 512 / cols;
-  if (s > kMaxSlots) s = kMaxSlots;
-  if (s < 1) s = 1;
-  *slots = s;
-  *wps = s <= 2 ? 8 : 4;
-  *slot_cols = cols;
+  int s_ss = (227 * 1024 - fixed) / plan.max_k_bytes;
+  if (s_ss > 512 / d_cols) s_ss = 512 / d_cols;
+  if (s_ss > kMaxSlots) s_ss = kMaxSlots;
+  int s_ts = 512 / (d_cols + a_cols);
+  if (s_ts > kMaxSlots) s_ts = kMaxSlots;
+  MlpShape sh;
+  sh.ts = !(s_ss >= kMaxSlots || s_ss > s_ts);
+  sh.slots = sh.ts ? s_ts : s_ss;
+  if (sh.slots < 1) sh.slots = 1;
+  sh.wps = sh.slots <= 2 ? 8 : 4;
+  sh.slot_cols = sh.ts ? d_cols + a_cols : d_cols;
+  sh.a_col = d_cols;
+  sh.a_bytes = sh.ts ? 0 : plan.max_k_bytes;
+  return sh;
 }
 
 int mlp_smem_bytes(const MlpPlan& plan) {
-  int s, w, c;
-  mlp_shape(plan, &s, &w, &c);
-  return plan.blob_bytes + s * plan.max_k_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 2 * kMaxSlots * 8 + 16 + 1024;
+  const MlpShape sh = mlp_shape(plan);
+  return plan.blob_bytes + sh.slots * sh.a_bytes + ((plan.bias_floats + 3) & ~3) * 4 + 2 * kMaxSlots * 8 + 16 + 1024;
 }
 
 int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
@@ -597,7 +727,8 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
   a.blob = blob; a.bias = bias;
   a.out_internal = out_internal; a.out_user = out_user; a.user_light_stride = user_light_stride;
   a.plan = plan;
-  mlp_shape(plan, &a.slots, &a.wps, &a.slot_cols);
+  const MlpShape sh = mlp_shape(plan);
+  a.slots = sh.slots; a.wps = sh.wps; a.slot_cols = sh.slot_cols; a.a_col = sh.a_col; a.a_bytes = sh.a_bytes;
   const int smem = mlp_smem_bytes(plan);
   const int64_t units = (g.n + kRows - 1) / kRows;
   const int grid = (int)(units < num_sms ? units : num_sms);
@@ -611,9 +742,24 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
     kernel<<<grid, a.slots * a.wps * 32, smem, s>>>(a);
     return 1;
   };
-  static int cfg_smem[4] = {0, 0, 0, 0};
-  if (a.wps == 4) return relu ? launch(mlp_kernel<4, true>, &cfg_smem[0]) : launch(mlp_kernel<4, false>, &cfg_smem[1]);
-  return relu ? launch(mlp_kernel<8, true>, &cfg_smem[2]) : launch(mlp_kernel<8, false>, &cfg_smem[3]);
+  static int cfg_smem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  const int v = (a.wps == 8 ? 4 : 0) + (relu ? 2 : 0) + (sh.ts ? 1 : 0);
+  switch (v) {
+    case 0: return launch(mlp_kernel<4, false, false>, &cfg_smem[0]);
+    case 1: return launch(mlp_kernel<4, false, true>, &cfg_smem[1]);
+    case 2: return launch(mlp_kernel<4, true, false>, &cfg_smem[2]);
+    case 3: return launch(mlp_kernel<4, true, true>, &cfg_smem[3]);
+    case 4: return launch(mlp_kernel<8, false, false>, &cfg_smem[4]);
+    case 5: return launch(mlp_kernel<8, false, true>, &cfg_smem[5]);
+    case 6: return launch(mlp_kernel<8, true, false>, &cfg_smem[6]);
+    default: return launch(mlp_kernel<8, true, true>, &cfg_smem[7]);
+  }
 }
 
 }  // namespace sssgs
+
+#ifdef SSSGS_MLP_TIMELINE
+extern "C" int sssgs_debug_mlp_timeline(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, sssgs::g_timeline, sizeof(long long) * sssgs::kMaxSlots * 512);
+}
+#endif

@@ -447,8 +447,11 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   int64_t frame_stride_px, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
+  // Default shape: few tiles (small images) leave SMs idle behind the longest tile lists, so the
+  // lists are walked by 4 CTAs with 4 entry slots per warp; with many tiles the classic
+  // one-thread-per-pixel shape executes fewer instructions per blended pair (measured: DESIGN.md).
   int mode = raster_mode();
-  if (mode == 0) mode = 48;
+  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
 #define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s
 #define SSSGS_BY_LB(E, W, U)                                                   \
   do {                                                                         \
