@@ -33,9 +33,12 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2408_12282_b200 import scenes  # noqa: E402
+from paper_2408_12282_b200 import multi, scenes  # noqa: E402
 
 METRIC = "Mpix/s (MLP + G-buffer splat + deferred shading)"
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of a stage's kernel, from the
+# `ncu --set full` captures summarised under profiles/ (r01_ncu_full.md): (config, stage) -> bytes
+NCU_DRAM_BYTES_PER_LAUNCH = {}
 FP32_LANES_PER_SM = 128
 
 
@@ -102,14 +105,14 @@ def workload(cfg):
     return s, s.cameras[:1], s.lights[0], len(s.lights[0])
 
 
-def oracle_sample(scene, max_frames=1):
-    """Times the CPU oracle, as it stands, on a bounded sample (first frames of the first view)."""
+def oracle_sample(scene, min_seconds=0.0, max_frames=1):
+    """Times the CPU oracle, as it stands, on a bounded sample: whole-path renders of the first
+    (view, light) frame, repeated until `min_seconds` of CPU work (at least `max_frames` = 1 frame)."""
     import oracle
     t0 = time.perf_counter()
-    geo, frames, res = None, 0, None
-    for l in range(min(max_frames, len(scene.lights[0]))):
-        res = oracle.render_frame(scene, 0, l, mlp_mode=1, geometry=geo)
-        geo = geo or res
+    frames, res = 0, None
+    while frames < max_frames or time.perf_counter() - t0 < min_seconds:
+        res = oracle.render_frame(scene, 0, 0, mlp_mode=1)   # projection, lists, MLP, compositing, shading
         frames += 1
     dt = time.perf_counter() - t0
     cam = scene.cameras[0]
@@ -217,8 +220,7 @@ def run_gpu(args, rank, world, local_rank):
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
+        multi.barrier()
         torch.cuda.synchronize()
 
     stream = torch.cuda.current_stream(dev)
@@ -237,11 +239,8 @@ def run_gpu(args, rank, world, local_rank):
     t_wall = time.perf_counter() - t_wall
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * args.steps * fps * npix / (total_ms * 1e-3) / 1e6
+    total_ms = multi.max_over_ranks(total_ms, dev)
+    value = multi.whole_job_mpix_per_s(world, args.steps, fps, npix, total_ms)
 
     # ---- per-stage device times (events inside the library, same step, L2 flushed) --------------
     binding.sssgs_profile_enable(R.ctx, True)
@@ -264,11 +263,8 @@ def run_gpu(args, rank, world, local_rank):
     for _ in range(e2e_steps):
         H.render(cams, lights)
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_e2e = float(t.item())
-    e2e_val = world * e2e_steps * fps * npix / t_e2e / 1e6
+    t_e2e = multi.max_over_ranks(t_e2e, dev)
+    e2e_val = multi.whole_job_mpix_per_s(world, e2e_steps, fps, npix, t_e2e * 1e3)
     h2d, d2h = H.h2d_bytes, H.d2h_bytes
     H.close()
     if rank == 0 and len(sampler.rows) < 3:   # keep the GPU busy until a few samples exist
@@ -283,10 +279,10 @@ def run_gpu(args, rank, world, local_rank):
         cpu = None
         counters = None
         if world == 1 and not args.no_cpu_baseline:
-            r = oracle_sample(scene)
+            r = oracle_sample(scene, min_seconds=12.0)
             cpu = {"value": r["mpix_s"], "unit": "Mpix/s", "cores": r["cores"], "kind": "oracle",
-                   "sample": f"first (view, light) frame of configs[{args.config - 1}], whole path, "
-                             f"{r['seconds']:.2f} s"}
+                   "sample": f"{r['frames']} whole-path renders of the first (view, light) frame of "
+                             f"configs[{args.config - 1}] (bf16-emulating MLP), {r['seconds']:.1f} s of CPU work"}
             counters = (r["res"].comp.p_eval, r["res"].comp.p_blend)
         models, pk = stage_models(scene, nl, cnt[binding.CNT_NVIS], min(cnt[binding.CNT_INSTANCES], 20 * scene.n),
                                   counters, peaks, num_sms)
@@ -301,7 +297,8 @@ def run_gpu(args, rank, world, local_rank):
         dom = max(stage_ms, key=stage_ms.get)
         roof = {"kernel": dom, "bound": stages[dom].get("bound"), "achieved": stages[dom].get("achieved"),
                 "peak": round(pk[stages[dom]["bound"]][0], 2) if "bound" in stages[dom] else None,
-                "unit": stages[dom].get("unit"), "frac": stages[dom].get("frac"), "traffic": None,
+                "unit": stages[dom].get("unit"), "frac": stages[dom].get("frac"),
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, dom)),
                 "peak_source": peaks["source"] if stages[dom].get("bound") != "alu" else
                 "derived: SMs x 128 fp32 lanes x 2 x clocks.max.sm (DESIGN.md)",
                 "share_of_step": round(stage_ms[dom] / sum(stage_ms.values()), 3)}

@@ -5,7 +5,38 @@
 
 #include "../../include/sssgs.h"
 
+#include <utility>
+
 namespace sssgs {
+
+// ---- programmatic dependent launch ------------------------------------------------------------
+// The render path is a chain of short dependent kernels.  Each one is launched with the
+// programmatic-stream-serialization attribute and starts with pdl_prologue(): it lets the NEXT
+// kernel of the stream start launching once all of this kernel's CTAs are running, then waits
+// until the PREVIOUS kernel has completed and flushed.  Launch latency and CTA start-up of a
+// kernel thus overlap the tail of its predecessor; data dependences are unchanged (nothing is
+// read or written before the wait).  Without the attribute both instructions are no-ops.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_prologue() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                              cudaStream_t s, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 // ---- constants of the method (S4) -----------------------------------
 constexpr float kAlphaMin = 1.0f / 255.0f;
@@ -167,7 +198,7 @@ int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, fl
                     cudaStream_t s);
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
                const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
-               float4* out_internal, float* out_user, int64_t user_light_stride, int num_sms,
+               float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
                cudaStream_t s);
 int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,
                               float4* out_internal, cudaStream_t s);

@@ -38,6 +38,7 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ dvals0, const uint32_t* __r
   const unsigned tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t nchunks = (n + kEmitChunk - 1) / kEmitChunk;
   const uint32_t mask0 = (1u << bits0) - 1u, mask1 = bits1 ? (1u << bits1) - 1u : 0u;
+  pdl_prologue();
   s_hist[0][tid] = 0;
   s_hist[1][tid] = 0;
   // the depth-sorted index array sits in the buffer the last executed depth pass wrote
@@ -182,6 +183,7 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
               int64_t* __restrict__ counters_out) {
   __shared__ uint32_t s_cnt[32], s_start[32];
   __shared__ bool s_last;
+  pdl_prologue();
   const uint32_t n = min(counters[DC_INSTANCES], cap);
   for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i <= n; i += gridDim.x * 256u) {
     const int a = i == 0 ? -1 : (int)sorted_tiles[i - 1];
@@ -228,6 +230,7 @@ __global__ void __launch_bounds__(256)
 export_lists_kernel(const uint32_t* __restrict__ sorted_tiles, const uint32_t* __restrict__ sorted_vals,
                     const float4* __restrict__ rec_a, const uint32_t* __restrict__ counters,
                     uint32_t cap, uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out) {
+  pdl_prologue();
   const uint32_t n = min(counters[DC_INSTANCES], cap);
   for (uint32_t j = blockIdx.x * 256u + threadIdx.x; j < n; j += gridDim.x * 256u) {
     const uint32_t g = sorted_vals[j];
@@ -243,7 +246,7 @@ int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t
   if (n == 0) return 0;
   int64_t blocks = (n + kEmitChunk - 1) / kEmitChunk;
   if (blocks > 148 * 4) blocks = 148 * 4;
-  emit_kernel<<<(unsigned)blocks, kEmitThreads, 0, s>>>(
+  launch_pdl(emit_kernel, dim3((unsigned)blocks), dim3(kEmitThreads), 0, s,
       (uint32_t)n, gb.dvals[0], gb.dvals[1], gb.hist, gb.touched, gb.rect, cam.tiles_x, cap, gb.ikeys[0], gb.ivals[0],
       gb.hist + 4 * 256, gb.hist + 5 * 256, tile_shift0, tile_bits0, tile_shift1, tile_bits1, status,
       ticket, gb.counters);
@@ -255,7 +258,7 @@ int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const Geom
   const int tiles = cam.tiles_x * cam.tiles_y;
   int64_t blocks = ((int64_t)cap + 1 + 1023) / 1024;
   if (blocks > 148 * 4) blocks = 148 * 4;
-  ranges_kernel<<<(unsigned)blocks, 256, 0, s>>>(sorted_tiles, gb.counters, cap, tiles, gb.ranges,
+  launch_pdl(ranges_kernel, dim3((unsigned)blocks), dim3(256), 0, s, sorted_tiles, gb.counters, cap, tiles, gb.ranges,
                                                  ranges_user, gb.tile_slot, gb.tile_order, counters_out);
   return 1;
 }
@@ -266,7 +269,7 @@ int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_val
   int64_t blocks = ((int64_t)cap + 255) / 256;
   if (blocks > 148 * 8) blocks = 148 * 8;
   if (blocks < 1) blocks = 1;
-  export_lists_kernel<<<(unsigned)blocks, 256, 0, s>>>(sorted_tiles, sorted_vals, gb.rec_a,
+  launch_pdl(export_lists_kernel, dim3((unsigned)blocks), dim3(256), 0, s, sorted_tiles, sorted_vals, gb.rec_a,
                                                        gb.counters, cap, keys_out, vals_out);
   return 1;
 }

@@ -21,6 +21,8 @@
 // Output: float4 (L_SSS rgb, L_in) per (Gaussian, light), 16 B per row.
 #include <cuda_bf16.h>
 
+#include <cstdlib>
+
 #include "internal.cuh"
 
 namespace sssgs {
@@ -132,6 +134,7 @@ __device__ __forceinline__ uint32_t swz_off(int r, int c, int kblock_bytes) {
 __global__ void __launch_bounds__(256)
 mlp_pack_kernel(MlpPlan plan, const void* __restrict__ params, int dtype, uint8_t* __restrict__ blob,
                 float* __restrict__ bias) {
+  pdl_prologue();
   auto load = [&](int off) -> float {
     if (dtype == SSSGS_BF16)
       return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(params)[off]);
@@ -500,6 +503,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
   uint32_t* issue_lock = tmem_slot + 1;  // serialises the slots' MMA batches (see issue_stage)
   // bars[s] = a_ready of slot s, bars[kMaxSlots + s] = d_ready of slot s
 
+  pdl_prologue();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int64_t n_units = (a.n + kRows - 1) / kRows;
 
@@ -707,13 +711,13 @@ int mlp_smem_bytes(const MlpPlan& plan) {
 
 int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
                     cudaStream_t s) {
-  mlp_pack_kernel<<<32, 256, 0, s>>>(plan, mlp.params, mlp.dtype, blob, bias);
+  launch_pdl(mlp_pack_kernel, dim3(32), dim3(256), 0, s, plan, mlp.params, mlp.dtype, blob, bias);
   return 1;
 }
 
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
                const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
-               float4* out_internal, float* out_user, int64_t user_light_stride, int num_sms,
+               float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
                cudaStream_t s) {
   if (g.n == 0 || n_lights == 0) return 0;
   MlpArgs a;
@@ -731,7 +735,12 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
   a.slots = sh.slots; a.wps = sh.wps; a.slot_cols = sh.slot_cols; a.a_col = sh.a_col; a.a_bytes = sh.a_bytes;
   const int smem = mlp_smem_bytes(plan);
   const int64_t units = (g.n + kRows - 1) / kRows;
-  const int grid = (int)(units < num_sms ? units : num_sms);
+  int grid = (int)(units < max_ctas ? units : max_ctas);
+  {  // tuning aid: SSSGS_MLP_SMS caps the number of CTAs (= SMs) the MLP occupies
+    static int cap = -1;
+    if (cap < 0) { const char* e = getenv("SSSGS_MLP_SMS"); cap = e ? atoi(e) : 0; }
+    if (cap > 0 && grid > cap) grid = cap;
+  }
   const bool relu = plan.activation == SSSGS_ACT_RELU;
   auto launch = [&](auto kernel, int* configured_smem) -> int {
     if (smem > *configured_smem) {
@@ -739,7 +748,7 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
         return -1;
       *configured_smem = smem;
     }
-    kernel<<<grid, a.slots * a.wps * 32, smem, s>>>(a);
+    launch_pdl(kernel, dim3(grid), dim3(a.slots * a.wps * 32), (size_t)smem, s, a);
     return 1;
   };
   static int cfg_smem[8] = {0, 0, 0, 0, 0, 0, 0, 0};

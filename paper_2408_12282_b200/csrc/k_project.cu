@@ -40,6 +40,7 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
                uint32_t* __restrict__ dkeys, uint32_t* __restrict__ hist,
                uint32_t* __restrict__ counters) {
   __shared__ uint32_t s_hist[4 * 256];
+  pdl_prologue();
   for (int i = threadIdx.x; i < 4 * 256; i += kProjThreads) s_hist[i] = 0;
   __syncthreads();
 
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(256)
 pack_attr_kernel(int64_t n, const float* __restrict__ normals, const float* __restrict__ base,
                  const float* __restrict__ rough, const float* __restrict__ metal,
                  const float* __restrict__ sss, float4* __restrict__ attr) {
+  pdl_prologue();
   const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (i >= n) return;
   attr[3 * i + 0] = make_float4(normals[3 * i], normals[3 * i + 1], normals[3 * i + 2], rough[i]);
@@ -203,8 +205,8 @@ pack_attr_kernel(int64_t n, const float* __restrict__ normals, const float* __re
 int launch_pack_attr(const sssgs_gaussians& g, float4* attr, cudaStream_t s) {
   if (g.n == 0) return 0;
   const unsigned blocks = (unsigned)((g.n + 255) / 256);
-  pack_attr_kernel<<<blocks, 256, 0, s>>>(g.n, g.normals, g.base_color, g.roughness, g.metallic,
-                                          g.subsurface, attr);
+  launch_pdl(pack_attr_kernel, dim3(blocks), dim3(256), 0, s, g.n, g.normals, g.base_color, g.roughness,
+             g.metallic, g.subsurface, attr);
   return 1;
 }
 
@@ -212,9 +214,8 @@ int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuf
                    cudaStream_t s) {
   if (g.n == 0) return 0;
   const unsigned blocks = (unsigned)((g.n + kProjThreads - 1) / kProjThreads);
-  project_kernel<<<blocks, kProjThreads, 0, s>>>(g.n, g.means, g.scales, g.rotations, g.opacities,
-                                                 cam, gb.rec_a, gb.rec_b, gb.rect, gb.touched,
-                                                 gb.dkeys[0], gb.hist, gb.counters);
+  launch_pdl(project_kernel, dim3(blocks), dim3(kProjThreads), 0, s, g.n, g.means, g.scales, g.rotations,
+             g.opacities, cam, gb.rec_a, gb.rec_b, gb.rect, gb.touched, gb.dkeys[0], gb.hist, gb.counters);
   return 1;
 }
 

@@ -159,6 +159,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   uint32_t (*s_id)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + 2 * NC * kBatch);
   uint8_t (*s_q)[kBatch] = reinterpret_cast<uint8_t (*)[kBatch]>(s_id + 2);
 
+  pdl_prologue();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int slot = lane / P, pix = lane % P;
   const int tile = (int)tile_order[blockIdx.x / S::SUBS];  // longest lists first
@@ -424,9 +425,9 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
       return -1;
     configured = true;
   }
-  raster_shade_kernel<LB, E, WARPS, U><<<tiles * S::SUBS, S::THREADS, smem, s>>>(
-      cam, lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out,
-      rgb, gbuf, aov_d, aov_s, frame_stride_px);
+  launch_pdl(raster_shade_kernel<LB, E, WARPS, U>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam, lights,
+             n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
+             aov_d, aov_s, frame_stride_px);
   return 1;
 }
 

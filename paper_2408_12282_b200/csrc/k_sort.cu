@@ -202,6 +202,7 @@ radix_pass_kernel(uint32_t* __restrict__ k0, uint32_t* __restrict__ v0, uint32_t
                   uint32_t* __restrict__ err, int depth_pass) {
   __shared__ SortSmem sm;
   const unsigned tid = threadIdx.x;
+  pdl_prologue();
   if (tid == 0) sm.ticket = atomicAdd(ticket, 1u);
   const uint32_t n = count_ptr ? min(*count_ptr, count_cap) : count_cap;
   const uint32_t radix = 1u << bits, mask = radix - 1u;
@@ -244,9 +245,9 @@ int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t*
   if (count_cap == 0) return 0;
   int64_t blocks = (int64_t)sort_status_rows(count_cap);
   if (blocks > max_blocks) blocks = max_blocks;
-  radix_pass_kernel<<<(unsigned)blocks, kSortThreads, 0, s>>>(
-      const_cast<uint32_t*>(keys_in), const_cast<uint32_t*>(vals_in), keys_out, vals_out, count_ptr,
-      count_cap, shift, bits, hist, status, ticket, err, -1);
+  launch_pdl(radix_pass_kernel, dim3((unsigned)blocks), dim3(kSortThreads), 0, s,
+             const_cast<uint32_t*>(keys_in), const_cast<uint32_t*>(vals_in), keys_out, vals_out, count_ptr,
+             count_cap, shift, bits, hist, status, ticket, err, -1);
   return 1;
 }
 
@@ -256,9 +257,8 @@ int launch_depth_pass(uint32_t* const keys[2], uint32_t* const vals[2], uint32_t
   if (n == 0) return 0;
   int64_t blocks = (int64_t)sort_status_rows(n);
   if (blocks > max_blocks) blocks = max_blocks;
-  radix_pass_kernel<<<(unsigned)blocks, kSortThreads, 0, s>>>(keys[0], vals[0], keys[1], vals[1], nullptr,
-                                                              n, 8 * pass, 8, hist4, status, ticket, err,
-                                                              pass);
+  launch_pdl(radix_pass_kernel, dim3((unsigned)blocks), dim3(kSortThreads), 0, s, keys[0], vals[0], keys[1],
+             vals[1], (const uint32_t*)nullptr, n, 8 * pass, 8, hist4, status, ticket, err, pass);
   return 1;
 }
 
