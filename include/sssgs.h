@@ -21,6 +21,9 @@
  *   - Device pointers must be 16-byte aligned; arrays are dense, row-major, fp32 unless noted.
  *   - Work is enqueued on the given CUDA stream; sssgs_render never synchronises and is
  *     CUDA-graph-capture safe.  Results are valid once the caller has synchronised the stream.
+ *     Internally the MLP runs on a stream owned by the context, forked from and joined back to
+ *     the caller's stream with events inside the same call (so it overlaps the geometry stages);
+ *     to the caller the call behaves as if everything ran on the given stream.
  *   - Every function returns 0 (SSSGS_OK) or a negative sssgs_status; no exceptions or aborts
  *     cross the ABI.  sssgs_last_error() returns a human-readable description.
  *   - There is no CPU fallback: without an sm_100 device sssgs_create fails (SSSGS_EARCH).

@@ -7,16 +7,22 @@
 //   * persistent CTAs, one per SM; ALL layer weights live in shared memory for the whole kernel
 //     as UMMA operands (K-major, 128-byte swizzle), packed once per call by mlp_pack_kernel;
 //   * a row tile = 128 Gaussians x 1 light = the M of one tcgen05.mma (cta_group::1, M=128);
-//     its fp32 accumulator [128 x N] sits in TMEM (one 256-column slot per tile in flight);
-//   * two tiles are in flight per CTA ("slots"): while the four epilogue warps of slot 0 read
-//     their accumulator back (tcgen05.ld), add the bias, apply the activation, round to bf16 and
-//     write the NEXT layer's A operand straight into shared memory in the UMMA swizzled layout,
-//     the tensor core runs slot 1's layer -- activations never touch HBM;
-//   * the layer-0 A tile is COMPUTED, not loaded: the same warps assemble the 40+F inputs
+//     its fp32 accumulator [128 x N] sits in TMEM;
+//   * up to 4 tiles are in flight per CTA ("slots", 4 or 8 warps each).  A slot is a serial
+//     chain  A operand -> MMAs of the layer -> epilogue -> next layer's A operand ; the slots run
+//     out of phase so that one slot's epilogue (tcgen05.ld -> bias -> activation -> bf16) runs
+//     under the other slots' MMAs.  Activations never touch HBM;
+//   * the A operand of a layer is written by the epilogue warps either into shared memory in the
+//     UMMA swizzled layout (SS mode: 4 slots when the tiles fit next to the weights) or into
+//     TMEM behind the accumulator (TS mode, tcgen05.mma with A from tensor memory: nets whose
+//     weights fill shared memory; 2 slots x 8 warps) -- see mlp_shape();
+//   * the layer-0 A operand is COMPUTED, not loaded: the same warps assemble the 40+F inputs
 //     (unit directions, light distance, SH visibility, Fourier encoding of mu) in fp32 and store
-//     them as bf16;
-//   * warp 8 issues the MMAs (one elected thread) and owns the TMEM allocation; mbarriers
-//     (a_ready: 128 arrivals, d_ready: tcgen05.commit) hand tiles back and forth.
+//     them as bf16; a slot walks all lights of a block of 128 Gaussians so that the
+//     light-independent inputs are assembled once;
+//   * there is no dedicated MMA warp: the first warp of a slot waits for its slot's a_ready
+//     mbarrier (all rows written) and one elected lane issues the layer's K steps and commits
+//     them to the slot's d_ready mbarrier.
 //
 // Output: float4 (L_SSS rgb, L_in) per (Gaussian, light), 16 B per row.
 #include <cuda_bf16.h>
