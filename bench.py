@@ -134,7 +134,7 @@ def mlp_flops_per_row(mlp):
     return fl + 2 * di
 
 
-def stage_models(scene, nl, n_vis, inst, counters, peaks, num_sms):
+def stage_models(scene, nl, n_vis, inst, counters, peaks, num_sms, mlp_rows):
     """Algorithmic work of each stage for ONE step."""
     n = scene.n
     cam = scene.cameras[0]
@@ -146,7 +146,8 @@ def stage_models(scene, nl, n_vis, inst, counters, peaks, num_sms):
         "depth_sort": ("hbm", (3 * 16.0 + 12.0) * n),
         "emit": ("hbm", 16.0 * n + 8.0 * inst),
         "tile_sort": ("hbm", 16.0 * inst * (2 if (cam.width + 15) // 16 * ((cam.height + 15) // 16) > 256 else 1)),
-        "mlp": ("tensor", float(mlp_flops_per_row(scene.mlp)) * n * nl),
+        # rows the MLP actually evaluated (in a sweep: the Gaussians blended at some pixel of the view)
+        "mlp": ("tensor", float(mlp_flops_per_row(scene.mlp)) * mlp_rows * nl),
     }
     if counters is not None:
         p_eval, p_blend = counters
@@ -285,8 +286,9 @@ def run_gpu(args, rank, world, local_rank):
                    "sample": f"{r['frames']} whole-path renders of the first (view, light) frame of "
                              f"configs[{args.config - 1}] (bf16-emulating MLP), {r['seconds']:.1f} s of CPU work"}
             counters = (r["res"].comp.p_eval, r["res"].comp.p_blend)
+        mlp_rows = cnt[binding.CNT_MLP_ROWS] or scene.n
         models, pk = stage_models(scene, nl, cnt[binding.CNT_NVIS], min(cnt[binding.CNT_INSTANCES], 20 * scene.n),
-                                  counters, peaks, num_sms)
+                                  counters, peaks, num_sms, mlp_rows)
         stages = {}
         for k, ms in stage_ms.items():
             e = {"ms": round(ms, 5), "launches": nlaunch[k]}
@@ -311,7 +313,7 @@ def run_gpu(args, rank, world, local_rank):
             "config": {"workload": f"configs[{args.config - 1}] {scene.name}", "gaussians": scene.n,
                        "width": cam.width, "height": cam.height, "frames_per_step": fps,
                        "l2": "flushed between timed steps (256 MiB memset)", "launch": "CUDA graph replay",
-                       "instances": cnt[binding.CNT_INSTANCES]},
+                       "instances": cnt[binding.CNT_INSTANCES], "mlp_rows_per_light": mlp_rows},
             "ms_per_frame": total_ms / args.steps / fps,
             "gaussians_per_s": world * args.steps * fps * scene.n / (total_ms * 1e-3),
             "clocks": clocks,

@@ -62,6 +62,8 @@ enum {
   SSSGS_CNT_INSTANCES = 1, /* I = sum of tiles touched (tile list length, before clamping)   */
   SSSGS_CNT_OVERFLOW = 2,  /* 1 if I > max_instances: the frame content is then undefined    */
   SSSGS_CNT_SORT_ERROR = 3,/* non-zero if a look-back wait exceeded its spin bound (bug trap) */
+  SSSGS_CNT_MLP_ROWS = 4,  /* Gaussians the MLP evaluated per light: n, or -- in a sweep of >= 4
+                              lights per view without mlp_out -- those blended at some pixel     */
   SSSGS_NCOUNTERS = 8
 };
 

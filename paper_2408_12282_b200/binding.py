@@ -26,7 +26,7 @@ SSSGS_MAX_INC_HIDDEN = 2
 SSSGS_LIGHTS_PER_CAMERA = 1
 SSSGS_F32, SSSGS_BF16 = 0, 1
 (SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
-CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR = 0, 1, 2, 3
+CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3, 4
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",

@@ -125,6 +125,7 @@ enum {
   DC_SORT_ERROR = 3,
   DC_TICKET_BASE = 8, // tickets: one per ticketed kernel launch
   DC_RANGES_DONE = 24,   // blocks of ranges_kernel that have finished
+  DC_CONTRIB_ROWS = 25,  // Gaussians kept by the visibility pre-pass (MLP rows of a sweep)
   DC_WORDS = 64
 };
 
@@ -190,7 +191,8 @@ int launch_depth_pass(uint32_t* const keys[2], uint32_t* const vals[2], uint32_t
 int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
                 uint32_t* status, uint32_t* ticket, cudaStream_t s);
 int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
-                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, cudaStream_t s);
+                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, int mlp_writes_rows,
+                  cudaStream_t s);
 int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_vals,
                         const GeomBuffers& gb, uint32_t cap, uint64_t* keys_out, uint32_t* vals_out,
                         cudaStream_t s);
@@ -199,7 +201,13 @@ int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, fl
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
                const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
                float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
-               cudaStream_t s);
+               const uint32_t* rows, const uint32_t* row_count, int64_t* rows_out, cudaStream_t s);
+// visibility pre-pass of a light sweep and its compaction
+int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_vals,
+                        uint8_t* contrib, cudaStream_t s);
+int raster_reads_unblended_rows(int tiles);
+int launch_compact_contrib(const uint8_t* contrib, int64_t n, uint32_t* rows, uint32_t* count,
+                           int zero_rest, float4* out0, float4* out1, int lights, cudaStream_t s);
 int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,
                               float4* out_internal, cudaStream_t s);
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,

@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(256)
 ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ counters,
               uint32_t cap, int tiles, uint2* __restrict__ ranges, uint2* __restrict__ ranges_user,
               uint32_t* __restrict__ lb, uint32_t* __restrict__ tile_order,
-              int64_t* __restrict__ counters_out) {
+              int64_t* __restrict__ counters_out, int mlp_writes_rows) {
   __shared__ uint32_t s_cnt[32], s_start[32];
   __shared__ bool s_last;
   pdl_prologue();
@@ -203,7 +203,8 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
     if (threadIdx.x == SSSGS_CNT_INSTANCES) v = counters[DC_INSTANCES];
     if (threadIdx.x == SSSGS_CNT_OVERFLOW) v = counters[DC_OVERFLOW];
     if (threadIdx.x == SSSGS_CNT_SORT_ERROR) v = counters[DC_SORT_ERROR];
-    counters_out[threadIdx.x] = v;
+    // SSSGS_CNT_MLP_ROWS is written by the MLP kernel (possibly before this kernel runs)
+    if (threadIdx.x != SSSGS_CNT_MLP_ROWS || !mlp_writes_rows) counters_out[threadIdx.x] = v;
   }
   __syncthreads();
   for (int t = threadIdx.x; t < tiles; t += 256) {
@@ -239,7 +240,49 @@ export_lists_kernel(const uint32_t* __restrict__ sorted_tiles, const uint32_t* _
   }
 }
 
+// Compaction of the visibility pre-pass: indices of the Gaussians with contrib[g] != 0, in
+// blocks (order inside a block ascending; blocks in arrival order -- the order only decides which
+// MLP tile a row lands in, never a result).  With zero_rest, the MLP-output rows of the other
+// Gaussians are zero-filled in both output buffers (see raster_reads_unblended_rows).
+__global__ void __launch_bounds__(256)
+compact_contrib_kernel(const uint8_t* __restrict__ contrib, uint32_t n, uint32_t* __restrict__ rows,
+                       uint32_t* __restrict__ count, int zero_rest, float4* __restrict__ out0,
+                       float4* __restrict__ out1, int lights) {
+  __shared__ uint32_t s_w[8], s_base;
+  pdl_prologue();
+  const uint32_t g = blockIdx.x * 256u + threadIdx.x;
+  const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const bool on = g < n && contrib[g] != 0;
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, on);
+  if (lane == 0) s_w[warp] = __popc(m);
+  __syncthreads();
+  uint32_t before = 0, total = 0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    if ((unsigned)w < warp) before += s_w[w];
+    total += s_w[w];
+  }
+  if (threadIdx.x == 0) s_base = total ? atomicAdd(count, total) : 0u;
+  __syncthreads();
+  if (on) rows[s_base + before + __popc(m & ((1u << lane) - 1u))] = g;
+  if (zero_rest && g < n && !on) {
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int l = 0; l < lights; ++l) {
+      out0[(size_t)g * lights + l] = z;
+      out1[(size_t)g * lights + l] = z;
+    }
+  }
+}
+
 }  // namespace
+
+int launch_compact_contrib(const uint8_t* contrib, int64_t n, uint32_t* rows, uint32_t* count,
+                           int zero_rest, float4* out0, float4* out1, int lights, cudaStream_t s) {
+  if (n == 0) return 0;
+  launch_pdl(compact_contrib_kernel, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, s, contrib, (uint32_t)n,
+             rows, count, zero_rest, out0, out1, lights);
+  return 1;
+}
 
 int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t cap, int tile_shift0, int tile_bits0, int tile_shift1, int tile_bits1,
                 uint32_t* status, uint32_t* ticket, cudaStream_t s) {
@@ -254,12 +297,13 @@ int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t
 }
 
 int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const GeomBuffers& gb,
-                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, cudaStream_t s) {
+                  uint32_t cap, uint2* ranges_user, int64_t* counters_out, int mlp_writes_rows,
+                  cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   int64_t blocks = ((int64_t)cap + 1 + 1023) / 1024;
   if (blocks > 148 * 4) blocks = 148 * 4;
   launch_pdl(ranges_kernel, dim3((unsigned)blocks), dim3(256), 0, s, sorted_tiles, gb.counters, cap, tiles, gb.ranges,
-                                                 ranges_user, gb.tile_slot, gb.tile_order, counters_out);
+                                                 ranges_user, gb.tile_slot, gb.tile_order, counters_out, mlp_writes_rows);
   return 1;
 }
 

@@ -194,6 +194,9 @@ struct MlpArgs {
   int slot_cols;               // TMEM columns per slot: accumulator D (then the A operand, TS mode)
   int a_col;                   // TS mode: column offset of the A operand inside a slot
   int a_bytes;                 // SS mode: bytes of one slot's A tile in shared memory
+  const uint32_t* rows;        // optional: evaluate only the Gaussians rows[0 .. *row_count)
+  const uint32_t* row_count;
+  int64_t* rows_out;           // optional: receives the number of rows evaluated (SSSGS_CNT_MLP_ROWS)
   MlpPlan plan;
 };
 
@@ -511,7 +514,9 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
 
   pdl_prologue();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int64_t n_units = (a.n + kRows - 1) / kRows;
+  const int64_t n_rows = a.rows ? (int64_t)*a.row_count : a.n;
+  const int64_t n_units = (n_rows + kRows - 1) / kRows;
+  if (a.rows_out && blockIdx.x == 0 && threadIdx.x == 0) *a.rows_out = n_rows;
 
   // ---- prologue: weights + biases to smem, barriers, TMEM -------------------------------------
   for (int i = tid * 16; i < plan.blob_bytes; i += blockDim.x * 16)
@@ -609,9 +614,10 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
     const int c_end = (WPS == 8 && half == 0) ? c_split : nchunks;
     uint32_t pd = 0;
     for (int64_t u = (int64_t)slot * gridDim.x + blockIdx.x; u < n_units; u += (int64_t)S * gridDim.x) {
-      const int64_t g_raw = u * kRows + r;
-      const bool row_ok = g_raw < a.n;
-      const int64_t g = row_ok ? g_raw : a.n - 1;
+      const int64_t row = u * kRows + r;
+      const bool row_ok = row < n_rows;
+      const int64_t row_c = row_ok ? row : n_rows - 1;
+      const int64_t g = a.rows ? (int64_t)a.rows[row_c] : row_c;
       uint4 keep[kKeepChunks];
       float mu[3], wout[3];
       assemble_static(a, g, c_begin, c_end, keep, mu, wout);
@@ -724,7 +730,7 @@ int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, fl
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
                const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
                float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
-               cudaStream_t s) {
+               const uint32_t* rows, const uint32_t* row_count, int64_t* rows_out, cudaStream_t s) {
   if (g.n == 0 || n_lights == 0) return 0;
   MlpArgs a;
   a.n = g.n;
@@ -737,6 +743,7 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
   a.blob = blob; a.bias = bias;
   a.out_internal = out_internal; a.out_user = out_user; a.user_light_stride = user_light_stride;
   a.plan = plan;
+  a.rows = rows; a.row_count = row_count; a.rows_out = rows_out;
   const MlpShape sh = mlp_shape(plan);
   a.slots = sh.slots; a.wps = sh.wps; a.slot_cols = sh.slot_cols; a.a_col = sh.a_col; a.a_bytes = sh.a_bytes;
   const int smem = mlp_smem_bytes(plan);

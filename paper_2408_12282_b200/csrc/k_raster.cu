@@ -17,6 +17,7 @@
 #include <cuda_fp16.h>
 
 #include <cstdlib>
+#include <cstring>
 
 #include "internal.cuh"
 
@@ -139,7 +140,11 @@ struct RasterShape {
   static_assert(RH >= PH && RH <= kTile && (RW % PW) == 0 && (RH % PH) == 0, "bad raster shape");
 };
 
-template <int LB, int E, int WARPS, int U>
+// MARK = true is the visibility pre-pass of a light sweep: the same walk (same culling, alphas,
+// transmittance chain and stop rule, hence the same set of blended entries) without channels,
+// shading or outputs; it sets contrib[g] = 1 for every Gaussian that is blended at some pixel.  The
+// MLP of the sweep then only evaluates those Gaussians (the others are never read by a blend).
+template <int LB, int E, int WARPS, int U, bool MARK>
 __global__ void __launch_bounds__(WARPS * 32)
 raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
@@ -148,16 +153,18 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
-                    int64_t frame_stride_px) {
+                    int64_t frame_stride_px, uint8_t* __restrict__ contrib) {
   using S = RasterShape<E, WARPS>;
   constexpr int P = S::P, THREADS = S::THREADS;
-  constexpr int NC = 5 + LB;  // float4 components per list entry
+  constexpr int NC = MARK ? 2 : 5 + LB;  // float4 components per list entry
   constexpr unsigned FULL = 0xFFFFFFFFu;
   extern __shared__ float4 s_dyn[];
   // two stages of component-major entry data, two stages of entry ids, one hit queue per warp
   float4 (*s_c)[NC][kBatch] = reinterpret_cast<float4 (*)[NC][kBatch]>(s_dyn);
   uint32_t (*s_id)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + 2 * NC * kBatch);
   uint8_t (*s_q)[kBatch] = reinterpret_cast<uint8_t (*)[kBatch]>(s_id + 2);
+  // MARK: Gaussian ids of the two staged batches (s_id is recycled two batches ahead)
+  uint32_t (*s_gid)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_q + WARPS);
 
   pdl_prologue();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -194,8 +201,10 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
       if (e < cnt) {
         const uint32_t g = s_id[st][e];
         const float4* src;
-        if (comp == 0) src = rec_a + g;
-        else if (comp == 1) src = rec_b + g;
+        if (comp == 0) {
+          src = rec_a + g;
+          if (MARK) s_gid[st][e] = g;
+        } else if (comp == 1) src = rec_b + g;
         else if (comp < 5) src = attr + 3 * (size_t)g + (comp - 2);
         else src = mlp_out + (size_t)g * n_lights + min(comp - 5, n_lights - 1);
         cp_async16(&s_c[st][comp][e], src);
@@ -300,7 +309,9 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
           T = Tk;
           w = alpha[u] * myT;
         }
-        if (__any_sync(FULL, w > 0.f)) {
+        if (MARK) {
+          if (w > 0.f) contrib[s_gid[st][j[u]]] = 1;
+        } else if (__any_sync(FULL, w > 0.f)) {
           const int jj = j[u];
           const float4 a0 = s_c[st][2][jj], a1 = s_c[st][3][jj], a2 = s_c[st][4][jj];
           acc[0] = fmaf(w, zed[u], acc[0]);
@@ -328,6 +339,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     }
   }
   cp_async_wait_all();
+  if (MARK) return;
 
   // ---- combine the E per-slot partial sums of every pixel (all E lanes end up with the total) ----
   if (E > 1) {
@@ -411,23 +423,24 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
 }
 
 // Launches one rasteriser variant: LB lights per walk, E entry slots per warp, WARPS warps per CTA.
-template <int LB, int E, int WARPS, int U>
+template <int LB, int E, int WARPS, int U, bool MARK = false>
 static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_lights,
                           const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                           const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                          int64_t frame_stride_px, int tiles, cudaStream_t s) {
+                          int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr) {
   using S = RasterShape<E, WARPS>;
-  constexpr int smem = 2 * (5 + LB) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch;
+  constexpr int smem = 2 * (MARK ? 2 : 5 + LB) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch +
+                       (MARK ? 2 * kBatch * 4 : 0);
   static bool configured = false;
   if (!configured) {
-    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U>,
+    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U, MARK>,
                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
       return -1;
     configured = true;
   }
-  launch_pdl(raster_shade_kernel<LB, E, WARPS, U>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam, lights,
-             n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
-             aov_d, aov_s, frame_stride_px);
+  launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
+             lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
+             aov_d, aov_s, frame_stride_px, contrib);
   return 1;
 }
 
@@ -471,6 +484,33 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   }
 #undef SSSGS_BY_LB
 #undef SSSGS_ARGS
+}
+
+// Visibility pre-pass of a light sweep (see raster_shade_kernel, MARK): same tile order and shape
+// choice as the render walks.
+int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_vals,
+                        uint8_t* contrib, cudaStream_t s) {
+  const int tiles = cam.tiles_x * cam.tiles_y;
+  if (tiles == 0) return 0;
+  LightBatch none;
+  memset(&none, 0, sizeof none);
+  int mode = raster_mode();
+  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
+  const int e = mode / (mode >= 100 ? 100 : 10);
+  if (e == 1)
+    return launch_variant<1, 1, 8, 4, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                            nullptr, 0, tiles, s, contrib);
+  return launch_variant<1, 4, 8, 2, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                          nullptr, 0, tiles, s, contrib);
+}
+
+// 1 when the render walks of an image of `tiles` tiles use more than one entry slot per warp: a
+// blend then also multiplies (by a zero weight) the MLP outputs of entries that contribute nowhere,
+// so those rows must hold finite values (the compaction kernel zero-fills them).
+int raster_reads_unblended_rows(int tiles) {
+  int mode = raster_mode();
+  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
+  return mode / (mode >= 100 ? 100 : 10) != 1;
 }
 
 }  // namespace sssgs

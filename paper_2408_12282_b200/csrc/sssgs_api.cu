@@ -30,7 +30,9 @@ struct sssgs_ctx {
   uint32_t* status_emit = nullptr;
   float4* mlp_out[2] = {};     // double-buffered: the MLP of batch k+1 overlaps the raster of batch k
   cudaStream_t side = nullptr; // the MLP runs here, concurrently with the geometry stages
-  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_mlp[2] = {}, ev_raster[2] = {};
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_mlp[2] = {}, ev_raster[2] = {}, ev_mask = nullptr;
+  uint8_t* contrib = nullptr;   // [n] visibility pre-pass flags (inside the control block)
+  uint32_t* rows = nullptr;     // [n] Gaussians kept by the pre-pass
   uint8_t* mlp_blob = nullptr;
   float* mlp_bias = nullptr;
   int64_t launches = 0;
@@ -103,6 +105,7 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   p = take(tiles * 4); if (c) c->gb.tile_order = (uint32_t*)p;
   p = take((tiles + 1) * 4); if (c) c->gb.tile_slot = (uint32_t*)p;
   for (int k = 0; k < 2; ++k) { p = take(n * (size_t)lb * 16); if (c) c->mlp_out[k] = (float4*)p; }
+  p = take(n * 4); if (c) c->rows = (uint32_t*)p;
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
   p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
   // control block: everything that must be zero at the start of a camera
@@ -114,6 +117,7 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   for (int k = 0; k < 4; ++k) { p = take(nblk_d * kRadixMax * 4); if (c) c->status_depth[k] = (uint32_t*)p; }
   for (int k = 0; k < 2; ++k) { p = take(nblk_i * kRadixMax * 4); if (c) c->status_tile[k] = (uint32_t*)p; }
   p = take(((n + kEmitChunk - 1) / kEmitChunk) * 4); if (c) c->status_emit = (uint32_t*)p;
+  p = take(n); if (c) c->contrib = p;
   if (c) c->control_bytes = off - ctrl_begin;
   return off;
 }
@@ -260,8 +264,18 @@ int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
     c->owns_ws = true;
   }
   carve(c, *cfg, c->ws);
+  // rows of the MLP output buffers that a sweep skips are still multiplied by zero weights in some
+  // rasteriser shapes: they must never hold non-finite bit patterns
+  const int lb0 = cfg->max_lights_per_pass ? cfg->max_lights_per_pass : 8;
+  if (cfg->max_gaussians > 0 &&
+      (cudaMemset(c->mlp_out[0], 0, (size_t)cfg->max_gaussians * lb0 * 16) != cudaSuccess ||
+       cudaMemset(c->mlp_out[1], 0, (size_t)cfg->max_gaussians * lb0 * 16) != cudaSuccess)) {
+    sssgs_destroy(c);
+    return fail(nullptr, SSSGS_ECUDA, "workspace initialisation failed");
+  }
   bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess;
-  cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_join, &c->ev_mlp[0], &c->ev_mlp[1], &c->ev_raster[0], &c->ev_raster[1]};
+  cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_join, &c->ev_mlp[0], &c->ev_mlp[1], &c->ev_raster[0], &c->ev_raster[1],
+                        &c->ev_mask};
   for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
   if (!ok) {
     sssgs_destroy(c);
@@ -277,7 +291,7 @@ void sssgs_destroy(sssgs_ctx* c) {
     if (s.first) cudaFree(s.first);
   for (auto& sp : c->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto& e : c->pool) cudaEventDestroy(e);
-  cudaEvent_t evs[] = {c->ev_fork, c->ev_join, c->ev_mlp[0], c->ev_mlp[1], c->ev_raster[0], c->ev_raster[1]};
+  cudaEvent_t evs[] = {c->ev_fork, c->ev_join, c->ev_mlp[0], c->ev_mlp[1], c->ev_raster[0], c->ev_raster[1], c->ev_mask};
   for (cudaEvent_t e : evs)
     if (e) cudaEventDestroy(e);
   if (c->side) cudaStreamDestroy(c->side);
@@ -387,6 +401,12 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   // the previous light batch).  With per-stage timing on, everything is serialised on `s` so that
   // each stage is timed alone.
   const bool overlap = run_mlp && !c->profile && g->n > 0 && n_light > 0 && n_cam > 0;
+  // MLP work avoidance in light sweeps: which Gaussians are ever blended depends on the view, not
+  // on the light.  A visibility pre-pass (the render walk without channels) flags them, and the
+  // MLP of every light of that view evaluates the flagged rows only -- the others are never read by
+  // a blend, so every output is unchanged.  Worth a pre-pass from 4 lights per view on; off when
+  // the caller wants the MLP outputs of all Gaussians.
+  const bool use_mask = run_mlp && g->n > 0 && n_light >= 4 && !out->mlp_out;
   cudaStream_t sm = overlap ? c->side : s;
   if (overlap) {
     if (cudaEventRecord(c->ev_fork, s) != cudaSuccess || cudaStreamWaitEvent(sm, c->ev_fork, 0) != cudaSuccess)
@@ -444,12 +464,22 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     begin(SSSGS_STAGE_RANGES);
     add(launch_ranges(sorted_tiles, cam, c->gb, cap,
                       out->tile_ranges ? (uint2*)(out->tile_ranges + (size_t)v * tiles * 2) : nullptr,
-                      out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr, s));
+                      out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS : nullptr,
+                      run_mlp && g->n > 0 && n_light > 0, s));
     if (out->sorted_keys || out->sorted_vals)
       add(launch_export_lists(sorted_tiles, sorted_vals, c->gb, cap,
                               out->sorted_keys ? out->sorted_keys + (size_t)v * cap : nullptr,
                               out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr, s));
     end();
+    if (use_mask) {
+      begin(SSSGS_STAGE_RASTER);
+      add(launch_mark_contrib(cam, c->gb, sorted_vals, c->contrib, s));
+      add(launch_compact_contrib(c->contrib, g->n, c->rows, cnt + DC_CONTRIB_ROWS, raster_reads_unblended_rows(tiles),
+                                 c->mlp_out[0], c->mlp_out[1], n_light < c->max_lb ? n_light : c->max_lb, s));
+      end();
+      if (overlap && (cudaEventRecord(c->ev_mask, s) != cudaSuccess || cudaStreamWaitEvent(sm, c->ev_mask, 0) != cudaSuccess))
+        return fail(c, SSSGS_ECUDA, "stream wait failed");
+    }
     // ---- per light batch: a1+a2 MLP, a7+a8 raster + shade -------------------------------------------
     for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
       const int nl = n_light - l0 < c->max_lb ? n_light - l0 : c->max_lb;
@@ -474,7 +504,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         // kernels keep the rest (estimates: ~35 % of the bf16 peak for the MLP, 60 us + 0.35 us per
         // 1000 Gaussians for the chain; measured on configs 2 and 4: -7 % per frame).
         int mlp_ctas = c->num_sms;
-        if (overlap && l0 == 0) {
+        if (overlap && l0 == 0 && !use_mask) {
           double flop_row = 0.0;
           for (int q = 0; q < plan.n_stages; ++q) flop_row += 2.0 * plan.st[q].k_pad * plan.st[q].n_pad;
           const double mlp_half_us = 20.0 + 2.0 * (double)g->n * nl * flop_row / 580e12 * 1e6;
@@ -483,7 +513,8 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         }
         const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, mlp_buf,
                                  out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
-                                 mlp_ctas, sm);
+                                 mlp_ctas, use_mask ? c->rows : nullptr, use_mask ? cnt + DC_CONTRIB_ROWS : nullptr,
+                                 out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_MLP_ROWS : nullptr, sm);
         if (k < 0) return fail(c, SSSGS_ECUDA, "MLP kernel configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
         add(k);
         if (overlap && (cudaEventRecord(c->ev_mlp[buf], sm) != cudaSuccess || cudaStreamWaitEvent(s, c->ev_mlp[buf], 0) != cudaSuccess))

@@ -35,6 +35,11 @@ def _render_full(scene):
         torch.cuda.synchronize()
         res = {k: v.cpu().numpy() for k, v in out.items()}
         res["launches"] = R.launch_count()
+        # the call bench.py times asks for RGB and counters only: in a sweep (>= 4 lights) the MLP then
+        # runs on the rows a visibility pre-pass keeps.  Same frames, bit for bit.
+        out = R.render(cams=scene.cameras[:1], lights=scene.lights[0], want=("rgb", "counters"))
+        torch.cuda.synchronize()
+        res["rgb_as_benchmarked"] = out["rgb"].cpu().numpy()
     finally:
         R.close()
     return res
@@ -63,6 +68,8 @@ def test_full_size_config(cfg, n_lights):
     scene = scenes.make_scene(cfg, views=1, lights=n_lights)
     cam = scene.cameras[0]
     gpu = _render_full(scene)
+
+    np.testing.assert_array_equal(gpu["rgb_as_benchmarked"].view(np.uint32), gpu["rgb"].view(np.uint32))
 
     # ---- lists, ranges, counters: full, bit-exact ------------------------------------------------
     proj = oracle.project(scene, cam)

@@ -194,6 +194,26 @@ def test_light_batching_is_consistent():
     np.testing.assert_allclose(a["rgb"], c["rgb"], rtol=2e-6, atol=1e-6)
 
 
+@pytest.mark.parametrize("width", [200, 656])   # 169 tiles -> 4 entry slots per warp; 1681 tiles -> 1
+def test_sweep_row_skipping_changes_nothing(width):
+    # From 4 lights per view on, a visibility pre-pass restricts the MLP to the Gaussians that are
+    # blended somewhere (unless the MLP outputs of all Gaussians are requested).  Frames must be
+    # bit-identical with and without it, and the skipped rows must really be skippable.
+    scene = scenes.make_scene(3, n=40000, width=width, height=width, lights=6)
+    on = gpu_render(scene, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters"), lights=scene.lights[0])
+    off = gpu_render(scene, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters", "mlp_out"),
+                     lights=scene.lights[0])
+    assert on["launches"] > off["launches"]          # pre-pass + compaction were launched
+    assert off["counters"][0][4] == scene.n
+    for k in ("rgb", "gbuffer", "aov_diffuse", "aov_specular"):
+        np.testing.assert_array_equal(on[k].view(np.uint32), off[k].view(np.uint32))
+    r = oracle.render_frame(scene, 0, 0, mlp_out=off["mlp_out"][0].astype(np.float64))
+    # the rows the pre-pass keeps are the Gaussians the oracle blends at some pixel (pixels whose
+    # skip / stop decisions sit within rounding of a threshold may add or drop a few)
+    kept, ref = int(on["counters"][0][4]), int(r.comp.contrib.sum())
+    assert 0 < kept < scene.n and abs(kept - ref) <= max(8, int(2e-3 * ref)), (kept, ref)
+
+
 def test_run_to_run_determinism():
     scene = scenes.make_scene(2, n=50000, width=320, height=240)
     a = gpu_render(scene)
