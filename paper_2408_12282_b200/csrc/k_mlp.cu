@@ -515,7 +515,16 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
   pdl_prologue();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int64_t n_rows = a.rows ? (int64_t)*a.row_count : a.n;
-  const int64_t n_units = (n_rows + kRows - 1) / kRows;
+  // A unit = 128 rows x a range of the batch's lights.  All lights when there are plenty of row
+  // blocks (the light-independent inputs are then assembled once per block); with few blocks the
+  // lights are split so that every slot of every CTA gets about 3 units or more.
+  const int64_t n_blocks = (n_rows + kRows - 1) / kRows;
+  int split = 1;
+  while (split < a.n_lights && n_blocks * split < 3ll * S * gridDim.x) split *= 2;
+  if (split > a.n_lights) split = a.n_lights;
+  const int lights_per_unit = (a.n_lights + split - 1) / split;
+  split = (a.n_lights + lights_per_unit - 1) / lights_per_unit;
+  const int64_t n_units = n_blocks * split;
   if (a.rows_out && blockIdx.x == 0 && threadIdx.x == 0) *a.rows_out = n_rows;
 
   // ---- prologue: weights + biases to smem, barriers, TMEM -------------------------------------
@@ -614,14 +623,16 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
     const int c_end = (WPS == 8 && half == 0) ? c_split : nchunks;
     uint32_t pd = 0;
     for (int64_t u = (int64_t)slot * gridDim.x + blockIdx.x; u < n_units; u += (int64_t)S * gridDim.x) {
-      const int64_t row = u * kRows + r;
+      const int64_t row = (u / split) * kRows + r;
+      const int light0 = (int)(u % split) * lights_per_unit;
+      const int light1 = min(a.n_lights, light0 + lights_per_unit);
       const bool row_ok = row < n_rows;
       const int64_t row_c = row_ok ? row : n_rows - 1;
       const int64_t g = a.rows ? (int64_t)a.rows[row_c] : row_c;
       uint4 keep[kKeepChunks];
       float mu[3], wout[3];
       assemble_static(a, g, c_begin, c_end, keep, mu, wout);
-      for (int light = 0; light < a.n_lights; ++light) {
+      for (int light = light0; light < light1; ++light) {
         uint4 lc = make_uint4(0u, 0u, 0u, 0u);
         if (c_begin == 0) lc = assemble_light(a, g, a.lights.l[light], mu, wout);
         write_row<TS>(a, g, ar, c_begin, c_end, keep, lc);
