@@ -91,7 +91,7 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
     // ---- 1. load + per-warp stable ranking ------------------------------------------------
     const uint32_t tile_base = t * TILE;
     const uint32_t tile_count = min(TILE, n - tile_base);
-    uint32_t key[ITEMS], val[ITEMS], rank[ITEMS];
+    uint32_t key[ITEMS], rank[ITEMS];
     unsigned peers[ITEMS];
     const uint32_t first = tile_base + warp * (32u * ITEMS) + lane;
 #pragma unroll
@@ -99,20 +99,25 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
       const uint32_t idx = first + 32u * i;
       const bool ok = idx < n;
       key[i] = ok ? keys_in[idx] : 0xFFFFFFFFu;
-      val[i] = ok ? (vals_in ? vals_in[idx] : idx) : 0u;
     }
     for (uint32_t d = lane; d < radix; d += 32) sm.wcnt[warp][d] = 0;
-    // the matches of all items are independent of each other: issue them back to back
+    // Short tickets (latency-bound small sorts): the matches of all items are independent of each
+    // other and are issued back to back.  Long tickets keep the match inside the loop: 15 more live
+    // registers would cost a resident CTA per SM, and large sorts are bandwidth-bound.
+    constexpr bool kHoist = ITEMS <= 7;
+    if (kHoist) {
 #pragma unroll
-    for (int i = 0; i < ITEMS; ++i) peers[i] = __match_any_sync(0xFFFFFFFFu, (key[i] >> shift) & mask);
+      for (int i = 0; i < ITEMS; ++i) peers[i] = __match_any_sync(0xFFFFFFFFu, (key[i] >> shift) & mask);
+    }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
       const uint32_t d = (key[i] >> shift) & mask;
-      const uint32_t r = __popc(peers[i] & ((1u << lane) - 1u));
+      const unsigned pe = kHoist ? peers[i] : __match_any_sync(0xFFFFFFFFu, d);
+      const uint32_t r = __popc(pe & ((1u << lane) - 1u));
       const uint32_t base = sm.wcnt[warp][d];
       __syncwarp();
-      if (r == 0) sm.wcnt[warp][d] = base + __popc(peers[i]);
+      if (r == 0) sm.wcnt[warp][d] = base + __popc(pe);
       __syncwarp();
       rank[i] = base + r;
     }
@@ -179,7 +184,9 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
       const uint32_t d = (key[i] >> shift) & mask;
       const uint32_t pos = sm.digstart[d] + sm.wcnt[warp][d] + rank[i];
       sm.keys[pos] = key[i];
-      sm.vals[pos] = val[i];
+      // the payload is only read here (fewer live registers while ranking): L2 serves it
+      const uint32_t idx = first + 32u * i;
+      sm.vals[pos] = idx < n ? (vals_in ? vals_in[idx] : idx) : 0u;
     }
     __syncthreads();
     for (uint32_t j = tid; j < tile_count; j += kSortThreads) {
@@ -194,7 +201,7 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
 // depth_pass >= 0: pass `depth_pass` of the 4-pass depth sort over the ping-pong buffers
 // (k0,v0) <-> (k1,v1); `hist` then points at all four histograms and trivial passes are skipped.
 // depth_pass < 0: a plain pass from (k0,v0) to (k1,v1) with its own histogram.
-__global__ void __launch_bounds__(kSortThreads)
+__global__ void __launch_bounds__(kSortThreads, 3)
 radix_pass_kernel(uint32_t* __restrict__ k0, uint32_t* __restrict__ v0, uint32_t* __restrict__ k1,
                   uint32_t* __restrict__ v1, const uint32_t* __restrict__ count_ptr,
                   uint32_t count_cap, int shift, int bits, const uint32_t* __restrict__ hist,
