@@ -31,6 +31,11 @@ struct sssgs_ctx {
   float4* mlp_out[2] = {};     // double-buffered: the MLP of batch k+1 overlaps the raster of batch k
   cudaStream_t side = nullptr; // the MLP runs here, concurrently with the geometry stages
   cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_mlp[2] = {}, ev_raster[2] = {}, ev_mask = nullptr;
+  // sssgs_render_host: the arrays the geometry chain does not need are uploaded on `copy`; the
+  // next sssgs_render makes its MLP / attribute work (or, without overlap, everything) wait for them
+  cudaStream_t copy = nullptr;
+  cudaEvent_t ev_upload = nullptr;
+  bool upload_pending = false;
   uint8_t* contrib = nullptr;   // [n] visibility pre-pass flags (inside the control block)
   uint32_t* rows = nullptr;     // [n] Gaussians kept by the pre-pass
   uint8_t* mlp_blob = nullptr;
@@ -273,9 +278,10 @@ int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
     sssgs_destroy(c);
     return fail(nullptr, SSSGS_ECUDA, "workspace initialisation failed");
   }
-  bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess;
+  bool ok = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&c->copy, cudaStreamNonBlocking) == cudaSuccess;
   cudaEvent_t* evs[] = {&c->ev_fork, &c->ev_join, &c->ev_mlp[0], &c->ev_mlp[1], &c->ev_raster[0], &c->ev_raster[1],
-                        &c->ev_mask};
+                        &c->ev_mask, &c->ev_upload};
   for (cudaEvent_t* e : evs) ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
   if (!ok) {
     sssgs_destroy(c);
@@ -291,10 +297,12 @@ void sssgs_destroy(sssgs_ctx* c) {
     if (s.first) cudaFree(s.first);
   for (auto& sp : c->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
   for (auto& e : c->pool) cudaEventDestroy(e);
-  cudaEvent_t evs[] = {c->ev_fork, c->ev_join, c->ev_mlp[0], c->ev_mlp[1], c->ev_raster[0], c->ev_raster[1], c->ev_mask};
+  cudaEvent_t evs[] = {c->ev_fork, c->ev_join, c->ev_mlp[0], c->ev_mlp[1], c->ev_raster[0], c->ev_raster[1], c->ev_mask,
+                       c->ev_upload};
   for (cudaEvent_t e : evs)
     if (e) cudaEventDestroy(e);
   if (c->side) cudaStreamDestroy(c->side);
+  if (c->copy) cudaStreamDestroy(c->copy);
   if (c->owns_ws && c->ws) cudaFree(c->ws);
   delete c;
 }
@@ -413,6 +421,10 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       return fail(c, SSSGS_ECUDA, "stream fork failed");
   }
 
+  if (c->upload_pending) {  // set by sssgs_render_host: late uploads gate the MLP / attribute work
+    c->upload_pending = false;
+    if (cudaStreamWaitEvent(sm, c->ev_upload, 0) != cudaSuccess) return fail(c, SSSGS_ECUDA, "stream wait failed");
+  }
   begin(SSSGS_STAGE_PACK);
   if (add(launch_pack_attr(*g, c->attr, sm)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
   if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, sm));
@@ -581,10 +593,14 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   const size_t ncoef = (size_t)(g->vis_sh_degree + 1) * (g->vis_sh_degree + 1);
   size_t idx = 0;
   bool ok = true;
+  // What projection / sort / binning read goes up first, on the stream the render runs on; the
+  // rest (what only the MLP and the attribute packing read) goes up on the context's copy stream,
+  // so that the geometry chain runs under the second part of the upload.
+  cudaStream_t up_stream = s;
   auto up = [&](const void* host, size_t bytes) -> void* {
     void* d = stage_buf(c, idx++, bytes);
     if (!d) { ok = false; return nullptr; }
-    if (host && bytes && cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) ok = false;
+    if (host && bytes && cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, up_stream) != cudaSuccess) ok = false;
     return d;
   };
   sssgs_gaussians dg = *g;
@@ -592,6 +608,8 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   dg.scales = (const float*)up(g->scales, n * 12);
   dg.rotations = (const float*)up(g->rotations, n * 16);
   dg.opacities = (const float*)up(g->opacities, n * 4);
+  const bool split = mlp->precomputed_out == nullptr && n > 0 && n_light > 0 && n_cam > 0;
+  if (split) up_stream = c->copy;
   dg.normals = (const float*)up(g->normals, n * 12);
   dg.base_color = (const float*)up(g->base_color, n * 12);
   dg.roughness = (const float*)up(g->roughness, n * 4);
@@ -604,6 +622,10 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   const size_t frames = (size_t)n_cam * n_light;
   dm.precomputed_out = mlp->precomputed_out ? (const float*)up(mlp->precomputed_out, frames * n * 16) : nullptr;
   if (!mlp->precomputed_out) idx++;
+  if (split) {
+    if (cudaEventRecord(c->ev_upload, c->copy) != cudaSuccess) ok = false;
+    c->upload_pending = true;
+  }
 
   size_t npix = 0, tiles = 0;  // all cameras of one call share the frame size of the first
   if (n_cam > 0 && cams) {
