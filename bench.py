@@ -209,7 +209,7 @@ def run_gpu(args, rank, world, local_rank):
         sampler.start()
     # ---- warm-up (un-captured), then capture one step into a CUDA graph -------------------------
     for _ in range(2):
-        R.render(cams=cams, lights=lights, outputs=outs)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
     torch.cuda.synchronize()
     cnt = outs["counters"][0].tolist()
     if cnt[binding.CNT_OVERFLOW] or cnt[binding.CNT_SORT_ERROR]:
@@ -217,7 +217,7 @@ def run_gpu(args, rank, world, local_rank):
     launches_per_step = R.launch_count()
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.graph(graph):
-        R.render(cams=cams, lights=lights, outputs=outs)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
@@ -249,7 +249,7 @@ def run_gpu(args, rank, world, local_rank):
     acc, nlaunch = None, None
     for _ in range(args.steps):
         flush.zero_()
-        R.render(cams=cams, lights=lights, outputs=outs)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
         ms, nlaunch = binding.sssgs_profile_read(R.ctx)
         acc = ms if acc is None else {k: acc[k] + ms[k] for k in ms}
     binding.sssgs_profile_enable(R.ctx, False)
@@ -313,7 +313,8 @@ def run_gpu(args, rank, world, local_rank):
             "config": {"workload": f"configs[{args.config - 1}] {scene.name}", "gaussians": scene.n,
                        "width": cam.width, "height": cam.height, "frames_per_step": fps,
                        "l2": "flushed between timed steps (256 MiB memset)", "launch": "CUDA graph replay",
-                       "instances": cnt[binding.CNT_INSTANCES], "mlp_rows_per_light": mlp_rows},
+                       "instances": cnt[binding.CNT_INSTANCES], "mlp_rows_per_light": mlp_rows,
+                       "sum_lights": bool(args.sum_lights)},
             "ms_per_frame": total_ms / args.steps / fps,
             "gaussians_per_s": world * args.steps * fps * scene.n / (total_ms * 1e-3),
             "clocks": clocks,
@@ -335,6 +336,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sum-lights", action="store_true",
+                    help="image-based-lighting mode (SSSGS_SUM_LIGHTS): the lights of a step are summed into one frame")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -52,8 +52,14 @@ enum { SSSGS_F32 = 0, SSSGS_BF16 = 1 };
 
 /* flags of sssgs_render */
 enum {
-  SSSGS_LIGHTS_PER_CAMERA = 1u /* lights is [n_cam][n_light] (camera c uses its own n_light
+  SSSGS_LIGHTS_PER_CAMERA = 1u,/* lights is [n_cam][n_light] (camera c uses its own n_light
                                   lights) instead of one shared [n_light] list            */
+  SSSGS_SUM_LIGHTS = 2u        /* image-based lighting as a sum of point lights (PAPER.md L301,
+                                  App. D): out.rgb holds ONE frame per camera, [n_cam][H][W][3] =
+                                  sum over the call's lights of intensity_l * A * L_out,l, plus the
+                                  background term (1 - A) bg once.  The sum is formed in the
+                                  rasteriser's epilogue (no per-light frames are written).
+                                  gbuffer / mlp_out stay per light; the AOVs must be NULL.    */
 };
 
 /* indices into sssgs_out.counters (int64 each, per camera: counters[cam*SSSGS_NCOUNTERS + k]) */

@@ -213,7 +213,9 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                   const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                  int64_t frame_stride_px, cudaStream_t s);
+                  int64_t frame_stride_px, int sum_mode, cudaStream_t s);
+// sum_mode: 0 = one RGB frame per light; 1 = ONE frame = sum over the batch's lights + background
+// term (first batch of a camera); 2 = add the batch's lights to the frame already there
 
 int mlp_smem_bytes(const MlpPlan& plan);
 

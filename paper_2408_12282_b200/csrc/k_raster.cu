@@ -36,7 +36,7 @@ struct ShadeIn {
 __device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3], float lin,
                                             float A, int px, int py, const CamParams& cam,
                                             const LightParams& lt, float rgb[3], float dif[3],
-                                            float spc[3]) {
+                                            float spc[3], bool with_bg = true) {
   // back-projection of the pixel at depth q.depth, camera -> world: x = R^T (x_c - t)
   const float xc0 = ((float)px - cam.cx) / cam.fx * q.depth - cam.t[0];
   const float xc1 = ((float)py - cam.cy) / cam.fy * q.depth - cam.t[1];
@@ -103,7 +103,7 @@ __device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const float lout = q.sss * lsss[c] + (1.f - q.sss) * brdf[c];
-    rgb[c] = lt.intensity[c] * A * lout + (1.f - A) * cam.bg[c];
+    rgb[c] = lt.intensity[c] * A * lout + (with_bg ? (1.f - A) * cam.bg[c] : 0.f);
   }
 }
 
@@ -153,7 +153,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
-                    int64_t frame_stride_px, uint8_t* __restrict__ contrib) {
+                    int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode) {
   using S = RasterShape<E, WARPS>;
   constexpr int P = S::P, THREADS = S::THREADS;
   constexpr int NC = MARK ? 2 : 5 + LB;  // float4 components per list entry
@@ -365,6 +365,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   q.depth = acc[0] * iA; q.nx = acc[1] * iA; q.ny = acc[2] * iA; q.nz = acc[3] * iA;
   q.br = acc[4] * iA; q.bg = acc[5] * iA; q.bb = acc[6] * iA;
   q.rough = acc[7] * iA; q.metal = acc[8] * iA; q.sss = acc[9] * iA;
+  float sum[3] = {0.f, 0.f, 0.f};  // SSSGS_SUM_LIGHTS: this lane's share of the sum over the lights
 #pragma unroll
   for (int l = 0; l < LB; ++l) {
     if (l >= n_lights) break;
@@ -380,9 +381,13 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
     if (covered) {
       const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
-      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc);
+      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc, sum_mode == 0);
     } else {
       rgb[0] = cam.bg[0]; rgb[1] = cam.bg[1]; rgb[2] = cam.bg[2];
+    }
+    if (sum_mode != 0) {
+      if (covered) { sum[0] += rgb[0]; sum[1] += rgb[1]; sum[2] += rgb[2]; }
+      continue;
     }
     if (rgb_out) {
       float* o = rgb_out + fp * 3;
@@ -395,6 +400,22 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     if (aovs_out) {
       float* o = aovs_out + fp * 3;
       o[0] = spc[0]; o[1] = spc[1]; o[2] = spc[2];
+    }
+  }
+  if (sum_mode != 0) {
+    // the lights were dealt to the E lanes of a pixel: add the shares (all lanes of the warp are
+    // still here: `inside` lanes only diverge below), then one lane per pixel writes
+    if (E > 1) {
+#pragma unroll
+      for (int o = P; o < 32; o <<= 1)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sum[c] += __shfl_xor_sync(__activemask(), sum[c], o);
+    }
+    if (slot == 0 && rgb_out) {
+      float* o = rgb_out + pidx * 3;
+      const float bgw = covered ? 1.f - A : 1.f;  // background term, once per pixel
+#pragma unroll
+      for (int c = 0; c < 3; ++c) o[c] = sum_mode == 1 ? sum[c] + bgw * cam.bg[c] : o[c] + sum[c];
     }
   }
 }
@@ -427,7 +448,8 @@ template <int LB, int E, int WARPS, int U, bool MARK = false>
 static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_lights,
                           const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                           const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                          int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr) {
+                          int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr,
+                          int sum_mode = 0) {
   using S = RasterShape<E, WARPS>;
   constexpr int smem = 2 * (MARK ? 2 : 5 + LB) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch +
                        (MARK ? 2 * kBatch * 4 : 0);
@@ -440,7 +462,7 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
   }
   launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
              lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
-             aov_d, aov_s, frame_stride_px, contrib);
+             aov_d, aov_s, frame_stride_px, contrib, sum_mode);
   return 1;
 }
 
@@ -458,7 +480,7 @@ static int raster_mode() {
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                   const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                  int64_t frame_stride_px, cudaStream_t s) {
+                  int64_t frame_stride_px, int sum_mode, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
   // Default shape: few tiles (small images) leave SMs idle behind the longest tile lists, so the
@@ -466,7 +488,7 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   // one-thread-per-pixel shape executes fewer instructions per blended pair (measured: DESIGN.md).
   int mode = raster_mode();
   if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
-#define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s
+#define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, nullptr, sum_mode
 #define SSSGS_BY_LB(E, W, U)                                                   \
   do {                                                                         \
     if (n_lights <= 1) return launch_variant<1, E, W, U>(SSSGS_ARGS);          \

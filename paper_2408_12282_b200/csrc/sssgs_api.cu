@@ -336,7 +336,10 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   if (!c) return SSSGS_EINVAL;
   if (!g || !mlp || !out || (n_cam > 0 && !cams) || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
   if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
-  if (flags & ~(uint32_t)SSSGS_LIGHTS_PER_CAMERA) return fail(c, SSSGS_EINVAL, "unknown flags");
+  if (flags & ~(uint32_t)(SSSGS_LIGHTS_PER_CAMERA | SSSGS_SUM_LIGHTS)) return fail(c, SSSGS_EINVAL, "unknown flags");
+  const bool sum_lights = (flags & SSSGS_SUM_LIGHTS) != 0;
+  if (sum_lights && (out->aov_diffuse || out->aov_specular))
+    return fail(c, SSSGS_EINVAL, "SSSGS_SUM_LIGHTS: the AOV outputs must be NULL");
   if (g->n < 0) return fail(c, SSSGS_EINVAL, "n < 0");
   if (g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n %lld > max_gaussians %lld", (long long)g->n, (long long)c->cfg.max_gaussians);
   if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(c, SSSGS_EINVAL, "vis_sh_degree must be 0 or 1");
@@ -541,10 +544,11 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       end();
       begin(SSSGS_STAGE_RASTER);
       add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf,
-                        out->rgb ? out->rgb + frame0 * npix * 3 : nullptr,
+                        out->rgb ? out->rgb + (sum_lights ? (int64_t)v : frame0) * npix * 3 : nullptr,
                         out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr,
                         out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr,
-                        out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix, s));
+                        out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix,
+                        sum_lights ? (l0 == 0 ? 1 : 2) : 0, s));
       end();
       if (overlap && cudaEventRecord(c->ev_raster[buf], s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "event record failed");
       ++batch_no;
@@ -646,7 +650,7 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
     return d;
   };
   sssgs_out dout;
-  dout.rgb = (float*)down(out->rgb, frames * npix * 12);
+  dout.rgb = (float*)down(out->rgb, ((flags & SSSGS_SUM_LIGHTS) ? (size_t)n_cam : frames) * npix * 12);
   dout.gbuffer = (float*)down(out->gbuffer, frames * npix * 64);
   dout.aov_diffuse = (float*)down(out->aov_diffuse, frames * npix * 12);
   dout.aov_specular = (float*)down(out->aov_specular, frames * npix * 12);

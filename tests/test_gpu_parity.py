@@ -214,6 +214,46 @@ def test_sweep_row_skipping_changes_nothing(width):
     assert 0 < kept < scene.n and abs(kept - ref) <= max(8, int(2e-3 * ref)), (kept, ref)
 
 
+@pytest.mark.parametrize("width,n_lights", [(96, 3), (128, 11), (656, 9)])
+def test_sum_lights_is_the_sum_of_the_frames(width, n_lights):
+    # SSSGS_SUM_LIGHTS (image-based lighting as a sum of point lights, App. D): one frame
+    # per camera = sum_l intensity_l A L_out,l + (1 - A) bg, formed in the rasteriser's epilogue.
+    import dataclasses
+    import torch
+    from paper_2408_12282_b200 import binding
+    scene = scenes.make_scene(3, n=30000, width=width, height=width, lights=n_lights)
+    rng = np.random.default_rng(5)
+    lights = [dataclasses.replace(l, intensity=rng.uniform(0.2, 1.5, 3).astype(np.float32)) for l in scene.lights[0]]
+    cam = dataclasses.replace(scene.cameras[0], bg=np.float32([0.3, 0.1, 0.2]))
+    R = binding.Renderer(scene)
+    try:
+        per = R.render(cams=[cam], lights=lights, want=("rgb", "gbuffer", "mlp_out"))
+        torch.cuda.synchronize()
+        per = {k: v.cpu().numpy() for k, v in per.items()}
+        tot = R.render(cams=[cam], lights=lights, want=("rgb",), sum_lights=True)
+        torch.cuda.synchronize()
+        tot = tot["rgb"].cpu().numpy()
+    finally:
+        R.close()
+    assert tot.shape == (1, width, width, 3)
+    A = per["gbuffer"][0][..., 14:15].astype(np.float64)
+    bg_term = (1.0 - np.where(A >= 1e-6, A, 0.0)) * cam.bg.astype(np.float64)
+    # every per-light frame carries the background term once: remove the extra copies
+    want = per["rgb"].astype(np.float64).sum(axis=0) - (n_lights - 1) * bg_term
+    np.testing.assert_allclose(tot[0], want, rtol=2e-5, atol=2e-5)
+    # and against the oracle: shading of the GPU's G-buffers, summed in float64
+    ref = np.zeros_like(want)
+    for l, lt in enumerate(lights):
+        ref += oracle.shade(cam, lt, per["gbuffer"][l].astype(np.float64))[0]
+    ref -= (n_lights - 1) * bg_term
+    rgb32 = np.zeros_like(want)
+    for l, lt in enumerate(lights):
+        rgb32 += oracle.shade(cam, lt, per["gbuffer"][l].astype(np.float64), f32=True)[0].astype(np.float64)
+    rgb32 -= (n_lights - 1) * bg_term
+    tol = np.maximum(1e-4 * np.maximum(1.0, np.abs(ref)), 4.0 * np.abs(rgb32 - ref) + 1e-5)
+    assert (np.abs(tot[0] - ref) <= tol).all()
+
+
 def test_run_to_run_determinism():
     scene = scenes.make_scene(2, n=50000, width=320, height=240)
     a = gpu_render(scene)
