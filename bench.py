@@ -209,7 +209,7 @@ def run_gpu(args, rank, world, local_rank):
         sampler.start()
     # ---- warm-up (un-captured), then capture one step into a CUDA graph -------------------------
     for _ in range(2):
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
     torch.cuda.synchronize()
     cnt = outs["counters"][0].tolist()
     if cnt[binding.CNT_OVERFLOW] or cnt[binding.CNT_SORT_ERROR]:
@@ -217,7 +217,7 @@ def run_gpu(args, rank, world, local_rank):
     launches_per_step = R.launch_count()
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.graph(graph):
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
@@ -249,7 +249,7 @@ def run_gpu(args, rank, world, local_rank):
     acc, nlaunch = None, None
     for _ in range(args.steps):
         flush.zero_()
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights)
+        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
         ms, nlaunch = binding.sssgs_profile_read(R.ctx)
         acc = ms if acc is None else {k: acc[k] + ms[k] for k in ms}
     binding.sssgs_profile_enable(R.ctx, False)
@@ -314,7 +314,7 @@ def run_gpu(args, rank, world, local_rank):
                        "width": cam.width, "height": cam.height, "frames_per_step": fps,
                        "l2": "flushed between timed steps (256 MiB memset)", "launch": "CUDA graph replay",
                        "instances": cnt[binding.CNT_INSTANCES], "mlp_rows_per_light": mlp_rows,
-                       "sum_lights": bool(args.sum_lights)},
+                       "sum_lights": bool(args.sum_lights), "forward_shading": bool(args.forward)},
             "ms_per_frame": total_ms / args.steps / fps,
             "gaussians_per_s": world * args.steps * fps * scene.n / (total_ms * 1e-3),
             "clocks": clocks,
@@ -336,6 +336,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--forward", action="store_true",
+                    help="the paper's 'w/o deferred' variant (SSSGS_FORWARD_SHADING): Eq. 7 per Gaussian, RGB composited")
     ap.add_argument("--sum-lights", action="store_true",
                     help="image-based-lighting mode (SSSGS_SUM_LIGHTS): the lights of a step are summed into one frame")
     args = ap.parse_args()

@@ -54,12 +54,18 @@ enum { SSSGS_F32 = 0, SSSGS_BF16 = 1 };
 enum {
   SSSGS_LIGHTS_PER_CAMERA = 1u,/* lights is [n_cam][n_light] (camera c uses its own n_light
                                   lights) instead of one shared [n_light] list            */
-  SSSGS_SUM_LIGHTS = 2u        /* image-based lighting as a sum of point lights (PAPER.md L301,
+  SSSGS_SUM_LIGHTS = 2u,       /* image-based lighting as a sum of point lights (PAPER.md L301,
                                   App. D): out.rgb holds ONE frame per camera, [n_cam][H][W][3] =
                                   sum over the call's lights of intensity_l * A * L_out,l, plus the
                                   background term (1 - A) bg once.  The sum is formed in the
                                   rasteriser's epilogue (no per-light frames are written).
                                   gbuffer / mlp_out stay per light; the AOVs must be NULL.    */
+  SSSGS_FORWARD_SHADING = 4u   /* the "w/o deferred" variant of the paper's ablation (PAPER.md L283
+                                  Tab. 2, Fig. 5): Eq. 7 is evaluated per Gaussian (at its
+                                  centre, with its own normal and material) and the RGB values are
+                                  composited (Eq. 3): out.rgb = sum_i T_i alpha_i c_i + (1 - A) bg.
+                                  gbuffer and the AOVs must be NULL; not combinable with
+                                  SSSGS_SUM_LIGHTS.                                            */
 };
 
 /* indices into sssgs_out.counters (int64 each, per camera: counters[cam*SSSGS_NCOUNTERS + k]) */

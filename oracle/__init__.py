@@ -225,3 +225,83 @@ def render_frame(scene, view: int = 0, light: int = 0, mlp_mode: int = 0, mlp_ou
     r.n_vis = int(r.proj.visible.sum())
     r.n_instances = int(r.keys.shape[0])
     return r
+
+
+# -------------------------------------------------------------------------------------------------
+# "w/o deferred" variant (Tab. 2 "w/o deferred", Fig. 5; L114 explains what the
+# deferred pipeline replaces): Eq. 7 is evaluated per Gaussian and the resulting RGB is splatted.
+# Written out in numpy, float64, independently of the C++ pixel shader (which pins it, see
+# tests/test_oracle_forward.py).
+# -------------------------------------------------------------------------------------------------
+def shade_gaussians(scene, cam, light, mlp_out) -> np.ndarray:
+    """c_i = intensity * L_out,i with Eq. 7 (L104-106) at the Gaussian's centre mu_i:
+        L_out = sss L_SSS + (1 - sss)(f_spec + f_diff) L_in (n . w_in),
+    w_in / w_out towards the light / the camera from mu_i, n and the material of the Gaussian itself,
+    BRDF of Eq. 4 (L76-80) with the readings S8 (Cook-Torrance with the 4, GGX D with alpha_r = r^2
+    floored at 1e-3, Schlick F, Smith-Schlick visibility, k = alpha_r / 2) and the guards of the
+    pixel shader (|n| < 1e-8 -> SSS term only; |l + v| < 1e-8 -> h = n; n.v floored at 1e-4).
+    mlp_out: [n, 4] (L_SSS rgb, L_in).  Returns [n, 3] float64."""
+    f8 = np.float64
+    mu = np.asarray(scene.means, f8)
+    nrm = np.asarray(scene.normals, f8)
+    b = np.asarray(scene.base_color, f8)
+    r = np.asarray(scene.roughness, f8)
+    m = np.asarray(scene.metallic, f8)
+    sss = np.asarray(scene.subsurface, f8)
+    mo = np.asarray(mlp_out, f8)
+    R = np.asarray(cam.R, f8).reshape(3, 3)
+    t = np.asarray(cam.t, f8)
+    p_cam = -R.T @ t
+    l = np.asarray(light.position, f8)[None, :] - mu
+    v = p_cam[None, :] - mu
+    l /= np.linalg.norm(l, axis=1, keepdims=True)
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    nn = np.linalg.norm(nrm, axis=1)
+    ok = nn >= 1e-8
+    n = nrm / np.where(ok, nn, 1.0)[:, None]
+    h = l + v
+    hl = np.linalg.norm(h, axis=1)
+    h = np.where((hl >= 1e-8)[:, None], h / np.where(hl >= 1e-8, hl, 1.0)[:, None], n)
+    dot = lambda a, c: np.sum(a * c, axis=1)  # noqa: E731
+    nl = np.maximum(0.0, dot(n, l))
+    nv = np.maximum(1e-4, dot(n, v))
+    nh = np.clip(dot(n, h), 0.0, 1.0)
+    vh = np.clip(dot(v, h), 0.0, 1.0)
+    ar = np.maximum(1e-3, r * r)
+    a2 = ar * ar
+    s2 = np.sum(np.cross(n, h) ** 2, axis=1)              # 1 - nh^2 without cancellation (S9)
+    D = a2 / (np.pi * np.maximum(1e-12, a2 * nh * nh + s2) ** 2)  # floor: n = -h exactly (see shade_impl)
+    k = 0.5 * ar
+    V = 1.0 / (4.0 * (nl * (1.0 - k) + k) * (nv * (1.0 - k) + k))
+    F0 = 0.04 * (1.0 - m)[:, None] + b * m[:, None]
+    F = F0 + (1.0 - F0) * ((1.0 - vh) ** 5)[:, None]
+    f_spec = (D * V)[:, None] * F
+    f_diff = (1.0 - m)[:, None] * b / np.pi
+    brdf = (f_spec + f_diff) * (mo[:, 3] * nl)[:, None]
+    brdf = np.where(ok[:, None], brdf, 0.0)
+    lout = sss[:, None] * mo[:, :3] + (1.0 - sss)[:, None] * brdf
+    return np.asarray(light.intensity, f8)[None, :] * lout
+
+
+def forward_frame(scene, view: int = 0, light: int = 0, mlp_mode: int = 0, mlp_out=None, geometry=None):
+    """Whole "w/o deferred" path for one (view, light): C = sum_i T_i alpha_i c_i + (1 - A) bg (Eq. 3)
+    with c_i from shade_gaussians.  The compositor is the one of the deferred path (the per-Gaussian
+    colour rides in channels 10-12)."""
+    cam = scene.cameras[view]
+    lt = scene.lights[view][light]
+    r = SimpleNamespace()
+    if geometry is None:
+        r.proj = project(scene, cam)
+        r.keys, r.vals, r.ranges = build_lists(r.proj)
+    else:
+        r.proj, r.keys, r.vals, r.ranges = geometry.proj, geometry.keys, geometry.vals, geometry.ranges
+    if mlp_out is None:
+        mlp_out = mlp_forward(mlp_inputs(scene, cam, lt.position), scene.mlp, mlp_mode)
+    r.mlp_out = np.asarray(mlp_out, np.float64)
+    r.colors = shade_gaussians(scene, cam, lt, r.mlp_out)
+    ch = np.zeros((int(scene.n), 14), np.float64)
+    ch[:, 10:13] = r.colors
+    r.comp = composite(scene, cam, r.proj, ch, r.vals, r.ranges)
+    A = r.comp.gbuf[..., 14:15]
+    r.rgb = r.comp.gbuf[..., 10:13] + (1.0 - A) * np.asarray(cam.bg, np.float64)
+    return r

@@ -601,7 +601,9 @@ static void shade_impl(int width, int height, const OrcCamera* cam, const float*
           const real cx = n[1] * h[2] - n[2] * h[1], cy = n[2] * h[0] - n[0] * h[2],
                      cz = n[0] * h[1] - n[1] * h[0];
           const real s2 = cx * cx + cy * cy + cz * cz;
-          const real dd = a2 * nh * nh + s2;
+          // >= a2 >= 1e-6 for any unit n, h with nh in [0,1]; the floor only catches n = -h exactly
+          // (nh clamped to 0 and |n x h| = 0), where D would be a2 / 0
+          const real dd = std::max((real)1e-12, a2 * nh * nh + s2);
           const real D = a2 / (pi * dd * dd);
           const real k = ar * (real)0.5;
           const real V = (real)1 / ((real)4 * (nl * ((real)1 - k) + k) * (nv * ((real)1 - k) + k));

@@ -25,6 +25,7 @@ SSSGS_MAX_TRUNK = 8
 SSSGS_MAX_INC_HIDDEN = 2
 SSSGS_LIGHTS_PER_CAMERA = 1
 SSSGS_SUM_LIGHTS = 2
+SSSGS_FORWARD_SHADING = 4
 SSSGS_F32, SSSGS_BF16 = 0, 1
 (SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
 CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3, 4
@@ -272,7 +273,7 @@ class Renderer:
         return {k: torch.zeros(shapes[k][0], dtype=shapes[k][1], device=self.device) for k in want}
 
     def render(self, cams=None, lights=None, want=("rgb",), outputs=None, precomputed=None,
-               lights_per_camera=False, stream=None, sum_lights=False):
+               lights_per_camera=False, stream=None, sum_lights=False, forward=False):
         """Enqueue one sssgs_render on the current torch stream.  cams: list of scene cameras;
         lights: list of lights (or list per camera with lights_per_camera).  Returns the dict of
         output tensors (device)."""
@@ -301,7 +302,8 @@ class Renderer:
         m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr)
         st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         sssgs_render(self.ctx, self.g, m, carr, n_cam, larr, n_light, o,
-                     (SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0) | (SSSGS_SUM_LIGHTS if sum_lights else 0), st)
+                     (SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0) | (SSSGS_SUM_LIGHTS if sum_lights else 0) |
+                     (SSSGS_FORWARD_SHADING if forward else 0), st)
         return outputs
 
     def launch_count(self) -> int:

@@ -202,6 +202,12 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
                const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
                float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
                const uint32_t* rows, const uint32_t* row_count, int64_t* rows_out, cudaStream_t s);
+// "w/o deferred" variant (Tab. 2): Eq. 7 per Gaussian, then RGB compositing
+int launch_shade_gaussians(int64_t n, int n_lights, const float* means, const float4* attr,
+                           const CamParams& cam, const LightBatch& lights, float4* io, cudaStream_t s);
+int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers& gb,
+                          const uint32_t* sorted_vals, const float4* shaded, float* rgb,
+                          int64_t frame_stride_px, cudaStream_t s);
 // visibility pre-pass of a light sweep and its compaction
 int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_vals,
                         uint8_t* contrib, cudaStream_t s);

@@ -32,19 +32,15 @@ struct ShadeIn {
   float depth, nx, ny, nz, br, bg, bb, rough, metal, sss;  // already divided by coverage A
 };
 
-// Deferred shading of one pixel for one light.  fp32 restatement of DESIGN.md "Shading".
-__device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3], float lin,
-                                            float A, int px, int py, const CamParams& cam,
+// Eq. 7 with the BRDF of Eq. 4 (L76-80) at the world-space point xw, for one
+// light: rgb = intensity * A * L_out (+ (1 - A) bg).  fp32 restatement of DESIGN.md "Shading".
+__device__ __forceinline__ void shade_point(const ShadeIn& q, const float lsss[3], float lin, float A,
+                                            const float xw[3], const CamParams& cam,
                                             const LightParams& lt, float rgb[3], float dif[3],
-                                            float spc[3], bool with_bg = true) {
-  // back-projection of the pixel at depth q.depth, camera -> world: x = R^T (x_c - t)
-  const float xc0 = ((float)px - cam.cx) / cam.fx * q.depth - cam.t[0];
-  const float xc1 = ((float)py - cam.cy) / cam.fy * q.depth - cam.t[1];
-  const float xc2 = q.depth - cam.t[2];
-  float xw[3], l[3], v[3];
+                                            float spc[3], bool with_bg) {
+  float l[3], v[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    xw[k] = cam.R[0 + k] * xc0 + cam.R[3 + k] * xc1 + cam.R[6 + k] * xc2;
     l[k] = lt.pos[k] - xw[k];
     v[k] = cam.pos[k] - xw[k];
   }
@@ -80,7 +76,7 @@ __device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3
     const float cx = n[1] * h[2] - n[2] * h[1], cy = n[2] * h[0] - n[0] * h[2],
                 cz = n[0] * h[1] - n[1] * h[0];
     const float s2 = cx * cx + cy * cy + cz * cz;
-    const float dd = a2 * nh * nh + s2;
+    const float dd = fmaxf(1e-12f, a2 * nh * nh + s2);  // floor: only n = -h exactly (DESIGN.md readings)
     const float D = a2 / (kPi * dd * dd);
     const float k = 0.5f * ar;
     const float V = 1.f / (4.f * (nl * (1.f - k) + k) * (nv * (1.f - k) + k));
@@ -105,6 +101,21 @@ __device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3
     const float lout = q.sss * lsss[c] + (1.f - q.sss) * brdf[c];
     rgb[c] = lt.intensity[c] * A * lout + (with_bg ? (1.f - A) * cam.bg[c] : 0.f);
   }
+}
+
+// Deferred shading of one pixel for one light (L114): the pixel is projected back to 3-D at its
+// composited depth, camera -> world: x = R^T (x_c - t).
+__device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3], float lin,
+                                            float A, int px, int py, const CamParams& cam,
+                                            const LightParams& lt, float rgb[3], float dif[3],
+                                            float spc[3], bool with_bg = true) {
+  const float xc0 = ((float)px - cam.cx) / cam.fx * q.depth - cam.t[0];
+  const float xc1 = ((float)py - cam.cy) / cam.fy * q.depth - cam.t[1];
+  const float xc2 = q.depth - cam.t[2];
+  float xw[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) xw[k] = cam.R[0 + k] * xc0 + cam.R[3 + k] * xc1 + cam.R[6 + k] * xc2;
+  shade_point(q, lsss, lin, A, xw, cam, lt, rgb, dif, spc, with_bg);
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -144,7 +155,10 @@ struct RasterShape {
 // transmittance chain and stop rule, hence the same set of blended entries) without channels,
 // shading or outputs; it sets contrib[g] = 1 for every Gaussian that is blended at some pixel.  The
 // MLP of the sweep then only evaluates those Gaussians (the others are never read by a blend).
-template <int LB, int E, int WARPS, int U, bool MARK>
+// FWD = true is the "w/o deferred" variant (Tab. 2, Fig. 5): Eq. 7 was evaluated
+// per Gaussian (shade_gaussians_kernel), the walk composites those RGB values per light (Eq. 3)
+// and the epilogue only adds the background: no G-buffer channels, no per-pixel shading.
+template <int LB, int E, int WARPS, int U, bool MARK, bool FWD = false>
 __global__ void __launch_bounds__(WARPS * 32)
 raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
@@ -156,7 +170,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode) {
   using S = RasterShape<E, WARPS>;
   constexpr int P = S::P, THREADS = S::THREADS;
-  constexpr int NC = MARK ? 2 : 5 + LB;  // float4 components per list entry
+  constexpr int NC = MARK ? 2 : (FWD ? 2 + LB : 5 + LB);  // float4 components per list entry
   constexpr unsigned FULL = 0xFFFFFFFFu;
   extern __shared__ float4 s_dyn[];
   // two stages of component-major entry data, two stages of entry ids, one hit queue per warp
@@ -205,6 +219,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
           src = rec_a + g;
           if (MARK) s_gid[st][e] = g;
         } else if (comp == 1) src = rec_b + g;
+        else if (FWD) src = mlp_out + (size_t)g * n_lights + min(comp - 2, n_lights - 1);
         else if (comp < 5) src = attr + 3 * (size_t)g + (comp - 2);
         else src = mlp_out + (size_t)g * n_lights + min(comp - 5, n_lights - 1);
         cp_async16(&s_c[st][comp][e], src);
@@ -311,6 +326,18 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
         }
         if (MARK) {
           if (w > 0.f) contrib[s_gid[st][j[u]]] = 1;
+        } else if (FWD) {
+          if (__any_sync(FULL, w > 0.f)) {
+            const int jj = j[u];
+#pragma unroll
+            for (int l = 0; l < LB; ++l) {
+              const float4 c = s_c[st][2 + l][jj];  // per-Gaussian shaded RGB for light l
+              accl[l][0] = fmaf(w, c.x, accl[l][0]);
+              accl[l][1] = fmaf(w, c.y, accl[l][1]);
+              accl[l][2] = fmaf(w, c.z, accl[l][2]);
+            }
+            A += w;
+          }
         } else if (__any_sync(FULL, w > 0.f)) {
           const int jj = j[u];
           const float4 a0 = s_c[st][2][jj], a1 = s_c[st][3][jj], a2 = s_c[st][4][jj];
@@ -359,6 +386,17 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   // ---- epilogue: G-buffer stores + deferred shading; lights and store quarters are dealt to the
   //      E lanes of a pixel round-robin ---------------------------------------------------------------
   const int64_t pidx = (int64_t)py * cam.width + px;
+  if (FWD) {  // C = sum_i T_i alpha_i c_i + (1 - A) bg  (Eq. 3), lights dealt to the E lanes of a pixel
+#pragma unroll
+    for (int l = 0; l < LB; ++l) {
+      if (l >= n_lights) break;
+      if (l % E != slot || !rgb_out) continue;
+      float* o = rgb_out + ((int64_t)l * frame_stride_px + pidx) * 3;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) o[c] = accl[l][c] + (1.f - A) * cam.bg[c];
+    }
+    return;
+  }
   ShadeIn q;
   const bool covered = A >= 1e-6f;
   const float iA = covered ? 1.f / A : 0.f;
@@ -444,23 +482,23 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
 }
 
 // Launches one rasteriser variant: LB lights per walk, E entry slots per warp, WARPS warps per CTA.
-template <int LB, int E, int WARPS, int U, bool MARK = false>
+template <int LB, int E, int WARPS, int U, bool MARK = false, bool FWD = false>
 static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_lights,
                           const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                           const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
                           int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr,
                           int sum_mode = 0) {
   using S = RasterShape<E, WARPS>;
-  constexpr int smem = 2 * (MARK ? 2 : 5 + LB) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch +
+  constexpr int smem = 2 * (MARK ? 2 : (FWD ? 2 + LB : 5 + LB)) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch +
                        (MARK ? 2 * kBatch * 4 : 0);
   static bool configured = false;
   if (!configured) {
-    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U, MARK>,
+    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>,
                              cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
       return -1;
     configured = true;
   }
-  launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
+  launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
              lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
              aov_d, aov_s, frame_stride_px, contrib, sum_mode);
   return 1;
@@ -506,6 +544,65 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   }
 #undef SSSGS_BY_LB
 #undef SSSGS_ARGS
+}
+
+int raster_reads_unblended_rows(int tiles);
+
+namespace {
+// "w/o deferred" variant, step 1: Eq. 7 per Gaussian, at the Gaussian's centre with the Gaussian's
+// own normal and material (Tab. 2: shading before rasterisation).  Replaces the MLP
+// outputs (L_SSS rgb, L_in) of row (g, l) in place by (intensity * L_out rgb, 0).
+__global__ void __launch_bounds__(256)
+shade_gaussians_kernel(int64_t n, int n_lights, const float* __restrict__ means,
+                       const float4* __restrict__ attr, CamParams cam, LightBatch lights,
+                       float4* __restrict__ io) {
+  pdl_prologue();
+  const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n * n_lights) return;
+  const int64_t g = i / n_lights;
+  const int l = (int)(i % n_lights);
+  const float4 a0 = attr[3 * g], a1 = attr[3 * g + 1], a2 = attr[3 * g + 2];
+  ShadeIn q;
+  q.depth = 0.f;
+  q.nx = a0.x; q.ny = a0.y; q.nz = a0.z; q.rough = a0.w;
+  q.br = a1.x; q.bg = a1.y; q.bb = a1.z; q.metal = a1.w;
+  q.sss = a2.x;
+  const float4 mo = io[i];
+  const float lsss[3] = {mo.x, mo.y, mo.z};
+  const float xw[3] = {means[3 * g], means[3 * g + 1], means[3 * g + 2]};
+  float rgb[3], dif[3], spc[3];
+  shade_point(q, lsss, mo.w, 1.f, xw, cam, lights.l[l], rgb, dif, spc, false);
+  io[i] = make_float4(rgb[0], rgb[1], rgb[2], 0.f);
+}
+}  // namespace
+
+int launch_shade_gaussians(int64_t n, int n_lights, const float* means, const float4* attr,
+                           const CamParams& cam, const LightBatch& lights, float4* io, cudaStream_t s) {
+  if (n == 0 || n_lights == 0) return 0;
+  const int64_t total = n * n_lights;
+  launch_pdl(shade_gaussians_kernel, dim3((unsigned)((total + 255) / 256)), dim3(256), 0, s, n, n_lights, means,
+             attr, cam, lights, io);
+  return 1;
+}
+
+// "w/o deferred" variant, step 2: composite the per-Gaussian RGB of every light of the batch.
+int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers& gb,
+                          const uint32_t* sorted_vals, const float4* shaded, float* rgb,
+                          int64_t frame_stride_px, cudaStream_t s) {
+  const int tiles = cam.tiles_x * cam.tiles_y;
+  if (tiles == 0) return 0;
+  LightBatch none;
+  memset(&none, 0, sizeof none);
+  const bool e1 = !raster_reads_unblended_rows(tiles);
+#define SSSGS_FWD(LB)                                                                                     \
+  return e1 ? launch_variant<LB, 1, 8, 4, false, true>(cam, none, n_lights, gb, sorted_vals, nullptr, shaded, rgb, \
+                                                       nullptr, nullptr, nullptr, frame_stride_px, tiles, s)      \
+            : launch_variant<LB, 4, 8, 2, false, true>(cam, none, n_lights, gb, sorted_vals, nullptr, shaded, rgb, \
+                                                       nullptr, nullptr, nullptr, frame_stride_px, tiles, s)
+  if (n_lights <= 1) SSSGS_FWD(1);
+  if (n_lights <= 4) SSSGS_FWD(4);
+  SSSGS_FWD(8);
+#undef SSSGS_FWD
 }
 
 // Visibility pre-pass of a light sweep (see raster_shade_kernel, MARK): same tile order and shape

@@ -336,7 +336,11 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   if (!c) return SSSGS_EINVAL;
   if (!g || !mlp || !out || (n_cam > 0 && !cams) || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
   if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
-  if (flags & ~(uint32_t)(SSSGS_LIGHTS_PER_CAMERA | SSSGS_SUM_LIGHTS)) return fail(c, SSSGS_EINVAL, "unknown flags");
+  if (flags & ~(uint32_t)(SSSGS_LIGHTS_PER_CAMERA | SSSGS_SUM_LIGHTS | SSSGS_FORWARD_SHADING))
+    return fail(c, SSSGS_EINVAL, "unknown flags");
+  const bool forward = (flags & SSSGS_FORWARD_SHADING) != 0;
+  if (forward && ((flags & SSSGS_SUM_LIGHTS) || out->gbuffer || out->aov_diffuse || out->aov_specular))
+    return fail(c, SSSGS_EINVAL, "SSSGS_FORWARD_SHADING: no gbuffer / AOV outputs, not with SSSGS_SUM_LIGHTS");
   const bool sum_lights = (flags & SSSGS_SUM_LIGHTS) != 0;
   if (sum_lights && (out->aov_diffuse || out->aov_specular))
     return fail(c, SSSGS_EINVAL, "SSSGS_SUM_LIGHTS: the AOV outputs must be NULL");
@@ -532,6 +536,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                                  out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_MLP_ROWS : nullptr, sm);
         if (k < 0) return fail(c, SSSGS_ECUDA, "MLP kernel configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
         add(k);
+        if (forward) add(launch_shade_gaussians(g->n, nl, g->means, c->attr, cam, lb, mlp_buf, sm));
         if (overlap && (cudaEventRecord(c->ev_mlp[buf], sm) != cudaSuccess || cudaStreamWaitEvent(s, c->ev_mlp[buf], 0) != cudaSuccess))
           return fail(c, SSSGS_ECUDA, "stream join failed");
       } else {
@@ -543,6 +548,11 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       }
       end();
       begin(SSSGS_STAGE_RASTER);
+      if (forward) {
+        if (!run_mlp) add(launch_shade_gaussians(g->n, nl, g->means, c->attr, cam, lb, mlp_buf, s));
+        add(launch_raster_forward(cam, nl, c->gb, sorted_vals, mlp_buf,
+                                  out->rgb ? out->rgb + frame0 * npix * 3 : nullptr, npix, s));
+      } else
       add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf,
                         out->rgb ? out->rgb + (sum_lights ? (int64_t)v : frame0) * npix * 3 : nullptr,
                         out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr,
