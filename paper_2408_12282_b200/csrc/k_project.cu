@@ -187,7 +187,7 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
 
 // Light- and view-independent channels packed as 3 x float4 per Gaussian so that the
 // rasteriser gathers them with 128-bit loads:
-//   a0 = (n.x, n.y, n.z, roughness)  a1 = (b.r, b.g, b.b, metallic)  a2 = (sss, 0, 0, 0)
+//   a0 = (n.x, n.y, n.z, roughness)  a1 = (b.r, b.g, b.b, metallic)  a2 = (sss, 1, 0, 0)
 __global__ void __launch_bounds__(256)
 pack_attr_kernel(int64_t n, const float* __restrict__ normals, const float* __restrict__ base,
                  const float* __restrict__ rough, const float* __restrict__ metal,
@@ -197,7 +197,7 @@ pack_attr_kernel(int64_t n, const float* __restrict__ normals, const float* __re
   if (i >= n) return;
   attr[3 * i + 0] = make_float4(normals[3 * i], normals[3 * i + 1], normals[3 * i + 2], rough[i]);
   attr[3 * i + 1] = make_float4(base[3 * i], base[3 * i + 1], base[3 * i + 2], metal[i]);
-  attr[3 * i + 2] = make_float4(sss[i], 0.f, 0.f, 0.f);
+  attr[3 * i + 2] = make_float4(sss[i], 1.f, 0.f, 0.f);  // the 1 accumulates the coverage A next to sss
 }
 
 }  // namespace

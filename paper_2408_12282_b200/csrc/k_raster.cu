@@ -128,6 +128,15 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// Packed fp32x2 arithmetic (sm_100 FFMA2): the walk is bound by instruction issue, and a blend is
+// a row of FMAs with one common factor w, so two accumulators ride in one 64-bit register pair.
+// Each half is an IEEE fma: results are bit-identical to scalar fmaf.
+typedef float2 f32x2;
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { lo = v.x; hi = v.y; }
+// acc += (w, w) * (b0, b1)
+__device__ __forceinline__ void fma2(f32x2& acc, f32x2 ww, float b0, float b1) {
+  acc = __ffma2_rn(ww, make_float2(b0, b1), acc);
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -198,14 +207,14 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
 
   const uint2 range = ranges[tile];
   float T = 1.f, A = 0.f;  // T is identical in the E lanes of a pixel; A is a per-lane partial sum
-  float acc[10];
-  float accl[LB][4];
+  // accumulators of the walk, two per register pair: (n.x, n.y) (n.z, rough) (b.r, b.g) (b.b, metal)
+  // (sss, A), per light (L_SSS.r, L_SSS.g) (L_SSS.b, L_in); the depth rides alone
+  float acc_depth = 0.f;
+  f32x2 pacc[5], paccl[LB][2];
 #pragma unroll
-  for (int c = 0; c < 10; ++c) acc[c] = 0.f;
+  for (int c = 0; c < 5; ++c) pacc[c] = make_float2(0.f, 0.f);
 #pragma unroll
-  for (int l = 0; l < LB; ++l)
-#pragma unroll
-    for (int c = 0; c < 4; ++c) accl[l][c] = 0.f;
+  for (int l = 0; l < LB; ++l) paccl[l][0] = paccl[l][1] = make_float2(0.f, 0.f);
   bool done = !inside;
 
   // gathers one batch of entries into stage `st` with 16-byte cp.async (all threads share the work)
@@ -329,37 +338,31 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
         } else if (FWD) {
           if (__any_sync(FULL, w > 0.f)) {
             const int jj = j[u];
+            const f32x2 ww = make_float2(w, w);
 #pragma unroll
             for (int l = 0; l < LB; ++l) {
-              const float4 c = s_c[st][2 + l][jj];  // per-Gaussian shaded RGB for light l
-              accl[l][0] = fmaf(w, c.x, accl[l][0]);
-              accl[l][1] = fmaf(w, c.y, accl[l][1]);
-              accl[l][2] = fmaf(w, c.z, accl[l][2]);
+              const float4 c = s_c[st][2 + l][jj];  // per-Gaussian shaded RGB for light l (w = 0)
+              fma2(paccl[l][0], ww, c.x, c.y);
+              fma2(paccl[l][1], ww, c.z, c.w);
             }
             A += w;
           }
         } else if (__any_sync(FULL, w > 0.f)) {
           const int jj = j[u];
           const float4 a0 = s_c[st][2][jj], a1 = s_c[st][3][jj], a2 = s_c[st][4][jj];
-          acc[0] = fmaf(w, zed[u], acc[0]);
-          acc[1] = fmaf(w, a0.x, acc[1]);
-          acc[2] = fmaf(w, a0.y, acc[2]);
-          acc[3] = fmaf(w, a0.z, acc[3]);
-          acc[4] = fmaf(w, a1.x, acc[4]);
-          acc[5] = fmaf(w, a1.y, acc[5]);
-          acc[6] = fmaf(w, a1.z, acc[6]);
-          acc[7] = fmaf(w, a0.w, acc[7]);
-          acc[8] = fmaf(w, a1.w, acc[8]);
-          acc[9] = fmaf(w, a2.x, acc[9]);
+          const f32x2 ww = make_float2(w, w);
+          acc_depth = fmaf(w, zed[u], acc_depth);
+          fma2(pacc[0], ww, a0.x, a0.y);
+          fma2(pacc[1], ww, a0.z, a0.w);
+          fma2(pacc[2], ww, a1.x, a1.y);
+          fma2(pacc[3], ww, a1.z, a1.w);
+          fma2(pacc[4], ww, a2.x, a2.y);  // a2 = (sss, 1, 0, 0): the second half is A += w
 #pragma unroll
           for (int l = 0; l < LB; ++l) {
             const float4 mo = s_c[st][5 + l][jj];
-            accl[l][0] = fmaf(w, mo.x, accl[l][0]);
-            accl[l][1] = fmaf(w, mo.y, accl[l][1]);
-            accl[l][2] = fmaf(w, mo.z, accl[l][2]);
-            accl[l][3] = fmaf(w, mo.w, accl[l][3]);
+            fma2(paccl[l][0], ww, mo.x, mo.y);
+            fma2(paccl[l][1], ww, mo.z, mo.w);
           }
-          A += w;
         }
       }
       if (__all_sync(FULL, done)) break;
@@ -367,6 +370,24 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   }
   cp_async_wait_all();
   if (MARK) return;
+
+  // unpack: acc[] in G-buffer channel order (depth, n3, b3, rough, metal, sss), accl[l] = MLP channels
+  float acc[10], accl[LB][4];
+  acc[0] = acc_depth;
+  unpack2(pacc[0], acc[1], acc[2]);
+  unpack2(pacc[1], acc[3], acc[7]);
+  unpack2(pacc[2], acc[4], acc[5]);
+  unpack2(pacc[3], acc[6], acc[8]);
+  {
+    float a_sum;
+    unpack2(pacc[4], acc[9], a_sum);
+    if (!FWD) A = a_sum;
+  }
+#pragma unroll
+  for (int l = 0; l < LB; ++l) {
+    unpack2(paccl[l][0], accl[l][0], accl[l][1]);
+    unpack2(paccl[l][1], accl[l][2], accl[l][3]);
+  }
 
   // ---- combine the E per-slot partial sums of every pixel (all E lanes end up with the total) ----
   if (E > 1) {
