@@ -26,6 +26,12 @@ namespace sssgs {
 namespace {
 
 constexpr int kBatch = 128;
+// stages of the staging ring and its shared-memory footprint, per kernel variant
+__host__ __device__ constexpr int raster_stages(int lb, bool mark, bool fwd) { return (!mark && lb > 4) ? 3 : 4; }
+__host__ __device__ constexpr int raster_comps(int lb, bool mark, bool fwd) { return mark ? 2 : (fwd ? 2 + lb : 5 + lb); }
+__host__ __device__ constexpr int raster_smem(int lb, bool mark, bool fwd, int warps) {
+  return raster_stages(lb, mark, fwd) * (raster_comps(lb, mark, fwd) * kBatch * 16 + kBatch * 4 + 16) + warps * kBatch + 16;
+}
 constexpr float kPi = 3.14159265358979323846f;
 
 struct ShadeIn {
@@ -137,7 +143,47 @@ __device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { lo = v.
 __device__ __forceinline__ void fma2(f32x2& acc, f32x2 ww, float b0, float b1) {
   acc = __ffma2_rn(ww, make_float2(b0, b1), acc);
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+// mbarriers of the staging ring
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(
+                   (uint32_t)__cvta_generic_to_shared(bar))
+               : "memory");
+}
+// this thread's arrival happens when all cp.async it has issued so far have landed
+__device__ __forceinline__ void mbar_arrive_on_copies(uint64_t* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(bar))
+               : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {  // non-blocking
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // Work decomposition of one rasteriser variant.  A warp covers P = 32/E pixels (a PW x PH block)
@@ -181,13 +227,17 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   constexpr int P = S::P, THREADS = S::THREADS;
   constexpr int NC = MARK ? 2 : (FWD ? 2 + LB : 5 + LB);  // float4 components per list entry
   constexpr unsigned FULL = 0xFFFFFFFFu;
+  constexpr int NS = raster_stages(LB, MARK, FWD);
   extern __shared__ float4 s_dyn[];
-  // two stages of component-major entry data, two stages of entry ids, one hit queue per warp
+  // a ring of NS stages of component-major entry data, the Gaussian ids of the staged entries (MARK),
+  // one hit queue per warp, and the ring's mbarriers: full[s] completes when every thread's copies of a
+  // batch have landed in stage s, empty[s] when every warp has finished reading it
   float4 (*s_c)[NC][kBatch] = reinterpret_cast<float4 (*)[NC][kBatch]>(s_dyn);
-  uint32_t (*s_id)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + 2 * NC * kBatch);
-  uint8_t (*s_q)[kBatch] = reinterpret_cast<uint8_t (*)[kBatch]>(s_id + 2);
-  // MARK: Gaussian ids of the two staged batches (s_id is recycled two batches ahead)
-  uint32_t (*s_gid)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_q + WARPS);
+  uint32_t (*s_gid)[kBatch] = reinterpret_cast<uint32_t (*)[kBatch]>(s_dyn + NS * NC * kBatch);
+  uint8_t (*s_q)[kBatch] = reinterpret_cast<uint8_t (*)[kBatch]>(s_gid + NS);
+  uint64_t* s_full = reinterpret_cast<uint64_t*>(s_q + WARPS);
+  uint64_t* s_empty = s_full + NS;
+  uint32_t* s_done = reinterpret_cast<uint32_t*>(s_empty + NS);  // warps whose pixels are all finished
 
   pdl_prologue();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -217,48 +267,83 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   for (int l = 0; l < LB; ++l) paccl[l][0] = paccl[l][1] = make_float2(0.f, 0.f);
   bool done = !inside;
 
-  // gathers one batch of entries into stage `st` with 16-byte cp.async (all threads share the work)
-  auto gather = [&](int st, int cnt) {
-    for (int q = tid; q < NC * kBatch; q += THREADS) {
-      const int comp = q / kBatch, e = q % kBatch;
-      if (e < cnt) {
-        const uint32_t g = s_id[st][e];
-        const float4* src;
-        if (comp == 0) {
-          src = rec_a + g;
-          if (MARK) s_gid[st][e] = g;
-        } else if (comp == 1) src = rec_b + g;
-        else if (FWD) src = mlp_out + (size_t)g * n_lights + min(comp - 2, n_lights - 1);
-        else if (comp < 5) src = attr + 3 * (size_t)g + (comp - 2);
-        else src = mlp_out + (size_t)g * n_lights + min(comp - 5, n_lights - 1);
-        cp_async16(&s_c[st][comp][e], src);
-      }
-    }
-    cp_async_commit();
-  };
-
   const uint32_t n_entries = range.y - range.x;
   const int n_batches = (int)((n_entries + kBatch - 1) / kBatch);
-  if (n_batches > 0) {
-    if (tid < kBatch && (uint32_t)tid < n_entries) s_id[0][tid] = sorted_vals[range.x + tid];
-    __syncthreads();
-    gather(0, (int)min((uint32_t)kBatch, n_entries));
-    if (n_batches > 1 && tid < kBatch && (uint32_t)(kBatch + tid) < n_entries)
-      s_id[1][tid] = sorted_vals[range.x + kBatch + tid];
-  }
-
-  for (int b = 0; b < n_batches; ++b) {
-    const int st = b & 1;
-    const int cnt = (int)min((uint32_t)kBatch, n_entries - (uint32_t)b * kBatch);
-    cp_async_wait_all();
-    // every thread's copies of batch b have landed; all warps have left batch b-1 (stage st^1)
-    if (__syncthreads_and(done)) break;
-    if (b + 1 < n_batches) {
-      gather(st ^ 1, (int)min((uint32_t)kBatch, n_entries - (uint32_t)(b + 1) * kBatch));
-      const uint32_t nxt = (uint32_t)(b + 2) * kBatch + tid;   // ids of batch b+2 reuse s_id[st]
-      if (tid < kBatch && nxt < n_entries) s_id[st][tid] = sorted_vals[range.x + nxt];
+  if (tid == 0) {
+    for (int st = 0; st < NS; ++st) {
+      mbar_init(s_full + st, THREADS);
+      mbar_init(s_empty + st, WARPS);
     }
-    if (__all_sync(FULL, done)) continue;  // this warp's pixel block is finished
+    *s_done = 0u;
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // ---- staging ring ---------------------------------------------------------------------------
+  // Batches of 128 list entries travel through a ring of NS shared-memory stages.  Every thread
+  // copies the same slice of every batch (entry tid % 128, components tid / 128, + THREADS / 128, ...)
+  // with cp.async and arrives on the stage's `full` barrier when its copies have landed; a warp
+  // arrives on `empty` when it has finished a stage.  A warp therefore only ever waits for data,
+  // or -- NS batches ahead of the slowest warp of the CTA -- for a free stage: warps whose pixel
+  // blocks see few entries run ahead instead of idling at a CTA-wide barrier per batch.
+  const int my_e = tid & (kBatch - 1);
+  int next_fill = 0;                       // next batch this thread has to copy its slice of
+  uint32_t next_gid = (uint32_t)my_e < n_entries ? sorted_vals[range.x + my_e] : 0u;
+  auto all_done = [&]() { return *reinterpret_cast<volatile uint32_t*>(s_done) >= (uint32_t)WARPS; };
+  // copies this thread's slice of batch next_fill if that batch's stage is free (blocking: wait for it);
+  // returns false if nothing was issued
+  auto fill = [&](bool blocking) -> bool {
+    const int g = next_fill;
+    if (g >= n_batches) return false;
+    const int st = g % NS;
+    if (g >= NS) {  // the stage still holds batch g - NS until every warp has released it
+      const uint32_t par = (uint32_t)((g / NS - 1) & 1);
+      if (!mbar_test(s_empty + st, par)) {
+        if (!blocking) return false;
+        while (!mbar_test(s_empty + st, par))
+          if (all_done()) return false;
+      }
+    }
+    if ((uint32_t)(g * kBatch + my_e) < n_entries) {
+      const uint32_t gid = next_gid;
+      for (int comp = tid / kBatch; comp < NC; comp += THREADS / kBatch) {
+        const float4* src;
+        if (comp == 0) src = rec_a + gid;
+        else if (comp == 1) src = rec_b + gid;
+        else if (FWD) src = mlp_out + (size_t)gid * n_lights + min(comp - 2, n_lights - 1);
+        else if (comp < 5) src = attr + 3 * (size_t)gid + (comp - 2);
+        else src = mlp_out + (size_t)gid * n_lights + min(comp - 5, n_lights - 1);
+        cp_async16(&s_c[st][comp][my_e], src);
+      }
+      if (MARK && tid < kBatch) cp_async4(&s_gid[st][my_e], sorted_vals + range.x + (size_t)g * kBatch + my_e);
+    }
+    mbar_arrive_on_copies(s_full + st);
+    ++next_fill;
+    const uint32_t nxt = (uint32_t)(next_fill * kBatch + my_e);
+    if (nxt < n_entries) next_gid = sorted_vals[range.x + nxt];
+    return true;
+  };
+
+  bool counted = false;  // this warp has been added to s_done
+  for (int b = 0; b < n_batches; ++b) {
+    const int st = b % NS;
+    const int cnt = (int)min((uint32_t)kBatch, n_entries - (uint32_t)b * kBatch);
+    bool alive = true;
+    while (next_fill <= b && alive) alive = fill(true);        // my slice of batch b itself
+    if (!alive) break;                                         // every warp of the CTA is finished
+    while (next_fill < b + NS && fill(false)) {                // and of the batches ahead, as stages free up
+    }
+    const bool warp_done = __all_sync(FULL, done);
+    if (warp_done) {
+      if (!counted) {
+        counted = true;
+        if (lane == 0) atomicAdd(s_done, 1u);
+      }
+      if (lane == 0) mbar_arrive(s_empty + st);                // releases the stage without reading it
+      if (all_done()) break;
+      continue;
+    }
+    mbar_wait(s_full + st, (uint32_t)((b / NS) & 1));          // every thread's copies of batch b have landed
 
     // ---- cull: lane <-> entry; queue the entries whose alpha >= 1/255 support box overlaps this
     //      warp's pixel block, in list order --------------------------------------------------------
@@ -367,6 +452,8 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
       }
       if (__all_sync(FULL, done)) break;
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(s_empty + st);
   }
   cp_async_wait_all();
   if (MARK) return;
@@ -510,8 +597,7 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
                           int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr,
                           int sum_mode = 0) {
   using S = RasterShape<E, WARPS>;
-  constexpr int smem = 2 * (MARK ? 2 : (FWD ? 2 + LB : 5 + LB)) * kBatch * 16 + 2 * kBatch * 4 + WARPS * kBatch +
-                       (MARK ? 2 * kBatch * 4 : 0);
+  constexpr int smem = raster_smem(LB, MARK, FWD, WARPS);
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>,
