@@ -629,10 +629,11 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
   // Default shape: few tiles (small images) leave SMs idle behind the longest tile lists, so the
-  // lists are walked by 4 CTAs with 4 entry slots per warp; with many tiles the classic
-  // one-thread-per-pixel shape executes fewer instructions per blended pair (measured: DESIGN.md).
+  // lists are walked by 2 CTAs per tile with 2 entry slots per warp (4x4-pixel blocks); with many
+  // tiles the classic one-thread-per-pixel shape executes fewer instructions per blended pair
+  // (measured: DESIGN.md).
   int mode = raster_mode();
-  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
+  if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
 #define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, nullptr, sum_mode
 #define SSSGS_BY_LB(E, W, U)                                                   \
   do {                                                                         \
@@ -721,7 +722,7 @@ int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint3
   LightBatch none;
   memset(&none, 0, sizeof none);
   int mode = raster_mode();
-  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
+  if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
   const int e = mode / (mode >= 100 ? 100 : 10);
   if (e == 1)
     return launch_variant<1, 1, 8, 4, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
@@ -735,7 +736,7 @@ int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint3
 // so those rows must hold finite values (the compaction kernel zero-fills them).
 int raster_reads_unblended_rows(int tiles) {
   int mode = raster_mode();
-  if (mode == 0) mode = tiles <= 1600 ? 48 : 18;
+  if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
   return mode / (mode >= 100 ? 100 : 10) != 1;
 }
 
