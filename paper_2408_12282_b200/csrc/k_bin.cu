@@ -288,7 +288,7 @@ int launch_emit(int64_t n, const CamParams& cam, const GeomBuffers& gb, uint32_t
                 uint32_t* status, uint32_t* ticket, cudaStream_t s) {
   if (n == 0) return 0;
   int64_t blocks = (n + kEmitChunk - 1) / kEmitChunk;
-  if (blocks > 148 * 4) blocks = 148 * 4;
+  if (blocks > 148 * 8) blocks = 148 * 8;  // 8 CTAs fit an SM: a chunk is a chain of dependent loads
   launch_pdl(emit_kernel, dim3((unsigned)blocks), dim3(kEmitThreads), 0, s,
       (uint32_t)n, gb.dvals[0], gb.dvals[1], gb.hist, gb.touched, gb.rect, cam.tiles_x, cap, gb.ikeys[0], gb.ivals[0],
       gb.hist + 4 * 256, gb.hist + 5 * 256, tile_shift0, tile_bits0, tile_shift1, tile_bits1, status,
@@ -301,7 +301,7 @@ int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const Geom
                   cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   int64_t blocks = ((int64_t)cap + 1 + 1023) / 1024;
-  if (blocks > 148 * 4) blocks = 148 * 4;
+  if (blocks > 148 * 8) blocks = 148 * 8;
   launch_pdl(ranges_kernel, dim3((unsigned)blocks), dim3(256), 0, s, sorted_tiles, gb.counters, cap, tiles, gb.ranges,
                                                  ranges_user, gb.tile_slot, gb.tile_order, counters_out, mlp_writes_rows);
   return 1;
