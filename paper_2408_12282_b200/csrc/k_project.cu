@@ -44,7 +44,9 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
   for (int i = threadIdx.x; i < 4 * 256; i += kProjThreads) s_hist[i] = 0;
   __syncthreads();
 
-  const int64_t i = (int64_t)blockIdx.x * kProjThreads + threadIdx.x;
+  // grid-stride over blocks of 256 Gaussians: the block's digit histograms are flushed once
+  for (int64_t base = (int64_t)blockIdx.x * kProjThreads; base < n; base += (int64_t)gridDim.x * kProjThreads) {
+  const int64_t i = base + threadIdx.x;
   const bool in_range = i < n;
   bool vis = false;
   uint32_t key = 0xFFFFFFFFu;
@@ -178,6 +180,7 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
   }
   const unsigned vmask = __ballot_sync(0xFFFFFFFFu, vis);
   if ((threadIdx.x & 31) == 0 && vmask) atomicAdd(&counters[DC_NVIS], __popc(vmask));
+  }
   __syncthreads();
   for (int k = threadIdx.x; k < 4 * 256; k += kProjThreads) {
     const uint32_t v = s_hist[k];
@@ -213,7 +216,8 @@ int launch_pack_attr(const sssgs_gaussians& g, float4* attr, cudaStream_t s) {
 int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb,
                    cudaStream_t s) {
   if (g.n == 0) return 0;
-  const unsigned blocks = (unsigned)((g.n + kProjThreads - 1) / kProjThreads);
+  unsigned blocks = (unsigned)((g.n + kProjThreads - 1) / kProjThreads);
+  if (blocks > 148 * 8) blocks = 148 * 8;
   launch_pdl(project_kernel, dim3(blocks), dim3(kProjThreads), 0, s, g.n, g.means, g.scales, g.rotations,
              g.opacities, cam, gb.rec_a, gb.rec_b, gb.rect, gb.touched, gb.dkeys[0], gb.hist, gb.counters);
   return 1;
