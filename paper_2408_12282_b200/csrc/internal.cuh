@@ -126,6 +126,8 @@ enum {
   DC_TICKET_BASE = 8, // tickets: one per ticketed kernel launch
   DC_RANGES_DONE = 24,   // blocks of ranges_kernel that have finished
   DC_CONTRIB_ROWS = 25,  // Gaussians kept by the visibility pre-pass (MLP rows of a sweep)
+  DC_WC_CHUNKS = 26,     // weight cache: chunks handed out
+  DC_WC_OVERFLOW = 27,   // weight cache: 1 if the pool ran out (the sweep then walks the lists again)
   DC_WORDS = 64
 };
 
@@ -145,6 +147,26 @@ struct GeomBuffers {
   uint32_t* hist;     // [6][256] digit histograms: 4 depth passes + 2 tile passes
   uint32_t* status;   // look-back status words, carved per pass
   uint32_t* counters; // [DC_WORDS]
+};
+
+// ---- weight cache of a light sweep ----------------------------------------------------------
+// The compositing weights T_i alpha_i of a view do not depend on the light.  In a sweep the
+// visibility pre-pass stores, per 8x4-pixel block (= warp) of every tile, the entries it blends
+// -- (Gaussian id, depth) and the 32 per-pixel weights -- in chunks of 32 entries chained through
+// `next`; the per-light walks then only stream those chunks and blend (no staging, culling, alpha
+// evaluation or transmittance chain).  The pool is bounded: if it runs out, `overflow` is set and
+// the sweep falls back to walking the lists.
+constexpr int kWcChunk = 32;
+struct WeightCache {
+  uint32_t* head;     // [tiles * 8] first chunk of the block's chain
+  uint32_t* count;    // [tiles * 8] entries in the chain
+  uint32_t* next;     // [capacity] chunk -> next chunk
+  uint2* hdr;         // [capacity * 32] (Gaussian id, bits(depth)) per entry
+  float* weights;     // [capacity * 32 * 32] weight of the entry at each of the block's 32 pixels
+  float* T;           // [H * W] final transmittance per pixel
+  uint32_t* chunks;   // device counter: chunks handed out (DC_WC_CHUNKS)
+  uint32_t* overflow; // device flag (DC_WC_OVERFLOW)
+  uint32_t capacity;  // chunks in the pool
 };
 
 // ---- MLP description on the device ----------------------------------------------------------
@@ -210,7 +232,12 @@ int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers&
                           int64_t frame_stride_px, cudaStream_t s);
 // visibility pre-pass of a light sweep and its compaction
 int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_vals,
-                        uint8_t* contrib, cudaStream_t s);
+                        uint8_t* contrib, const WeightCache* wc, cudaStream_t s);
+// per-light walk over the weight cache (returns immediately on the device if the cache overflowed)
+int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_lights,
+                         const GeomBuffers& gb, const WeightCache& wc, const float4* attr,
+                         const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
+                         int64_t frame_stride_px, int sum_mode, cudaStream_t s);
 int raster_reads_unblended_rows(int tiles);
 int launch_compact_contrib(const uint8_t* contrib, int64_t n, uint32_t* rows, uint32_t* count,
                            int zero_rest, float4* out0, float4* out1, int lights, cudaStream_t s);
@@ -219,7 +246,9 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                   const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                  int64_t frame_stride_px, int sum_mode, cudaStream_t s);
+                  int64_t frame_stride_px, int sum_mode, cudaStream_t s,
+                  const uint32_t* only_if_set = nullptr);
+// only_if_set: if given, the kernel returns at once unless *only_if_set != 0 (weight-cache fallback)
 // sum_mode: 0 = one RGB frame per light; 1 = ONE frame = sum over the batch's lights + background
 // term (first batch of a camera); 2 = add the batch's lights to the frame already there
 

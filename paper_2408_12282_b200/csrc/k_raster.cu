@@ -206,6 +206,126 @@ struct RasterShape {
   static_assert(RH >= PH && RH <= kTile && (RW % PW) == 0 && (RH % PH) == 0, "bad raster shape");
 };
 
+// End of a pixel's walk, shared by the list walk and the cached walk: unpacks the accumulators, adds
+// the E per-slot partial sums of a pixel, writes the G-buffer and shades (L114) -- or, FWD, adds the
+// background to the composited per-Gaussian colours.
+template <int LB, int E, bool FWD>
+__device__ __forceinline__ void raster_finish(float acc_depth, const f32x2* pacc, const f32x2 (*paccl)[2], float A,
+                                              float T, bool inside, int px, int py, int slot,
+                                              const CamParams& cam, const LightBatch& lights, int n_lights,
+                                              float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
+                                              float* __restrict__ aovd_out, float* __restrict__ aovs_out,
+                                              int64_t frame_stride_px, int sum_mode) {
+  constexpr int P = 32 / E;
+  constexpr unsigned FULL = 0xFFFFFFFFu;
+  // unpack: acc[] in G-buffer channel order (depth, n3, b3, rough, metal, sss), accl[l] = MLP channels
+  float acc[10], accl[LB][4];
+  acc[0] = acc_depth;
+  unpack2(pacc[0], acc[1], acc[2]);
+  unpack2(pacc[1], acc[3], acc[7]);
+  unpack2(pacc[2], acc[4], acc[5]);
+  unpack2(pacc[3], acc[6], acc[8]);
+  {
+    float a_sum;
+    unpack2(pacc[4], acc[9], a_sum);
+    if (!FWD) A = a_sum;
+  }
+#pragma unroll
+  for (int l = 0; l < LB; ++l) {
+    unpack2(paccl[l][0], accl[l][0], accl[l][1]);
+    unpack2(paccl[l][1], accl[l][2], accl[l][3]);
+  }
+
+  // ---- combine the E per-slot partial sums of every pixel (all E lanes end up with the total) ----
+  if (E > 1) {
+#pragma unroll
+    for (int o = P; o < 32; o <<= 1) {
+#pragma unroll
+      for (int c = 0; c < 10; ++c) acc[c] += __shfl_xor_sync(FULL, acc[c], o);
+#pragma unroll
+      for (int l = 0; l < LB; ++l)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) accl[l][c] += __shfl_xor_sync(FULL, accl[l][c], o);
+      A += __shfl_xor_sync(FULL, A, o);
+    }
+  }
+
+  if (!inside) return;
+  // ---- epilogue: G-buffer stores + deferred shading; lights and store quarters are dealt to the
+  //      E lanes of a pixel round-robin ---------------------------------------------------------------
+  const int64_t pidx = (int64_t)py * cam.width + px;
+  if (FWD) {  // C = sum_i T_i alpha_i c_i + (1 - A) bg  (Eq. 3), lights dealt to the E lanes of a pixel
+#pragma unroll
+    for (int l = 0; l < LB; ++l) {
+      if (l >= n_lights) break;
+      if (l % E != slot || !rgb_out) continue;
+      float* o = rgb_out + ((int64_t)l * frame_stride_px + pidx) * 3;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) o[c] = accl[l][c] + (1.f - A) * cam.bg[c];
+    }
+    return;
+  }
+  ShadeIn q;
+  const bool covered = A >= 1e-6f;
+  const float iA = covered ? 1.f / A : 0.f;
+  q.depth = acc[0] * iA; q.nx = acc[1] * iA; q.ny = acc[2] * iA; q.nz = acc[3] * iA;
+  q.br = acc[4] * iA; q.bg = acc[5] * iA; q.bb = acc[6] * iA;
+  q.rough = acc[7] * iA; q.metal = acc[8] * iA; q.sss = acc[9] * iA;
+  float sum[3] = {0.f, 0.f, 0.f};  // SSSGS_SUM_LIGHTS: this lane's share of the sum over the lights
+#pragma unroll
+  for (int l = 0; l < LB; ++l) {
+    if (l >= n_lights) break;
+    const int64_t fp = (int64_t)l * frame_stride_px + pidx;
+    if (gbuf_out) {
+      float4* gp = reinterpret_cast<float4*>(gbuf_out + fp * SSSGS_GBUF_CHANNELS);
+      if (0 % E == slot) gp[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      if (1 % E == slot) gp[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      if (2 % E == slot) gp[2] = make_float4(acc[8], acc[9], accl[l][0], accl[l][1]);
+      if (3 % E == slot) gp[3] = make_float4(accl[l][2], accl[l][3], A, T);
+    }
+    if (l % E != slot) continue;
+    float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
+    if (covered) {
+      const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
+      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc, sum_mode == 0);
+    } else {
+      rgb[0] = cam.bg[0]; rgb[1] = cam.bg[1]; rgb[2] = cam.bg[2];
+    }
+    if (sum_mode != 0) {
+      if (covered) { sum[0] += rgb[0]; sum[1] += rgb[1]; sum[2] += rgb[2]; }
+      continue;
+    }
+    if (rgb_out) {
+      float* o = rgb_out + fp * 3;
+      o[0] = rgb[0]; o[1] = rgb[1]; o[2] = rgb[2];
+    }
+    if (aovd_out) {
+      float* o = aovd_out + fp * 3;
+      o[0] = dif[0]; o[1] = dif[1]; o[2] = dif[2];
+    }
+    if (aovs_out) {
+      float* o = aovs_out + fp * 3;
+      o[0] = spc[0]; o[1] = spc[1]; o[2] = spc[2];
+    }
+  }
+  if (sum_mode != 0) {
+    // the lights were dealt to the E lanes of a pixel: add the shares (all lanes of the warp are
+    // still here: `inside` lanes only diverge below), then one lane per pixel writes
+    if (E > 1) {
+#pragma unroll
+      for (int o = P; o < 32; o <<= 1)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sum[c] += __shfl_xor_sync(__activemask(), sum[c], o);
+    }
+    if (slot == 0 && rgb_out) {
+      float* o = rgb_out + pidx * 3;
+      const float bgw = covered ? 1.f - A : 1.f;  // background term, once per pixel
+#pragma unroll
+      for (int c = 0; c < 3; ++c) o[c] = sum_mode == 1 ? sum[c] + bgw * cam.bg[c] : o[c] + sum[c];
+    }
+  }
+}
+
 // MARK = true is the visibility pre-pass of a light sweep: the same walk (same culling, alphas,
 // transmittance chain and stop rule, hence the same set of blended entries) without channels,
 // shading or outputs; it sets contrib[g] = 1 for every Gaussian that is blended at some pixel.  The
@@ -222,7 +342,8 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                     const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
-                    int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode) {
+                    int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode,
+                    WeightCache wc, const uint32_t* __restrict__ only_if_set) {
   using S = RasterShape<E, WARPS>;
   constexpr int P = S::P, THREADS = S::THREADS;
   constexpr int NC = MARK ? 2 : (FWD ? 2 + LB : 5 + LB);  // float4 components per list entry
@@ -240,6 +361,7 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   uint32_t* s_done = reinterpret_cast<uint32_t*>(s_empty + NS);  // warps whose pixels are all finished
 
   pdl_prologue();
+  if (only_if_set && *only_if_set == 0u) return;  // weight-cache fallback walk, not needed
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int slot = lane / P, pix = lane % P;
   const int tile = (int)tile_order[blockIdx.x / S::SUBS];  // longest lists first
@@ -266,6 +388,10 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
 #pragma unroll
   for (int l = 0; l < LB; ++l) paccl[l][0] = paccl[l][1] = make_float2(0.f, 0.f);
   bool done = !inside;
+  // weight cache (MARK, E == 1, wc.weights != nullptr): this warp's chain
+  const bool caching = MARK && E == 1 && wc.weights != nullptr;
+  bool wc_off = !caching;
+  uint32_t wc_chunk = 0, wc_items = 0;
 
   const uint32_t n_entries = range.y - range.x;
   const int n_batches = (int)((n_entries + kBatch - 1) / kBatch);
@@ -419,6 +545,30 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
           w = alpha[u] * myT;
         }
         if (MARK) {
+          if (!wc_off && __any_sync(FULL, w > 0.f)) {
+            const uint32_t in_chunk = wc_items % kWcChunk;
+            if (in_chunk == 0) {  // the chain needs a new chunk
+              uint32_t c = 0;
+              if (lane == 0) c = atomicAdd(wc.chunks, 1u);
+              c = __shfl_sync(FULL, c, 0);
+              if (c >= wc.capacity) {
+                if (lane == 0) *wc.overflow = 1u;
+                wc_off = true;
+              } else {
+                if (lane == 0) {
+                  if (wc_items == 0) wc.head[tile * 8 + warp] = c;
+                  else wc.next[wc_chunk] = c;
+                }
+                wc_chunk = c;
+              }
+            }
+            if (!wc_off) {
+              wc.weights[((size_t)wc_chunk * kWcChunk + in_chunk) * 32 + lane] = w;
+              if (lane == 0)
+                wc.hdr[(size_t)wc_chunk * kWcChunk + in_chunk] = make_uint2(s_gid[st][j[u]], __float_as_uint(zed[u]));
+              ++wc_items;
+            }
+          }
           if (w > 0.f) contrib[s_gid[st][j[u]]] = 1;
         } else if (FWD) {
           if (__any_sync(FULL, w > 0.f)) {
@@ -456,114 +606,16 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
     if (lane == 0) mbar_arrive(s_empty + st);
   }
   cp_async_wait_all();
-  if (MARK) return;
-
-  // unpack: acc[] in G-buffer channel order (depth, n3, b3, rough, metal, sss), accl[l] = MLP channels
-  float acc[10], accl[LB][4];
-  acc[0] = acc_depth;
-  unpack2(pacc[0], acc[1], acc[2]);
-  unpack2(pacc[1], acc[3], acc[7]);
-  unpack2(pacc[2], acc[4], acc[5]);
-  unpack2(pacc[3], acc[6], acc[8]);
-  {
-    float a_sum;
-    unpack2(pacc[4], acc[9], a_sum);
-    if (!FWD) A = a_sum;
-  }
-#pragma unroll
-  for (int l = 0; l < LB; ++l) {
-    unpack2(paccl[l][0], accl[l][0], accl[l][1]);
-    unpack2(paccl[l][1], accl[l][2], accl[l][3]);
-  }
-
-  // ---- combine the E per-slot partial sums of every pixel (all E lanes end up with the total) ----
-  if (E > 1) {
-#pragma unroll
-    for (int o = P; o < 32; o <<= 1) {
-#pragma unroll
-      for (int c = 0; c < 10; ++c) acc[c] += __shfl_xor_sync(FULL, acc[c], o);
-#pragma unroll
-      for (int l = 0; l < LB; ++l)
-#pragma unroll
-        for (int c = 0; c < 4; ++c) accl[l][c] += __shfl_xor_sync(FULL, accl[l][c], o);
-      A += __shfl_xor_sync(FULL, A, o);
-    }
-  }
-
-  if (!inside) return;
-  // ---- epilogue: G-buffer stores + deferred shading; lights and store quarters are dealt to the
-  //      E lanes of a pixel round-robin ---------------------------------------------------------------
-  const int64_t pidx = (int64_t)py * cam.width + px;
-  if (FWD) {  // C = sum_i T_i alpha_i c_i + (1 - A) bg  (Eq. 3), lights dealt to the E lanes of a pixel
-#pragma unroll
-    for (int l = 0; l < LB; ++l) {
-      if (l >= n_lights) break;
-      if (l % E != slot || !rgb_out) continue;
-      float* o = rgb_out + ((int64_t)l * frame_stride_px + pidx) * 3;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) o[c] = accl[l][c] + (1.f - A) * cam.bg[c];
+  if (MARK) {
+    if (caching) {
+      if (lane == 0) wc.count[tile * 8 + warp] = wc_items;
+      if (inside) wc.T[(int64_t)py * cam.width + px] = T;
     }
     return;
   }
-  ShadeIn q;
-  const bool covered = A >= 1e-6f;
-  const float iA = covered ? 1.f / A : 0.f;
-  q.depth = acc[0] * iA; q.nx = acc[1] * iA; q.ny = acc[2] * iA; q.nz = acc[3] * iA;
-  q.br = acc[4] * iA; q.bg = acc[5] * iA; q.bb = acc[6] * iA;
-  q.rough = acc[7] * iA; q.metal = acc[8] * iA; q.sss = acc[9] * iA;
-  float sum[3] = {0.f, 0.f, 0.f};  // SSSGS_SUM_LIGHTS: this lane's share of the sum over the lights
-#pragma unroll
-  for (int l = 0; l < LB; ++l) {
-    if (l >= n_lights) break;
-    const int64_t fp = (int64_t)l * frame_stride_px + pidx;
-    if (gbuf_out) {
-      float4* gp = reinterpret_cast<float4*>(gbuf_out + fp * SSSGS_GBUF_CHANNELS);
-      if (0 % E == slot) gp[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-      if (1 % E == slot) gp[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-      if (2 % E == slot) gp[2] = make_float4(acc[8], acc[9], accl[l][0], accl[l][1]);
-      if (3 % E == slot) gp[3] = make_float4(accl[l][2], accl[l][3], A, T);
-    }
-    if (l % E != slot) continue;
-    float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
-    if (covered) {
-      const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
-      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc, sum_mode == 0);
-    } else {
-      rgb[0] = cam.bg[0]; rgb[1] = cam.bg[1]; rgb[2] = cam.bg[2];
-    }
-    if (sum_mode != 0) {
-      if (covered) { sum[0] += rgb[0]; sum[1] += rgb[1]; sum[2] += rgb[2]; }
-      continue;
-    }
-    if (rgb_out) {
-      float* o = rgb_out + fp * 3;
-      o[0] = rgb[0]; o[1] = rgb[1]; o[2] = rgb[2];
-    }
-    if (aovd_out) {
-      float* o = aovd_out + fp * 3;
-      o[0] = dif[0]; o[1] = dif[1]; o[2] = dif[2];
-    }
-    if (aovs_out) {
-      float* o = aovs_out + fp * 3;
-      o[0] = spc[0]; o[1] = spc[1]; o[2] = spc[2];
-    }
-  }
-  if (sum_mode != 0) {
-    // the lights were dealt to the E lanes of a pixel: add the shares (all lanes of the warp are
-    // still here: `inside` lanes only diverge below), then one lane per pixel writes
-    if (E > 1) {
-#pragma unroll
-      for (int o = P; o < 32; o <<= 1)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) sum[c] += __shfl_xor_sync(__activemask(), sum[c], o);
-    }
-    if (slot == 0 && rgb_out) {
-      float* o = rgb_out + pidx * 3;
-      const float bgw = covered ? 1.f - A : 1.f;  // background term, once per pixel
-#pragma unroll
-      for (int c = 0; c < 3; ++c) o[c] = sum_mode == 1 ? sum[c] + bgw * cam.bg[c] : o[c] + sum[c];
-    }
-  }
+
+  raster_finish<LB, E, FWD>(acc_depth, pacc, paccl, A, T, inside, px, py, slot, cam, lights, n_lights, rgb_out,
+                            gbuf_out, aovd_out, aovs_out, frame_stride_px, sum_mode);
 }
 
 // Copies caller-supplied MLP outputs ([n_light][n][4], light stride given) into the internal
@@ -595,7 +647,7 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
                           const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                           const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
                           int64_t frame_stride_px, int tiles, cudaStream_t s, uint8_t* contrib = nullptr,
-                          int sum_mode = 0) {
+                          int sum_mode = 0, const WeightCache* wc = nullptr, const uint32_t* only_if_set = nullptr) {
   using S = RasterShape<E, WARPS>;
   constexpr int smem = raster_smem(LB, MARK, FWD, WARPS);
   static bool configured = false;
@@ -607,7 +659,7 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
   }
   launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
              lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
-             aov_d, aov_s, frame_stride_px, contrib, sum_mode);
+             aov_d, aov_s, frame_stride_px, contrib, sum_mode, wc ? *wc : WeightCache{}, only_if_set);
   return 1;
 }
 
@@ -625,7 +677,7 @@ static int raster_mode() {
 int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
                   const GeomBuffers& gb, const uint32_t* sorted_vals, const float4* attr,
                   const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                  int64_t frame_stride_px, int sum_mode, cudaStream_t s) {
+                  int64_t frame_stride_px, int sum_mode, cudaStream_t s, const uint32_t* only_if_set) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
   // Default shape: few tiles (small images) leave SMs idle behind the longest tile lists, so the
@@ -634,7 +686,7 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   // (measured: DESIGN.md).
   int mode = raster_mode();
   if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
-#define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, nullptr, sum_mode
+#define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, nullptr, sum_mode, nullptr, only_if_set
 #define SSSGS_BY_LB(E, W, U)                                                   \
   do {                                                                         \
     if (n_lights <= 1) return launch_variant<1, E, W, U>(SSSGS_ARGS);          \
@@ -713,10 +765,125 @@ int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers&
 #undef SSSGS_FWD
 }
 
+namespace {
+// Per-light walk of a sweep over the weight cache: one warp per 8x4-pixel block streams the block's
+// chain -- per entry (Gaussian id, depth) and the 32 weights -- and blends the entry's channels,
+// fetched with warp-uniform loads (a Gaussian's rows are shared by neighbouring blocks and tiles: L1 /
+// L2 hits).  Same accumulation order and arithmetic as the list walk: bit-identical frames.
+template <int LB>
+__global__ void __launch_bounds__(256, 2)
+raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint32_t* __restrict__ tile_order,
+                     WeightCache wc, const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
+                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out, float* __restrict__ aovd_out,
+                     float* __restrict__ aovs_out, int64_t frame_stride_px, int sum_mode) {
+  pdl_prologue();
+  if (*wc.overflow != 0u) return;  // the pool ran out: the list walk launched next does the work
+  using S = RasterShape<1, 8>;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tile = (int)tile_order[blockIdx.x];
+  const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
+  constexpr int WPR = S::RW / S::PW;
+  const int px = tx * kTile + (warp % WPR) * S::PW + lane % S::PW;
+  const int py = ty * kTile + (warp / WPR) * S::PH + lane / S::PW;
+  const bool inside = px < cam.width && py < cam.height;
+
+  float acc_depth = 0.f;
+  f32x2 pacc[5], paccl[LB][2];
+#pragma unroll
+  for (int c = 0; c < 5; ++c) pacc[c] = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int l = 0; l < LB; ++l) paccl[l][0] = paccl[l][1] = make_float2(0.f, 0.f);
+
+  // Per warp and chunk of 32 entries: lane k gathers the rows (3 attribute float4 + LB MLP float4) of
+  // entry k and every lane fetches an eighth of the chunk's 4 KB of weights -- 11-19 independent
+  // loads per lane issued back to back, one memory latency per chunk -- into this warp's shared
+  // memory; the entries are then blended from broadcast (rows) and conflict-free (weights) reads.
+  constexpr int NR = 3 + LB;
+  constexpr int kWarpBytes = NR * kWcChunk * 16 + kWcChunk * 32 * 4;
+  extern __shared__ float4 s_dyn[];
+  float4 (*s_rows)[kWcChunk] = reinterpret_cast<float4 (*)[kWcChunk]>(reinterpret_cast<char*>(s_dyn) + warp * kWarpBytes);
+  float* s_w = reinterpret_cast<float*>(s_rows + NR);  // [entry][pixel]
+
+  const uint32_t n_items = wc.count[tile * 8 + warp];
+  uint32_t chunk = n_items ? wc.head[tile * 8 + warp] : 0u;
+  for (uint32_t i0 = 0; i0 < n_items; i0 += kWcChunk) {
+    const uint32_t m = min((uint32_t)kWcChunk, n_items - i0);
+    const uint2 my_hdr = lane < m ? wc.hdr[(size_t)chunk * kWcChunk + lane] : make_uint2(0u, 0u);
+    const uint32_t nxt = i0 + kWcChunk < n_items ? wc.next[chunk] : 0u;
+    __syncwarp();  // every lane has left the previous chunk's staging
+    {
+      const float4* wsrc = reinterpret_cast<const float4*>(wc.weights + (size_t)chunk * kWcChunk * 32);
+      float4 wv[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) wv[q] = (uint32_t)(q * 4 + lane / 8) < m ? wsrc[q * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+      if (lane < m) {
+        const size_t g = my_hdr.x;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) s_rows[c][lane] = attr[3 * g + c];
+#pragma unroll
+        for (int l = 0; l < LB; ++l) s_rows[3 + l][lane] = mlp_out[g * n_lights + min(l, n_lights - 1)];
+      }
+#pragma unroll
+      for (int q = 0; q < 8; ++q) reinterpret_cast<float4*>(s_w)[q * 32 + lane] = wv[q];
+    }
+    __syncwarp();
+#pragma unroll 4
+    for (uint32_t k = 0; k < m; ++k) {
+      const float depth = __uint_as_float(__shfl_sync(0xFFFFFFFFu, my_hdr.y, k));
+      const float w = s_w[k * 32 + lane];
+      const float4 a0 = s_rows[0][k], a1 = s_rows[1][k], a2 = s_rows[2][k];
+      const f32x2 ww = make_float2(w, w);
+      acc_depth = fmaf(w, depth, acc_depth);
+      fma2(pacc[0], ww, a0.x, a0.y);
+      fma2(pacc[1], ww, a0.z, a0.w);
+      fma2(pacc[2], ww, a1.x, a1.y);
+      fma2(pacc[3], ww, a1.z, a1.w);
+      fma2(pacc[4], ww, a2.x, a2.y);
+#pragma unroll
+      for (int l = 0; l < LB; ++l) {
+        const float4 mo = s_rows[3 + l][k];
+        fma2(paccl[l][0], ww, mo.x, mo.y);
+        fma2(paccl[l][1], ww, mo.z, mo.w);
+      }
+    }
+    chunk = nxt;
+  }
+  const float T = inside ? wc.T[(int64_t)py * cam.width + px] : 1.f;
+  raster_finish<LB, 1, false>(acc_depth, pacc, paccl, 0.f, T, inside, px, py, 0, cam, lights, n_lights, rgb_out,
+                              gbuf_out, aovd_out, aovs_out, frame_stride_px, sum_mode);
+}
+}  // namespace
+
+int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_lights,
+                         const GeomBuffers& gb, const WeightCache& wc, const float4* attr,
+                         const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
+                         int64_t frame_stride_px, int sum_mode, cudaStream_t s) {
+  const int tiles = cam.tiles_x * cam.tiles_y;
+  if (tiles == 0) return 0;
+#define SSSGS_CACHED(LB)                                                                                \
+  do {                                                                                                  \
+    constexpr int smem = 8 * ((3 + LB) * kWcChunk * 16 + kWcChunk * 32 * 4);                            \
+    static bool configured = false;                                                                     \
+    if (!configured) {                                                                                  \
+      if (cudaFuncSetAttribute(raster_cached_kernel<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                               smem) != cudaSuccess)                                                    \
+        return -1;                                                                                      \
+      configured = true;                                                                                \
+    }                                                                                                   \
+    launch_pdl(raster_cached_kernel<LB>, dim3(tiles), dim3(256), smem, s, cam, lights, n_lights,        \
+               gb.tile_order, wc, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, sum_mode);   \
+  } while (0)
+  if (n_lights <= 1) SSSGS_CACHED(1);
+  else if (n_lights <= 4) SSSGS_CACHED(4);
+  else SSSGS_CACHED(8);
+#undef SSSGS_CACHED
+  return 1;
+}
+
 // Visibility pre-pass of a light sweep (see raster_shade_kernel, MARK): same tile order and shape
 // choice as the render walks.
 int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint32_t* sorted_vals,
-                        uint8_t* contrib, cudaStream_t s) {
+                        uint8_t* contrib, const WeightCache* wc, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
   LightBatch none;
@@ -724,9 +891,9 @@ int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint3
   int mode = raster_mode();
   if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
   const int e = mode / (mode >= 100 ? 100 : 10);
-  if (e == 1)
+  if (e == 1 || wc)  // the weight cache is organised by the 8x4-pixel blocks of the one-slot shape
     return launch_variant<1, 1, 8, 4, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
-                                            nullptr, 0, tiles, s, contrib);
+                                            nullptr, 0, tiles, s, contrib, 0, wc);
   return launch_variant<1, 4, 8, 2, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
                                           nullptr, 0, tiles, s, contrib);
 }

@@ -4,6 +4,7 @@
 // every step of the path runs in the kernels of this directory.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -36,6 +37,7 @@ struct sssgs_ctx {
   cudaStream_t copy = nullptr;
   cudaEvent_t ev_upload = nullptr;
   bool upload_pending = false;
+  WeightCache wc{};             // weight cache of a sweep (pool sized from max_instances)
   uint8_t* contrib = nullptr;   // [n] visibility pre-pass flags (inside the control block)
   uint32_t* rows = nullptr;     // [n] Gaussians kept by the pre-pass
   uint8_t* mlp_blob = nullptr;
@@ -111,6 +113,19 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
   p = take((tiles + 1) * 4); if (c) c->gb.tile_slot = (uint32_t*)p;
   for (int k = 0; k < 2; ++k) { p = take(n * (size_t)lb * 16); if (c) c->mlp_out[k] = (float4*)p; }
   p = take(n * 4); if (c) c->rows = (uint32_t*)p;
+  {  // weight cache: the blended (block, entry) pairs of a view; half an entry per tile instance
+     // covers the scenes measured so far (0.13-0.5); beyond that the sweep falls back to the list walks
+    size_t chunks = (cap / 2 + 65536) / kWcChunk;
+    if (const char* e = getenv("SSSGS_WC_CHUNKS")) chunks = (size_t)atoll(e);  // tuning / test aid
+    const size_t npix = (size_t)cfg.max_width * cfg.max_height;
+    p = take(tiles * 8 * 4); if (c) c->wc.head = (uint32_t*)p;
+    p = take(tiles * 8 * 4); if (c) c->wc.count = (uint32_t*)p;
+    p = take(chunks * 4); if (c) c->wc.next = (uint32_t*)p;
+    p = take(chunks * kWcChunk * 8); if (c) c->wc.hdr = (uint2*)p;
+    p = take(chunks * kWcChunk * 32 * 4); if (c) c->wc.weights = (float*)p;
+    p = take(npix * 4); if (c) c->wc.T = (float*)p;
+    if (c) c->wc.capacity = (uint32_t)chunks;
+  }
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
   p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
   // control block: everything that must be zero at the start of a camera
@@ -490,9 +505,14 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                               out->sorted_keys ? out->sorted_keys + (size_t)v * cap : nullptr,
                               out->sorted_vals ? out->sorted_vals + (size_t)v * cap : nullptr, s));
     end();
+    // The pre-pass also caches the compositing weights of the view (deferred path): the per-light
+    // walks then stream the cache instead of walking the lists again.
+    const bool use_cache = use_mask && !forward && c->wc.capacity > 0;
     if (use_mask) {
+      c->wc.chunks = cnt + DC_WC_CHUNKS;
+      c->wc.overflow = cnt + DC_WC_OVERFLOW;
       begin(SSSGS_STAGE_RASTER);
-      add(launch_mark_contrib(cam, c->gb, sorted_vals, c->contrib, s));
+      add(launch_mark_contrib(cam, c->gb, sorted_vals, c->contrib, use_cache ? &c->wc : nullptr, s));
       add(launch_compact_contrib(c->contrib, g->n, c->rows, cnt + DC_CONTRIB_ROWS, raster_reads_unblended_rows(tiles),
                                  c->mlp_out[0], c->mlp_out[1], n_light < c->max_lb ? n_light : c->max_lb, s));
       end();
@@ -552,6 +572,16 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         if (!run_mlp) add(launch_shade_gaussians(g->n, nl, g->means, c->attr, cam, lb, mlp_buf, s));
         add(launch_raster_forward(cam, nl, c->gb, sorted_vals, mlp_buf,
                                   out->rgb ? out->rgb + frame0 * npix * 3 : nullptr, npix, s));
+      } else {
+      float* o_rgb = out->rgb ? out->rgb + (sum_lights ? (int64_t)v : frame0) * npix * 3 : nullptr;
+      float* o_gbuf = out->gbuffer ? out->gbuffer + frame0 * npix * SSSGS_GBUF_CHANNELS : nullptr;
+      float* o_ad = out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr;
+      float* o_as = out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr;
+      const int smode = sum_lights ? (l0 == 0 ? 1 : 2) : 0;
+      if (use_cache) {  // cached walk; the list walk behind it only runs if the cache overflowed
+        add(launch_raster_cached(cam, lb, nl, c->gb, c->wc, c->attr, mlp_buf, o_rgb, o_gbuf, o_ad, o_as, npix, smode, s));
+        add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf, o_rgb, o_gbuf, o_ad, o_as, npix, smode, s,
+                          cnt + DC_WC_OVERFLOW));
       } else
       add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf,
                         out->rgb ? out->rgb + (sum_lights ? (int64_t)v : frame0) * npix * 3 : nullptr,
@@ -559,6 +589,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
                         out->aov_diffuse ? out->aov_diffuse + frame0 * npix * 3 : nullptr,
                         out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr, npix,
                         sum_lights ? (l0 == 0 ? 1 : 2) : 0, s));
+      }
       end();
       if (overlap && cudaEventRecord(c->ev_raster[buf], s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "event record failed");
       ++batch_no;

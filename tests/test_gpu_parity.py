@@ -206,7 +206,11 @@ def test_sweep_row_skipping_changes_nothing(width):
     assert on["launches"] > off["launches"]          # pre-pass + compaction were launched
     assert off["counters"][0][4] == scene.n
     for k in ("rgb", "gbuffer", "aov_diffuse", "aov_specular"):
-        np.testing.assert_array_equal(on[k].view(np.uint32), off[k].view(np.uint32))
+        if width > 640:   # same one-slot walk order with and without the pre-pass: bit-identical
+            np.testing.assert_array_equal(on[k].view(np.uint32), off[k].view(np.uint32))
+        else:             # small images walk 2 entries per warp step without the pre-pass: the per-slot
+            # partial sums are added in another order than the cached one-slot walk (both within 1e-4)
+            np.testing.assert_allclose(on[k], off[k], rtol=2e-5, atol=2e-6)
     r = oracle.render_frame(scene, 0, 0, mlp_out=off["mlp_out"][0].astype(np.float64))
     # the rows the pre-pass keeps are the Gaussians the oracle blends at some pixel (pixels whose
     # skip / stop decisions sit within rounding of a threshold may add or drop a few)
@@ -294,6 +298,21 @@ def test_forward_shading_variant_matches_oracle(width, n_lights):
         assert (err[st] <= tol[st]).all(), f"light {l}: worst {err[st].max():.3e}"
         assert (err[~st] <= 2e-2 * np.maximum(1.0, np.abs(r.rgb[~st]))).all()
         assert np.percentile(np.abs(own[l] - r.rgb)[st], 99.9) <= 5e-3
+
+
+def test_weight_cache_overflow_falls_back_to_the_list_walks(monkeypatch):
+    # In a sweep the visibility pre-pass caches the compositing weights and the per-light walks stream
+    # the cache.  The pool is bounded: when it runs out the list walks run instead.  Same frames.
+    scene = scenes.make_scene(3, n=40000, width=656, height=656, lights=6)
+    want = ("rgb", "gbuffer", "counters")
+    cached = gpu_render(scene, want=want, lights=scene.lights[0])
+    monkeypatch.setenv("SSSGS_WC_CHUNKS", "16")       # 512 cached entries for a frame that needs ~1e5
+    fallback = gpu_render(scene, want=want, lights=scene.lights[0])
+    monkeypatch.delenv("SSSGS_WC_CHUNKS")
+    full = gpu_render(scene, want=want + ("mlp_out",), lights=scene.lights[0])  # no pre-pass at all
+    for k in ("rgb", "gbuffer"):
+        np.testing.assert_array_equal(cached[k].view(np.uint32), full[k].view(np.uint32))
+        np.testing.assert_array_equal(fallback[k].view(np.uint32), full[k].view(np.uint32))
 
 
 def test_run_to_run_determinism():
