@@ -806,10 +806,14 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
 
   const uint32_t n_items = wc.count[tile * 8 + warp];
   uint32_t chunk = n_items ? wc.head[tile * 8 + warp] : 0u;
+  uint2 hdr_pre = (uint32_t)lane < n_items ? wc.hdr[(size_t)chunk * kWcChunk + lane] : make_uint2(0u, 0u);
   for (uint32_t i0 = 0; i0 < n_items; i0 += kWcChunk) {
     const uint32_t m = min((uint32_t)kWcChunk, n_items - i0);
-    const uint2 my_hdr = lane < m ? wc.hdr[(size_t)chunk * kWcChunk + lane] : make_uint2(0u, 0u);
-    const uint32_t nxt = i0 + kWcChunk < n_items ? wc.next[chunk] : 0u;
+    const uint2 my_hdr = hdr_pre;
+    const bool more = i0 + kWcChunk < n_items;
+    const uint32_t nxt = more ? wc.next[chunk] : 0u;
+    // the next chunk's headers are fetched a chunk ahead (they gate its gathers)
+    if (more && i0 + kWcChunk + lane < n_items) hdr_pre = wc.hdr[(size_t)nxt * kWcChunk + lane];
     __syncwarp();  // every lane has left the previous chunk's staging
     {
       const float4* wsrc = reinterpret_cast<const float4*>(wc.weights + (size_t)chunk * kWcChunk * 32);
