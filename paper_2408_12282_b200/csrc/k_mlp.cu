@@ -721,6 +721,17 @@ static MlpShape mlp_shape(const MlpPlan& plan) {
   sh.slots = sh.ts ? s_ts : s_ss;
   if (sh.slots < 1) sh.slots = 1;
   sh.wps = sh.slots <= 2 ? 8 : 4;
+  {  // tuning aid: SSSGS_MLP_SHAPE=<ts><slots><wps>, e.g. 124 = TS mode, 2 slots, 4 warps per slot
+    static int force = -1;
+    if (force < 0) { const char* e = getenv("SSSGS_MLP_SHAPE"); force = e ? atoi(e) : 0; }
+    if (force > 0) {
+      const bool ts = force / 100 != 0;
+      const int slots = force / 10 % 10, wps = force % 10;
+      if (slots >= 1 && slots <= (ts ? s_ts : s_ss) && (wps == 4 || wps == 8)) {
+        sh.ts = ts; sh.slots = slots; sh.wps = wps;
+      }
+    }
+  }
   sh.slot_cols = sh.ts ? d_cols + a_cols : d_cols;
   sh.a_col = d_cols;
   sh.a_bytes = sh.ts ? 0 : plan.max_k_bytes;

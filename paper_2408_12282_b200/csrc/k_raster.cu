@@ -38,90 +38,138 @@ struct ShadeIn {
   float depth, nx, ny, nz, br, bg, bb, rough, metal, sss;  // already divided by coverage A
 };
 
-// Eq. 7 with the BRDF of Eq. 4 (L76-80) at the world-space point xw, for one
-// light: rgb = intensity * A * L_out (+ (1 - A) bg).  fp32 restatement of DESIGN.md "Shading".
-__device__ __forceinline__ void shade_point(const ShadeIn& q, const float lsss[3], float lin, float A,
-                                            const float xw[3], const CamParams& cam,
-                                            const LightParams& lt, float rgb[3], float dif[3],
-                                            float spc[3], bool with_bg) {
-  float l[3], v[3];
+// Approximate reciprocal / reciprocal square root, one MUFU each (about 1 ulp; the shading tolerance
+// is 1e-4).  The operands are floored away from zero and denormals by the caller.
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float rsqrt_approx(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+constexpr float kInvPi = 0.31830988618379067154f;
+
+// Eq. 7 with the BRDF of Eq. 4 (L76-80), fp32 restatement of DESIGN.md "Shading",
+// split in the part that depends on the shaded point and the view only (ShadeView: shared by all
+// lights of a walk) and the part per light (shade_light).
+struct ShadeView {
+  float xw[3], v[3], n[3];
+  bool has_n;           // |n| >= 1e-8: otherwise only the SSS term is shaded
+  float nv_k;           // nv (1 - k) + k, nv = max(1e-4, n.v)
+  float a2, k, omk;     // alpha^2, k = alpha / 2, 1 - k
+  float F0[3], omF0[3]; // Fresnel at normal incidence and its complement
+  float fd[3];          // diffuse lobe (1 - metal) base / pi
+  float difc;           // (1 - sss) (1 - metal) / pi
+  float sss, oms;
+};
+
+__device__ __forceinline__ void shade_view(const ShadeIn& q, const float xw[3], const CamParams& cam, ShadeView& s) {
+  float vv = 0.f;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    l[k] = lt.pos[k] - xw[k];
-    v[k] = cam.pos[k] - xw[k];
+    s.xw[k] = xw[k];
+    s.v[k] = cam.pos[k] - xw[k];
+    vv = fmaf(s.v[k], s.v[k], vv);
   }
-  const float il = rsqrtf(l[0] * l[0] + l[1] * l[1] + l[2] * l[2]);
-  const float iv = rsqrtf(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+  const float iv = rsqrt_approx(vv);
 #pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    l[k] *= il;
-    v[k] *= iv;
+  for (int k = 0; k < 3; ++k) s.v[k] *= iv;
+  const float nn2 = q.nx * q.nx + q.ny * q.ny + q.nz * q.nz;
+  s.has_n = nn2 >= 1e-16f;
+  const float in = rsqrt_approx(fmaxf(nn2, 1e-16f));
+  s.n[0] = q.nx * in; s.n[1] = q.ny * in; s.n[2] = q.nz * in;
+  const float nv = fmaxf(1e-4f, s.n[0] * s.v[0] + s.n[1] * s.v[1] + s.n[2] * s.v[2]);
+  const float ar = fmaxf(1e-3f, q.rough * q.rough);
+  s.a2 = ar * ar;
+  s.k = 0.5f * ar;
+  s.omk = 1.f - s.k;
+  s.nv_k = fmaf(nv, s.omk, s.k);
+  const float base[3] = {q.br, q.bg, q.bb};
+  const float omm = 1.f - q.metal;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    s.F0[c] = 0.04f * omm + base[c] * q.metal;
+    s.omF0[c] = 1.f - s.F0[c];
+    s.fd[c] = omm * base[c] * kInvPi;
   }
+  s.sss = q.sss;
+  s.oms = 1.f - q.sss;
+  s.difc = s.oms * omm * kInvPi;
+}
+
+// rgb = intensity * A * L_out (+ (1 - A) bg) for one light; dif / spc are the AOVs of L320.
+__device__ __forceinline__ void shade_light(const ShadeView& s, const float lsss[3], float lin, float A,
+                                            const CamParams& cam, const LightParams& lt, float rgb[3],
+                                            float dif[3], float spc[3], bool with_bg) {
   float brdf[3] = {0.f, 0.f, 0.f};
 #pragma unroll
   for (int c = 0; c < 3; ++c) dif[c] = spc[c] = 0.f;
-  const float nn2 = q.nx * q.nx + q.ny * q.ny + q.nz * q.nz;
-  if (nn2 >= 1e-16f) {
-    const float in = rsqrtf(nn2);
-    const float n[3] = {q.nx * in, q.ny * in, q.nz * in};
-    float h[3] = {l[0] + v[0], l[1] + v[1], l[2] + v[2]};
-    const float hl2 = h[0] * h[0] + h[1] * h[1] + h[2] * h[2];
-    if (hl2 >= 1e-16f) {
-      const float ih = rsqrtf(hl2);
-      h[0] *= ih; h[1] *= ih; h[2] *= ih;
-    } else {
-      h[0] = n[0]; h[1] = n[1]; h[2] = n[2];
+  if (s.has_n) {
+    float l[3], ll = 0.f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      l[k] = lt.pos[k] - s.xw[k];
+      ll = fmaf(l[k], l[k], ll);
     }
+    const float il = rsqrt_approx(ll);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) l[k] *= il;
+    float h[3] = {l[0] + s.v[0], l[1] + s.v[1], l[2] + s.v[2]};
+    const float hl2 = h[0] * h[0] + h[1] * h[1] + h[2] * h[2];
+    const bool has_h = hl2 >= 1e-16f;
+    const float ih = rsqrt_approx(fmaxf(hl2, 1e-16f));
+#pragma unroll
+    for (int k = 0; k < 3; ++k) h[k] = has_h ? h[k] * ih : s.n[k];
+    const float* n = s.n;
     const float nl = fmaxf(0.f, n[0] * l[0] + n[1] * l[1] + n[2] * l[2]);
-    const float nv = fmaxf(1e-4f, n[0] * v[0] + n[1] * v[1] + n[2] * v[2]);
-    const float nh = fminf(1.f, fmaxf(0.f, n[0] * h[0] + n[1] * h[1] + n[2] * h[2]));
-    const float vh = fminf(1.f, fmaxf(0.f, v[0] * h[0] + v[1] * h[1] + v[2] * h[2]));
-    const float ar = fmaxf(1e-3f, q.rough * q.rough);
-    const float a2 = ar * ar;
+    const float nh = __saturatef(n[0] * h[0] + n[1] * h[1] + n[2] * h[2]);
+    const float vh = __saturatef(s.v[0] * h[0] + s.v[1] * h[1] + s.v[2] * h[2]);
     // cancellation-free GGX: 1 - nh^2 = |n x h|^2
     const float cx = n[1] * h[2] - n[2] * h[1], cy = n[2] * h[0] - n[0] * h[2],
                 cz = n[0] * h[1] - n[1] * h[0];
     const float s2 = cx * cx + cy * cy + cz * cz;
-    const float dd = fmaxf(1e-12f, a2 * nh * nh + s2);  // floor: only n = -h exactly (DESIGN.md readings)
-    const float D = a2 / (kPi * dd * dd);
-    const float k = 0.5f * ar;
-    const float V = 1.f / (4.f * (nl * (1.f - k) + k) * (nv * (1.f - k) + k));
+    const float dd = fmaxf(1e-12f, s.a2 * nh * nh + s2);  // floor: only n = -h exactly (DESIGN.md readings)
+    // D V = a2 / (pi dd^2) / (4 (nl (1 - k) + k) (nv (1 - k) + k))
+    const float DV = s.a2 * rcp_approx(kPi * dd * dd * 4.f * fmaf(nl, s.omk, s.k) * s.nv_k);
     const float om = 1.f - vh;
     const float om2 = om * om;
     const float om5 = om2 * om2 * om;
-    const float base[3] = {q.br, q.bg, q.bb};
     const float lnl = lin * nl;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const float F0 = 0.04f * (1.f - q.metal) + base[c] * q.metal;
-      const float F = F0 + (1.f - F0) * om5;
-      const float fs = D * F * V;
-      const float fd = (1.f - q.metal) * base[c] / kPi;
-      brdf[c] = (fs + fd) * lnl;
-      spc[c] = (1.f - q.sss) * fs * lnl;
-      dif[c] = (1.f - q.sss) * (1.f - q.metal) / kPi * lnl;
+      const float fs = DV * fmaf(s.omF0[c], om5, s.F0[c]);
+      brdf[c] = (fs + s.fd[c]) * lnl;
+      spc[c] = s.oms * fs * lnl;
+      dif[c] = s.difc * lnl;
     }
   }
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const float lout = q.sss * lsss[c] + (1.f - q.sss) * brdf[c];
+    const float lout = s.sss * lsss[c] + s.oms * brdf[c];
     rgb[c] = lt.intensity[c] * A * lout + (with_bg ? (1.f - A) * cam.bg[c] : 0.f);
   }
 }
 
-// Deferred shading of one pixel for one light (L114): the pixel is projected back to 3-D at its
-// composited depth, camera -> world: x = R^T (x_c - t).
-__device__ __forceinline__ void shade_pixel(const ShadeIn& q, const float lsss[3], float lin,
-                                            float A, int px, int py, const CamParams& cam,
+__device__ __forceinline__ void shade_point(const ShadeIn& q, const float lsss[3], float lin, float A,
+                                            const float xw[3], const CamParams& cam,
                                             const LightParams& lt, float rgb[3], float dif[3],
-                                            float spc[3], bool with_bg = true) {
-  const float xc0 = ((float)px - cam.cx) / cam.fx * q.depth - cam.t[0];
-  const float xc1 = ((float)py - cam.cy) / cam.fy * q.depth - cam.t[1];
-  const float xc2 = q.depth - cam.t[2];
-  float xw[3];
+                                            float spc[3], bool with_bg) {
+  ShadeView s;
+  shade_view(q, xw, cam, s);
+  shade_light(s, lsss, lin, A, cam, lt, rgb, dif, spc, with_bg);
+}
+
+// Deferred shading of one pixel (L114): the pixel is projected back to 3-D at its composited depth,
+// camera -> world: x = R^T (x_c - t).
+__device__ __forceinline__ void backproject(float depth, int px, int py, const CamParams& cam, float xw[3]) {
+  const float xc0 = ((float)px - cam.cx) / cam.fx * depth - cam.t[0];
+  const float xc1 = ((float)py - cam.cy) / cam.fy * depth - cam.t[1];
+  const float xc2 = depth - cam.t[2];
 #pragma unroll
   for (int k = 0; k < 3; ++k) xw[k] = cam.R[0 + k] * xc0 + cam.R[3 + k] * xc1 + cam.R[6 + k] * xc2;
-  shade_point(q, lsss, lin, A, xw, cam, lt, rgb, dif, spc, with_bg);
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -271,6 +319,12 @@ __device__ __forceinline__ void raster_finish(float acc_depth, const f32x2* pacc
   q.depth = acc[0] * iA; q.nx = acc[1] * iA; q.ny = acc[2] * iA; q.nz = acc[3] * iA;
   q.br = acc[4] * iA; q.bg = acc[5] * iA; q.bb = acc[6] * iA;
   q.rough = acc[7] * iA; q.metal = acc[8] * iA; q.sss = acc[9] * iA;
+  ShadeView sv;  // light-independent part of the shading, once per pixel
+  {
+    float xw[3];
+    backproject(q.depth, px, py, cam, xw);
+    shade_view(q, xw, cam, sv);
+  }
   float sum[3] = {0.f, 0.f, 0.f};  // SSSGS_SUM_LIGHTS: this lane's share of the sum over the lights
 #pragma unroll
   for (int l = 0; l < LB; ++l) {
@@ -287,7 +341,7 @@ __device__ __forceinline__ void raster_finish(float acc_depth, const f32x2* pacc
     float rgb[3], dif[3] = {0.f, 0.f, 0.f}, spc[3] = {0.f, 0.f, 0.f};
     if (covered) {
       const float lsss[3] = {accl[l][0] * iA, accl[l][1] * iA, accl[l][2] * iA};
-      shade_pixel(q, lsss, accl[l][3] * iA, A, px, py, cam, lights.l[l], rgb, dif, spc, sum_mode == 0);
+      shade_light(sv, lsss, accl[l][3] * iA, A, cam, lights.l[l], rgb, dif, spc, sum_mode == 0);
     } else {
       rgb[0] = cam.bg[0]; rgb[1] = cam.bg[1]; rgb[2] = cam.bg[2];
     }
@@ -766,6 +820,8 @@ int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers&
 }
 
 namespace {
+// staging buffer of one warp and one 16-entry step of the cached walk: rows [16][4 * RPG] float4 + weights
+__host__ __device__ constexpr int cached_buf_bytes(int lb) { return (kWcChunk / 2) * (4 * ((lb + 4 + 3) / 4)) * 16 + (kWcChunk / 2) * 32 * 4; }
 // Per-light walk of a sweep over the weight cache: one warp per 8x4-pixel block streams the block's
 // chain -- per entry (Gaussian id, depth) and the 32 weights -- and blends the entry's channels,
 // fetched with warp-uniform loads (a Gaussian's rows are shared by neighbouring blocks and tiles: L1 /
@@ -787,70 +843,130 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
   const int py = ty * kTile + (warp / WPR) * S::PH + lane / S::PW;
   const bool inside = px < cam.width && py < cam.height;
 
-  float acc_depth = 0.f;
-  f32x2 pacc[5], paccl[LB][2];
+  // Blend layout: an entry is 4 * RPG float4 "rows" of channels (3 attribute rows, LB MLP rows, one row
+  // holding the depth, padding) and 32 weights.  A lane owns 4 pixels x RPG rows (lane = pixel group * 4
+  // + row group), so an entry costs it 1 + RPG 16-byte shared-memory loads for 8 * RPG packed FMAs --
+  // the one-pixel-per-lane layout needs 3 + LB broadcast loads for the same FMAs per lane and is bound
+  // by the shared-memory return path.  Every (pixel, channel) sum is still one fma per entry in list
+  // order: bit-identical to the list walk.  The sums are transposed to one pixel per lane at the end.
+  constexpr int RPG = (LB + 4 + 3) / 4;
+  constexpr int NR4 = 4 * RPG;
+  constexpr int H = kWcChunk / 2;
+  constexpr int kBufBytes = cached_buf_bytes(LB);
+  static_assert(kBufBytes == H * NR4 * 16 + H * 32 * 4, "staging buffer size");
+  static_assert(32 * (NR4 + 1) * 16 <= 2 * kBufBytes, "transpose fits in the warp's staging buffers");
+  const int pg = lane >> 2, cg = lane & 3;
+  f32x2 acc[4][2 * RPG];
 #pragma unroll
-  for (int c = 0; c < 5; ++c) pacc[c] = make_float2(0.f, 0.f);
+  for (int q = 0; q < 4; ++q)
 #pragma unroll
-  for (int l = 0; l < LB; ++l) paccl[l][0] = paccl[l][1] = make_float2(0.f, 0.f);
+    for (int c = 0; c < 2 * RPG; ++c) acc[q][c] = make_float2(0.f, 0.f);
 
-  // Per warp and chunk of 32 entries: lane k gathers the rows (3 attribute float4 + LB MLP float4) of
-  // entry k and every lane fetches an eighth of the chunk's 4 KB of weights -- 11-19 independent
-  // loads per lane issued back to back, one memory latency per chunk -- into this warp's shared
-  // memory; the entries are then blended from broadcast (rows) and conflict-free (weights) reads.
-  constexpr int NR = 3 + LB;
-  constexpr int kWarpBytes = NR * kWcChunk * 16 + kWcChunk * 32 * 4;
+  // The chain is staged in steps of 16 entries (half a cache chunk), double-buffered in this warp's
+  // shared memory with cp.async: the rows of the step's entries are gathered by (entry = lane % 16,
+  // every other row by lane / 16), its 2 KB of weights copied 4 x 16 B per lane; step j+1 is in flight
+  // while step j is blended.  Headers and chunk links run one and two chunks ahead of the walk.
   extern __shared__ float4 s_dyn[];
-  float4 (*s_rows)[kWcChunk] = reinterpret_cast<float4 (*)[kWcChunk]>(reinterpret_cast<char*>(s_dyn) + warp * kWarpBytes);
-  float* s_w = reinterpret_cast<float*>(s_rows + NR);  // [entry][pixel]
+  char* s_warp = reinterpret_cast<char*>(s_dyn) + warp * 2 * kBufBytes;
 
   const uint32_t n_items = wc.count[tile * 8 + warp];
+  const uint32_t n_steps = (n_items + H - 1) / H, n_chunks = (n_items + kWcChunk - 1) / kWcChunk;
   uint32_t chunk = n_items ? wc.head[tile * 8 + warp] : 0u;
-  uint2 hdr_pre = (uint32_t)lane < n_items ? wc.hdr[(size_t)chunk * kWcChunk + lane] : make_uint2(0u, 0u);
-  for (uint32_t i0 = 0; i0 < n_items; i0 += kWcChunk) {
-    const uint32_t m = min((uint32_t)kWcChunk, n_items - i0);
-    const uint2 my_hdr = hdr_pre;
-    const bool more = i0 + kWcChunk < n_items;
-    const uint32_t nxt = more ? wc.next[chunk] : 0u;
-    // the next chunk's headers are fetched a chunk ahead (they gate its gathers)
-    if (more && i0 + kWcChunk + lane < n_items) hdr_pre = wc.hdr[(size_t)nxt * kWcChunk + lane];
-    __syncwarp();  // every lane has left the previous chunk's staging
-    {
-      const float4* wsrc = reinterpret_cast<const float4*>(wc.weights + (size_t)chunk * kWcChunk * 32);
-      float4 wv[8];
+  uint32_t nxt = n_chunks > 1 ? wc.next[chunk] : 0u;
+  uint2 hdr_cur = (uint32_t)lane < n_items ? wc.hdr[(size_t)chunk * kWcChunk + lane] : make_uint2(0u, 0u);
+  uint2 hdr_nxt = (uint32_t)(kWcChunk + lane) < n_items ? wc.hdr[(size_t)nxt * kWcChunk + lane] : make_uint2(0u, 0u);
+  uint32_t nxt2 = n_chunks > 2 ? wc.next[nxt] : 0u;
+
+  auto stage = [&](uint32_t j, uint2 hdr_of_lane, uint32_t chunk_id) {
+    const uint32_t m = min((uint32_t)H, n_items - j * H);
+    const uint32_t e = lane & (H - 1), part = lane / H, half = j & 1u;
+    const size_t g = __shfl_sync(0xFFFFFFFFu, hdr_of_lane.x, half * H + e);
+    const float depth = __uint_as_float(__shfl_sync(0xFFFFFFFFu, hdr_of_lane.y, half * H + e));
+    char* buf = s_warp + half * kBufBytes;
+    float4* rows = reinterpret_cast<float4*>(buf) + e * NR4;
+    if (e < m) {
 #pragma unroll
-      for (int q = 0; q < 8; ++q) wv[q] = (uint32_t)(q * 4 + lane / 8) < m ? wsrc[q * 32 + lane] : make_float4(0.f, 0.f, 0.f, 0.f);
-      if (lane < m) {
-        const size_t g = my_hdr.x;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) s_rows[c][lane] = attr[3 * g + c];
-#pragma unroll
-        for (int l = 0; l < LB; ++l) s_rows[3 + l][lane] = mlp_out[g * n_lights + min(l, n_lights - 1)];
+      for (int r = 0; r < 3 + LB; ++r) {
+        if ((r & 1) != (int)part) continue;
+        const float4* src = r < 3 ? attr + 3 * g + r : mlp_out + g * n_lights + min(r - 3, n_lights - 1);
+        cp_async16(rows + r, src);
       }
-#pragma unroll
-      for (int q = 0; q < 8; ++q) reinterpret_cast<float4*>(s_w)[q * 32 + lane] = wv[q];
+      if (part == 0) rows[3 + LB] = make_float4(depth, 0.f, 0.f, 0.f);
     }
-    __syncwarp();
+    float4* w4 = reinterpret_cast<float4*>(buf + H * NR4 * 16);
+    const float4* wsrc = reinterpret_cast<const float4*>(wc.weights + ((size_t)chunk_id * kWcChunk + half * H) * 32);
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if ((uint32_t)(q * 4 + lane / 8) < m) cp_async16(&w4[q * 32 + lane], wsrc + q * 32 + lane);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  if (n_steps) stage(0, hdr_cur, chunk);
+  for (uint32_t j = 0; j < n_steps; ++j) {
+    const uint32_t half = j & 1u;
+    if (j + 1 < n_steps) {
+      if (half) stage(j + 1, hdr_nxt, nxt);
+      else stage(j + 1, hdr_cur, chunk);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncwarp();  // the step's copies of all lanes have landed
+    const uint32_t m = min((uint32_t)H, n_items - j * H);
+    const char* buf = s_warp + half * kBufBytes;
+    const float4* s_rows = reinterpret_cast<const float4*>(buf) + cg * RPG;       // [entry][NR4]
+    const float4* s_w4 = reinterpret_cast<const float4*>(buf + H * NR4 * 16) + pg;  // [entry][8]
 #pragma unroll 4
     for (uint32_t k = 0; k < m; ++k) {
-      const float depth = __uint_as_float(__shfl_sync(0xFFFFFFFFu, my_hdr.y, k));
-      const float w = s_w[k * 32 + lane];
-      const float4 a0 = s_rows[0][k], a1 = s_rows[1][k], a2 = s_rows[2][k];
-      const f32x2 ww = make_float2(w, w);
-      acc_depth = fmaf(w, depth, acc_depth);
-      fma2(pacc[0], ww, a0.x, a0.y);
-      fma2(pacc[1], ww, a0.z, a0.w);
-      fma2(pacc[2], ww, a1.x, a1.y);
-      fma2(pacc[3], ww, a1.z, a1.w);
-      fma2(pacc[4], ww, a2.x, a2.y);
+      const float4 wv = s_w4[k * 8];
+      const float w[4] = {wv.x, wv.y, wv.z, wv.w};
+      float4 c[RPG];
 #pragma unroll
-      for (int l = 0; l < LB; ++l) {
-        const float4 mo = s_rows[3 + l][k];
-        fma2(paccl[l][0], ww, mo.x, mo.y);
-        fma2(paccl[l][1], ww, mo.z, mo.w);
+      for (int r = 0; r < RPG; ++r) c[r] = s_rows[k * NR4 + r];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const f32x2 ww = make_float2(w[q], w[q]);
+#pragma unroll
+        for (int r = 0; r < RPG; ++r) {
+          fma2(acc[q][2 * r], ww, c[r].x, c[r].y);
+          fma2(acc[q][2 * r + 1], ww, c[r].z, c[r].w);
+        }
       }
     }
-    chunk = nxt;
+    __syncwarp();  // every lane has left this buffer before step j+2 is copied into it
+    if (half) {
+      const uint32_t ci = j / 2 + 1;  // index of the chunk the walk enters now
+      chunk = nxt; hdr_cur = hdr_nxt; nxt = nxt2;
+      hdr_nxt = (ci + 1) * kWcChunk + lane < n_items ? wc.hdr[(size_t)nxt * kWcChunk + lane] : make_uint2(0u, 0u);
+      nxt2 = ci + 2 < n_chunks ? wc.next[nxt] : 0u;
+    }
+  }
+
+  // transpose: (4 pixels x RPG rows) per lane -> all rows of one pixel per lane
+  float acc_depth;
+  f32x2 pacc[5], paccl[LB][2];
+  {
+    float4* t4 = reinterpret_cast<float4*>(s_warp);
+    constexpr int TS = NR4 + 1;  // padded pixel stride: conflict-free 16-byte reads
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+#pragma unroll
+      for (int r = 0; r < RPG; ++r)
+        t4[(4 * pg + q) * TS + cg * RPG + r] =
+            make_float4(acc[q][2 * r].x, acc[q][2 * r].y, acc[q][2 * r + 1].x, acc[q][2 * r + 1].y);
+    __syncwarp();
+    const float4* mine = t4 + lane * TS;
+    const float4 a0 = mine[0], a1 = mine[1], a2 = mine[2];
+    pacc[0] = make_float2(a0.x, a0.y); pacc[1] = make_float2(a0.z, a0.w);
+    pacc[2] = make_float2(a1.x, a1.y); pacc[3] = make_float2(a1.z, a1.w);
+    pacc[4] = make_float2(a2.x, a2.y);
+#pragma unroll
+    for (int l = 0; l < LB; ++l) {
+      const float4 mo = mine[3 + l];
+      paccl[l][0] = make_float2(mo.x, mo.y);
+      paccl[l][1] = make_float2(mo.z, mo.w);
+    }
+    acc_depth = mine[3 + LB].x;
   }
   const float T = inside ? wc.T[(int64_t)py * cam.width + px] : 1.f;
   raster_finish<LB, 1, false>(acc_depth, pacc, paccl, 0.f, T, inside, px, py, 0, cam, lights, n_lights, rgb_out,
@@ -866,7 +982,7 @@ int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_l
   if (tiles == 0) return 0;
 #define SSSGS_CACHED(LB)                                                                                \
   do {                                                                                                  \
-    constexpr int smem = 8 * ((3 + LB) * kWcChunk * 16 + kWcChunk * 32 * 4);                            \
+    constexpr int smem = 8 * 2 * cached_buf_bytes(LB);                                                  \
     static bool configured = false;                                                                     \
     if (!configured) {                                                                                  \
       if (cudaFuncSetAttribute(raster_cached_kernel<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
