@@ -16,7 +16,10 @@
 //  Parity status of the readings that cannot be pinned from the paper
 //  ("parity unpinned"): S1 (which 2 rotation components feed the MLP),
 //  S8 (choice of D/F/G lobes and the factor 4 in Eq. 4), S10 (coverage normalisation
-//  before shading).  Every function below is otherwise pinned by tests/test_oracle_*.py
+//  before shading), and the ray rule of orc_bake_visibility (the paper only says rays are
+//  traced "similar to [10]": where along the ray a Gaussian acts, the opacity rule and the
+//  ray offset t_min are this build's reading; its arithmetic IS pinned).
+//  Every function below is otherwise pinned by tests/test_oracle_*.py
 //  against closed forms, invariants, library special cases or brute force.
 // =====================================================================================
 #include <algorithm>
@@ -642,6 +645,99 @@ void orc_shade_f32(int width, int height, const OrcCamera* cam, const float* lig
                    const float* light_intensity, const double* gbuf, float* rgb, float* aov_d,
                    float* aov_s) {
   shade_impl<float>(width, height, cam, light_pos, light_intensity, gbuf, rgb, aov_d, aov_s);
+}
+
+}  // extern "C"
+
+extern "C" {
+
+// ---------------------------------------------------------------------------------------------
+// Ray-traced per-Gaussian visibility and its SH fit ("we trace
+// rays using a BVH to quickly estimate the visibility for each Gaussian and learn this as a per
+// Gaussian SH visibility term v"; L81: "efficient ray-tracing for 3D GS").  The paper gives no
+// formula; the reading is the one of its reference [10]: along the ray
+// x(t) = mu_i + (t_min + t) w, t >= 0, every other Gaussian j acts at the point of its largest
+// response, with the opacity rule of the rasteriser (Eq. 3: alpha = o * falloff, capped,
+// thresholded), and the transmittances multiply:
+//   m2_ij  = min_{t >= 0} (x(t) - mu_j)^T Sigma_j^-1 (x(t) - mu_j)
+//   a_ij   = min(0.99, o_j exp(-m2_ij / 2)), counted iff a_ij >= 1/255
+//   V_i(w) = prod_{j != i} (1 - a_ij), set to 0 below 1e-4 (the product is order independent)
+//   c_i,lm = sum_k weight_k V_i(w_k) Y_lm(w_k)      (quadrature of the SH projection, degree <= 1,
+//            real basis and order of the render path: Y00, Y1-1 ~ y, Y10 ~ z, Y11 ~ x)
+// Brute force over all pairs, in double; no BVH here: the tree only prunes pairs whose a_ij is
+// below the threshold.  `unstable` counts, per ray, the pairs whose a_ij lies within 1e-4 relative
+// of 1/255 plus one if the product lies within 1e-2 relative of 1e-4 (a float evaluation may
+// decide these the other way).
+void orc_bake_visibility(int64_t n, const float* means, const float* scales, const float* rotations,
+                         const float* opacities, int n_dirs, const float* dirs, const float* weights,
+                         float t_min, int sh_degree, double* sh_out, double* vis_out,
+                         int32_t* unstable) {
+  const int nc = (sh_degree + 1) * (sh_degree + 1);
+  std::vector<double> Sinv((size_t)n * 9);
+  for (int64_t j = 0; j < n; ++j) {
+    const double qr = rotations[4 * j], qx = rotations[4 * j + 1], qy = rotations[4 * j + 2],
+                 qz = rotations[4 * j + 3];
+    double R[9];
+    R[0] = 1 - 2 * (qy * qy + qz * qz); R[1] = 2 * (qx * qy - qr * qz); R[2] = 2 * (qx * qz + qr * qy);
+    R[3] = 2 * (qx * qy + qr * qz); R[4] = 1 - 2 * (qx * qx + qz * qz); R[5] = 2 * (qy * qz - qr * qx);
+    R[6] = 2 * (qx * qz - qr * qy); R[7] = 2 * (qy * qz + qr * qx); R[8] = 1 - 2 * (qx * qx + qy * qy);
+    // Sigma = R S^2 R^T  =>  Sigma^-1 = R S^-2 R^T
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) {
+        double s = 0;
+        for (int k = 0; k < 3; ++k) {
+          const double sk = scales[3 * j + k];
+          s += R[3 * a + k] * R[3 * b + k] / (sk * sk);
+        }
+        Sinv[9 * j + 3 * a + b] = s;
+      }
+  }
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t i = 0; i < n; ++i) {
+    double c[4] = {0, 0, 0, 0};
+    for (int k = 0; k < n_dirs; ++k) {
+      const double w[3] = {dirs[3 * k], dirs[3 * k + 1], dirs[3 * k + 2]};
+      double o[3];
+      for (int a = 0; a < 3; ++a) o[a] = (double)means[3 * i + a] + (double)t_min * w[a];
+      double T = 1.0;
+      int flips = 0;
+      for (int64_t j = 0; j < n; ++j) {
+        if (j == i) continue;
+        const double* S = &Sinv[9 * j];
+        double d[3], Sw[3], Sd[3];
+        for (int a = 0; a < 3; ++a) d[a] = o[a] - (double)means[3 * j + a];
+        for (int a = 0; a < 3; ++a) {
+          Sw[a] = S[3 * a] * w[0] + S[3 * a + 1] * w[1] + S[3 * a + 2] * w[2];
+          Sd[a] = S[3 * a] * d[0] + S[3 * a + 1] * d[1] + S[3 * a + 2] * d[2];
+        }
+        const double ww = w[0] * Sw[0] + w[1] * Sw[1] + w[2] * Sw[2];
+        const double wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
+        double t = -wd / ww;  // minimiser of the quadratic along the line
+        if (t < 0) t = 0;
+        double e[3], Se[3];
+        for (int a = 0; a < 3; ++a) e[a] = d[a] + t * w[a];
+        for (int a = 0; a < 3; ++a) Se[a] = S[3 * a] * e[0] + S[3 * a + 1] * e[1] + S[3 * a + 2] * e[2];
+        const double m2 = e[0] * Se[0] + e[1] * Se[1] + e[2] * Se[2];
+        double a_ij = (double)opacities[j] * std::exp(-0.5 * m2);
+        if (std::fabs(a_ij * 255.0 - 1.0) < 1e-4) ++flips;
+        if (a_ij < 1.0 / 255.0) continue;
+        if (a_ij > 0.99) a_ij = 0.99;
+        T *= 1.0 - a_ij;
+      }
+      if (std::fabs(T * 1e4 - 1.0) < 1e-2) ++flips;
+      const double V = T >= 1e-4 ? T : 0.0;
+      if (vis_out) vis_out[i * n_dirs + k] = V;
+      if (unstable) unstable[i * n_dirs + k] = flips;
+      const double wk = weights[k];
+      c[0] += wk * V * 0.2820948;
+      if (nc == 4) {
+        c[1] += wk * V * 0.4886025 * w[1];
+        c[2] += wk * V * 0.4886025 * w[2];
+        c[3] += wk * V * 0.4886025 * w[0];
+      }
+    }
+    for (int m = 0; m < nc; ++m) sh_out[i * nc + m] = c[m];
+  }
 }
 
 }  // extern "C"
