@@ -200,6 +200,32 @@ int sssgs_render_host(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp*
                       const sssgs_camera* cams, int n_cam, const sssgs_light* lights, int n_light,
                       const sssgs_out* out, uint32_t flags);
 
+/* Ray-traced per-Gaussian visibility and its SH fit ("we trace
+ * rays using a BVH to quickly estimate the visibility for each Gaussian and learn this as a per
+ * Gaussian SH visibility term v"; L81).  Produces the `vis_sh` input of sssgs_gaussians.  For every
+ * Gaussian i and direction w_k the ray x(t) = mu_i + (t_min + t) w_k, t >= 0, is traced through a
+ * BVH over the alpha >= 1/255 supports of all Gaussians; every other Gaussian j acts at the point of
+ * its largest response along the ray, with the opacity rule of the rasteriser (Eq. 3):
+ *   m2 = min_{t>=0} (x(t)-mu_j)^T Sigma_j^-1 (x(t)-mu_j),  a = min(0.99, o_j exp(-m2/2)) iff >= 1/255,
+ *   V_i(w_k) = prod_{j != i} (1 - a), set to 0 below 1e-4;
+ *   vis_sh_out[i][lm] = sum_k weights[k] V_i(w_k) Y_lm(w_k)   (basis and order of vis_sh above).
+ * Only means, scales, rotations and opacities of `g` are read (device pointers, n <=
+ * max_gaussians).  The call enqueues on `stream`, never synchronises and uses the context's
+ * workspace: it must not overlap a render on the same context (same stream, or ordered by the
+ * caller).  The tree and the traversal order are deterministic: results are bit-reproducible.
+ * Errors: SSSGS_EINVAL (NULL / n_dirs < 1 or > 4096 / sh_degree not 0 or 1 / t_min < 0 or not
+ * finite), SSSGS_ECAPACITY (n > max_gaussians), SSSGS_ECUDA.                                   */
+typedef struct {
+  int n_dirs;            /* K                                                                 */
+  const float* dirs;     /* [K,3] unit vectors (device)                                       */
+  const float* weights;  /* [K] quadrature weights, e.g. 4 pi / K (device)                    */
+  float t_min;           /* ray start offset from the Gaussian's centre, world units          */
+  int sh_degree;         /* 0 or 1                                                            */
+  float* vis_sh_out;     /* [n,(deg+1)^2] (device), required                                  */
+  float* vis_out;        /* [n,K] raw visibilities (device), may be NULL                      */
+} sssgs_bake;
+int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_bake* bake, void* stream);
+
 /* Per-stage device timing (measurement aid, off by default).  When enabled, sssgs_render
  * records CUDA events around each stage on the caller's stream (not capture-safe while on);
  * sssgs_profile_read synchronises those events and writes the milliseconds each stage of the

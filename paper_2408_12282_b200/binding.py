@@ -32,7 +32,7 @@ CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
-           "sssgs_profile_enable", "sssgs_profile_read"]
+           "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility"]
 STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster"]
 
 _f = ctypes.c_float
@@ -77,6 +77,11 @@ class sssgs_out(ctypes.Structure):
                 ("counters", _vp)]
 
 
+class sssgs_bake(ctypes.Structure):
+    _fields_ = [("n_dirs", ctypes.c_int), ("dirs", _vp), ("weights", _vp), ("t_min", _f),
+                ("sh_degree", ctypes.c_int), ("vis_sh_out", _vp), ("vis_out", _vp)]
+
+
 class SssgsError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__(f"libsssgs error {code}: {msg}")
@@ -107,6 +112,8 @@ def lib() -> ctypes.CDLL:
         L.sssgs_render.argtypes = render_args + [_vp]
         L.sssgs_render_host.restype = ctypes.c_int
         L.sssgs_render_host.argtypes = render_args
+        L.sssgs_bake_visibility.restype = ctypes.c_int
+        L.sssgs_bake_visibility.argtypes = [_vp, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_bake), _vp]
         L.sssgs_last_launch_count.restype = ctypes.c_int64
         L.sssgs_last_launch_count.argtypes = [_vp]
         L.sssgs_profile_enable.restype = ctypes.c_int
@@ -149,6 +156,10 @@ def sssgs_render(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0, stream
 def sssgs_render_host(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0) -> None:
     _check(ctx, lib().sssgs_render_host(ctx, ctypes.byref(g), ctypes.byref(mlp), cams, n_cam, lights,
                                         n_light, ctypes.byref(out), flags))
+
+
+def sssgs_bake_visibility(ctx, g, bake, stream=None) -> None:
+    _check(ctx, lib().sssgs_bake_visibility(ctx, ctypes.byref(g), ctypes.byref(bake), _vp(stream or 0)))
 
 
 def sssgs_last_launch_count(ctx) -> int:
@@ -305,6 +316,25 @@ class Renderer:
                      (SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0) | (SSSGS_SUM_LIGHTS if sum_lights else 0) |
                      (SSSGS_FORWARD_SHADING if forward else 0), st)
         return outputs
+
+    def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None):
+        """Enqueue one sssgs_bake_visibility on the current torch stream.  dirs [K,3], weights [K] (numpy or
+        device tensors).  Returns (vis_sh [n,(deg+1)^2], vis [n,K] or None), device tensors."""
+        torch = self.torch
+        def dev(a):
+            return a if torch.is_tensor(a) else torch.from_numpy(np.ascontiguousarray(a, np.float32)).to(self.device)
+        self._bake_in = (dev(dirs).reshape(-1, 3).contiguous(), dev(weights).reshape(-1).contiguous())
+        K = int(self._bake_in[0].shape[0])
+        nc = (sh_degree + 1) ** 2
+        sh = torch.zeros((max(self.n, 1), nc), dtype=torch.float32, device=self.device)
+        vis = torch.zeros((max(self.n, 1), K), dtype=torch.float32, device=self.device) if want_vis else None
+        b = sssgs_bake()
+        b.n_dirs, b.dirs, b.weights = K, self._bake_in[0].data_ptr(), self._bake_in[1].data_ptr()
+        b.t_min, b.sh_degree = float(t_min), int(sh_degree)
+        b.vis_sh_out, b.vis_out = sh.data_ptr(), (vis.data_ptr() if want_vis else None)
+        st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
+        sssgs_bake_visibility(self.ctx, self.g, b, st)
+        return sh[:self.n], (vis[:self.n] if want_vis else None)
 
     def launch_count(self) -> int:
         return sssgs_last_launch_count(self.ctx)

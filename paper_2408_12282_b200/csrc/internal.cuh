@@ -128,6 +128,7 @@ enum {
   DC_CONTRIB_ROWS = 25,  // Gaussians kept by the visibility pre-pass (MLP rows of a sweep)
   DC_WC_CHUNKS = 26,     // weight cache: chunks handed out
   DC_WC_OVERFLOW = 27,   // weight cache: 1 if the pool ran out (the sweep then walks the lists again)
+  DC_BVH_BOUNDS = 32,    // 6 words: box of the centres (sssgs_bake_visibility)
   DC_WORDS = 64
 };
 
@@ -239,6 +240,24 @@ int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_l
                          const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
                          int64_t frame_stride_px, int sum_mode, cudaStream_t s);
 int raster_reads_unblended_rows(int tiles);
+// BVH of sssgs_bake_visibility (k_bvh.cu); nodes: internal 0 .. n-2 (root 0), leaf of sorted position k = n-1+k
+struct BvhBuffers {
+  uint32_t* code_of;       // [n] Morton code of Gaussian g
+  uint32_t* sorted_codes;  // [n] codes in sorted order
+  uint32_t* sorted_gid;    // [n] Gaussian index of sorted position k
+  float4* leaf;            // [3n] (mu, o), (Sigma^-1 xx xy xz yy), (yz zz, cut-off, index)
+  float4* box_lo;          // [2n-1] (min xyz, left child)
+  float4* box_hi;          // [2n-1] (max xyz, right child)
+  int* parent;             // [2n-1]
+  uint32_t* flags;         // [n-1] refit arrival counters, zeroed by the caller
+};
+int launch_bvh_bounds(int64_t n, const float* means, uint32_t* bounds, int max_blocks, cudaStream_t s);
+int launch_bvh_morton(int64_t n, const float* means, const uint32_t* bounds, uint32_t* keys, uint32_t* vals,
+                      uint32_t* code_of, uint32_t* hist, int max_blocks, cudaStream_t s);
+int launch_bvh_build(const sssgs_gaussians& g, const BvhBuffers& b, const uint32_t* depth_hist,
+                     const uint32_t* vals0, const uint32_t* vals1, cudaStream_t s);
+int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* dirs, const float* weights, float t_min,
+                     int n_coef, float* sh_out, float* vis_out, cudaStream_t s);
 int launch_compact_contrib(const uint8_t* contrib, int64_t n, uint32_t* rows, uint32_t* count,
                            int zero_rest, float4* out0, float4* out1, int lights, cudaStream_t s);
 int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,

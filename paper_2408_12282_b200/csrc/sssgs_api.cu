@@ -342,6 +342,56 @@ int sssgs_profile_read(sssgs_ctx* c, float* stage_ms, int* stage_launches) {
   return SSSGS_OK;
 }
 
+// BVH build + ray-traced visibility + SH fit.  The tree lives in workspace regions a
+// render rewrites before reading (attribute pack, projection records, MLP outputs, tile rects), so a
+// bake needs no memory of its own and leaves nothing a later render depends on.
+int sssgs_bake_visibility(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_bake* b, void* cuda_stream) {
+  if (!c) return SSSGS_EINVAL;
+  if (!g || !b) return fail(c, SSSGS_EINVAL, "NULL argument");
+  if (g->n < 0) return fail(c, SSSGS_EINVAL, "n < 0");
+  if (g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n %lld > max_gaussians %lld", (long long)g->n, (long long)c->cfg.max_gaussians);
+  if (b->n_dirs < 1 || b->n_dirs > 4096) return fail(c, SSSGS_EINVAL, "n_dirs must be in [1,4096]");
+  if (b->sh_degree < 0 || b->sh_degree > 1) return fail(c, SSSGS_EINVAL, "sh_degree must be 0 or 1");
+  if (!(b->t_min >= 0.f) || b->t_min > 3.0e38f) return fail(c, SSSGS_EINVAL, "t_min must be finite and >= 0");
+  if (!b->dirs || !b->weights || !b->vis_sh_out) return fail(c, SSSGS_EINVAL, "dirs / weights / vis_sh_out is NULL");
+  if (!aligned16(b->vis_sh_out)) return fail(c, SSSGS_EINVAL, "vis_sh_out is not 16-byte aligned");
+  c->launches = 0;
+  if (g->n == 0) return SSSGS_OK;
+  if (!g->means || !g->scales || !g->rotations || !g->opacities) return fail(c, SSSGS_EINVAL, "means / scales / rotations / opacities is NULL");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (c->upload_pending) {  // a preceding sssgs_render_host may still be uploading on the copy stream
+    if (cudaStreamWaitEvent(s, c->ev_upload, 0) != cudaSuccess) return fail(c, SSSGS_ECUDA, "stream wait failed");
+  }
+  const int64_t n = g->n;
+  BvhBuffers bb;
+  bb.code_of = c->rows;
+  bb.sorted_codes = c->gb.dkeys[0];  // free once the codes are sorted (only the index array is read)
+  bb.sorted_gid = c->gb.dkeys[1];
+  bb.leaf = c->attr;                 // 48 B per Gaussian
+  bb.box_lo = c->gb.rec_a;           // rec_a + rec_b are adjacent: 32 B per Gaussian
+  bb.box_hi = c->mlp_out[0];         // mlp_out[0] + mlp_out[1] are adjacent: >= 32 B per Gaussian
+  bb.parent = (int*)c->gb.rect;      // 8 B per Gaussian
+  bb.flags = c->gb.touched;
+  uint32_t* cnt = c->gb.counters;
+  const int max_blocks = c->num_sms * 4;
+  if (cudaMemsetAsync(c->control, 0, c->control_bytes, s) != cudaSuccess ||
+      cudaMemsetAsync(bb.flags, 0, (size_t)n * 4, s) != cudaSuccess)
+    return fail(c, SSSGS_ECUDA, "memset failed");
+  int launches = 0;
+  launches += launch_bvh_bounds(n, g->means, cnt + DC_BVH_BOUNDS, max_blocks, s);
+  launches += launch_bvh_morton(n, g->means, cnt + DC_BVH_BOUNDS, c->gb.dkeys[0], c->gb.dvals[0], bb.code_of,
+                                c->gb.hist, max_blocks, s);
+  for (int p = 0; p < 4; ++p)
+    launches += launch_depth_pass(c->gb.dkeys, c->gb.dvals, (uint32_t)n, p, c->gb.hist, c->status_depth[p],
+                                  cnt + DC_TICKET_BASE + p, cnt + DC_SORT_ERROR, max_blocks, s);
+  launches += launch_bvh_build(*g, bb, c->gb.hist, c->gb.dvals[0], c->gb.dvals[1], s);
+  launches += launch_bvh_trace(n, bb, b->n_dirs, b->dirs, b->weights, b->t_min, (b->sh_degree + 1) * (b->sh_degree + 1),
+                               b->vis_sh_out, b->vis_out, s);
+  c->launches = launches;
+  if (cudaGetLastError() != cudaSuccess) return fail(c, SSSGS_ECUDA, "a bake kernel launch failed");
+  return SSSGS_OK;
+}
+
 const char* sssgs_last_error(const sssgs_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
 int64_t sssgs_last_launch_count(const sssgs_ctx* c) { return c ? c->launches : 0; }
 
