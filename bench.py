@@ -328,6 +328,58 @@ def run_gpu(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def fibonacci_dirs(K):
+    k = np.arange(K) + 0.5
+    z = 1 - 2 * k / K
+    phi = k * np.pi * (3 - np.sqrt(5))
+    r = np.sqrt(1 - z * z)
+    return np.stack([r * np.cos(phi), r * np.sin(phi), z], 1).astype(np.float32), np.full(K, 4 * np.pi / K, np.float32)
+
+
+def run_bake(args, local_rank):
+    """--bake K: times sssgs_bake_visibility on the config's Gaussians, K Fibonacci directions.
+    A side measurement: its JSON line has its own metric (rays/s) and is not the headline."""
+    import torch
+    from paper_2408_12282_b200 import binding
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    scene, cams, lights, fps = workload(args.config)
+    K, t_min = args.bake, 0.05
+    dirs, wts = fibonacci_dirs(K)
+    R = binding.Renderer(scene, max_instances=int(20 * scene.n), device=local_rank)
+    d_dirs, d_wts = torch.from_numpy(dirs).to(dev), torch.from_numpy(wts).to(dev)
+    for _ in range(max(args.warmup, 3)):
+        sh, _ = R.bake_visibility(d_dirs, d_wts, t_min)
+    torch.cuda.synchronize()
+    launches = R.launch_count()
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        sh, _ = R.bake_visibility(d_dirs, d_wts, t_min)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle   # cpu_baseline leg only
+        rows = np.random.default_rng(0).choice(scene.n, size=min(scene.n, max(8, int(2e9 / (scene.n * K)))), replace=False)
+        t0 = time.perf_counter()
+        oracle.bake_visibility(scene, dirs, wts, t_min, rows=rows)
+        dt = time.perf_counter() - t0
+        cpu = {"value": len(rows) * K / dt / 1e6, "unit": "Mrays/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{len(rows)} of {scene.n} Gaussians x {K} directions, brute force over all pairs, {dt:.1f} s"}
+    R.close()
+    print(json.dumps({"metric": "Mrays/s (BVH build + traversal + SH fit)", "value": scene.n * K / ms / 1e3, "unit": "Mrays/s",
+                      "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                      "higher_is_better": True, "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"configs[{args.config - 1}] {scene.name}", "gaussians": scene.n, "dirs": K,
+                                 "t_min": t_min, "l2": "flushed between timed steps (256 MiB memset)"},
+                      "gpu_launches": launches * args.steps, "cpu_baseline": cpu}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -340,6 +392,8 @@ def main():
                     help="the paper's 'w/o deferred' variant (SSSGS_FORWARD_SHADING): Eq. 7 per Gaussian, RGB composited")
     ap.add_argument("--sum-lights", action="store_true",
                     help="image-based-lighting mode (SSSGS_SUM_LIGHTS): the lights of a step are summed into one frame")
+    ap.add_argument("--bake", type=int, default=0, metavar="K",
+                    help="time sssgs_bake_visibility with K directions instead of the render step (side measurement)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -348,6 +402,10 @@ def main():
         if args.steps > 60:
             args.steps = 60  # bounded: each step is seconds of CPU work
         run_reference(args, rank)
+        return
+    if args.bake:
+        if rank == 0:
+            run_bake(args, local_rank)
         return
     run_gpu(args, rank, world, local_rank)
 

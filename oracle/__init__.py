@@ -307,21 +307,24 @@ def forward_frame(scene, view: int = 0, light: int = 0, mlp_mode: int = 0, mlp_o
     return r
 
 
-def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1):
+def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1, rows=None):
     """Ray-traced visibility of every Gaussian towards K directions and its SH projection
     (reading in DESIGN.md section 7d).  Returns (sh [n,(deg+1)^2] float64,
-    vis [n,K] float64, unstable [n,K] int32 = number of threshold decisions a float evaluation may flip)."""
+    vis [n,K] float64, unstable [n,K] int32 = number of threshold decisions a float evaluation may flip).
+    rows: optional indices of the Gaussians whose rays are traced (outputs then have len(rows) rows)."""
     n = int(scene.n)
     dirs = _f32(dirs).reshape(-1, 3)
     weights = _f32(weights).reshape(-1)
     K = dirs.shape[0]
     assert weights.shape[0] == K and sh_degree in (0, 1)
     nc = (sh_degree + 1) ** 2
-    sh = np.zeros((n, nc), np.float64)
-    vis = np.zeros((n, K), np.float64)
-    unstable = np.zeros((n, K), np.int32)
+    rows_arr = None if rows is None else np.ascontiguousarray(rows, np.int64)
+    m = n if rows_arr is None else len(rows_arr)
+    sh = np.zeros((m, nc), np.float64)
+    vis = np.zeros((m, K), np.float64)
+    unstable = np.zeros((m, K), np.int32)
     means, scales, rot, opac = _f32(scene.means), _f32(scene.scales), _f32(scene.rotations), _f32(scene.opacities)
     lib().orc_bake_visibility(ctypes.c_int64(n), _p(means), _p(scales), _p(rot), _p(opac), ctypes.c_int(K),
                               _p(dirs), _p(weights), ctypes.c_float(t_min), ctypes.c_int(sh_degree),
-                              _p(sh), _p(vis), _p(unstable))
+                              ctypes.c_int64(m), _p(rows_arr), _p(sh), _p(vis), _p(unstable))
     return sh, vis, unstable

@@ -670,8 +670,9 @@ extern "C" {
 // decide these the other way).
 void orc_bake_visibility(int64_t n, const float* means, const float* scales, const float* rotations,
                          const float* opacities, int n_dirs, const float* dirs, const float* weights,
-                         float t_min, int sh_degree, double* sh_out, double* vis_out,
-                         int32_t* unstable) {
+                         float t_min, int sh_degree, int64_t n_rows, const int64_t* rows,
+                         double* sh_out, double* vis_out, int32_t* unstable) {
+  // rows: the Gaussians whose rays are traced (all n if NULL); outputs are indexed by position in rows
   const int nc = (sh_degree + 1) * (sh_degree + 1);
   std::vector<double> Sinv((size_t)n * 9);
   for (int64_t j = 0; j < n; ++j) {
@@ -692,8 +693,10 @@ void orc_bake_visibility(int64_t n, const float* means, const float* scales, con
         Sinv[9 * j + 3 * a + b] = s;
       }
   }
+  if (!rows) n_rows = n;
 #pragma omp parallel for schedule(dynamic, 16)
-  for (int64_t i = 0; i < n; ++i) {
+  for (int64_t r = 0; r < n_rows; ++r) {
+    const int64_t i = rows ? rows[r] : r;
     double c[4] = {0, 0, 0, 0};
     for (int k = 0; k < n_dirs; ++k) {
       const double w[3] = {dirs[3 * k], dirs[3 * k + 1], dirs[3 * k + 2]};
@@ -726,8 +729,8 @@ void orc_bake_visibility(int64_t n, const float* means, const float* scales, con
       }
       if (std::fabs(T * 1e4 - 1.0) < 1e-2) ++flips;
       const double V = T >= 1e-4 ? T : 0.0;
-      if (vis_out) vis_out[i * n_dirs + k] = V;
-      if (unstable) unstable[i * n_dirs + k] = flips;
+      if (vis_out) vis_out[r * n_dirs + k] = V;
+      if (unstable) unstable[r * n_dirs + k] = flips;
       const double wk = weights[k];
       c[0] += wk * V * 0.2820948;
       if (nc == 4) {
@@ -736,7 +739,7 @@ void orc_bake_visibility(int64_t n, const float* means, const float* scales, con
         c[3] += wk * V * 0.4886025 * w[0];
       }
     }
-    for (int m = 0; m < nc; ++m) sh_out[i * nc + m] = c[m];
+    for (int m = 0; m < nc; ++m) sh_out[r * nc + m] = c[m];
   }
 }
 

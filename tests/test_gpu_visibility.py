@@ -148,3 +148,21 @@ def test_invalid_arguments():
         torch.cuda.synchronize()
     finally:
         r.close()
+
+
+@pytest.mark.parametrize("cfg,K,n_rows,t_min", [(2, 32, 192, 0.05), (3, 16, 96, 0.05)])
+def test_full_size_sampled_rows(cfg, K, n_rows, t_min):
+    """BASELINE-size scenes as they are (no rescaling): the oracle traces the rays of a seeded sample of
+    Gaussians against ALL Gaussians; the GPU result of those rows must match."""
+    scene = scenes.make_scene(cfg, views=1, lights=1)
+    dirs, wts = fib(K)
+    sh, vis, _ = gpu_bake(scene, dirs, wts, t_min)
+    assert np.isfinite(sh).all() and (vis >= 0).all() and (vis <= 1).all()
+    rows = np.sort(np.random.default_rng(50 + cfg).choice(scene.n, size=n_rows, replace=False))
+    sh_ref, vis_ref, unstable = oracle.bake_visibility(scene, dirs, wts, t_min, rows=rows)
+    tol = np.where(unstable == 0, 5e-5, 1e-4 + 5e-3 * unstable)
+    err = np.abs(vis[rows].astype(np.float64) - vis_ref)
+    assert (err <= tol).all(), f"worst {err.max():.3e}"
+    assert (vis_ref < 0.999).mean() > 0.05 and vis_ref.max() > 0.5
+    bound = (tol * np.abs(wts * Y00)[None, :]).sum(1) + 1e-5
+    assert (np.abs(sh[rows, 0] - sh_ref[:, 0]) <= bound).all()

@@ -178,3 +178,15 @@ def test_sh_projection_of_full_and_half_space_visibility():
     assert abs(sh[0, 0] - (2 * np.pi * Y00 * (1 + 0.01))) < 0.03
     got = np.array([sh[0, 3], sh[0, 1], sh[0, 2]])
     np.testing.assert_allclose(got, np.pi * Y1 * nrm * (1 - 0.01), atol=0.03)
+
+
+def test_row_subset_equals_rows_of_the_full_result():
+    rng = np.random.default_rng(8)
+    sc = _random_scene(rng, 25)
+    dirs, wts = _fib(6)
+    sh, vis, un = oracle.bake_visibility(sc, dirs, wts, t_min=0.05)
+    rows = [3, 17, 4]
+    sh2, vis2, un2 = oracle.bake_visibility(sc, dirs, wts, t_min=0.05, rows=rows)
+    np.testing.assert_array_equal(sh2, sh[rows])
+    np.testing.assert_array_equal(vis2, vis[rows])
+    np.testing.assert_array_equal(un2, un[rows])
