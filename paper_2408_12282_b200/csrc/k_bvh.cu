@@ -226,14 +226,16 @@ bvh_refit_kernel(int n, float4* box_lo, float4* box_hi, const int* __restrict__ 
   }
 }
 
-// slab test of the ray o + t w, t >= 0 (iw = 1 / w, components of w nudged away from 0)
-__device__ __forceinline__ bool hit_box(const float4& lo, const float4& hi, const float o[3], const float iw[3]) {
+// slab test of the ray o + t w, t >= 0 (iw = 1 / w, components of w nudged away from 0): entry
+// distance, or -1 on a miss
+__device__ __forceinline__ float hit_box(const float4& lo, const float4& hi, const float o[3], const float iw[3]) {
   const float tx0 = (lo.x - o[0]) * iw[0], tx1 = (hi.x - o[0]) * iw[0];
   const float ty0 = (lo.y - o[1]) * iw[1], ty1 = (hi.y - o[1]) * iw[1];
   const float tz0 = (lo.z - o[2]) * iw[2], tz1 = (hi.z - o[2]) * iw[2];
   const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fmaxf(fminf(tz0, tz1), 0.f));
   const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
-  return tn <= tf && lo.x <= hi.x;  // an inverted box is empty (Gaussians that never reach alpha_min)
+  // an inverted box is empty (Gaussians that never reach alpha_min)
+  return (tn <= tf && lo.x <= hi.x) ? tn : -1.f;
 }
 
 constexpr int kBvhStack = 96;
@@ -242,15 +244,18 @@ __global__ void __launch_bounds__(128)
 bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* __restrict__ leaf,
                  const float4* __restrict__ box_lo, const float4* __restrict__ box_hi, int n_dirs,
                  const float* __restrict__ dirs, const float* __restrict__ weights, float t_min, int n_coef,
-                 float* __restrict__ sh_out, float* __restrict__ vis_out) {
+                 float* __restrict__ sh_out, float* __restrict__ vis_out, int dirs_per_group,
+                 float4* __restrict__ partial) {
   pdl_prologue();
   const int k = blockIdx.x * 128 + threadIdx.x;
   if (k >= n) return;
+  // blockIdx.y = group of directions (more threads for small scenes); a group's sums go to `partial`
+  const int dir_begin = blockIdx.y * dirs_per_group, dir_end = min(n_dirs, dir_begin + dirs_per_group);
   const uint32_t gid = sorted_gid[k];
   const float4 me = leaf[3 * (size_t)k];
   float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;
   int stack[kBvhStack];
-  for (int dk = 0; dk < n_dirs; ++dk) {
+  for (int dk = dir_begin; dk < dir_end; ++dk) {
     const float w[3] = {dirs[3 * dk], dirs[3 * dk + 1], dirs[3 * dk + 2]};
     const float o[3] = {fmaf(t_min, w[0], me.x), fmaf(t_min, w[1], me.y), fmaf(t_min, w[2], me.z)};
     float iw[3];
@@ -259,38 +264,48 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
     float T = 1.f;
     if (n >= 2 && finite3(o[0], o[1], o[2])) {
       int sp = 0;
-      stack[sp++] = 0;
-      while (sp) {
-        const int node = stack[--sp];
-        const int child[2] = {__float_as_int(box_lo[node].w), __float_as_int(box_hi[node].w)};
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-          const int c = child[q];
-          const float4 lo = box_lo[c], hi = box_hi[c];
-          if (!hit_box(lo, hi, o, iw)) continue;
-          if (c < n - 1) {
-            if (sp < kBvhStack) stack[sp++] = c;
-            continue;
-          }
-          const size_t j = (size_t)(c - (n - 1));
-          const float4 l0 = leaf[3 * j], l1 = leaf[3 * j + 1], l2 = leaf[3 * j + 2];
-          if (__float_as_uint(l2.w) == gid) continue;
-          // point of the largest response along the ray, clamped to its start
-          const float d[3] = {o[0] - l0.x, o[1] - l0.y, o[2] - l0.z};
-          const float Sw[3] = {l1.x * w[0] + l1.y * w[1] + l1.z * w[2], l1.y * w[0] + l1.w * w[1] + l2.x * w[2],
-                               l1.z * w[0] + l2.x * w[1] + l2.y * w[2]};
-          const float Sd[3] = {l1.x * d[0] + l1.y * d[1] + l1.z * d[2], l1.y * d[0] + l1.w * d[1] + l2.x * d[2],
-                               l1.z * d[0] + l2.x * d[1] + l2.y * d[2]};
-          const float ww = w[0] * Sw[0] + w[1] * Sw[1] + w[2] * Sw[2];
-          const float wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
-          const float t = fmaxf(0.f, -wd / ww);
-          const float e[3] = {fmaf(t, w[0], d[0]), fmaf(t, w[1], d[1]), fmaf(t, w[2], d[2])};
-          const float m2 = e[0] * (l1.x * e[0] + l1.y * e[1] + l1.z * e[2]) + e[1] * (l1.y * e[0] + l1.w * e[1] + l2.x * e[2]) +
-                           e[2] * (l1.z * e[0] + l2.x * e[1] + l2.y * e[2]);
-          const float a = l0.w * __expf(-0.5f * m2);
-          if (!(a >= kBvhAlphaMin)) continue;
-          T *= 1.f - fminf(a, kBvhAlphaMax);
-          if (T < kBvhTMin) { sp = 0; break; }
+      // nearer child first: the opaque surface next to the ray's start ends most blocked rays early
+      // (the product is order independent, the early exit is not a change of the result)
+      auto leaf_hit = [&](int c) -> bool {  // true: the ray is extinguished
+        const size_t j = (size_t)(c - (n - 1));
+        const float4 l0 = leaf[3 * j], l1 = leaf[3 * j + 1], l2 = leaf[3 * j + 2];
+        if (__float_as_uint(l2.w) == gid) return false;
+        // point of the largest response along the ray, clamped to its start
+        const float d[3] = {o[0] - l0.x, o[1] - l0.y, o[2] - l0.z};
+        const float Sw[3] = {l1.x * w[0] + l1.y * w[1] + l1.z * w[2], l1.y * w[0] + l1.w * w[1] + l2.x * w[2],
+                             l1.z * w[0] + l2.x * w[1] + l2.y * w[2]};
+        const float Sd[3] = {l1.x * d[0] + l1.y * d[1] + l1.z * d[2], l1.y * d[0] + l1.w * d[1] + l2.x * d[2],
+                             l1.z * d[0] + l2.x * d[1] + l2.y * d[2]};
+        const float ww = w[0] * Sw[0] + w[1] * Sw[1] + w[2] * Sw[2];
+        const float wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
+        const float t = fmaxf(0.f, -wd / ww);
+        const float e[3] = {fmaf(t, w[0], d[0]), fmaf(t, w[1], d[1]), fmaf(t, w[2], d[2])};
+        const float m2 = e[0] * (l1.x * e[0] + l1.y * e[1] + l1.z * e[2]) + e[1] * (l1.y * e[0] + l1.w * e[1] + l2.x * e[2]) +
+                         e[2] * (l1.z * e[0] + l2.x * e[1] + l2.y * e[2]);
+        const float a = l0.w * __expf(-0.5f * m2);
+        if (!(a >= kBvhAlphaMin)) return false;
+        T *= 1.f - fminf(a, kBvhAlphaMax);
+        return T < kBvhTMin;
+      };
+      int node = 0;
+      while (true) {
+        const int cl = __float_as_int(box_lo[node].w), cr = __float_as_int(box_hi[node].w);
+        float tl = hit_box(box_lo[cl], box_hi[cl], o, iw), tr = hit_box(box_lo[cr], box_hi[cr], o, iw);
+        bool dead = false;
+        if (tl >= 0.f && cl >= n - 1) { dead = leaf_hit(cl); tl = -1.f; }
+        if (!dead && tr >= 0.f && cr >= n - 1) { dead = leaf_hit(cr); tr = -1.f; }
+        if (dead) break;
+        if (tl >= 0.f && tr >= 0.f) {
+          const bool left_first = tl <= tr;
+          if (sp < kBvhStack) stack[sp++] = left_first ? cr : cl;
+          node = left_first ? cl : cr;
+        } else if (tl >= 0.f) {
+          node = cl;
+        } else if (tr >= 0.f) {
+          node = cr;
+        } else {
+          if (!sp) break;
+          node = stack[--sp];
         }
       }
     }
@@ -302,11 +317,28 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
     c2 = fmaf(wv * kBvhY1, w[2], c2);
     c3 = fmaf(wv * kBvhY1, w[0], c3);
   }
-  if (n_coef == 1) {
+  if (partial) {
+    partial[(size_t)blockIdx.y * n + gid] = make_float4(c0, c1, c2, c3);
+  } else if (n_coef == 1) {
     sh_out[gid] = c0;
   } else {
     reinterpret_cast<float4*>(sh_out)[gid] = make_float4(c0, c1, c2, c3);
   }
+}
+
+// sums the direction groups' partial SH sums in group order (deterministic)
+__global__ void __launch_bounds__(kBvhThreads)
+bvh_sh_reduce_kernel(int n, int groups, const float4* __restrict__ partial, int n_coef, float* __restrict__ sh_out) {
+  pdl_prologue();
+  const int g = blockIdx.x * kBvhThreads + threadIdx.x;
+  if (g >= n) return;
+  float4 c = partial[g];
+  for (int q = 1; q < groups; ++q) {
+    const float4 p = partial[(size_t)q * n + g];
+    c.x += p.x; c.y += p.y; c.z += p.z; c.w += p.w;
+  }
+  if (n_coef == 1) sh_out[g] = c.x;
+  else reinterpret_cast<float4*>(sh_out)[g] = c;
 }
 
 }  // namespace
@@ -342,12 +374,23 @@ int launch_bvh_build(const sssgs_gaussians& g, const BvhBuffers& b, const uint32
 }
 
 int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* dirs, const float* weights, float t_min,
-                     int n_coef, float* sh_out, float* vis_out, cudaStream_t s) {
+                     int n_coef, float* sh_out, float* vis_out, int num_sms, float4* scratch, size_t scratch_bytes,
+                     cudaStream_t s) {
+  // enough threads to fill the device: split the directions in groups when there are few Gaussians
+  int groups = (int)(((int64_t)num_sms * 2048 * 2 + n - 1) / n);
+  if (groups > 8) groups = 8;
+  if (groups > n_dirs) groups = n_dirs;
+  if ((size_t)groups * n * 16 > scratch_bytes) groups = 1;
+  const int per = (n_dirs + groups - 1) / groups;
+  groups = (n_dirs + per - 1) / per;
   const unsigned blocks = (unsigned)((n + 127) / 128);
-  launch_pdl(bvh_trace_kernel, dim3(blocks), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
+  launch_pdl(bvh_trace_kernel, dim3(blocks, groups), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
              (const float4*)b.leaf, (const float4*)b.box_lo, (const float4*)b.box_hi, n_dirs, dirs, weights, t_min, n_coef,
-             sh_out, vis_out);
-  return 1;
+             sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr);
+  if (groups == 1) return 1;
+  launch_pdl(bvh_sh_reduce_kernel, dim3((unsigned)((n + kBvhThreads - 1) / kBvhThreads)), dim3(kBvhThreads), 0, s, (int)n,
+             groups, (const float4*)scratch, n_coef, sh_out);
+  return 2;
 }
 
 }  // namespace sssgs
