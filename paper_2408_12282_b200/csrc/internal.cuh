@@ -67,6 +67,7 @@ __host__ __device__ inline uint32_t sort_status_rows(uint32_t cap) {
   return (cap > kSortFill * (uint32_t)kSortThreads * 3u && rows < kSortFill) ? kSortFill : rows;
 }
 constexpr int kRadixMax = 256;
+constexpr int kLongListLog2 = 10;  // lists of >= 1024 entries are walked by more CTAs on small images
 constexpr uint32_t kFlagAgg = 1u << 30;  // look-back status: aggregate of this tile only
 constexpr uint32_t kFlagInc = 2u << 30;  // inclusive prefix up to and including this tile
 constexpr uint32_t kFlagMask = 3u << 30;
@@ -129,7 +130,8 @@ enum {
   DC_WC_CHUNKS = 26,     // weight cache: chunks handed out
   DC_WC_OVERFLOW = 27,   // weight cache: 1 if the pool ran out (the sweep then walks the lists again)
   DC_BVH_BOUNDS = 32,    // 6 words: box of the centres (sssgs_bake_visibility)
-  DC_WORDS = 64
+  DC_BUCKET_STARTS = 64, // 32 words: tiles with a list of at least 2^k entries, k = 0..31 (raster work order)
+  DC_WORDS = 96
 };
 
 // Geometry buffers of one camera view.

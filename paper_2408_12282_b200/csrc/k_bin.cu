@@ -218,6 +218,8 @@ ranges_kernel(const uint32_t* __restrict__ sorted_tiles, uint32_t* __restrict__ 
     uint32_t start = 0;
     for (int k = 31; k > (int)threadIdx.x; --k) start += s_cnt[k];
     s_start[threadIdx.x] = start;
+    // bucket b holds lengths in [2^(b-1), 2^b): `start` tiles have at least 2^b entries, and come first
+    counters[DC_BUCKET_STARTS + threadIdx.x] = start;
   }
   __syncthreads();
   for (int t = threadIdx.x; t < tiles; t += 256) {

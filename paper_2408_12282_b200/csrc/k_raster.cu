@@ -387,17 +387,18 @@ __device__ __forceinline__ void raster_finish(float acc_depth, const f32x2* pacc
 // FWD = true is the "w/o deferred" variant (Tab. 2, Fig. 5): Eq. 7 was evaluated
 // per Gaussian (shade_gaussians_kernel), the walk composites those RGB values per light (Eq. 3)
 // and the epilogue only adds the background: no G-buffer channels, no per-pixel shading.
+// `block` = position in the work order (tile_order index * CTAs per tile + sub-region)
 template <int LB, int E, int WARPS, int U, bool MARK, bool FWD = false>
-__global__ void __launch_bounds__(WARPS * 32)
-raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
-                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
-                    const uint32_t* __restrict__ sorted_vals,
-                    const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
-                    const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
-                    float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
-                    float* __restrict__ aovd_out, float* __restrict__ aovs_out,
-                    int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode,
-                    WeightCache wc, const uint32_t* __restrict__ only_if_set) {
+__device__ __forceinline__ void
+raster_body(const CamParams& cam, const LightBatch& lights, int n_lights,
+            const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
+            const uint32_t* __restrict__ sorted_vals,
+            const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
+            const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
+            float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
+            float* __restrict__ aovd_out, float* __restrict__ aovs_out,
+            int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode,
+            const WeightCache& wc, const uint32_t* __restrict__ only_if_set, int block) {
   using S = RasterShape<E, WARPS>;
   constexpr int P = S::P, THREADS = S::THREADS;
   constexpr int NC = MARK ? 2 : (FWD ? 2 + LB : 5 + LB);  // float4 components per list entry
@@ -418,8 +419,8 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
   if (only_if_set && *only_if_set == 0u) return;  // weight-cache fallback walk, not needed
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int slot = lane / P, pix = lane % P;
-  const int tile = (int)tile_order[blockIdx.x / S::SUBS];  // longest lists first
-  const int sub = blockIdx.x % S::SUBS;
+  const int tile = (int)tile_order[block / S::SUBS];  // longest lists first
+  const int sub = block % S::SUBS;
   const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
   constexpr int WPR = S::RW / S::PW;  // warps per region row
   const int bx = tx * kTile + (sub % S::SX) * S::RW + (warp % WPR) * S::PW;
@@ -695,6 +696,54 @@ int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t
   return 1;
 }
 
+template <int LB, int E, int WARPS, int U, bool MARK, bool FWD = false>
+__global__ void __launch_bounds__(WARPS * 32)
+raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
+                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
+                    const uint32_t* __restrict__ sorted_vals,
+                    const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
+                    const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
+                    float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
+                    float* __restrict__ aovd_out, float* __restrict__ aovs_out,
+                    int64_t frame_stride_px, uint8_t* __restrict__ contrib, int sum_mode,
+                    WeightCache wc, const uint32_t* __restrict__ only_if_set) {
+  raster_body<LB, E, WARPS, U, MARK, FWD>(cam, lights, n_lights, ranges, tile_order, sorted_vals, rec_a, rec_b, attr,
+                                          mlp_out, rgb_out, gbuf_out, aovd_out, aovs_out, frame_stride_px, contrib,
+                                          sum_mode, wc, only_if_set, (int)blockIdx.x);
+}
+
+// Small images: the few longest tile lists (the first *n_long_ptr tiles of the work order, at most
+// cap_long) decide when the kernel ends if they are walked like the others.  The first cap_long * 4
+// CTAs of this kernel walk them with 4 entry slots per warp and 4 CTAs per tile (half the sequential
+// length), the other CTAs walk the remaining tiles with 2 slots and 2 CTAs per tile.
+template <int LB, int EL>
+__global__ void __launch_bounds__(256)
+raster_mixed_kernel(CamParams cam, LightBatch lights, int n_lights,
+                    const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
+                    const uint32_t* __restrict__ sorted_vals,
+                    const float4* __restrict__ rec_a, const float4* __restrict__ rec_b,
+                    const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
+                    float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
+                    float* __restrict__ aovd_out, float* __restrict__ aovs_out,
+                    int64_t frame_stride_px, int sum_mode, const uint32_t* __restrict__ only_if_set,
+                    const uint32_t* __restrict__ n_long_ptr, int cap_long) {
+  pdl_prologue();
+  const int n_long = min((int)*n_long_ptr, cap_long);
+  const WeightCache none{};
+  if ((int)blockIdx.x < cap_long * EL) {
+    if ((int)blockIdx.x >= n_long * EL) return;
+    raster_body<LB, EL, 8, (EL == 8 ? 1 : 2), false, false>(cam, lights, n_lights, ranges, tile_order, sorted_vals, rec_a, rec_b, attr,
+                                           mlp_out, rgb_out, gbuf_out, aovd_out, aovs_out, frame_stride_px, nullptr,
+                                           sum_mode, none, only_if_set, (int)blockIdx.x);
+  } else {
+    const int block = (int)blockIdx.x - cap_long * EL;
+    if (block < n_long * 2) return;
+    raster_body<LB, 2, 8, 2, false, false>(cam, lights, n_lights, ranges, tile_order, sorted_vals, rec_a, rec_b, attr,
+                                           mlp_out, rgb_out, gbuf_out, aovd_out, aovs_out, frame_stride_px, nullptr,
+                                           sum_mode, none, only_if_set, block);
+  }
+}
+
 // Launches one rasteriser variant: LB lights per walk, E entry slots per warp, WARPS warps per CTA.
 template <int LB, int E, int WARPS, int U, bool MARK = false, bool FWD = false>
 static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_lights,
@@ -715,6 +764,45 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
              lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
              aov_d, aov_s, frame_stride_px, contrib, sum_mode, wc ? *wc : WeightCache{}, only_if_set);
   return 1;
+}
+
+constexpr int kLongTilesCap = 64;  // tiles the mixed kernel can walk with 4 CTAs each
+
+template <int LB, int EL>
+static int launch_mixed_e(const CamParams& cam, const LightBatch& lights, int n_lights, const GeomBuffers& gb,
+                          const uint32_t* sorted_vals, const float4* attr, const float4* mlp_out, float* rgb, float* gbuf,
+                          float* aov_d, float* aov_s, int64_t frame_stride_px, int tiles, cudaStream_t s, int sum_mode,
+                          const uint32_t* only_if_set, int long_log2) {
+  constexpr int smem = raster_smem(LB, false, false, 8);
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(raster_mixed_kernel<LB, EL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+      return -1;
+    configured = true;
+  }
+  launch_pdl(raster_mixed_kernel<LB, EL>, dim3(kLongTilesCap * EL + tiles * 2), dim3(256), smem, s, cam, lights, n_lights,
+             gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf, aov_d, aov_s,
+             frame_stride_px, sum_mode, only_if_set, (const uint32_t*)(gb.counters + DC_BUCKET_STARTS + long_log2),
+             kLongTilesCap);
+  return 1;
+}
+template <int LB>
+static int launch_mixed(const CamParams& cam, const LightBatch& lights, int n_lights, const GeomBuffers& gb,
+                        const uint32_t* sorted_vals, const float4* attr, const float4* mlp_out, float* rgb, float* gbuf,
+                        float* aov_d, float* aov_s, int64_t frame_stride_px, int tiles, cudaStream_t s, int sum_mode,
+                        const uint32_t* only_if_set) {
+  static int log2len = -1, el = 4;
+  if (log2len < 0) {  // tuning aids
+    const char* e = getenv("SSSGS_LONG_LOG2");
+    log2len = e ? atoi(e) : kLongListLog2;
+    const char* f = getenv("SSSGS_LONG_E");
+    el = f ? atoi(f) : 4;
+  }
+  if (el == 8)
+    return launch_mixed_e<LB, 8>(cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s,
+                                 frame_stride_px, tiles, s, sum_mode, only_if_set, log2len);
+  return launch_mixed_e<LB, 4>(cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s,
+                               frame_stride_px, tiles, s, sum_mode, only_if_set, log2len);
 }
 
 // Tuning aid: SSSGS_RASTER_MODE = "<E><W>" digits, e.g. "18" (E=1, 8 warps: one CTA per tile, one
@@ -739,7 +827,14 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
   // tiles the classic one-thread-per-pixel shape executes fewer instructions per blended pair
   // (measured: DESIGN.md).
   int mode = raster_mode();
-  if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
+  if (mode == 0) {
+    if (tiles <= 1600) {  // 2 slots / 2 CTAs per tile, the longest lists with 4 / 4
+      if (n_lights <= 1) return launch_mixed<1>(cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, sum_mode, only_if_set);
+      if (n_lights <= 4) return launch_mixed<4>(cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, sum_mode, only_if_set);
+      return launch_mixed<8>(cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, sum_mode, only_if_set);
+    }
+    mode = 18;
+  }
 #define SSSGS_ARGS cam, lights, n_lights, gb, sorted_vals, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, tiles, s, nullptr, sum_mode, nullptr, only_if_set
 #define SSSGS_BY_LB(E, W, U)                                                   \
   do {                                                                         \
