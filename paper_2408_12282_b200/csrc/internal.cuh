@@ -167,6 +167,7 @@ struct WeightCache {
   uint2* hdr;         // [capacity * 32] (Gaussian id, bits(depth)) per entry
   float* weights;     // [capacity * 32 * 32] weight of the entry at each of the block's 32 pixels
   float* T;           // [H * W] final transmittance per pixel
+  float4* gsum;       // [H * W * 3] sums of the light-independent channels (first light batch of the view)
   uint32_t* chunks;   // device counter: chunks handed out (DC_WC_CHUNKS)
   uint32_t* overflow; // device flag (DC_WC_OVERFLOW)
   uint32_t capacity;  // chunks in the pool
@@ -240,7 +241,7 @@ int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint3
 int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_lights,
                          const GeomBuffers& gb, const WeightCache& wc, const float4* attr,
                          const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                         int64_t frame_stride_px, int sum_mode, cudaStream_t s);
+                         int64_t frame_stride_px, int sum_mode, int first_batch, cudaStream_t s);
 int raster_reads_unblended_rows(int tiles);
 // BVH of sssgs_bake_visibility (k_bvh.cu); nodes: internal 0 .. n-2 (root 0), leaf of sorted position k = n-1+k
 struct BvhBuffers {

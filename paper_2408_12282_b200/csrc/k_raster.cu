@@ -916,12 +916,20 @@ int launch_raster_forward(const CamParams& cam, int n_lights, const GeomBuffers&
 
 namespace {
 // staging buffer of one warp and one 16-entry step of the cached walk: rows [16][4 * RPG] float4 + weights
-__host__ __device__ constexpr int cached_buf_bytes(int lb) { return (kWcChunk / 2) * (4 * ((lb + 4 + 3) / 4)) * 16 + (kWcChunk / 2) * 32 * 4; }
+// (rows per entry: 3 attribute rows + LB MLP rows + the depth row; the MLP rows only in a REST walk)
+__host__ __device__ constexpr int cached_rows(int lb, bool rest) { return rest ? lb : lb + 4; }
+__host__ __device__ constexpr int cached_buf_bytes(int lb, bool rest) {
+  return (kWcChunk / 2) * (4 * ((cached_rows(lb, rest) + 3) / 4)) * 16 + (kWcChunk / 2) * 32 * 4;
+}
 // Per-light walk of a sweep over the weight cache: one warp per 8x4-pixel block streams the block's
 // chain -- per entry (Gaussian id, depth) and the 32 weights -- and blends the entry's channels,
 // fetched with warp-uniform loads (a Gaussian's rows are shared by neighbouring blocks and tiles: L1 /
 // L2 hits).  Same accumulation order and arithmetic as the list walk: bit-identical frames.
-template <int LB>
+// The sums of the light-independent channels (depth, normal, base colour, roughness, metalness, sss, A)
+// are the same for every light batch of the view: the first batch's walk (REST = false) blends all
+// channels and stores those sums per pixel (wc.gsum), the later ones (REST = true) blend the MLP
+// channels only and read them back.
+template <int LB, bool REST>
 __global__ void __launch_bounds__(256, 2)
 raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint32_t* __restrict__ tile_order,
                      WeightCache wc, const float4* __restrict__ attr, const float4* __restrict__ mlp_out,
@@ -944,10 +952,11 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
   // the one-pixel-per-lane layout needs 3 + LB broadcast loads for the same FMAs per lane and is bound
   // by the shared-memory return path.  Every (pixel, channel) sum is still one fma per entry in list
   // order: bit-identical to the list walk.  The sums are transposed to one pixel per lane at the end.
-  constexpr int RPG = (LB + 4 + 3) / 4;
+  constexpr int ROWS = cached_rows(LB, REST), A0 = REST ? 0 : 3;  // A0 = first MLP row
+  constexpr int RPG = (ROWS + 3) / 4;
   constexpr int NR4 = 4 * RPG;
   constexpr int H = kWcChunk / 2;
-  constexpr int kBufBytes = cached_buf_bytes(LB);
+  constexpr int kBufBytes = cached_buf_bytes(LB, REST);
   static_assert(kBufBytes == H * NR4 * 16 + H * 32 * 4, "staging buffer size");
   static_assert(32 * (NR4 + 1) * 16 <= 2 * kBufBytes, "transpose fits in the warp's staging buffers");
   const int pg = lane >> 2, cg = lane & 3;
@@ -981,12 +990,12 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
     float4* rows = reinterpret_cast<float4*>(buf) + e * NR4;
     if (e < m) {
 #pragma unroll
-      for (int r = 0; r < 3 + LB; ++r) {
+      for (int r = 0; r < A0 + LB; ++r) {
         if ((r & 1) != (int)part) continue;
-        const float4* src = r < 3 ? attr + 3 * g + r : mlp_out + g * n_lights + min(r - 3, n_lights - 1);
+        const float4* src = r < A0 ? attr + 3 * g + r : mlp_out + g * n_lights + min(r - A0, n_lights - 1);
         cp_async16(rows + r, src);
       }
-      if (part == 0) rows[3 + LB] = make_float4(depth, 0.f, 0.f, 0.f);
+      if (!REST && part == 0) rows[A0 + LB] = make_float4(depth, 0.f, 0.f, 0.f);
     }
     float4* w4 = reinterpret_cast<float4*>(buf + H * NR4 * 16);
     const float4* wsrc = reinterpret_cast<const float4*>(wc.weights + ((size_t)chunk_id * kWcChunk + half * H) * 32);
@@ -1051,17 +1060,25 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
             make_float4(acc[q][2 * r].x, acc[q][2 * r].y, acc[q][2 * r + 1].x, acc[q][2 * r + 1].y);
     __syncwarp();
     const float4* mine = t4 + lane * TS;
-    const float4 a0 = mine[0], a1 = mine[1], a2 = mine[2];
+    float4 a0, a1, a2;
+    float4* gs = wc.gsum + 3 * ((int64_t)min(py, cam.height - 1) * cam.width + min(px, cam.width - 1));
+    if (REST) {
+      a0 = gs[0]; a1 = gs[1]; a2 = gs[2];
+    } else {
+      a0 = mine[0]; a1 = mine[1]; a2 = mine[2];
+      a2.z = mine[A0 + LB].x;  // the depth sum rides in the free slot of the third row
+      if (inside) { gs[0] = a0; gs[1] = a1; gs[2] = a2; }
+    }
     pacc[0] = make_float2(a0.x, a0.y); pacc[1] = make_float2(a0.z, a0.w);
     pacc[2] = make_float2(a1.x, a1.y); pacc[3] = make_float2(a1.z, a1.w);
     pacc[4] = make_float2(a2.x, a2.y);
+    acc_depth = a2.z;
 #pragma unroll
     for (int l = 0; l < LB; ++l) {
-      const float4 mo = mine[3 + l];
+      const float4 mo = mine[A0 + l];
       paccl[l][0] = make_float2(mo.x, mo.y);
       paccl[l][1] = make_float2(mo.z, mo.w);
     }
-    acc_depth = mine[3 + LB].x;
   }
   const float T = inside ? wc.T[(int64_t)py * cam.width + px] : 1.f;
   raster_finish<LB, 1, false>(acc_depth, pacc, paccl, 0.f, T, inside, px, py, 0, cam, lights, n_lights, rgb_out,
@@ -1072,25 +1089,31 @@ raster_cached_kernel(CamParams cam, LightBatch lights, int n_lights, const uint3
 int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_lights,
                          const GeomBuffers& gb, const WeightCache& wc, const float4* attr,
                          const float4* mlp_out, float* rgb, float* gbuf, float* aov_d, float* aov_s,
-                         int64_t frame_stride_px, int sum_mode, cudaStream_t s) {
+                         int64_t frame_stride_px, int sum_mode, int first_batch, cudaStream_t s) {
   const int tiles = cam.tiles_x * cam.tiles_y;
   if (tiles == 0) return 0;
-#define SSSGS_CACHED(LB)                                                                                \
-  do {                                                                                                  \
-    constexpr int smem = 8 * 2 * cached_buf_bytes(LB);                                                  \
-    static bool configured = false;                                                                     \
-    if (!configured) {                                                                                  \
-      if (cudaFuncSetAttribute(raster_cached_kernel<LB>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
-                               smem) != cudaSuccess)                                                    \
-        return -1;                                                                                      \
-      configured = true;                                                                                \
-    }                                                                                                   \
-    launch_pdl(raster_cached_kernel<LB>, dim3(tiles), dim3(256), smem, s, cam, lights, n_lights,        \
-               gb.tile_order, wc, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, sum_mode);   \
+#define SSSGS_CACHED(LB, REST)                                                                              \
+  do {                                                                                                      \
+    constexpr int smem = 8 * 2 * cached_buf_bytes(LB, REST);                                                \
+    static bool configured = false;                                                                         \
+    if (!configured) {                                                                                      \
+      if (cudaFuncSetAttribute(raster_cached_kernel<LB, REST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                               smem) != cudaSuccess)                                                        \
+        return -1;                                                                                          \
+      configured = true;                                                                                    \
+    }                                                                                                       \
+    launch_pdl(raster_cached_kernel<LB, REST>, dim3(tiles), dim3(256), smem, s, cam, lights, n_lights,      \
+               gb.tile_order, wc, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, sum_mode);       \
   } while (0)
-  if (n_lights <= 1) SSSGS_CACHED(1);
-  else if (n_lights <= 4) SSSGS_CACHED(4);
-  else SSSGS_CACHED(8);
+#define SSSGS_CACHED_LB(REST)            \
+  do {                                   \
+    if (n_lights <= 1) SSSGS_CACHED(1, REST);      \
+    else if (n_lights <= 4) SSSGS_CACHED(4, REST); \
+    else SSSGS_CACHED(8, REST);          \
+  } while (0)
+  if (first_batch) SSSGS_CACHED_LB(false);
+  else SSSGS_CACHED_LB(true);
+#undef SSSGS_CACHED_LB
 #undef SSSGS_CACHED
   return 1;
 }

@@ -124,6 +124,7 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
     p = take(chunks * kWcChunk * 8); if (c) c->wc.hdr = (uint2*)p;
     p = take(chunks * kWcChunk * 32 * 4); if (c) c->wc.weights = (float*)p;
     p = take(npix * 4); if (c) c->wc.T = (float*)p;
+    p = take(npix * 48); if (c) c->wc.gsum = (float4*)p;
     if (c) c->wc.capacity = (uint32_t)chunks;
   }
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
@@ -630,7 +631,8 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
       float* o_as = out->aov_specular ? out->aov_specular + frame0 * npix * 3 : nullptr;
       const int smode = sum_lights ? (l0 == 0 ? 1 : 2) : 0;
       if (use_cache) {  // cached walk; the list walk behind it only runs if the cache overflowed
-        add(launch_raster_cached(cam, lb, nl, c->gb, c->wc, c->attr, mlp_buf, o_rgb, o_gbuf, o_ad, o_as, npix, smode, s));
+        add(launch_raster_cached(cam, lb, nl, c->gb, c->wc, c->attr, mlp_buf, o_rgb, o_gbuf, o_ad, o_as, npix, smode,
+                                 l0 == 0, s));
         add(launch_raster(cam, lb, nl, c->gb, sorted_vals, c->attr, mlp_buf, o_rgb, o_gbuf, o_ad, o_as, npix, smode, s,
                           cnt + DC_WC_OVERFLOW));
       } else
