@@ -611,7 +611,7 @@ raster_body(const CamParams& cam, const LightBatch& lights, int n_lights,
                 wc_off = true;
               } else {
                 if (lane == 0) {
-                  if (wc_items == 0) wc.head[tile * 8 + warp] = c;
+                  if (wc_items == 0) wc.head[tile * 8 + sub * WARPS + warp] = c;
                   else wc.next[wc_chunk] = c;
                 }
                 wc_chunk = c;
@@ -663,7 +663,7 @@ raster_body(const CamParams& cam, const LightBatch& lights, int n_lights,
   cp_async_wait_all();
   if (MARK) {
     if (caching) {
-      if (lane == 0) wc.count[tile * 8 + warp] = wc_items;
+      if (lane == 0) wc.count[tile * 8 + sub * WARPS + warp] = wc_items;
       if (inside) wc.T[(int64_t)py * cam.width + px] = T;
     }
     return;
@@ -1129,7 +1129,14 @@ int launch_mark_contrib(const CamParams& cam, const GeomBuffers& gb, const uint3
   int mode = raster_mode();
   if (mode == 0) mode = tiles <= 1600 ? 28 : 18;
   const int e = mode / (mode >= 100 ? 100 : 10);
-  if (e == 1 || wc)  // the weight cache is organised by the 8x4-pixel blocks of the one-slot shape
+  static int half_tiles = -1;  // tuning aid: SSSGS_MARK_HALF=0 walks a tile with one 8-warp CTA
+  if (half_tiles < 0) { const char* h = getenv("SSSGS_MARK_HALF"); half_tiles = h ? atoi(h) : 1; }
+  // the weight cache is organised by the 8x4-pixel blocks of the one-slot shape; two 4-warp CTAs per
+  // tile (block = sub * 4 + warp) balance the kernel's tail better than one 8-warp CTA
+  if (wc && half_tiles)
+    return launch_variant<1, 1, 4, 4, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
+                                            nullptr, 0, tiles, s, contrib, 0, wc);
+  if (e == 1 || wc)
     return launch_variant<1, 1, 8, 4, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
                                             nullptr, 0, tiles, s, contrib, 0, wc);
   return launch_variant<1, 4, 8, 2, true>(cam, none, 0, gb, sorted_vals, nullptr, nullptr, nullptr, nullptr, nullptr,
