@@ -194,12 +194,14 @@ def test_light_batching_is_consistent():
     np.testing.assert_allclose(a["rgb"], c["rgb"], rtol=2e-6, atol=1e-6)
 
 
-@pytest.mark.parametrize("width", [200, 656])   # 169 tiles -> 4 entry slots per warp; 1681 tiles -> 1
-def test_sweep_row_skipping_changes_nothing(width):
+# 169 tiles -> several entry slots per warp; 1681 tiles -> 1.  19 lights = three light batches: the first
+# cached walk blends all channels, the next two (8 and 3 lights) only the MLP channels
+@pytest.mark.parametrize("width,n_lights", [(200, 6), (656, 6), (656, 19), (200, 12)])
+def test_sweep_row_skipping_changes_nothing(width, n_lights):
     # From 4 lights per view on, a visibility pre-pass restricts the MLP to the Gaussians that are
     # blended somewhere (unless the MLP outputs of all Gaussians are requested).  Frames must be
     # bit-identical with and without it, and the skipped rows must really be skippable.
-    scene = scenes.make_scene(3, n=40000, width=width, height=width, lights=6)
+    scene = scenes.make_scene(3, n=40000, width=width, height=width, lights=n_lights)
     on = gpu_render(scene, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters"), lights=scene.lights[0])
     off = gpu_render(scene, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters", "mlp_out"),
                      lights=scene.lights[0])
@@ -210,7 +212,7 @@ def test_sweep_row_skipping_changes_nothing(width):
             np.testing.assert_array_equal(on[k].view(np.uint32), off[k].view(np.uint32))
         else:             # small images walk 2 entries per warp step without the pre-pass: the per-slot
             # partial sums are added in another order than the cached one-slot walk (both within 1e-4)
-            np.testing.assert_allclose(on[k], off[k], rtol=2e-5, atol=2e-6)
+            np.testing.assert_allclose(on[k], off[k], rtol=5e-5, atol=2e-6)
     r = oracle.render_frame(scene, 0, 0, mlp_out=off["mlp_out"][0].astype(np.float64))
     # the rows the pre-pass keeps are the Gaussians the oracle blends at some pixel (pixels whose
     # skip / stop decisions sit within rounding of a threshold may add or drop a few)
