@@ -307,11 +307,12 @@ def forward_frame(scene, view: int = 0, light: int = 0, mlp_mode: int = 0, mlp_o
     return r
 
 
-def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1, rows=None):
+def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1, rows=None, positions: bool = False):
     """Ray-traced visibility of every Gaussian towards K directions and its SH projection
     (reading in DESIGN.md section 7d).  Returns (sh [n,(deg+1)^2] float64,
     vis [n,K] float64, unstable [n,K] int32 = number of threshold decisions a float evaluation may flip).
-    rows: optional indices of the Gaussians whose rays are traced (outputs then have len(rows) rows)."""
+    rows: optional indices of the Gaussians whose rays are traced (outputs then have len(rows) rows).
+    positions: `dirs` are points (light positions); rays end there."""
     n = int(scene.n)
     dirs = _f32(dirs).reshape(-1, 3)
     weights = _f32(weights).reshape(-1)
@@ -326,5 +327,5 @@ def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1, rows
     means, scales, rot, opac = _f32(scene.means), _f32(scene.scales), _f32(scene.rotations), _f32(scene.opacities)
     lib().orc_bake_visibility(ctypes.c_int64(n), _p(means), _p(scales), _p(rot), _p(opac), ctypes.c_int(K),
                               _p(dirs), _p(weights), ctypes.c_float(t_min), ctypes.c_int(sh_degree),
-                              ctypes.c_int64(m), _p(rows_arr), _p(sh), _p(vis), _p(unstable))
+                              ctypes.c_int(1 if positions else 0), ctypes.c_int64(m), _p(rows_arr), _p(sh), _p(vis), _p(unstable))
     return sh, vis, unstable

@@ -670,8 +670,11 @@ extern "C" {
 // decide these the other way).
 void orc_bake_visibility(int64_t n, const float* means, const float* scales, const float* rotations,
                          const float* opacities, int n_dirs, const float* dirs, const float* weights,
-                         float t_min, int sh_degree, int64_t n_rows, const int64_t* rows,
+                         float t_min, int sh_degree, int positions, int64_t n_rows, const int64_t* rows,
                          double* sh_out, double* vis_out, int32_t* unstable) {
+  // positions != 0: `dirs` holds K points p_k (the OLAT lights of L110, "the position of the light
+  // source is known"): the ray of Gaussian i runs from mu_i towards p_k and ends there,
+  // w = (p_k - mu_i) / d, t in [0, d - t_min]; nothing occludes if d <= t_min.
   // rows: the Gaussians whose rays are traced (all n if NULL); outputs are indexed by position in rows
   const int nc = (sh_degree + 1) * (sh_degree + 1);
   std::vector<double> Sinv((size_t)n * 9);
@@ -699,13 +702,21 @@ void orc_bake_visibility(int64_t n, const float* means, const float* scales, con
     const int64_t i = rows ? rows[r] : r;
     double c[4] = {0, 0, 0, 0};
     for (int k = 0; k < n_dirs; ++k) {
-      const double w[3] = {dirs[3 * k], dirs[3 * k + 1], dirs[3 * k + 2]};
+      double w[3] = {dirs[3 * k], dirs[3 * k + 1], dirs[3 * k + 2]};
+      double t_max = INFINITY;
+      if (positions) {
+        double d2 = 0;
+        for (int a = 0; a < 3; ++a) { w[a] -= (double)means[3 * i + a]; d2 += w[a] * w[a]; }
+        const double d = std::sqrt(d2);
+        for (int a = 0; a < 3; ++a) w[a] = d > 0 ? w[a] / d : 0.0;
+        t_max = d - (double)t_min;
+      }
       double o[3];
       for (int a = 0; a < 3; ++a) o[a] = (double)means[3 * i + a] + (double)t_min * w[a];
       double T = 1.0;
       int flips = 0;
       for (int64_t j = 0; j < n; ++j) {
-        if (j == i) continue;
+        if (j == i || !(t_max > 0)) continue;
         const double* S = &Sinv[9 * j];
         double d[3], Sw[3], Sd[3];
         for (int a = 0; a < 3; ++a) d[a] = o[a] - (double)means[3 * j + a];
@@ -717,6 +728,7 @@ void orc_bake_visibility(int64_t n, const float* means, const float* scales, con
         const double wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
         double t = -wd / ww;  // minimiser of the quadratic along the line
         if (t < 0) t = 0;
+        if (t > t_max) t = t_max;
         double e[3], Se[3];
         for (int a = 0; a < 3; ++a) e[a] = d[a] + t * w[a];
         for (int a = 0; a < 3; ++a) Se[a] = S[3 * a] * e[0] + S[3 * a + 1] * e[1] + S[3 * a + 2] * e[2];

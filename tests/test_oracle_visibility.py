@@ -190,3 +190,35 @@ def test_row_subset_equals_rows_of_the_full_result():
     np.testing.assert_array_equal(sh2, sh[rows])
     np.testing.assert_array_equal(vis2, vis[rows])
     np.testing.assert_array_equal(un2, un[rows])
+
+
+def test_positions_mode_segment_ends_at_the_light():
+    sigma, o = 0.1, 0.8
+    # occluder between the Gaussian and the light: same as the direction ray; occluder behind the light: free
+    sc = _scene([[0, 0, 0], [2, 0.05, 0], [6, 0.05, 0]], [[1e-3] * 3, [sigma] * 3, [sigma] * 3], [IDQ] * 3, [0.0, o, 0.0])
+    _, vis_dir, _ = oracle.bake_visibility(sc, [[1, 0, 0]], [1], t_min=0.01)
+    _, vis_pos, _ = oracle.bake_visibility(sc, [[4, 0, 0]], [1], t_min=0.01, positions=True)
+    assert abs(vis_pos[0, 0] - vis_dir[0, 0]) < 1e-12 and vis_pos[0, 0] < 0.5
+    sc.opacities[:] = [0.0, 0.0, o]
+    _, vis_pos, _ = oracle.bake_visibility(sc, [[4, 0, 0]], [1], t_min=0.01, positions=True)
+    # the closest point of the segment is its end (4, 0, 0), 2 units from the occluder: nothing
+    assert vis_pos[0, 0] == 1.0
+    # occluder just behind the light: acts at the segment's end, m2 = (0.15^2 + 0.05^2) / sigma^2
+    sc.means[2] = [4.15, 0.05, 0]
+    _, vis_pos, _ = oracle.bake_visibility(sc, [[4, 0, 0]], [1], t_min=0.01, positions=True)
+    want = 1 - o * np.exp(-0.5 * (0.15**2 + 0.05**2) / sigma**2)
+    assert abs(vis_pos[0, 0] - want) < 1e-6
+    # light closer than the ray start: no segment, nothing occludes; SH uses the direction to the light
+    sh, vis_pos, _ = oracle.bake_visibility(sc, [[0, 0.005, 0]], [2.0], t_min=0.01, positions=True)
+    assert vis_pos[0, 0] == 1.0
+    np.testing.assert_allclose(sh[0], [2 * Y00, 2 * Y1, 0, 0], atol=1e-6)   # w = +y
+
+
+def test_positions_mode_matches_directions_for_far_lights():
+    rng = np.random.default_rng(9)
+    sc = _random_scene(rng, 30)
+    dirs, wts = _fib(8)
+    _, vis_dir, un1 = oracle.bake_visibility(sc, dirs, wts, t_min=0.05)
+    _, vis_pos, un2 = oracle.bake_visibility(sc, dirs.astype(np.float64) * 1e6, wts, t_min=0.05, positions=True)
+    ok = (un1 == 0) & (un2 == 0)
+    np.testing.assert_allclose(vis_pos[ok], vis_dir[ok], atol=2e-5)
