@@ -209,6 +209,9 @@ int sssgs_render_host(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp*
  *   m2 = min_{t>=0} (x(t)-mu_j)^T Sigma_j^-1 (x(t)-mu_j),  a = min(0.99, o_j exp(-m2/2)) iff >= 1/255,
  *   V_i(w_k) = prod_{j != i} (1 - a), set to 0 below 1e-4;
  *   vis_sh_out[i][lm] = sum_k weights[k] V_i(w_k) Y_lm(w_k)   (basis and order of vis_sh above).
+ * With positions != 0 the K entries of `dirs` are points p_k (the known OLAT light positions of L110):
+ * the ray of Gaussian i runs towards p_k and ends there, w = (p_k - mu_i) / d, t in [0, d - t_min]
+ * (nothing occludes if d <= t_min), and the SH sum uses that per-Gaussian direction.
  * Only means, scales, rotations and opacities of `g` are read (device pointers, n <=
  * max_gaussians).  The call enqueues on `stream`, never synchronises and uses the context's
  * workspace: it must not overlap a render on the same context (same stream, or ordered by the
@@ -217,12 +220,13 @@ int sssgs_render_host(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp*
  * finite), SSSGS_ECAPACITY (n > max_gaussians), SSSGS_ECUDA.                                   */
 typedef struct {
   int n_dirs;            /* K                                                                 */
-  const float* dirs;     /* [K,3] unit vectors (device)                                       */
+  const float* dirs;     /* [K,3] unit vectors, or points if positions != 0 (device)          */
   const float* weights;  /* [K] quadrature weights, e.g. 4 pi / K (device)                    */
   float t_min;           /* ray start offset from the Gaussian's centre, world units          */
   int sh_degree;         /* 0 or 1                                                            */
   float* vis_sh_out;     /* [n,(deg+1)^2] (device), required                                  */
   float* vis_out;        /* [n,K] raw visibilities (device), may be NULL                      */
+  int positions;         /* 0: dirs are unit directions; 1: dirs are points, rays end there   */
 } sssgs_bake;
 int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_bake* bake, void* stream);
 

@@ -79,7 +79,7 @@ class sssgs_out(ctypes.Structure):
 
 class sssgs_bake(ctypes.Structure):
     _fields_ = [("n_dirs", ctypes.c_int), ("dirs", _vp), ("weights", _vp), ("t_min", _f),
-                ("sh_degree", ctypes.c_int), ("vis_sh_out", _vp), ("vis_out", _vp)]
+                ("sh_degree", ctypes.c_int), ("vis_sh_out", _vp), ("vis_out", _vp), ("positions", ctypes.c_int)]
 
 
 class SssgsError(RuntimeError):
@@ -317,7 +317,8 @@ class Renderer:
                      (SSSGS_FORWARD_SHADING if forward else 0), st)
         return outputs
 
-    def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None):
+    def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None,
+                        positions: bool = False):
         """Enqueue one sssgs_bake_visibility on the current torch stream.  dirs [K,3], weights [K] (numpy or
         device tensors).  Returns (vis_sh [n,(deg+1)^2], vis [n,K] or None), device tensors."""
         torch = self.torch
@@ -332,6 +333,7 @@ class Renderer:
         b.n_dirs, b.dirs, b.weights = K, self._bake_in[0].data_ptr(), self._bake_in[1].data_ptr()
         b.t_min, b.sh_degree = float(t_min), int(sh_degree)
         b.vis_sh_out, b.vis_out = sh.data_ptr(), (vis.data_ptr() if want_vis else None)
+        b.positions = 1 if positions else 0
         st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         sssgs_bake_visibility(self.ctx, self.g, b, st)
         return sh[:self.n], (vis[:self.n] if want_vis else None)

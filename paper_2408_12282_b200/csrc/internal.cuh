@@ -260,8 +260,8 @@ int launch_bvh_morton(int64_t n, const float* means, const uint32_t* bounds, uin
 int launch_bvh_build(const sssgs_gaussians& g, const BvhBuffers& b, const uint32_t* depth_hist,
                      const uint32_t* vals0, const uint32_t* vals1, cudaStream_t s);
 int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* dirs, const float* weights, float t_min,
-                     int n_coef, float* sh_out, float* vis_out, int num_sms, float4* scratch, size_t scratch_bytes,
-                     cudaStream_t s);
+                     int n_coef, float* sh_out, float* vis_out, int positions, int num_sms, float4* scratch,
+                     size_t scratch_bytes, cudaStream_t s);
 int launch_compact_contrib(const uint8_t* contrib, int64_t n, uint32_t* rows, uint32_t* count,
                            int zero_rest, float4* out0, float4* out1, int lights, cudaStream_t s);
 int launch_gather_precomputed(const float* pre, int64_t n, int n_lights, int64_t light_stride,

@@ -228,12 +228,13 @@ bvh_refit_kernel(int n, float4* box_lo, float4* box_hi, const int* __restrict__ 
 
 // slab test of the ray o + t w, t >= 0 (iw = 1 / w, components of w nudged away from 0): entry
 // distance, or -1 on a miss
-__device__ __forceinline__ float hit_box(const float4& lo, const float4& hi, const float o[3], const float iw[3]) {
+__device__ __forceinline__ float hit_box(const float4& lo, const float4& hi, const float o[3], const float iw[3],
+                                         float t_max) {
   const float tx0 = (lo.x - o[0]) * iw[0], tx1 = (hi.x - o[0]) * iw[0];
   const float ty0 = (lo.y - o[1]) * iw[1], ty1 = (hi.y - o[1]) * iw[1];
   const float tz0 = (lo.z - o[2]) * iw[2], tz1 = (hi.z - o[2]) * iw[2];
   const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fmaxf(fminf(tz0, tz1), 0.f));
-  const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
+  const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fminf(fmaxf(tz0, tz1), t_max));
   // an inverted box is empty (Gaussians that never reach alpha_min)
   return (tn <= tf && lo.x <= hi.x) ? tn : -1.f;
 }
@@ -245,7 +246,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
                  const float4* __restrict__ box_lo, const float4* __restrict__ box_hi, int n_dirs,
                  const float* __restrict__ dirs, const float* __restrict__ weights, float t_min, int n_coef,
                  float* __restrict__ sh_out, float* __restrict__ vis_out, int dirs_per_group,
-                 float4* __restrict__ partial) {
+                 float4* __restrict__ partial, int positions) {
   pdl_prologue();
   const int k = blockIdx.x * 128 + threadIdx.x;
   if (k >= n) return;
@@ -256,13 +257,21 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
   float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;
   int stack[kBvhStack];
   for (int dk = dir_begin; dk < dir_end; ++dk) {
-    const float w[3] = {dirs[3 * dk], dirs[3 * dk + 1], dirs[3 * dk + 2]};
+    float w[3] = {dirs[3 * dk], dirs[3 * dk + 1], dirs[3 * dk + 2]};
+    float t_max = 3.0e38f;
+    if (positions) {  // the ray ends at the point dirs[dk]
+      w[0] -= me.x; w[1] -= me.y; w[2] -= me.z;
+      const float d = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+      const float id = d > 0.f ? 1.f / d : 0.f;
+      w[0] *= id; w[1] *= id; w[2] *= id;
+      t_max = d - t_min;
+    }
     const float o[3] = {fmaf(t_min, w[0], me.x), fmaf(t_min, w[1], me.y), fmaf(t_min, w[2], me.z)};
     float iw[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) iw[a] = 1.f / (fabsf(w[a]) < 1e-20f ? copysignf(1e-20f, w[a]) : w[a]);
     float T = 1.f;
-    if (n >= 2 && finite3(o[0], o[1], o[2])) {
+    if (n >= 2 && finite3(o[0], o[1], o[2]) && t_max > 0.f) {
       int sp = 0;
       // nearer child first: the opaque surface next to the ray's start ends most blocked rays early
       // (the product is order independent, the early exit is not a change of the result)
@@ -278,7 +287,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
                              l1.z * d[0] + l2.x * d[1] + l2.y * d[2]};
         const float ww = w[0] * Sw[0] + w[1] * Sw[1] + w[2] * Sw[2];
         const float wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
-        const float t = fmaxf(0.f, -wd / ww);
+        const float t = fminf(t_max, fmaxf(0.f, -wd / ww));
         const float e[3] = {fmaf(t, w[0], d[0]), fmaf(t, w[1], d[1]), fmaf(t, w[2], d[2])};
         const float m2 = e[0] * (l1.x * e[0] + l1.y * e[1] + l1.z * e[2]) + e[1] * (l1.y * e[0] + l1.w * e[1] + l2.x * e[2]) +
                          e[2] * (l1.z * e[0] + l2.x * e[1] + l2.y * e[2]);
@@ -290,7 +299,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
       int node = 0;
       while (true) {
         const int cl = __float_as_int(box_lo[node].w), cr = __float_as_int(box_hi[node].w);
-        float tl = hit_box(box_lo[cl], box_hi[cl], o, iw), tr = hit_box(box_lo[cr], box_hi[cr], o, iw);
+        float tl = hit_box(box_lo[cl], box_hi[cl], o, iw, t_max), tr = hit_box(box_lo[cr], box_hi[cr], o, iw, t_max);
         bool dead = false;
         if (tl >= 0.f && cl >= n - 1) { dead = leaf_hit(cl); tl = -1.f; }
         if (!dead && tr >= 0.f && cr >= n - 1) { dead = leaf_hit(cr); tr = -1.f; }
@@ -374,8 +383,8 @@ int launch_bvh_build(const sssgs_gaussians& g, const BvhBuffers& b, const uint32
 }
 
 int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* dirs, const float* weights, float t_min,
-                     int n_coef, float* sh_out, float* vis_out, int num_sms, float4* scratch, size_t scratch_bytes,
-                     cudaStream_t s) {
+                     int n_coef, float* sh_out, float* vis_out, int positions, int num_sms, float4* scratch,
+                     size_t scratch_bytes, cudaStream_t s) {
   // enough threads to fill the device: split the directions in groups when there are few Gaussians
   int groups = (int)(((int64_t)num_sms * 2048 * 2 + n - 1) / n);
   if (groups > 8) groups = 8;
@@ -386,7 +395,7 @@ int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* di
   const unsigned blocks = (unsigned)((n + 127) / 128);
   launch_pdl(bvh_trace_kernel, dim3(blocks, groups), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
              (const float4*)b.leaf, (const float4*)b.box_lo, (const float4*)b.box_hi, n_dirs, dirs, weights, t_min, n_coef,
-             sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr);
+             sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr, positions);
   if (groups == 1) return 1;
   launch_pdl(bvh_sh_reduce_kernel, dim3((unsigned)((n + kBvhThreads - 1) / kBvhThreads)), dim3(kBvhThreads), 0, s, (int)n,
              groups, (const float4*)scratch, n_coef, sh_out);

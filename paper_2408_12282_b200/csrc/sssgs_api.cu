@@ -387,7 +387,7 @@ int sssgs_bake_visibility(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ba
                                   cnt + DC_TICKET_BASE + p, cnt + DC_SORT_ERROR, max_blocks, s);
   launches += launch_bvh_build(*g, bb, c->gb.hist, c->gb.dvals[0], c->gb.dvals[1], s);
   launches += launch_bvh_trace(n, bb, b->n_dirs, b->dirs, b->weights, b->t_min, (b->sh_degree + 1) * (b->sh_degree + 1),
-                               b->vis_sh_out, b->vis_out, c->num_sms, (float4*)c->wc.weights,
+                               b->vis_sh_out, b->vis_out, b->positions != 0, c->num_sms, (float4*)c->wc.weights,
                                (size_t)c->wc.capacity * kWcChunk * 32 * 4, s);
   c->launches = launches;
   if (cudaGetLastError() != cudaSuccess) return fail(c, SSSGS_ECUDA, "a bake kernel launch failed");

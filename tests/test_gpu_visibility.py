@@ -26,12 +26,12 @@ def fib(K):
     return np.stack([r * np.cos(phi), r * np.sin(phi), z], 1).astype(np.float32), np.full(K, 4 * np.pi / K, np.float32)
 
 
-def gpu_bake(scene, dirs, wts, t_min, sh_degree=1):
+def gpu_bake(scene, dirs, wts, t_min, sh_degree=1, positions=False):
     import torch
     from paper_2408_12282_b200 import binding
     r = binding.Renderer(scene)
     try:
-        sh, vis = r.bake_visibility(dirs, wts, t_min, sh_degree=sh_degree, want_vis=True)
+        sh, vis = r.bake_visibility(dirs, wts, t_min, sh_degree=sh_degree, want_vis=True, positions=positions)
         torch.cuda.synchronize()
         out = sh.cpu().numpy(), vis.cpu().numpy(), r.launch_count()
     finally:
@@ -39,9 +39,9 @@ def gpu_bake(scene, dirs, wts, t_min, sh_degree=1):
     return out
 
 
-def check(scene, dirs, wts, t_min, sh_degree=1, min_occluded=0.0):
-    sh, vis, launches = gpu_bake(scene, dirs, wts, t_min, sh_degree)
-    sh_ref, vis_ref, unstable = oracle.bake_visibility(scene, dirs, wts, t_min, sh_degree)
+def check(scene, dirs, wts, t_min, sh_degree=1, min_occluded=0.0, positions=False):
+    sh, vis, launches = gpu_bake(scene, dirs, wts, t_min, sh_degree, positions)
+    sh_ref, vis_ref, unstable = oracle.bake_visibility(scene, dirs, wts, t_min, sh_degree, positions=positions)
     assert launches >= 9 or scene.n < 2
     tol = np.where(unstable == 0, 5e-5, 1e-4 + 5e-3 * unstable)
     err = np.abs(vis.astype(np.float64) - vis_ref)
@@ -49,8 +49,10 @@ def check(scene, dirs, wts, t_min, sh_degree=1, min_occluded=0.0):
     assert not bad.any(), f"{bad.sum()} rays off, worst {err[bad].max():.3e} (stable worst {err[unstable == 0].max():.3e})"
     assert (vis_ref < 0.999).mean() >= min_occluded, "case is trivial"
     basis = [np.full(len(dirs), Y00)] + ([Y1 * dirs[:, 1], Y1 * dirs[:, 2], Y1 * dirs[:, 0]] if sh_degree else [])
+    if positions:   # per-Gaussian directions: bound every basis function by its maximum
+        basis = [np.full(len(dirs), Y00)] + ([np.full(len(dirs), Y1)] * 3 if sh_degree else [])
     for m, b in enumerate(basis):
-        bound = (tol * np.abs(wts * b)[None, :]).sum(1) + 1e-5
+        bound = (tol * np.abs(wts * b)[None, :]).sum(1) + 2e-5
         assert (np.abs(sh[:, m] - sh_ref[:, m]) <= bound).all(), f"SH coefficient {m}"
     return vis, vis_ref, unstable
 
@@ -166,3 +168,20 @@ def test_full_size_sampled_rows(cfg, K, n_rows, t_min):
     assert (vis_ref < 0.999).mean() > 0.05 and vis_ref.max() > 0.5
     bound = (tol * np.abs(wts * Y00)[None, :]).sum(1) + 1e-5
     assert (np.abs(sh[rows, 0] - sh_ref[:, 0]) <= bound).all()
+
+
+def test_positions_mode_matches_oracle():
+    """Rays towards known light positions: the OLAT lights of config 3 around the object, and
+    points inside the scene's bounding box (segments that end between the Gaussians)."""
+    scene = scaled(scenes.make_scene(3, n=3000, width=64, height=64, lights=24), 4.0)
+    lights = np.stack([np.asarray(l.position, np.float32) for l in scene.lights[0]])
+    wts = np.full(len(lights), 4 * np.pi / len(lights), np.float32)
+    vis, vis_ref, _ = check(scene, lights, wts, 0.05, min_occluded=0.2, positions=True)
+    assert vis_ref.min() < 0.05 and vis_ref.max() > 0.9
+    rng = np.random.default_rng(11)
+    inner = rng.uniform(-1.0, 1.0, size=(12, 3)).astype(np.float32)
+    check(scene, inner, np.ones(12, np.float32), 0.05, min_occluded=0.2, positions=True)
+    # a light on top of a Gaussian (closer than the ray start): nothing occludes
+    on_top = scene.means[:4] + np.float32(0.01)
+    sh, vis, _ = gpu_bake(scene, on_top, np.ones(4, np.float32), 0.05, positions=True)
+    assert vis[0, 0] == 1.0 and vis[1, 1] == 1.0 and vis[3, 3] == 1.0
