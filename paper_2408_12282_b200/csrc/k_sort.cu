@@ -9,7 +9,7 @@
 //
 // Structure of a pass (persistent CTAs pulling tickets, so a CTA only ever waits on tickets
 // that are already running -> forward progress):
-//   1. load 256 x ITEMS keys (ITEMS = 3, 7 or 15 by problem size) warp-striped (coalesced), rank them per warp with __match_any_sync
+//   1. load 256 x ITEMS keys (ITEMS = 3, 7 or 15 by problem size) warp-striped (coalesced), rank them per warp (lanes with the same digit, found with one ballot per digit bit)
 //      (stable: item order, then lane order), combine the per-warp digit counts,
 //   2. publish the CTA's digit counts and resolve its global offsets by decoupled look-back
 //      over the status words of earlier tickets (flag and 30-bit count share one word, so no
@@ -65,6 +65,17 @@ struct SortSmem {
   uint32_t ticket;
 };
 
+// Lanes of the warp whose digit equals this lane's: one ballot per digit bit (measured faster than
+// __match_any_sync on sm_100: 3 M keys x 4 passes 0.144 -> 0.109 ms).
+__device__ __forceinline__ unsigned same_digit_lanes(uint32_t d, uint32_t mask) {
+  unsigned pe = 0xFFFFFFFFu;
+  for (uint32_t b = 1; b <= mask; b <<= 1) {
+    const unsigned bal = __ballot_sync(0xFFFFFFFFu, (d & b) != 0u);
+    pe &= (d & b) ? bal : ~bal;
+  }
+  return pe;
+}
+
 // Processes tickets of 256 x ITEMS keys until the ticket counter runs out.
 template <int ITEMS>
 __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __restrict__ keys_in,
@@ -107,13 +118,13 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
     constexpr bool kHoist = ITEMS <= 7;
     if (kHoist) {
 #pragma unroll
-      for (int i = 0; i < ITEMS; ++i) peers[i] = __match_any_sync(0xFFFFFFFFu, (key[i] >> shift) & mask);
+      for (int i = 0; i < ITEMS; ++i) peers[i] = same_digit_lanes((key[i] >> shift) & mask, mask);
     }
     __syncwarp();
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
       const uint32_t d = (key[i] >> shift) & mask;
-      const unsigned pe = kHoist ? peers[i] : __match_any_sync(0xFFFFFFFFu, d);
+      const unsigned pe = kHoist ? peers[i] : same_digit_lanes(d, mask);
       const uint32_t r = __popc(pe & ((1u << lane) - 1u));
       const uint32_t base = sm.wcnt[warp][d];
       __syncwarp();
