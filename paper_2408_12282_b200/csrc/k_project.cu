@@ -171,11 +171,23 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
   const unsigned active = __ballot_sync(0xFFFFFFFFu, in_range);
   if (in_range) {
     const unsigned lane = threadIdx.x & 31;
+    // low digits are spread out: plain shared-memory atomics; the high digits (exponent, top of the
+    // mantissa) are usually the same in the whole warp: one atomic then (match.any is slow on sm_100)
 #pragma unroll
     for (int d = 0; d < 4; ++d) {
       const uint32_t dig = (key >> (8 * d)) & 255u;
-      const unsigned peers = __match_any_sync(active, dig);
-      if ((peers & ((1u << lane) - 1u)) == 0) atomicAdd(&s_hist[d * 256 + dig], __popc(peers));
+      if (d < 2) {
+        atomicAdd(&s_hist[d * 256 + dig], 1u);
+      } else {
+        const int leader = __ffs(active) - 1;
+        const uint32_t dig0 = __shfl_sync(active, dig, leader);
+        const bool uniform = __all_sync(active, dig == dig0);
+        if (uniform) {
+          if ((int)lane == leader) atomicAdd(&s_hist[d * 256 + dig], __popc(active));
+        } else {
+          atomicAdd(&s_hist[d * 256 + dig], 1u);
+        }
+      }
     }
   }
   const unsigned vmask = __ballot_sync(0xFFFFFFFFu, vis);
