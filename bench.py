@@ -38,7 +38,7 @@ from paper_2408_12282_b200 import multi, scenes  # noqa: E402
 METRIC = "Mpix/s (MLP + G-buffer splat + deferred shading)"
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of a stage's kernel, from the
 # `ncu --set full` captures summarised under profiles/ (r01_ncu_full.md): (config, stage) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, "raster"): 11663104, (3, "mlp"): 31867392, (3, "raster"): 267091712,
+NCU_DRAM_BYTES_PER_LAUNCH = {(2, "raster"): 11665664, (3, "mlp"): 31867392, (3, "raster"): 267091712,
                              (4, "raster"): 274415360, (5, "mlp"): 221394688, (5, "raster"): 1027052288}
 FP32_LANES_PER_SM = 128
 

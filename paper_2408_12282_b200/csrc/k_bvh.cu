@@ -228,25 +228,28 @@ bvh_refit_kernel(int n, float4* box_lo, float4* box_hi, const int* __restrict__ 
 
 // slab test of the ray o + t w, t >= 0 (iw = 1 / w, components of w nudged away from 0): entry
 // distance, or -1 on a miss
+template <bool POS>
 __device__ __forceinline__ float hit_box(const float4& lo, const float4& hi, const float o[3], const float iw[3],
                                          float t_max) {
   const float tx0 = (lo.x - o[0]) * iw[0], tx1 = (hi.x - o[0]) * iw[0];
   const float ty0 = (lo.y - o[1]) * iw[1], ty1 = (hi.y - o[1]) * iw[1];
   const float tz0 = (lo.z - o[2]) * iw[2], tz1 = (hi.z - o[2]) * iw[2];
   const float tn = fmaxf(fmaxf(fminf(tx0, tx1), fminf(ty0, ty1)), fmaxf(fminf(tz0, tz1), 0.f));
-  const float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fminf(fmaxf(tz0, tz1), t_max));
+  float tf = fminf(fminf(fmaxf(tx0, tx1), fmaxf(ty0, ty1)), fmaxf(tz0, tz1));
+  if (POS) tf = fminf(tf, t_max);
   // an inverted box is empty (Gaussians that never reach alpha_min)
   return (tn <= tf && lo.x <= hi.x) ? tn : -1.f;
 }
 
 constexpr int kBvhStack = 96;
 
+template <bool POS>
 __global__ void __launch_bounds__(128)
 bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* __restrict__ leaf,
                  const float4* __restrict__ box_lo, const float4* __restrict__ box_hi, int n_dirs,
                  const float* __restrict__ dirs, const float* __restrict__ weights, float t_min, int n_coef,
                  float* __restrict__ sh_out, float* __restrict__ vis_out, int dirs_per_group,
-                 float4* __restrict__ partial, int positions) {
+                 float4* __restrict__ partial) {
   pdl_prologue();
   const int k = blockIdx.x * 128 + threadIdx.x;
   if (k >= n) return;
@@ -259,7 +262,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
   for (int dk = dir_begin; dk < dir_end; ++dk) {
     float w[3] = {dirs[3 * dk], dirs[3 * dk + 1], dirs[3 * dk + 2]};
     float t_max = 3.0e38f;
-    if (positions) {  // the ray ends at the point dirs[dk]
+    if (POS) {  // the ray ends at the point dirs[dk]
       w[0] -= me.x; w[1] -= me.y; w[2] -= me.z;
       const float d = sqrtf(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
       const float id = d > 0.f ? 1.f / d : 0.f;
@@ -271,7 +274,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
 #pragma unroll
     for (int a = 0; a < 3; ++a) iw[a] = 1.f / (fabsf(w[a]) < 1e-20f ? copysignf(1e-20f, w[a]) : w[a]);
     float T = 1.f;
-    if (n >= 2 && finite3(o[0], o[1], o[2]) && t_max > 0.f) {
+    if (n >= 2 && finite3(o[0], o[1], o[2]) && (!POS || t_max > 0.f)) {
       int sp = 0;
       // nearer child first: the opaque surface next to the ray's start ends most blocked rays early
       // (the product is order independent, the early exit is not a change of the result)
@@ -287,7 +290,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
                              l1.z * d[0] + l2.x * d[1] + l2.y * d[2]};
         const float ww = w[0] * Sw[0] + w[1] * Sw[1] + w[2] * Sw[2];
         const float wd = w[0] * Sd[0] + w[1] * Sd[1] + w[2] * Sd[2];
-        const float t = fminf(t_max, fmaxf(0.f, -wd / ww));
+        const float t = POS ? fminf(t_max, fmaxf(0.f, -wd / ww)) : fmaxf(0.f, -wd / ww);
         const float e[3] = {fmaf(t, w[0], d[0]), fmaf(t, w[1], d[1]), fmaf(t, w[2], d[2])};
         const float m2 = e[0] * (l1.x * e[0] + l1.y * e[1] + l1.z * e[2]) + e[1] * (l1.y * e[0] + l1.w * e[1] + l2.x * e[2]) +
                          e[2] * (l1.z * e[0] + l2.x * e[1] + l2.y * e[2]);
@@ -299,7 +302,7 @@ bvh_trace_kernel(int n, const uint32_t* __restrict__ sorted_gid, const float4* _
       int node = 0;
       while (true) {
         const int cl = __float_as_int(box_lo[node].w), cr = __float_as_int(box_hi[node].w);
-        float tl = hit_box(box_lo[cl], box_hi[cl], o, iw, t_max), tr = hit_box(box_lo[cr], box_hi[cr], o, iw, t_max);
+        float tl = hit_box<POS>(box_lo[cl], box_hi[cl], o, iw, t_max), tr = hit_box<POS>(box_lo[cr], box_hi[cr], o, iw, t_max);
         bool dead = false;
         if (tl >= 0.f && cl >= n - 1) { dead = leaf_hit(cl); tl = -1.f; }
         if (!dead && tr >= 0.f && cr >= n - 1) { dead = leaf_hit(cr); tr = -1.f; }
@@ -393,9 +396,14 @@ int launch_bvh_trace(int64_t n, const BvhBuffers& b, int n_dirs, const float* di
   const int per = (n_dirs + groups - 1) / groups;
   groups = (n_dirs + per - 1) / per;
   const unsigned blocks = (unsigned)((n + 127) / 128);
-  launch_pdl(bvh_trace_kernel, dim3(blocks, groups), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
-             (const float4*)b.leaf, (const float4*)b.box_lo, (const float4*)b.box_hi, n_dirs, dirs, weights, t_min, n_coef,
-             sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr, positions);
+  if (positions)
+    launch_pdl(bvh_trace_kernel<true>, dim3(blocks, groups), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
+               (const float4*)b.leaf, (const float4*)b.box_lo, (const float4*)b.box_hi, n_dirs, dirs, weights, t_min,
+               n_coef, sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr);
+  else
+    launch_pdl(bvh_trace_kernel<false>, dim3(blocks, groups), dim3(128), 0, s, (int)n, (const uint32_t*)b.sorted_gid,
+               (const float4*)b.leaf, (const float4*)b.box_lo, (const float4*)b.box_hi, n_dirs, dirs, weights, t_min,
+               n_coef, sh_out, vis_out, per, groups > 1 ? scratch : (float4*)nullptr);
   if (groups == 1) return 1;
   launch_pdl(bvh_sh_reduce_kernel, dim3((unsigned)((n + kBvhThreads - 1) / kBvhThreads)), dim3(kBvhThreads), 0, s, (int)n,
              groups, (const float4*)scratch, n_coef, sh_out);
