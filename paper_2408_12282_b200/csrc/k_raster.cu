@@ -220,6 +220,18 @@ __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {  // 
       : "memory");
   return ok != 0;
 }
+// one try_wait: the hardware may park the thread until the phase completes or a time limit passes
+__device__ __forceinline__ bool mbar_try(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
   do {
@@ -481,7 +493,7 @@ raster_body(const CamParams& cam, const LightBatch& lights, int n_lights,
       const uint32_t par = (uint32_t)((g / NS - 1) & 1);
       if (!mbar_test(s_empty + st, par)) {
         if (!blocking) return false;
-        while (!mbar_test(s_empty + st, par))
+        while (!mbar_try(s_empty + st, par))  // parked between polls: the issue slots go to the working warps
           if (all_done()) return false;
       }
     }
