@@ -724,8 +724,8 @@ raster_shade_kernel(CamParams cam, LightBatch lights, int n_lights,
                                           sum_mode, wc, only_if_set, (int)blockIdx.x);
 }
 
-// Small images: the few longest tile lists (the first *n_long_ptr tiles of the work order, at most
-// cap_long) decide when the kernel ends if they are walked like the others.  The first cap_long * 4
+// Small images: the few longest tile lists (the first tiles of the work order, at most cap_long)
+// decide when the kernel ends if they are walked like the others.  The first cap_long * 4
 // CTAs of this kernel walk them with 4 entry slots per warp and 4 CTAs per tile (half the sequential
 // length), the other CTAs walk the remaining tiles with 2 slots and 2 CTAs per tile.
 template <int LB, int EL>
@@ -738,9 +738,15 @@ raster_mixed_kernel(CamParams cam, LightBatch lights, int n_lights,
                     float* __restrict__ rgb_out, float* __restrict__ gbuf_out,
                     float* __restrict__ aovd_out, float* __restrict__ aovs_out,
                     int64_t frame_stride_px, int sum_mode, const uint32_t* __restrict__ only_if_set,
-                    const uint32_t* __restrict__ n_long_ptr, int cap_long) {
+                    const uint32_t* __restrict__ bucket_starts, int long_log2, int cap_long) {
   pdl_prologue();
-  const int n_long = min((int)*n_long_ptr, cap_long);
+  // bucket_starts[k] = tiles with at least 2^k entries (they come first in the work order).  The long
+  // class is "at least 2^k entries" for the smallest k >= long_log2 that fits the cap_long * EL CTAs
+  // reserved for it: a rule on the list length alone, so that which tiles are walked in which shape
+  // (hence the order of their partial sums) does not depend on the arbitrary order inside a bucket.
+  int k = long_log2;
+  while (k < 31 && bucket_starts[k] > (uint32_t)cap_long) ++k;
+  const int n_long = (int)bucket_starts[k];
   const WeightCache none{};
   if ((int)blockIdx.x < cap_long * EL) {
     if ((int)blockIdx.x >= n_long * EL) return;
@@ -794,7 +800,7 @@ static int launch_mixed_e(const CamParams& cam, const LightBatch& lights, int n_
   }
   launch_pdl(raster_mixed_kernel<LB, EL>, dim3(kLongTilesCap * EL + tiles * 2), dim3(256), smem, s, cam, lights, n_lights,
              gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf, aov_d, aov_s,
-             frame_stride_px, sum_mode, only_if_set, (const uint32_t*)(gb.counters + DC_BUCKET_STARTS + long_log2),
+             frame_stride_px, sum_mode, only_if_set, (const uint32_t*)(gb.counters + DC_BUCKET_STARTS), long_log2,
              kLongTilesCap);
   return 1;
 }

@@ -317,12 +317,21 @@ def test_weight_cache_overflow_falls_back_to_the_list_walks(monkeypatch):
         np.testing.assert_array_equal(fallback[k].view(np.uint32), full[k].view(np.uint32))
 
 
-def test_run_to_run_determinism():
-    scene = scenes.make_scene(2, n=50000, width=320, height=240)
+@pytest.mark.parametrize("cfg,n,width,height", [
+    (2, 50000, 320, 240),
+    (1, 50000, 656, 200),   # dense small image: more long tile lists than the long-list CTAs of the mixed kernel
+])
+def test_run_to_run_determinism(cfg, n, width, height):
+    scene = scenes.make_scene(cfg, n=n, width=width, height=height)
     a = gpu_render(scene)
-    b = gpu_render(scene)
-    for k in ("rgb", "gbuffer", "sorted_vals", "tile_ranges", "mlp_out"):
-        np.testing.assert_array_equal(a[k], b[k])
+    for _ in range(3):
+        b = gpu_render(scene)
+        for k in ("rgb", "gbuffer", "sorted_vals", "tile_ranges", "mlp_out"):
+            np.testing.assert_array_equal(a[k].view(np.uint32) if a[k].dtype == np.float32 else a[k],
+                                          b[k].view(np.uint32) if b[k].dtype == np.float32 else b[k])
+    # and the same frame when other outputs are requested
+    c = gpu_render(scene, want=("rgb", "counters"))
+    np.testing.assert_array_equal(a["rgb"].view(np.uint32), c["rgb"].view(np.uint32))
 
 
 def test_empty_scene_and_zero_opacity():
