@@ -548,7 +548,7 @@ static void shade_impl(int width, int height, const OrcCamera* cam, const float*
     pc[k] = -((real)cam->R[0 + k] * (real)cam->t[0] + (real)cam->R[3 + k] * (real)cam->t[1] +
               (real)cam->R[6 + k] * (real)cam->t[2]);
   const real pi = (real)kPi;
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for schedule(static) if (height > 4)
   for (int py = 0; py < height; ++py)
     for (int px = 0; px < width; ++px) {
       const int64_t pidx = (int64_t)py * width + px;
