@@ -4,14 +4,19 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
 A step = one pass of the whole hot path (MLP + projection + sort + tile binning + G-buffer
-compositing + deferred shading) over one batch of synthetic input = one sssgs_render call
-producing every frame of one view of the workload (BASELINE.json configs[C-1]; default C=2, the
-configuration the metric is quoted on).  Prints ONE JSON line.
+compositing + deferred shading) over one batch of synthetic input = ONE sssgs_render call producing
+every frame of one view of the workload.  BASELINE.json's `metric` names no configuration, so the
+default workload is the largest single-GPU one, configs[4] (C = 5): 3 M Gaussians, 1024 x 1024, one
+view x its 16 lights per step.  Prints ONE JSON line:
 
   value     Mpix/s, inputs resident in HBM, CUDA events around each step, L2 flushed between
-            steps, step replayed from a CUDA graph (the launch configuration the tests check)
+            steps, step replayed from a CUDA graph (the launch configuration the tests check);
+            ms_per_step is the mean over the K timed steps, ms_per_step_median / _min beside it
   e2e       same metric through sssgs_render_host with pinned HOST buffers (H2D + D2H inside)
   roofline  the step's dominant kernel against its bound, timed with events inside the library
+  stages    every stage of the step: ms, launches, achieved vs measured (and nominal) peak
+  configs   the same protocol on all five BASELINE configs (ms/step median and min, Mpix/s,
+            Gaussians/s, dominant stage and its roofline fraction)
   cpu_baseline  the CPU oracle, as it stands, on this box's host cores (rank 0, N = 1)
 
 --impl reference times the CPU oracle alone (the reference arm of this tier).
@@ -36,11 +41,16 @@ sys.path.insert(0, ROOT)
 from paper_2408_12282_b200 import multi, scenes  # noqa: E402
 
 METRIC = "Mpix/s (MLP + G-buffer splat + deferred shading)"
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of a stage's kernel, from the
-# `ncu --set full` captures summarised under profiles/ (r01_ncu_full.md): (config, stage) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {(2, "raster"): 11665664, (3, "mlp"): 31867392, (3, "raster"): 267091712,
-                             (4, "raster"): 274415360, (5, "mlp"): 221394688, (5, "raster"): 1027052288}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of a stage's kernel, from the
+# `ncu --set full` captures summarised under profiles/ (r02_ncu_full.md): (config, stage) -> bytes
+NCU_DRAM_BYTES_PER_LAUNCH = {}
+_ncu_path = os.path.join(ROOT, "profiles", "r02_dram_bytes_per_launch.json")
+if os.path.exists(_ncu_path):
+    NCU_DRAM_BYTES_PER_LAUNCH = {tuple(k.split(":")): v for k, v in json.load(open(_ncu_path)).items()
+                                 if not k.startswith("_")}
 FP32_LANES_PER_SM = 128
+HBM_NOMINAL_GBS = 8000.0   # BASELINE.json north_star: "~8 TB/s"
+MAX_INSTANCES_PER_GAUSSIAN = 20
 
 
 def load_peaks():
@@ -51,6 +61,13 @@ def load_peaks():
                     bf16_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
                     sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
     return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sustained=1400.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def load_oracle_counters():
+    """Work counters of every config's first frame, written by oracle/make_workload_counters.py
+    (oracle only).  They are the denominators of the raster / pre-pass roofline figures."""
+    p = os.path.join(ROOT, "oracle", "workload_counters.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
 
 
 class ClockSampler:
@@ -85,19 +102,20 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in self.rows:
             try:
                 sm.append(float(r[0]))
                 mx.append(float(r[1]))
+                pw.append(float(r[2]))
                 for k, nm in enumerate(names):
                     if r[3 + k].lower().startswith("active"):
                         reasons.add(nm)
             except Exception:
                 pass
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def workload(cfg):
@@ -106,21 +124,89 @@ def workload(cfg):
     return s, s.cameras[:1], s.lights[0], len(s.lights[0])
 
 
-def oracle_sample(scene, min_seconds=0.0, max_frames=1):
-    """Times the CPU oracle, as it stands, on a bounded sample: whole-path renders of the first
-    (view, light) frame, repeated until `min_seconds` of CPU work (at least `max_frames` = 1 frame)."""
-    import oracle
-    t0 = time.perf_counter()
-    frames, res = 0, None
-    while frames < max_frames or time.perf_counter() - t0 < min_seconds:
-        res = oracle.render_frame(scene, 0, 0, mlp_mode=1)   # projection, lists, MLP, compositing, shading
-        frames += 1
-    dt = time.perf_counter() - t0
+def config_dict(cfg, scene, fps):
+    """The `config` object: identical in the GPU arm and in the reference arm (same workload)."""
     cam = scene.cameras[0]
-    return dict(seconds=dt, frames=frames, mpix_s=frames * cam.width * cam.height / dt / 1e6,
-                cores=oracle.num_threads(), res=res)
+    m = scene.mlp
+    return {"workload": f"configs[{cfg - 1}] {scene.name}: {scene.n} Gaussians, {cam.width}x{cam.height}, "
+                        f"one view x {fps} light(s) per step (view 0 of {len(scene.cameras)})",
+            "gaussians": int(scene.n), "width": int(cam.width), "height": int(cam.height),
+            "frames_per_step": int(fps), "views_in_config": len(scene.cameras),
+            "mlp": f"{m.in_dim} -> {'x'.join(str(w) for w in m.trunk_width)} -> 3+1",
+            "mlp_compute": "fp16 x fp16 -> fp32 (weights bf16-exact)",
+            "l2": "flushed between timed steps (256 MiB memset)", "launch": "CUDA graph replay"}
 
 
+# ---------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample(scene, mlp_rows_budget=200_000):
+    """One whole-path render of the first (view, light) frame by the CPU oracle, as it stands.  A BOUNDED sample:
+    projection, lists, compositing and shading run in full; the MLP (plain loops, ~60 us per row and core) runs
+    on a seeded sample of at most `mlp_rows_budget` rows and its time is extrapolated linearly to all rows (a
+    row's cost does not depend on the row)."""
+    import oracle
+    cam, lt = scene.cameras[0], scene.lights[0][0]
+    t0 = time.perf_counter()
+    proj = oracle.project(scene, cam)
+    keys, vals, ranges = oracle.build_lists(proj)
+    t_geo = time.perf_counter() - t0
+    n = int(scene.n)
+    if n > mlp_rows_budget:
+        rows = np.sort(np.random.default_rng(0).choice(n, size=mlp_rows_budget, replace=False))
+        sub = scenes.subset(scene, rows)
+    else:
+        rows, sub = np.arange(n), scene
+    t0 = time.perf_counter()
+    x = oracle.mlp_inputs(sub, cam, lt.position)
+    y = oracle.mlp_forward(x, scene.mlp, 2)
+    t_mlp_sample = time.perf_counter() - t0
+    t_mlp = t_mlp_sample * n / max(len(rows), 1)
+    mlp_out = np.zeros((n, 4))
+    mlp_out[rows] = y
+    t0 = time.perf_counter()
+    comp = oracle.composite(scene, cam, proj, oracle.channels(scene, proj, mlp_out), vals, ranges)
+    oracle.shade(cam, lt, comp.gbuf)
+    t_img = time.perf_counter() - t0
+    total = t_geo + t_mlp + t_img
+    return dict(seconds=total, cpu_seconds_spent=t_geo + t_mlp_sample + t_img, frames=1,
+                mpix_s=cam.width * cam.height / total / 1e6, cores=oracle.num_threads(),
+                mlp_rows_timed=int(len(rows)), p_eval=comp.p_eval, p_blend=comp.p_blend,
+                sample=(f"one whole-path render of the first (view, light) frame of {scene.name}: projection, lists, "
+                        f"compositing, shading in full ({t_geo + t_img:.1f} s); fp16-emulating MLP timed on "
+                        f"{len(rows)} of {n} rows ({t_mlp_sample:.1f} s) and scaled to all rows ({t_mlp:.1f} s)"))
+
+
+def run_reference(args, rank):
+    """Reference arm of this tier: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    scene, cams, lights, fps = workload(args.config)
+    cam = cams[0]
+    steps = min(args.steps, 6 if scene.n > 200_000 else 30)      # bounded: a step is seconds of CPU work
+    warm = min(args.warmup, 1 if scene.n > 200_000 else 3)
+    for _ in range(warm):
+        oracle_sample(scene)
+    t, cores, sample = 0.0, 1, ""
+    for _ in range(steps):
+        r = oracle_sample(scene)
+        t += r["seconds"]
+        cores, sample = r["cores"], r["sample"]
+    val = steps * cam.width * cam.height / t / 1e6
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "Mpix/s", "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": t / steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(args.config, scene, fps),
+        "cpu_baseline": {"value": val, "unit": "Mpix/s", "cores": cores, "kind": "oracle",
+                         "sample": sample + "; one frame per step (the oracle has no light batching)"},
+        "e2e": {"value": val, "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---------------------------------------------------------------------------------------------------
+# Work models (DESIGN.md section 5): algorithmic bytes / flops of each stage for ONE step
+# ---------------------------------------------------------------------------------------------------
 def mlp_flops_per_row(mlp):
     d, fl = mlp.in_dim, 0
     for w in mlp.trunk_width:
@@ -134,54 +220,123 @@ def mlp_flops_per_row(mlp):
     return fl + 2 * di
 
 
-def stage_models(scene, nl, n_vis, inst, counters, peaks, num_sms, mlp_rows):
-    """Algorithmic work of each stage for ONE step."""
+def stage_models(scene, nl, n_vis, inst, ocnt, peaks, num_sms, mlp_rows, swept):
     n = scene.n
-    cam = scene.cameras[0]
-    npix = cam.width * cam.height
-    feat = scene.feat.shape[1]
     alu_peak = num_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s
     m = {
         "project": ("hbm", 44.0 * n + 48.0 * n_vis),
         "depth_sort": ("hbm", (3 * 16.0 + 12.0) * n),
         "emit": ("hbm", 16.0 * n + 8.0 * inst),
-        "tile_sort": ("hbm", 16.0 * inst * (2 if (cam.width + 15) // 16 * ((cam.height + 15) // 16) > 256 else 1)),
+        "tile_sort": ("hbm", 16.0 * inst),     # ONE stable pass over (tile, index) pairs is the algorithmic minimum
+        "ranges": ("hbm", 4.0 * inst),
         # rows the MLP actually evaluated (in a sweep: the Gaussians blended at some pixel of the view)
         "mlp": ("tensor", float(mlp_flops_per_row(scene.mlp)) * mlp_rows * nl),
     }
-    if counters is not None:
-        p_eval, p_blend = counters
-        m["raster"] = ("alu", 10.0 * p_eval + (17.0 + 8.0 * (nl - 1)) * p_blend)
-    else:
-        m["raster"] = ("alu", None)
+    if ocnt:
+        pe, pb = float(ocnt["p_eval"]), float(ocnt["p_blend"])
+        if swept:   # pre-pass: alpha + transmittance chain once per view; walks: blends only
+            m["prepass"] = ("alu", 10.0 * pe + 3.0 * pb)
+            m["raster"] = ("alu", 2.0 * (11.0 + 4.0 * nl) * pb)
+        else:
+            m["raster"] = ("alu", 10.0 * pe + (17.0 + 8.0 * (nl - 1)) * pb)
     pk = {"hbm": (peaks["hbm"], "GB/s"), "tensor": (peaks["bf16_burst"], "TFLOP/s"), "alu": (alu_peak, "TFLOP/s")}
     return m, pk
 
 
-def run_reference(args, rank):
-    """Reference arm of this tier: the CPU oracle, as it stands, on the host cores."""
-    if rank != 0:
-        return
-    scene, cams, lights, fps = workload(args.config)
-    cam = cams[0]
-    for _ in range(args.warmup if args.config <= 2 else 0):
-        oracle_sample(scene)
-    t, frames, cores = 0.0, 0, 1
-    for _ in range(args.steps):
-        r = oracle_sample(scene)
-        t += r["seconds"]
-        frames += r["frames"]
-        cores = r["cores"]
-    val = frames * cam.width * cam.height / t / 1e6
-    sample = f"first (view, light) frame of configs[{args.config - 1}] per step, whole path, bf16-emulating MLP"
-    print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": val, "unit": "Mpix/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{args.config - 1}] {scene.name}", "frames_per_step": 1},
-        "cpu_baseline": {"value": val, "unit": "Mpix/s", "cores": cores, "kind": "oracle", "sample": sample},
-        "e2e": {"value": val, "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gpu_launches": 0}))
+class ConfigRun:
+    """One config on one GPU: device-resident scene, a CUDA graph of one step, timed replays, per-stage
+    device times.  The timing protocol of the headline number and of every row of `configs`."""
+
+    def __init__(self, cfg, local_rank, args, scene=None):
+        import torch
+        from paper_2408_12282_b200 import binding
+        self.torch, self.binding, self.cfg = torch, binding, cfg
+        self.dev = torch.device("cuda", local_rank)
+        if scene is None:
+            self.scene, self.cams, self.lights, self.fps = workload(cfg)
+        else:
+            self.scene, self.cams, self.lights, self.fps = scene, scene.cameras[:1], scene.lights[0], len(scene.lights[0])
+        self.cam = self.cams[0]
+        self.npix = self.cam.width * self.cam.height
+        self.kw = dict(sum_lights=args.sum_lights, forward=args.forward)
+        self.R = binding.Renderer(self.scene, max_instances=int(MAX_INSTANCES_PER_GAUSSIAN * self.scene.n),
+                                  device=local_rank,
+                                  compute=binding.SSSGS_COMPUTE_BF16 if args.bf16 else binding.SSSGS_COMPUTE_FP16)
+        self.outs = self.R.alloc_outputs(1, len(self.lights), self.cam.width, self.cam.height, ("rgb", "counters"))
+        for _ in range(2):
+            self.render()
+        torch.cuda.synchronize()
+        self.cnt = self.outs["counters"][0].tolist()
+        if self.cnt[binding.CNT_OVERFLOW] or self.cnt[binding.CNT_SORT_ERROR]:
+            raise RuntimeError(f"render failed: counters {self.cnt}")
+        self.launches = self.R.launch_count()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph):
+            self.render()
+
+    def render(self):
+        self.R.render(cams=self.cams, lights=self.lights, outputs=self.outs, **self.kw)
+
+    def timed(self, steps, warmup, flush, barrier=lambda: None):
+        torch = self.torch
+        stream = torch.cuda.current_stream(self.dev)
+        for _ in range(max(warmup, 3)):
+            flush.zero_()
+            self.graph.replay()
+        barrier()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        t_wall = time.perf_counter()
+        for a, b in ev:
+            flush.zero_()            # L2 flush between timed iterations (outside the event pair)
+            a.record(stream)
+            self.graph.replay()
+            b.record(stream)
+        barrier()
+        t_wall = time.perf_counter() - t_wall
+        return [a.elapsed_time(b) for a, b in ev], t_wall
+
+    def stage_times(self, reps, flush):
+        """Per-stage device times: events inside the library, stages serialised, L2 flushed."""
+        b = self.binding
+        b.sssgs_profile_enable(self.R.ctx, True)
+        acc, nlaunch = None, None
+        for _ in range(reps):
+            flush.zero_()
+            self.render()
+            ms, nlaunch = b.sssgs_profile_read(self.R.ctx)
+            acc = ms if acc is None else {k: acc[k] + ms[k] for k in ms}
+        b.sssgs_profile_enable(self.R.ctx, False)
+        return {k: v / reps for k, v in acc.items()}, nlaunch
+
+    def stages(self, stage_ms, nlaunch, ocnt, peaks, num_sms):
+        b = self.binding
+        nl = len(self.lights)
+        mlp_rows = self.cnt[b.CNT_MLP_ROWS] or self.scene.n
+        swept = nlaunch.get("prepass", 0) > 0
+        inst = min(self.cnt[b.CNT_INSTANCES], MAX_INSTANCES_PER_GAUSSIAN * self.scene.n)
+        models, pk = stage_models(self.scene, nl, self.cnt[b.CNT_NVIS], inst, ocnt, peaks, num_sms, mlp_rows, swept)
+        out = {}
+        for k, ms in stage_ms.items():
+            if nlaunch[k] == 0:
+                continue
+            e = {"ms": round(ms, 5), "launches": nlaunch[k]}
+            if k in models and ms > 0:
+                bound, work = models[k]
+                ach = work / (ms * 1e-3) / (1e9 if bound == "hbm" else 1e12)
+                e.update(bound=bound, achieved=round(ach, 3), unit=pk[bound][1], frac=round(ach / pk[bound][0], 4))
+                if bound == "hbm":
+                    e["frac_of_nominal_8TBs"] = round(ach / HBM_NOMINAL_GBS, 4)
+            out[k] = e
+        return out, pk
+
+    def close(self):
+        self.graph = None
+        self.R.close()
+
+
+def summarize(step_ms):
+    a = np.asarray(step_ms, np.float64)
+    return float(a.mean()), float(np.median(a)), float(a.min())
 
 
 def run_gpu(args, rank, world, local_rank):
@@ -194,136 +349,132 @@ def run_gpu(args, rank, world, local_rank):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     peaks = load_peaks()
-    scene, cams, lights, fps = workload(args.config)
-    cam = cams[0]
-    npix = cam.width * cam.height
-    nl = len(lights)
-    R = binding.Renderer(scene, max_instances=int(20 * scene.n), device=local_rank)
-    outs = R.alloc_outputs(1, nl, cam.width, cam.height, ("rgb", "counters"))
+    ocnt_all = load_oracle_counters()
     num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
-    # nvidia-smi samples clocks / throttle reasons from here to the end of the e2e loop: the timed
-    # region itself lasts only tens of milliseconds, so every sample is taken under this load
+    # nvidia-smi samples clocks / throttle reasons from here to the end of the e2e loop
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    # ---- warm-up (un-captured), then capture one step into a CUDA graph -------------------------
-    for _ in range(2):
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
-    torch.cuda.synchronize()
-    cnt = outs["counters"][0].tolist()
-    if cnt[binding.CNT_OVERFLOW] or cnt[binding.CNT_SORT_ERROR]:
-        raise RuntimeError(f"render failed: counters {cnt}")
-    launches_per_step = R.launch_count()
-    graph = torch.cuda.CUDAGraph()
-    with torch.cuda.graph(graph):
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
     def barrier():
         torch.cuda.synchronize()
         multi.barrier()
         torch.cuda.synchronize()
 
-    stream = torch.cuda.current_stream(dev)
-    for _ in range(max(args.warmup, 3)):
-        flush.zero_()
-        graph.replay()
-    barrier()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    t_wall = time.perf_counter()
-    for a, b in ev:
-        flush.zero_()            # L2 flush between timed iterations (outside the event pair)
-        a.record(stream)
-        graph.replay()
-        b.record(stream)
-    barrier()
-    t_wall = time.perf_counter() - t_wall
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    total_ms = multi.max_over_ranks(total_ms, dev)
+    run = ConfigRun(args.config, local_rank, args)
+    scene, cam, fps, npix = run.scene, run.cam, run.fps, run.npix
+    step_ms, t_wall = run.timed(args.steps, args.warmup, flush, barrier)
+    total_ms = multi.max_over_ranks(float(sum(step_ms)), dev)
     value = multi.whole_job_mpix_per_s(world, args.steps, fps, npix, total_ms)
-
-    # ---- per-stage device times (events inside the library, same step, L2 flushed) --------------
-    binding.sssgs_profile_enable(R.ctx, True)
-    acc, nlaunch = None, None
-    for _ in range(args.steps):
-        flush.zero_()
-        R.render(cams=cams, lights=lights, outputs=outs, sum_lights=args.sum_lights, forward=args.forward)
-        ms, nlaunch = binding.sssgs_profile_read(R.ctx)
-        acc = ms if acc is None else {k: acc[k] + ms[k] for k in ms}
-    binding.sssgs_profile_enable(R.ctx, False)
-    stage_ms = {k: v / args.steps for k, v in acc.items()}
+    mean_ms, med_ms, min_ms = summarize(step_ms)
+    stage_ms, nlaunch = run.stage_times(min(args.steps, 10), flush)
 
     # ---- end to end through the C ABI with pinned host buffers -------------------------------------
-    H = binding.HostRenderer(scene, max_instances=int(20 * scene.n), device=local_rank)
+    H = binding.HostRenderer(scene, max_instances=int(MAX_INSTANCES_PER_GAUSSIAN * scene.n), device=local_rank)
     for _ in range(2):
-        H.render(cams, lights)
+        H.render(run.cams, run.lights)
     barrier()
     t0 = time.perf_counter()
-    e2e_steps = max(3, min(args.steps, 20))
+    e2e_steps = max(3, min(args.steps, 10))
     for _ in range(e2e_steps):
-        H.render(cams, lights)
-    t_e2e = time.perf_counter() - t0
-    t_e2e = multi.max_over_ranks(t_e2e, dev)
+        H.render(run.cams, run.lights)
+    t_e2e = multi.max_over_ranks(time.perf_counter() - t0, dev)
     e2e_val = multi.whole_job_mpix_per_s(world, e2e_steps, fps, npix, t_e2e * 1e3)
     h2d, d2h = H.h2d_bytes, H.d2h_bytes
     H.close()
+    del H
     if rank == 0 and len(sampler.rows) < 3:   # keep the GPU busy until a few samples exist
         t_end = time.perf_counter() + 1.5
         while time.perf_counter() < t_end and len(sampler.rows) < 3:
             flush.zero_()
-            graph.replay()
+            run.graph.replay()
             torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
 
     if rank == 0:
-        cpu = None
-        counters = None
-        if world == 1 and not args.no_cpu_baseline:
-            r = oracle_sample(scene, min_seconds=12.0)
-            cpu = {"value": r["mpix_s"], "unit": "Mpix/s", "cores": r["cores"], "kind": "oracle",
-                   "sample": f"{r['frames']} whole-path renders of the first (view, light) frame of "
-                             f"configs[{args.config - 1}] (bf16-emulating MLP), {r['seconds']:.1f} s of CPU work"}
-            counters = (r["res"].comp.p_eval, r["res"].comp.p_blend)
-        mlp_rows = cnt[binding.CNT_MLP_ROWS] or scene.n
-        models, pk = stage_models(scene, nl, cnt[binding.CNT_NVIS], min(cnt[binding.CNT_INSTANCES], 20 * scene.n),
-                                  counters, peaks, num_sms, mlp_rows)
-        stages = {}
-        for k, ms in stage_ms.items():
-            e = {"ms": round(ms, 5), "launches": nlaunch[k]}
-            if k in models and models[k][1] is not None and ms > 0:
-                bound, work = models[k]
-                ach = work / (ms * 1e-3) / (1e9 if bound == "hbm" else 1e12)
-                e.update(bound=bound, achieved=round(ach, 3), unit=pk[bound][1], frac=round(ach / pk[bound][0], 4))
-            stages[k] = e
+        key = f"configs[{args.config - 1}]"
+        ocnt = ocnt_all.get(key)
+        stages, pk = run.stages(stage_ms, nlaunch, ocnt, peaks, num_sms)
+        if ocnt and not args.sum_lights and not args.forward:   # the device's own counters against the oracle's
+            assert ocnt["instances"] == run.cnt[binding.CNT_INSTANCES] and ocnt["n_vis"] == run.cnt[binding.CNT_NVIS], \
+                (ocnt, run.cnt)
         dom = max(stage_ms, key=stage_ms.get)
-        roof = {"kernel": dom, "bound": stages[dom].get("bound"), "achieved": stages[dom].get("achieved"),
-                "peak": round(pk[stages[dom]["bound"]][0], 2) if "bound" in stages[dom] else None,
-                "unit": stages[dom].get("unit"), "frac": stages[dom].get("frac"),
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, dom)),
-                "peak_source": peaks["source"] if stages[dom].get("bound") != "alu" else
+        sd = stages[dom]
+        roof = {"kernel": dom, "bound": sd.get("bound"), "achieved": sd.get("achieved"),
+                "peak": round(pk[sd["bound"]][0], 2) if "bound" in sd else None,
+                "unit": sd.get("unit"), "frac": sd.get("frac"),
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((str(args.config), dom)),
+                "launches_per_step": sd.get("launches"),
+                "peak_source": peaks["source"] if sd.get("bound") != "alu" else
                 "derived: SMs x 128 fp32 lanes x 2 x clocks.max.sm (DESIGN.md)",
                 "share_of_step": round(stage_ms[dom] / sum(stage_ms.values()), 3)}
+        if sd.get("bound") == "hbm":
+            roof["frac_of_nominal_8TBs"] = sd.get("frac_of_nominal_8TBs")
+        row = dict(ms_per_step_median=round(med_ms, 5), ms_per_step_min=round(min_ms, 5), frames_per_step=fps,
+                   mpix_s=round(fps * npix / med_ms / 1e3, 1), gaussians_per_s=round(fps * scene.n / (med_ms * 1e-3), 0),
+                   dominant_stage=dom, dominant_frac=sd.get("frac"), dominant_bound=sd.get("bound"),
+                   mlp_tensor_frac=stages.get("mlp", {}).get("frac"),
+                   stage_ms={k: v["ms"] for k, v in stages.items()})
+        table = {key: row}
+        launches_per_step = run.launches
+        cnt_head, mlp_rows_head = run.cnt, (run.cnt[binding.CNT_MLP_ROWS] or scene.n)
+        run.close()
+        del run
+        torch.cuda.empty_cache()
+        # ---- the same protocol on the other BASELINE configs ---------------------------------------
+        if world == 1 and not args.no_table and not args.sum_lights and not args.forward:
+            for c in (1, 2, 3, 4, 5):
+                k = f"configs[{c - 1}]"
+                if k in table:
+                    continue
+                r = ConfigRun(c, local_rank, args)
+                sm, _ = r.timed(min(args.steps, 10), 3, flush)
+                st_ms, nl_ = r.stage_times(3, flush)
+                st, _pk = r.stages(st_ms, nl_, ocnt_all.get(k), peaks, num_sms)
+                _, med, mn = summarize(sm)
+                d = max(st_ms, key=st_ms.get)
+                table[k] = dict(ms_per_step_median=round(med, 5), ms_per_step_min=round(mn, 5), frames_per_step=r.fps,
+                                mpix_s=round(r.fps * r.npix / med / 1e3, 1),
+                                gaussians_per_s=round(r.fps * r.scene.n / (med * 1e-3), 0),
+                                dominant_stage=d, dominant_frac=st[d].get("frac"), dominant_bound=st[d].get("bound"),
+                                mlp_tensor_frac=st.get("mlp", {}).get("frac"),
+                                stage_ms={kk: v["ms"] for kk, v in st.items()})
+                r.close()
+                del r
+                torch.cuda.empty_cache()
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            r = oracle_sample(scene)
+            cpu = {"value": r["mpix_s"], "unit": "Mpix/s", "cores": r["cores"], "kind": "oracle",
+                   "sample": r["sample"] + f"; {r['cpu_seconds_spent']:.1f} s of CPU work"}
+        cfg_d = config_dict(args.config, scene, fps)
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32 (raster/shade) + bf16 x bf16 -> f32 (MLP)",
-            "data": "synthetic",
-            "config": {"workload": f"configs[{args.config - 1}] {scene.name}", "gaussians": scene.n,
-                       "width": cam.width, "height": cam.height, "frames_per_step": fps,
-                       "l2": "flushed between timed steps (256 MiB memset)", "launch": "CUDA graph replay",
-                       "instances": cnt[binding.CNT_INSTANCES], "mlp_rows_per_light": mlp_rows,
-                       "sum_lights": bool(args.sum_lights), "forward_shading": bool(args.forward)},
-            "ms_per_frame": total_ms / args.steps / fps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "ms_per_step_median": med_ms, "ms_per_step_min": min_ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 (raster/shade) + " + ("bf16 x bf16" if args.bf16 else "fp16 x fp16") + " -> f32 (MLP)",
+            "data": "synthetic", "config": cfg_d,
+            "variant": {"sum_lights": bool(args.sum_lights), "forward_shading": bool(args.forward)},
+            "counters": {"n_vis": cnt_head[binding.CNT_NVIS], "instances": cnt_head[binding.CNT_INSTANCES],
+                         "mlp_rows_per_light": mlp_rows_head, "oracle": ocnt},
+            "ms_per_frame": med_ms / fps,
             "gaussians_per_s": world * args.steps * fps * scene.n / (total_ms * 1e-3),
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": "Mpix/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps},
+                    "steps": e2e_steps,
+                    "note": "sssgs_render_host uploads the WHOLE scene and downloads every frame in each call "
+                            "(one crossing per call by design): PCIe-bound"},
             "gpu_launches": launches_per_step * args.steps,
-            "roofline": roof, "stages": stages, "cpu_baseline": cpu,
+            "roofline": roof, "stages": stages, "configs": table, "cpu_baseline": cpu,
+            "peaks": {"hbm_gbs_measured": peaks["hbm"], "hbm_gbs_nominal": HBM_NOMINAL_GBS,
+                      "bf16_tflops_burst": peaks["bf16_burst"], "bf16_tflops_sustained": peaks["bf16_sustained"],
+                      "source": peaks["source"]},
             "wall_s_timed_region": round(t_wall, 4)}))
-    R.close()
+    else:
+        run.close()
     if world > 1:
         dist.destroy_process_group()
 
@@ -346,7 +497,7 @@ def run_bake(args, local_rank):
     scene, cams, lights, fps = workload(args.config)
     K, t_min = args.bake, 0.05
     dirs, wts = fibonacci_dirs(K)
-    R = binding.Renderer(scene, max_instances=int(20 * scene.n), device=local_rank)
+    R = binding.Renderer(scene, max_instances=int(MAX_INSTANCES_PER_GAUSSIAN * scene.n), device=local_rank)
     d_dirs, d_wts = torch.from_numpy(dirs).to(dev), torch.from_numpy(wts).to(dev)
     for _ in range(max(args.warmup, 3)):
         sh, _ = R.bake_visibility(d_dirs, d_wts, t_min)
@@ -383,11 +534,14 @@ def run_bake(args, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5, 6])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6],
+                    help="BASELINE.json configs[C-1]; default 5 = the largest single-GPU configuration")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-table", action="store_true", help="skip the per-config table (`configs`)")
+    ap.add_argument("--bf16", action="store_true", help="MLP with bf16 layer inputs (SSSGS_COMPUTE_BF16) instead of fp16")
     ap.add_argument("--forward", action="store_true",
                     help="the paper's 'w/o deferred' variant (SSSGS_FORWARD_SHADING): Eq. 7 per Gaussian, RGB composited")
     ap.add_argument("--sum-lights", action="store_true",
@@ -399,8 +553,6 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
-        if args.steps > 60:
-            args.steps = 60  # bounded: each step is seconds of CPU work
         run_reference(args, rank)
         return
     if args.bake:

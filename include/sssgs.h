@@ -16,6 +16,7 @@
  * Conventions
  *   - Every pointer inside sssgs_gaussians / sssgs_mlp / sssgs_out is a DEVICE pointer for
  *     sssgs_render and a HOST pointer for sssgs_render_host.  cams / lights are HOST arrays.
+ *     All cameras of one call must share one image size (frames are laid out [F][H][W]).
  *   - All memory reachable through the argument structs is caller-owned: the library never
  *     frees it and never keeps a pointer to it after the call's work has finished.
  *   - Device pointers must be 16-byte aligned; arrays are dense, row-major, fp32 unless noted.
@@ -27,6 +28,9 @@
  *   - Every function returns 0 (SSSGS_OK) or a negative sssgs_status; no exceptions or aborts
  *     cross the ABI.  sssgs_last_error() returns a human-readable description.
  *   - There is no CPU fallback: without an sm_100 device sssgs_create fails (SSSGS_EARCH).
+ *   - A context belongs to the device of sssgs_config.device: every entry point makes that device
+ *     current for the duration of the call and restores the caller's device before returning, so
+ *     contexts on several GPUs can be driven from one thread.
  */
 #ifndef SSSGS_H_
 #define SSSGS_H_
@@ -49,6 +53,8 @@ typedef enum {
 
 enum { SSSGS_ACT_RELU = 0, SSSGS_ACT_LEAKY_RELU = 1 };
 enum { SSSGS_F32 = 0, SSSGS_BF16 = 1 };
+/* sssgs_mlp.compute: 16-bit type of the tensor-core operands (weights and every layer input) */
+enum { SSSGS_COMPUTE_FP16 = 0, SSSGS_COMPUTE_BF16 = 1 };
 
 /* flags of sssgs_render */
 enum {
@@ -71,7 +77,8 @@ enum {
 /* indices into sssgs_out.counters (int64 each, per camera: counters[cam*SSSGS_NCOUNTERS + k]) */
 enum {
   SSSGS_CNT_NVIS = 0,      /* Gaussians that survive projection/culling                       */
-  SSSGS_CNT_INSTANCES = 1, /* I = sum of tiles touched (tile list length, before clamping)   */
+  SSSGS_CNT_INSTANCES = 1, /* I = sum of tiles touched (tile list length, before clamping to
+                              max_instances; saturates at 2^30 - 1, which always flags overflow) */
   SSSGS_CNT_OVERFLOW = 2,  /* 1 if I > max_instances: the frame content is then undefined    */
   SSSGS_CNT_SORT_ERROR = 3,/* non-zero if a look-back wait exceeded its spin bound (bug trap) */
   SSSGS_CNT_MLP_ROWS = 4,  /* Gaussians the MLP evaluated per light: n, or -- in a sweep of >= 4
@@ -125,8 +132,13 @@ typedef struct {
  *     v(1) | gamma(mu)(24) = for k=0..3 [sin(2^k pi mu_xyz), cos(2^k pi mu_xyz)] | feat(F) ]
  * params: packed fp32 (or bf16), per layer W[out][in] row-major then b[out]; order = trunk
  * layers, SSS head (3 outputs, sigmoid), incident-head hidden layers, incident output (1,
- * ReLU).  Hidden layers use `activation`.  Compute is bf16 x bf16 -> fp32 on the tensor cores:
- * weights and every layer input are rounded to bf16 (RNE); biases stay fp32.
+ * ReLU).  Hidden layers use `activation`.  Compute is 16 bit x 16 bit -> fp32 on the tensor cores:
+ * weights and every layer input are rounded (RNE) to `compute` = binary16 (default; finite overflow
+ * saturates to +-65504) or bf16; accumulation, biases and activations are fp32.  binary16 is the
+ * default because the incident-light output is an unbounded ReLU: with bf16 layer inputs it misses the
+ * 1e-2 bound of the specification on up to ~1 % of the rows, with binary16 (same tensor-core rate) it
+ * stays within 3e-3.  bf16-stored weights convert to binary16 exactly unless
+ * they are below 2^-14 in magnitude.
  * All widths must be multiples of 16 and <= 128.
  * precomputed_out: if non-NULL the MLP is skipped and these values are used instead
  * ([n_cam][n_light][n][4], = (L_SSS rgb, L_in)); lets a caller edit the residual (L169) and
@@ -143,6 +155,7 @@ typedef struct {
   const void* params;
   size_t params_bytes;
   const float* precomputed_out;
+  int compute;       /* SSSGS_COMPUTE_FP16 (0, default) | SSSGS_COMPUTE_BF16 */
 } sssgs_mlp;
 
 /* Pinhole camera.  World -> camera: p_c = R p + t (R row-major); the camera looks down +z,
@@ -242,8 +255,9 @@ enum {
   SSSGS_STAGE_TILE_SORT = 4,  /* a5, instances by tile                         */
   SSSGS_STAGE_RANGES = 5,     /* a6 (+ optional list export)                   */
   SSSGS_STAGE_MLP = 6,        /* a1 + a2                                       */
-  SSSGS_STAGE_RASTER = 7,     /* a7 + a8                                       */
-  SSSGS_NSTAGES = 8
+  SSSGS_STAGE_RASTER = 7,     /* a7 + a8: the per-light-batch walks            */
+  SSSGS_STAGE_PREPASS = 8,    /* light sweeps: visibility pre-pass of a view (fills the weight cache) + compaction */
+  SSSGS_NSTAGES = 9
 };
 int sssgs_profile_enable(sssgs_ctx* ctx, int enable);
 int sssgs_profile_read(sssgs_ctx* ctx, float* stage_ms /* [SSSGS_NSTAGES] */,

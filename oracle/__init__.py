@@ -87,9 +87,25 @@ def mlp_inputs(scene, cam, light_pos) -> np.ndarray:
     return x
 
 
+def round_bf16(x) -> np.ndarray:
+    """The oracle's bf16 rounding (float64 in, float64 out), for the pins."""
+    x = np.ascontiguousarray(x, np.float64)
+    out = np.empty_like(x)
+    lib().orc_round_bf16(ctypes.c_int64(x.size), _p(x), _p(out))
+    return out
+
+
+def round_fp16(x) -> np.ndarray:
+    """The oracle's binary16 rounding (float64 in, float64 out), for the pins."""
+    x = np.ascontiguousarray(x, np.float64)
+    out = np.empty_like(x)
+    lib().orc_round_fp16(ctypes.c_int64(x.size), _p(x), _p(out))
+    return out
+
+
 def mlp_forward(x, mlp, mode: int = 0) -> np.ndarray:
     """Step 2: x [n, in_dim] float64 -> [n, 4] float64.
-    mode 0 = double reference, 1 = bf16-emulating."""
+    mode 0 = double reference, 1 = bf16-emulating, 2 = fp16-emulating."""
     x = np.ascontiguousarray(x, np.float64)
     n = x.shape[0]
     assert x.shape[1] == mlp.in_dim
@@ -166,7 +182,7 @@ def composite(scene, cam, proj, ch, order, ranges, tile=16):
     W, H = int(cam.width), int(cam.height)
     gbuf = np.zeros((H, W, GBUF_CH), np.float64)
     unstable = np.zeros((H, W), np.uint8)
-    counters = np.zeros(4, np.int64)
+    counters = np.zeros(8, np.int64)
     contrib = np.zeros(max(int(scene.n), 1), np.uint8)
     order = np.ascontiguousarray(order, np.uint32)
     rg = np.ascontiguousarray(ranges, np.uint32) if ranges is not None else None
@@ -175,8 +191,11 @@ def composite(scene, cam, proj, ch, order, ranges, tile=16):
                         _p(np.ascontiguousarray(ch, np.float64)), _p(order),
                         ctypes.c_int64(order.shape[0]), _p(rg), _p(gbuf), _p(unstable),
                         _p(counters), _p(contrib))
-    return SimpleNamespace(gbuf=gbuf, unstable=unstable.astype(bool), p_eval=int(counters[0]),
+    # unstable: True where a skip / stop decision sits within fp32 rounding of its threshold (S7); flags: which
+    # rule (bit 0 power ~ 0, bit 1 alpha ~ 1/255, bit 2 T' ~ 1e-4), bits 4-7 = flagged alpha decisions at the pixel
+    return SimpleNamespace(gbuf=gbuf, unstable=unstable != 0, flags=unstable, p_eval=int(counters[0]),
                            p_blend=int(counters[1]), n_unstable=int(counters[2]),
+                           n_rule_power=int(counters[3]), n_rule_alpha=int(counters[4]), n_rule_T=int(counters[5]),
                            contrib=contrib[:int(scene.n)].astype(bool))
 
 

@@ -61,9 +61,37 @@ inline double round_bf16(double v) {
   return (double)f;
 }
 
+// value -> float32 -> IEEE binary16 (round to nearest even, subnormals kept, finite overflow
+// saturates to +-65504 as the kernel's cvt.rn.satfinite does) -> double.  Written from the format's
+// definition: the binary16 numbers of a binade [2^(e-1), 2^e) are spaced q = 2^(e-1-10) apart, q is
+// 2^-24 below the smallest normal 2^-14; x / q is exact (a power-of-two scaling) and nearbyint rounds
+// it to the nearest integer, ties to even (default rounding mode).
+inline double round_fp16(double v) {
+  const float f = (float)v;
+  if (std::isnan(f)) return (double)f;
+  const double a = std::fabs((double)f);
+  if (a > 65504.0) return std::copysign(65504.0, (double)f);  // includes +-inf (satfinite)
+  if (a == 0.0) return (double)f;
+  int e;
+  std::frexp(a, &e);  // a = m 2^e, m in [0.5, 1)
+  const int eq = (e - 1 < -14 ? -14 : e - 1) - 10;
+  const double q = std::ldexp(1.0, eq);
+  const double r = std::nearbyint(a / q) * q;
+  return std::copysign(r > 65504.0 ? 65504.0 : r, (double)f);
+}
+
 }  // namespace
 
 extern "C" {
+
+// The two rounding helpers, exposed so that tests can pin them against independent library
+// conversions (torch bfloat16, numpy float16).
+void orc_round_bf16(int64_t n, const double* in, double* out) {
+  for (int64_t i = 0; i < n; ++i) out[i] = round_bf16(in[i]);
+}
+void orc_round_fp16(int64_t n, const double* in, double* out) {
+  for (int64_t i = 0; i < n; ++i) out[i] = round_fp16(in[i]);
+}
 
 // Camera as passed by the tests (mirrors the fields of sssgs_camera, include/sssgs.h).
 struct OrcCamera {
@@ -154,7 +182,10 @@ void orc_mlp_inputs(int64_t n, const float* means, const float* normals, const f
 // SSS head, incident hidden layers, incident output.
 // mode 0: double reference.  mode 1: bf16-emulating -- every layer INPUT (and the weights,
 // already bf16 in the generator) rounded to bf16 RNE, products and sums in double, bias and
-// activation in double.  out[i] = (L_SSS r,g,b, L_in).
+// activation in double.  mode 2: fp16-emulating -- the same with binary16
+// roundings (round_fp16: RNE, subnormals, finite saturation), the activation precision the
+// kernel uses to meet the 1e-2 bound on the unbounded incident output (SURVEY 8(c) measured
+// note).  out[i] = (L_SSS r,g,b, L_in).
 // -------------------------------------------------------------------------------------
 void orc_mlp_forward(int64_t n, const double* x_in, int in_dim, int n_trunk,
                      const int* trunk_width, int n_inc_hidden, const int* inc_hidden_width,
@@ -195,6 +226,7 @@ void orc_mlp_forward(int64_t n, const double* x_in, int in_dim, int n_trunk,
       for (int k = 0; k < L.i; ++k) {
         double a = h[k], w = L.W[(size_t)o * L.i + k];
         if (mode == 1) { a = round_bf16(a); w = round_bf16(w); }
+        if (mode == 2) { a = round_fp16(a); w = round_fp16(w); }
         s += a * w;
       }
       y[o] = s + (double)L.b[o];
@@ -454,10 +486,14 @@ int64_t orc_build_lists(int64_t n, const int32_t* rect, const float* depth, cons
 // order/ranges: tiled mode  -> order = sorted values list, ranges = per-tile [begin,end);
 //               brute mode  -> ranges == nullptr, order = ALL visible Gaussians sorted by
 //                              (depth bits, index), n_order entries; no tiles involved.
-// unstable[p] = 1 if any skip/stop decision at p sits within the fp32 evaluation error of
+// unstable[p] != 0 if any skip/stop decision at p sits within the fp32 evaluation error of
 // its threshold (S7): such pixels may legitimately differ between correct implementations.
+// The value says which rule flagged the pixel: bit 0 = power within rounding of 0 (skip vs
+// blend at alpha = o), bit 1 = alpha within rounding of 1/255, bit 2 = T' within 1e-3 relative
+// of 1e-4; bits 4-7 = number of alpha-threshold decisions flagged at the pixel (saturating at 15).
 // counters: [0] P_eval (list entries visited, up to and including the stopping entry),
-//           [1] P_blend (blended entries), [2] unstable pixels.
+//           [1] P_blend (blended entries), [2] unstable pixels, [3] / [4] / [5] pixels flagged
+//           by the power / alpha / T rule.
 // contrib[g] = 1 if Gaussian g was blended at >= 1 pixel (may be nullptr).
 // -------------------------------------------------------------------------------------
 void orc_composite(int width, int height, int tile_w, int tile_h, const float* pix,
@@ -465,8 +501,8 @@ void orc_composite(int width, int height, int tile_w, int tile_h, const float* p
                    const uint32_t* order, int64_t n_order, const uint32_t* ranges,
                    double* gbuf, uint8_t* unstable, int64_t* counters, uint8_t* contrib) {
   const int tiles_x = (width + tile_w - 1) / tile_w;
-  int64_t p_eval = 0, p_blend = 0, n_unstable = 0;
-#pragma omp parallel for schedule(dynamic, 4) reduction(+ : p_eval, p_blend, n_unstable)
+  int64_t p_eval = 0, p_blend = 0, n_unstable = 0, n_rule_p = 0, n_rule_a = 0, n_rule_t = 0;
+#pragma omp parallel for schedule(dynamic, 4) reduction(+ : p_eval, p_blend, n_unstable, n_rule_p, n_rule_a, n_rule_t)
   for (int py = 0; py < height; ++py) {
     for (int px = 0; px < width; ++px) {
       int64_t begin = 0, end = n_order;
@@ -477,7 +513,7 @@ void orc_composite(int width, int height, int tile_w, int tile_h, const float* p
       }
       double acc[14] = {0};
       double T = 1.0, A = 0.0;
-      bool shaky = false;
+      unsigned flags = 0, n_alpha_flags = 0;  // which rule flagged the pixel (diagnostic only)
       for (int64_t j = begin; j < end; ++j) {
         const uint32_t g = order[j];
         ++p_eval;
@@ -489,15 +525,15 @@ void orc_composite(int width, int height, int tile_w, int tile_h, const float* p
         const double perr = 1e-5 + 16.0 * 5.96e-8 * mag;
         if (std::fabs(power) < perr && power > -perr) {
           // power within rounding of 0: skip-vs-blend is ambiguous only if alpha matters
-          if ((double)opacities[g] >= kAlphaMin) shaky = true;
+          if ((double)opacities[g] >= kAlphaMin) flags |= 1u;
         }
         if (power > 0.0) continue;
         const double araw = (double)opacities[g] * std::exp(power);
         const double alpha = std::min(kAlphaMax, araw);
-        if (std::fabs(alpha - kAlphaMin) <= perr * kAlphaMin) shaky = true;
+        if (std::fabs(alpha - kAlphaMin) <= perr * kAlphaMin) { flags |= 2u; ++n_alpha_flags; }
         if (alpha < kAlphaMin) continue;
         const double Tn = T * (1.0 - alpha);
-        if (std::fabs(Tn - kTMin) <= 1e-3 * kTMin) shaky = true;
+        if (std::fabs(Tn - kTMin) <= 1e-3 * kTMin) flags |= 4u;
         if (Tn < kTMin) break;
         const double w = T * alpha;
         for (int c = 0; c < 14; ++c) acc[c] += w * ch[14 * (int64_t)g + c];
@@ -510,13 +546,19 @@ void orc_composite(int width, int height, int tile_w, int tile_h, const float* p
       for (int c = 0; c < 14; ++c) o[c] = acc[c];
       o[14] = A;
       o[15] = T;
-      unstable[(int64_t)py * width + px] = shaky ? 1 : 0;
-      n_unstable += shaky ? 1 : 0;
+      unstable[(int64_t)py * width + px] = (uint8_t)(flags | ((n_alpha_flags > 15u ? 15u : n_alpha_flags) << 4));
+      n_unstable += flags ? 1 : 0;
+      n_rule_p += (flags & 1u) ? 1 : 0;
+      n_rule_a += (flags & 2u) ? 1 : 0;
+      n_rule_t += (flags & 4u) ? 1 : 0;
     }
   }
   counters[0] = p_eval;
   counters[1] = p_blend;
   counters[2] = n_unstable;
+  counters[3] = n_rule_p;
+  counters[4] = n_rule_a;
+  counters[5] = n_rule_t;
 }
 
 // -------------------------------------------------------------------------------------

@@ -27,13 +27,14 @@ SSSGS_LIGHTS_PER_CAMERA = 1
 SSSGS_SUM_LIGHTS = 2
 SSSGS_FORWARD_SHADING = 4
 SSSGS_F32, SSSGS_BF16 = 0, 1
+SSSGS_COMPUTE_FP16, SSSGS_COMPUTE_BF16 = 0, 1
 (SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
 CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3, 4
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
            "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility"]
-STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster"]
+STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster", "prepass"]
 
 _f = ctypes.c_float
 _vp = ctypes.c_void_p
@@ -58,7 +59,8 @@ class sssgs_mlp(ctypes.Structure):
                 ("trunk_width", ctypes.c_int * SSSGS_MAX_TRUNK), ("n_inc_hidden", ctypes.c_int),
                 ("inc_hidden_width", ctypes.c_int * SSSGS_MAX_INC_HIDDEN),
                 ("activation", ctypes.c_int), ("leaky_slope", _f), ("dtype", ctypes.c_int),
-                ("params", _vp), ("params_bytes", ctypes.c_size_t), ("precomputed_out", _vp)]
+                ("params", _vp), ("params_bytes", ctypes.c_size_t), ("precomputed_out", _vp),
+                ("compute", ctypes.c_int)]
 
 
 class sssgs_camera(ctypes.Structure):
@@ -197,7 +199,8 @@ def make_light(light) -> sssgs_light:
     return l
 
 
-def make_mlp(spec, params_ptr, params_bytes, dtype=SSSGS_F32, precomputed_ptr=None) -> sssgs_mlp:
+def make_mlp(spec, params_ptr, params_bytes, dtype=SSSGS_F32, precomputed_ptr=None,
+             compute=SSSGS_COMPUTE_FP16) -> sssgs_mlp:
     m = sssgs_mlp()
     m.in_dim = spec.in_dim
     m.n_trunk = len(spec.trunk_width)
@@ -212,6 +215,7 @@ def make_mlp(spec, params_ptr, params_bytes, dtype=SSSGS_F32, precomputed_ptr=No
     m.params = params_ptr
     m.params_bytes = params_bytes
     m.precomputed_out = precomputed_ptr
+    m.compute = compute
     return m
 
 
@@ -233,10 +237,12 @@ class Renderer:
     """Device-resident scene + context.  torch is used for memory and streams only."""
 
     def __init__(self, scene, max_instances: Optional[int] = None, max_lights_per_pass: int = 0,
-                 device: int = 0, max_width: Optional[int] = None, max_height: Optional[int] = None):
+                 device: int = 0, max_width: Optional[int] = None, max_height: Optional[int] = None,
+                 compute: int = SSSGS_COMPUTE_FP16):
         import torch
         self.torch = torch
         self.scene = scene
+        self.compute = compute
         self.device = torch.device("cuda", device)
         self.n = int(scene.n)
         W = max_width or max(c.width for c in scene.cameras)
@@ -310,7 +316,7 @@ class Renderer:
             self._pre = torch.as_tensor(np.ascontiguousarray(precomputed, np.float32)).to(self.device) \
                 if not torch.is_tensor(precomputed) else precomputed
             pre_ptr = self._pre.data_ptr()
-        m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr)
+        m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr, self.compute)
         st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         sssgs_render(self.ctx, self.g, m, carr, n_cam, larr, n_light, o,
                      (SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0) | (SSSGS_SUM_LIGHTS if sum_lights else 0) |

@@ -5,9 +5,31 @@
 
 #include "../../include/sssgs.h"
 
+#include <map>
+#include <mutex>
 #include <utility>
 
 namespace sssgs {
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute of a kernel: the opt-in is
+// remembered per (kernel, device ordinal of the calling thread's current device), so that contexts on
+// several GPUs of one process each get it, and a warmed-up context makes no attribute call any more
+// (CUDA-graph capture of sssgs_render).
+inline cudaError_t ensure_dyn_smem(const void* kernel, int bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<const void*, int>, int> done;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  int& cur = done[std::make_pair(kernel, dev)];
+  if (bytes > cur) {
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) return e;
+    cur = bytes;
+  }
+  return cudaSuccess;
+}
 
 // ---- programmatic dependent launch ------------------------------------------------------------
 // The render path is a chain of short dependent kernels.  Each one is launched with the
@@ -194,6 +216,7 @@ struct MlpPlan {
   int feat_dim;
   int activation;
   float leaky_slope;
+  int f16;          // tensor-core operand type: 1 = binary16 (default), 0 = bf16 (sssgs_mlp.compute)
   int blob_bytes;   // packed weights (all stages), multiple of 1024
   int bias_floats;
   int max_n;        // widest n_pad

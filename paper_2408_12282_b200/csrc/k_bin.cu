@@ -98,21 +98,24 @@ emit_kernel(uint32_t n, const uint32_t* __restrict__ dvals0, const uint32_t* __r
             __nanosleep(20);
             continue;
           }
+          // a chunk total is at most 256 x 65536 = 2^24 and an inclusive prefix at most kValMask: the 32
+          // values of a step sum to less than 2^32; the running prefix SATURATES at kValMask (2^30 - 1,
+          // above any capacity) instead of wrapping, and saturation counts as overflow
           uint32_t val = lane <= stop ? (v & kValMask) : 0u;
 #pragma unroll
           for (int o = 16; o >= 1; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
-          excl += val;
+          excl = (uint32_t)min((uint64_t)excl + val, (uint64_t)kValMask);
           if (inc) break;
           first -= 32;
         }
-        if (lane == 0) st_volatile(status + t, kFlagInc | ((excl + total) & kValMask));
+        if (lane == 0) st_volatile(status + t, kFlagInc | (uint32_t)min((uint64_t)excl + total, (uint64_t)kValMask));
       }
       if (lane == 0) {
         s_base = excl;
         if (t == nchunks - 1) {
-          const uint32_t all = excl + total;
-          counters[DC_INSTANCES] = all;
-          if (all > cap) counters[DC_OVERFLOW] = 1u;
+          const uint32_t all = (uint32_t)min((uint64_t)excl + total, (uint64_t)kValMask);
+          counters[DC_INSTANCES] = all;  // saturated at 2^30 - 1
+          if (all > cap || all == kValMask) counters[DC_OVERFLOW] = 1u;
         }
       }
     }

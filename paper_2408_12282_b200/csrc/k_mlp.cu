@@ -119,14 +119,27 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
   d |= (uint64_t)2 << 61;              // SWIZZLE_128B
   return d;
 }
-// Instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = n.
-__device__ __forceinline__ uint32_t make_idesc(int n) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
+// Instruction descriptor: D = F32, A and B both BF16 (format 1) or both F16 (format 0), both K-major,
+// M = 128, N = n.
+__device__ __forceinline__ uint32_t make_idesc(int n, bool f16) {
+  const uint32_t ab = f16 ? 0u : ((1u << 7) | (1u << 10));
+  return (1u << 4) | ab | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kRows >> 4) << 24);
 }
 
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
   __nv_bfloat162 h = __floats2bfloat162_rn(a, b);  // .x = a (low half), .y = b
   return *reinterpret_cast<uint32_t*>(&h);
+}
+// binary16 pair, round to nearest even, finite overflow saturates to +-65504
+__device__ __forceinline__ uint32_t pack_f16(float a, float b) {
+  uint32_t d;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(b), "f"(a));
+  return d;
+}
+// the 16-bit type of the tensor-core operands: F16 = binary16 (default), else bf16
+template <bool F16>
+__device__ __forceinline__ uint32_t pack2(float a, float b) {
+  return F16 ? pack_f16(a, b) : pack_bf16(a, b);
 }
 // byte offset of 16-byte chunk `c` (8 bf16 = columns 8c..8c+7) of row `r` inside a K-major
 // SWIZZLE_128B operand whose 64-column K blocks are `rows*128` bytes apart
@@ -140,6 +153,7 @@ __device__ __forceinline__ uint32_t swz_off(int r, int c, int kblock_bytes) {
 __global__ void __launch_bounds__(256)
 mlp_pack_kernel(MlpPlan plan, const void* __restrict__ params, int dtype, uint8_t* __restrict__ blob,
                 float* __restrict__ bias) {
+  const bool f16 = plan.f16 != 0;
   pdl_prologue();
   auto load = [&](int off) -> float {
     if (dtype == SSSGS_BF16)
@@ -161,8 +175,9 @@ mlp_pack_kernel(MlpPlan plan, const void* __restrict__ params, int dtype, uint8_
         const int k = c * 8 + e;
         v[e] = (src >= 0 && k < st.src_k) ? load(src + k) : 0.f;
       }
-      uint4 pk = make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
-                            pack_bf16(v[6], v[7]));
+      uint4 pk = f16 ? make_uint4(pack_f16(v[0], v[1]), pack_f16(v[2], v[3]), pack_f16(v[4], v[5]), pack_f16(v[6], v[7]))
+                     : make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
+                                  pack_bf16(v[6], v[7]));
       *reinterpret_cast<uint4*>(blob + st.w_off + swz_off(r, c, st.n_pad * 128)) = pk;
     }
     for (int r = blockIdx.x * 256 + threadIdx.x; r < st.n_pad; r += gridDim.x * 256) {
@@ -208,9 +223,10 @@ __device__ __forceinline__ float act_fn(float v, int activation, float slope) {
 }
 
 
+template <bool F16>
 __device__ __forceinline__ uint4 pack8(const float* v) {
-  return make_uint4(pack_bf16(v[0], v[1]), pack_bf16(v[2], v[3]), pack_bf16(v[4], v[5]),
-                    pack_bf16(v[6], v[7]));
+  return make_uint4(pack2<F16>(v[0], v[1]), pack2<F16>(v[2], v[3]), pack2<F16>(v[4], v[5]),
+                    pack2<F16>(v[6], v[7]));
 }
 
 // Step a1, light-independent part.  Input row layout (S1/S13/S14), in
@@ -218,16 +234,17 @@ __device__ __forceinline__ uint4 pack8(const float* v) {
 //   chunk 0: n(3) rot(2) scale(3) | chunk 1: w_in(3) w_out(3) d v | chunks 2-4: gamma(mu)(24) |
 //   chunks 5..: feat(F), zero padded to in_pad
 // Fills keep[0], keep[2..4] (when this thread owns them: c_begin == 0), mu and w_out.
+template <bool F16>
 __device__ __forceinline__ void assemble_static(const MlpArgs& a, int64_t g, int c_begin, int c_end,
                                                 uint4* keep, float mu[3], float wout[3]) {
   mu[0] = a.means[3 * g]; mu[1] = a.means[3 * g + 1]; mu[2] = a.means[3 * g + 2];
   if (c_begin == 0) {
     const float4 q = reinterpret_cast<const float4*>(a.rotations)[g];
     const float sgn = q.x < 0.f ? -1.f : 1.f;
-    keep[0] = make_uint4(pack_bf16(a.normals[3 * g], a.normals[3 * g + 1]),
-                         pack_bf16(a.normals[3 * g + 2], sgn * q.x),
-                         pack_bf16(sgn * q.y, a.scales[3 * g]),
-                         pack_bf16(a.scales[3 * g + 1], a.scales[3 * g + 2]));
+    keep[0] = make_uint4(pack2<F16>(a.normals[3 * g], a.normals[3 * g + 1]),
+                         pack2<F16>(a.normals[3 * g + 2], sgn * q.x),
+                         pack2<F16>(sgn * q.y, a.scales[3 * g]),
+                         pack2<F16>(a.scales[3 * g + 1], a.scales[3 * g + 2]));
     float wox = a.cam_pos[0] - mu[0], woy = a.cam_pos[1] - mu[1], woz = a.cam_pos[2] - mu[2];
     const float io = 1.f / sqrtf(wox * wox + woy * woy + woz * woz);
     wout[0] = wox * io; wout[1] = woy * io; wout[2] = woz * io;
@@ -246,13 +263,14 @@ __device__ __forceinline__ void assemble_static(const MlpArgs& a, int64_t g, int
         ga[6 * k + ax] = s; ga[6 * k + 3 + ax] = c;
       }
     }
-    keep[2] = pack8(ga);
-    keep[3] = pack8(ga + 8);
-    keep[4] = pack8(ga + 16);
+    keep[2] = pack8<F16>(ga);
+    keep[3] = pack8<F16>(ga + 8);
+    keep[4] = pack8<F16>(ga + 16);
   }
 }
 
 // Light-dependent chunk 1: (w_in, w_out, d, v) for light `lt`.
+template <bool F16>
 __device__ __forceinline__ uint4 assemble_light(const MlpArgs& a, int64_t g, const LightParams& lt,
                                                 const float mu[3], const float wout[3]) {
   float wix = lt.pos[0] - mu[0], wiy = lt.pos[1] - mu[1], wiz = lt.pos[2] - mu[2];
@@ -267,8 +285,8 @@ __device__ __forceinline__ uint4 assemble_light(const MlpArgs& a, int64_t g, con
     v = kY00 * a.vis_sh[g];
   }
   v = fminf(1.f, fmaxf(0.f, v));
-  return make_uint4(pack_bf16(wix, wiy), pack_bf16(wiz, wout[0]), pack_bf16(wout[1], wout[2]),
-                    pack_bf16(d, v));
+  return make_uint4(pack2<F16>(wix, wiy), pack2<F16>(wiz, wout[0]), pack2<F16>(wout[1], wout[2]),
+                    pack2<F16>(d, v));
 }
 
 // ---- TMEM helpers ---------------------------------------------------------------------------------
@@ -357,7 +375,7 @@ __device__ __forceinline__ void a_publish() {
 }
 
 // Writes the 16-byte chunks [c_begin, c_end) of this thread's row of the layer-0 A operand.
-template <bool TS>
+template <bool TS, bool F16>
 __device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, const ARow& ar, int c_begin,
                                           int c_end, const uint4* keep, const uint4& light_chunk) {
 #pragma unroll
@@ -370,8 +388,8 @@ __device__ __forceinline__ void write_row(const MlpArgs& a, int64_t g, const ARo
     float4 f0 = make_float4(0.f, 0.f, 0.f, 0.f), f1 = f0;
     if (j < F) f0 = *reinterpret_cast<const float4*>(a.feat + g * F + j);
     if (j + 4 < F) f1 = *reinterpret_cast<const float4*>(a.feat + g * F + j + 4);
-    a_store<TS>(ar, c, make_uint4(pack_bf16(f0.x, f0.y), pack_bf16(f0.z, f0.w), pack_bf16(f1.x, f1.y),
-                                  pack_bf16(f1.z, f1.w)));
+    a_store<TS>(ar, c, make_uint4(pack2<F16>(f0.x, f0.y), pack2<F16>(f0.z, f0.w), pack2<F16>(f1.x, f1.y),
+                                  pack2<F16>(f1.z, f1.w)));
   }
 }
 
@@ -394,10 +412,12 @@ __device__ __forceinline__ void tmem_wait16(uint32_t* r) {
 #pragma unroll
   for (int i = 0; i < 16; ++i) asm volatile("" : "+r"(r[i]));
 }
-// bf16x2 {lo, hi} = round-to-nearest-even of (max(lo, 0), max(hi, 0)): the ReLU rides on the convert
-__device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
+// 16-bit pair {lo, hi} = round-to-nearest-even of (max(lo, 0), max(hi, 0)): the ReLU rides on the convert
+template <bool F16>
+__device__ __forceinline__ uint32_t pack2_relu(float lo, float hi) {
   uint32_t d;
-  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  if (F16) asm("cvt.rn.relu.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  else asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
 // (x0, x1) += (y0, y1) as one packed fp32x2 add (sm_100 FADD2)
@@ -421,7 +441,7 @@ __device__ __forceinline__ void lds_bias16(uint32_t saddr, float4* b) {
 }
 
 // bias + activation + bf16 of the 16 accumulator columns c0 .. c0 + 15 -> next A operand.
-template <bool RELU, bool TS>
+template <bool RELU, bool TS, bool F16>
 __device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, const ARow& ar, int c0,
                                          int activation, float slope) {
   float v[16];
@@ -436,9 +456,9 @@ __device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, con
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     if (RELU) {
-      w[i] = pack_bf16_relu(v[2 * i], v[2 * i + 1]);
+      w[i] = pack2_relu<F16>(v[2 * i], v[2 * i + 1]);
     } else {
-      w[i] = pack_bf16(act_fn(v[2 * i], activation, slope), act_fn(v[2 * i + 1], activation, slope));
+      w[i] = pack2<F16>(act_fn(v[2 * i], activation, slope), act_fn(v[2 * i + 1], activation, slope));
     }
   }
   a_store<TS>(ar, c0 >> 3, make_uint4(w[0], w[1], w[2], w[3]));
@@ -449,7 +469,7 @@ __device__ __forceinline__ void finish16(const uint32_t* r, const float4* b, con
 // of 16, with the TMEM load of the next group in flight while the current one is finished.
 // WPS = 4: all columns; WPS = 8: the two warps of a row quarter take alternate 32-column blocks.
 // d_taddr: this thread's lane base in the slot's accumulator.
-template <int WPS_, bool RELU, bool TS>
+template <int WPS_, bool RELU, bool TS, bool F16>
 __device__ __forceinline__ void hidden_epilogue(uint32_t d_taddr, const ARow& ar, uint32_t bias_saddr,
                                                 int n_act, int half, int activation, float slope) {
   constexpr int G = WPS_ == 4 ? 8 : 4;  // groups of 16 columns per thread for 128 columns
@@ -465,7 +485,7 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t d_taddr, const ARow& ar
     lds_bias16(bias_saddr + 4u * c0, ba);
     tmem_wait16(ra);
     if (c1 + 16 <= n_act) tmem_ld16_async(d_taddr + c1, rb);
-    finish16<RELU, TS>(ra, ba, ar, c0, activation, slope);
+    finish16<RELU, TS, F16>(ra, ba, ar, c0, activation, slope);
     if (c1 + 16 > n_act) break;
     lds_bias16(bias_saddr + 4u * c1, bb);
     tmem_wait16(rb);
@@ -473,7 +493,7 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t d_taddr, const ARow& ar
       const int c2 = col(2 * gp + 2);
       if (c2 + 16 <= n_act) tmem_ld16_async(d_taddr + c2, ra);
     }
-    finish16<RELU, TS>(rb, bb, ar, c1, activation, slope);
+    finish16<RELU, TS, F16>(rb, bb, ar, c1, activation, slope);
   }
 }
 
@@ -498,7 +518,7 @@ constexpr int kMlpThreadsMax = 512;  // up to 16 warps: 4 slots x 4 warps or 2 s
 // Work distribution: a "unit" is a block of 128 Gaussians with all the lights of the batch; slot s of
 // CTA b owns the units (i * slots + s) * gridDim.x + b, i = 0, 1, ...  Within a unit the lights are
 // walked in order so that the light-independent inputs of a row are assembled once.
-template <int WPS, bool RELU, bool TS>
+template <int WPS, bool RELU, bool TS, bool F16>
 __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_constant__ MlpArgs a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -585,7 +605,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
         }
         TL_STAMP(6);
         const MlpStage& st = plan.st[s_idx];
-        const uint32_t idesc = make_idesc(st.n_pad);
+        const uint32_t idesc = make_idesc(st.n_pad, F16);
         const uint32_t w_addr = smem_u32(sW + st.w_off);
         const uint32_t d_addr = tmem_base + slot * a.slot_cols;
         const uint32_t a_addr = d_addr + a.a_col;                          // TS: A operand in TMEM
@@ -631,11 +651,11 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
       const int64_t g = a.rows ? (int64_t)a.rows[row_c] : row_c;
       uint4 keep[kKeepChunks];
       float mu[3], wout[3];
-      assemble_static(a, g, c_begin, c_end, keep, mu, wout);
+      assemble_static<F16>(a, g, c_begin, c_end, keep, mu, wout);
       for (int light = light0; light < light1; ++light) {
         uint4 lc = make_uint4(0u, 0u, 0u, 0u);
-        if (c_begin == 0) lc = assemble_light(a, g, a.lights.l[light], mu, wout);
-        write_row<TS>(a, g, ar, c_begin, c_end, keep, lc);
+        if (c_begin == 0) lc = assemble_light<F16>(a, g, a.lights.l[light], mu, wout);
+        write_row<TS, F16>(a, g, ar, c_begin, c_end, keep, lc);
         a_publish<TS>();
         mbar_arrive(bar_a);
         issue_stage(0);
@@ -650,7 +670,7 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
           TL_STAMP(3);
           if (st.type == ST_HIDDEN || st.type == ST_HEAD_SPLIT_A) {
             // activated columns [0, n_act) -> bf16 -> next stage's A operand
-            hidden_epilogue<WPS, RELU, TS>(taddr, ar, smem_u32(bias), st.n_act, half, plan.activation, plan.leaky_slope);
+            hidden_epilogue<WPS, RELU, TS, F16>(taddr, ar, smem_u32(bias), st.n_act, half, plan.activation, plan.leaky_slope);
             if (st.type == ST_HEAD_SPLIT_A && half == 0) {  // SSS logits sit right after the activated columns
               float v[16];
               tmem_ld16(taddr + st.n_act, v);
@@ -777,26 +797,29 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
     if (cap > 0 && grid > cap) grid = cap;
   }
   const bool relu = plan.activation == SSSGS_ACT_RELU;
-  auto launch = [&](auto kernel, int* configured_smem) -> int {
-    if (smem > *configured_smem) {
-      if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-        return -1;
-      *configured_smem = smem;
-    }
+  auto launch = [&](auto kernel) -> int {
+    if (ensure_dyn_smem(reinterpret_cast<const void*>(kernel), smem) != cudaSuccess) return -1;
     launch_pdl(kernel, dim3(grid), dim3(a.slots * a.wps * 32), (size_t)smem, s, a);
     return 1;
   };
-  static int cfg_smem[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  const int v = (a.wps == 8 ? 4 : 0) + (relu ? 2 : 0) + (sh.ts ? 1 : 0);
+  const int v = (plan.f16 ? 8 : 0) + (a.wps == 8 ? 4 : 0) + (relu ? 2 : 0) + (sh.ts ? 1 : 0);
   switch (v) {
-    case 0: return launch(mlp_kernel<4, false, false>, &cfg_smem[0]);
-    case 1: return launch(mlp_kernel<4, false, true>, &cfg_smem[1]);
-    case 2: return launch(mlp_kernel<4, true, false>, &cfg_smem[2]);
-    case 3: return launch(mlp_kernel<4, true, true>, &cfg_smem[3]);
-    case 4: return launch(mlp_kernel<8, false, false>, &cfg_smem[4]);
-    case 5: return launch(mlp_kernel<8, false, true>, &cfg_smem[5]);
-    case 6: return launch(mlp_kernel<8, true, false>, &cfg_smem[6]);
-    default: return launch(mlp_kernel<8, true, true>, &cfg_smem[7]);
+    case 0: return launch(mlp_kernel<4, false, false, false>);
+    case 1: return launch(mlp_kernel<4, false, true, false>);
+    case 2: return launch(mlp_kernel<4, true, false, false>);
+    case 3: return launch(mlp_kernel<4, true, true, false>);
+    case 4: return launch(mlp_kernel<8, false, false, false>);
+    case 5: return launch(mlp_kernel<8, false, true, false>);
+    case 6: return launch(mlp_kernel<8, true, false, false>);
+    case 7: return launch(mlp_kernel<8, true, true, false>);
+    case 8: return launch(mlp_kernel<4, false, false, true>);
+    case 9: return launch(mlp_kernel<4, false, true, true>);
+    case 10: return launch(mlp_kernel<4, true, false, true>);
+    case 11: return launch(mlp_kernel<4, true, true, true>);
+    case 12: return launch(mlp_kernel<8, false, false, true>);
+    case 13: return launch(mlp_kernel<8, false, true, true>);
+    case 14: return launch(mlp_kernel<8, true, false, true>);
+    default: return launch(mlp_kernel<8, true, true, true>);
   }
 }
 

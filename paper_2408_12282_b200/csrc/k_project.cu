@@ -149,7 +149,9 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
               ex = sqrtf(2.f * tau * a) * 1.001f + 0.01f;
               ey = sqrtf(2.f * tau * c) * 1.001f + 0.01f;
             }
-            const __half2 ext = __halves2half2(__float2half_ru(fminf(ex, 60000.f)), __float2half_ru(fminf(ey, 60000.f)));
+            // beyond the fp16 range the round-up conversion yields +inf = "never cull" (a clamp would drop a
+            // huge near-plane splat for blocks far from its centre although its tiles are in the lists)
+            const __half2 ext = __halves2half2(__float2half_ru(ex), __float2half_ru(ey));
             ra = make_float4(pix_x, pix_y, z, __uint_as_float(*reinterpret_cast<const uint32_t*>(&ext)));
             // the rasteriser evaluates alpha = o * 2^(A' dx^2 + B' dx dy + C' dy^2): conic pre-scaled
             // by log2(e) (and the -1/2); not part of any key or rect

@@ -771,13 +771,8 @@ static int launch_variant(const CamParams& cam, const LightBatch& lights, int n_
                           int sum_mode = 0, const WeightCache* wc = nullptr, const uint32_t* only_if_set = nullptr) {
   using S = RasterShape<E, WARPS>;
   constexpr int smem = raster_smem(LB, MARK, FWD, WARPS);
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>,
-                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-      return -1;
-    configured = true;
-  }
+  if (ensure_dyn_smem(reinterpret_cast<const void*>(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>), smem) != cudaSuccess)
+    return -1;
   launch_pdl(raster_shade_kernel<LB, E, WARPS, U, MARK, FWD>, dim3(tiles * S::SUBS), dim3(S::THREADS), smem, s, cam,
              lights, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf,
              aov_d, aov_s, frame_stride_px, contrib, sum_mode, wc ? *wc : WeightCache{}, only_if_set);
@@ -792,12 +787,7 @@ static int launch_mixed_e(const CamParams& cam, const LightBatch& lights, int n_
                           float* aov_d, float* aov_s, int64_t frame_stride_px, int tiles, cudaStream_t s, int sum_mode,
                           const uint32_t* only_if_set, int long_log2) {
   constexpr int smem = raster_smem(LB, false, false, 8);
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(raster_mixed_kernel<LB, EL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-      return -1;
-    configured = true;
-  }
+  if (ensure_dyn_smem(reinterpret_cast<const void*>(raster_mixed_kernel<LB, EL>), smem) != cudaSuccess) return -1;
   launch_pdl(raster_mixed_kernel<LB, EL>, dim3(kLongTilesCap * EL + tiles * 2), dim3(256), smem, s, cam, lights, n_lights,
              gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, mlp_out, rgb, gbuf, aov_d, aov_s,
              frame_stride_px, sum_mode, only_if_set, (const uint32_t*)(gb.counters + DC_BUCKET_STARTS), long_log2,
@@ -1113,13 +1103,8 @@ int launch_raster_cached(const CamParams& cam, const LightBatch& lights, int n_l
 #define SSSGS_CACHED(LB, REST)                                                                              \
   do {                                                                                                      \
     constexpr int smem = 8 * 2 * cached_buf_bytes(LB, REST);                                                \
-    static bool configured = false;                                                                         \
-    if (!configured) {                                                                                      \
-      if (cudaFuncSetAttribute(raster_cached_kernel<LB, REST>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                               smem) != cudaSuccess)                                                        \
-        return -1;                                                                                          \
-      configured = true;                                                                                    \
-    }                                                                                                       \
+    if (ensure_dyn_smem(reinterpret_cast<const void*>(raster_cached_kernel<LB, REST>), smem) != cudaSuccess) \
+      return -1;                                                                                            \
     launch_pdl(raster_cached_kernel<LB, REST>, dim3(tiles), dim3(256), smem, s, cam, lights, n_lights,      \
                gb.tile_order, wc, attr, mlp_out, rgb, gbuf, aov_d, aov_s, frame_stride_px, sum_mode);       \
   } while (0)

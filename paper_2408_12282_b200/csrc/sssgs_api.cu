@@ -145,6 +145,20 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
 
 bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
+// Makes the context's device current for the duration of an ABI call and restores the caller's.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    if (prev == dev) prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
 // Builds the tensor-core stage list of the MLP.
 int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
   if (m.in_dim != 40 + feat_dim) return fail(c, SSSGS_EINVAL, "mlp.in_dim %d != 40 + feat_dim %d", m.in_dim, feat_dim);
@@ -152,6 +166,7 @@ int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
   if (m.n_inc_hidden < 0 || m.n_inc_hidden > SSSGS_MAX_INC_HIDDEN) return fail(c, SSSGS_EINVAL, "mlp.n_inc_hidden out of range");
   if (m.activation != SSSGS_ACT_RELU && m.activation != SSSGS_ACT_LEAKY_RELU) return fail(c, SSSGS_EINVAL, "mlp.activation");
   if (m.dtype != SSSGS_F32 && m.dtype != SSSGS_BF16) return fail(c, SSSGS_EINVAL, "mlp.dtype");
+  if (m.compute != SSSGS_COMPUTE_FP16 && m.compute != SSSGS_COMPUTE_BF16) return fail(c, SSSGS_EINVAL, "mlp.compute");
   for (int l = 0; l < m.n_trunk; ++l)
     if (m.trunk_width[l] < 16 || m.trunk_width[l] > 128 || m.trunk_width[l] % 16) return fail(c, SSSGS_EINVAL, "trunk width must be a multiple of 16 in [16,128]");
   for (int l = 0; l < m.n_inc_hidden; ++l)
@@ -162,6 +177,7 @@ int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
   plan->feat_dim = feat_dim;
   plan->activation = m.activation;
   plan->leaky_slope = m.leaky_slope;
+  plan->f16 = m.compute == SSSGS_COMPUTE_FP16 ? 1 : 0;
   int off = 0;       // element offset into params
   int d = m.in_dim;  // current un-padded input width
   int ns = 0, w_off = 0, b_off = 0, max_kb = 0, max_n = 0;
@@ -264,7 +280,8 @@ int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "cudaGetDeviceProperties failed");
   if (prop.major != 10) return fail(nullptr, SSSGS_EARCH, "device is sm_%d%d; libsssgs is built for sm_100a only", prop.major, prop.minor);
-  if (cudaSetDevice(cfg->device) != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "cudaSetDevice failed");
+  DeviceGuard guard(cfg->device);
+  if (!guard.ok) return fail(nullptr, SSSGS_ECUDA, "cudaSetDevice failed");
   sssgs_ctx* c = new (std::nothrow) sssgs_ctx();
   if (!c) return fail(nullptr, SSSGS_ECUDA, "out of host memory");
   c->cfg = *cfg;
@@ -309,6 +326,7 @@ int sssgs_create(const sssgs_config* cfg, sssgs_ctx** out) {
 
 void sssgs_destroy(sssgs_ctx* c) {
   if (!c) return;
+  DeviceGuard guard(c->cfg.device);
   for (auto& s : c->staging)
     if (s.first) cudaFree(s.first);
   for (auto& sp : c->spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
@@ -359,6 +377,8 @@ int sssgs_bake_visibility(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ba
   c->launches = 0;
   if (g->n == 0) return SSSGS_OK;
   if (!g->means || !g->scales || !g->rotations || !g->opacities) return fail(c, SSSGS_EINVAL, "means / scales / rotations / opacities is NULL");
+  DeviceGuard guard(c->cfg.device);
+  if (!guard.ok) return fail(c, SSSGS_ECUDA, "cudaSetDevice(%d) failed", c->cfg.device);
   cudaStream_t s = (cudaStream_t)cuda_stream;
   if (c->upload_pending) {  // a preceding sssgs_render_host may still be uploading on the copy stream
     if (cudaStreamWaitEvent(s, c->ev_upload, 0) != cudaSuccess) return fail(c, SSSGS_ECUDA, "stream wait failed");
@@ -441,7 +461,13 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     if (cm.width > c->cfg.max_width || cm.height > c->cfg.max_height)
       return fail(c, SSSGS_ECAPACITY, "camera %d: %dx%d exceeds the context's %dx%d", v, cm.width, cm.height, c->cfg.max_width, c->cfg.max_height);
     if (!(cm.fx > 0.f) || !(cm.fy > 0.f) || !(cm.znear > 0.f)) return fail(c, SSSGS_EINVAL, "camera %d: fx, fy, znear must be > 0", v);
+    // every output is laid out [F][H][W]...: one image size per call
+    if (cm.width != cams[0].width || cm.height != cams[0].height)
+      return fail(c, SSSGS_EINVAL, "camera %d: %dx%d differs from camera 0 (%dx%d); all cameras of a call must share one image size",
+                  v, cm.width, cm.height, cams[0].width, cams[0].height);
   }
+  DeviceGuard guard(c->cfg.device);
+  if (!guard.ok) return fail(c, SSSGS_ECUDA, "cudaSetDevice(%d) failed", c->cfg.device);
 
   cudaStream_t s = (cudaStream_t)cuda_stream;
   const uint32_t cap = (uint32_t)c->cfg.max_instances;
@@ -563,7 +589,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     if (use_mask) {
       c->wc.chunks = cnt + DC_WC_CHUNKS;
       c->wc.overflow = cnt + DC_WC_OVERFLOW;
-      begin(SSSGS_STAGE_RASTER);
+      begin(SSSGS_STAGE_PREPASS);
       add(launch_mark_contrib(cam, c->gb, sorted_vals, c->contrib, use_cache ? &c->wc : nullptr, s));
       add(launch_compact_contrib(c->contrib, g->n, c->rows, cnt + DC_CONTRIB_ROWS, raster_reads_unblended_rows(tiles),
                                  c->mlp_out[0], c->mlp_out[1], n_light < c->max_lb ? n_light : c->max_lb, s));
@@ -688,7 +714,29 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   if (!g || !mlp || !out) return fail(c, SSSGS_EINVAL, "NULL argument");
   if (g->n < 0 || g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n out of range");
   if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
-  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1 || g->feat_dim < 0) return fail(c, SSSGS_EINVAL, "bad Gaussian description");
+  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(c, SSSGS_EINVAL, "vis_sh_degree must be 0 or 1");
+  if (g->feat_dim < 0 || g->feat_dim > 88 || g->feat_dim % 4) return fail(c, SSSGS_EINVAL, "feat_dim must be a multiple of 4 in [0,88]");
+  // everything is validated BEFORE anything is staged or uploaded: a NULL host array must never be rendered
+  // from uninitialised staging memory
+  if ((n_cam > 0 && !cams) || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
+  if (g->n > 0) {
+    const void* req[] = {g->means, g->scales, g->rotations, g->opacities, g->normals, g->base_color,
+                         g->roughness, g->metallic, g->subsurface, g->vis_sh};
+    for (const void* p : req)
+      if (!p) return fail(c, SSSGS_EINVAL, "a Gaussian attribute pointer is NULL");
+    if (g->feat_dim > 0 && !g->feat) return fail(c, SSSGS_EINVAL, "feat is NULL");
+  }
+  if (!mlp->precomputed_out && g->n > 0 && n_light > 0 && n_cam > 0) {
+    if (!mlp->params) return fail(c, SSSGS_EINVAL, "mlp.params is NULL");
+    MlpPlan plan;  // checks the architecture and params_bytes against it
+    const int rc = build_plan(c, *mlp, g->feat_dim, &plan);
+    if (rc != SSSGS_OK) return rc;
+  }
+  for (int v = 1; v < n_cam; ++v)
+    if (cams[v].width != cams[0].width || cams[v].height != cams[0].height)
+      return fail(c, SSSGS_EINVAL, "sssgs_render_host: all cameras of a call must share one image size");
+  DeviceGuard guard(c->cfg.device);
+  if (!guard.ok) return fail(c, SSSGS_ECUDA, "cudaSetDevice(%d) failed", c->cfg.device);
   cudaStream_t s = 0;
   const size_t n = (size_t)g->n;
   const size_t ncoef = (size_t)(g->vis_sh_degree + 1) * (g->vis_sh_degree + 1);
@@ -732,9 +780,6 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   if (n_cam > 0 && cams) {
     npix = (size_t)cams[0].width * cams[0].height;
     tiles = (size_t)((cams[0].width + kTile - 1) / kTile) * ((cams[0].height + kTile - 1) / kTile);
-    for (int v = 1; v < n_cam; ++v)
-      if (cams[v].width != cams[0].width || cams[v].height != cams[0].height)
-        return fail(c, SSSGS_EINVAL, "sssgs_render_host: all cameras of a call must share one image size");
   }
   const size_t cap = (size_t)c->cfg.max_instances;
   struct Back { void* host; void* dev; size_t bytes; };
@@ -759,10 +804,26 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   std::vector<int64_t> cnt_host((size_t)(n_cam > 0 ? n_cam : 1) * SSSGS_NCOUNTERS, 0);
   dout.counters = (int64_t*)stage_buf(c, idx++, cnt_host.size() * 8);
   if (!dout.counters) ok = false;
-  if (!ok) return fail(c, SSSGS_ECUDA, "device staging allocation or upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+  // error paths after the uploads were enqueued: the copies read caller memory, so they are drained and the
+  // pending-upload mark is cleared before returning
+  auto drain = [&]() {
+    cudaStreamSynchronize(c->copy);
+    cudaStreamSynchronize(s);
+    c->upload_pending = false;
+  };
+  if (!ok) {
+    const cudaError_t e = cudaGetLastError();
+    drain();
+    return fail(c, SSSGS_ECUDA, "device staging allocation or upload failed: %s", cudaGetErrorString(e));
+  }
 
   const int rc = sssgs_render(c, &dg, &dm, cams, n_cam, lights, n_light, &dout, flags, s);
-  if (rc != SSSGS_OK) return rc;
+  if (rc != SSSGS_OK) {
+    const std::string msg = c->err;
+    drain();
+    c->err = msg;
+    return rc;
+  }
   for (const Back& b : back)
     if (b.bytes && cudaMemcpyAsync(b.host, b.dev, b.bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess)
       return fail(c, SSSGS_ECUDA, "download failed");

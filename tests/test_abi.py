@@ -38,6 +38,8 @@ def test_struct_layouts_match_header(libpath):
     assert ctypes.sizeof(binding.sssgs_out) == 9 * 8
     assert ctypes.sizeof(binding.sssgs_gaussians) == 8 + 10 * 8 + 8 + 8 + 8
     assert ctypes.sizeof(binding.sssgs_config) == 64
+    assert ctypes.sizeof(binding.sssgs_mlp) == 4 * (2 + 8 + 1 + 2 + 3) + 3 * 8 + 8   # ints/float, 3 pointers/size_t, compute + pad
+    assert binding.sssgs_mlp.compute.offset == 88 and binding.sssgs_mlp.params.offset == 64
 
 
 def test_workspace_bytes_and_config_validation(libpath):

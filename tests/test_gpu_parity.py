@@ -6,8 +6,8 @@ Bars (BASELINE.json north_star):
   * G-buffer and RGB: 1e-4 absolute on stable pixels (pixels whose skip/stop decisions sit within
     fp32 rounding of a threshold are flagged by the oracle, S7, and compared at 2e-2);
     RGB at ill-conditioned highlights: max(1e-4 max(1,|ref|), 4 |ref32 - ref64|) (S9);
-  * MLP: vs the bf16-emulating oracle >= 99.9 % of outputs within 1e-3 and max <= 2e-2;
-    vs the fp64 reference L_SSS <= 1e-2 (the ReLU incident output is reported).
+  * MLP (default: binary16 layer inputs): all four outputs within 1e-2 of the fp64 reference, and within 3e-3
+    of the fp16-emulating oracle; compute = bf16: max <= 2e-2 vs the bf16-emulating oracle, L_SSS <= 1e-2 vs fp64.
 """
 import numpy as np
 import pytest
@@ -50,15 +50,43 @@ def check_lists(scene, res, ref, view=0):
     np.testing.assert_array_equal(res["tile_ranges"][view].view(np.uint32), ref.ranges)
 
 
-def check_gbuffer(gpu_gbuf, ref, atol=1e-4):
-    d = np.abs(gpu_gbuf.astype(np.float64) - ref.gbuf)
-    stable = ~ref.comp.unstable
+def unstable_bound(ref_gbuf, flags, ch):
+    """What the flagged decisions of a pixel can move a G-buffer value by (S7).
+    ch: [n, 14] per-Gaussian channel values (M_c = max |ch_c|; 1 for the A and T channels).
+      * an alpha ~ 1/255 decision flipped: the entry is blended or not with weight <= 1/255, and every later
+        weight (and the final T) scales by (1 - 1/255): |delta| <= (M_c + |ref|) / 255 per flagged decision;
+      * the T' ~ 1e-4 stop flipped: the stopping entry is blended or not; T' = T (1 - alpha) ~ 1e-4 with
+        alpha <= 0.99 means T <= 1e-2, so its weight T alpha and the final T move by <= 1e-2, the entries
+        behind it carry <= 1e-4 in total: |delta| <= 1.02e-2 M_c;
+      * power ~ 0 (pixel on the centre of a Gaussian whose exponent rounds either side of 0): the entry is
+        skipped or blended with alpha = o: |delta| <= M_c.
+    5 % slack for the fp32 evaluation on top, plus the 1e-4 bar of stable pixels."""
+    M = np.concatenate([np.abs(ch).max(axis=0) if len(ch) else np.zeros(14), [1.0, 1.0]])
+    n_alpha = (flags >> 4).astype(np.float64)[..., None]
+    t_rule = ((flags & 4) != 0).astype(np.float64)[..., None]
+    p_rule = ((flags & 1) != 0).astype(np.float64)[..., None]
+    return 1e-4 + 1.05 * (n_alpha / 255.0 * (M + np.abs(ref_gbuf)) + t_rule * 1.02e-2 * M + p_rule * M)
+
+
+def check_gbuffer(gpu_gbuf, ref, atol=1e-4, mask=None, comp=None, ch=None, label=""):
+    """G-buffer vs the oracle: 1e-4 on stable pixels, the derived bound of the flagged decisions on the others.
+    mask restricts the comparison to sampled pixels; comp / ch default to ref.comp / ref.ch."""
+    comp = comp if comp is not None else ref.comp
+    ch = ch if ch is not None else ref.ch
+    d = np.abs(gpu_gbuf.astype(np.float64) - comp.gbuf)
+    stable = ~comp.unstable if mask is None else (mask & ~comp.unstable)
+    unst = comp.unstable if mask is None else (mask & comp.unstable)
     worst = d[stable].max() if stable.any() else 0.0
-    assert worst <= atol, f"stable-pixel G-buffer error {worst:.3e} > {atol}"
-    if (~stable).any():
-        bound = 2e-2 * np.maximum(1.0, np.abs(ref.gbuf[~stable]))
-        assert (d[~stable] <= bound).all(), f"unstable-pixel error {d[~stable].max():.3e}"
-    return worst, int((~stable).sum())
+    assert worst <= atol, f"{label} stable-pixel G-buffer error {worst:.3e} > {atol}"
+    if unst.any():
+        bound = unstable_bound(comp.gbuf, comp.flags, ch)
+        bad = unst[..., None] & (d > bound)
+        assert not bad.any(), f"{label} unstable-pixel error beyond the flagged decisions' reach: {d[bad].max():.3e}"
+    f = comp.flags[unst] if unst.any() else np.zeros(0, np.uint8)
+    print(f"{label} G-buffer: stable worst {worst:.2e}; unstable pixels {int(unst.sum())} "
+          f"(power ~ 0: {int(((f & 1) != 0).sum())}, alpha ~ 1/255: {int(((f & 2) != 0).sum())}, "
+          f"T' ~ 1e-4: {int(((f & 4) != 0).sum())})")
+    return worst, int(unst.sum())
 
 
 def check_shading(scene, gpu, frame, view, light):
@@ -140,12 +168,19 @@ def test_gbuffer_and_shading_with_reference_mlp(name, scene):
         np.testing.assert_array_equal(gpu["mlp_out"][f], pre[f])
 
 
+# MLP bars.  Default compute = binary16 layer inputs: every output within 1e-2 of the float64
+# reference (BASELINE north_star) and within 3e-3 of the fp16-emulating oracle (same rounding points, double instead
+# of fp32 accumulation: a rare rounding flip of a hidden activation moves an output by <= 2^-11 x |activation| x
+# |weight path| ~ 1e-3).  compute = bf16: the kernel-correctness bar against the bf16-emulating oracle (2e-2, flips
+# are 8x larger) and the L_SSS bar against float64; the unbounded ReLU output L_in exceeds 1e-2 there -- which is why
+# bf16 is not the default -- and is reported.
+@pytest.mark.parametrize("compute", ["fp16", "bf16"])
 @pytest.mark.parametrize("name,scene", list(_small_scenes()))
-def test_mlp_outputs(name, scene):
+def test_mlp_outputs(name, scene, compute):
     nv, nl = len(scene.cameras), len(scene.lights[0])
     import torch
     from paper_2408_12282_b200 import binding
-    R = binding.Renderer(scene)
+    R = binding.Renderer(scene, compute=binding.SSSGS_COMPUTE_FP16 if compute == "fp16" else binding.SSSGS_COMPUTE_BF16)
     try:
         out = R.render(cams=scene.cameras, lights=[scene.lights[v] for v in range(nv)],
                        want=("mlp_out", "rgb"), lights_per_camera=True)
@@ -156,24 +191,28 @@ def test_mlp_outputs(name, scene):
     for v in range(nv):
         for l in range(nl):
             x = oracle.mlp_inputs(scene, scene.cameras[v], scene.lights[v][l].position)
-            y_bf = oracle.mlp_forward(x, scene.mlp, 1)
+            y_em = oracle.mlp_forward(x, scene.mlp, 2 if compute == "fp16" else 1)
             y_ref = oracle.mlp_forward(x, scene.mlp, 0)
-            e_bf = np.abs(got[v * nl + l] - y_bf)
+            e_em = np.abs(got[v * nl + l] - y_em)
             e_ref = np.abs(got[v * nl + l] - y_ref)
-            frac = (e_bf <= 1e-3).mean()
-            print(f"{name} v{v} l{l}: vs bf16 oracle max {e_bf.max():.3e} frac<=1e-3 {frac:.5f}; "
+            frac = (e_em <= 1e-3).mean()
+            print(f"{name} {compute} v{v} l{l}: vs emulating oracle max {e_em.max():.3e} frac<=1e-3 {frac:.5f}; "
                   f"vs fp64 L_SSS max {e_ref[:, :3].max():.3e} L_in max {e_ref[:, 3].max():.3e} "
                   f"L_in frac>1e-2 {(e_ref[:, 3] > 1e-2).mean():.5f}")
-            assert frac >= 0.999, f"only {frac:.5f} of MLP outputs within 1e-3 of the bf16 oracle"
-            assert e_bf.max() <= 2e-2
-            assert e_ref[:, :3].max() <= 1e-2
+            assert frac >= 0.999, f"only {frac:.5f} of MLP outputs within 1e-3 of the emulating oracle"
+            if compute == "fp16":
+                assert e_em.max() <= 3e-3
+                assert e_ref.max() <= 1e-2, f"MLP vs float64: {e_ref.max():.3e} > 1e-2 (north_star)"
+            else:
+                assert e_em.max() <= 2e-2
+                assert e_ref[:, :3].max() <= 1e-2
 
 
 def test_end_to_end_rgb_cfg1():
-    # whole path on the GPU (its own bf16 MLP) vs the oracle with the bf16-emulating MLP
+    # whole path on the GPU (its own MLP, binary16 layer inputs) vs the oracle with the fp16-emulating MLP
     scene = scenes.make_scene(1)
     gpu = gpu_render(scene)
-    r = oracle.render_frame(scene, mlp_mode=1)
+    r = oracle.render_frame(scene, mlp_mode=2)
     check_lists(scene, gpu, r)
     st = ~r.comp.unstable
     err = np.abs(gpu["rgb"][0] - r.rgb)
@@ -410,11 +449,12 @@ def test_full_size_cfg2_matches_oracle():
     # BASELINE configs[1] at full size, in the launch configuration bench.py times
     scene = scenes.make_scene(2)
     gpu = gpu_render(scene)
-    r = oracle.render_frame(scene, mlp_mode=1)
+    r = oracle.render_frame(scene, mlp_mode=2)
     check_lists(scene, gpu, r)
-    y_bf = r.mlp_out
-    e = np.abs(gpu["mlp_out"][0] - y_bf)
-    assert (e <= 1e-3).mean() >= 0.999 and e.max() <= 2e-2
+    e = np.abs(gpu["mlp_out"][0] - r.mlp_out)
+    assert (e <= 1e-3).mean() >= 0.999 and e.max() <= 3e-3
+    y_ref = oracle.mlp_forward(r.x, scene.mlp, 0)
+    assert np.abs(gpu["mlp_out"][0] - y_ref).max() <= 1e-2   # north_star's bar, all four outputs
     # light-independent channels do not depend on the MLP: 1e-4 on stable pixels
     st = ~r.comp.unstable
     assert np.abs(gpu["gbuffer"][0][..., :10] - r.gbuf[..., :10])[st].max() <= 1e-4
