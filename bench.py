@@ -140,7 +140,7 @@ def config_dict(cfg, scene, fps):
 # ---------------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample(scene, mlp_rows_budget=200_000):
+def oracle_sample(scene, mlp_rows_budget=1_000_000):
     """One whole-path render of the first (view, light) frame by the CPU oracle, as it stands.  A BOUNDED sample:
     projection, lists, compositing and shading run in full; the MLP (plain loops, ~60 us per row and core) runs
     on a seeded sample of at most `mlp_rows_budget` rows and its time is extrapolated linearly to all rows (a

@@ -219,16 +219,19 @@ void orc_mlp_forward(int64_t n, const double* x_in, int in_dim, int n_trunk,
     if (activation == ACT_LEAKY_RELU) return v > 0 ? v : leaky_slope * v;
     return v > 0 ? v : 0.0;
   };
+  // the rounding of the emulating modes: applied to every weight and to every layer input
+  auto rnd = [&](double v) { return mode == 1 ? round_bf16(v) : (mode == 2 ? round_fp16(v) : v); };
+  // weights as the tensor cores see them: rounded once (the same value whichever row uses it)
+  std::vector<double> Wr((size_t)((p + di + 1) - params));
+  for (size_t q = 0; q < Wr.size(); ++q) Wr[q] = rnd((double)params[q]);
   auto linear = [&](const Layer& L, const std::vector<double>& h, std::vector<double>& y) {
+    std::vector<double> hr(L.i);
+    for (int k = 0; k < L.i; ++k) hr[k] = rnd(h[k]);   // the layer input, rounded
+    const double* W = Wr.data() + (L.W - params);
     y.assign(L.o, 0.0);
     for (int o = 0; o < L.o; ++o) {
       double s = 0;
-      for (int k = 0; k < L.i; ++k) {
-        double a = h[k], w = L.W[(size_t)o * L.i + k];
-        if (mode == 1) { a = round_bf16(a); w = round_bf16(w); }
-        if (mode == 2) { a = round_fp16(a); w = round_fp16(w); }
-        s += a * w;
-      }
+      for (int k = 0; k < L.i; ++k) s += hr[k] * W[(size_t)o * L.i + k];
       y[o] = s + (double)L.b[o];
     }
   };
