@@ -292,6 +292,7 @@ class ConfigRun:
             self.graph.replay()
             b.record(stream)
         barrier()
+        torch.cuda.synchronize()
         t_wall = time.perf_counter() - t_wall
         return [a.elapsed_time(b) for a, b in ev], t_wall
 

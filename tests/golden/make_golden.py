@@ -27,7 +27,7 @@ PIXELS = [(20, 24), (13, 30), (27, 17), (5, 5), (33, 41), (20, 8)]  # (row, col)
 
 def compute():
     scene = scenes.make_scene(SCENE["cfg"], n=SCENE["n"], width=SCENE["width"], height=SCENE["height"])
-    r = oracle.render_frame(scene, mlp_mode=1)  # bf16-emulating MLP: what the tensor-core path computes
+    r = oracle.render_frame(scene, mlp_mode=2)  # fp16-emulating MLP: what the tensor-core path computes by default
     out = {
         "scene": SCENE,
         "n_vis": r.n_vis,
