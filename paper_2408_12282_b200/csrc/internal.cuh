@@ -204,7 +204,6 @@ struct MlpStage {
   int n_act;        // outputs that go through the hidden activation and feed the next stage
   int type;
   int w_off;        // byte offset of this stage's packed bf16 weights in the blob
-  int b_off;        // float offset of this stage's bias vector (n_pad floats) in the bias block
   // where the rows come from in the caller's packed parameter array (element offsets):
   // rows [0, src_rows[0]) from source 0, rows [src_rows[0], src_rows[0]+src_rows[1]) from source 1
   int src_w[2], src_b[2], src_rows[2];
@@ -217,8 +216,8 @@ struct MlpPlan {
   int activation;
   float leaky_slope;
   int f16;          // tensor-core operand type: 1 = binary16 (default), 0 = bf16 (sssgs_mlp.compute)
-  int blob_bytes;   // packed weights (all stages), multiple of 1024
-  int bias_floats;
+  int blob_bytes;   // packed weights (all stages) + bias blocks, multiple of 1024
+  int bias_off;     // byte offset of the bias blocks in the blob: block q = stages 4q .. 4q + 3, max_n x 128 bytes each
   int max_n;        // widest n_pad
   int max_k_bytes;  // bytes of the largest A tile (128 rows)
   MlpStage st[kMlpMaxStages];
@@ -245,10 +244,9 @@ int launch_ranges(const uint32_t* sorted_tiles, const CamParams& cam, const Geom
 int launch_export_lists(const uint32_t* sorted_tiles, const uint32_t* sorted_vals,
                         const GeomBuffers& gb, uint32_t cap, uint64_t* keys_out, uint32_t* vals_out,
                         cudaStream_t s);
-int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, float* bias,
-                    cudaStream_t s);
+int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, cudaStream_t s);
 int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blob,
-               const float* bias, const CamParams& cam, const LightBatch& lights, int n_lights,
+               const CamParams& cam, const LightBatch& lights, int n_lights,
                float4* out_internal, float* out_user, int64_t user_light_stride, int max_ctas,
                const uint32_t* rows, const uint32_t* row_count, int64_t* rows_out, cudaStream_t s);
 // "w/o deferred" variant (Tab. 2): Eq. 7 per Gaussian, then RGB compositing

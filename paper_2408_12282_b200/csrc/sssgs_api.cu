@@ -41,7 +41,6 @@ struct sssgs_ctx {
   uint8_t* contrib = nullptr;   // [n] visibility pre-pass flags (inside the control block)
   uint32_t* rows = nullptr;     // [n] Gaussians kept by the pre-pass
   uint8_t* mlp_blob = nullptr;
-  float* mlp_bias = nullptr;
   int64_t launches = 0;
   // optional per-stage timing
   bool profile = false;
@@ -59,7 +58,6 @@ namespace {
 std::string g_create_err;
 
 constexpr size_t kMaxBlobBytes = 512 * 1024;
-constexpr size_t kMaxBiasFloats = 4096;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -128,7 +126,6 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
     if (c) c->wc.capacity = (uint32_t)chunks;
   }
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
-  p = take(kMaxBiasFloats * 4); if (c) c->mlp_bias = (float*)p;
   // control block: everything that must be zero at the start of a camera
   const size_t ctrl_begin = off;
   if (c) c->control = base ? base + off : nullptr;
@@ -180,7 +177,7 @@ int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
   plan->f16 = m.compute == SSSGS_COMPUTE_FP16 ? 1 : 0;
   int off = 0;       // element offset into params
   int d = m.in_dim;  // current un-padded input width
-  int ns = 0, w_off = 0, b_off = 0, max_kb = 0, max_n = 0;
+  int ns = 0, w_off = 0, max_kb = 0, max_n = 0;
   auto add = [&](int type, int k, int n_pad, int n_act) -> MlpStage& {
     MlpStage& st = plan->st[ns++];
     st.type = type;
@@ -189,10 +186,8 @@ int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
     st.n_act = n_act;
     st.src_k = k;
     st.w_off = w_off;
-    st.b_off = b_off;
     const int kblocks = (st.k_pad + 63) / 64;
     w_off += kblocks * n_pad * 128;
-    b_off += n_pad;
     if (kblocks > max_kb) max_kb = kblocks;
     if (n_pad > max_n) max_n = n_pad;
     st.src_w[0] = st.src_w[1] = st.src_b[0] = st.src_b[1] = 0;
@@ -233,14 +228,15 @@ int build_plan(sssgs_ctx* c, const sssgs_mlp& m, int feat_dim, MlpPlan* plan) {
     off += di + 1;
   }
   plan->n_stages = ns;
-  plan->blob_bytes = (int)align_up((size_t)w_off, 1024);
-  plan->bias_floats = b_off;
+  // the biases follow the weights as UMMA operands too (k_mlp.cu: they are added by the tensor core)
+  plan->bias_off = (int)align_up((size_t)w_off, 1024);
+  plan->blob_bytes = (int)align_up((size_t)plan->bias_off + (size_t)((ns + 3) / 4) * max_n * 128, 1024);
   plan->max_n = max_n;
   plan->max_k_bytes = max_kb * 128 * 128;
   const size_t elem = m.dtype == SSSGS_BF16 ? 2 : 4;
   if (m.params_bytes != (size_t)off * elem)
     return fail(c, SSSGS_EINVAL, "mlp.params_bytes %zu != expected %zu", m.params_bytes, (size_t)off * elem);
-  if ((size_t)plan->blob_bytes > kMaxBlobBytes || (size_t)b_off > kMaxBiasFloats || max_n > 256)
+  if ((size_t)plan->blob_bytes > kMaxBlobBytes || max_n > 256)
     return fail(c, SSSGS_ECAPACITY, "MLP too large for the context");
   if (mlp_smem_bytes(*plan) > 227 * 1024)
     return fail(c, SSSGS_ECAPACITY, "MLP weights (%d B) + activations do not fit in shared memory", plan->blob_bytes);
@@ -527,7 +523,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   }
   begin(SSSGS_STAGE_PACK);
   if (add(launch_pack_attr(*g, c->attr, sm)) < 0) return fail(c, SSSGS_ECUDA, "launch failed");
-  if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, c->mlp_bias, sm));
+  if (run_mlp && g->n > 0 && n_light > 0) add(launch_mlp_pack(*mlp, plan, c->mlp_blob, sm));
   end();
   int64_t batch_no = 0;
 
@@ -631,7 +627,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
           if (20.0 + 3.0 * mlp_all_us <= 1.4 * chain_us) mlp_ctas = (c->num_sms + 2) / 3;
           else if (20.0 + 2.0 * mlp_all_us <= chain_us) mlp_ctas = c->num_sms / 2;
         }
-        const int k = launch_mlp(*g, plan, c->mlp_blob, c->mlp_bias, cam, lb, nl, mlp_buf,
+        const int k = launch_mlp(*g, plan, c->mlp_blob, cam, lb, nl, mlp_buf,
                                  out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
                                  mlp_ctas, use_mask ? c->rows : nullptr, use_mask ? cnt + DC_CONTRIB_ROWS : nullptr,
                                  out->counters ? out->counters + (size_t)v * SSSGS_NCOUNTERS + SSSGS_CNT_MLP_ROWS : nullptr, sm);
