@@ -66,6 +66,16 @@ enum {
                                   background term (1 - A) bg once.  The sum is formed in the
                                   rasteriser's epilogue (no per-light frames are written).
                                   gbuffer / mlp_out stay per light; the AOVs must be NULL.    */
+  SSSGS_TIGHT_LISTS = 8u,      /* tight tile lists (reading S5; "efficiently designed
+                                  splatting technique"): a (tile, Gaussian) pair of the canonical list is
+                                  kept only if the Gaussian's alpha >= 1/255 support box reaches a pixel of
+                                  the tile.  The list is a sub-sequence of the canonical one (same order),
+                                  contains every pair with alpha >= 1/255 at some pixel of the tile, and
+                                  blends the same (pixel, entry) pairs: frames are bit-identical to the
+                                  canonical list's on images of more than 1600 tiles, and equal up to the
+                                  order of the per-slot partial sums (last bits) on smaller ones; sorted_keys /
+                                  sorted_vals / tile_ranges / SSSGS_CNT_INSTANCES then describe the tight
+                                  list.  ~0.6-0.75 x the instances: less to emit, sort and walk.        */
   SSSGS_FORWARD_SHADING = 4u   /* the "w/o deferred" variant of the paper's ablation (PAPER.md L283
                                   Tab. 2, Fig. 5): Eq. 7 is evaluated per Gaussian (at its
                                   centre, with its own normal and material) and the RGB values are

@@ -199,6 +199,17 @@ def composite(scene, cam, proj, ch, order, ranges, tile=16):
                            contrib=contrib[:int(scene.n)].astype(bool))
 
 
+def tile_hits(scene, cam, proj, vals, ranges, tile=16) -> np.ndarray:
+    """S5: for every entry of the canonical sorted list, True iff its Gaussian reaches alpha >= 1/255 at some
+    pixel of the entry's tile -- the pairs every valid tight tile list must keep."""
+    hit = np.zeros(max(len(vals), 1), np.uint8)
+    lib().orc_tile_hits(ctypes.c_int(int(cam.width)), ctypes.c_int(int(cam.height)), ctypes.c_int(tile),
+                        ctypes.c_int(tile), _p(proj.pix), _p(proj.conic), _p(_f32(scene.opacities)),
+                        _p(np.ascontiguousarray(vals, np.uint32)), _p(np.ascontiguousarray(ranges, np.uint32)),
+                        ctypes.c_int(proj.tiles_x), ctypes.c_int(proj.tiles_y), _p(hit))
+    return hit[:len(vals)].astype(bool)
+
+
 def brute_order(proj) -> np.ndarray:
     """All visible Gaussians sorted by (depth bits, index) -- the order of step 7."""
     vis = np.nonzero(proj.visible)[0]

@@ -565,6 +565,41 @@ void orc_composite(int width, int height, int tile_w, int tile_h, const float* p
 }
 
 // -------------------------------------------------------------------------------------
+// Tight tile lists ("efficiently designed splatting technique").  The
+// canonical list holds every (tile, Gaussian) pair of the Gaussian's tile rectangle; a valid tight
+// list is a sub-sequence of it that still contains every pair with alpha >= 1/255 at SOME pixel of
+// the tile (only those can ever be blended, whatever the transmittance).  This function computes that
+// minimal set from the definition: for entry j of the sorted list, lying in tile t, hit[j] = 1 iff
+//   exists pixel p of tile t (inside the image):  power(p) <= 0  and  min(0.99, o exp(power(p))) >= 1/255,
+// with power as in orc_composite.  Brute force over the pixels of the tile.
+// -------------------------------------------------------------------------------------
+void orc_tile_hits(int width, int height, int tile_w, int tile_h, const float* pix, const float* conic,
+                   const float* opacities, const uint32_t* order, const uint32_t* ranges, int tiles_x,
+                   int tiles_y, uint8_t* hit) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int t = 0; t < tiles_x * tiles_y; ++t) {
+    const int px0 = (t % tiles_x) * tile_w, py0 = (t / tiles_x) * tile_h;
+    const int px1 = std::min(px0 + tile_w, width), py1 = std::min(py0 + tile_h, height);
+    for (uint32_t j = ranges[2 * t]; j < ranges[2 * t + 1]; ++j) {
+      const uint32_t g = order[j];
+      const double ca = conic[3 * g], cb = conic[3 * g + 1], cc = conic[3 * g + 2];
+      uint8_t h = 0;
+      for (int py = py0; py < py1 && !h; ++py)
+        for (int px = px0; px < px1; ++px) {
+          const double dx = (double)px - (double)pix[2 * g], dy = (double)py - (double)pix[2 * g + 1];
+          const double power = -0.5 * (ca * dx * dx + cc * dy * dy) - cb * dx * dy;
+          if (power > 0.0) continue;
+          if (std::min(kAlphaMax, (double)opacities[g] * std::exp(power)) >= kAlphaMin) {
+            h = 1;
+            break;
+          }
+        }
+      hit[j] = h;
+    }
+  }
+}
+
+// -------------------------------------------------------------------------------------
 // Step 6 -- per-pixel deferred shading.  PAPER.md L114: "evaluate the BRDF model in image
 // space after the rasterization ... The image space surface position is projected back to
 // the 3D space"; L76-80 Eq. 4 (Disney/Cook-Torrance: f_diffuse = (1-m)/pi b,

@@ -26,6 +26,7 @@ SSSGS_MAX_INC_HIDDEN = 2
 SSSGS_LIGHTS_PER_CAMERA = 1
 SSSGS_SUM_LIGHTS = 2
 SSSGS_FORWARD_SHADING = 4
+SSSGS_TIGHT_LISTS = 8
 SSSGS_F32, SSSGS_BF16 = 0, 1
 SSSGS_COMPUTE_FP16, SSSGS_COMPUTE_BF16 = 0, 1
 (SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
@@ -290,7 +291,7 @@ class Renderer:
         return {k: torch.zeros(shapes[k][0], dtype=shapes[k][1], device=self.device) for k in want}
 
     def render(self, cams=None, lights=None, want=("rgb",), outputs=None, precomputed=None,
-               lights_per_camera=False, stream=None, sum_lights=False, forward=False):
+               lights_per_camera=False, stream=None, sum_lights=False, forward=False, tight=False):
         """Enqueue one sssgs_render on the current torch stream.  cams: list of scene cameras;
         lights: list of lights (or list per camera with lights_per_camera).  Returns the dict of
         output tensors (device)."""
@@ -320,7 +321,7 @@ class Renderer:
         st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
         sssgs_render(self.ctx, self.g, m, carr, n_cam, larr, n_light, o,
                      (SSSGS_LIGHTS_PER_CAMERA if lights_per_camera else 0) | (SSSGS_SUM_LIGHTS if sum_lights else 0) |
-                     (SSSGS_FORWARD_SHADING if forward else 0), st)
+                     (SSSGS_FORWARD_SHADING if forward else 0) | (SSSGS_TIGHT_LISTS if tight else 0), st)
         return outputs
 
     def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None,

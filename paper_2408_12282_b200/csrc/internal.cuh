@@ -225,7 +225,7 @@ struct MlpPlan {
 
 // ---- launchers (each enqueues on `s`, returns the number of kernels launched) ---------------
 int launch_pack_attr(const sssgs_gaussians& g, float4* attr, cudaStream_t s);
-int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb,
+int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb, int tight,
                    cudaStream_t s);
 int launch_sort_pass(const uint32_t* keys_in, const uint32_t* vals_in, uint32_t* keys_out,
                      uint32_t* vals_out, const uint32_t* count_ptr, uint32_t count_cap, int shift,

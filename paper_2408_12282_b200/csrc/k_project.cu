@@ -38,7 +38,7 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
                CamParams cam, float4* __restrict__ rec_a, float4* __restrict__ rec_b,
                uint2* __restrict__ rect_out, uint32_t* __restrict__ touched_out,
                uint32_t* __restrict__ dkeys, uint32_t* __restrict__ hist,
-               uint32_t* __restrict__ counters) {
+               uint32_t* __restrict__ counters, int tight) {
   __shared__ uint32_t s_hist[4 * 256];
   pdl_prologue();
   for (int i = threadIdx.x; i < 4 * 256; i += kProjThreads) s_hist[i] = 0;
@@ -153,11 +153,33 @@ project_kernel(int64_t n, const float* __restrict__ means, const float* __restri
             // huge near-plane splat for blocks far from its centre although its tiles are in the lists)
             const __half2 ext = __halves2half2(__float2half_ru(ex), __float2half_ru(ey));
             ra = make_float4(pix_x, pix_y, z, __uint_as_float(*reinterpret_cast<const uint32_t*>(&ext)));
+            int tx0 = x0, tx1 = x1, ty0 = y0, ty1 = y1;
+            if (tight) {
+              // SSSGS_TIGHT_LISTS: keep only the tiles of the canonical rect that hold a pixel
+              // inside the support box [pix - e, pix + e] -- the box the rasteriser culls its 8x4-pixel blocks
+              // with (same fp16 half-extents), widened by 0.02 px so that a block test can never pass in a
+              // tile dropped here: every tile dropped would have been culled in all of its blocks, hence the
+              // image is bit-identical.  Tile t holds the pixel centres 16 t .. 16 t + 15.
+              if (o < kAlphaMin) {                     // alpha <= o < 1/255 everywhere: never blended
+                tx1 = tx0; ty1 = ty0;
+              } else {
+                const float2 e = __half22float2(ext);  // +inf beyond the fp16 range: the canonical rect stays
+                const float lo_x = ceilf((pix_x - e.x - 0.02f - (float)(kTile - 1)) / tl), hi_x = floorf((pix_x + e.x + 0.02f) / tl);
+                const float lo_y = ceilf((pix_y - e.y - 0.02f - (float)(kTile - 1)) / tl), hi_y = floorf((pix_y + e.y + 0.02f) / tl);
+                tx0 = max(x0, (int)fmaxf(lo_x, 0.f));
+                ty0 = max(y0, (int)fmaxf(lo_y, 0.f));
+                tx1 = min(x1, (int)fminf(hi_x, 65535.f) + 1);
+                ty1 = min(y1, (int)fminf(hi_y, 65535.f) + 1);
+                if (tx1 < tx0) tx1 = tx0;
+                if (ty1 < ty0) ty1 = ty0;
+              }
+              cnt = (uint32_t)((tx1 - tx0) * (ty1 - ty0));
+            }
             // the rasteriser evaluates alpha = o * 2^(A' dx^2 + B' dx dy + C' dy^2): conic pre-scaled
             // by log2(e) (and the -1/2); not part of any key or rect
             constexpr float kLog2e = 1.4426950408889634f;
             rb = make_float4(-0.5f * kLog2e * con_a, -kLog2e * con_b, -0.5f * kLog2e * con_c, o);
-            rc = make_uint2((uint32_t)x0 | ((uint32_t)x1 << 16), (uint32_t)y0 | ((uint32_t)y1 << 16));
+            rc = make_uint2((uint32_t)tx0 | ((uint32_t)tx1 << 16), (uint32_t)ty0 | ((uint32_t)ty1 << 16));
           }
         }
       }
@@ -227,13 +249,13 @@ int launch_pack_attr(const sssgs_gaussians& g, float4* attr, cudaStream_t s) {
   return 1;
 }
 
-int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb,
+int launch_project(const sssgs_gaussians& g, const CamParams& cam, const GeomBuffers& gb, int tight,
                    cudaStream_t s) {
   if (g.n == 0) return 0;
   unsigned blocks = (unsigned)((g.n + kProjThreads - 1) / kProjThreads);
   if (blocks > 148 * 8) blocks = 148 * 8;
   launch_pdl(project_kernel, dim3(blocks), dim3(kProjThreads), 0, s, g.n, g.means, g.scales, g.rotations,
-             g.opacities, cam, gb.rec_a, gb.rec_b, gb.rect, gb.touched, gb.dkeys[0], gb.hist, gb.counters);
+             g.opacities, cam, gb.rec_a, gb.rec_b, gb.rect, gb.touched, gb.dkeys[0], gb.hist, gb.counters, tight);
   return 1;
 }
 

@@ -419,7 +419,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   if (!c) return SSSGS_EINVAL;
   if (!g || !mlp || !out || (n_cam > 0 && !cams) || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
   if (n_cam < 0 || n_light < 0) return fail(c, SSSGS_EINVAL, "negative count");
-  if (flags & ~(uint32_t)(SSSGS_LIGHTS_PER_CAMERA | SSSGS_SUM_LIGHTS | SSSGS_FORWARD_SHADING))
+  if (flags & ~(uint32_t)(SSSGS_LIGHTS_PER_CAMERA | SSSGS_SUM_LIGHTS | SSSGS_FORWARD_SHADING | SSSGS_TIGHT_LISTS))
     return fail(c, SSSGS_EINVAL, "unknown flags");
   const bool forward = (flags & SSSGS_FORWARD_SHADING) != 0;
   if (forward && ((flags & SSSGS_SUM_LIGHTS) || out->gbuffer || out->aov_diffuse || out->aov_specular))
@@ -537,7 +537,7 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
     uint32_t* cnt = c->gb.counters;
     // ---- a3: projection ------------------------------------------------------------------------
     begin(SSSGS_STAGE_PROJECT);
-    add(launch_project(*g, cam, c->gb, s));
+    add(launch_project(*g, cam, c->gb, (flags & SSSGS_TIGHT_LISTS) ? 1 : 0, s));
     end();
     begin(SSSGS_STAGE_DEPTH_SORT);
     // ---- a5 (1/2): all Gaussians by depth, 4 x 8 bits, stable ------------------------------------

@@ -25,7 +25,7 @@ import pytest
 
 import oracle
 from paper_2408_12282_b200 import scenes
-from test_gpu_parity import check_gbuffer, check_lists, check_shading
+from test_gpu_parity import check_gbuffer, check_lists, check_shading, check_tight_lists
 
 pytestmark = pytest.mark.gpu
 
@@ -49,13 +49,20 @@ def _render_both(scene, view, lights_checked):
         full = {k: (v.index_select(0, sel) if k in per_frame else v).cpu().numpy() for k, v in out.items()}
         full["rgb_all"] = out["rgb"].cpu().numpy()
         del out
-        # the call bench.py times asks for frames and counters only: in a sweep (>= 4 lights) the MLP then runs
-        # on the rows a visibility pre-pass keeps and the walks stream the weight cache
-        out = R.render(cams=cams, lights=lights, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters"))
+        # the call bench.py times asks for frames and counters only, over TIGHT tile lists: in a sweep (>= 4 lights)
+        # the MLP then runs on the rows a visibility pre-pass keeps and the walks stream the weight cache
+        out = R.render(cams=cams, lights=lights, want=("rgb", "gbuffer", "aov_diffuse", "aov_specular", "counters"),
+                       tight=True)
         torch.cuda.synchronize()
         bench = {k: (v.index_select(0, sel) if k in per_frame else v).cpu().numpy() for k, v in out.items()}
         bench["rgb_all"] = out["rgb"].cpu().numpy()
         bench["launches"] = R.launch_count()
+        del out
+        # the tight lists themselves, exported by a geometry-only call
+        out = R.render(cams=cams, lights=lights[:1], want=("sorted_keys", "sorted_vals", "tile_ranges", "counters"),
+                       tight=True, precomputed=torch.zeros((1, scene.n, 4), device="cuda"))
+        torch.cuda.synchronize()
+        bench["tight"] = {k: v.cpu().numpy() for k, v in out.items()}
         del out
     finally:
         R.close()
@@ -117,6 +124,15 @@ def test_full_size_config(cfg, view, n_lights, checked):
     check_lists(scene, full, ref, 0)
 
     rng = np.random.default_rng(1000 + 10 * cfg + view)
+    # ---- the tight lists of the benchmarked call: S5 conditions, the minimal set on 256 sampled tiles --------
+    nonempty = np.nonzero(ranges[:, 1] > ranges[:, 0])[0]
+    t_sel = np.sort(rng.choice(nonempty, size=min(256, len(nonempty)), replace=False))
+    masked_r = np.zeros_like(ranges)
+    masked_r[t_sel] = ranges[t_sel]
+    hit = oracle.tile_hits(scene, cam, proj, vals, masked_r)
+    It, _ = check_tight_lists(bench["tight"], keys, vals, ranges, hit, tiles_checked=t_sel)
+    assert It == bench["counters"][0][1] and It < len(keys)
+    print(f"cfg {cfg} view {view}: canonical {len(keys)} instances, tight {It} ({It / len(keys):.3f})")
     # ---- MLP on a sample of Gaussians --------------------------------------------------------------
     idx = np.sort(rng.choice(scene.n, size=N_ROWS, replace=False))
     sub = scenes.subset(scene, idx)

@@ -22,12 +22,12 @@ ALL = ("rgb", "gbuffer", "aov_diffuse", "aov_specular", "mlp_out", "sorted_keys"
        "tile_ranges", "counters")
 
 
-def gpu_render(scene, want=ALL, precomputed=None, cams=None, lights=None, **kw):
+def gpu_render(scene, want=ALL, precomputed=None, cams=None, lights=None, tight=False, **kw):
     import torch
     from paper_2408_12282_b200 import binding
     r = binding.Renderer(scene, **kw)
     try:
-        out = r.render(cams=cams, lights=lights, want=want, precomputed=precomputed)
+        out = r.render(cams=cams, lights=lights, want=want, precomputed=precomputed, tight=tight)
         torch.cuda.synchronize()
         res = {k: v.cpu().numpy() for k, v in out.items()}
         res["launches"] = r.launch_count()
@@ -48,6 +48,40 @@ def check_lists(scene, res, ref, view=0):
     np.testing.assert_array_equal(keys, ref.keys)
     np.testing.assert_array_equal(vals, ref.vals)
     np.testing.assert_array_equal(res["tile_ranges"][view].view(np.uint32), ref.ranges)
+
+
+def check_tight_lists(res, keys, vals, ranges, hit, view=0, tiles_checked=None):
+    """SURVEY S5 conditions of a tight tile list (SSSGS_TIGHT_LISTS) against the oracle's canonical list
+    (keys, vals, ranges) and its minimal set `hit` (oracle.tile_hits): the tight list is a sub-sequence of the
+    canonical one (same pairs, same order), keeps every pair with alpha >= 1/255 at some pixel of its tile, and
+    its ranges / instance counter describe it.  tiles_checked: `hit` was only computed for these tiles."""
+    cnt = res["counters"][view]
+    It = int(cnt[1])
+    assert cnt[2] == 0 and cnt[3] == 0
+    tk = res["sorted_keys"][view].view(np.uint64)[:It]
+    tv = res["sorted_vals"][view].view(np.uint32)[:It]
+    assert It <= len(keys)
+    # position of every tight pair in the canonical list: equal keys (same tile, same depth bits) are rare
+    lo = np.searchsorted(keys, tk, "left")
+    hi = np.searchsorted(keys, tk, "right")
+    assert (hi > lo).all(), "a tight pair's key is not in the canonical list"
+    pos = lo.copy()
+    for j in np.nonzero(hi - lo > 1)[0]:
+        m = np.nonzero(vals[lo[j]:hi[j]] == tv[j])[0]
+        assert len(m) == 1
+        pos[j] = lo[j] + m[0]
+    assert (vals[pos] == tv).all(), "a tight pair is not in the canonical list"
+    assert (np.diff(pos.astype(np.int64)) > 0).all(), "tight list is not in canonical order"
+    kept = np.zeros(len(keys), bool)
+    kept[pos] = True
+    must = hit if tiles_checked is None else hit & np.isin((keys >> np.uint64(32)).astype(np.int64), tiles_checked)
+    assert kept[must].all(), f"{int((must & ~kept).sum())} pairs with alpha >= 1/255 in their tile were dropped"
+    # ranges of the tight list
+    tt = (tk >> np.uint64(32)).astype(np.int64)
+    n_tiles = ranges.shape[0]
+    want = np.stack([np.searchsorted(tt, np.arange(n_tiles), "left"), np.searchsorted(tt, np.arange(n_tiles), "right")], 1)
+    np.testing.assert_array_equal(res["tile_ranges"][view].view(np.uint32).astype(np.int64), want)
+    return It, int(hit.sum())
 
 
 def unstable_bound(ref_gbuf, flags, ch):
@@ -371,6 +405,56 @@ def test_run_to_run_determinism(cfg, n, width, height):
     # and the same frame when other outputs are requested
     c = gpu_render(scene, want=("rgb", "counters"))
     np.testing.assert_array_equal(a["rgb"].view(np.uint32), c["rgb"].view(np.uint32))
+
+
+def _tight_scenes():
+    yield from _small_scenes()
+    yield "full_image", custom_scene([[0, 0, 0]], 5.0, width=50, height=37)
+    yield "huge_near_plane", custom_scene([[0, -3.7, 0], [0.1, 0, 0]], [[2.0, 0.01, 2.0], [0.05] * 3], width=96, height=64)
+    yield "sub_threshold_opacity", custom_scene(np.random.default_rng(2).uniform(-0.5, 0.5, (200, 3)), 0.08,
+                                                opacities=np.random.default_rng(3).choice([0.002, 1.0 / 255, 0.004, 0.5], 200))
+    yield "dense_1080_like", scenes.make_scene(4, n=20000, width=200, height=120, views=1)
+    yield "one_slot_walk", scenes.make_scene(3, n=30000, width=672, height=640, lights=2)   # 1680 tiles: bit-identical
+
+
+@pytest.mark.parametrize("name,scene", list(_tight_scenes()))
+def test_tight_lists_satisfy_s5_and_render_the_same_frames(name, scene):
+    # SSSGS_TIGHT_LISTS: sub-sequence of the canonical list, superset of the pairs with
+    # alpha >= 1/255 at a pixel of the tile, same order, identical image (bit for bit).
+    want = ("rgb", "gbuffer", "sorted_keys", "sorted_vals", "tile_ranges", "counters")
+    cam = scene.cameras[0]
+    lights = scene.lights[0]
+    canon = gpu_render(scene, want=want, cams=[cam], lights=lights)
+    tight = gpu_render(scene, want=want, cams=[cam], lights=lights, tight=True)
+    proj = oracle.project(scene, cam)
+    keys, vals, ranges = oracle.build_lists(proj)
+    hit = oracle.tile_hits(scene, cam, proj, vals, ranges)
+    It, n_hit = check_tight_lists(tight, keys, vals, ranges, hit)
+    print(f"{name}: canonical {len(keys)}, tight {It}, minimal {n_hit}")
+    assert canon["counters"][0][1] == len(keys) and tight["counters"][0][0] == canon["counters"][0][0]
+    assert n_hit <= It <= len(keys)
+    if len(keys) > 2000:
+        assert It < len(keys)       # it really is tighter
+    # the blended (pixel, entry) pairs are the same; with one entry slot per warp (> 1600 tiles) so is the order of
+    # every sum: bit-identical frames.  The 2- and 4-slot walks of small images group the entries of a staged batch
+    # by position, so another list changes which partial sum an entry joins (last-bit differences).
+    tiles = proj.tiles_x * proj.tiles_y
+    for k in ("rgb", "gbuffer"):
+        if tiles > 1600:
+            np.testing.assert_array_equal(tight[k].view(np.uint32), canon[k].view(np.uint32))
+        else:
+            np.testing.assert_allclose(tight[k], canon[k], rtol=5e-5, atol=2e-6)
+
+
+def test_tight_lists_in_a_sweep_render_the_same_frames():
+    # the call shape bench.py times: sweep (pre-pass, row-skipping MLP, cached walks) over tight lists
+    scene = scenes.make_scene(3, n=40000, width=656, height=656, lights=11)
+    want = ("rgb", "gbuffer", "counters")
+    a = gpu_render(scene, want=want, lights=scene.lights[0])
+    b = gpu_render(scene, want=want, lights=scene.lights[0], tight=True)
+    assert 0 < b["counters"][0][1] < a["counters"][0][1] and b["counters"][0][4] == a["counters"][0][4]
+    for k in ("rgb", "gbuffer"):
+        np.testing.assert_array_equal(a[k].view(np.uint32), b[k].view(np.uint32))
 
 
 def test_empty_scene_and_zero_opacity():

@@ -133,3 +133,70 @@ def test_counters():
     lens = (r.ranges[:, 1].astype(np.int64) - r.ranges[:, 0])
     assert r.comp.p_eval <= int(lens.sum()) * 256
     assert r.comp.contrib.sum() <= r.n_vis
+
+
+# ---- tight tile lists: the minimal set of (tile, Gaussian) pairs --------------------------
+def _hits_of(s):
+    cam = s.cameras[0]
+    proj = oracle.project(s, cam)
+    keys, vals, ranges = oracle.build_lists(proj)
+    return proj, keys, vals, ranges, oracle.tile_hits(s, cam, proj, vals, ranges)
+
+
+def test_tile_hits_closed_form_isotropic():
+    # One isotropic Gaussian: alpha(p) = o exp(-|p - c|^2 / 2 s^2) with s^2 = (f sigma / z)^2 + 0.3 (low-pass; the
+    # x^2 / z^2 terms of the Jacobian change s by < 0.3 % this close to the axis), so alpha >= 1/255 inside the disc
+    # of radius R = s sqrt(2 ln(255 o)) ~ 11 px.  A tile is hit iff its nearest pixel CENTRE (coordinates 16 t ..
+    # 16 t + 15) lies within R of the projected centre c ~ (27, 32): tile column 0 is in the canonical rectangle
+    # (27 - 3.33 s = 15.7 < 16) but its nearest pixel centre, x = 15, is 12 px away: not hit.
+    s = custom_scene([[-0.224, 0, 0]], 0.15, opacities=0.8, width=65, height=65)
+    cam = s.cameras[0]
+    proj, keys, vals, ranges, hit = _hits_of(s)
+    cx, cy = float(proj.pix[0, 0]), float(proj.pix[0, 1])
+    var = (cam.fx * 0.15 / float(proj.depth[0])) ** 2 + 0.3
+    R = np.sqrt(var * 2 * np.log(255 * 0.8))
+    assert 26.0 < cx < 28.0 and abs(cy - 32) < 1e-3 and 10.5 < R < 11.5
+    tiles = (keys >> np.uint64(32)).astype(int)
+    seen = []
+    for t, h in zip(tiles, hit):
+        ty, tx = divmod(int(t), proj.tiles_x)
+        nx = min(max(cx, 16 * tx), min(16 * tx + 15, 64))   # nearest point of the tile's pixel-centre box
+        ny = min(max(cy, 16 * ty), min(16 * ty + 15, 64))
+        # the nearest pixel CENTRE is the nearest integer point: on the axes through c it is the rounding of c
+        nx, ny = (round(nx) if 16 * tx <= cx <= 16 * tx + 15 else nx), (round(ny) if 16 * ty <= cy <= 16 * ty + 15 else ny)
+        d = np.hypot(nx - cx, ny - cy)
+        assert abs(d - R) > 0.3                               # no borderline tile in this construction
+        assert bool(h) == (d <= R), (tx, ty, d, R)
+        seen.append((tx, ty, bool(h)))
+    assert (0, 2, False) in seen and (1, 2, True) in seen and (2, 2, True) in seen
+    assert 0 < hit.sum() < len(hit)
+
+
+def test_tile_hits_equal_what_each_tile_blends_without_saturation():
+    # With low opacities no pixel ever stops (T stays far above 1e-4), so within ONE tile the Gaussians the
+    # compositor blends somewhere are exactly the tile's entries with a pixel at alpha >= 1/255: orc_tile_hits
+    # against orc_composite (pinned on its own) restricted to one tile at a time.
+    s = scenes.make_scene(2, n=3000, width=96, height=80)
+    s.opacities[:] = np.minimum(s.opacities, 0.02)
+    cam = s.cameras[0]
+    proj, keys, vals, ranges, hit = _hits_of(s)
+    ch = np.zeros((s.n, 14))
+    checked = 0
+    for t in range(proj.tiles_x * proj.tiles_y):
+        b, e = int(ranges[t, 0]), int(ranges[t, 1])
+        if e == b:
+            continue
+        one = np.zeros_like(ranges)
+        one[t] = ranges[t]
+        comp = oracle.composite(s, cam, proj, ch, vals, one)
+        assert comp.gbuf[..., 15].min() > 0.05                       # nothing saturates
+        blended = set(np.nonzero(comp.contrib)[0].tolist())
+        assert blended == set(vals[b:e][hit[b:e]].tolist()), t
+        checked += 1
+    assert checked > 20 and 0 < hit.sum() < len(hit)
+
+
+def test_tile_hits_zero_below_threshold_opacity():
+    s = custom_scene([[0, 0, 0], [0.2, 0, 0.1]], 0.05, opacities=[1.0 / 300, 0.5], width=64, height=64)
+    proj, keys, vals, ranges, hit = _hits_of(s)
+    assert not hit[vals == 0].any() and hit[vals == 1].any()
