@@ -77,6 +77,15 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {
   }
 }
+// TMA bulk copy (no tensor map: a linear range), global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async() {
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
@@ -226,6 +235,8 @@ struct MlpArgs {
   int h_base;                  // accumulator of the last stage (16 columns of its own)
   int a_base, a_stride;        // A operand of the hidden layers and the last stage
   int a0_base, a0_stride;      // A operand of layer 0 (its own region: see write_static)
+  int stagger;                 // SM clocks by which consecutive slots start apart
+  int plain_copy;              // measurement aid: weights copied by all threads instead of TMA bulk copies
   const uint32_t* rows;        // optional: evaluate only the Gaussians rows[0 .. *row_count)
   const uint32_t* row_count;
   int64_t* rows_out;           // optional: receives the number of rows evaluated (SSSGS_CNT_MLP_ROWS)
@@ -500,8 +511,8 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
   const int S = a.slots;
   uint8_t* sW = smem;
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + plan.blob_bytes);
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kMaxSlots);
-  // bars[s] = a_ready of slot s, bars[kMaxSlots + s] = d_ready of slot s
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * kMaxSlots + 1);
+  // bars[s] = a_ready of slot s, bars[kMaxSlots + s] = d_ready of slot s, bars[2 kMaxSlots] = weights landed
 
   pdl_prologue();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -518,18 +529,35 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
   const int64_t n_units = n_blocks * split;
   if (a.rows_out && blockIdx.x == 0 && threadIdx.x == 0) *a.rows_out = n_rows;
 
-  // ---- prologue: weights to smem, barriers, TMEM, the constant-ones operand ----------------------
-  for (int i = tid * 16; i < plan.blob_bytes; i += blockDim.x * 16)
-    *reinterpret_cast<uint4*>(sW + i) = *reinterpret_cast<const uint4*>(a.blob + i);
+  // ---- prologue: barriers, weights to smem, TMEM, the constant-ones operand ----------------------
+  // The packed weights (100-170 KB) come in with TMA bulk copies issued by one thread (32 KB each, completion
+  // counted on an mbarrier): they land through the async proxy the tensor core reads with, and the other
+  // threads go on to allocate TMEM and assemble their first rows meanwhile.  (Before: 16-byte LDG + STS by
+  // every thread, ~20 round trips each, and a proxy fence.)
+  const uint32_t bar_w = smem_u32(bars + 2 * kMaxSlots);
   if (tid == 0) {
     for (int s = 0; s < S; ++s) {
       mbar_init(smem_u32(bars + s), WPS * 32);
       mbar_init(smem_u32(bars + kMaxSlots + s), 1);
     }
+    mbar_init(bar_w, 1);
     fence_barrier_init();
+    if (a.plain_copy) mbar_arrive(bar_w);
+    else mbar_expect_tx(bar_w, (uint32_t)plan.blob_bytes);
+    // 4 KB pieces, every CTA starting at another one: all CTAs of the grid read the same blob at the same time,
+    // and in the same order they would queue on the same L2 slices
+    const int n_pieces = (plan.blob_bytes + 4095) / 4096;
+    for (int q = 0; q < n_pieces && !a.plain_copy; ++q) {
+      const int off = ((q + (int)blockIdx.x * 7) % n_pieces) * 4096;
+      bulk_copy_g2s(smem_u32(sW + off), a.blob + off, (uint32_t)min(4096, plan.blob_bytes - off), bar_w);
+    }
+  }
+  if (a.plain_copy) {  // measurement aid (SSSGS_MLP_PLAIN_COPY=1): the round-1 copy, 16-byte LDG + STS by every thread
+    for (int i = tid * 16; i < plan.blob_bytes; i += blockDim.x * 16)
+      *reinterpret_cast<uint4*>(sW + i) = *reinterpret_cast<const uint4*>(a.blob + i);
+    fence_proxy_async();
   }
   if (warp == 0) tmem_alloc(smem_u32(tmem_slot), kTmemCols);
-  fence_proxy_async();  // weights were written with generic stores; UMMA reads via the async proxy
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -622,6 +650,13 @@ __global__ void __launch_bounds__(kMlpThreadsMax, 1) mlp_kernel(const __grid_con
     const int c_begin = (WPS == 8 && half == 1) ? c_split : 0;
     const int c_end = (WPS == 8 && half == 0) ? c_split : nchunks;
     uint32_t pd = 0;
+    if (wq == 0) mbar_wait(bar_w, 0);   // the issuing warps: the bulk copies of the weights have landed
+    // The slots of a CTA should run out of phase (one slot's epilogue under the other's MMAs); started together
+    // they tend to stay in step.  Slot s starts s * stagger clocks late (tuning aid SSSGS_MLP_STAGGER).
+    if (slot > 0 && a.stagger > 0) {
+      const long long t_go = clock64() + (long long)slot * a.stagger;
+      while (clock64() < t_go) __nanosleep(100);
+    }
     for (int64_t u = (int64_t)slot * gridDim.x + blockIdx.x; u < n_units; u += (int64_t)S * gridDim.x) {
       const int64_t row = (u / split) * kRows + r;
       const int light0 = (int)(u % split) * lights_per_unit;
@@ -748,7 +783,7 @@ static MlpShape mlp_shape(const MlpPlan& plan) {
 }
 
 int mlp_smem_bytes(const MlpPlan& plan) {
-  return plan.blob_bytes + 2 * kMaxSlots * 8 + 16 + 1024;
+  return plan.blob_bytes + (2 * kMaxSlots + 1) * 8 + 16 + 1024;
 }
 
 int launch_mlp_pack(const sssgs_mlp& mlp, const MlpPlan& plan, uint8_t* blob, cudaStream_t s) {
@@ -776,6 +811,14 @@ int launch_mlp(const sssgs_gaussians& g, const MlpPlan& plan, const uint8_t* blo
   const MlpShape sh = mlp_shape(plan);
   a.slots = sh.slots; a.wps = sh.wps; a.d_stride = sh.d_stride; a.h_base = sh.h_base; a.a_base = sh.a_base;
   a.a_stride = sh.a_stride; a.a0_base = sh.a0_base; a.a0_stride = sh.a0_stride;
+  {
+    static int stagger = -1;
+    if (stagger < 0) { const char* e = getenv("SSSGS_MLP_STAGGER"); stagger = e ? atoi(e) : 0; }
+    a.stagger = stagger;
+    static int plain = -1;
+    if (plain < 0) { const char* e = getenv("SSSGS_MLP_PLAIN_COPY"); plain = e ? atoi(e) : 0; }
+    a.plain_copy = plain;
+  }
   const int smem = mlp_smem_bytes(plan);
   const int64_t units = (g.n + kRows - 1) / kRows;
   int grid = (int)(units < max_ctas ? units : max_ctas);

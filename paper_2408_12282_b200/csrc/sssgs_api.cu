@@ -611,22 +611,13 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
         // buffer `buf` was last read by the raster of batch_no - 2
         if (overlap && batch_no >= 2 && cudaStreamWaitEvent(sm, c->ev_raster[buf], 0) != cudaSuccess)
           return fail(c, SSSGS_ECUDA, "stream wait failed");
-        // The MLP of a camera's first light batch runs next to the latency-bound geometry chain.
-        // One MLP CTA fills an SM (registers, TMEM), so when that MLP is expected to finish before
-        // the chain even on a part of the SMs, it is confined to a third or half of them and the geometry
-        // kernels keep the rest (estimates: ~35 % of the bf16 peak for the MLP, 60 us + 0.35 us per
-        // 1000 Gaussians for the chain; measured on configs 2 and 4: -7 % per frame).
+        // The MLP of a camera's first light batch runs next to the geometry chain (side stream).  One MLP
+        // CTA fills an SM (512 threads x 128 registers, TMEM), so the two do not share SMs: the MLP is
+        // confined to a third of them and the latency-bound geometry kernels keep the rest.  Measured on
+        // configs 2 and 4 (profiles/r02_notes.md): the step time is flat from a third of the SMs upwards
+        // (cfg 4: 0.812 ms at 49 SMs, 0.806 at 60 ... 148) and rises below it (0.95 at 37, 1.21 at 25).
         int mlp_ctas = c->num_sms;
-        if (overlap && l0 == 0 && !use_mask) {
-          double flop_row = 0.0;
-          for (int q = 0; q < plan.n_stages; ++q) flop_row += 2.0 * plan.st[q].k_pad * plan.st[q].n_pad;
-          const double mlp_all_us = (double)g->n * nl * flop_row / 580e12 * 1e6;
-          const double chain_us = 60.0 + 0.35e-3 * (double)g->n;
-          // measured on configs 2 and 4: a third of the SMs is the best split up to an estimated MLP time
-          // of ~1.4x the chain's (50 SMs: 0.797 ms on config 4, 74: 0.809, 40: 0.88)
-          if (20.0 + 3.0 * mlp_all_us <= 1.4 * chain_us) mlp_ctas = (c->num_sms + 2) / 3;
-          else if (20.0 + 2.0 * mlp_all_us <= chain_us) mlp_ctas = c->num_sms / 2;
-        }
+        if (overlap && l0 == 0 && !use_mask) mlp_ctas = (c->num_sms + 2) / 3;
         const int k = launch_mlp(*g, plan, c->mlp_blob, cam, lb, nl, mlp_buf,
                                  out->mlp_out ? out->mlp_out + frame0 * g->n * 4 : nullptr, g->n * 4,
                                  mlp_ctas, use_mask ? c->rows : nullptr, use_mask ? cnt + DC_CONTRIB_ROWS : nullptr,
