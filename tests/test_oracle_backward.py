@@ -1,0 +1,167 @@
+"""Pins of the backward oracle (oracle/backward.py: steps a2 / a7 / a8 differentiated; PAPER.md L11, L112,
+L343-349): its forward restatements equal the C++ oracle, every gradient equals central finite differences of
+the C++ FORWARD oracle, and closed forms of one and two Gaussians on a pixel centre.  CPU only."""
+import dataclasses
+
+import numpy as np
+import torch
+
+import oracle
+from oracle import backward as ob
+from paper_2408_12282_b200 import scenes
+from util import custom_scene, with_mlp_params
+
+
+def _setup(scene, view=0):
+    cam = scene.cameras[view]
+    proj = oracle.project(scene, cam)
+    keys, vals, ranges = oracle.build_lists(proj)
+    xs = [oracle.mlp_inputs(scene, cam, lt.position) for lt in scene.lights[view]]
+    return cam, proj, vals, ranges, xs
+
+
+def _cpp_loss(scene, proj, vals, ranges, xs, G, view=0):
+    """L = sum_l <G_l, rgb_l> through the C++ forward oracle (MLP mode 0, compositing, shading)."""
+    cam = scene.cameras[view]
+    tot = 0.0
+    for li, lt in enumerate(scene.lights[view]):
+        mo = oracle.mlp_forward(xs[li], scene.mlp, 0)
+        comp = oracle.composite(scene, cam, proj, oracle.channels(scene, proj, mo), vals, ranges)
+        rgb = oracle.shade(cam, lt, comp.gbuf)[0]
+        tot += float((rgb * G[li]).sum())
+    return tot
+
+
+def _scene():
+    s = scenes.make_scene(3, n=400, width=40, height=32, lights=2)
+    # moderate opacities: most pixels keep T well above 1e-4, few decisions near a threshold
+    return dataclasses.replace(s, opacities=np.clip(s.opacities, 0.05, 0.6).astype(np.float32))
+
+
+def test_forward_restatements_equal_the_cpp_oracle():
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    mo_ref = oracle.mlp_forward(xs[0], s.mlp, 0)
+    mo = ob.mlp_torch(ob._t(xs[0]), s.mlp, ob._t(s.mlp.params)).numpy()
+    np.testing.assert_allclose(mo, mo_ref, rtol=1e-12, atol=1e-13)
+    s6 = scenes.make_scene(6, n=50)                                   # paper architecture: split heads, Leaky-ReLU
+    x6 = oracle.mlp_inputs(s6, s6.cameras[0], s6.lights[0][0].position)
+    np.testing.assert_allclose(ob.mlp_torch(ob._t(x6), s6.mlp, ob._t(s6.mlp.params)).numpy(),
+                               oracle.mlp_forward(x6, s6.mlp, 0), rtol=1e-12, atol=1e-13)
+    ch = oracle.channels(s, proj, mo_ref)
+    comp = oracle.composite(s, cam, proj, ch, vals, ranges)
+    gb = ob.composite_torch(cam.width, cam.height, ob._t(proj.pix), ob._t(proj.conic), ob._t(s.opacities), ob._t(ch),
+                            vals, ranges, proj.tiles_x).numpy()
+    np.testing.assert_allclose(gb, comp.gbuf, rtol=1e-12, atol=1e-13)
+    assert comp.p_blend > 1000 and (comp.gbuf[..., 15] < 0.5).any()
+    lt = s.lights[0][1]
+    rgb = ob.shade_torch(cam, lt.position, lt.intensity, ob._t(comp.gbuf)).numpy()
+    np.testing.assert_allclose(rgb, oracle.shade(cam, lt, comp.gbuf)[0], rtol=1e-11, atol=1e-13)
+
+
+def test_gradients_equal_finite_differences_of_the_cpp_forward():
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    rng = np.random.default_rng(11)
+    G = rng.standard_normal((2, cam.height, cam.width, 3))
+    r = ob.render_backward(s, proj, vals, ranges, xs, G)
+    np.testing.assert_allclose(r.loss, _cpp_loss(s, proj, vals, ranges, xs, G), rtol=1e-11)
+
+    def fd(apply, h):
+        """central difference; apply(delta) -> (scene', proj', actual +delta, actual -delta)"""
+        sp, pp, dp = apply(+h)
+        sm, pm, dm = apply(-h)
+        return (_cpp_loss(sp, pp, vals, ranges, xs, G) - _cpp_loss(sm, pm, vals, ranges, xs, G)) / (dp - dm)
+
+    def pick(g):     # the largest gradients and a few random ones
+        flat = np.abs(g).ravel()
+        return sorted(set(np.argsort(-flat)[:3].tolist() + rng.choice(flat.size, 3, replace=False).tolist()))
+
+    def check(name, got, ref):
+        assert abs(got - ref) <= 2e-5 * max(1.0, abs(ref)) + 1e-7, (name, got, ref)
+
+    # per-Gaussian float32 inputs of the scene
+    for name, field, h in [("d_opacity", "opacities", 1e-4), ("d_normals", "normals", 1e-4), ("d_base", "base_color", 1e-4),
+                           ("d_rough", "roughness", 1e-4), ("d_metal", "metallic", 1e-4), ("d_sss", "subsurface", 1e-4)]:
+        g = getattr(r, name)
+        for k in pick(g):
+            def apply(d, field=field, k=k):
+                a = getattr(s, field).copy()
+                a.ravel()[k] = np.float32(a.ravel()[k] + d)
+                return dataclasses.replace(s, **{field: a}), proj, float(a.ravel()[k])
+            check((name, k), g.ravel()[k], fd(apply, h))
+    # projected quantities (inputs of step 5): 2-D mean, conic, depth
+    for name, field, h in [("d_pix", "pix", 2e-4), ("d_conic", "conic", 1e-5), ("d_depth", "depth", 1e-4)]:
+        g = getattr(r, name)
+        for k in pick(g):
+            def apply(d, field=field, k=k):
+                p2 = type(proj)(**vars(proj))
+                a = getattr(proj, field).copy()
+                a.ravel()[k] = np.float32(a.ravel()[k] + d)
+                setattr(p2, field, a)
+                return s, p2, float(a.ravel()[k])
+            check((name, k), g.ravel()[k], fd(apply, h))
+    # MLP parameters (weights and biases of every layer)
+    for k in pick(r.d_params):
+        def apply(d, k=k):
+            p = s.mlp.params.copy()
+            p[k] = np.float32(p[k] + d)
+            return with_mlp_params(s, p), proj, float(p[k])
+        check(("d_params", k), r.d_params[k], fd(apply, 2e-6))   # small step: a larger one crosses ReLU kinks of some rows
+    assert np.abs(r.d_params).max() > 1e-3 and np.abs(r.d_pix).max() > 1e-3 and np.abs(r.d_conic).max() > 1e-3
+
+
+def test_per_stage_gradients_chain_together():
+    # d_gbuf is the shading backward alone (central differences of orc_shade on single G-buffer values), and
+    # d_mlp_out is the compositing backward of channels 10-13: sum_p w_i(p) d_gbuf[p, 10 + c]
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    rng = np.random.default_rng(5)
+    G = rng.standard_normal((2, cam.height, cam.width, 3))
+    r = ob.render_backward(s, proj, vals, ranges, xs, G)
+    lt = s.lights[0][0]
+    covered = np.argwhere(r.gbuf[0][..., 14] > 0.3)
+    for (y, x) in covered[rng.choice(len(covered), 4, replace=False)]:
+        for c in (0, 2, 5, 7, 8, 9, 11, 13, 14):
+            gp, gm = r.gbuf[0].copy(), r.gbuf[0].copy()
+            h = 1e-6 * max(1.0, abs(gp[y, x, c]))
+            gp[y, x, c] += h
+            gm[y, x, c] -= h
+            d = ((oracle.shade(cam, lt, gp)[0] - oracle.shade(cam, lt, gm)[0]) * G[0]).sum() / (2 * h)
+            assert abs(r.d_gbuf[0][y, x, c] - d) <= 1e-6 * max(1.0, abs(d)), (y, x, c)
+    assert (r.d_gbuf[..., 15] == 0).all()          # the final transmittance is not an input of the shading
+    # weights of Gaussian i at every pixel, from two composites that differ in one channel value of i
+    i = int(np.argmax(np.abs(r.d_mlp_out[0]).sum(1)))
+    ch0 = oracle.channels(s, proj, r.mlp_out[0])
+    ch1 = ch0.copy()
+    ch1[i, 10] += 1.0
+    w = (oracle.composite(s, cam, proj, ch1, vals, ranges).gbuf - oracle.composite(s, cam, proj, ch0, vals, ranges).gbuf)[..., 10]
+    for c in range(4):
+        np.testing.assert_allclose(r.d_mlp_out[0][i, c], (w * r.d_gbuf[0][..., 10 + c]).sum(), rtol=1e-9, atol=1e-12)
+
+
+def test_closed_forms_on_a_pixel_centre():
+    # sss = 1, bg = 0: rgb = sum_i T_i alpha_i L_SSS,i (Eq. 7 reduces to the residual, Eq. 3 composites it).
+    # One Gaussian whose centre projects onto pixel (32, 32): alpha there = o  =>  d rgb_c / d o = L_SSS_c,
+    # d rgb_c / d L_SSS_c = o.  Two Gaussians on that pixel, the first nearer: C = o1 c1 + (1 - o1) o2 c2  =>
+    # dC/do1 = c1 - o2 c2, dC/do2 = (1 - o1) c2, dC/dc1 = o1, dC/dc2 = (1 - o1) o2.
+    for means, ops in ([[0, 0, 0]], [0.7]), ([[0, -0.5, 0], [0, 0, 0]], [0.6, 0.8]):
+        s = custom_scene(means, 0.05, opacities=ops, subsurface=1.0, width=65, height=65)
+        cam, proj, vals, ranges, xs = _setup(s)
+        G = np.zeros((1, 65, 65, 3))
+        G[0, 32, 32] = [1.0, 2.0, -0.5]
+        r = ob.render_backward(s, proj, vals, ranges, xs, G)
+        c = r.mlp_out[0][:, :3]                                      # L_SSS of each Gaussian
+        gvec = G[0, 32, 32]
+        if len(ops) == 1:
+            np.testing.assert_allclose(r.rgb[0][32, 32], ops[0] * c[0], rtol=1e-6)
+            np.testing.assert_allclose(r.d_opacity[0], (gvec * c[0]).sum(), rtol=1e-6)
+            np.testing.assert_allclose(r.d_mlp_out[0][0, :3], ops[0] * gvec, rtol=1e-6)
+        else:
+            o1, o2 = ops
+            np.testing.assert_allclose(r.rgb[0][32, 32], o1 * c[0] + (1 - o1) * o2 * c[1], rtol=1e-6)
+            np.testing.assert_allclose(r.d_opacity, [(gvec * (c[0] - o2 * c[1])).sum(), (gvec * (1 - o1) * c[1]).sum()], rtol=1e-6)
+            np.testing.assert_allclose(r.d_mlp_out[0][:, :3], [o1 * gvec, (1 - o1) * o2 * gvec], rtol=1e-6)
+        # on the centre the exponent is stationary: no gradient to the 2-D mean or the conic from this pixel
+        # (the fp32 projection puts the centre within ~1e-5 px of the pixel centre, hence the tolerances)
+        assert np.abs(r.d_pix).max() < 1e-3 and np.abs(r.d_conic).max() < 1e-8
