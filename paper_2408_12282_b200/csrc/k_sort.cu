@@ -212,7 +212,7 @@ __device__ __forceinline__ void sort_tickets(SortSmem& sm, const uint32_t* __res
 // depth_pass >= 0: pass `depth_pass` of the 4-pass depth sort over the ping-pong buffers
 // (k0,v0) <-> (k1,v1); `hist` then points at all four histograms and trivial passes are skipped.
 // depth_pass < 0: a plain pass from (k0,v0) to (k1,v1) with its own histogram.
-__global__ void __launch_bounds__(kSortThreads, 3)
+__global__ void __launch_bounds__(kSortThreads, 4)
 radix_pass_kernel(uint32_t* __restrict__ k0, uint32_t* __restrict__ v0, uint32_t* __restrict__ k1,
                   uint32_t* __restrict__ v1, const uint32_t* __restrict__ count_ptr,
                   uint32_t count_cap, int shift, int bits, const uint32_t* __restrict__ hist,
