@@ -375,12 +375,12 @@ def run_gpu(args, rank, world, local_rank):
     # ---- end to end through the C ABI with pinned host buffers -------------------------------------
     H = binding.HostRenderer(scene, max_instances=int(MAX_INSTANCES_PER_GAUSSIAN * scene.n), device=local_rank)
     for _ in range(2):
-        H.render(run.cams, run.lights)
+        H.render(run.cams, run.lights, tight=not args.canonical_lists)
     barrier()
     t0 = time.perf_counter()
     e2e_steps = max(3, min(args.steps, 10))
     for _ in range(e2e_steps):
-        H.render(run.cams, run.lights)
+        H.render(run.cams, run.lights, tight=not args.canonical_lists)
     t_e2e = multi.max_over_ranks(time.perf_counter() - t0, dev)
     e2e_val = multi.whole_job_mpix_per_s(world, e2e_steps, fps, npix, t_e2e * 1e3)
     h2d, d2h = H.h2d_bytes, H.d2h_bytes

@@ -253,6 +253,41 @@ typedef struct {
 } sssgs_bake;
 int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_bake* bake, void* stream);
 
+/* Backward pass of the render path's steps a8 (deferred shading), a7 (compositing) and a2 (the MLP)
+ * ("optimize all parameters jointly via raytraced differentiable
+ * rendering", L112, L343-349: the training losses are functions of the rendered image and of the
+ * rasterised property images).  For ONE camera and its n_light lights, with
+ *   L = sum_l < grad_rgb[l], rgb_l >
+ * it computes dL/d of: the G-buffer of every light; the MLP outputs per (light, Gaussian); the MLP
+ * parameters Theta; and per Gaussian the opacity, the 2-D mean, the conic (inverse 2-D covariance,
+ * entries a, b, c of  power = -(a dx^2 + c dy^2) / 2 - b dx dy), the depth, the normal, the base
+ * colour, roughness, metalness and subsurfaceness.  The 2-D mean / conic / depth gradients are the
+ * interface to the projection's backward (step a3: not part of this call).  The forward decisions
+ * (alpha >= 1/255, the T' < 1e-4 stop, the 0.99 clamp, ReLUs) are constants of the differentiation.
+ * All pointers are DEVICE pointers, 16-byte aligned, fp32; every gradient array is overwritten.
+ * gbuffer must be the G-buffer sssgs_render wrote for the same scene, camera and lights.
+ * mlp.dtype must be SSSGS_F32 (mlp.precomputed_out, if given, is used for the forward values and
+ * grad_params is then left zero).  Arithmetic is fp32; the MLP is re-evaluated in fp32 (not in the
+ * 16-bit operand precision of the forward kernel).  Per-Gaussian sums use float atomics: results are
+ * reproducible to rounding, not bit for bit.  Enqueues on the stream, never synchronises.
+ * With n_light = 0 (or n = 0) the per-Gaussian and parameter gradients are zeroed and the per-light
+ * pointers are not read.  Errors: SSSGS_EINVAL (NULL / misaligned / dtype), SSSGS_ECAPACITY (n, image size). */
+typedef struct {
+  const float* grad_rgb;     /* [n_light][H][W][3]  dL / d rgb                         (in)          */
+  const float* gbuffer;      /* [n_light][H][W][16] the forward call's G-buffer        (in)          */
+  float* grad_gbuffer;       /* [n_light][H][W][16] dL / d gbuffer                     (out, required) */
+  float* grad_mlp_out;       /* [n_light][n][4]     dL / d (L_SSS rgb, L_in)           (out, required) */
+  float* grad_params;        /* [params_bytes / 4]  dL / d Theta, packing of sssgs_mlp.params (out, may be NULL) */
+  float* grad_opacity;       /* [n]                                                    (out, required) */
+  float* grad_mean2d;        /* [n][2]  dL / d (pix_x, pix_y)                          (out, required) */
+  float* grad_conic;         /* [n][3]  dL / d (a, b, c)                               (out, required) */
+  float* grad_depth;         /* [n]                                                    (out, required) */
+  float* grad_attr;          /* [n][9]  normal (3), base colour (3), roughness, metalness, sss (out, required) */
+} sssgs_grads;
+int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
+                          const sssgs_camera* cam, const sssgs_light* lights, int n_light,
+                          const sssgs_grads* grads, uint32_t flags, void* cuda_stream);
+
 /* Per-stage device timing (measurement aid, off by default).  When enabled, sssgs_render
  * records CUDA events around each stage on the caller's stream (not capture-safe while on);
  * sssgs_profile_read synchronises those events and writes the milliseconds each stage of the

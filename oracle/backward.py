@@ -176,11 +176,14 @@ def shade_torch(cam, light_pos, light_intensity, gbuf: torch.Tensor) -> torch.Te
 # ---------------------------------------------------------------------------------------------------
 # The gradients
 # ---------------------------------------------------------------------------------------------------
-def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16):
+def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16,
+                    given_mlp_out=None):
     """Gradients of L = sum_l <grad_rgb[l], rgb_l> for one view.
 
     proj / vals / ranges: the oracle's projection and tile lists of the view (oracle.project / build_lists);
     mlp_inputs: [L][n, in_dim] float64 (oracle.mlp_inputs per light); grad_rgb [L, H, W, 3].
+    given_mlp_out: [L, n, 4] or None: the MLP outputs are these constants instead of mlp(mlp_inputs) (isolates
+    the walks: d_params is then zero).
     Returns a namespace of numpy float64 arrays:
       rgb [L,H,W,3], gbuf [L,H,W,16]              forward values of the restatement
       d_gbuf [L,H,W,16]                           step a8 backward (per light)
@@ -205,7 +208,10 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
     rgbs, gbufs, mlp_outs = [], [], []
     loss = torch.zeros((), dtype=F8)
     for li, lt in enumerate(lights):
-        mo = mlp_torch(_t(mlp_inputs[li]), scene.mlp, params)
+        if given_mlp_out is None:
+            mo = mlp_torch(_t(mlp_inputs[li]), scene.mlp, params)
+        else:
+            mo = _t(given_mlp_out[li]).clone().requires_grad_(True)
         mo.retain_grad()
         ch = torch.cat([depth[:, None], normals, base, rough[:, None], metal[:, None], sss[:, None], mo], dim=1)
         gb = composite_torch(cam.width, cam.height, pix, conic, opac, ch, vals, ranges, proj.tiles_x, tile)

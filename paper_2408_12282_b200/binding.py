@@ -34,7 +34,7 @@ CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
-           "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility"]
+           "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility", "sssgs_render_backward"]
 STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster", "prepass"]
 
 _f = ctypes.c_float
@@ -80,6 +80,11 @@ class sssgs_out(ctypes.Structure):
                 ("counters", _vp)]
 
 
+class sssgs_grads(ctypes.Structure):
+    _fields_ = [(k, _vp) for k in ("grad_rgb", "gbuffer", "grad_gbuffer", "grad_mlp_out", "grad_params",
+                                   "grad_opacity", "grad_mean2d", "grad_conic", "grad_depth", "grad_attr")]
+
+
 class sssgs_bake(ctypes.Structure):
     _fields_ = [("n_dirs", ctypes.c_int), ("dirs", _vp), ("weights", _vp), ("t_min", _f),
                 ("sh_degree", ctypes.c_int), ("vis_sh_out", _vp), ("vis_out", _vp), ("positions", ctypes.c_int)]
@@ -115,6 +120,10 @@ def lib() -> ctypes.CDLL:
         L.sssgs_render.argtypes = render_args + [_vp]
         L.sssgs_render_host.restype = ctypes.c_int
         L.sssgs_render_host.argtypes = render_args
+        L.sssgs_render_backward.restype = ctypes.c_int
+        L.sssgs_render_backward.argtypes = [_vp, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_mlp),
+                                            ctypes.POINTER(sssgs_camera), ctypes.POINTER(sssgs_light), ctypes.c_int,
+                                            ctypes.POINTER(sssgs_grads), ctypes.c_uint32, _vp]
         L.sssgs_bake_visibility.restype = ctypes.c_int
         L.sssgs_bake_visibility.argtypes = [_vp, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_bake), _vp]
         L.sssgs_last_launch_count.restype = ctypes.c_int64
@@ -159,6 +168,11 @@ def sssgs_render(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0, stream
 def sssgs_render_host(ctx, g, mlp, cams, n_cam, lights, n_light, out, flags=0) -> None:
     _check(ctx, lib().sssgs_render_host(ctx, ctypes.byref(g), ctypes.byref(mlp), cams, n_cam, lights,
                                         n_light, ctypes.byref(out), flags))
+
+
+def sssgs_render_backward(ctx, g, mlp, cam, lights, n_light, grads, flags=0, stream=None) -> None:
+    _check(ctx, lib().sssgs_render_backward(ctx, ctypes.byref(g), ctypes.byref(mlp), ctypes.byref(cam), lights,
+                                            n_light, ctypes.byref(grads), flags, _vp(stream or 0)))
 
 
 def sssgs_bake_visibility(ctx, g, bake, stream=None) -> None:
@@ -324,6 +338,30 @@ class Renderer:
                      (SSSGS_FORWARD_SHADING if forward else 0) | (SSSGS_TIGHT_LISTS if tight else 0), st)
         return outputs
 
+    def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None):
+        """Enqueue one sssgs_render_backward: cam one scene camera, lights its lights, grad_rgb [L,H,W,3] and
+        gbuffer [L,H,W,16] device tensors (the forward call's G-buffer).  Returns the dict of gradient tensors."""
+        torch = self.torch
+        L, n, W, H = len(lights), max(self.n, 1), cam.width, cam.height
+        z = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)  # noqa: E731
+        out = {"grad_gbuffer": z(L, H, W, 16), "grad_mlp_out": z(L, n, 4), "grad_params": z(self.params.numel()),
+               "grad_opacity": z(n), "grad_mean2d": z(n, 2), "grad_conic": z(n, 3), "grad_depth": z(n),
+               "grad_attr": z(n, 9)}
+        gr = sssgs_grads()
+        self._bwd_in = (grad_rgb.contiguous(), gbuffer.contiguous())
+        gr.grad_rgb, gr.gbuffer = self._bwd_in[0].data_ptr(), self._bwd_in[1].data_ptr()
+        for k, v in out.items():
+            setattr(gr, k, v.data_ptr())
+        larr = (sssgs_light * max(L, 1))(*[make_light(l) for l in lights])
+        pre_ptr = None
+        if precomputed is not None:
+            self._pre = precomputed
+            pre_ptr = precomputed.data_ptr()
+        m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr, self.compute)
+        st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
+        sssgs_render_backward(self.ctx, self.g, m, make_camera(cam), larr, L, gr, SSSGS_TIGHT_LISTS if tight else 0, st)
+        return out
+
     def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None,
                         positions: bool = False):
         """Enqueue one sssgs_bake_visibility on the current torch stream.  dirs [K,3], weights [K] (numpy or
@@ -434,7 +472,7 @@ class HostRenderer:
             sssgs_destroy(self.ctx)
             self.ctx = None
 
-    def render(self, cams, lights, want=("rgb",)):
+    def render(self, cams, lights, want=("rgb",), tight=False):
         torch = self.torch
         n_cam, n_light = len(cams), len(lights)
         W, H = cams[0].width, cams[0].height
@@ -450,6 +488,6 @@ class HostRenderer:
         carr = (sssgs_camera * max(n_cam, 1))(*[make_camera(c) for c in cams])
         larr = (sssgs_light * max(n_light, 1))(*[make_light(l) for l in lights])
         m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4)
-        sssgs_render_host(self.ctx, self.g, m, carr, n_cam, larr, n_light, o, 0)
+        sssgs_render_host(self.ctx, self.g, m, carr, n_cam, larr, n_light, o, SSSGS_TIGHT_LISTS if tight else 0)
         self.d2h_bytes = d2h
         return {k: self.out[k] for k in want}

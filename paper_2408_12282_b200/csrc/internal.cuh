@@ -296,6 +296,17 @@ int launch_raster(const CamParams& cam, const LightBatch& lights, int n_lights,
 // sum_mode: 0 = one RGB frame per light; 1 = ONE frame = sum over the batch's lights + background
 // term (first batch of a camera); 2 = add the batch's lights to the frame already there
 
+// backward pass (k_backward.cu)
+int launch_zero(float* p, int64_t n, cudaStream_t s);
+int launch_shade_backward(const CamParams& cam, const LightBatch& lights, int n_lights, const float* gbuf,
+                          const float* grad_rgb, float* grad_gbuf, cudaStream_t s);
+int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuffers& gb, const uint32_t* sorted_vals,
+                              const float4* attr, const float4* mlp_out, int mlp_stride, const float* grad_gbuf,
+                              float* g_opacity, float* g_mean2d, float* g_conic, float* g_depth, float* g_attr,
+                              float* g_mlp_out, int64_t n, cudaStream_t s);
+int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
+                        int n_lights, int light0, const float* g_mlp_out, float* g_params, int num_sms, cudaStream_t s);
+
 int mlp_smem_bytes(const MlpPlan& plan);
 
 }  // namespace sssgs

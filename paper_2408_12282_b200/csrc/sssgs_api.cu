@@ -674,6 +674,127 @@ int sssgs_render(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, c
   return SSSGS_OK;
 }
 
+// backward of a8 / a7 / a2 for one camera.  Geometry and the MLP forward are run again (they
+// are cheap next to the walks), then shading backward per light batch, the back-to-front compositing walk
+// and the MLP backward.
+int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_mlp* mlp, const sssgs_camera* cam_in,
+                          const sssgs_light* lights, int n_light, const sssgs_grads* gr, uint32_t flags,
+                          void* cuda_stream) {
+  if (!c) return SSSGS_EINVAL;
+  if (!g || !mlp || !cam_in || !gr || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
+  if (flags & ~(uint32_t)SSSGS_TIGHT_LISTS) return fail(c, SSSGS_EINVAL, "sssgs_render_backward: only SSSGS_TIGHT_LISTS is accepted");
+  if (n_light < 0 || g->n < 0) return fail(c, SSSGS_EINVAL, "negative count");
+  if (g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n exceeds max_gaussians");
+  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(c, SSSGS_EINVAL, "vis_sh_degree must be 0 or 1");
+  if (g->feat_dim < 0 || g->feat_dim > 88 || g->feat_dim % 4) return fail(c, SSSGS_EINVAL, "feat_dim must be a multiple of 4 in [0,88]");
+  const void* must[] = {gr->grad_opacity, gr->grad_mean2d, gr->grad_conic, gr->grad_depth, gr->grad_attr};
+  for (const void* p : must)
+    if (!p || !aligned16(p)) return fail(c, SSSGS_EINVAL, "a gradient pointer is NULL or not 16-byte aligned");
+  const void* per_light[] = {gr->grad_rgb, gr->gbuffer, gr->grad_gbuffer, gr->grad_mlp_out};
+  for (const void* p : per_light)   // per-light arrays are empty without lights
+    if (n_light > 0 && (!p || !aligned16(p))) return fail(c, SSSGS_EINVAL, "a per-light gradient pointer is NULL or not 16-byte aligned");
+  if (gr->grad_params && !aligned16(gr->grad_params)) return fail(c, SSSGS_EINVAL, "grad_params misaligned");
+  if (g->n > 0) {
+    const void* req[] = {g->means, g->scales, g->rotations, g->opacities, g->normals, g->base_color,
+                         g->roughness, g->metallic, g->subsurface, g->vis_sh};
+    for (const void* p : req)
+      if (!p || !aligned16(p)) return fail(c, SSSGS_EINVAL, "a Gaussian attribute pointer is NULL or not 16-byte aligned");
+    if (g->feat_dim > 0 && (!g->feat || !aligned16(g->feat))) return fail(c, SSSGS_EINVAL, "feat is NULL or misaligned");
+  }
+  const sssgs_camera& cm = *cam_in;
+  if (cm.width <= 0 || cm.height <= 0 || cm.width > c->cfg.max_width || cm.height > c->cfg.max_height)
+    return fail(c, SSSGS_ECAPACITY, "camera size out of range");
+  if (!(cm.fx > 0.f) || !(cm.fy > 0.f) || !(cm.znear > 0.f)) return fail(c, SSSGS_EINVAL, "fx, fy, znear must be > 0");
+  MlpPlan plan;
+  const bool run_mlp = mlp->precomputed_out == nullptr;
+  if (run_mlp) {
+    if (!mlp->params || !aligned16(mlp->params)) return fail(c, SSSGS_EINVAL, "mlp.params is NULL or misaligned");
+    if (mlp->dtype != SSSGS_F32) return fail(c, SSSGS_EINVAL, "sssgs_render_backward needs fp32 parameters (mlp.dtype = SSSGS_F32)");
+    const int rc = build_plan(c, *mlp, g->feat_dim, &plan);
+    if (rc != SSSGS_OK) return rc;
+  }
+  DeviceGuard guard(c->cfg.device);
+  if (!guard.ok) return fail(c, SSSGS_ECUDA, "cudaSetDevice(%d) failed", c->cfg.device);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (c->upload_pending) {
+    c->upload_pending = false;
+    if (cudaStreamWaitEvent(s, c->ev_upload, 0) != cudaSuccess) return fail(c, SSSGS_ECUDA, "stream wait failed");
+  }
+  const int64_t n = g->n;
+  const CamParams cam = make_cam(cm);
+  const int tiles = cam.tiles_x * cam.tiles_y;
+  const int64_t npix = (int64_t)cam.width * cam.height;
+  const uint32_t cap = (uint32_t)c->cfg.max_instances;
+  const int max_blocks = c->num_sms * 4;
+  int64_t launches = 0;
+  // every output starts from zero (the walks accumulate with atomics)
+  launches += launch_zero(gr->grad_mlp_out, (int64_t)n_light * n * 4, s);
+  launches += launch_zero(gr->grad_opacity, n, s);
+  launches += launch_zero(gr->grad_mean2d, n * 2, s);
+  launches += launch_zero(gr->grad_conic, n * 3, s);
+  launches += launch_zero(gr->grad_depth, n, s);
+  launches += launch_zero(gr->grad_attr, n * 9, s);
+  if (gr->grad_params) launches += launch_zero(gr->grad_params, (int64_t)(mlp->params_bytes / 4), s);
+  launches += launch_zero(gr->grad_gbuffer, (int64_t)n_light * npix * 16, s);
+  if (n == 0 || n_light == 0) { c->launches = launches; return SSSGS_OK; }
+  // ---- forward state: attributes, geometry of the camera (as sssgs_render) -------------------------
+  launches += launch_pack_attr(*g, c->attr, s);
+  if (run_mlp) launches += launch_mlp_pack(*mlp, plan, c->mlp_blob, s);
+  if (cudaMemsetAsync(c->control, 0, c->control_bytes, s) != cudaSuccess) return fail(c, SSSGS_ECUDA, "memset failed");
+  uint32_t* cnt = c->gb.counters;
+  launches += launch_project(*g, cam, c->gb, (flags & SSSGS_TIGHT_LISTS) ? 1 : 0, s);
+  for (int p = 0; p < 4; ++p)
+    launches += launch_depth_pass(c->gb.dkeys, c->gb.dvals, (uint32_t)n, p, c->gb.hist, c->status_depth[p],
+                                  cnt + DC_TICKET_BASE + p, cnt + DC_SORT_ERROR, max_blocks, s);
+  int tb = 1;
+  while ((1 << tb) < tiles) ++tb;
+  const int npass = tb > 8 ? 2 : 1;
+  const int bits0 = npass == 2 ? (tb + 1) / 2 : tb, bits1 = npass == 2 ? tb - bits0 : 0;
+  launches += launch_emit(n, cam, c->gb, cap, 0, bits0, bits0, bits1, c->status_emit, cnt + DC_TICKET_BASE + 4, s);
+  launches += launch_sort_pass(c->gb.ikeys[0], c->gb.ivals[0], c->gb.ikeys[1], c->gb.ivals[1], cnt + DC_INSTANCES, cap, 0,
+                               bits0, c->gb.hist + 4 * 256, c->status_tile[0], cnt + DC_TICKET_BASE + 5,
+                               cnt + DC_SORT_ERROR, max_blocks, s);
+  if (npass == 2)
+    launches += launch_sort_pass(c->gb.ikeys[1], c->gb.ivals[1], c->gb.ikeys[0], c->gb.ivals[0], cnt + DC_INSTANCES, cap,
+                                 bits0, bits1, c->gb.hist + 5 * 256, c->status_tile[1], cnt + DC_TICKET_BASE + 6,
+                                 cnt + DC_SORT_ERROR, max_blocks, s);
+  const int fi = npass & 1;
+  const uint32_t* sorted_tiles = c->gb.ikeys[fi];
+  const uint32_t* sorted_vals = c->gb.ivals[fi];
+  launches += launch_ranges(sorted_tiles, cam, c->gb, cap, nullptr, nullptr, 0, s);
+  // ---- per light batch -----------------------------------------------------------------------------
+  for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
+    const int nl = n_light - l0 < c->max_lb ? n_light - l0 : c->max_lb;
+    LightBatch lb;
+    memset(&lb, 0, sizeof lb);
+    for (int l = 0; l < nl; ++l) {
+      memcpy(lb.l[l].pos, lights[l0 + l].position, 12);
+      memcpy(lb.l[l].intensity, lights[l0 + l].intensity, 12);
+    }
+    float4* mlp_buf = c->mlp_out[0];
+    if (run_mlp) {
+      const int k = launch_mlp(*g, plan, c->mlp_blob, cam, lb, nl, mlp_buf, nullptr, 0, c->num_sms, nullptr, nullptr, nullptr, s);
+      if (k < 0) return fail(c, SSSGS_ECUDA, "MLP kernel configuration failed");
+      launches += k;
+    } else {
+      launches += launch_gather_precomputed(mlp->precomputed_out + (int64_t)l0 * n * 4, n, nl, n * 4, mlp_buf, s);
+    }
+    launches += launch_shade_backward(cam, lb, nl, gr->gbuffer + (int64_t)l0 * npix * 16, gr->grad_rgb + (int64_t)l0 * npix * 3,
+                                      gr->grad_gbuffer + (int64_t)l0 * npix * 16, s);
+    launches += launch_composite_backward(cam, nl, c->gb, sorted_vals, c->attr, mlp_buf, nl,
+                                          gr->grad_gbuffer + (int64_t)l0 * npix * 16, gr->grad_opacity, gr->grad_mean2d,
+                                          gr->grad_conic, gr->grad_depth, gr->grad_attr,
+                                          gr->grad_mlp_out + (int64_t)l0 * n * 4, n, s);
+    if (run_mlp && gr->grad_params)
+      launches += launch_mlp_backward(*g, *mlp, cam, lb, nl, 0, gr->grad_mlp_out + (int64_t)l0 * n * 4, gr->grad_params,
+                                      c->num_sms, s);
+  }
+  c->launches = launches;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, SSSGS_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
+  return SSSGS_OK;
+}
+
 }  // extern "C"
 
 // ---------------------------------------------------------------------------------------------
