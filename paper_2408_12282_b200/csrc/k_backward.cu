@@ -384,80 +384,221 @@ __device__ __forceinline__ void mlp_input_row(const sssgs_gaussians& g, int64_t 
 // Layer table of the MLP in the caller's parameter packing (sssgs_mlp.params, fp32).
 struct BwdLayer { int w, b, out, in, src, kind; };   // src: index of the layer whose output feeds this one (-1: x)
 struct BwdNet {
-  int n_layers, in_dim, activation;
+  int n_layers, in_dim, activation, trunk_last;
   float slope;
   BwdLayer L[SSSGS_MAX_TRUNK + SSSGS_MAX_INC_HIDDEN + 2];
 };
 enum { K_HIDDEN = 0, K_SSS = 1, K_INC_OUT = 2 };
-constexpr int kBwdMaxW = 128;
-constexpr int kBwdMaxIn = 128;
 
-// One CTA of 128 threads per (Gaussian, light) row, looping over rows; thread t = neuron t.  Activations of
-// all layers of the row stay in shared memory; the weight gradients are accumulated straight into global
-// memory (atomicAdd of delta_t * h_k: 128 threads sweep the 128 x in matrix of a layer).
-__global__ void __launch_bounds__(128)
-mlp_backward_kernel(sssgs_gaussians g, BwdNet net, const float* __restrict__ params, CamParams cam, LightBatch lights,
-                    int n_lights, int light0, const float* __restrict__ g_mlp_out, int64_t n,
-                    float* __restrict__ g_params) {
-  __shared__ float s_h[SSSGS_MAX_TRUNK + SSSGS_MAX_INC_HIDDEN + 3][kBwdMaxIn];   // s_h[0] = x, s_h[l + 1] = output of layer l
-  __shared__ float s_d[2][kBwdMaxW];
-  __shared__ float s_dacc[SSSGS_MAX_TRUNK + SSSGS_MAX_INC_HIDDEN + 3][kBwdMaxW];   // gradient wrt each layer's OUTPUT
-  const int t = threadIdx.x;
-  (void)s_d;
-  for (int64_t row = blockIdx.x; row < n * n_lights; row += gridDim.x) {
-    const int64_t i = row % n;
-    const int l_idx = (int)(row / n);
-    const float* go = g_mlp_out + ((size_t)(light0 + l_idx) * n + i) * 4;
-    const float go4[4] = {go[0], go[1], go[2], go[3]};
-    if (go4[0] == 0.f && go4[1] == 0.f && go4[2] == 0.f && go4[3] == 0.f) continue;   // row never blended: no gradient
-    __syncthreads();
-    if (t == 0) mlp_input_row(g, i, cam.pos, lights.l[l_idx].pos, s_h[0]);
-    for (int l = 0; l <= net.n_layers; ++l) s_dacc[l][t] = 0.f;
-    __syncthreads();
-    // ---- forward, fp32 ----
-    for (int l = 0; l < net.n_layers; ++l) {
-      const BwdLayer& L = net.L[l];
-      const float* hin = s_h[L.src + 1];
-      if (t < L.out) {
-        float s = params[L.b + t];
-        const float* W = params + L.w + (size_t)t * L.in;
-        for (int k = 0; k < L.in; ++k) s = fmaf(W[k], hin[k], s);
-        float y;
-        if (L.kind == K_HIDDEN) y = s > 0.f ? s : (net.activation == SSSGS_ACT_LEAKY_RELU ? net.slope * s : 0.f);
-        else if (L.kind == K_SSS) y = 1.f / (1.f + expf(-s));
-        else y = fmaxf(0.f, s);
-        s_h[l + 1][t] = y;
-      }
-      __syncthreads();
+constexpr int kBR = 16;    // rows of a tile
+constexpr int kWS = 132;   // row stride of the staged weight matrix (floats): 16-byte aligned rows, conflict-free LDS.128 down a column
+
+// Rows of the batch whose dL/d(mlp_out) is not all zero (a Gaussian no pixel blended gets no gradient: 88 % of the
+// rows of a large scene), compacted into a list; order is arbitrary (the sums below are atomics anyway).
+__global__ void __launch_bounds__(256)
+bwd_rows_kernel(const float4* __restrict__ g_mlp_out, int64_t total, uint32_t* __restrict__ list, uint32_t* __restrict__ count) {
+  for (int64_t base = (int64_t)blockIdx.x * 256; base < total; base += (int64_t)gridDim.x * 256) {
+    const int64_t idx = base + threadIdx.x;
+    bool on = false;
+    if (idx < total) {
+      const float4 v = g_mlp_out[idx];
+      on = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
     }
-    // ---- backward ----
-    for (int l = net.n_layers - 1; l >= 0; --l) {
-      const BwdLayer& L = net.L[l];
-      // delta_t = dL/d(pre-activation of neuron t of layer l)
-      float delta = 0.f;
-      if (t < L.out) {
-        const float y = s_h[l + 1][t];
-        if (L.kind == K_SSS) delta = go4[t] * y * (1.f - y);
-        else if (L.kind == K_INC_OUT) delta = y > 0.f ? go4[3] : 0.f;
-        else delta = s_dacc[l + 1][t] * (y > 0.f ? 1.f : (net.activation == SSSGS_ACT_LEAKY_RELU ? net.slope : 0.f));
+    const unsigned m = __ballot_sync(0xffffffffu, on);
+    const int lane = threadIdx.x & 31;
+    unsigned at = 0;
+    if (lane == 0 && m) at = atomicAdd(count, (unsigned)__popc(m));
+    at = __shfl_sync(0xffffffffu, at, 0);
+    if (on) list[at + __popc(m & ((1u << lane) - 1u))] = (uint32_t)idx;
+  }
+}
+
+__device__ __forceinline__ float dot4(const float4 a, const float4 b, float s) {
+  return fmaf(a.w, b.w, fmaf(a.z, b.z, fmaf(a.y, b.y, fmaf(a.x, b.x, s))));
+}
+
+// MLP backward (step a2 differentiated), fp32 on the CUDA cores.  blockIdx.y = the layer whose weight gradient this
+// CTA accumulates (64 register accumulators per thread cover its out x in <= 128 x 128 matrix); blockIdx.x strides
+// over tiles of kBR listed rows.  Per tile: inputs (recomputed from the Gaussian, as the forward kernel does), the
+// forward pass through every layer (activations stay in shared memory), the delta recursion from the two heads down
+// to the target layer, and  dW += delta^T h,  db += sum delta.  Each layer's weights are staged in shared memory
+// once per tile and pass.  The accumulators go to global memory once, with atomics, when the CTA has no tiles left.
+__global__ void __launch_bounds__(256, 1)
+mlp_backward_kernel(sssgs_gaussians g, BwdNet net, const float* __restrict__ params, CamParams cam, LightBatch lights,
+                    int64_t n, const uint32_t* __restrict__ list, const uint32_t* __restrict__ count,
+                    const float* __restrict__ g_mlp_out, float* __restrict__ g_params) {
+  extern __shared__ __align__(16) float bw_smem[];
+  float* sW = bw_smem;                           // [128][kWS]
+  float* sGA = sW + 128 * kWS;                   // [kBR][128] gradient wrt a trunk layer's output
+  float* sGB = sGA + kBR * 128;                  // [kBR][128] ... an incident-head layer's output
+  float* sD = sGB + kBR * 128;                   // [kBR][128] delta of the current layer
+  float* sGo = sD + kBR * 128;                   // [kBR][4]   dL/d(mlp_out) of the rows
+  float* sAct = sGo + kBR * 4;                   // [n_layers + 1][kBR][128]: x, then each layer's output
+  const int tid = threadIdx.x;
+  const int target = blockIdx.y;
+  const BwdLayer T = net.L[target];
+  const int trunk_last = net.trunk_last;
+  const unsigned nrows = *count;
+  const unsigned ntiles = (nrows + kBR - 1) / kBR;
+  float acc[8][8];
+  float accb[8];
+#pragma unroll
+  for (int a = 0; a < 8; ++a) {
+    accb[a] = 0.f;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) acc[a][b] = 0.f;
+  }
+  const int rg = tid >> 6, oc = tid & 63;        // forward / delta recursion: rows 4 rg .. 4 rg + 3
+  const int to = tid >> 4, ti = tid & 15;        // dW: outputs 4 to + {0..3}, 64 + 4 to + {0..3}; inputs likewise with ti
+  bool any = false;
+
+  auto stage_weights = [&](const BwdLayer& L) {   // sW[o][k] = W[o][k], zero outside out x in
+    __syncthreads();
+    for (int idx = tid; idx < 128 * 128; idx += 256) {
+      const int o = idx >> 7, k = idx & 127;
+      sW[o * kWS + k] = (o < L.out && k < L.in) ? params[L.w + (size_t)o * L.in + k] : 0.f;
+    }
+    __syncthreads();
+  };
+
+  for (unsigned tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    any = true;
+    __syncthreads();
+    // ---- rows of the tile: inputs and upstream gradients ----
+    for (int idx = tid; idx < kBR * 128; idx += 256) sAct[idx] = 0.f;
+    __syncthreads();
+    if (tid < kBR) {
+      const unsigned r = tile * kBR + tid;
+      float4 go = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (r < nrows) {
+        const uint32_t idx = list[r];
+        const int64_t i = idx % n;
+        const int l_idx = (int)(idx / n);
+        go = reinterpret_cast<const float4*>(g_mlp_out)[idx];
+        mlp_input_row(g, i, cam.pos, lights.l[l_idx].pos, sAct + tid * 128);
       }
-      __syncthreads();
-      s_d[0][t] = delta;
-      __syncthreads();
-      const float* hin = s_h[L.src + 1];
-      // dW[t'][k] += delta_t' h_k, db[t'] += delta_t'; d hin[k] += sum_t' W[t'][k] delta_t'
-      if (t < L.out && delta != 0.f) atomicAdd(&g_params[L.b + t], delta);
-      for (int tp = 0; tp < L.out; ++tp) {
-        const float dt = s_d[0][tp];
-        if (dt == 0.f) continue;
-        if (t < L.in) atomicAdd(&g_params[L.w + (size_t)tp * L.in + t], dt * hin[t]);
+      reinterpret_cast<float4*>(sGo)[tid] = go;
+    }
+    // ---- forward ----
+    for (int l = 0; l < net.n_layers; ++l) {
+      const BwdLayer L = net.L[l];
+      stage_weights(L);
+      const float* hin = sAct + (size_t)(L.src + 1) * kBR * 128;
+      float* hout = sAct + (size_t)(l + 1) * kBR * 128;
+      if (oc < L.out || L.out > 64) {
+        float sum[4][2];
+        const float b0 = oc < L.out ? params[L.b + oc] : 0.f, b1 = oc + 64 < L.out ? params[L.b + oc + 64] : 0.f;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) sum[r][0] = b0, sum[r][1] = b1;
+        const int in4 = (L.in + 3) & ~3;
+        for (int k = 0; k < in4; k += 4) {
+          const float4 w0 = *reinterpret_cast<const float4*>(sW + oc * kWS + k);
+          const float4 w1 = *reinterpret_cast<const float4*>(sW + (oc + 64) * kWS + k);
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float4 h = *reinterpret_cast<const float4*>(hin + (4 * rg + r) * 128 + k);
+            sum[r][0] = dot4(h, w0, sum[r][0]);
+            sum[r][1] = dot4(h, w1, sum[r][1]);
+          }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const int o = oc + 64 * j;
+            const float v = sum[r][j];
+            float y;
+            if (L.kind == K_HIDDEN) y = v > 0.f ? v : (net.activation == SSSGS_ACT_LEAKY_RELU ? net.slope * v : 0.f);
+            else if (L.kind == K_SSS) y = 1.f / (1.f + expf(-v));
+            else y = fmaxf(0.f, v);
+            hout[(4 * rg + r) * 128 + o] = o < L.out ? y : 0.f;
+          }
+      } else {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) hout[(4 * rg + r) * 128 + oc] = 0.f, hout[(4 * rg + r) * 128 + oc + 64] = 0.f;
       }
-      if (L.src >= 0 && t < L.in) {
-        float s = 0.f;
-        for (int tp = 0; tp < L.out; ++tp) s = fmaf(params[L.w + (size_t)tp * L.in + t], s_d[0][tp], s);
-        s_dacc[L.src + 1][t] += s;
-      }
+    }
+    __syncthreads();
+    for (int idx = tid; idx < kBR * 128; idx += 256) sGA[idx] = 0.f;
+    // ---- delta recursion, from the last layer down to the target ----
+    for (int l = net.n_layers - 1; l >= target; --l) {
+      const BwdLayer L = net.L[l];
+      const float* y = sAct + (size_t)(l + 1) * kBR * 128;
+      const float* gout = l <= trunk_last ? sGA : sGB;
       __syncthreads();
+      for (int idx = tid; idx < kBR * 128; idx += 256) {
+        const int r = idx >> 7, o = idx & 127;
+        float d = 0.f;
+        if (o < L.out) {
+          const float yy = y[idx];
+          if (L.kind == K_SSS) d = sGo[4 * r + o] * yy * (1.f - yy);
+          else if (L.kind == K_INC_OUT) d = yy > 0.f ? sGo[4 * r + 3] : 0.f;
+          else d = gout[idx] * (yy > 0.f ? 1.f : (net.activation == SSSGS_ACT_LEAKY_RELU ? net.slope : 0.f));
+        }
+        sD[idx] = d;
+      }
+      if (l == target) break;
+      if (L.src < 0) continue;
+      stage_weights(L);     // (syncs: sD is complete)
+      // gradient wrt the source layer's output: G[r][i] (+)= sum_o D[r][o] W[o][i]; thread: 4 rows x inputs 2 oc, 2 oc + 1
+      float* gdst = L.src <= trunk_last ? sGA : sGB;
+      const bool accumulate = L.src == trunk_last;      // both heads feed the last trunk layer
+      float s2[4][2];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) s2[r][0] = s2[r][1] = 0.f;
+      const int out4 = (L.out + 3) & ~3;
+      for (int o = 0; o < out4; o += 4) {
+        float4 d4[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) d4[r] = *reinterpret_cast<const float4*>(sD + (4 * rg + r) * 128 + o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float2 w = *reinterpret_cast<const float2*>(sW + (o + j) * kWS + 2 * oc);
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float d = j == 0 ? d4[r].x : j == 1 ? d4[r].y : j == 2 ? d4[r].z : d4[r].w;
+            s2[r][0] = fmaf(d, w.x, s2[r][0]);
+            s2[r][1] = fmaf(d, w.y, s2[r][1]);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        float2* dst = reinterpret_cast<float2*>(gdst + (4 * rg + r) * 128 + 2 * oc);
+        float2 v = make_float2(s2[r][0], s2[r][1]);
+        if (accumulate) { const float2 old = *dst; v.x += old.x; v.y += old.y; }
+        *dst = v;
+      }
+    }
+    __syncthreads();
+    // ---- dW[o][i] += sum_r D[r][o] h[r][i],  db[o] += sum_r D[r][o] ----
+    const float* hsrc = sAct + (size_t)(T.src + 1) * kBR * 128;
+#pragma unroll 2
+    for (int r = 0; r < kBR; ++r) {
+      const float4 d0 = *reinterpret_cast<const float4*>(sD + r * 128 + 4 * to);
+      const float4 d1 = *reinterpret_cast<const float4*>(sD + r * 128 + 64 + 4 * to);
+      const float4 h0 = *reinterpret_cast<const float4*>(hsrc + r * 128 + 4 * ti);
+      const float4 h1 = *reinterpret_cast<const float4*>(hsrc + r * 128 + 64 + 4 * ti);
+      const float dd[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+      const float hh[8] = {h0.x, h0.y, h0.z, h0.w, h1.x, h1.y, h1.z, h1.w};
+#pragma unroll
+      for (int a = 0; a < 8; ++a) {
+        accb[a] += dd[a];
+#pragma unroll
+        for (int b = 0; b < 8; ++b) acc[a][b] = fmaf(dd[a], hh[b], acc[a][b]);
+      }
+    }
+  }
+  if (!any) return;
+#pragma unroll
+  for (int a = 0; a < 8; ++a) {
+    const int o = (a < 4 ? 0 : 60) + 4 * to + a;      // a >= 4: 64 + 4 to + (a - 4)
+    if (o >= T.out) continue;
+    if (ti == 0) atomicAdd(&g_params[T.b + o], accb[a]);
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+      const int i = (b < 4 ? 0 : 60) + 4 * ti + b;
+      if (i < T.in && acc[a][b] != 0.f) atomicAdd(&g_params[T.w + (size_t)o * T.in + i], acc[a][b]);
     }
   }
 }
@@ -504,7 +645,8 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
 }
 
 int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
-                        int n_lights, int light0, const float* g_mlp_out, float* g_params, int num_sms, cudaStream_t s) {
+                        int n_lights, const float* g_mlp_out, float* g_params, uint32_t* row_list, uint32_t* row_count,
+                        int num_sms, cudaStream_t s) {
   if (g.n == 0 || n_lights == 0 || !g_params) return 0;
   BwdNet net;
   net.in_dim = mlp.in_dim;
@@ -519,6 +661,7 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
     ++nl;
   }
   const int trunk_last = nl - 1;
+  net.trunk_last = trunk_last;
   net.L[nl] = BwdLayer{off, off + 3 * d, 3, d, trunk_last, K_SSS};
   off += 3 * d + 3;
   ++nl;
@@ -535,10 +678,17 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
   ++nl;
   net.n_layers = nl;
   const int64_t rows = g.n * n_lights;
-  int64_t blocks = rows < (int64_t)num_sms * 8 ? rows : (int64_t)num_sms * 8;
-  mlp_backward_kernel<<<(unsigned)blocks, 128, 0, s>>>(g, net, (const float*)mlp.params, cam, lights, n_lights, light0,
-                                                        g_mlp_out, g.n, g_params);
-  return 1;
+  if (cudaMemsetAsync(row_count, 0, 4, s) != cudaSuccess) return 0;
+  int64_t cb = (rows + 255) / 256;
+  if (cb > (int64_t)num_sms * 8) cb = (int64_t)num_sms * 8;
+  bwd_rows_kernel<<<(unsigned)cb, 256, 0, s>>>(reinterpret_cast<const float4*>(g_mlp_out), rows, row_list, row_count);
+  const int smem = (128 * kWS + 3 * kBR * 128 + kBR * 4 + (nl + 1) * kBR * 128) * 4;
+  if (ensure_dyn_smem((const void*)mlp_backward_kernel, smem) != cudaSuccess) return 1;
+  int gx = num_sms / nl;
+  if (gx < 1) gx = 1;
+  mlp_backward_kernel<<<dim3((unsigned)gx, (unsigned)nl), 256, smem, s>>>(g, net, (const float*)mlp.params, cam, lights, g.n,
+                                                                        row_list, row_count, g_mlp_out, g_params);
+  return 2;
 }
 
 }  // namespace sssgs

@@ -786,8 +786,8 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
                                           gr->grad_conic, gr->grad_depth, gr->grad_attr,
                                           gr->grad_mlp_out + (int64_t)l0 * n * 4, n, s);
     if (run_mlp && gr->grad_params)
-      launches += launch_mlp_backward(*g, *mlp, cam, lb, nl, 0, gr->grad_mlp_out + (int64_t)l0 * n * 4, gr->grad_params,
-                                      c->num_sms, s);
+      launches += launch_mlp_backward(*g, *mlp, cam, lb, nl, gr->grad_mlp_out + (int64_t)l0 * n * 4, gr->grad_params,
+                                      reinterpret_cast<uint32_t*>(c->mlp_out[1]), cnt + DC_BWD_ROWS, c->num_sms, s);
   }
   c->launches = launches;
   const cudaError_t e = cudaGetLastError();
