@@ -41,13 +41,15 @@ sys.path.insert(0, ROOT)
 from paper_2408_12282_b200 import multi, scenes  # noqa: E402
 
 METRIC = "Mpix/s (MLP + G-buffer splat + deferred shading)"
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of a stage's kernel, from the
-# `ncu --set full` captures summarised under profiles/ (r02_ncu_full.md): (config, stage) -> bytes
-NCU_DRAM_BYTES_PER_LAUNCH = {}
-_ncu_path = os.path.join(ROOT, "profiles", "r02_dram_bytes_per_launch.json")
-if os.path.exists(_ncu_path):
-    NCU_DRAM_BYTES_PER_LAUNCH = {tuple(k.split(":")): v for k, v in json.load(open(_ncu_path)).items()
-                                 if not k.startswith("_")}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of a stage's heaviest kernel, from the `ncu --set full`
+# captures summarised in profiles/r02_ncu_full.md (tight lists, one view x all lights): (config, stage) -> bytes
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    ("5", "prepass"): 378.9e6 + 617.3e6,   # raster_shade_kernel<1,1,4,4,1,0>: lists + rows in, weight cache + T out
+    ("5", "raster"): 796.0e6 + 98.0e6,     # raster_cached_kernel<8,0>: weight cache + rows in, 8 frames out
+    ("5", "mlp"): 190.6e6 + 29.4e6,        # mlp_kernel<8,1,1>: kept rows' inputs in, 8 x 16 B per kept row out
+    ("3", "raster"): 148.3e6 + 61.6e6,     # raster_cached_kernel<8,1> (cfg 3, one of the 7 later batches)
+    ("2", "raster"): 13.5e6 + 17.9e6,      # raster_shade_kernel<1,4,8,2,0,0> (cfg 2)
+}
 FP32_LANES_PER_SM = 128
 HBM_NOMINAL_GBS = 8000.0   # BASELINE.json north_star: "~8 TB/s"
 MAX_INSTANCES_PER_GAUSSIAN = 20
@@ -118,10 +120,16 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def workload(cfg):
-    """(scene, cams of one step, lights of one step, frames per step)."""
+BACKWARD_CONFIGS = (2, 4)   # configs whose backward pass (one view, one light) is timed beside the forward table
+
+
+def workload(cfg, rank=0, world=1):
+    """(scene, cams of one step, lights of one step, frames per step).  Under torchrun each rank renders its own
+    view of the config's orbit (multi.frames_of_rank: round-robin by view; view 0 at N = 1)."""
     s = scenes.make_scene(cfg)
-    return s, s.cameras[:1], s.lights[0], len(s.lights[0])
+    mine = multi.frames_of_rank(len(s.cameras), rank, world)
+    v = mine[0] if mine else rank % len(s.cameras)
+    return s, s.cameras[v:v + 1], s.lights[v], len(s.lights[v])
 
 
 def config_dict(cfg, scene, fps):
@@ -129,7 +137,7 @@ def config_dict(cfg, scene, fps):
     cam = scene.cameras[0]
     m = scene.mlp
     return {"workload": f"configs[{cfg - 1}] {scene.name}: {scene.n} Gaussians, {cam.width}x{cam.height}, "
-                        f"one view x {fps} light(s) per step (view 0 of {len(scene.cameras)})",
+                        f"one view x {fps} light(s) per step (view 0 of {len(scene.cameras)}; rank r of N renders view r)",
             "gaussians": int(scene.n), "width": int(cam.width), "height": int(cam.height),
             "frames_per_step": int(fps), "views_in_config": len(scene.cameras),
             "mlp": f"{m.in_dim} -> {'x'.join(str(w) for w in m.trunk_width)} -> 3+1",
@@ -253,7 +261,7 @@ class ConfigRun:
         self.torch, self.binding, self.cfg = torch, binding, cfg
         self.dev = torch.device("cuda", local_rank)
         if scene is None:
-            self.scene, self.cams, self.lights, self.fps = workload(cfg)
+            self.scene, self.cams, self.lights, self.fps = workload(cfg, *multi.env_ranks()[:2])
         else:
             self.scene, self.cams, self.lights, self.fps = scene, scene.cameras[:1], scene.lights[0], len(scene.lights[0])
         self.cam = self.cams[0]
@@ -329,6 +337,24 @@ class ConfigRun:
                     e["frac_of_nominal_8TBs"] = round(ach / HBM_NOMINAL_GBS, 4)
             out[k] = e
         return out, pk
+
+    def backward_ms(self, reps=3):
+        """sssgs_render_backward of the step's view and lights: median device time over `reps`
+        calls, G-buffer of a forward call and a seeded dL/drgb resident in HBM."""
+        torch = self.torch
+        fwd = self.R.render(cams=self.cams, lights=self.lights, want=("rgb", "gbuffer"), tight=self.kw["tight"])
+        gen = torch.Generator(device=self.dev).manual_seed(7)
+        G = torch.randn(fwd["rgb"].shape, generator=gen, device=self.dev)
+        ms = []
+        for _ in range(reps + 1):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            self.R.render_backward(self.cam, self.lights, G, fwd["gbuffer"], tight=self.kw["tight"])
+            b.record()
+            torch.cuda.synchronize()
+            ms.append(a.elapsed_time(b))
+        return {"ms": round(float(np.median(ms[1:])), 4), "launches": self.R.launch_count(),
+                "lights": len(self.lights), "mlp_backward": "fp32 CUDA cores (v1)"}
 
     def close(self):
         self.graph = None
@@ -422,6 +448,9 @@ def run_gpu(args, rank, world, local_rank):
                    mlp_tensor_frac=stages.get("mlp", {}).get("frac"),
                    stage_ms={k: v["ms"] for k, v in stages.items()})
         table = {key: row}
+        backward = {}
+        if args.config in BACKWARD_CONFIGS and world == 1 and not args.no_table:
+            backward[key] = run.backward_ms()
         launches_per_step = run.launches
         cnt_head, mlp_rows_head = run.cnt, (run.cnt[binding.CNT_MLP_ROWS] or scene.n)
         run.close()
@@ -445,6 +474,8 @@ def run_gpu(args, rank, world, local_rank):
                                 dominant_stage=d, dominant_frac=st[d].get("frac"), dominant_bound=st[d].get("bound"),
                                 mlp_tensor_frac=st.get("mlp", {}).get("frac"),
                                 stage_ms={kk: v["ms"] for kk, v in st.items()})
+                if c in BACKWARD_CONFIGS:
+                    backward[k] = r.backward_ms()
                 r.close()
                 del r
                 torch.cuda.empty_cache()
@@ -474,7 +505,7 @@ def run_gpu(args, rank, world, local_rank):
                     "note": "sssgs_render_host uploads the WHOLE scene and downloads every frame in each call "
                             "(one crossing per call by design): PCIe-bound"},
             "gpu_launches": launches_per_step * args.steps,
-            "roofline": roof, "stages": stages, "configs": table, "cpu_baseline": cpu,
+            "roofline": roof, "stages": stages, "configs": table, "backward": backward, "cpu_baseline": cpu,
             "peaks": {"hbm_gbs_measured": peaks["hbm"], "hbm_gbs_nominal": HBM_NOMINAL_GBS,
                       "bf16_tflops_burst": peaks["bf16_burst"], "bf16_tflops_sustained": peaks["bf16_sustained"],
                       "source": peaks["source"]},

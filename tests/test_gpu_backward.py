@@ -99,9 +99,9 @@ def test_walks_backward_given_mlp_outputs(n, w, h, lights, tight):
     out = _gpu(s, G, precomputed=mo32, tight=tight)
     assert out["launches"] > 0
     np.testing.assert_allclose(out["gbuffer"][:, ~comp.unstable], r.gbuf[:, ~comp.unstable], rtol=0, atol=1e-4)
-    # fp32 products and sums of up to a few hundred terms per pixel and a few thousand per Gaussian: 2e-4 of the
+    # fp32 products and sums of up to a few hundred terms per pixel and a few thousand per Gaussian: 5e-5 of the
     # largest gradient (DESIGN 7e derives it; measured values are printed)
-    _check_all(out, r, s, 2e-4, f"walks n={n} {w}x{h} L={lights}:")
+    _check_all(out, r, s, 5e-5, f"walks n={n} {w}x{h} L={lights}:")
     assert not out["grad_params"].any()         # outputs were given: no parameter gradient
 
 
@@ -122,7 +122,7 @@ def test_mlp_backward_alone():
     print(f"MLP backward alone: {e:.2e} of max |dL/dTheta| = {np.abs(ref).max():.3e}")
     # fp32 forward re-evaluation + fp32 atomics over ~10^3 rows; a ReLU decided differently in fp32 than in
     # float64 (pre-activation within rounding of 0) moves one row's contribution of one unit
-    assert e <= 5e-4
+    assert e <= 5e-5
 
 
 @pytest.mark.parametrize("cfg", [3, 6])
@@ -136,11 +136,11 @@ def test_whole_chain_backward(cfg):
     out = _gpu(s, G)
     # the forward MLP outputs the walks read are the fp16-operand kernel's (<= 1e-2 from float64, north_star):
     # they enter dL/dgbuffer through the shaded L_SSS / L_in channels and every upstream gradient through the
-    # suffix sums, linearly: a few 1e-2 of the largest gradient
-    _check_all(out, r, s, 3e-2, f"chain cfg {cfg}:")
+    # suffix sums, linearly: measured <= 1.5e-3 of the largest gradient, bar 5e-3 (DESIGN 6)
+    _check_all(out, r, s, 5e-3, f"chain cfg {cfg}:")
     e = _rel(out["grad_params"], r.d_params)
     print(f"chain cfg {cfg}: grad_params {e:.2e}")
-    assert e <= 3e-2
+    assert e <= 5e-3
 
 
 def test_backward_rejects_bad_arguments():
