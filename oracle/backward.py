@@ -51,20 +51,29 @@ def mlp_layers(mlp, params: torch.Tensor):
     return out
 
 
-def mlp_torch(x: torch.Tensor, mlp, params: torch.Tensor) -> torch.Tensor:
-    """x [n, in_dim] -> [n, 4] = (sigmoid SSS head (3), relu incident head (1))."""
+def mlp_torch(x: torch.Tensor, mlp, params: torch.Tensor, mode: int = 0) -> torch.Tensor:
+    """x [n, in_dim] -> [n, 4] = (sigmoid SSS head (3), relu incident head (1)).
+    mode 0: float64.  mode 2: the binary16-operand arithmetic of oracle.mlp_forward(mode 2) (weights rounded once,
+    every layer input rounded to binary16, float64 accumulation), the rounding treated as the identity by the
+    differentiation (straight-through): the ReLU decisions are then taken in the kernel's precision, which is
+    what the tensor-core backward differentiates."""
+    if mode == 0:
+        rnd = lambda t: t  # noqa: E731
+    else:
+        rnd = lambda t: t + (t.to(torch.float16).to(F8) - t).detach()  # noqa: E731
     act = (lambda t: torch.where(t > 0, t, mlp.leaky_slope * t)) if mlp.activation == 1 else torch.relu
     h, hi, sss, inc = x, None, None, None
     for W, b, kind in mlp_layers(mlp, params):
+        W = rnd(W)
         if kind == "trunk":
-            h = act(h @ W.T + b)
+            h = act(rnd(h) @ W.T + b)
         elif kind == "sss":
-            sss = torch.sigmoid(h @ W.T + b)
+            sss = torch.sigmoid(rnd(h) @ W.T + b)
             hi = h
         elif kind == "inc_hidden":
-            hi = act(hi @ W.T + b)
+            hi = act(rnd(hi) @ W.T + b)
         else:
-            inc = torch.relu(hi @ W.T + b)
+            inc = torch.relu(rnd(hi) @ W.T + b)
     return torch.cat([sss, inc], dim=1)
 
 

@@ -7,7 +7,9 @@ every BASELINE config at full size.  They are the denominators of bench.py's roo
   p_eval     list entries a per-pixel walker visits, up to and including the entry it stops at (step 5)
   p_blend    blended (pixel, entry) pairs
   g_contrib  Gaussians blended at >= 1 pixel (the rows an MLP-skipping sweep must still evaluate)
-  tight      instances of the tightest valid list ((tile, i) with alpha >= 1/255 at some pixel)
+  unstable_pixels  pixels with a decision inside the margin of a threshold (S7)
+(The size of the minimal S5 list is not stored: oracle.tile_hits is brute force over every pixel of every listed
+tile, which the full-size tests run on 256 sampled tiles per view instead.)
 
 Calls only oracle/ and the seeded input generators; no value comes from the CUDA path.
 

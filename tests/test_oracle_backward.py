@@ -165,3 +165,62 @@ def test_closed_forms_on_a_pixel_centre():
         # on the centre the exponent is stationary: no gradient to the 2-D mean or the conic from this pixel
         # (the fp32 projection puts the centre within ~1e-5 px of the pixel centre, hence the tolerances)
         assert np.abs(r.d_pix).max() < 1e-3 and np.abs(r.d_conic).max() < 1e-8
+
+
+def test_fp16_emulating_restatement():
+    """mode 2 of mlp_torch: forward == the C++ oracle's binary16-emulating mode; its gradient (rounding = identity)
+    equals the float64 network's wherever the two take the same ReLU decisions, up to the 2^-11 operand rounding."""
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    x = ob._t(xs[0])
+    y2 = ob.mlp_torch(x, s.mlp, ob._t(s.mlp.params), mode=2).numpy()
+    np.testing.assert_allclose(y2, oracle.mlp_forward(xs[0], s.mlp, 2), rtol=1e-12, atol=1e-13)
+    assert np.abs(y2 - oracle.mlp_forward(xs[0], s.mlp, 0)).max() > 1e-6      # it does round
+    s6 = scenes.make_scene(6, n=50)
+    x6 = oracle.mlp_inputs(s6, s6.cameras[0], s6.lights[0][0].position)
+    np.testing.assert_allclose(ob.mlp_torch(ob._t(x6), s6.mlp, ob._t(s6.mlp.params), mode=2).numpy(),
+                               oracle.mlp_forward(x6, s6.mlp, 2), rtol=1e-12, atol=1e-13)
+    # gradient: one row at a time; rows whose hidden pre-activations all stay clear of 0 take the same decisions
+    rng = np.random.default_rng(3)
+    go = ob._t(rng.standard_normal((len(xs[0]), 4)))
+    grads = []
+    for mode in (0, 2):
+        p = ob._t(s.mlp.params).requires_grad_(True)
+        (ob.mlp_torch(x, s.mlp, p, mode=mode) * go).sum().backward()
+        grads.append(p.grad.numpy())
+    rel = np.abs(grads[1] - grads[0]).max() / np.abs(grads[0]).max()
+    assert 0 < rel < 5e-2        # close (a few flipped decisions among 400 x 384 units), not identical
+    # a one-row case with every pre-activation far from 0: decisions agree, the difference is rounding only
+    w = np.abs(oracle.mlp_forward(xs[0], s.mlp, 0) - oracle.mlp_forward(xs[0], s.mlp, 2)).max(axis=1)
+    r = int(np.argmin(w))
+    g1 = []
+    for mode in (0, 2):
+        p = ob._t(s.mlp.params).requires_grad_(True)
+        (ob.mlp_torch(x[r:r + 1], s.mlp, p, mode=mode) * go[r:r + 1]).sum().backward()
+        g1.append(p.grad.numpy())
+    same = (g1[0] != 0) == (g1[1] != 0)
+    if same.all():
+        assert np.abs(g1[1] - g1[0]).max() <= 5e-3 * np.abs(g1[0]).max()
+
+
+def test_fp16_emulation_decides_in_the_rounded_arithmetic():
+    """Hand-made one-unit net: x = 1 + 2^-12 rounds to 1 in binary16; with W = 1, b = -(1 + 2^-13) (kept in fp32)
+    the float64 pre-activation is +2^-13 (ReLU on: dL/dW = x dL/dh) and the emulated one is -2^-13 (off: 0)."""
+    x = ob._t(np.array([[1.0 + 2.0 ** -12]]))
+    b0 = -(1.0 + 2.0 ** -13)
+    params = np.array([1.0, b0,  1.0, 0.0, 0.0,  0.0, 0.0, 0.0,  2.0,  0.5], np.float64)   # trunk, sss 3x1 + b, inc 1x1 + b
+    mlp = scenes.MlpSpec(in_dim=1, trunk_width=[1], inc_hidden_width=[], activation=0, leaky_slope=0.01,
+                         params=params.astype(np.float32))
+    assert float(np.float32(b0)) == b0
+    got = {}
+    for mode in (0, 2):
+        p = ob._t(params).requires_grad_(True)
+        y = ob.mlp_torch(x, mlp, p, mode=mode)
+        y[0, 3].backward()          # incident head: relu(2 h + 0.5)
+        got[mode] = (y.detach().numpy()[0], p.grad.numpy())
+    h0 = 2.0 ** -13
+    np.testing.assert_allclose(got[0][0][3], 2 * h0 + 0.5, rtol=1e-14)
+    np.testing.assert_allclose(got[0][1][0], 2.0 * (1.0 + 2.0 ** -12), rtol=1e-14)   # dL/dW0 = w_inc * x
+    np.testing.assert_allclose(got[0][1][8], h0, rtol=1e-12)                            # dL/dw_inc = h
+    assert got[2][0][3] == 0.5 and got[2][1][0] == 0.0 and got[2][1][1] == 0.0 and got[2][1][8] == 0.0
+    assert got[2][1][9] == 1.0
