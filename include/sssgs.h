@@ -76,12 +76,15 @@ enum {
                                   order of the per-slot partial sums (last bits) on smaller ones; sorted_keys /
                                   sorted_vals / tile_ranges / SSSGS_CNT_INSTANCES then describe the tight
                                   list.  ~0.6-0.75 x the instances: less to emit, sort and walk.        */
-  SSSGS_FORWARD_SHADING = 4u   /* the "w/o deferred" variant of the paper's ablation (PAPER.md L283
+  SSSGS_FORWARD_SHADING = 4u,  /* the "w/o deferred" variant of the paper's ablation (PAPER.md L283
                                   Tab. 2, Fig. 5): Eq. 7 is evaluated per Gaussian (at its
                                   centre, with its own normal and material) and the RGB values are
                                   composited (Eq. 3): out.rgb = sum_i T_i alpha_i c_i + (1 - A) bg.
                                   gbuffer and the AOVs must be NULL; not combinable with
                                   SSSGS_SUM_LIGHTS.                                            */
+  SSSGS_BACKWARD_FP32 = 16u    /* sssgs_render_backward only: run the MLP backward in fp32 on the CUDA
+                                  cores instead of the tensor cores (slower; the reference path of the
+                                  parity tests, and what MLPs with incident-head hidden layers use).  */
 };
 
 /* indices into sssgs_out.counters (int64 each, per camera: counters[cam*SSSGS_NCOUNTERS + k]) */
@@ -267,8 +270,11 @@ int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_
  * All pointers are DEVICE pointers, 16-byte aligned, fp32; every gradient array is overwritten.
  * gbuffer must be the G-buffer sssgs_render wrote for the same scene, camera and lights.
  * mlp.dtype must be SSSGS_F32 (mlp.precomputed_out, if given, is used for the forward values and
- * grad_params is then left zero).  Arithmetic is fp32; the MLP is re-evaluated in fp32 (not in the
- * 16-bit operand precision of the forward kernel).  Per-Gaussian sums use float atomics: results are
+ * grad_params is then left zero).  Shading and compositing backward are fp32.  The MLP backward runs on the
+ * tensor cores (binary16 operands, fp32 accumulation: the forward pass of the listed rows is re-evaluated with
+ * the forward kernel's arithmetic; dL/d(mlp_out) is scaled by a power of two so that the deltas fit binary16)
+ * when the MLP has no incident-head hidden layers and at most 4 trunk layers; otherwise, or with
+ * SSSGS_BACKWARD_FP32, in fp32 on the CUDA cores (forward re-evaluated in fp32).  Per-Gaussian sums use float atomics: results are
  * reproducible to rounding, not bit for bit.  Enqueues on the stream, never synchronises.
  * With n_light = 0 (or n = 0) the per-Gaussian and parameter gradients are zeroed and the per-light
  * pointers are not read.  Errors: SSSGS_EINVAL (NULL / misaligned / dtype), SSSGS_ECAPACITY (n, image size). */

@@ -186,11 +186,12 @@ def shade_torch(cam, light_pos, light_intensity, gbuf: torch.Tensor) -> torch.Te
 # The gradients
 # ---------------------------------------------------------------------------------------------------
 def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16,
-                    given_mlp_out=None):
+                    given_mlp_out=None, mlp_mode: int = 0):
     """Gradients of L = sum_l <grad_rgb[l], rgb_l> for one view.
 
     proj / vals / ranges: the oracle's projection and tile lists of the view (oracle.project / build_lists);
     mlp_inputs: [L][n, in_dim] float64 (oracle.mlp_inputs per light); grad_rgb [L, H, W, 3].
+    mlp_mode: 0 float64 MLP, 2 its binary16-emulating restatement (mlp_torch).
     given_mlp_out: [L, n, 4] or None: the MLP outputs are these constants instead of mlp(mlp_inputs) (isolates
     the walks: d_params is then zero).
     Returns a namespace of numpy float64 arrays:
@@ -218,7 +219,7 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
     loss = torch.zeros((), dtype=F8)
     for li, lt in enumerate(lights):
         if given_mlp_out is None:
-            mo = mlp_torch(_t(mlp_inputs[li]), scene.mlp, params)
+            mo = mlp_torch(_t(mlp_inputs[li]), scene.mlp, params, mode=mlp_mode)
         else:
             mo = _t(given_mlp_out[li]).clone().requires_grad_(True)
         mo.retain_grad()

@@ -27,6 +27,7 @@ SSSGS_LIGHTS_PER_CAMERA = 1
 SSSGS_SUM_LIGHTS = 2
 SSSGS_FORWARD_SHADING = 4
 SSSGS_TIGHT_LISTS = 8
+SSSGS_BACKWARD_FP32 = 16
 SSSGS_F32, SSSGS_BF16 = 0, 1
 SSSGS_COMPUTE_FP16, SSSGS_COMPUTE_BF16 = 0, 1
 (SSSGS_OK, SSSGS_EINVAL, SSSGS_ECAPACITY, SSSGS_ECUDA, SSSGS_EARCH, SSSGS_EOVERFLOW) = (0, -1, -2, -3, -4, -5)
@@ -338,7 +339,7 @@ class Renderer:
                      (SSSGS_FORWARD_SHADING if forward else 0) | (SSSGS_TIGHT_LISTS if tight else 0), st)
         return outputs
 
-    def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None):
+    def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None, fp32=False):
         """Enqueue one sssgs_render_backward: cam one scene camera, lights its lights, grad_rgb [L,H,W,3] and
         gbuffer [L,H,W,16] device tensors (the forward call's G-buffer).  Returns the dict of gradient tensors."""
         torch = self.torch
@@ -359,7 +360,8 @@ class Renderer:
             pre_ptr = precomputed.data_ptr()
         m = make_mlp(self.scene.mlp, self.params.data_ptr(), self.params.numel() * 4, SSSGS_F32, pre_ptr, self.compute)
         st = stream if stream is not None else torch.cuda.current_stream(self.device).cuda_stream
-        sssgs_render_backward(self.ctx, self.g, m, make_camera(cam), larr, L, gr, SSSGS_TIGHT_LISTS if tight else 0, st)
+        sssgs_render_backward(self.ctx, self.g, m, make_camera(cam), larr, L, gr,
+                              (SSSGS_TIGHT_LISTS if tight else 0) | (SSSGS_BACKWARD_FP32 if fp32 else 0), st)
         return out
 
     def bake_visibility(self, dirs, weights, t_min: float, sh_degree: int = 1, want_vis: bool = False, stream=None,

@@ -152,6 +152,7 @@ enum {
   DC_WC_CHUNKS = 26,     // weight cache: chunks handed out
   DC_WC_OVERFLOW = 27,   // weight cache: 1 if the pool ran out (the sweep then walks the lists again)
   DC_BWD_ROWS = 28,      // backward: rows of the light batch with a non-zero dL/d(mlp_out)
+  DC_BWD_GOMAX = 29,     // backward: bits of the largest |dL/d(mlp_out)| of the light batch (follows DC_BWD_ROWS)
   DC_BVH_BOUNDS = 32,    // 6 words: box of the centres (sssgs_bake_visibility)
   DC_BUCKET_STARTS = 64, // 32 words: tiles with a list of at least 2^k entries, k = 0..31 (raster work order)
   DC_WORDS = 96
@@ -305,9 +306,11 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
                               const float4* attr, const float4* mlp_out, int mlp_stride, const float* grad_gbuf,
                               float* g_opacity, float* g_mean2d, float* g_conic, float* g_depth, float* g_attr,
                               float* g_mlp_out, int64_t n, cudaStream_t s);
+// row_count: two control words (rows listed, bits of max |dL/d(mlp_out)|); blob: kBwdBlobBytes, packed when `pack`
+constexpr size_t kBwdBlobBytes = 4 * 32768 + 4096 + 5 * 512;
 int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
                         int n_lights, const float* g_mlp_out, float* g_params, uint32_t* row_list, uint32_t* row_count,
-                        int num_sms, cudaStream_t s);
+                        uint8_t* blob, bool pack, bool force_fp32, int num_sms, cudaStream_t s);
 
 int mlp_smem_bytes(const MlpPlan& plan);
 

@@ -13,6 +13,10 @@
 // re-evaluated in fp32 from the caller's parameters (this first version runs on the CUDA cores: the
 // tensor-core forward keeps no activations, DESIGN.md section 7e says what a tcgen05 version needs).
 // Per-Gaussian sums are formed with float atomics: results are reproducible to rounding, not bit for bit.
+#include <cuda_fp16.h>
+
+#include <cstring>
+
 #include "internal.cuh"
 
 namespace sssgs {
@@ -397,13 +401,19 @@ constexpr int kWS = 132;   // row stride of the staged weight matrix (floats): 1
 // rows of a large scene), compacted into a list; order is arbitrary (the sums below are atomics anyway).
 __global__ void __launch_bounds__(256)
 bwd_rows_kernel(const float4* __restrict__ g_mlp_out, int64_t total, uint32_t* __restrict__ list, uint32_t* __restrict__ count) {
+  // count[0] = rows listed, count[1] = bits of the largest |dL/d(mlp_out)| (non-negative floats order as integers)
   for (int64_t base = (int64_t)blockIdx.x * 256; base < total; base += (int64_t)gridDim.x * 256) {
     const int64_t idx = base + threadIdx.x;
     bool on = false;
+    uint32_t mx = 0u;
     if (idx < total) {
       const float4 v = g_mlp_out[idx];
       on = v.x != 0.f || v.y != 0.f || v.z != 0.f || v.w != 0.f;
+      mx = __float_as_uint(fmaxf(fmaxf(fabsf(v.x), fabsf(v.y)), fmaxf(fabsf(v.z), fabsf(v.w))));
+      if (mx >= 0x7F800000u) mx = 0u;   // inf / NaN do not set the scale
     }
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0 && mx > 0u) atomicMax(count + 1, mx);
     const unsigned m = __ballot_sync(0xffffffffu, on);
     const int lane = threadIdx.x & 31;
     unsigned at = 0;
@@ -603,6 +613,415 @@ mlp_backward_kernel(sssgs_gaussians g, BwdNet net, const float* __restrict__ par
   }
 }
 
+// ---- a2 backward on the tensor cores (tcgen05) -------------------------------------------------------
+// For MLPs without incident-head hidden layers (every BASELINE config).  Per tile of 128 listed rows, a CTA
+// recomputes the forward pass with the forward kernel's arithmetic (binary16 operands, fp32 accumulators in
+// tensor memory, A operand from tensor memory), runs the delta recursion  G_{l-1} = delta_l W_l  as
+// tcgen05.mma with the SAME shared-memory weight tile read MN-major (B[n][k] = W_l[k][n]: no transposed
+// copy), and accumulates the weight gradient of ONE layer (blockIdx.y)  dW_t += delta_t^T h_{t-1}  over all
+// of its tiles in 128 tensor-memory columns, both operands MN-major from shared memory (the 128 rows of the
+// tile are the K dimension).  dL/d(mlp_out) is scaled by a power of two (largest magnitude of the batch in
+// (0.5, 1]) so that the deltas fit binary16; the sums are un-scaled when they leave tensor memory.
+namespace tc {
+
+constexpr int kRowsT = 128;            // rows per tile = UMMA M (forward, recursion) = UMMA K (weight gradient)
+constexpr int kTileBytes = 32768;      // one [128][128] 16-bit operand tile: two 64-column blocks of 16 KB
+constexpr int kHeadTileBytes = 4096;   // head weights: [2 blocks][16 rows][128 B]
+constexpr uint32_t kColDW = 0, kColD = 128, kColA = 256, kColAH = 320;   // tensor-memory columns
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {
+  }
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* w) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+               "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
+  uint32_t r[16];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    asm volatile("" : "+r"(r[i]));
+    v[i] = __uint_as_float(r[i]);
+  }
+}
+__device__ __forceinline__ uint32_t pack_f16(float a, float b) {   // .lo = a, .hi = b, RNE, saturating
+  uint32_t d;
+  asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(b), "f"(a));
+  return d;
+}
+__device__ __forceinline__ uint32_t elect_one() {
+  uint32_t e;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(e));
+  return e;
+}
+// Shared-memory operand descriptor, 128-byte swizzle, version 1.  K-major: rows of 128 B, 8-row groups `sbo`
+// bytes apart (lbo unused).  MN-major: 64 MN elements contiguous (128 B) per K row, 8 K rows per 1024-byte atom,
+// atoms `sbo` apart along K and `lbo` apart along MN.
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr >> 4) & 0x3FFFu);
+  d |= (uint64_t)((lbo >> 4) & 0x3FFFu) << 16;
+  d |= (uint64_t)((sbo >> 4) & 0x3FFFu) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+// D = F32, A = B = F16, M = 128, N = n; a_mn / b_mn: operand is MN-major
+__device__ __forceinline__ uint32_t make_idesc(int n, bool a_mn, bool b_mn) {
+  return (1u << 4) | ((a_mn ? 1u : 0u) << 15) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) |
+         ((uint32_t)(kRowsT >> 4) << 24);
+}
+// The whole issuing warp runs these with warp-uniform operands; the instruction is predicated on one lane.
+__device__ __forceinline__ void umma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc, uint32_t acc,
+                                        uint32_t issue) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "setp.ne.u32 p, %4, 0;\n\t"
+      "setp.ne.u32 q, %5, 0;\n\t"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(acc), "r"(issue) : "memory");
+}
+__device__ __forceinline__ void umma_ss(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t acc,
+                                        uint32_t issue) {
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "setp.ne.u32 p, %4, 0;\n\t"
+      "setp.ne.u32 q, %5, 0;\n\t"
+      "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(acc), "r"(issue) : "memory");
+}
+__device__ __forceinline__ void umma_commit_if(uint32_t bar, uint32_t issue) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\t"
+      "setp.ne.u32 q, %1, 0;\n\t"
+      "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}"
+      ::"r"(bar), "r"(issue) : "memory");
+}
+// byte offset of element (row r, column c) of a [rows][128] 16-bit tile stored as two 64-column blocks
+// `block_bytes` apart, rows of 128 B, 128-byte swizzle (16-byte chunk index xor row % 8)
+__device__ __forceinline__ uint32_t tile_off(int r, int c, int block_bytes) {
+  return (uint32_t)((c >> 6) * block_bytes + r * 128 + ((((c & 63) >> 3) ^ (r & 7)) << 4) + (c & 7) * 2);
+}
+
+// Layer table of the tensor-core backward: layers 0 .. n_trunk - 1 = trunk, layer n_trunk = the two heads as one
+// 4-row layer (rows 0-2 SSS, row 3 incident light).
+struct TcNet {
+  int n_trunk, in_dim, k0_pad, activation;
+  float slope;
+  int out[SSSGS_MAX_TRUNK], in[SSSGS_MAX_TRUNK], w[SSSGS_MAX_TRUNK], b[SSSGS_MAX_TRUNK];   // caller's packing (floats)
+  int sss_w, sss_b, inc_w, inc_b, head_in;
+};
+
+// blob: trunk tiles (32 KB each, K-major = [out row][in column]), head tile (4 KB), then biases fp32 [n_trunk + 1][128]
+__global__ void __launch_bounds__(256)
+bwd_pack_kernel(TcNet net, const float* __restrict__ params, uint8_t* __restrict__ blob) {
+  const int L = net.n_trunk;
+  const int total = L * 128 * 128 + 16 * 128 + (L + 1) * 128;
+  for (int idx = blockIdx.x * 256 + threadIdx.x; idx < total; idx += gridDim.x * 256) {
+    if (idx < L * 128 * 128) {
+      const int l = idx >> 14, n = (idx >> 7) & 127, k = idx & 127;
+      const float v = (n < net.out[l] && k < net.in[l]) ? params[net.w[l] + n * net.in[l] + k] : 0.f;
+      *reinterpret_cast<__half*>(blob + (size_t)l * kTileBytes + tile_off(n, k, 16384)) = __float2half_rn(v);
+    } else if (idx < L * 128 * 128 + 16 * 128) {
+      const int j = idx - L * 128 * 128, n = j >> 7, k = j & 127;
+      float v = 0.f;
+      if (k < net.head_in) {
+        if (n < 3) v = params[net.sss_w + n * net.head_in + k];
+        else if (n == 3) v = params[net.inc_w + k];
+      }
+      *reinterpret_cast<__half*>(blob + (size_t)L * kTileBytes + tile_off(n, k, 2048)) = __float2half_rn(v);
+    } else {
+      const int j = idx - L * 128 * 128 - 16 * 128, l = j >> 7, n = j & 127;
+      float v = 0.f;
+      if (l < L) { if (n < net.out[l]) v = params[net.b[l] + n]; }
+      else if (n < 3) v = params[net.sss_b + n];
+      else if (n == 3) v = params[net.inc_b];
+      reinterpret_cast<float*>(blob + (size_t)L * kTileBytes + kHeadTileBytes)[j] = v;
+    }
+  }
+}
+
+struct TcArgs {
+  sssgs_gaussians g;
+  TcNet net;
+  CamParams cam;
+  LightBatch lights;
+  int64_t n;
+  const uint32_t* list;        // rows of the batch with a gradient (index = light * n + Gaussian)
+  const uint32_t* count;
+  const uint32_t* gomax_bits;  // bits of max |dL/d(mlp_out)| over the batch
+  const float* g_mlp_out;      // [n_lights][n][4]
+  const uint8_t* blob;         // bwd_pack_kernel's output
+  float* g_params;
+};
+
+__host__ __device__ inline int tc_smem_bytes(int n_trunk) {
+  return n_trunk * kTileBytes + kHeadTileBytes + 2 * kTileBytes + (n_trunk + 1) * 128 * 4 + 64 + 1024;
+}
+
+__global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_constant__ TcArgs a) {
+  extern __shared__ uint8_t tc_smem_raw[];
+  uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tc_smem_raw) + 1023) & ~(uintptr_t)1023);
+  const TcNet& net = a.net;
+  const int L = net.n_trunk;
+  uint8_t* sW = sm;
+  uint8_t* sDelta = sW + (size_t)L * kTileBytes + kHeadTileBytes;
+  uint8_t* sH = sDelta + kTileBytes;
+  float* sBias = reinterpret_cast<float*>(sH + kTileBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sBias + (L + 1) * 128);
+  uint32_t* s_tmem = reinterpret_cast<uint32_t*>(bars + 2);
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int t = blockIdx.y;                      // target layer: t < L trunk, t == L the heads
+  const uint32_t bar = smem_u32(bars);
+
+  // ---- set-up: weights and biases into shared memory, operand tiles zeroed, tensor memory --------------
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(a.blob);
+    uint4* dst = reinterpret_cast<uint4*>(sW);
+    const int nw = (L * kTileBytes + kHeadTileBytes) / 16;
+    for (int i = tid; i < nw; i += 128) dst[i] = src[i];
+    const float* bsrc = reinterpret_cast<const float*>(a.blob + (size_t)L * kTileBytes + kHeadTileBytes);
+    for (int i = tid; i < (L + 1) * 128; i += 128) sBias[i] = bsrc[i];
+    uint4* z = reinterpret_cast<uint4*>(sDelta);
+    for (int i = tid; i < 2 * kTileBytes / 16; i += 128) z[i] = make_uint4(0u, 0u, 0u, 0u);
+  }
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  fence_proxy_async();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = *s_tmem;
+  const uint32_t lane_off = (uint32_t)(warp * 32) << 16;
+  const uint32_t tD = tmem + kColD, tA = tmem + kColA, tAH = tmem + kColAH, tDW = tmem + kColDW;
+  const uint32_t sW_addr = smem_u32(sW), sDelta_addr = smem_u32(sDelta), sH_addr = smem_u32(sH);
+  uint32_t phase = 0;
+
+  const int k_t = t == 0 ? net.k0_pad : (t < L ? net.in[t] : net.head_in);   // K of the target layer (padded)
+  const uint32_t nrows = *a.count;
+  const uint32_t ntiles = (nrows + kRowsT - 1) / kRowsT;
+  // power-of-two scale: the largest |dL/d(mlp_out)| of the batch lands in (0.5, 1]
+  const uint32_t mbits = *a.gomax_bits;
+  int e = (int)(mbits >> 23) - 127;
+  e = e < -100 ? -100 : (e > 100 ? 100 : e);
+  const float scale = __uint_as_float((uint32_t)(126 - e) << 23), inv_scale = __uint_as_float((uint32_t)(128 + e) << 23);
+  const bool leaky = net.activation == SSSGS_ACT_LEAKY_RELU;
+  const float neg_slope = leaky ? net.slope : 0.f;
+  float db = 0.f;
+  uint32_t tiles_done = 0;
+
+  auto publish = [&]() {   // this thread's operand writes (tensor memory and shared memory) before the next MMAs
+    tmem_wait_st();
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  };
+  auto wait_mma = [&]() {
+    mbar_wait(bar, phase);
+    phase ^= 1u;
+    tc_fence_after();
+  };
+  // 16 consecutive 16-bit values of this thread's row (columns c0 .. c0 + 15) into a shared-memory operand tile
+  auto store_row16 = [&](uint8_t* tile, int c0, const uint32_t* w) {
+    *reinterpret_cast<uint4*>(tile + tile_off(tid, c0, 16384)) = make_uint4(w[0], w[1], w[2], w[3]);
+    *reinterpret_cast<uint4*>(tile + tile_off(tid, c0 + 8, 16384)) = make_uint4(w[4], w[5], w[6], w[7]);
+  };
+
+  for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    // ---- the rows of the tile: inputs (as the forward kernel assembles them) and upstream gradients ------
+    const uint32_t ridx = tile * kRowsT + tid;
+    float4 go = make_float4(0.f, 0.f, 0.f, 0.f);
+    float x[128];
+    for (int k = 0; k < net.k0_pad; ++k) x[k] = 0.f;
+    if (ridx < nrows) {
+      const uint32_t idx = a.list[ridx];
+      go = reinterpret_cast<const float4*>(a.g_mlp_out)[idx];
+      mlp_input_row(a.g, (int64_t)(idx % a.n), a.cam.pos, a.lights.l[idx / a.n].pos, x);
+    }
+    for (int c = 0; c < net.k0_pad; c += 16) {
+      uint32_t w[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) w[i] = pack_f16(x[c + 2 * i], x[c + 2 * i + 1]);
+      tmem_st8(tA + lane_off + (uint32_t)(c >> 1), w);
+      if (t == 0) store_row16(sH, c, w);
+    }
+    publish();
+
+    // ---- forward, trunk ----------------------------------------------------------------------------------
+    uint32_t mask[SSSGS_MAX_TRUNK][4];
+    for (int l = 0; l < L; ++l) {
+      const int kl = l == 0 ? net.k0_pad : net.in[l], nl = net.out[l];
+      if (warp == 0) {
+        const uint32_t issue = elect_one();
+        const uint32_t idesc = make_idesc(nl, false, false);
+        for (int ks = 0; ks < kl / 16; ++ks)
+          umma_ts(tD, tA + ks * 8, make_desc(sW_addr + l * kTileBytes + (ks >> 2) * 16384 + (ks & 3) * 32, 16, 1024), idesc,
+                  ks > 0, issue);
+        umma_commit_if(bar, issue);
+      }
+      wait_mma();
+      for (int q = 0; q < 4; ++q) mask[l][q] = 0u;
+      for (int c0 = 0; c0 < nl; c0 += 16) {
+        float v[16];
+        tmem_ld16(tD + lane_off + c0, v);
+        uint32_t bits = 0u;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const float s = v[i] + sBias[l * 128 + c0 + i];
+          const bool pos = s > 0.f;
+          bits |= (pos ? 1u : 0u) << i;
+          v[i] = pos ? s : neg_slope * s;
+        }
+        mask[l][c0 >> 5] |= bits << (c0 & 31);
+        uint32_t w[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) w[i] = pack_f16(v[2 * i], v[2 * i + 1]);
+        tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);
+        if (l == t - 1) store_row16(sH, c0, w);
+      }
+      publish();
+    }
+    // ---- heads: outputs, then delta of the four head pre-activations (scaled) ---------------------------
+    if (warp == 0) {
+      const uint32_t issue = elect_one();
+      const uint32_t idesc = make_idesc(16, false, false);
+      for (int ks = 0; ks < net.head_in / 16; ++ks)
+        umma_ts(tD, tA + ks * 8, make_desc(sW_addr + L * kTileBytes + (ks >> 2) * 2048 + (ks & 3) * 32, 16, 1024), idesc,
+                ks > 0, issue);
+      umma_commit_if(bar, issue);
+    }
+    wait_mma();
+    {
+      float v[16];
+      tmem_ld16(tD + lane_off, v);
+      float dh[4];
+      const float gs[3] = {go.x * scale, go.y * scale, go.z * scale};
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float y = 1.f / (1.f + __expf(-(v[c] + sBias[L * 128 + c])));
+        dh[c] = gs[c] * y * (1.f - y);
+      }
+      dh[3] = (v[3] + sBias[L * 128 + 3]) > 0.f ? go.w * scale : 0.f;
+      uint32_t w[8] = {pack_f16(dh[0], dh[1]), pack_f16(dh[2], dh[3]), 0u, 0u, 0u, 0u, 0u, 0u};
+      tmem_st8(tAH + lane_off, w);
+      if (t == L) *reinterpret_cast<uint4*>(sDelta + tile_off(tid, 0, 16384)) = make_uint4(w[0], w[1], 0u, 0u);
+    }
+    // ---- delta recursion down to the target layer ---------------------------------------------------------
+    if (t < L) {
+      publish();
+      if (warp == 0) {   // G_{L-1} = delta_head W_head: K = the 16 rows of the head tile, read MN-major
+        const uint32_t issue = elect_one();
+        umma_ts(tD, tAH, make_desc(sW_addr + L * kTileBytes, 2048, 1024), make_idesc(net.head_in, false, true), 0u, issue);
+        umma_commit_if(bar, issue);
+      }
+      wait_mma();
+      for (int l = L - 1; l >= t; --l) {
+        const int nl = net.out[l];
+        for (int c0 = 0; c0 < nl; c0 += 16) {
+          float v[16];
+          tmem_ld16(tD + lane_off + c0, v);
+          const uint32_t bits = mask[l][c0 >> 5] >> (c0 & 31);
+          uint32_t w[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            w[i] = pack_f16(((bits >> (2 * i)) & 1u) ? v[2 * i] : neg_slope * v[2 * i],
+                            ((bits >> (2 * i + 1)) & 1u) ? v[2 * i + 1] : neg_slope * v[2 * i + 1]);
+          if (l == t) store_row16(sDelta, c0, w);
+          else tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);
+        }
+        if (l == t) break;
+        publish();
+        if (warp == 0) {   // G_{l-1} = delta_l W_l: B[n][k] = W_l[k][n], the forward tile read MN-major
+          const uint32_t issue = elect_one();
+          const uint32_t idesc = make_idesc(net.in[l], false, true);
+          for (int ks = 0; ks < nl / 16; ++ks)
+            umma_ts(tD, tA + ks * 8, make_desc(sW_addr + l * kTileBytes + ks * 2048, 16384, 1024), idesc, ks > 0, issue);
+          umma_commit_if(bar, issue);
+        }
+        wait_mma();
+      }
+    }
+    // ---- dW_t += delta_t^T h_{t-1}: K = the 128 rows of the tile, both operands MN-major ---------------------
+    publish();
+    if (warp == 0) {
+      const uint32_t issue = elect_one();
+      const uint32_t idesc = make_idesc(k_t, true, true);
+      for (int ks = 0; ks < kRowsT / 16; ++ks)
+        umma_ss(tDW, make_desc(sDelta_addr + ks * 2048, 16384, 1024), make_desc(sH_addr + ks * 2048, 16384, 1024), idesc,
+                (tiles_done > 0 || ks > 0) ? 1u : 0u, issue);
+      umma_commit_if(bar, issue);
+    }
+    {   // db_t[f] += sum over the rows of delta_t[row][f], f = tid (read while the MMAs run)
+      float s = 0.f;
+      for (int r = 0; r < kRowsT; ++r) s += __half2float(*reinterpret_cast<const __half*>(sDelta + tile_off(r, tid, 16384)));
+      db += s;
+    }
+    wait_mma();   // the operand tiles are free again
+    ++tiles_done;
+  }
+
+  // ---- the accumulators leave tensor memory: un-scale, one atomic per weight and CTA -----------------------
+  if (tiles_done > 0) {
+    const int m = tid;   // output neuron of the target layer
+    int w_row = -1, b_at = -1, n_in = 0;
+    if (t < L) {
+      if (m < net.out[t]) { w_row = net.w[t] + m * net.in[t]; b_at = net.b[t] + m; }
+      n_in = net.in[t];
+    } else {
+      if (m < 3) { w_row = net.sss_w + m * net.head_in; b_at = net.sss_b + m; }
+      else if (m == 3) { w_row = net.inc_w; b_at = net.inc_b; }
+      n_in = net.head_in;
+    }
+    for (int c0 = 0; c0 < k_t; c0 += 16) {
+      float v[16];
+      tmem_ld16(tDW + lane_off + c0, v);
+      if (w_row >= 0) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+          if (c0 + i < n_in && v[i] != 0.f) atomicAdd(&a.g_params[w_row + c0 + i], v[i] * inv_scale);
+      }
+    }
+    if (b_at >= 0 && db != 0.f) atomicAdd(&a.g_params[b_at], db * inv_scale);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
+}
+
+}  // namespace tc
+
 __global__ void __launch_bounds__(256) zero_kernel(float* p, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) p[i] = 0.f;
 }
@@ -646,8 +1065,56 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
 
 int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
                         int n_lights, const float* g_mlp_out, float* g_params, uint32_t* row_list, uint32_t* row_count,
-                        int num_sms, cudaStream_t s) {
+                        uint8_t* blob, bool pack, bool force_fp32, int num_sms, cudaStream_t s) {
   if (g.n == 0 || n_lights == 0 || !g_params) return 0;
+  int launches = 0;
+  const int64_t rows = g.n * n_lights;
+  if (cudaMemsetAsync(row_count, 0, 8, s) != cudaSuccess) return 0;
+  int64_t cb = (rows + 255) / 256;
+  if (cb > (int64_t)num_sms * 8) cb = (int64_t)num_sms * 8;
+  bwd_rows_kernel<<<(unsigned)cb, 256, 0, s>>>(reinterpret_cast<const float4*>(g_mlp_out), rows, row_list, row_count);
+  ++launches;
+
+  // ---- tensor-core path: a chain of <= 4 trunk layers and the two heads -------------------------------------
+  bool use_tc = !force_fp32 && mlp.n_inc_hidden == 0 && mlp.n_trunk >= 1 && mlp.n_trunk <= 4 && mlp.in_dim <= 128;
+  for (int l = 0; l < mlp.n_trunk && use_tc; ++l)
+    use_tc = mlp.trunk_width[l] % 16 == 0 && mlp.trunk_width[l] >= 16 && mlp.trunk_width[l] <= 128;
+  if (use_tc) {
+    tc::TcNet net;
+    memset(&net, 0, sizeof net);
+    net.n_trunk = mlp.n_trunk;
+    net.in_dim = mlp.in_dim;
+    net.k0_pad = (mlp.in_dim + 15) & ~15;
+    net.activation = mlp.activation;
+    net.slope = mlp.leaky_slope;
+    int off = 0, d = mlp.in_dim;
+    for (int l = 0; l < mlp.n_trunk; ++l) {
+      const int o = mlp.trunk_width[l];
+      net.out[l] = o; net.in[l] = d; net.w[l] = off; net.b[l] = off + o * d;
+      off += o * d + o;
+      d = o;
+    }
+    net.head_in = d;
+    net.sss_w = off; net.sss_b = off + 3 * d;
+    off += 3 * d + 3;
+    net.inc_w = off; net.inc_b = off + d;
+    if (pack) {
+      tc::bwd_pack_kernel<<<64, 256, 0, s>>>(net, (const float*)mlp.params, blob);
+      ++launches;
+    }
+    const int smem = tc::tc_smem_bytes(net.n_trunk);
+    if (ensure_dyn_smem((const void*)tc::mlp_backward_tc_kernel, smem) != cudaSuccess) return launches;
+    tc::TcArgs a;
+    a.g = g; a.net = net; a.cam = cam; a.lights = lights; a.n = g.n;
+    a.list = row_list; a.count = row_count; a.gomax_bits = row_count + 1;
+    a.g_mlp_out = g_mlp_out; a.blob = blob; a.g_params = g_params;
+    int gx = num_sms / (net.n_trunk + 1);
+    if (gx < 1) gx = 1;
+    tc::mlp_backward_tc_kernel<<<dim3((unsigned)gx, (unsigned)(net.n_trunk + 1)), 128, smem, s>>>(a);
+    return launches + 1;
+  }
+
+  // ---- fp32 CUDA-core path ------------------------------------------------------------------------------------
   BwdNet net;
   net.in_dim = mlp.in_dim;
   net.activation = mlp.activation;
@@ -677,18 +1144,13 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
   net.L[nl] = BwdLayer{off, off + di, 1, di, src, K_INC_OUT};
   ++nl;
   net.n_layers = nl;
-  const int64_t rows = g.n * n_lights;
-  if (cudaMemsetAsync(row_count, 0, 4, s) != cudaSuccess) return 0;
-  int64_t cb = (rows + 255) / 256;
-  if (cb > (int64_t)num_sms * 8) cb = (int64_t)num_sms * 8;
-  bwd_rows_kernel<<<(unsigned)cb, 256, 0, s>>>(reinterpret_cast<const float4*>(g_mlp_out), rows, row_list, row_count);
   const int smem = (128 * kWS + 3 * kBR * 128 + kBR * 4 + (nl + 1) * kBR * 128) * 4;
-  if (ensure_dyn_smem((const void*)mlp_backward_kernel, smem) != cudaSuccess) return 1;
+  if (ensure_dyn_smem((const void*)mlp_backward_kernel, smem) != cudaSuccess) return launches;
   int gx = num_sms / nl;
   if (gx < 1) gx = 1;
   mlp_backward_kernel<<<dim3((unsigned)gx, (unsigned)nl), 256, smem, s>>>(g, net, (const float*)mlp.params, cam, lights, g.n,
                                                                         row_list, row_count, g_mlp_out, g_params);
-  return 2;
+  return launches + 1;
 }
 
 }  // namespace sssgs

@@ -41,6 +41,7 @@ struct sssgs_ctx {
   uint8_t* contrib = nullptr;   // [n] visibility pre-pass flags (inside the control block)
   uint32_t* rows = nullptr;     // [n] Gaussians kept by the pre-pass
   uint8_t* mlp_blob = nullptr;
+  uint8_t* bwd_blob = nullptr;
   int64_t launches = 0;
   // optional per-stage timing
   bool profile = false;
@@ -126,6 +127,7 @@ size_t carve(sssgs_ctx* c, const sssgs_config& cfg, uint8_t* base) {
     if (c) c->wc.capacity = (uint32_t)chunks;
   }
   p = take(kMaxBlobBytes); if (c) c->mlp_blob = p;
+  p = take(kBwdBlobBytes); if (c) c->bwd_blob = p;   // packed weights of the tensor-core MLP backward
   // control block: everything that must be zero at the start of a camera
   const size_t ctrl_begin = off;
   if (c) c->control = base ? base + off : nullptr;
@@ -682,7 +684,8 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
                           void* cuda_stream) {
   if (!c) return SSSGS_EINVAL;
   if (!g || !mlp || !cam_in || !gr || (n_light > 0 && !lights)) return fail(c, SSSGS_EINVAL, "NULL argument");
-  if (flags & ~(uint32_t)SSSGS_TIGHT_LISTS) return fail(c, SSSGS_EINVAL, "sssgs_render_backward: only SSSGS_TIGHT_LISTS is accepted");
+  if (flags & ~(uint32_t)(SSSGS_TIGHT_LISTS | SSSGS_BACKWARD_FP32))
+    return fail(c, SSSGS_EINVAL, "sssgs_render_backward: only SSSGS_TIGHT_LISTS and SSSGS_BACKWARD_FP32 are accepted");
   if (n_light < 0 || g->n < 0) return fail(c, SSSGS_EINVAL, "negative count");
   if (g->n > c->cfg.max_gaussians) return fail(c, SSSGS_ECAPACITY, "n exceeds max_gaussians");
   if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(c, SSSGS_EINVAL, "vis_sh_degree must be 0 or 1");
@@ -787,7 +790,8 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
                                           gr->grad_mlp_out + (int64_t)l0 * n * 4, n, s);
     if (run_mlp && gr->grad_params)
       launches += launch_mlp_backward(*g, *mlp, cam, lb, nl, gr->grad_mlp_out + (int64_t)l0 * n * 4, gr->grad_params,
-                                      reinterpret_cast<uint32_t*>(c->mlp_out[1]), cnt + DC_BWD_ROWS, c->num_sms, s);
+                                      reinterpret_cast<uint32_t*>(c->mlp_out[1]), cnt + DC_BWD_ROWS, c->bwd_blob,
+                                      l0 == 0, (flags & SSSGS_BACKWARD_FP32) != 0, c->num_sms, s);
   }
   c->launches = launches;
   const cudaError_t e = cudaGetLastError();

@@ -45,7 +45,7 @@ def _rel(got, ref):
     return float(np.abs(np.asarray(got, np.float64) - ref).max() / max(np.abs(ref).max(), 1e-30))
 
 
-def _gpu(s, G, view=0, precomputed=None, tight=False):
+def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False):
     import torch
     from paper_2408_12282_b200 import binding
     R = binding.Renderer(s)
@@ -54,7 +54,7 @@ def _gpu(s, G, view=0, precomputed=None, tight=False):
         pre = None if precomputed is None else torch.from_numpy(np.ascontiguousarray(precomputed, np.float32)).cuda()
         fwd = R.render(cams=[cam], lights=lights, want=("rgb", "gbuffer", "mlp_out"), precomputed=pre, tight=tight)
         g = R.render_backward(cam, lights, torch.from_numpy(np.ascontiguousarray(G, np.float32)).cuda(), fwd["gbuffer"],
-                              tight=tight, precomputed=pre)
+                              tight=tight, precomputed=pre, fp32=fp32)
         torch.cuda.synchronize()
         launches = R.launch_count()
         out = {k: v.cpu().numpy() for k, v in g.items()}
@@ -105,35 +105,37 @@ def test_walks_backward_given_mlp_outputs(n, w, h, lights, tight):
     assert not out["grad_params"].any()         # outputs were given: no parameter gradient
 
 
-def test_mlp_backward_alone():
-    import torch
+@pytest.mark.parametrize("fp32", [False, True])
+def test_mlp_backward_alone(fp32):
     s = _scene(3000, 96, 80, 2)
     cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
     rng = np.random.default_rng(17)
     G = rng.standard_normal((2, cam.height, cam.width, 3))
-    out = _gpu(s, G)
+    out = _gpu(s, G, fp32=fp32)
     gm = out["grad_mlp_out"][:, :s.n].astype(np.float64)
     assert (np.abs(gm).sum(axis=2) > 0).sum() > 500          # rows that reach a pixel
     params = ob._t(s.mlp.params).requires_grad_(True)
-    loss = sum((ob.mlp_torch(ob._t(xs[l]), s.mlp, params) * ob._t(gm[l])).sum() for l in range(2))
+    # the tensor-core path differentiates the binary16-operand network (decisions in the kernel's precision)
+    loss = sum((ob.mlp_torch(ob._t(xs[l]), s.mlp, params, mode=0 if fp32 else 2) * ob._t(gm[l])).sum() for l in range(2))
     loss.backward()
     ref = params.grad.numpy()
     e = _rel(out["grad_params"], ref)
-    print(f"MLP backward alone: {e:.2e} of max |dL/dTheta| = {np.abs(ref).max():.3e}")
-    # fp32 forward re-evaluation + fp32 atomics over ~10^3 rows; a ReLU decided differently in fp32 than in
-    # float64 (pre-activation within rounding of 0) moves one row's contribution of one unit
-    assert e <= 5e-5
+    print(f"MLP backward alone ({'fp32 CUDA cores' if fp32 else 'tcgen05 fp16'}): {e:.2e} of max |dL/dTheta| = {np.abs(ref).max():.3e}")
+    # fp32 path: fp32 forward re-evaluation + fp32 sums over ~10^3 rows.  Tensor-core path: activations and deltas
+    # are binary16 (2^-11 relative each), products summed in fp32 over the rows: DESIGN 7e
+    assert e <= (5e-5 if fp32 else 1e-3)
 
 
-@pytest.mark.parametrize("cfg", [3, 6])
-def test_whole_chain_backward(cfg):
+@pytest.mark.parametrize("cfg,fp32", [(3, False), (3, True), (6, False), (2, False)])
+def test_whole_chain_backward(cfg, fp32):
     s = _scene(2000, 80, 64, 2, cfg=cfg)
     cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
     rng = np.random.default_rng(23)
     G = rng.standard_normal((2, cam.height, cam.width, 3))
     G[:, comp.unstable] = 0.0
-    r = ob.render_backward(s, proj, vals, ranges, xs, G)
-    out = _gpu(s, G)
+    tc = not fp32 and cfg != 6      # cfg 6 (incident-head hidden layers) always takes the fp32 MLP backward
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, mlp_mode=2 if tc else 0)
+    out = _gpu(s, G, fp32=fp32)
     # the forward MLP outputs the walks read are the fp16-operand kernel's (<= 1e-2 from float64, north_star):
     # they enter dL/dgbuffer through the shaded L_SSS / L_in channels and every upstream gradient through the
     # suffix sums, linearly: measured <= 1.5e-3 of the largest gradient, bar 5e-3 (DESIGN 6)

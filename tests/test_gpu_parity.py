@@ -525,6 +525,11 @@ def test_invalid_arguments_fail_cleanly():
         with pytest.raises(binding.SssgsError) as ei:
             r.render(cams=[big])
         assert ei.value.code == binding.SSSGS_ECAPACITY
+        # one image size per call: frames are laid out [F][H][W]
+        small = scenes.look_at_camera((0, -4, 0), 16, 32, 40.0)
+        with pytest.raises(binding.SssgsError) as ei:
+            r.render(cams=[s.cameras[0], small])
+        assert ei.value.code == binding.SSSGS_EINVAL
     finally:
         r.close()
 
