@@ -222,6 +222,9 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
   const int px = tx * kTile + (warp & 1) * 8 + (lane & 7), py = ty * kTile + (warp >> 1) * 4 + (lane >> 3);
   const bool inside = px < cam.width && py < cam.height;
   const int64_t pidx = (int64_t)min(py, cam.height - 1) * cam.width + min(px, cam.width - 1);
+  // centre and half size of the warp's 8 x 4 pixel block: entries whose alpha >= 1/255 support box (rec_a.w, the
+  // half-extents the forward walk culls with) misses the block are skipped by the whole warp, as in the forward
+  const float bcx = (float)(tx * kTile + (warp & 1) * 8) + 3.5f, bcy = (float)(ty * kTile + (warp >> 1) * 4) + 1.5f;
   const uint2 range = ranges[tile];
   const int n_entries = (int)(range.y - range.x);
   constexpr float kInvLog2e = 0.6931471805599453f;   // rec_b holds the conic scaled by -log2(e)/2, -log2(e), -log2(e)/2
@@ -255,24 +258,57 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
       s_b[tid] = rec_b[gid];
     }
     __syncthreads();
-    for (int j = 0; j < cnt && !done; ++j) {
-      const float4 ra = s_a[j], rb = s_b[j];
-      const float dx = (float)px - ra.x, dy = (float)py - ra.y;
-      const float p2 = fmaf(fmaf(rb.y, dy, rb.x * dx), dx, rb.z * dy * dy);   // log2(e) * power, as in the forward walk
-      float al;
-      asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(al) : "f"(p2));
-      al = fminf(kAlphaMax, rb.w * al);
-      if (p2 <= 0.f && al >= kAlphaMin) {
-        const float Tn = T * (1.f - al);
-        if (Tn < kTMin) { done = true; break; }
-        T = Tn;
-        last = b0 + j + 1;
+    for (int c0 = 0; c0 < cnt; c0 += 32) {
+      // cull 32 entries at a time (lane <-> entry), then walk the hits in list order
+      bool hit = false;
+      if (c0 + lane < cnt) {
+        const float4 ra = s_a[c0 + lane];
+        const float2 ext = __half22float2(*reinterpret_cast<const __half2*>(&ra.w));
+        hit = fabsf(ra.x - bcx) <= ext.x + 3.5f && fabsf(ra.y - bcy) <= ext.y + 1.5f;
+      }
+      unsigned m = __ballot_sync(0xFFFFFFFFu, hit);
+      while (m) {
+        const int j = c0 + __ffs(m) - 1;
+        m &= m - 1;
+        const float4 ra = s_a[j], rb = s_b[j];
+        const float dx = (float)px - ra.x, dy = (float)py - ra.y;
+        const float p2 = fmaf(fmaf(rb.y, dy, rb.x * dx), dx, rb.z * dy * dy);   // log2(e) * power, as in the forward walk
+        float al;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(al) : "f"(p2));
+        al = fminf(kAlphaMax, rb.w * al);
+        if (!done && p2 <= 0.f && al >= kAlphaMin) {
+          const float Tn = T * (1.f - al);
+          if (Tn < kTMin) {
+            done = true;
+          } else {
+            T = Tn;
+            last = b0 + j + 1;
+          }
+        }
       }
     }
   }
   atomicMax(&s_last, last);
   __syncthreads();
   const int max_last = s_last;
+  // destination of value k = 32 q + lane of an entry (see the reduction below): base pointer and per-Gaussian stride
+  float* dst[(16 + 4 * LB + 31) / 32];
+  int dst_stride[(16 + 4 * LB + 31) / 32];
+#pragma unroll
+  for (int q = 0; q < (16 + 4 * LB + 31) / 32; ++q) {
+    const int k = 32 * q + lane;
+    dst[q] = nullptr;
+    dst_stride[q] = 0;
+    if (k == 0) { dst[q] = g_opacity; dst_stride[q] = 1; }
+    else if (k <= 2) { dst[q] = g_mean2d + (k - 1); dst_stride[q] = 2; }
+    else if (k <= 5) { dst[q] = g_conic + (k - 3); dst_stride[q] = 3; }
+    else if (k == 6) { dst[q] = g_depth; dst_stride[q] = 1; }
+    else if (k <= 15) { dst[q] = g_attr + (k - 7); dst_stride[q] = 9; }
+    else if (k < 16 + 4 * LB && (k - 16) / 4 < n_lights) {
+      dst[q] = g_mlp_out + (size_t)((k - 16) / 4) * n * 4 + ((k - 16) & 3);
+      dst_stride[q] = 4;
+    }
+  }
   // ---- phase B: back to front ---------------------------------------------------------------------
   float R = 0.f;   // sum_{j > i} w_j Phi_j
   for (int b1 = max_last; b1 > 0; b1 -= kBwdBatch) {
@@ -285,8 +321,20 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
       s_b[tid] = rec_b[gid];
     }
     __syncthreads();
-    for (int j = cnt - 1; j >= 0; --j) {
-      const float4 ra = s_a[j], rb = s_b[j];
+    for (int c0 = ((cnt - 1) >> 5) << 5; c0 >= 0; c0 -= 32) {
+     bool hit = false;
+     if (c0 + lane < cnt) {
+       const float4 ra = s_a[c0 + lane];
+       const float2 ext = __half22float2(*reinterpret_cast<const __half2*>(&ra.w));
+       hit = fabsf(ra.x - bcx) <= ext.x + 3.5f && fabsf(ra.y - bcy) <= ext.y + 1.5f;
+     }
+     unsigned hits = __ballot_sync(0xFFFFFFFFu, hit);
+     while (hits) {   // the hits of the chunk, last entry first
+      const int hb = 31 - __clz(hits);
+      hits &= ~(1u << hb);
+      const int j = c0 + hb;
+      const float4 ra = s_a[j];
+      const float4 rb = s_b[j];
       const uint32_t gid = s_g[j];
       const float dx = (float)px - ra.x, dy = (float)py - ra.y;
       const float p2 = fmaf(fmaf(rb.y, dy, rb.x * dx), dx, rb.z * dy * dy);
@@ -296,6 +344,7 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
       const float al = fminf(kAlphaMax, araw);
       const bool blended = inside && (b0 + j) < last && p2 <= 0.f && al >= kAlphaMin;
       float w = 0.f, d_alpha = 0.f;
+      if (!__any_sync(0xFFFFFFFFu, blended)) continue;
       // channel vector of the entry: warp-uniform loads (L1 / L2 hits)
       const float4 a0 = attr[3 * (size_t)gid], a1 = attr[3 * (size_t)gid + 1], a2 = attr[3 * (size_t)gid + 2];
       float4 mo[LB];
@@ -311,46 +360,48 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
         T = Ti;
       }
       // ---- sums over the pixels of the warp, then one atomic per value -----------------------------
-      if (__any_sync(0xFFFFFFFFu, blended)) {
+      {
         // alpha = o e^power (unclamped); power = -(a dx^2 + c dy^2) / 2 - b dx dy
         const bool unclamped = araw < kAlphaMax;
         const float d_o = (blended && unclamped) ? d_alpha * e : 0.f;
         const float d_pow = (blended && unclamped) ? d_alpha * al : 0.f;
         const float ca = -2.f * kInvLog2e * rb.x, cb = -kInvLog2e * rb.y, cc = -2.f * kInvLog2e * rb.z;
-        float vals[6 + 11 + 4 * LB];
+        // value k of the entry: 0 opacity, 1-2 mean, 3-5 conic, 6 depth, 7-15 attributes, 16 + 4 l + c MLP output c of
+        // light l.  Groups of 32 values are summed over the 32 pixels of the warp with a halving exchange (31
+        // shuffles per group instead of 5 per value); lane k of group q ends up with the sum of value 32 q + k and
+        // adds it to its own destination: the atomics of an entry are issued by 16 + 4 LB lanes at once.
+        constexpr int NG = (16 + 4 * LB + 31) / 32;
+        float vals[32 * NG];
         vals[0] = d_o;
         vals[1] = d_pow * (ca * dx + cb * dy);      // d power / d pix_x
         vals[2] = d_pow * (cc * dy + cb * dx);
         vals[3] = d_pow * (-0.5f * dx * dx);         // d power / d conic a, b, c
         vals[4] = d_pow * (-dx * dy);
         vals[5] = d_pow * (-0.5f * dy * dy);
+#pragma unroll
         for (int c = 0; c < 10; ++c) vals[6 + c] = w * dGs[c];
-        vals[16] = 0.f;
+#pragma unroll
         for (int l = 0; l < LB; ++l)
-          for (int c = 0; c < 4; ++c) vals[17 + 4 * l + c] = w * dGl[l][c];
 #pragma unroll
-        for (int q = 0; q < 6 + 11 + 4 * LB; ++q) {
-          float s = vals[q];
+          for (int c = 0; c < 4; ++c) vals[16 + 4 * l + c] = w * dGl[l][c];
 #pragma unroll
-          for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
-          vals[q] = s;
-        }
-        if (lane == 0) {
-          atomicAdd(&g_opacity[gid], vals[0]);
-          atomicAdd(&g_mean2d[2 * (size_t)gid], vals[1]);
-          atomicAdd(&g_mean2d[2 * (size_t)gid + 1], vals[2]);
-          atomicAdd(&g_conic[3 * (size_t)gid], vals[3]);
-          atomicAdd(&g_conic[3 * (size_t)gid + 1], vals[4]);
-          atomicAdd(&g_conic[3 * (size_t)gid + 2], vals[5]);
-          atomicAdd(&g_depth[gid], vals[6]);
-          // g_attr: [n][9] = normal (3), base colour (3), roughness, metalness, sss
-          for (int c = 0; c < 9; ++c) atomicAdd(&g_attr[9 * (size_t)gid + c], vals[7 + c]);
-          for (int l = 0; l < LB; ++l) {
-            if (l >= n_lights) break;
-            for (int c = 0; c < 4; ++c) atomicAdd(&g_mlp_out[((size_t)l * n + gid) * 4 + c], vals[17 + 4 * l + c]);
+        for (int k = 16 + 4 * LB; k < 32 * NG; ++k) vals[k] = 0.f;
+#pragma unroll
+        for (int q = 0; q < NG; ++q) {
+#pragma unroll
+          for (int half = 16; half >= 1; half >>= 1) {
+            const bool up = (lane & half) != 0;
+#pragma unroll
+            for (int i = 0; i < half; ++i) {
+              const float send = up ? vals[32 * q + i] : vals[32 * q + i + half];
+              const float recv = __shfl_xor_sync(0xFFFFFFFFu, send, half);
+              vals[32 * q + i] = (up ? vals[32 * q + i + half] : vals[32 * q + i]) + recv;
+            }
           }
+          if (dst[q] != nullptr) atomicAdd(dst[q] + (size_t)gid * dst_stride[q], vals[32 * q]);
         }
       }
+     }
     }
   }
 }
