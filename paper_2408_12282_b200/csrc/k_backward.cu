@@ -15,6 +15,7 @@
 // Per-Gaussian sums are formed with float atomics: results are reproducible to rounding, not bit for bit.
 #include <cuda_fp16.h>
 
+#include <cstdio>
 #include <cstring>
 
 #include "internal.cuh"
@@ -408,17 +409,23 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
 
 // ---- a2 backward (fp32, CUDA cores) ----------------------------------------------------------------
 // The MLP input row of (Gaussian, light), as the forward kernel assembles it.
-__device__ __forceinline__ void mlp_input_row(const sssgs_gaussians& g, int64_t i, const float* cam_pos,
+// x[0 .. 39]: the 40 inputs of the paper; every index is a compile-time constant once the loops are unrolled, so a
+// caller's `float x[40]` stays in registers
+__device__ __forceinline__ void mlp_input_geo(const sssgs_gaussians& g, int64_t i, const float* cam_pos,
                                               const float* light_pos, float* x) {
   const float mu[3] = {g.means[3 * i], g.means[3 * i + 1], g.means[3 * i + 2]};
+#pragma unroll
   for (int k = 0; k < 3; ++k) x[k] = g.normals[3 * i + k];
   const float sgn = g.rotations[4 * i] < 0.f ? -1.f : 1.f;
   x[3] = sgn * g.rotations[4 * i];
   x[4] = sgn * g.rotations[4 * i + 1];
+#pragma unroll
   for (int k = 0; k < 3; ++k) x[5 + k] = g.scales[3 * i + k];
   float wi[3], wo[3];
+#pragma unroll
   for (int k = 0; k < 3; ++k) { wi[k] = light_pos[k] - mu[k]; wo[k] = cam_pos[k] - mu[k]; }
   const float d = sqrtf(dot3f(wi, wi)), dn = sqrtf(dot3f(wo, wo));
+#pragma unroll
   for (int k = 0; k < 3; ++k) { x[8 + k] = wi[k] / d; x[11 + k] = wo[k] / dn; }
   x[14] = d;
   const int nc = (g.vis_sh_degree + 1) * (g.vis_sh_degree + 1);
@@ -426,13 +433,19 @@ __device__ __forceinline__ void mlp_input_row(const sssgs_gaussians& g, int64_t 
   if (g.vis_sh_degree >= 1)
     v += 0.4886025f * (g.vis_sh[nc * i + 1] * x[9] + g.vis_sh[nc * i + 2] * x[10] + g.vis_sh[nc * i + 3] * x[8]);
   x[15] = fminf(1.f, fmaxf(0.f, v));
+#pragma unroll
   for (int k = 0; k < 4; ++k)
+#pragma unroll
     for (int a = 0; a < 3; ++a) {
       float s, c;
       sincospif((float)(1 << k) * mu[a], &s, &c);
       x[16 + 6 * k + a] = s;
       x[16 + 6 * k + 3 + a] = c;
     }
+}
+__device__ __forceinline__ void mlp_input_row(const sssgs_gaussians& g, int64_t i, const float* cam_pos,
+                                              const float* light_pos, float* x) {
+  mlp_input_geo(g, i, cam_pos, light_pos, x);
   for (int k = 0; k < g.feat_dim; ++k) x[40 + k] = g.feat[(int64_t)g.feat_dim * i + k];
 }
 
@@ -835,7 +848,9 @@ __host__ __device__ inline int tc_smem_bytes(int n_trunk) {
   return n_trunk * kTileBytes + kHeadTileBytes + 2 * kTileBytes + (n_trunk + 1) * 128 * 4 + 64 + 1024;
 }
 
-__global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_constant__ TcArgs a) {
+// 256 threads: thread pair (row, half) = (tid % 128, tid / 128); the two halves of a row split every epilogue's
+// 16-column groups alternately (warps w and w + 4 read the same 32 tensor-memory lanes).
+__global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_constant__ TcArgs a) {
   extern __shared__ uint8_t tc_smem_raw[];
   uint8_t* sm = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tc_smem_raw) + 1023) & ~(uintptr_t)1023);
   const TcNet& net = a.net;
@@ -847,6 +862,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
   uint64_t* bars = reinterpret_cast<uint64_t*>(sBias + (L + 1) * 128);
   uint32_t* s_tmem = reinterpret_cast<uint32_t*>(bars + 2);
   const int tid = threadIdx.x, warp = tid >> 5;
+  const int row = tid & 127, half = tid >> 7;   // this thread's row of the tile and its share of the column groups
   const int t = blockIdx.y;                      // target layer: t < L trunk, t == L the heads
   const uint32_t bar = smem_u32(bars);
 
@@ -855,11 +871,11 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
     const uint4* src = reinterpret_cast<const uint4*>(a.blob);
     uint4* dst = reinterpret_cast<uint4*>(sW);
     const int nw = (L * kTileBytes + kHeadTileBytes) / 16;
-    for (int i = tid; i < nw; i += 128) dst[i] = src[i];
+    for (int i = tid; i < nw; i += 256) dst[i] = src[i];
     const float* bsrc = reinterpret_cast<const float*>(a.blob + (size_t)L * kTileBytes + kHeadTileBytes);
-    for (int i = tid; i < (L + 1) * 128; i += 128) sBias[i] = bsrc[i];
+    for (int i = tid; i < (L + 1) * 128; i += 256) sBias[i] = bsrc[i];
     uint4* z = reinterpret_cast<uint4*>(sDelta);
-    for (int i = tid; i < 2 * kTileBytes / 16; i += 128) z[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < 2 * kTileBytes / 16; i += 256) z[i] = make_uint4(0u, 0u, 0u, 0u);
   }
   if (tid == 0) {
     mbar_init(bar, 1);
@@ -874,7 +890,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *s_tmem;
-  const uint32_t lane_off = (uint32_t)(warp * 32) << 16;
+  const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
   const uint32_t tD = tmem + kColD, tA = tmem + kColA, tAH = tmem + kColAH, tDW = tmem + kColDW;
   const uint32_t sW_addr = smem_u32(sW), sDelta_addr = smem_u32(sDelta), sH_addr = smem_u32(sH);
   uint32_t phase = 0;
@@ -891,6 +907,12 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
   const float neg_slope = leaky ? net.slope : 0.f;
   float db = 0.f;
   uint32_t tiles_done = 0;
+#ifdef SSSGS_BWD_TIMELINE
+  long long tl[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tl_t = clock64();
+#define TL(i) do { const long long c_ = clock64(); tl[i] += c_ - tl_t; tl_t = c_; } while (0)
+#else
+#define TL(i) do {} while (0)
+#endif
 
   auto publish = [&]() {   // this thread's operand writes (tensor memory and shared memory) before the next MMAs
     tmem_wait_st();
@@ -900,35 +922,72 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
     tc_fence_after();
   };
   auto wait_mma = [&]() {
+    TL(6);
     mbar_wait(bar, phase);
     phase ^= 1u;
     tc_fence_after();
+    TL(7);
   };
   // 16 consecutive 16-bit values of this thread's row (columns c0 .. c0 + 15) into a shared-memory operand tile
   auto store_row16 = [&](uint8_t* tile, int c0, const uint32_t* w) {
-    *reinterpret_cast<uint4*>(tile + tile_off(tid, c0, 16384)) = make_uint4(w[0], w[1], w[2], w[3]);
-    *reinterpret_cast<uint4*>(tile + tile_off(tid, c0 + 8, 16384)) = make_uint4(w[4], w[5], w[6], w[7]);
+    *reinterpret_cast<uint4*>(tile + tile_off(row, c0, 16384)) = make_uint4(w[0], w[1], w[2], w[3]);
+    *reinterpret_cast<uint4*>(tile + tile_off(row, c0 + 8, 16384)) = make_uint4(w[4], w[5], w[6], w[7]);
   };
 
   for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     // ---- the rows of the tile: inputs (as the forward kernel assembles them) and upstream gradients ------
-    const uint32_t ridx = tile * kRowsT + tid;
+    const uint32_t ridx = tile * kRowsT + row;
     float4 go = make_float4(0.f, 0.f, 0.f, 0.f);
-    float x[128];
-    for (int k = 0; k < net.k0_pad; ++k) x[k] = 0.f;
+    const int F = a.g.feat_dim;
+    int64_t gi = -1;
+    uint32_t li = 0;
     if (ridx < nrows) {
       const uint32_t idx = a.list[ridx];
+      li = idx / (uint32_t)a.n;
+      gi = (int64_t)(idx - li * (uint32_t)a.n);
       go = reinterpret_cast<const float4*>(a.g_mlp_out)[idx];
-      mlp_input_row(a.g, (int64_t)(idx % a.n), a.cam.pos, a.lights.l[idx / a.n].pos, x);
     }
-    for (int c = 0; c < net.k0_pad; c += 16) {
-      uint32_t w[8];
+    const float4* fp = gi >= 0 ? reinterpret_cast<const float4*>(a.g.feat + gi * F) : nullptr;   // the row's feature
+    auto feat4 = [&](int q) {   // features 4 q .. 4 q + 3
+      return (fp != nullptr && 4 * q < F) ? fp[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+    };
+    // Columns 0-47 (the 40 computed inputs, in registers, and the first 8 features) by half 0, the remaining
+    // feature columns by half 1 (16-byte loads, four in flight): no input is computed twice.
+    if (half == 0) {
+      const float4 f0 = feat4(0), f1 = feat4(1);
+      float e[40];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) w[i] = pack_f16(x[c + 2 * i], x[c + 2 * i + 1]);
-      tmem_st8(tA + lane_off + (uint32_t)(c >> 1), w);
-      if (t == 0) store_row16(sH, c, w);
+      for (int k = 0; k < 40; ++k) e[k] = 0.f;
+      if (gi >= 0) mlp_input_geo(a.g, gi, a.cam.pos, a.lights.l[li].pos, e);
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        uint32_t w[8];
+        if (c < 2) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) w[i] = pack_f16(e[16 * c + 2 * i], e[16 * c + 2 * i + 1]);
+        } else {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) w[i] = pack_f16(e[32 + 2 * i], e[33 + 2 * i]);
+          w[4] = pack_f16(f0.x, f0.y); w[5] = pack_f16(f0.z, f0.w);
+          w[6] = pack_f16(f1.x, f1.y); w[7] = pack_f16(f1.z, f1.w);
+        }
+        tmem_st8(tA + lane_off + (uint32_t)(8 * c), w);
+        if (t == 0) store_row16(sH, 16 * c, w);
+      }
+    } else {
+      for (int c = 3; 16 * c < net.k0_pad; ++c) {
+        float4 f[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) f[j] = feat4(4 * c - 10 + j);
+        uint32_t w[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { w[2 * j] = pack_f16(f[j].x, f[j].y); w[2 * j + 1] = pack_f16(f[j].z, f[j].w); }
+        tmem_st8(tA + lane_off + (uint32_t)(8 * c), w);
+        if (t == 0) store_row16(sH, 16 * c, w);
+      }
     }
     publish();
+    TL(0);
 
     // ---- forward, trunk ----------------------------------------------------------------------------------
     uint32_t mask[SSSGS_MAX_TRUNK][4];
@@ -944,7 +1003,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       }
       wait_mma();
       for (int q = 0; q < 4; ++q) mask[l][q] = 0u;
-      for (int c0 = 0; c0 < nl; c0 += 16) {
+      for (int c0 = 16 * half; c0 < nl; c0 += 32) {
         float v[16];
         tmem_ld16(tD + lane_off + c0, v);
         uint32_t bits = 0u;
@@ -964,6 +1023,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       }
       publish();
     }
+    TL(1);
     // ---- heads: outputs, then delta of the four head pre-activations (scaled) ---------------------------
     if (warp == 0) {
       const uint32_t issue = elect_one();
@@ -974,7 +1034,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       umma_commit_if(bar, issue);
     }
     wait_mma();
-    {
+    if (half == 0) {
       float v[16];
       tmem_ld16(tD + lane_off, v);
       float dh[4];
@@ -987,8 +1047,9 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       dh[3] = (v[3] + sBias[L * 128 + 3]) > 0.f ? go.w * scale : 0.f;
       uint32_t w[8] = {pack_f16(dh[0], dh[1]), pack_f16(dh[2], dh[3]), 0u, 0u, 0u, 0u, 0u, 0u};
       tmem_st8(tAH + lane_off, w);
-      if (t == L) *reinterpret_cast<uint4*>(sDelta + tile_off(tid, 0, 16384)) = make_uint4(w[0], w[1], 0u, 0u);
+      if (t == L) *reinterpret_cast<uint4*>(sDelta + tile_off(row, 0, 16384)) = make_uint4(w[0], w[1], 0u, 0u);
     }
+    TL(2);
     // ---- delta recursion down to the target layer ---------------------------------------------------------
     if (t < L) {
       publish();
@@ -1000,7 +1061,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       wait_mma();
       for (int l = L - 1; l >= t; --l) {
         const int nl = net.out[l];
-        for (int c0 = 0; c0 < nl; c0 += 16) {
+        for (int c0 = 16 * half; c0 < nl; c0 += 32) {
           float v[16];
           tmem_ld16(tD + lane_off + c0, v);
           const uint32_t bits = mask[l][c0 >> 5] >> (c0 & 31);
@@ -1024,6 +1085,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
         wait_mma();
       }
     }
+    TL(3);
     // ---- dW_t += delta_t^T h_{t-1}: K = the 128 rows of the tile, both operands MN-major ---------------------
     publish();
     if (warp == 0) {
@@ -1036,16 +1098,17 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
     }
     {   // db_t[f] += sum over the rows of delta_t[row][f], f = tid (read while the MMAs run)
       float s = 0.f;
-      for (int r = 0; r < kRowsT; ++r) s += __half2float(*reinterpret_cast<const __half*>(sDelta + tile_off(r, tid, 16384)));
+      for (int r = 64 * half; r < 64 * half + 64; ++r) s += __half2float(*reinterpret_cast<const __half*>(sDelta + tile_off(r, row, 16384)));
       db += s;
     }
     wait_mma();   // the operand tiles are free again
     ++tiles_done;
+    TL(4);
   }
 
   // ---- the accumulators leave tensor memory: un-scale, one atomic per weight and CTA -----------------------
   if (tiles_done > 0) {
-    const int m = tid;   // output neuron of the target layer
+    const int m = row;   // output neuron of the target layer
     int w_row = -1, b_at = -1, n_in = 0;
     if (t < L) {
       if (m < net.out[t]) { w_row = net.w[t] + m * net.in[t]; b_at = net.b[t] + m; }
@@ -1055,7 +1118,7 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
       else if (m == 3) { w_row = net.inc_w; b_at = net.inc_b; }
       n_in = net.head_in;
     }
-    for (int c0 = 0; c0 < k_t; c0 += 16) {
+    for (int c0 = 16 * half; c0 < k_t; c0 += 32) {
       float v[16];
       tmem_ld16(tDW + lane_off + c0, v);
       if (w_row >= 0) {
@@ -1066,6 +1129,13 @@ __global__ void __launch_bounds__(128, 1) mlp_backward_tc_kernel(const __grid_co
     }
     if (b_at >= 0 && db != 0.f) atomicAdd(&a.g_params[b_at], db * inv_scale);
   }
+#ifdef SSSGS_BWD_TIMELINE
+  TL(5);
+  if (tid == 0 && blockIdx.x == 0)
+    printf("target %d tiles %u: x %lld fwd %lld head %lld rec %lld dW %lld out %lld | before-wait %lld in-wait %lld (clk per tile)\n", t, tiles_done,
+           tl[0] / max(tiles_done, 1u), tl[1] / max(tiles_done, 1u), tl[2] / max(tiles_done, 1u), tl[3] / max(tiles_done, 1u),
+           tl[4] / max(tiles_done, 1u), tl[5], tl[6] / max(tiles_done, 1u), tl[7] / max(tiles_done, 1u));
+#endif
   tc_fence_before();
   __syncthreads();
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512u) : "memory");
@@ -1161,7 +1231,7 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
     a.g_mlp_out = g_mlp_out; a.blob = blob; a.g_params = g_params;
     int gx = num_sms / (net.n_trunk + 1);
     if (gx < 1) gx = 1;
-    tc::mlp_backward_tc_kernel<<<dim3((unsigned)gx, (unsigned)(net.n_trunk + 1)), 128, smem, s>>>(a);
+    tc::mlp_backward_tc_kernel<<<dim3((unsigned)gx, (unsigned)(net.n_trunk + 1)), 256, smem, s>>>(a);
     return launches + 1;
   }
 
