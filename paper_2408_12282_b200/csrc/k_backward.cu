@@ -733,6 +733,36 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
     v[i] = __uint_as_float(r[i]);
   }
 }
+// asynchronous form: r[] is valid only after tmem_wait_ld(r)
+__device__ __forceinline__ void tmem_ld16_async(uint32_t taddr, uint32_t* r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld(uint32_t* r) {
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) asm volatile("" : "+r"(r[i]));
+}
+// Walks this thread's (up to four) 16-column groups c0 = first + 32 i < n of an accumulator: f(r, c0, i) gets the 16
+// columns as bits and the group index as a compile-time constant (state indexed by it stays in registers); the
+// tensor-memory load of the next group is in flight while a group is processed.
+template <typename Fn>
+__device__ __forceinline__ void for_groups(uint32_t taddr, int first, int n, Fn f) {
+  uint32_t r[2][16];
+  if (first < n) tmem_ld16_async(taddr + first, r[0]);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int c0 = first + 32 * i;
+    if (c0 >= n) break;
+    tmem_wait_ld(r[i & 1]);
+    if (i + 1 < 4 && c0 + 32 < n) tmem_ld16_async(taddr + c0 + 32, r[(i + 1) & 1]);
+    f(r[i & 1], c0, i);
+  }
+}
 __device__ __forceinline__ uint32_t pack_f16(float a, float b) {   // .lo = a, .hi = b, RNE, saturating
   uint32_t d;
   asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(b), "f"(a));
@@ -914,9 +944,11 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
 #define TL(i) do {} while (0)
 #endif
 
-  auto publish = [&]() {   // this thread's operand writes (tensor memory and shared memory) before the next MMAs
+  // this thread's operand writes before the next MMAs: tensor memory always, shared memory (generic -> async proxy
+  // fence) only when an operand tile was written since the last call
+  auto publish = [&](bool smem_written) {
     tmem_wait_st();
-    fence_proxy_async();
+    if (smem_written) fence_proxy_async();
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -986,12 +1018,14 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
         if (t == 0) store_row16(sH, 16 * c, w);
       }
     }
-    publish();
+    publish(t == 0);
     TL(0);
 
     // ---- forward, trunk ----------------------------------------------------------------------------------
-    uint32_t mask[SSSGS_MAX_TRUNK][4];
-    for (int l = 0; l < L; ++l) {
+    uint32_t mask[4][4];   // ReLU decisions: layer (<= 4 on this path), this thread's column group; registers
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      if (l >= L) break;
       const int kl = l == 0 ? net.k0_pad : net.in[l], nl = net.out[l];
       if (warp == 0) {
         const uint32_t issue = elect_one();
@@ -1002,26 +1036,33 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
         umma_commit_if(bar, issue);
       }
       wait_mma();
+#pragma unroll
       for (int q = 0; q < 4; ++q) mask[l][q] = 0u;
-      for (int c0 = 16 * half; c0 < nl; c0 += 32) {
+      for_groups(tD + lane_off, 16 * half, nl, [&](const uint32_t* r, int c0, int gi_) {
         float v[16];
-        tmem_ld16(tD + lane_off + c0, v);
         uint32_t bits = 0u;
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
-          const float s = v[i] + sBias[l * 128 + c0 + i];
-          const bool pos = s > 0.f;
-          bits |= (pos ? 1u : 0u) << i;
-          v[i] = pos ? s : neg_slope * s;
+        for (int q = 0; q < 4; ++q) {
+          const float4 b4 = *reinterpret_cast<const float4*>(sBias + l * 128 + c0 + 4 * q);
+          v[4 * q] = __uint_as_float(r[4 * q]) + b4.x;
+          v[4 * q + 1] = __uint_as_float(r[4 * q + 1]) + b4.y;
+          v[4 * q + 2] = __uint_as_float(r[4 * q + 2]) + b4.z;
+          v[4 * q + 3] = __uint_as_float(r[4 * q + 3]) + b4.w;
         }
-        mask[l][c0 >> 5] |= bits << (c0 & 31);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          const bool pos = v[i] > 0.f;
+          bits |= (pos ? 1u : 0u) << i;
+          v[i] = pos ? v[i] : neg_slope * v[i];
+        }
+        mask[l][gi_] = bits;
         uint32_t w[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) w[i] = pack_f16(v[2 * i], v[2 * i + 1]);
         tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);
         if (l == t - 1) store_row16(sH, c0, w);
-      }
-      publish();
+      });
+      publish(l == t - 1);
     }
     TL(1);
     // ---- heads: outputs, then delta of the four head pre-activations (scaled) ---------------------------
@@ -1052,7 +1093,7 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
     TL(2);
     // ---- delta recursion down to the target layer ---------------------------------------------------------
     if (t < L) {
-      publish();
+      publish(false);
       if (warp == 0) {   // G_{L-1} = delta_head W_head: K = the 16 rows of the head tile, read MN-major
         const uint32_t issue = elect_one();
         umma_ts(tD, tAH, make_desc(sW_addr + L * kTileBytes, 2048, 1024), make_idesc(net.head_in, false, true), 0u, issue);
@@ -1061,20 +1102,22 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
       wait_mma();
       for (int l = L - 1; l >= t; --l) {
         const int nl = net.out[l];
-        for (int c0 = 16 * half; c0 < nl; c0 += 32) {
-          float v[16];
-          tmem_ld16(tD + lane_off + c0, v);
-          const uint32_t bits = mask[l][c0 >> 5] >> (c0 & 31);
+        for_groups(tD + lane_off, 16 * half, nl, [&](const uint32_t* r, int c0, int gi_) {
+          uint32_t bits = 0u;
+#pragma unroll
+          for (int ll = 0; ll < 4; ++ll)
+            if (ll == l) bits = mask[ll][gi_];
           uint32_t w[8];
 #pragma unroll
-          for (int i = 0; i < 8; ++i)
-            w[i] = pack_f16(((bits >> (2 * i)) & 1u) ? v[2 * i] : neg_slope * v[2 * i],
-                            ((bits >> (2 * i + 1)) & 1u) ? v[2 * i + 1] : neg_slope * v[2 * i + 1]);
+          for (int i = 0; i < 8; ++i) {
+            const float lo = __uint_as_float(r[2 * i]), hi = __uint_as_float(r[2 * i + 1]);
+            w[i] = pack_f16(((bits >> (2 * i)) & 1u) ? lo : neg_slope * lo, ((bits >> (2 * i + 1)) & 1u) ? hi : neg_slope * hi);
+          }
           if (l == t) store_row16(sDelta, c0, w);
           else tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);
-        }
+        });
         if (l == t) break;
-        publish();
+        publish(false);
         if (warp == 0) {   // G_{l-1} = delta_l W_l: B[n][k] = W_l[k][n], the forward tile read MN-major
           const uint32_t issue = elect_one();
           const uint32_t idesc = make_idesc(net.in[l], false, true);
@@ -1087,7 +1130,7 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
     }
     TL(3);
     // ---- dW_t += delta_t^T h_{t-1}: K = the 128 rows of the tile, both operands MN-major ---------------------
-    publish();
+    publish(true);
     if (warp == 0) {
       const uint32_t issue = elect_one();
       const uint32_t idesc = make_idesc(k_t, true, true);
