@@ -354,7 +354,7 @@ class ConfigRun:
             torch.cuda.synchronize()
             ms.append(a.elapsed_time(b))
         return {"ms": round(float(np.median(ms[1:])), 4), "launches": self.R.launch_count(),
-                "lights": len(self.lights), "mlp_backward": "fp32 CUDA cores (v1)"}
+                "lights": len(self.lights), "mlp_backward": "tcgen05, binary16 operands (fp32 CUDA-core path: SSSGS_BACKWARD_FP32)"}
 
     def close(self):
         self.graph = None

@@ -7,11 +7,12 @@
 //   composite_backward_kernel  per tile, walking its list back to front: dL / d (opacity, 2-D mean, conic,
 //                              depth, normal, base colour, roughness, metalness, sss) per Gaussian and
 //                              dL / d (L_SSS, L_in) per (Gaussian, light)                        (Eq. 3)
-//   mlp_backward_*             dL / d Theta (weights and biases of every layer)             (Eq. 6)
+//   mlp_backward_tc_kernel     dL / d Theta (weights and biases of every layer) on the tensor cores (Eq. 6):
+//                              binary16 operands, fp32 accumulation, the forward re-evaluated per row tile
+//   mlp_backward_kernel        the same in fp32 on the CUDA cores (SSSGS_BACKWARD_FP32; MLPs with incident-head
+//                              hidden layers or more than 4 trunk layers)
 // The discontinuous decisions of the forward pass (alpha >= 1/255, power <= 0, the T' < 1e-4 stop, the 0.99
-// clamp, the ReLUs) are constants of the differentiation.  Arithmetic is fp32 throughout; the MLP is
-// re-evaluated in fp32 from the caller's parameters (this first version runs on the CUDA cores: the
-// tensor-core forward keeps no activations, DESIGN.md section 7e says what a tcgen05 version needs).
+// clamp, the ReLUs) are constants of the differentiation.  Shading and compositing backward are fp32.
 // Per-Gaussian sums are formed with float atomics: results are reproducible to rounding, not bit for bit.
 #include <cuda_fp16.h>
 
@@ -407,7 +408,7 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
   }
 }
 
-// ---- a2 backward (fp32, CUDA cores) ----------------------------------------------------------------
+// ---- a2 backward: input rows, and the fp32 CUDA-core path ------------------------------------------
 // The MLP input row of (Gaussian, light), as the forward kernel assembles it.
 // x[0 .. 39]: the 40 inputs of the paper; every index is a compile-time constant once the loops are unrolled, so a
 // caller's `float x[40]` stays in registers

@@ -124,6 +124,13 @@ def test_mlp_backward_alone(fp32):
     # fp32 path: fp32 forward re-evaluation + fp32 sums over ~10^3 rows.  Tensor-core path: activations and deltas
     # are binary16 (2^-11 relative each), products summed in fp32 over the rows: DESIGN 7e
     assert e <= (5e-5 if fp32 else 1e-3)
+    if not fp32:   # for the record: the same gradients against the float64 network (other ReLU decisions where a
+        #            hidden pre-activation lies within the binary16 rounding error of 0): per cent, not 1e-4
+        p64 = ob._t(s.mlp.params).requires_grad_(True)
+        sum((ob.mlp_torch(ob._t(xs[l]), s.mlp, p64, mode=0) * ob._t(gm[l])).sum() for l in range(2)).backward()
+        e64 = _rel(out["grad_params"], p64.grad.numpy())
+        print(f"   vs the float64 network: {e64:.2e}")
+        assert e < e64 < 0.1
 
 
 @pytest.mark.parametrize("cfg,fp32", [(3, False), (3, True), (6, False), (2, False)])
