@@ -152,6 +152,44 @@ def test_whole_chain_backward(cfg, fp32):
     assert e <= 5e-3
 
 
+def test_backward_full_size_cfg2_sampled_tiles():
+    """BASELINE configs[1] at full size, the call bench.py times under `backward` (tight lists, tensor-core MLP
+    backward).  The oracle cannot differentiate the whole 512 x 512 frame in seconds, so dL/drgb is non-zero on the
+    pixels of 48 sampled tiles only (the longest list, the median one, random non-empty ones; zero on unstable
+    pixels): every gradient then depends on those tiles alone and the oracle composites exactly those."""
+    s = scenes.make_scene(2)
+    cam = s.cameras[0]
+    proj = oracle.project(s, cam)
+    keys, vals, ranges = oracle.build_lists(proj)
+    xs = [oracle.mlp_inputs(s, cam, s.lights[0][0].position)]
+    rng = np.random.default_rng(29)
+    length = ranges[:, 1].astype(np.int64) - ranges[:, 0].astype(np.int64)
+    nonempty = np.nonzero(length > 0)[0]
+    picks = {int(np.argmax(length)), int(nonempty[np.argsort(length[nonempty])[len(nonempty) // 2]])}
+    for t in rng.permutation(nonempty):
+        if len(picks) >= 48:
+            break
+        picks.add(int(t))
+    masked = np.zeros_like(ranges)
+    pix = np.zeros((cam.height, cam.width), bool)
+    for t in picks:
+        masked[t] = ranges[t]
+        ty, tx = divmod(t, proj.tiles_x)
+        pix[ty * 16:(ty + 1) * 16, tx * 16:(tx + 1) * 16] = True
+    mo = oracle.mlp_forward(xs[0], s.mlp, 2)
+    comp = oracle.composite(s, cam, proj, oracle.channels(s, proj, mo), vals, masked)
+    G = rng.standard_normal((1, cam.height, cam.width, 3))
+    G[0, ~pix | comp.unstable] = 0.0
+    assert (G[0] != 0).any(axis=-1).sum() > 5000
+    r = ob.render_backward(s, proj, vals, masked, xs, G, mlp_mode=2)
+    out = _gpu(s, G, tight=True)
+    _check_all({k: (v[:, pix][None] if k == "grad_gbuffer" else v) for k, v in out.items()},
+               type("R", (), {**r.__dict__, "d_gbuf": r.d_gbuf[:, pix][None]}), s, 5e-3, "cfg 2 full size:")
+    e = _rel(out["grad_params"], r.d_params)
+    print(f"cfg 2 full size: grad_params {e:.2e}")
+    assert e <= 5e-3
+
+
 def test_backward_rejects_bad_arguments():
     import torch
     from paper_2408_12282_b200 import binding
