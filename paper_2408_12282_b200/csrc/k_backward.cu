@@ -208,7 +208,7 @@ struct BwdEntry {
 
 template <int LB>
 __global__ void __launch_bounds__(256)
-composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__ ranges,
+composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__ ranges, const uint32_t* __restrict__ tile_order,
                           const uint32_t* __restrict__ sorted_vals, const float4* __restrict__ rec_a,
                           const float4* __restrict__ rec_b, const float4* __restrict__ attr,
                           const float4* __restrict__ mlp_out, int mlp_stride, const float* __restrict__ grad_gbuf,
@@ -219,7 +219,7 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
   __shared__ uint32_t s_g[kBwdBatch];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int tile = blockIdx.x;
+  const int tile = (int)tile_order[blockIdx.x];   // longest lists first (the forward's work order): a short tail
   const int tx = tile % cam.tiles_x, ty = tile / cam.tiles_x;
   const int px = tx * kTile + (warp & 1) * 8 + (lane & 7), py = ty * kTile + (warp >> 1) * 4 + (lane >> 3);
   const bool inside = px < cam.width && py < cam.height;
@@ -1218,7 +1218,7 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
   if (tiles == 0 || n_lights == 0) return 0;
   const int64_t npix = (int64_t)cam.width * cam.height;
 #define SSSGS_CB(LB)                                                                                              \
-  composite_backward_kernel<LB><<<tiles, 256, 0, s>>>(cam, n_lights, gb.ranges, sorted_vals, gb.rec_a, gb.rec_b, attr, \
+  composite_backward_kernel<LB><<<tiles, 256, 0, s>>>(cam, n_lights, gb.ranges, gb.tile_order, sorted_vals, gb.rec_a, gb.rec_b, attr, \
                                                       mlp_out, mlp_stride, grad_gbuf, npix, g_opacity, g_mean2d,   \
                                                       g_conic, g_depth, g_attr, g_mlp_out, n)
   if (n_lights <= 1) SSSGS_CB(1);
