@@ -193,9 +193,9 @@ def test_gbuffer_and_shading_with_reference_mlp(name, scene):
         worst, nun = check_gbuffer(gpu["gbuffer"][f], r)
         np.testing.assert_allclose(gpu["gbuffer"][f][..., 14] + gpu["gbuffer"][f][..., 15], 1.0, atol=2e-6)
         check_shading(scene, gpu, f, v, l)
-        # end to end against the oracle's own RGB on stable pixels (conditioning-aware tolerance)
-        rgb32 = oracle.shade(scene.cameras[v], scene.lights[v][l], r.gbuf, f32=True)[0]
-        tol = np.maximum(2e-4 * np.maximum(1.0, np.abs(r.rgb)), 50.0 * np.abs(rgb32 - r.rgb) + 1e-4)
+        # end to end against the oracle's own RGB on stable pixels: north_star's 1e-4 bar (HDR highlights scale it:
+        # S9); measured <= 0.23 of it on these scenes, so no conditioning term is needed here
+        tol = 1e-4 * np.maximum(1.0, np.abs(r.rgb))
         err = np.abs(gpu["rgb"][f] - r.rgb)
         st = ~r.comp.unstable
         assert (err[st] <= tol[st]).all(), f"rgb vs oracle: worst {err[st].max():.3e}"
@@ -250,7 +250,8 @@ def test_end_to_end_rgb_cfg1():
     check_lists(scene, gpu, r)
     st = ~r.comp.unstable
     err = np.abs(gpu["rgb"][0] - r.rgb)
-    assert np.percentile(err[st], 99.9) <= 2e-3 and err[st].max() <= 5e-2
+    # the fp16 MLP outputs differ from the emulating oracle's by <= 3e-3 on rare rows: measured p99.9 8e-6, max 6e-5
+    assert np.percentile(err[st], 99.9) <= 1e-4 and err[st].max() <= 1e-3
     assert np.abs(gpu["gbuffer"][0][..., :10] - r.gbuf[..., :10])[st].max() <= 1e-4
 
 
@@ -353,7 +354,7 @@ def test_forward_shading_variant_matches_oracle(width, n_lights):
         out = R.render(cams=[cam], lights=lights, want=("rgb",), precomputed=pre, forward=True)
         torch.cuda.synchronize()
         got = out["rgb"].cpu().numpy()
-        # and with the library's own MLP: same frames up to the bf16 MLP tolerance
+        # and with the library's own MLP: same frames up to the fp16 MLP tolerance
         own = R.render(cams=[cam], lights=lights, want=("rgb",), forward=True)
         torch.cuda.synchronize()
         own = own["rgb"].cpu().numpy()
@@ -372,7 +373,7 @@ def test_forward_shading_variant_matches_oracle(width, n_lights):
         err = np.abs(got[l] - r.rgb)
         assert (err[st] <= tol[st]).all(), f"light {l}: worst {err[st].max():.3e}"
         assert (err[~st] <= 2e-2 * np.maximum(1.0, np.abs(r.rgb[~st]))).all()
-        assert np.percentile(np.abs(own[l] - r.rgb)[st], 99.9) <= 5e-3
+        assert np.percentile(np.abs(own[l] - r.rgb)[st], 99.9) <= 1e-3   # own fp16 MLP vs the float64 MLP's frames
 
 
 def test_weight_cache_overflow_falls_back_to_the_list_walks(monkeypatch):
@@ -550,7 +551,7 @@ def test_full_size_cfg2_matches_oracle():
     assert np.abs(gpu["gbuffer"][0][..., 14:] - r.gbuf[..., 14:])[st].max() <= 1e-4
     check_shading(scene, gpu, 0, 0, 0)
     err = np.abs(gpu["rgb"][0] - r.rgb)[st]
-    assert np.percentile(err, 99.9) <= 2e-3
+    assert np.percentile(err, 99.9) <= 1e-4 and err.max() <= 1e-3     # measured 1.8e-5 / 1.0e-4
 
 
 @pytest.mark.parametrize("seed", range(10))
