@@ -580,5 +580,5 @@ def test_random_scenes(seed):
     for l in sorted({0, nl - 1}):
         r = oracle.render_frame(scene, 0, l, mlp_out=off["mlp_out"][l].astype(np.float64))
         d = np.abs(off["rgb"][l].astype(np.float64) - r.rgb)
-        tol = np.where(r.comp.unstable[..., None], 5e-2, 3e-4) * np.maximum(1.0, np.abs(r.rgb))
+        tol = np.where(r.comp.unstable[..., None], 5e-2, 1e-4) * np.maximum(1.0, np.abs(r.rgb))
         assert (d <= tol).all(), f"light {l}: worst {d.max():.3e}"
