@@ -152,6 +152,25 @@ def test_whole_chain_backward(cfg, fp32):
     assert e <= 5e-3
 
 
+@pytest.mark.parametrize("trunk,act", [([48, 32], 0), ([64, 64, 64], 1), ([128], 0), ([16, 128, 16, 64], 1)])
+def test_mlp_backward_tensor_core_shapes(trunk, act):
+    """The tensor-core MLP backward on shapes the BASELINE configs do not have: widths that are not multiples of
+    32 (odd 16-column group counts per thread), one and four trunk layers, Leaky-ReLU."""
+    s = _scene(1500, 64, 48, 2)
+    mlp = scenes._make_mlp(np.random.default_rng(41), s.mlp.in_dim, trunk, [], act)
+    s = dataclasses.replace(s, mlp=mlp)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    G = np.random.default_rng(43).standard_normal((2, cam.height, cam.width, 3))
+    outs = {fp32: _gpu(s, G, fp32=fp32) for fp32 in (False, True)}
+    for fp32, out in outs.items():
+        gm = out["grad_mlp_out"][:, :s.n].astype(np.float64)
+        params = ob._t(s.mlp.params).requires_grad_(True)
+        sum((ob.mlp_torch(ob._t(xs[l]), s.mlp, params, mode=0 if fp32 else 2) * ob._t(gm[l])).sum() for l in range(2)).backward()
+        e = _rel(out["grad_params"], params.grad.numpy())
+        print(f"trunk {trunk} act {act} {'fp32' if fp32 else 'tcgen05'}: {e:.2e}")
+        assert e <= (5e-5 if fp32 else 1e-3)
+
+
 def test_backward_full_size_cfg2_sampled_tiles():
     """BASELINE configs[1] at full size, the call bench.py times under `backward` (tight lists, tensor-core MLP
     backward).  The oracle cannot differentiate the whole 512 x 512 frame in seconds, so dL/drgb is non-zero on the
