@@ -133,12 +133,13 @@ def test_mlp_backward_alone(fp32):
         assert e < e64 < 0.1
 
 
-@pytest.mark.parametrize("cfg,fp32", [(3, False), (3, True), (6, False), (2, False)])
-def test_whole_chain_backward(cfg, fp32):
-    s = _scene(2000, 80, 64, 2, cfg=cfg)
+@pytest.mark.parametrize("cfg,fp32,lights", [(3, False, 2), (3, True, 2), (6, False, 2), (2, False, 2), (3, False, 9)])
+def test_whole_chain_backward(cfg, fp32, lights):
+    # 9 lights = two light batches: dL/dTheta accumulates over the batches, the row list is rebuilt per batch
+    s = _scene(2000, 80, 64, lights, cfg=cfg)
     cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
     rng = np.random.default_rng(23)
-    G = rng.standard_normal((2, cam.height, cam.width, 3))
+    G = rng.standard_normal((lights, cam.height, cam.width, 3))
     G[:, comp.unstable] = 0.0
     tc = not fp32 and cfg != 6      # cfg 6 (incident-head hidden layers) always takes the fp32 MLP backward
     r = ob.render_backward(s, proj, vals, ranges, xs, G, mlp_mode=2 if tc else 0)
