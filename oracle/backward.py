@@ -1,4 +1,4 @@
-"""Backward pass of hot-path steps a2 / a7 / a8 -- CPU ORACLE (test infrastructure only).
+"""Backward pass of hot-path steps a2 / a3 / a7 / a8 -- CPU ORACLE (test infrastructure only).
 
 PAPER.md L11 ("optimize all parameters jointly via raytraced differentiable rendering"), L112 (the
 incident-light network is "jointly evaluated" and trained), L343-349 (App. F: the losses are functions
@@ -75,6 +75,49 @@ def mlp_torch(x: torch.Tensor, mlp, params: torch.Tensor, mode: int = 0) -> torc
         else:
             inc = torch.relu(rnd(hi) @ W.T + b)
     return torch.cat([sss, inc], dim=1)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Step 3: EWA projection (orc_project_f64: Eq. 2), for the gradients w.r.t. mean, scale, rotation
+# ---------------------------------------------------------------------------------------------------
+def project_torch(means, scales, rotations, cam):
+    """means [n,3], scales [n,3], rotations [n,4] (r,x,y,z) torch float64 -> (pix [n,2], conic [n,3], depth [n],
+    cov2d [n,3]).  Sigma' = J W Sigma W^T J^T + 0.3 I with the frustum clamp of the Jacobian (a constant of the
+    differentiation where it clamps), conic = Sigma'^-1.  No culling: the caller masks by the oracle's `visible`."""
+    R, t = _t(cam.R), _t(cam.t)
+    p = means @ R.T + t
+    z = p[:, 2]
+    u, w = p[:, 0] / z, p[:, 1] / z
+    pix = torch.stack([cam.fx * u + cam.cx, cam.fy * w + cam.cy], dim=1)
+    lx, ly = 1.3 * cam.tan_half_fovx, 1.3 * cam.tan_half_fovy
+    xc, yc = torch.clamp(u, -lx, lx) * z, torch.clamp(w, -ly, ly) * z
+    zero = torch.zeros_like(z)
+    J = torch.stack([torch.stack([cam.fx / z, zero, -cam.fx * xc / (z * z)], dim=1),
+                     torch.stack([zero, cam.fy / z, -cam.fy * yc / (z * z)], dim=1)], dim=1)       # [n,2,3]
+    r, x, y, zq = rotations[:, 0], rotations[:, 1], rotations[:, 2], rotations[:, 3]
+    Rq = torch.stack([1 - 2 * (y * y + zq * zq), 2 * (x * y - r * zq), 2 * (x * zq + r * y),
+                      2 * (x * y + r * zq), 1 - 2 * (x * x + zq * zq), 2 * (y * zq - r * x),
+                      2 * (x * zq - r * y), 2 * (y * zq + r * x), 1 - 2 * (x * x + y * y)], dim=1).reshape(-1, 3, 3)
+    M = Rq * scales[:, None, :]
+    Sg = M @ M.transpose(1, 2)
+    T = J @ R                                                                                     # [n,2,3]
+    c2 = T @ Sg @ T.transpose(1, 2)
+    a, b, c = c2[:, 0, 0] + 0.3, c2[:, 0, 1], c2[:, 1, 1] + 0.3
+    det = a * c - b * b
+    conic = torch.stack([c / det, -b / det, a / det], dim=1)
+    return pix, conic, z, torch.stack([a, b, c], dim=1)
+
+
+def project_backward(scene, cam, visible, d_pix, d_conic, d_depth):
+    """dL/d(means, scales, rotations) [n,3], [n,3], [n,4] from dL/d(pix, conic, depth) of the visible Gaussians."""
+    mu = _t(scene.means).requires_grad_(True)
+    sc = _t(scene.scales).requires_grad_(True)
+    q = _t(scene.rotations).requires_grad_(True)
+    pix, conic, depth, _ = project_torch(mu, sc, q, cam)
+    m = torch.as_tensor(np.asarray(visible) != 0)
+    loss = (pix[m] * _t(d_pix)[m]).sum() + (conic[m] * _t(d_conic)[m]).sum() + (depth[m] * _t(d_depth)[m]).sum()
+    loss.backward()
+    return mu.grad.numpy(), sc.grad.numpy(), q.grad.numpy()
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -186,12 +229,15 @@ def shade_torch(cam, light_pos, light_intensity, gbuf: torch.Tensor) -> torch.Te
 # The gradients
 # ---------------------------------------------------------------------------------------------------
 def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16,
-                    given_mlp_out=None, mlp_mode: int = 0):
+                    given_mlp_out=None, mlp_mode: int = 0, through_projection: bool = False):
     """Gradients of L = sum_l <grad_rgb[l], rgb_l> for one view.
 
     proj / vals / ranges: the oracle's projection and tile lists of the view (oracle.project / build_lists);
     mlp_inputs: [L][n, in_dim] float64 (oracle.mlp_inputs per light); grad_rgb [L, H, W, 3].
     mlp_mode: 0 float64 MLP, 2 its binary16-emulating restatement (mlp_torch).
+    through_projection: pix / conic / depth are computed from (means, scales, rotations) by project_torch, and
+    d_means [n,3], d_scales [n,3], d_rotations [n,4] are returned too (the MLP inputs stay constants: step a1 is
+    not differentiated).
     given_mlp_out: [L, n, 4] or None: the MLP outputs are these constants instead of mlp(mlp_inputs) (isolates
     the walks: d_params is then zero).
     Returns a namespace of numpy float64 arrays:
@@ -207,9 +253,22 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
     L, n = len(lights), int(scene.n)
     params = _t(scene.mlp.params).requires_grad_(True)
     opac = _t(scene.opacities).requires_grad_(True)
-    pix = _t(proj.pix).requires_grad_(True)
-    conic = _t(proj.conic).requires_grad_(True)
-    depth = _t(proj.depth).requires_grad_(True)
+    mu = sc = rot = None
+    if through_projection:
+        mu = _t(scene.means).requires_grad_(True)
+        sc = _t(scene.scales).requires_grad_(True)
+        rot = _t(scene.rotations).requires_grad_(True)
+        tp, tc, td, _ = project_torch(mu, sc, rot, cam)
+        vis = torch.as_tensor(np.asarray(proj.visible) != 0)
+        pix = torch.where(vis[:, None], tp, _t(proj.pix))
+        conic = torch.where(vis[:, None], tc, _t(proj.conic))
+        depth = torch.where(vis, td, _t(proj.depth))
+        for t_ in (pix, conic, depth):
+            t_.retain_grad()
+    else:
+        pix = _t(proj.pix).requires_grad_(True)
+        conic = _t(proj.conic).requires_grad_(True)
+        depth = _t(proj.depth).requires_grad_(True)
     normals = _t(scene.normals).requires_grad_(True)
     base = _t(scene.base_color).requires_grad_(True)
     rough = _t(scene.roughness).requires_grad_(True)
@@ -239,4 +298,6 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
         mlp_out=np.stack([m.detach().numpy() for m in mlp_outs]),
         d_gbuf=np.stack([z(g) for g in gbufs]), d_mlp_out=np.stack([z(m) for m in mlp_outs]),
         d_params=z(params), d_opacity=z(opac), d_pix=z(pix), d_conic=z(conic), d_depth=z(depth),
-        d_normals=z(normals), d_base=z(base), d_rough=z(rough), d_metal=z(metal), d_sss=z(sss))
+        d_normals=z(normals), d_base=z(base), d_rough=z(rough), d_metal=z(metal), d_sss=z(sss),
+        d_means=z(mu) if through_projection else None, d_scales=z(sc) if through_projection else None,
+        d_rotations=z(rot) if through_projection else None)

@@ -224,3 +224,70 @@ def test_fp16_emulation_decides_in_the_rounded_arithmetic():
     np.testing.assert_allclose(got[0][1][8], h0, rtol=1e-12)                            # dL/dw_inc = h
     assert got[2][0][3] == 0.5 and got[2][1][0] == 0.0 and got[2][1][1] == 0.0 and got[2][1][8] == 0.0
     assert got[2][1][9] == 1.0
+
+
+def test_projection_restatement_and_its_gradient():
+    """project_torch == the C++ double projection (orc_project_f64) and, inverted, the canonical fp32 conic;
+    its reverse-mode gradient == central finite differences of the C++ function; closed form on the optical axis."""
+    s = _scene()
+    cam = s.cameras[0]
+    proj = oracle.project(s, cam)
+    cov, pix, depth = oracle.project_f64(s, cam)
+    tp, tc, td, tcov = ob.project_torch(ob._t(s.means), ob._t(s.scales), ob._t(s.rotations), cam)
+    np.testing.assert_allclose(tcov.numpy(), cov, rtol=1e-12)
+    np.testing.assert_allclose(tp.numpy(), pix, rtol=1e-12)
+    np.testing.assert_allclose(td.numpy(), depth, rtol=1e-13)
+    vis = proj.visible != 0
+    assert vis.sum() > 100
+    np.testing.assert_allclose(tc.numpy()[vis], proj.conic[vis], rtol=2e-4, atol=1e-7)
+    np.testing.assert_allclose(tp.numpy()[vis], proj.pix[vis], rtol=1e-5, atol=1e-4)
+    # finite differences of L = <gp, pix> + <gc, conic(cov)> + <gd, depth> through the C++ function
+    rng = np.random.default_rng(5)
+    gp, gc, gd = rng.standard_normal((s.n, 2)), rng.standard_normal((s.n, 3)), rng.standard_normal(s.n)
+    dm, dsc, dq = ob.project_backward(s, cam, vis, gp, gc, gd)
+
+    def loss(sc_):
+        cov_, pix_, dep_ = oracle.project_f64(sc_, cam)
+        det = cov_[:, 0] * cov_[:, 2] - cov_[:, 1] ** 2
+        con = np.stack([cov_[:, 2] / det, -cov_[:, 1] / det, cov_[:, 0] / det], 1)
+        return float((pix_[vis] * gp[vis]).sum() + (con[vis] * gc[vis]).sum() + (dep_[vis] * gd[vis]).sum())
+
+    ids = np.nonzero(vis)[0][:6]
+    for field, grad, ncomp in (("means", dm, 3), ("scales", dsc, 3), ("rotations", dq, 4)):
+        for i in ids[:3]:
+            for k in range(ncomp):
+                base = np.array(getattr(s, field), np.float32)
+                h = np.float32(2.0 ** -10) * max(1e-3, abs(float(base[i, k])))   # float32 fields: a relative step
+                hi, lo = base.copy(), base.copy()
+                hi[i, k] += h
+                lo[i, k] -= h
+                num = (loss(dataclasses.replace(s, **{field: hi})) - loss(dataclasses.replace(s, **{field: lo}))) \
+                    / (float(hi[i, k]) - float(lo[i, k]))
+                assert abs(num - grad[i, k]) <= 2e-4 * max(1.0, abs(grad[i, k])) + 1e-3 * np.abs(grad[i]).max(), \
+                    (field, i, k, num, grad[i, k])
+    assert not dm[~vis].any() and not dsc[~vis].any() and not dq[~vis].any()
+    # closed form: isotropic Gaussian (sigma) on the optical axis, identity rotation: Sigma' = ((f sigma / z)^2 + 0.3) I
+    cam0 = scenes.look_at_camera((0.0, -4.0, 0.0), 64, 64, 40.0)
+    sig, z = 0.25, 4.0
+    one = custom_scene([[0.0, 0.0, 0.0]], [[sig, sig, sig]], width=64, height=64)
+    one = dataclasses.replace(one, cameras=[cam0])
+    v = (cam0.fx * sig / z) ** 2 + 0.3
+    _, sc1, _ = ob.project_backward(one, cam0, np.ones(1), np.zeros((1, 2)), np.array([[1.0, 0.0, 0.0]]), np.zeros(1))
+    # conic_a = 1 / v; the image x axis is fed by one world axis only: d conic_a / d s_k = -(2 f^2 s_k / z^2) / v^2 for that k
+    assert np.isclose(np.abs(sc1).sum(), 2 * cam0.fx ** 2 * sig / z ** 2 / v ** 2, rtol=1e-9)
+
+
+def test_render_backward_through_the_projection_chains():
+    """through_projection: dL/d(means, scales, rotations) == project_backward fed the same call's dL/d(pix, conic,
+    depth) (chain rule across the two restatements), and the forward image is unchanged to rounding."""
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    G = np.random.default_rng(13).standard_normal((2, cam.height, cam.width, 3))
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, through_projection=True)
+    r0 = ob.render_backward(s, proj, vals, ranges, xs, G)
+    np.testing.assert_allclose(r.rgb, r0.rgb, rtol=0, atol=2e-5)     # float64 projection vs the canonical fp32 values
+    dm, dsc, dq = ob.project_backward(s, cam, proj.visible, r.d_pix, r.d_conic, r.d_depth)
+    np.testing.assert_allclose(r.d_means, dm, rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(r.d_scales, dsc, rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(r.d_rotations, dq, rtol=1e-9, atol=1e-12)
+    assert np.abs(r.d_means).max() > 0 and np.abs(r.d_rotations).max() > 0
