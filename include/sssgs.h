@@ -264,8 +264,9 @@ int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_
  * it computes dL/d of: the G-buffer of every light; the MLP outputs per (light, Gaussian); the MLP
  * parameters Theta; and per Gaussian the opacity, the 2-D mean, the conic (inverse 2-D covariance,
  * entries a, b, c of  power = -(a dx^2 + c dy^2) / 2 - b dx dy), the depth, the normal, the base
- * colour, roughness, metalness and subsurfaceness.  The 2-D mean / conic / depth gradients are the
- * interface to the projection's backward (step a3: not part of this call).  The forward decisions
+ * colour, roughness, metalness and subsurfaceness; and, when grad_means / grad_scales / grad_rotations are
+ * given, the 2-D mean / conic / depth gradients pushed through the EWA projection (step a3) to the mean,
+ * the scale and the rotation.  The forward decisions
  * (alpha >= 1/255, the T' < 1e-4 stop, the 0.99 clamp, ReLUs) are constants of the differentiation.
  * All pointers are DEVICE pointers, 16-byte aligned, fp32; every gradient array is overwritten.
  * gbuffer must be the G-buffer sssgs_render wrote for the same scene, camera and lights.
@@ -289,6 +290,11 @@ typedef struct {
   float* grad_conic;         /* [n][3]  dL / d (a, b, c)                               (out, required) */
   float* grad_depth;         /* [n]                                                    (out, required) */
   float* grad_attr;          /* [n][9]  normal (3), base colour (3), roughness, metalness, sss (out, required) */
+  /* step a3 differentiated (Eq. 2): the three above pushed through the EWA projection.  All
+     three or none (NULL).  The dependence of the MLP INPUTS on these (step a1) is not differentiated.          */
+  float* grad_means;         /* [n][3]  dL / d mu                                      (out, may be NULL)  */
+  float* grad_scales;        /* [n][3]  dL / d s (activated scales, as given)          (out, may be NULL)  */
+  float* grad_rotations;     /* [n][4]  dL / d q (r, x, y, z), the quaternion as given (out, may be NULL)  */
 } sssgs_grads;
 int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
                           const sssgs_camera* cam, const sssgs_light* lights, int n_light,

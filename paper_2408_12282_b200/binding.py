@@ -83,7 +83,8 @@ class sssgs_out(ctypes.Structure):
 
 class sssgs_grads(ctypes.Structure):
     _fields_ = [(k, _vp) for k in ("grad_rgb", "gbuffer", "grad_gbuffer", "grad_mlp_out", "grad_params",
-                                   "grad_opacity", "grad_mean2d", "grad_conic", "grad_depth", "grad_attr")]
+                                   "grad_opacity", "grad_mean2d", "grad_conic", "grad_depth", "grad_attr",
+                                   "grad_means", "grad_scales", "grad_rotations")]
 
 
 class sssgs_bake(ctypes.Structure):
@@ -347,7 +348,7 @@ class Renderer:
         z = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)  # noqa: E731
         out = {"grad_gbuffer": z(L, H, W, 16), "grad_mlp_out": z(L, n, 4), "grad_params": z(self.params.numel()),
                "grad_opacity": z(n), "grad_mean2d": z(n, 2), "grad_conic": z(n, 3), "grad_depth": z(n),
-               "grad_attr": z(n, 9)}
+               "grad_attr": z(n, 9), "grad_means": z(n, 3), "grad_scales": z(n, 3), "grad_rotations": z(n, 4)}
         gr = sssgs_grads()
         self._bwd_in = (grad_rgb.contiguous(), gbuffer.contiguous())
         gr.grad_rgb, gr.gbuffer = self._bwd_in[0].data_ptr(), self._bwd_in[1].data_ptr()

@@ -1,4 +1,4 @@
-// Backward pass of hot-path steps a8 (deferred shading), a7 (compositing) and a2 (the MLP)
+// Backward pass of hot-path steps a8 (deferred shading), a7 (compositing), a2 (the MLP) and a3 (projection)
 // ("optimize all parameters jointly via raytraced differentiable rendering",
 // L112, L343-349: the losses are functions of the rendered image and of the rasterised property images).
 //
@@ -7,6 +7,7 @@
 //   composite_backward_kernel  per tile, walking its list back to front: dL / d (opacity, 2-D mean, conic,
 //                              depth, normal, base colour, roughness, metalness, sss) per Gaussian and
 //                              dL / d (L_SSS, L_in) per (Gaussian, light)                        (Eq. 3)
+//   project_backward_kernel    dL / d (mean, scale, rotation) from dL / d (2-D mean, conic, depth)    (Eq. 2)
 //   mlp_backward_tc_kernel     dL / d Theta (weights and biases of every layer) on the tensor cores (Eq. 6):
 //                              binary16 operands, fp32 accumulation, the forward re-evaluated per row tile
 //   mlp_backward_kernel        the same in fp32 on the CUDA cores (SSSGS_BACKWARD_FP32; MLPs with incident-head
@@ -1187,6 +1188,125 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
 
 }  // namespace tc
 
+// ---- a3 backward: dL/d(2-D mean, conic, depth) -> dL/d(mean, scale, rotation) -------------------------------
+// Reverse mode of the EWA projection (Eq. 2), per Gaussian, hand derived:
+//   p = R mu + t, (u, w) = (p_x, p_y) / z, pix = (fx u + cx, fy w + cy), depth = z,
+//   J = [[fx/z, 0, -fx u_cl/z], [0, fy/z, -fy w_cl/z]] (u_cl, w_cl: frustum clamp, constant where it clamps),
+//   T = J R, Sigma = M M^T with M = Rq diag(s), (a, b, c) = T Sigma T^T + 0.3 I, conic = (c, -b, a) / (a c - b^2).
+// Plain fp32 (the canonical rounding sequence of project_kernel only matters for keys); Gaussians without an
+// upstream gradient (culled, never blended) get zeros.
+__global__ void __launch_bounds__(256)
+project_backward_kernel(int64_t n, const float* __restrict__ means, const float* __restrict__ scales,
+                        const float* __restrict__ rotations, CamParams cam, const float* __restrict__ g_mean2d,
+                        const float* __restrict__ g_conic, const float* __restrict__ g_depth,
+                        float* __restrict__ d_means, float* __restrict__ d_scales, float* __restrict__ d_rot) {
+  const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  const float gpx = g_mean2d[2 * i], gpy = g_mean2d[2 * i + 1];
+  const float gca = g_conic[3 * i], gcb = g_conic[3 * i + 1], gcc = g_conic[3 * i + 2];
+  const float gz = g_depth[i];
+  float dmu[3] = {0.f, 0.f, 0.f}, ds[3] = {0.f, 0.f, 0.f}, dq[4] = {0.f, 0.f, 0.f, 0.f};
+  if (gpx != 0.f || gpy != 0.f || gca != 0.f || gcb != 0.f || gcc != 0.f || gz != 0.f) {
+    const float* R = cam.R;
+    const float mu[3] = {means[3 * i], means[3 * i + 1], means[3 * i + 2]};
+    float p[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) p[k] = R[3 * k] * mu[0] + R[3 * k + 1] * mu[1] + R[3 * k + 2] * mu[2] + cam.t[k];
+    const float z = p[2], iz = 1.f / z;
+    const float u = p[0] * iz, w = p[1] * iz;
+    const float lx = kFrustumClamp * cam.tanx, ly = kFrustumClamp * cam.tany;
+    const bool free_x = u > -lx && u < lx, free_y = w > -ly && w < ly;
+    const float ucl = fminf(lx, fmaxf(-lx, u)), wcl = fminf(ly, fmaxf(-ly, w));
+    const float j00 = cam.fx * iz, j11 = cam.fy * iz, j02 = -cam.fx * ucl * iz, j12 = -cam.fy * wcl * iz;
+    float T0[3], T1[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      T0[k] = j00 * R[k] + j02 * R[6 + k];
+      T1[k] = j11 * R[3 + k] + j12 * R[6 + k];
+    }
+    const float qr = rotations[4 * i], qx = rotations[4 * i + 1], qy = rotations[4 * i + 2], qz = rotations[4 * i + 3];
+    const float sc[3] = {scales[3 * i], scales[3 * i + 1], scales[3 * i + 2]};
+    float Rq[9];
+    Rq[0] = 1.f - 2.f * (qy * qy + qz * qz); Rq[1] = 2.f * (qx * qy - qr * qz); Rq[2] = 2.f * (qx * qz + qr * qy);
+    Rq[3] = 2.f * (qx * qy + qr * qz); Rq[4] = 1.f - 2.f * (qx * qx + qz * qz); Rq[5] = 2.f * (qy * qz - qr * qx);
+    Rq[6] = 2.f * (qx * qz - qr * qy); Rq[7] = 2.f * (qy * qz + qr * qx); Rq[8] = 1.f - 2.f * (qx * qx + qy * qy);
+    float M[9], Sg[9];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) M[3 * a + b] = Rq[3 * a + b] * sc[b];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) Sg[3 * a + b] = M[3 * a] * M[3 * b] + M[3 * a + 1] * M[3 * b + 1] + M[3 * a + 2] * M[3 * b + 2];
+    float S0[3], S1[3];   // Sigma T0, Sigma T1
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      S0[k] = Sg[3 * k] * T0[0] + Sg[3 * k + 1] * T0[1] + Sg[3 * k + 2] * T0[2];
+      S1[k] = Sg[3 * k] * T1[0] + Sg[3 * k + 1] * T1[1] + Sg[3 * k + 2] * T1[2];
+    }
+    const float a = dot3f(T0, S0) + kLowPass, b = dot3f(T1, S0), c = dot3f(T1, S1) + kLowPass;
+    const float det = a * c - b * b;
+    if (det > 0.f && z > 0.f) {
+      // conic = (c, -b, a) / det
+      const float id = 1.f / det;
+      const float common = (gca * c - gcb * b + gcc * a) * id * id;
+      const float da = gcc * id - common * c;
+      const float dc = gca * id - common * a;
+      const float db = -gcb * id + common * 2.f * b;
+      // (a, b, c) -> T0, T1, Sigma
+      float dT0[3], dT1[3];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        dT0[k] = 2.f * da * S0[k] + db * S1[k];
+        dT1[k] = 2.f * dc * S1[k] + db * S0[k];
+      }
+      float dM[9];   // dM = (dSigma + dSigma^T) M, dSigma_ij = da T0_i T0_j + db T1_i T0_j + dc T1_i T1_j
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int col = 0; col < 3; ++col) {
+          float acc = 0.f;
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            const float dsym = 2.f * da * T0[r] * T0[k] + db * (T1[r] * T0[k] + T0[r] * T1[k]) + 2.f * dc * T1[r] * T1[k];
+            acc += dsym * M[3 * k + col];
+          }
+          dM[3 * r + col] = acc;
+        }
+      float dRq[9];
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int col = 0; col < 3; ++col) {
+          dRq[3 * r + col] = dM[3 * r + col] * sc[col];
+          ds[col] += dM[3 * r + col] * Rq[3 * r + col];
+        }
+      dq[0] = 2.f * (-qz * dRq[1] + qy * dRq[2] + qz * dRq[3] - qx * dRq[5] - qy * dRq[6] + qx * dRq[7]);
+      dq[1] = 2.f * (qy * dRq[1] + qz * dRq[2] + qy * dRq[3] - 2.f * qx * dRq[4] - qr * dRq[5] + qz * dRq[6] + qr * dRq[7] - 2.f * qx * dRq[8]);
+      dq[2] = 2.f * (-2.f * qy * dRq[0] + qx * dRq[1] + qr * dRq[2] + qx * dRq[3] + qz * dRq[5] - qr * dRq[6] + qz * dRq[7] - 2.f * qy * dRq[8]);
+      dq[3] = 2.f * (-2.f * qz * dRq[0] - qr * dRq[1] + qx * dRq[2] + qr * dRq[3] - 2.f * qz * dRq[4] + qy * dRq[5] + qx * dRq[6] + qy * dRq[7]);
+      // T -> J entries -> (u, w, z)
+      const float dj00 = dT0[0] * R[0] + dT0[1] * R[1] + dT0[2] * R[2];
+      const float dj02 = dT0[0] * R[6] + dT0[1] * R[7] + dT0[2] * R[8];
+      const float dj11 = dT1[0] * R[3] + dT1[1] * R[4] + dT1[2] * R[5];
+      const float dj12 = dT1[0] * R[6] + dT1[1] * R[7] + dT1[2] * R[8];
+      float du = cam.fx * gpx, dw = cam.fy * gpy, dz = gz;
+      dz += -cam.fx * iz * iz * dj00 - cam.fy * iz * iz * dj11 + cam.fx * ucl * iz * iz * dj02 + cam.fy * wcl * iz * iz * dj12;
+      if (free_x) du += -cam.fx * iz * dj02;
+      if (free_y) dw += -cam.fy * iz * dj12;
+      // (u, w) = (p_x, p_y) / z
+      const float dp[3] = {du * iz, dw * iz, dz - (u * du + w * dw) * iz};
+#pragma unroll
+      for (int k = 0; k < 3; ++k) dmu[k] = R[k] * dp[0] + R[3 + k] * dp[1] + R[6 + k] * dp[2];
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { d_means[3 * i + k] = dmu[k]; d_scales[3 * i + k] = ds[k]; }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) d_rot[4 * i + k] = dq[k];
+}
+
 __global__ void __launch_bounds__(256) zero_kernel(float* p, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (int64_t)gridDim.x * 256) p[i] = 0.f;
 }
@@ -1198,6 +1318,14 @@ int launch_zero(float* p, int64_t n, cudaStream_t s) {
   int64_t blocks = (n + 255) / 256;
   if (blocks > 148 * 8) blocks = 148 * 8;
   zero_kernel<<<(unsigned)blocks, 256, 0, s>>>(p, n);
+  return 1;
+}
+
+int launch_project_backward(const sssgs_gaussians& g, const CamParams& cam, const float* g_mean2d, const float* g_conic,
+                            const float* g_depth, float* d_means, float* d_scales, float* d_rot, cudaStream_t s) {
+  if (g.n == 0) return 0;
+  project_backward_kernel<<<(unsigned)((g.n + 255) / 256), 256, 0, s>>>(g.n, g.means, g.scales, g.rotations, cam, g_mean2d,
+                                                                       g_conic, g_depth, d_means, d_scales, d_rot);
   return 1;
 }
 

@@ -697,6 +697,10 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   for (const void* p : per_light)   // per-light arrays are empty without lights
     if (n_light > 0 && (!p || !aligned16(p))) return fail(c, SSSGS_EINVAL, "a per-light gradient pointer is NULL or not 16-byte aligned");
   if (gr->grad_params && !aligned16(gr->grad_params)) return fail(c, SSSGS_EINVAL, "grad_params misaligned");
+  const int n_geo = (gr->grad_means ? 1 : 0) + (gr->grad_scales ? 1 : 0) + (gr->grad_rotations ? 1 : 0);
+  if (n_geo != 0 && n_geo != 3) return fail(c, SSSGS_EINVAL, "grad_means, grad_scales and grad_rotations: all three or none");
+  if (n_geo == 3 && (!aligned16(gr->grad_means) || !aligned16(gr->grad_scales) || !aligned16(gr->grad_rotations)))
+    return fail(c, SSSGS_EINVAL, "grad_means / grad_scales / grad_rotations misaligned");
   if (g->n > 0) {
     const void* req[] = {g->means, g->scales, g->rotations, g->opacities, g->normals, g->base_color,
                          g->roughness, g->metallic, g->subsurface, g->vis_sh};
@@ -739,7 +743,15 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   launches += launch_zero(gr->grad_attr, n * 9, s);
   if (gr->grad_params) launches += launch_zero(gr->grad_params, (int64_t)(mlp->params_bytes / 4), s);
   launches += launch_zero(gr->grad_gbuffer, (int64_t)n_light * npix * 16, s);
-  if (n == 0 || n_light == 0) { c->launches = launches; return SSSGS_OK; }
+  if (n == 0 || n_light == 0) {
+    if (n_geo == 3) {
+      launches += launch_zero(gr->grad_means, n * 3, s);
+      launches += launch_zero(gr->grad_scales, n * 3, s);
+      launches += launch_zero(gr->grad_rotations, n * 4, s);
+    }
+    c->launches = launches;
+    return SSSGS_OK;
+  }
   // ---- forward state: attributes, geometry of the camera (as sssgs_render) -------------------------
   launches += launch_pack_attr(*g, c->attr, s);
   if (run_mlp) launches += launch_mlp_pack(*mlp, plan, c->mlp_blob, s);
@@ -793,6 +805,10 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
                                       reinterpret_cast<uint32_t*>(c->mlp_out[1]), cnt + DC_BWD_ROWS, c->bwd_blob,
                                       l0 == 0, (flags & SSSGS_BACKWARD_FP32) != 0, c->num_sms, s);
   }
+  // ---- a3 backward: the accumulated 2-D gradients through the projection ---------------------------
+  if (n_geo == 3)
+    launches += launch_project_backward(*g, cam, gr->grad_mean2d, gr->grad_conic, gr->grad_depth, gr->grad_means,
+                                        gr->grad_scales, gr->grad_rotations, s);
   c->launches = launches;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(c, SSSGS_ECUDA, "CUDA error: %s", cudaGetErrorString(e));

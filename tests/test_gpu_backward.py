@@ -172,6 +172,57 @@ def test_mlp_backward_tensor_core_shapes(trunk, act):
         assert e <= (5e-5 if fp32 else 1e-3)
 
 
+@pytest.mark.parametrize("n,w,h,lights", [(400, 40, 32, 2), (6000, 150, 100, 3)])
+def test_projection_backward(n, w, h, lights):
+    """Step a3 differentiated: (1) in isolation, the GPU's dL/d(mean, scale, rotation) against the oracle's reverse
+    mode of the projection fed the GPU's OWN dL/d(pix, conic, depth); (2) the whole chain given MLP outputs against
+    render_backward(through_projection)."""
+    s = _scene(n, w, h, lights)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    rng = np.random.default_rng(31 + n)
+    G = rng.standard_normal((lights, cam.height, cam.width, 3))
+    G[:, comp.unstable] = 0.0
+    mo32 = mo.astype(np.float32)
+    out = _gpu(s, G, precomputed=mo32)
+    dm, dsc, dq = ob.project_backward(s, cam, proj.visible, out["grad_mean2d"][:s.n], out["grad_conic"][:s.n],
+                                      out["grad_depth"][:s.n])
+    e = {"means": _rel(out["grad_means"][:s.n], dm), "scales": _rel(out["grad_scales"][:s.n], dsc),
+         "rotations": _rel(out["grad_rotations"][:s.n], dq)}
+    print(f"projection backward alone n={n}:", {k: f"{v:.2e}" for k, v in e.items()})
+    # fp32 evaluation of a rational function of the inputs: measured 3e-7 of the largest gradient, bar 5e-6
+    assert max(e.values()) <= 5e-6
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, given_mlp_out=mo32.astype(np.float64), through_projection=True)
+    e2 = {"means": _rel(out["grad_means"][:s.n], r.d_means), "scales": _rel(out["grad_scales"][:s.n], r.d_scales),
+          "rotations": _rel(out["grad_rotations"][:s.n], r.d_rotations)}
+    print(f"chain through the projection n={n}:", {k: f"{v:.2e}" for k, v in e2.items()})
+    assert max(e2.values()) <= 1e-4
+    assert np.abs(r.d_means).max() > 0 and np.abs(r.d_scales).max() > 0 and np.abs(r.d_rotations).max() > 0
+
+
+def test_projection_backward_with_the_frustum_clamp():
+    """Gaussians whose centre lies beyond 1.3 tan(fov/2) (the Jacobian is evaluated at the clamped position: the
+    clamped coordinate is a constant of the differentiation) but whose footprint reaches into the image, rotated
+    and anisotropic, next to unclamped ones."""
+    from util import custom_scene
+    means = [[2.2, 0.0, 0.3], [-2.3, 0.2, -0.2], [0.1, 0.0, 2.1], [0.3, 0.2, -0.1], [0.0, 0.5, 0.0]]
+    scales = [[0.8, 0.3, 0.5], [0.6, 0.7, 0.2], [0.4, 0.3, 0.9], [0.3, 0.2, 0.1], [0.2, 0.2, 0.3]]
+    q = np.random.default_rng(3).standard_normal((5, 4))
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    s = custom_scene(means, scales, rotations=q, opacities=[0.6, 0.5, 0.7, 0.4, 0.5], width=64, height=64, feat_dim=16)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    p = (np.asarray(s.means, np.float64) @ np.asarray(cam.R, np.float64).T + cam.t)
+    clamped = (np.abs(p[:, 0] / p[:, 2]) > 1.3 * cam.tan_half_fovx) | (np.abs(p[:, 1] / p[:, 2]) > 1.3 * cam.tan_half_fovy)
+    assert clamped[:3].all() and not clamped[3:].any() and (proj.visible != 0).all()
+    G = np.random.default_rng(7).standard_normal((1, 64, 64, 3))
+    G[:, comp.unstable] = 0.0
+    mo32 = mo.astype(np.float32)
+    out = _gpu(s, G, precomputed=mo32)
+    assert (np.abs(out["grad_conic"][:3]).max(axis=1) > 0).all()      # the clamped ones do reach pixels
+    dm, dsc, dq = ob.project_backward(s, cam, proj.visible, out["grad_mean2d"][:5], out["grad_conic"][:5], out["grad_depth"][:5])
+    for got, ref in ((out["grad_means"][:5], dm), (out["grad_scales"][:5], dsc), (out["grad_rotations"][:5], dq)):
+        assert _rel(got, ref) <= 5e-6, (got, ref)
+
+
 def test_backward_full_size_cfg2_sampled_tiles():
     """BASELINE configs[1] at full size, the call bench.py times under `backward` (tight lists, tensor-core MLP
     backward).  The oracle cannot differentiate the whole 512 x 512 frame in seconds, so dL/drgb is non-zero on the
@@ -227,6 +278,15 @@ def test_backward_rejects_bad_arguments():
         larr = (binding.sssgs_light * 1)(binding.make_light(s.lights[0][0]))
         with pytest.raises(binding.SssgsError):
             binding.sssgs_render_backward(R.ctx, R.g, m, binding.make_camera(cam), larr, 1, gr, 0, None)
+        # the three projection gradients: all or none
+        gr2 = binding.sssgs_grads()
+        outs = {k: torch.zeros(64, device="cuda") for k in ("grad_gbuffer", "grad_mlp_out", "grad_opacity", "grad_mean2d",
+                                                                "grad_conic", "grad_depth", "grad_attr", "grad_means")}
+        for k, v in outs.items():
+            setattr(gr2, k, v.data_ptr())
+        gr2.grad_rgb, gr2.gbuffer = G.data_ptr(), gb.data_ptr()
+        with pytest.raises(binding.SssgsError):
+            binding.sssgs_render_backward(R.ctx, R.g, m, binding.make_camera(cam), larr, 1, gr2, 0, None)
         # empty light list: outputs zeroed, no error
         out = R.render_backward(cam, [], G[:0], gb[:0])
         torch.cuda.synchronize()
