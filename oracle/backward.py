@@ -78,6 +78,41 @@ def mlp_torch(x: torch.Tensor, mlp, params: torch.Tensor, mode: int = 0) -> torc
 
 
 # ---------------------------------------------------------------------------------------------------
+# Step 1: the MLP input row (orc_mlp_inputs: Eq. 6 L98, L347), for the gradients that reach the Gaussians
+# through the MLP's inputs
+# ---------------------------------------------------------------------------------------------------
+Y00, Y1 = 0.2820948, 0.4886025
+
+
+def mlp_inputs_torch(means, normals, rotations, scales, vis_sh, feat, cam, light_pos, sh_degree: int):
+    """[n, 40 + F] float64: n (3), sign-canonical (q_r, q_x) (2), scale (3), w_in (3), w_out (3), light distance,
+    SH visibility towards the light clamped to [0, 1], Fourier encoding of mu (24), feature (F).  The clamp and the
+    quaternion sign are constants of the differentiation."""
+    R, t = _t(cam.R), _t(cam.t)
+    pc = -(R.T @ t)
+    sgn = torch.where(rotations[:, 0] < 0, -1.0, 1.0).detach()
+    wi = _t(light_pos)[None, :] - means
+    wo = pc[None, :] - means
+    di = torch.linalg.norm(wi, dim=1)
+    dn = torch.linalg.norm(wo, dim=1)
+    wi = wi / di[:, None]
+    wo = wo / dn[:, None]
+    v = Y00 * vis_sh[:, 0]
+    if sh_degree >= 1:
+        v = v + Y1 * (vis_sh[:, 1] * wi[:, 1] + vis_sh[:, 2] * wi[:, 2] + vis_sh[:, 3] * wi[:, 0])
+    v = torch.clamp(v, 0.0, 1.0)
+    enc = []
+    for k in range(4):
+        fr = float(1 << k) * math.pi
+        enc += [torch.sin(fr * means), torch.cos(fr * means)]
+    cols = [normals, (sgn * rotations[:, 0])[:, None], (sgn * rotations[:, 1])[:, None], scales, wi, wo, di[:, None],
+            v[:, None]] + enc
+    if feat is not None and feat.numel() and feat.shape[1] > 0:
+        cols.append(feat)
+    return torch.cat(cols, dim=1)
+
+
+# ---------------------------------------------------------------------------------------------------
 # Step 3: EWA projection (orc_project_f64: Eq. 2, L64-66), for the gradients w.r.t. mean, scale, rotation
 # ---------------------------------------------------------------------------------------------------
 def project_torch(means, scales, rotations, cam):
@@ -229,15 +264,18 @@ def shade_torch(cam, light_pos, light_intensity, gbuf: torch.Tensor) -> torch.Te
 # The gradients
 # ---------------------------------------------------------------------------------------------------
 def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16,
-                    given_mlp_out=None, mlp_mode: int = 0, through_projection: bool = False):
+                    given_mlp_out=None, mlp_mode: int = 0, through_projection: bool = False,
+                    through_inputs: bool = False):
     """Gradients of L = sum_l <grad_rgb[l], rgb_l> for one view.
 
     proj / vals / ranges: the oracle's projection and tile lists of the view (oracle.project / build_lists);
     mlp_inputs: [L][n, in_dim] float64 (oracle.mlp_inputs per light); grad_rgb [L, H, W, 3].
     mlp_mode: 0 float64 MLP, 2 its binary16-emulating restatement (mlp_torch).
     through_projection: pix / conic / depth are computed from (means, scales, rotations) by project_torch, and
-    d_means [n,3], d_scales [n,3], d_rotations [n,4] are returned too (the MLP inputs stay constants: step a1 is
-    not differentiated).
+    d_means [n,3], d_scales [n,3], d_rotations [n,4] are returned too.
+    through_inputs (needs through_projection): the MLP inputs are computed from the Gaussians by mlp_inputs_torch
+    (step a1) instead of being the constants `mlp_inputs`; d_means / d_scales / d_rotations / d_normals then hold the
+    sums over both paths, and d_feat [n,F], d_vis_sh [n,ncoef] are returned.
     given_mlp_out: [L, n, 4] or None: the MLP outputs are these constants instead of mlp(mlp_inputs) (isolates
     the walks: d_params is then zero).
     Returns a namespace of numpy float64 arrays:
@@ -274,10 +312,18 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
     rough = _t(scene.roughness).requires_grad_(True)
     metal = _t(scene.metallic).requires_grad_(True)
     sss = _t(scene.subsurface).requires_grad_(True)
+    feat_t = vsh_t = None
+    if through_inputs:
+        assert through_projection and given_mlp_out is None
+        feat_t = _t(scene.feat).requires_grad_(True)
+        vsh_t = _t(scene.vis_sh).requires_grad_(True)
     rgbs, gbufs, mlp_outs = [], [], []
     loss = torch.zeros((), dtype=F8)
     for li, lt in enumerate(lights):
-        if given_mlp_out is None:
+        if through_inputs:
+            x_in = mlp_inputs_torch(mu, normals, rot, sc, vsh_t, feat_t, cam, lt.position, scene.vis_sh_degree)
+            mo = mlp_torch(x_in, scene.mlp, params, mode=mlp_mode)
+        elif given_mlp_out is None:
             mo = mlp_torch(_t(mlp_inputs[li]), scene.mlp, params, mode=mlp_mode)
         else:
             mo = _t(given_mlp_out[li]).clone().requires_grad_(True)
@@ -300,4 +346,5 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
         d_params=z(params), d_opacity=z(opac), d_pix=z(pix), d_conic=z(conic), d_depth=z(depth),
         d_normals=z(normals), d_base=z(base), d_rough=z(rough), d_metal=z(metal), d_sss=z(sss),
         d_means=z(mu) if through_projection else None, d_scales=z(sc) if through_projection else None,
-        d_rotations=z(rot) if through_projection else None)
+        d_rotations=z(rot) if through_projection else None,
+        d_feat=z(feat_t) if through_inputs else None, d_vis_sh=z(vsh_t) if through_inputs else None)

@@ -291,3 +291,74 @@ def test_render_backward_through_the_projection_chains():
     np.testing.assert_allclose(r.d_scales, dsc, rtol=1e-9, atol=1e-12)
     np.testing.assert_allclose(r.d_rotations, dq, rtol=1e-9, atol=1e-12)
     assert np.abs(r.d_means).max() > 0 and np.abs(r.d_rotations).max() > 0
+
+
+def test_mlp_input_restatement_and_its_gradient():
+    """mlp_inputs_torch == orc_mlp_inputs (incl. a negative q_r and visibilities clamped at both ends); its
+    reverse-mode gradient == central differences of the C++ function."""
+    s = _scene()
+    rot = np.array(s.rotations, np.float32)
+    rot[::3] *= -1.0                                  # q and -q: the sign-canonical pair changes sign
+    vsh = np.array(s.vis_sh, np.float32)
+    vsh[1::7, 0] += 4.0                               # v > 1: clamped
+    vsh[2::7, 0] -= 4.0                               # v < 0: clamped
+    s = dataclasses.replace(s, rotations=rot, vis_sh=vsh)
+    cam, lt = s.cameras[0], s.lights[0][1]
+    x_ref = oracle.mlp_inputs(s, cam, lt.position)
+    assert (x_ref[:, 15] == 1.0).any() and (x_ref[:, 15] == 0.0).any() and ((x_ref[:, 15] > 0) & (x_ref[:, 15] < 1)).any()
+
+    def xt(sc_, leaf=None):
+        t = {k: ob._t(getattr(sc_, k)) for k in ("means", "normals", "rotations", "scales", "vis_sh", "feat")}
+        if leaf:
+            t[leaf].requires_grad_(True)
+        return t, ob.mlp_inputs_torch(t["means"], t["normals"], t["rotations"], t["scales"], t["vis_sh"], t["feat"], cam,
+                                      lt.position, sc_.vis_sh_degree)
+    np.testing.assert_allclose(xt(s)[1].numpy(), x_ref, rtol=1e-12, atol=1e-13)
+    rng = np.random.default_rng(9)
+    gx = rng.standard_normal(x_ref.shape)
+    for field in ("means", "normals", "rotations", "scales", "vis_sh", "feat"):
+        t, x = xt(s, field)
+        (x * ob._t(gx)).sum().backward()
+        grad = t[field].grad.numpy()
+        base = np.array(getattr(s, field), np.float32)
+        for i in (0, 1, 2, 3, 7):
+            for k in range(min(base.shape[1], 4)):
+                h = np.float32(2.0 ** -10) * max(1e-2, abs(float(base[i, k])))
+                hi, lo = base.copy(), base.copy()
+                hi[i, k] += h
+                lo[i, k] -= h
+                if field == "rotations" and (hi[i, 0] < 0) != (lo[i, 0] < 0):
+                    continue                              # the canonical sign flips inside the step
+                f = lambda b: float((oracle.mlp_inputs(dataclasses.replace(s, **{field: b}), cam, lt.position) * gx).sum())  # noqa: E731
+                num = (f(hi) - f(lo)) / (float(hi[i, k]) - float(lo[i, k]))
+                assert abs(num - grad[i, k]) <= 1e-4 * max(1.0, np.abs(grad[i]).max()), (field, i, k, num, grad[i, k])
+
+
+def test_render_backward_through_the_inputs_equals_finite_differences():
+    """through_inputs: dL/d(feat, vis_sh, normals) of the WHOLE chain (inputs -> MLP -> compositing -> shading) ==
+    central differences of the C++ forward oracle with the inputs recomputed by orc_mlp_inputs."""
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    rng = np.random.default_rng(21)
+    G = rng.standard_normal((2, cam.height, cam.width, 3))
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, through_projection=True, through_inputs=True)
+    r0 = ob.render_backward(s, proj, vals, ranges, xs, G, through_projection=True)
+    np.testing.assert_allclose(r.rgb, r0.rgb, rtol=0, atol=1e-12)
+    assert np.abs(r.d_means - r0.d_means).max() > 0            # the inputs add their share
+
+    def loss(sc_):
+        xs_ = [oracle.mlp_inputs(sc_, cam, lt.position) for lt in sc_.lights[0]]
+        return _cpp_loss(sc_, proj, vals, ranges, xs_, G)
+
+    for field, grad in (("feat", r.d_feat), ("vis_sh", r.d_vis_sh), ("normals", r.d_normals)):
+        flat = np.abs(grad).ravel()
+        for j in np.argsort(-flat)[:4]:
+            i, k = np.unravel_index(j, grad.shape)
+            base = np.array(getattr(s, field), np.float32)
+            h = np.float32(2.0 ** -8) * max(1e-2, abs(float(base[i, k])))
+            hi, lo = base.copy(), base.copy()
+            hi[i, k] += h
+            lo[i, k] -= h
+            num = (loss(dataclasses.replace(s, **{field: hi})) - loss(dataclasses.replace(s, **{field: lo}))) \
+                / (float(hi[i, k]) - float(lo[i, k]))
+            assert abs(num - grad[i, k]) <= 2e-3 * abs(grad[i, k]) + 1e-6, (field, i, k, num, grad[i, k])
