@@ -295,6 +295,12 @@ typedef struct {
   float* grad_means;         /* [n][3]  dL / d mu                                      (out, may be NULL)  */
   float* grad_scales;        /* [n][3]  dL / d s (activated scales, as given)          (out, may be NULL)  */
   float* grad_rotations;     /* [n][4]  dL / d q (r, x, y, z), the quaternion as given (out, may be NULL)  */
+  /* step a1 differentiated (Eq. 6: the MLP's input row): both or none (NULL); they need the
+     three above and the MLP to run (no precomputed_out).  The gradients that reach the Gaussian through the MLP's
+     inputs are then ADDED to grad_means / grad_scales / grad_rotations and to the normal in grad_attr; the
+     clamp of the visibility to [0, 1] and the sign of the canonical quaternion are constants.                   */
+  float* grad_feat;          /* [n][feat_dim]            dL / d feat                   (out, may be NULL)  */
+  float* grad_vis_sh;        /* [n][(vis_sh_degree+1)^2] dL / d vis_sh                 (out, may be NULL)  */
 } sssgs_grads;
 int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
                           const sssgs_camera* cam, const sssgs_light* lights, int n_light,

@@ -84,7 +84,7 @@ class sssgs_out(ctypes.Structure):
 class sssgs_grads(ctypes.Structure):
     _fields_ = [(k, _vp) for k in ("grad_rgb", "gbuffer", "grad_gbuffer", "grad_mlp_out", "grad_params",
                                    "grad_opacity", "grad_mean2d", "grad_conic", "grad_depth", "grad_attr",
-                                   "grad_means", "grad_scales", "grad_rotations")]
+                                   "grad_means", "grad_scales", "grad_rotations", "grad_feat", "grad_vis_sh")]
 
 
 class sssgs_bake(ctypes.Structure):
@@ -340,7 +340,8 @@ class Renderer:
                      (SSSGS_FORWARD_SHADING if forward else 0) | (SSSGS_TIGHT_LISTS if tight else 0), st)
         return outputs
 
-    def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None, fp32=False):
+    def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None, fp32=False,
+                        through_inputs=False):
         """Enqueue one sssgs_render_backward: cam one scene camera, lights its lights, grad_rgb [L,H,W,3] and
         gbuffer [L,H,W,16] device tensors (the forward call's G-buffer).  Returns the dict of gradient tensors."""
         torch = self.torch
@@ -349,6 +350,9 @@ class Renderer:
         out = {"grad_gbuffer": z(L, H, W, 16), "grad_mlp_out": z(L, n, 4), "grad_params": z(self.params.numel()),
                "grad_opacity": z(n), "grad_mean2d": z(n, 2), "grad_conic": z(n, 3), "grad_depth": z(n),
                "grad_attr": z(n, 9), "grad_means": z(n, 3), "grad_scales": z(n, 3), "grad_rotations": z(n, 4)}
+        if through_inputs:   # step a1: the gradients through the MLP's inputs (added to means / scales / rotations / normal)
+            out["grad_feat"] = z(n, max(self.feat_dim, 1))
+            out["grad_vis_sh"] = z(n, (self.scene.vis_sh_degree + 1) ** 2)
         gr = sssgs_grads()
         self._bwd_in = (grad_rgb.contiguous(), gbuffer.contiguous())
         gr.grad_rgb, gr.gbuffer = self._bwd_in[0].data_ptr(), self._bwd_in[1].data_ptr()

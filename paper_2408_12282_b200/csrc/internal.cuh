@@ -312,7 +312,7 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
 constexpr size_t kBwdBlobBytes = 4 * 32768 + 4096 + 5 * 512;
 int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
                         int n_lights, const float* g_mlp_out, float* g_params, uint32_t* row_list, uint32_t* row_count,
-                        uint8_t* blob, bool pack, bool force_fp32, int num_sms, cudaStream_t s);
+                        uint8_t* blob, bool pack, bool force_fp32, float* const input_grads[6], int num_sms, cudaStream_t s);
 
 int mlp_smem_bytes(const MlpPlan& plan);
 

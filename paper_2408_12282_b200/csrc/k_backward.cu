@@ -1,4 +1,5 @@
-// Backward pass of hot-path steps a8 (deferred shading), a7 (compositing), a2 (the MLP) and a3 (projection)
+// Backward pass of hot-path steps a8 (deferred shading), a7 (compositing), a2 (the MLP), a3 (projection) and a1
+// (the MLP's input assembly)
 // ("optimize all parameters jointly via raytraced differentiable rendering",
 // L112, L343-349: the losses are functions of the rendered image and of the rasterised property images).
 //
@@ -451,6 +452,132 @@ __device__ __forceinline__ void mlp_input_row(const sssgs_gaussians& g, int64_t 
   for (int k = 0; k < g.feat_dim; ++k) x[40 + k] = g.feat[(int64_t)g.feat_dim * i + k];
 }
 
+// ---- a1 backward: dL/d(input row) -> the Gaussian -----------------------------------------------------------
+// Where the gradients that arrive at the MLP's inputs go (all outputs are accumulated with atomics; NULL feat /
+// vis_sh = the whole step is off).
+struct InputGrads {
+  float* means;      // [n][3]
+  float* scales;     // [n][3]
+  float* rotations;  // [n][4]
+  float* attr;       // [n][9]: the normal is entries 0..2
+  float* feat;       // [n][F]
+  float* vis_sh;     // [n][ncoef]
+};
+// The row's quantities the Jacobian of mlp_input_geo needs, recomputed from the Gaussian (L2-hot).
+struct InputCtx {
+  float mu[3], wi[3], wo[3], di, dn, sgn, sh[4];
+  bool v_free, deg1;
+};
+__device__ __forceinline__ void input_ctx(const sssgs_gaussians& g, int64_t i, const float* cam_pos, const float* light_pos,
+                                          InputCtx& c) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    c.mu[k] = g.means[3 * i + k];
+    c.wi[k] = light_pos[k] - c.mu[k];
+    c.wo[k] = cam_pos[k] - c.mu[k];
+  }
+  c.di = sqrtf(dot3f(c.wi, c.wi));
+  c.dn = sqrtf(dot3f(c.wo, c.wo));
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { c.wi[k] /= c.di; c.wo[k] /= c.dn; }
+  c.sgn = g.rotations[4 * i] < 0.f ? -1.f : 1.f;
+  c.deg1 = g.vis_sh_degree >= 1;
+  const int nc = c.deg1 ? 4 : 1;
+  c.sh[0] = g.vis_sh[nc * i];
+#pragma unroll
+  for (int k = 1; k < 4; ++k) c.sh[k] = c.deg1 ? g.vis_sh[nc * i + k] : 0.f;
+  const float v = 0.2820948f * c.sh[0] + 0.4886025f * (c.sh[1] * c.wi[1] + c.sh[2] * c.wi[2] + c.sh[3] * c.wi[0]);
+  c.v_free = v > 0.f && v < 1.f;
+}
+// Partial sums of one thread's columns of a row.
+struct InputAcc { float mu[3], nrm[3], q[2], s[3], sh[4]; };
+__device__ __forceinline__ void input_acc_zero(InputAcc& a) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) a.mu[k] = a.nrm[k] = a.s[k] = 0.f;
+  a.q[0] = a.q[1] = 0.f;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) a.sh[k] = 0.f;
+}
+// d(mu) of a gradient dw arriving at the unit vector w = (p - mu) / dist
+__device__ __forceinline__ void unit_dir_back(const float* w, float dist, const float* dw, float* dmu) {
+  const float proj = dot3f(w, dw);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dmu[k] -= (dw[k] - w[k] * proj) / dist;
+}
+// Columns c0 .. c0 + cnt - 1 (< 40) of dL/d(input row): v[k] is the gradient of column c0 + k.
+__device__ __forceinline__ void input_cols_back(const InputCtx& c, int c0, int cnt, const float* v, InputAcc& a) {
+  float dwi[3] = {0.f, 0.f, 0.f}, dwo[3] = {0.f, 0.f, 0.f};
+  bool any_wi = false, any_wo = false;
+  for (int k = 0; k < cnt; ++k) {
+    const int col = c0 + k;
+    const float x = v[k];
+    if (col < 3) a.nrm[col] += x;
+    else if (col < 5) a.q[col - 3] += c.sgn * x;
+    else if (col < 8) a.s[col - 5] += x;
+    else if (col < 11) { dwi[col - 8] += x; any_wi = true; }
+    else if (col < 14) { dwo[col - 11] += x; any_wo = true; }
+    else if (col == 14) {
+#pragma unroll
+      for (int q = 0; q < 3; ++q) a.mu[q] -= x * c.wi[q];          // d = |L - mu|
+    } else if (col == 15) {
+      if (c.v_free) {                                               // the clamp to [0, 1] is a constant elsewhere
+        a.sh[0] += 0.2820948f * x;
+        if (c.deg1) {
+          a.sh[1] += 0.4886025f * c.wi[1] * x;
+          a.sh[2] += 0.4886025f * c.wi[2] * x;
+          a.sh[3] += 0.4886025f * c.wi[0] * x;
+          dwi[0] += 0.4886025f * c.sh[3] * x;
+          dwi[1] += 0.4886025f * c.sh[1] * x;
+          dwi[2] += 0.4886025f * c.sh[2] * x;
+          any_wi = true;
+        }
+      }
+    } else if (col < 40) {                                          // Fourier encoding of mu
+      const int j = col - 16, oct = j / 6, w6 = j - 6 * oct, ax = w6 % 3;
+      const float fr = (float)(1 << oct);
+      float sn, cs;
+      sincospif(fr * c.mu[ax], &sn, &cs);
+      a.mu[ax] += (w6 < 3 ? cs : -sn) * fr * kPiF * x;
+    }
+  }
+  if (any_wi) unit_dir_back(c.wi, c.di, dwi, a.mu);
+  if (any_wo) unit_dir_back(c.wo, c.dn, dwo, a.mu);
+}
+__device__ __forceinline__ void input_acc_flush(const InputAcc& a, const InputGrads& o, int64_t i, bool deg1) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    if (a.mu[k] != 0.f) atomicAdd(&o.means[3 * i + k], a.mu[k]);
+    if (a.nrm[k] != 0.f) atomicAdd(&o.attr[9 * i + k], a.nrm[k]);
+    if (a.s[k] != 0.f) atomicAdd(&o.scales[3 * i + k], a.s[k]);
+  }
+  if (a.q[0] != 0.f) atomicAdd(&o.rotations[4 * i], a.q[0]);
+  if (a.q[1] != 0.f) atomicAdd(&o.rotations[4 * i + 1], a.q[1]);
+  const int nc = deg1 ? 4 : 1;
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    if (k < nc && a.sh[k] != 0.f) atomicAdd(&o.vis_sh[nc * i + k], a.sh[k]);
+}
+// One call per (row, run of columns): geometric columns through the Jacobian, feature columns straight through.
+__device__ __forceinline__ void input_row_back(const sssgs_gaussians& g, int64_t i, const float* cam_pos, const float* light_pos,
+                                               int c0, int cnt, const float* v, const InputGrads& o) {
+  bool any = false;
+  for (int k = 0; k < cnt; ++k) any = any || v[k] != 0.f;
+  if (!any) return;
+  const int geo = c0 < 40 ? min(cnt, 40 - c0) : 0;
+  if (geo > 0) {
+    InputCtx ctx;
+    input_ctx(g, i, cam_pos, light_pos, ctx);
+    InputAcc acc;
+    input_acc_zero(acc);
+    input_cols_back(ctx, c0, geo, v, acc);
+    input_acc_flush(acc, o, i, ctx.deg1);
+  }
+  for (int k = geo; k < cnt; ++k) {
+    const int f = c0 + k - 40;
+    if (f < g.feat_dim && v[k] != 0.f) atomicAdd(&o.feat[(int64_t)g.feat_dim * i + f], v[k]);
+  }
+}
+
 // Layer table of the MLP in the caller's parameter packing (sssgs_mlp.params, fp32).
 struct BwdLayer { int w, b, out, in, src, kind; };   // src: index of the layer whose output feeds this one (-1: x)
 struct BwdNet {
@@ -502,7 +629,7 @@ __device__ __forceinline__ float dot4(const float4 a, const float4 b, float s) {
 __global__ void __launch_bounds__(256, 1)
 mlp_backward_kernel(sssgs_gaussians g, BwdNet net, const float* __restrict__ params, CamParams cam, LightBatch lights,
                     int64_t n, const uint32_t* __restrict__ list, const uint32_t* __restrict__ count,
-                    const float* __restrict__ g_mlp_out, float* __restrict__ g_params) {
+                    const float* __restrict__ g_mlp_out, float* __restrict__ g_params, InputGrads ig) {
   extern __shared__ __align__(16) float bw_smem[];
   float* sW = bw_smem;                           // [128][kWS]
   float* sGA = sW + 128 * kWS;                   // [kBR][128] gradient wrt a trunk layer's output
@@ -647,6 +774,44 @@ mlp_backward_kernel(sssgs_gaussians g, BwdNet net, const float* __restrict__ par
       }
     }
     __syncthreads();
+    // ---- a1: dL/dx = delta_0 W_0, pushed through the input assembly (CTAs of target 0 only) ----
+    if (target == 0 && ig.feat != nullptr) {
+      const BwdLayer L0 = net.L[0];
+      stage_weights(L0);
+      float s2[4][2];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) s2[r][0] = s2[r][1] = 0.f;
+      const int out4 = (L0.out + 3) & ~3;
+      for (int o = 0; o < out4; o += 4) {
+        float4 d4[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) d4[r] = *reinterpret_cast<const float4*>(sD + (4 * rg + r) * 128 + o);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float2 w = *reinterpret_cast<const float2*>(sW + (o + j) * kWS + 2 * oc);
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const float d = j == 0 ? d4[r].x : j == 1 ? d4[r].y : j == 2 ? d4[r].z : d4[r].w;
+            s2[r][0] = fmaf(d, w.x, s2[r][0]);
+            s2[r][1] = fmaf(d, w.y, s2[r][1]);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) *reinterpret_cast<float2*>(sGB + (4 * rg + r) * 128 + 2 * oc) = make_float2(s2[r][0], s2[r][1]);
+      __syncthreads();
+      // thread = (row, run of 8 columns)
+      const int r = tid >> 4, c0 = (tid & 15) * 8;
+      const unsigned ridx = tile * kBR + r;
+      if (ridx < nrows && c0 < net.in_dim) {
+        const uint32_t idx = list[ridx];
+        float v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = c0 + k < net.in_dim ? sGB[r * 128 + c0 + k] : 0.f;
+        input_row_back(g, (int64_t)(idx % n), cam.pos, lights.l[idx / n].pos, c0, min(8, net.in_dim - c0), v, ig);
+      }
+      __syncthreads();
+    }
     // ---- dW[o][i] += sum_r D[r][o] h[r][i],  db[o] += sum_r D[r][o] ----
     const float* hsrc = sAct + (size_t)(T.src + 1) * kBR * 128;
 #pragma unroll 2
@@ -874,6 +1039,7 @@ struct TcArgs {
   const float* g_mlp_out;      // [n_lights][n][4]
   const uint8_t* blob;         // bwd_pack_kernel's output
   float* g_params;
+  InputGrads ig;               // a1 backward (feat == nullptr: off)
 };
 
 __host__ __device__ inline int tc_smem_bytes(int n_trunk) {
@@ -935,6 +1101,7 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
   int e = (int)(mbits >> 23) - 127;
   e = e < -100 ? -100 : (e > 100 ? 100 : e);
   const float scale = __uint_as_float((uint32_t)(126 - e) << 23), inv_scale = __uint_as_float((uint32_t)(128 + e) << 23);
+  const bool want_x = a.ig.feat != nullptr;
   const bool leaky = net.activation == SSSGS_ACT_LEAKY_RELU;
   const float neg_slope = leaky ? net.slope : 0.f;
   float db = 0.f;
@@ -1116,7 +1283,7 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
             w[i] = pack_f16(((bits >> (2 * i)) & 1u) ? lo : neg_slope * lo, ((bits >> (2 * i + 1)) & 1u) ? hi : neg_slope * hi);
           }
           if (l == t) store_row16(sDelta, c0, w);
-          else tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);
+          if (l != t || (t == 0 && want_x)) tmem_st8(tA + lane_off + (uint32_t)(c0 >> 1), w);   // delta_0 also feeds dL/dx
         });
         if (l == t) break;
         publish(false);
@@ -1139,6 +1306,11 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
       for (int ks = 0; ks < kRowsT / 16; ++ks)
         umma_ss(tDW, make_desc(sDelta_addr + ks * 2048, 16384, 1024), make_desc(sH_addr + ks * 2048, 16384, 1024), idesc,
                 (tiles_done > 0 || ks > 0) ? 1u : 0u, issue);
+      if (t == 0 && want_x) {   // a1: dL/dx = delta_0 W_0 (the layer-0 tile read MN-major), into the free accumulator
+        const uint32_t idx_ = make_idesc(net.k0_pad, false, true);
+        for (int ks = 0; ks < net.out[0] / 16; ++ks)
+          umma_ts(tD, tA + ks * 8, make_desc(sW_addr + ks * 2048, 16384, 1024), idx_, ks > 0, issue);
+      }
       umma_commit_if(bar, issue);
     }
     {   // db_t[f] += sum over the rows of delta_t[row][f], f = tid (read while the MMAs run)
@@ -1147,6 +1319,19 @@ __global__ void __launch_bounds__(256, 1) mlp_backward_tc_kernel(const __grid_co
       db += s;
     }
     wait_mma();   // the operand tiles are free again
+    if (t == 0 && want_x) {   // dL/dx of this thread's column groups, through the input assembly to the Gaussian
+      for_groups(tD + lane_off, 16 * half, net.k0_pad, [&](const uint32_t* r, int c0, int) {
+        if (gi >= 0 && c0 < net.in_dim) {
+          float v[16];
+#pragma unroll
+          for (int k = 0; k < 16; ++k) v[k] = c0 + k < net.in_dim ? __uint_as_float(r[k]) * inv_scale : 0.f;
+          input_row_back(a.g, gi, a.cam.pos, a.lights.l[li].pos, c0, min(16, net.in_dim - c0), v, a.ig);
+        }
+      });
+      tc_fence_before();
+      __syncthreads();   // every thread has read the accumulator before the next tile's MMAs overwrite it
+      tc_fence_after();
+    }
     ++tiles_done;
     TL(4);
   }
@@ -1301,10 +1486,11 @@ project_backward_kernel(int64_t n, const float* __restrict__ means, const float*
       for (int k = 0; k < 3; ++k) dmu[k] = R[k] * dp[0] + R[3 + k] * dp[1] + R[6 + k] * dp[2];
     }
   }
+  // added to what the a1 backward may have accumulated (the arrays start from zero)
 #pragma unroll
-  for (int k = 0; k < 3; ++k) { d_means[3 * i + k] = dmu[k]; d_scales[3 * i + k] = ds[k]; }
+  for (int k = 0; k < 3; ++k) { d_means[3 * i + k] += dmu[k]; d_scales[3 * i + k] += ds[k]; }
 #pragma unroll
-  for (int k = 0; k < 4; ++k) d_rot[4 * i + k] = dq[k];
+  for (int k = 0; k < 4; ++k) d_rot[4 * i + k] += dq[k];
 }
 
 __global__ void __launch_bounds__(256) zero_kernel(float* p, int64_t n) {
@@ -1358,8 +1544,11 @@ int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuff
 
 int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const CamParams& cam, const LightBatch& lights,
                         int n_lights, const float* g_mlp_out, float* g_params, uint32_t* row_list, uint32_t* row_count,
-                        uint8_t* blob, bool pack, bool force_fp32, int num_sms, cudaStream_t s) {
+                        uint8_t* blob, bool pack, bool force_fp32, float* const input_grads[6], int num_sms, cudaStream_t s) {
   if (g.n == 0 || n_lights == 0 || !g_params) return 0;
+  InputGrads ig;   // means, scales, rotations, attr, feat, vis_sh
+  ig.means = input_grads[0]; ig.scales = input_grads[1]; ig.rotations = input_grads[2]; ig.attr = input_grads[3];
+  ig.feat = input_grads[4]; ig.vis_sh = input_grads[5];
   int launches = 0;
   const int64_t rows = g.n * n_lights;
   if (cudaMemsetAsync(row_count, 0, 8, s) != cudaSuccess) return 0;
@@ -1400,7 +1589,7 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
     tc::TcArgs a;
     a.g = g; a.net = net; a.cam = cam; a.lights = lights; a.n = g.n;
     a.list = row_list; a.count = row_count; a.gomax_bits = row_count + 1;
-    a.g_mlp_out = g_mlp_out; a.blob = blob; a.g_params = g_params;
+    a.g_mlp_out = g_mlp_out; a.blob = blob; a.g_params = g_params; a.ig = ig;
     int gx = num_sms / (net.n_trunk + 1);
     if (gx < 1) gx = 1;
     tc::mlp_backward_tc_kernel<<<dim3((unsigned)gx, (unsigned)(net.n_trunk + 1)), 256, smem, s>>>(a);
@@ -1442,7 +1631,7 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
   int gx = num_sms / nl;
   if (gx < 1) gx = 1;
   mlp_backward_kernel<<<dim3((unsigned)gx, (unsigned)nl), 256, smem, s>>>(g, net, (const float*)mlp.params, cam, lights, g.n,
-                                                                        row_list, row_count, g_mlp_out, g_params);
+                                                                        row_list, row_count, g_mlp_out, g_params, ig);
   return launches + 1;
 }
 

@@ -701,6 +701,10 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   if (n_geo != 0 && n_geo != 3) return fail(c, SSSGS_EINVAL, "grad_means, grad_scales and grad_rotations: all three or none");
   if (n_geo == 3 && (!aligned16(gr->grad_means) || !aligned16(gr->grad_scales) || !aligned16(gr->grad_rotations)))
     return fail(c, SSSGS_EINVAL, "grad_means / grad_scales / grad_rotations misaligned");
+  const int n_in = (gr->grad_feat ? 1 : 0) + (gr->grad_vis_sh ? 1 : 0);
+  if (n_in == 1) return fail(c, SSSGS_EINVAL, "grad_feat and grad_vis_sh: both or none");
+  if (n_in == 2 && (n_geo != 3 || !gr->grad_params || mlp->precomputed_out || !aligned16(gr->grad_feat) || !aligned16(gr->grad_vis_sh)))
+    return fail(c, SSSGS_EINVAL, "grad_feat / grad_vis_sh need grad_means, grad_scales, grad_rotations, grad_params and the MLP (no precomputed_out), 16-byte aligned");
   if (g->n > 0) {
     const void* req[] = {g->means, g->scales, g->rotations, g->opacities, g->normals, g->base_color,
                          g->roughness, g->metallic, g->subsurface, g->vis_sh};
@@ -743,15 +747,17 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   launches += launch_zero(gr->grad_attr, n * 9, s);
   if (gr->grad_params) launches += launch_zero(gr->grad_params, (int64_t)(mlp->params_bytes / 4), s);
   launches += launch_zero(gr->grad_gbuffer, (int64_t)n_light * npix * 16, s);
-  if (n == 0 || n_light == 0) {
-    if (n_geo == 3) {
-      launches += launch_zero(gr->grad_means, n * 3, s);
-      launches += launch_zero(gr->grad_scales, n * 3, s);
-      launches += launch_zero(gr->grad_rotations, n * 4, s);
-    }
-    c->launches = launches;
-    return SSSGS_OK;
+  if (n_geo == 3) {   // the a1 backward accumulates into these, the projection backward adds to them
+    launches += launch_zero(gr->grad_means, n * 3, s);
+    launches += launch_zero(gr->grad_scales, n * 3, s);
+    launches += launch_zero(gr->grad_rotations, n * 4, s);
   }
+  const int ncoef = (g->vis_sh_degree + 1) * (g->vis_sh_degree + 1);
+  if (n_in == 2) {
+    launches += launch_zero(gr->grad_feat, n * g->feat_dim, s);
+    launches += launch_zero(gr->grad_vis_sh, n * ncoef, s);
+  }
+  if (n == 0 || n_light == 0) { c->launches = launches; return SSSGS_OK; }
   // ---- forward state: attributes, geometry of the camera (as sssgs_render) -------------------------
   launches += launch_pack_attr(*g, c->attr, s);
   if (run_mlp) launches += launch_mlp_pack(*mlp, plan, c->mlp_blob, s);
@@ -777,6 +783,8 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   const uint32_t* sorted_tiles = c->gb.ikeys[fi];
   const uint32_t* sorted_vals = c->gb.ivals[fi];
   launches += launch_ranges(sorted_tiles, cam, c->gb, cap, nullptr, nullptr, 0, s);
+  float* const input_grads[6] = {gr->grad_means, gr->grad_scales, gr->grad_rotations, gr->grad_attr,
+                                 n_in == 2 ? gr->grad_feat : nullptr, n_in == 2 ? gr->grad_vis_sh : nullptr};
   // ---- per light batch -----------------------------------------------------------------------------
   for (int l0 = 0; l0 < n_light; l0 += c->max_lb) {
     const int nl = n_light - l0 < c->max_lb ? n_light - l0 : c->max_lb;
@@ -803,7 +811,7 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
     if (run_mlp && gr->grad_params)
       launches += launch_mlp_backward(*g, *mlp, cam, lb, nl, gr->grad_mlp_out + (int64_t)l0 * n * 4, gr->grad_params,
                                       reinterpret_cast<uint32_t*>(c->mlp_out[1]), cnt + DC_BWD_ROWS, c->bwd_blob,
-                                      l0 == 0, (flags & SSSGS_BACKWARD_FP32) != 0, c->num_sms, s);
+                                      l0 == 0, (flags & SSSGS_BACKWARD_FP32) != 0, input_grads, c->num_sms, s);
   }
   // ---- a3 backward: the accumulated 2-D gradients through the projection ---------------------------
   if (n_geo == 3)

@@ -45,7 +45,7 @@ def _rel(got, ref):
     return float(np.abs(np.asarray(got, np.float64) - ref).max() / max(np.abs(ref).max(), 1e-30))
 
 
-def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False):
+def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False, through_inputs=False):
     import torch
     from paper_2408_12282_b200 import binding
     R = binding.Renderer(s)
@@ -54,7 +54,7 @@ def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False):
         pre = None if precomputed is None else torch.from_numpy(np.ascontiguousarray(precomputed, np.float32)).cuda()
         fwd = R.render(cams=[cam], lights=lights, want=("rgb", "gbuffer", "mlp_out"), precomputed=pre, tight=tight)
         g = R.render_backward(cam, lights, torch.from_numpy(np.ascontiguousarray(G, np.float32)).cuda(), fwd["gbuffer"],
-                              tight=tight, precomputed=pre, fp32=fp32)
+                              tight=tight, precomputed=pre, fp32=fp32, through_inputs=through_inputs)
         torch.cuda.synchronize()
         launches = R.launch_count()
         out = {k: v.cpu().numpy() for k, v in g.items()}
@@ -221,6 +221,34 @@ def test_projection_backward_with_the_frustum_clamp():
     dm, dsc, dq = ob.project_backward(s, cam, proj.visible, out["grad_mean2d"][:5], out["grad_conic"][:5], out["grad_depth"][:5])
     for got, ref in ((out["grad_means"][:5], dm), (out["grad_scales"][:5], dsc), (out["grad_rotations"][:5], dq)):
         assert _rel(got, ref) <= 5e-6, (got, ref)
+
+
+@pytest.mark.parametrize("cfg,fp32", [(3, False), (3, True), (6, False), (5, False)])
+def test_backward_through_the_mlp_inputs(cfg, fp32):
+    """Step a1 differentiated: with grad_feat / grad_vis_sh requested the gradients that reach the Gaussian through
+    the MLP's inputs are added: feature, visibility SH, and the totals of mean / scale / rotation / normal against
+    render_backward(through_projection, through_inputs).  cfg 6 (paper architecture) takes the fp32 MLP backward."""
+    s = _scene(1500, 72, 56, 2, cfg=cfg)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    G = np.random.default_rng(51).standard_normal((2, cam.height, cam.width, 3))
+    G[:, comp.unstable] = 0.0
+    tc = not fp32 and cfg != 6
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, mlp_mode=2 if tc else 0, through_projection=True, through_inputs=True)
+    out = _gpu(s, G, fp32=fp32, through_inputs=True)
+    ref_attr = np.concatenate([r.d_normals, r.d_base, r.d_rough[:, None], r.d_metal[:, None], r.d_sss[:, None]], axis=1)
+    pairs = {"grad_feat": (out["grad_feat"][:s.n], r.d_feat), "grad_vis_sh": (out["grad_vis_sh"][:s.n], r.d_vis_sh),
+             "grad_means": (out["grad_means"][:s.n], r.d_means), "grad_scales": (out["grad_scales"][:s.n], r.d_scales),
+             "grad_rotations": (out["grad_rotations"][:s.n], r.d_rotations), "grad_attr": (out["grad_attr"][:s.n], ref_attr)}
+    if r.d_feat.shape[1] == 0:      # config 6: the paper's 40 inputs, no extra feature
+        del pairs["grad_feat"]
+    errs = {k: _rel(a, b) for k, (a, b) in pairs.items()}
+    print(f"through the inputs cfg {cfg} {'fp32' if fp32 else 'tcgen05'}:", {k: f"{v:.2e}" for k, v in errs.items()})
+    for k, (a, b) in pairs.items():
+        assert np.abs(b).max() > 0 and a.shape == b.shape, k
+    # and the inputs do contribute: without them the mean's gradient is a different one
+    r0 = ob.render_backward(s, proj, vals, ranges, xs, G, mlp_mode=2 if tc else 0, through_projection=True)
+    assert _rel(r0.d_means, r.d_means) > 1e-3
+    assert max(errs.values()) <= 5e-3
 
 
 def test_backward_full_size_cfg2_sampled_tiles():
