@@ -345,15 +345,19 @@ class ConfigRun:
         fwd = self.R.render(cams=self.cams, lights=self.lights, want=("rgb", "gbuffer"), tight=self.kw["tight"])
         gen = torch.Generator(device=self.dev).manual_seed(7)
         G = torch.randn(fwd["rgb"].shape, generator=gen, device=self.dev)
-        ms = []
-        for _ in range(reps + 1):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            self.R.render_backward(self.cam, self.lights, G, fwd["gbuffer"], tight=self.kw["tight"])
-            b.record()
-            torch.cuda.synchronize()
-            ms.append(a.elapsed_time(b))
-        return {"ms": round(float(np.median(ms[1:])), 4), "launches": self.R.launch_count(),
+        def timed(**kw):
+            ms = []
+            for _ in range(reps + 1):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                self.R.render_backward(self.cam, self.lights, G, fwd["gbuffer"], tight=self.kw["tight"], **kw)
+                b.record()
+                torch.cuda.synchronize()
+                ms.append(a.elapsed_time(b))
+            return round(float(np.median(ms[1:])), 4)
+        ms_all = timed(through_inputs=True)     # + step a1: feature, visibility SH, input-side shares
+        ms = timed()
+        return {"ms": ms, "ms_with_input_gradients": ms_all, "launches": self.R.launch_count(),
                 "lights": len(self.lights), "mlp_backward": "tcgen05, binary16 operands (fp32 CUDA-core path: SSSGS_BACKWARD_FP32)"}
 
     def close(self):
