@@ -251,6 +251,41 @@ def test_backward_through_the_mlp_inputs(cfg, fp32):
     assert max(errs.values()) <= 5e-3
 
 
+@pytest.mark.parametrize("fp32", [False, True])
+def test_input_backward_alone(fp32):
+    """Step a1 in isolation: the oracle's reverse mode of inputs -> MLP fed the GPU's OWN dL/d(mlp_out); the
+    input-side shares of mean / scale / rotation / normal are the difference of two GPU calls (with and without the
+    input gradients), feature and visibility SH come out directly."""
+    s = _scene(2500, 88, 72, 2)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    G = np.random.default_rng(61).standard_normal((2, cam.height, cam.width, 3))
+    a = _gpu(s, G, fp32=fp32, through_inputs=True)
+    b = _gpu(s, G, fp32=fp32)
+    gm = a["grad_mlp_out"][:, :s.n].astype(np.float64)
+    t = {k: ob._t(getattr(s, k)).requires_grad_(True) for k in ("means", "normals", "rotations", "scales", "vis_sh", "feat")}
+    params = ob._t(s.mlp.params)
+    loss = 0.0
+    for l, lt in enumerate(s.lights[0]):
+        x = ob.mlp_inputs_torch(t["means"], t["normals"], t["rotations"], t["scales"], t["vis_sh"], t["feat"], cam,
+                                lt.position, s.vis_sh_degree)
+        loss = loss + (ob.mlp_torch(x, s.mlp, params, mode=0 if fp32 else 2) * ob._t(gm[l])).sum()
+    loss.backward()
+    n = s.n
+    pairs = {"feat": (a["grad_feat"][:n], t["feat"].grad.numpy()), "vis_sh": (a["grad_vis_sh"][:n], t["vis_sh"].grad.numpy()),
+             "means": (a["grad_means"][:n].astype(np.float64) - b["grad_means"][:n], t["means"].grad.numpy()),
+             "scales": (a["grad_scales"][:n].astype(np.float64) - b["grad_scales"][:n], t["scales"].grad.numpy()),
+             "rotations": (a["grad_rotations"][:n].astype(np.float64) - b["grad_rotations"][:n], t["rotations"].grad.numpy()),
+             "normals": (a["grad_attr"][:n, :3].astype(np.float64) - b["grad_attr"][:n, :3], t["normals"].grad.numpy())}
+    errs = {k: _rel(x_, y_) for k, (x_, y_) in pairs.items()}
+    print(f"input backward alone ({'fp32' if fp32 else 'tcgen05'}):", {k: f"{v:.2e}" for k, v in errs.items()})
+    for k, (x_, y_) in pairs.items():
+        assert np.abs(y_).max() > 0, k
+    # the shares of mean / scale / rotation / normal are differences of two fp32 sums with atomics (another order in
+    # each call): their floor is the rounding of the LARGER projection / compositing terms
+    assert errs["feat"] <= (5e-5 if fp32 else 2e-3) and errs["vis_sh"] <= (5e-5 if fp32 else 2e-3)
+    assert max(errs.values()) <= 5e-3
+
+
 def test_backward_full_size_cfg2_sampled_tiles():
     """BASELINE configs[1] at full size, the call bench.py times under `backward` (tight lists, tensor-core MLP
     backward).  The oracle cannot differentiate the whole 512 x 512 frame in seconds, so dL/drgb is non-zero on the
