@@ -306,6 +306,56 @@ int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_
                           const sssgs_camera* cam, const sssgs_light* lights, int n_light,
                           const sssgs_grads* grads, uint32_t flags, void* cuda_stream);
 
+/* The per-Gaussian MLP alone (steps 1 of the path: input assembly + f_Theta, Eq. 6),
+ * for callers that must not allocate device memory and therefore cannot use a context.
+ *
+ * Who that is: code running inside a host program that claimed the whole GPU for its own memory pool at start-up
+ * (an inference server, a renderer plug-in host) -- a cudaMalloc issued from a library there fails or steals from
+ * the pool's head-room; and code on a latency-critical thread, because cudaMalloc / cudaFree take the driver's
+ * allocator lock and may wait for the device to go idle.  sssgs_create does allocate (its workspace unless one is
+ * supplied, and always a stream and events), so such callers get this one call that needs no context at all.
+ *
+ * What it computes: for every Gaussian i < g->n and light l < n_light
+ *     mlp_out[(i * n_light + l) * 4 + 0..3] = (L_SSS r, g, b, L_in)
+ * with exactly the kernel, operand precision (sssgs_mlp.compute) and per-row arithmetic of sssgs_render: the
+ * values are bit-identical to sssgs_out.mlp_out of a render with the same scene, camera and lights.  NOTE the
+ * layout: Gaussian-major [n][n_light][4] (the kernel's native one), not sssgs_out.mlp_out's [n_light][n][4]; with
+ * n_light = 1 the two coincide, so one call per light yields arrays usable as sssgs_mlp.precomputed_out.
+ * Of `g` only means, scales, rotations, normals, vis_sh (+ degree) and feat (+ feat_dim) are read; of `cam` only R
+ * and t (the camera position); all pointers inside g / mlp and mlp_out are DEVICE pointers of `device`, 16-byte
+ * aligned; cam and lights are HOST structs, read before the call returns.  mlp.precomputed_out must be NULL.
+ *
+ * The only intermediate the MLP needs in global memory -- the parameters repacked as 16-bit tensor-core operand
+ * tiles -- is kept in a fixed array of SSSGS_STATIC_SCRATCH_BYTES that is part of the library image: every GPU on
+ * which the library is used holds those bytes from module load until the process ends, whether or not this
+ * function is ever called.  The call itself issues no cudaMalloc / cudaFree and calls no allocating library
+ * routine; it enqueues two kernels on `cuda_stream` and returns without synchronising.
+ *
+ * Limits (beyond them: SSSGS_ECAPACITY and a message naming the limit, nothing is enqueued):
+ *   - the packed operands of the network (see build rule in DESIGN.md "MLP stages"; 148 KB for four 128-wide
+ *     trunk layers on a 64-wide input) must fit SSSGS_STATIC_SCRATCH_BYTES = 192 KB.  sssgs_render accepts
+ *     networks up to ~225 KB; those between need a context;
+ *   - n_light <= SSSGS_STATIC_MAX_LIGHTS = 8 per call (one light batch); g->n <= 2^30.
+ *
+ * First call on a device: looks up the array's device address and the SM count of `device` (a driver query, no
+ * allocation) and caches them for the life of the process.  Make that first call at start-up, outside any stream
+ * capture; later calls skip the lookup.
+ *
+ * Sharing: there is ONE array per GPU, used by every call from every thread, and it keeps whatever the last call
+ * packed into it.  Each call rewrites all the bytes its own network's tiles occupy before its MLP kernel reads
+ * them, so nothing needs clearing between calls and a smaller network after a larger one is fine.  But two calls
+ * whose kernels can run at the same time on one GPU (different streams without an ordering between them, or two
+ * host threads) race on the array and produce garbage: order them on one stream or with events.  A context-based
+ * sssgs_render does not touch the array and may overlap freely.
+ *
+ * Errors (text via sssgs_last_error(NULL)): SSSGS_EINVAL (NULL / misaligned pointer, architecture rules of
+ * sssgs_mlp, device ordinal outside [0, 64)), SSSGS_ECAPACITY (limits above), SSSGS_EARCH (not an sm_100 device),
+ * SSSGS_ECUDA.  With g->n = 0 or n_light = 0 the call validates its arguments and does nothing.                  */
+#define SSSGS_STATIC_SCRATCH_BYTES (192 * 1024)
+#define SSSGS_STATIC_MAX_LIGHTS 8
+int sssgs_mlp_eval_static(int device, const sssgs_gaussians* g, const sssgs_mlp* mlp, const sssgs_camera* cam,
+                          const sssgs_light* lights, int n_light, float* mlp_out, void* cuda_stream);
+
 /* Per-stage device timing (measurement aid, off by default).  When enabled, sssgs_render
  * records CUDA events around each stage on the caller's stream (not capture-safe while on);
  * sssgs_profile_read synchronises those events and writes the milliseconds each stage of the

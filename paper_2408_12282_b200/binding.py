@@ -35,7 +35,10 @@ CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3
 
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
-           "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility", "sssgs_render_backward"]
+           "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility", "sssgs_render_backward",
+           "sssgs_mlp_eval_static"]
+SSSGS_STATIC_SCRATCH_BYTES = 192 * 1024
+SSSGS_STATIC_MAX_LIGHTS = 8
 STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster", "prepass"]
 
 _f = ctypes.c_float
@@ -134,6 +137,10 @@ def lib() -> ctypes.CDLL:
         L.sssgs_profile_enable.argtypes = [_vp, ctypes.c_int]
         L.sssgs_profile_read.restype = ctypes.c_int
         L.sssgs_profile_read.argtypes = [_vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_int)]
+        L.sssgs_mlp_eval_static.restype = ctypes.c_int
+        L.sssgs_mlp_eval_static.argtypes = [ctypes.c_int, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_mlp),
+                                            ctypes.POINTER(sssgs_camera), ctypes.POINTER(sssgs_light), ctypes.c_int,
+                                            _vp, _vp]
         L.sssgs_last_error.restype = ctypes.c_char_p
         L.sssgs_last_error.argtypes = [_vp]
         _lib = L
@@ -179,6 +186,19 @@ def sssgs_render_backward(ctx, g, mlp, cam, lights, n_light, grads, flags=0, str
 
 def sssgs_bake_visibility(ctx, g, bake, stream=None) -> None:
     _check(ctx, lib().sssgs_bake_visibility(ctx, ctypes.byref(g), ctypes.byref(bake), _vp(stream or 0)))
+
+
+def sssgs_mlp_eval_static(device, g, mlp, cam, lights, n_light, mlp_out_ptr, stream=None) -> None:
+    """The MLP alone, without a context and without any device allocation (include/sssgs.h).
+
+    For callers that cannot call cudaMalloc -- hosts that gave all GPU memory to their own pool, latency-critical
+    threads.  mlp_out_ptr: device pointer to [n][n_light][4] floats (Gaussian-major).  The packed weights go through
+    one fixed array inside the library (192 KB per GPU, shared by all calls): calls that may overlap on the GPU
+    race on it.  Errors are reported through sssgs_last_error(NULL)."""
+    rc = lib().sssgs_mlp_eval_static(int(device), ctypes.byref(g), ctypes.byref(mlp), ctypes.byref(cam), lights,
+                                     int(n_light), _vp(mlp_out_ptr or 0), _vp(stream or 0))
+    if rc != SSSGS_OK:
+        raise SssgsError(rc, (lib().sssgs_last_error(None) or b"").decode())
 
 
 def sssgs_last_launch_count(ctx) -> int:

@@ -976,3 +976,121 @@ extern "C" int sssgs_render_host(sssgs_ctx* c, const sssgs_gaussians* g, const s
   }
   return SSSGS_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// sssgs_mlp_eval_static: the per-Gaussian MLP (steps a1 + a2) without a context and without any allocation.
+//
+// The tensor-core MLP kernel does not read the caller's fp32 parameters: mlp_pack_kernel first rewrites them as
+// swizzled 16-bit UMMA operands (weights + split biases) into a global-memory scratch block, and every CTA of
+// mlp_kernel pulls that block into shared memory.  In the render path the block lives in the context's
+// workspace (cudaMalloc'ed by sssgs_create unless the caller brings one).  Here it lives in the array below,
+// which is part of the library's device image: the driver places it when the module is loaded on a device and
+// it stays there until the process exits.
+//
+// g_static_blob is only a handle on the host side.  Host code that hands `g_static_blob` itself to a kernel
+// passes the address of a host shadow object, not device memory: the kernel would fault (or, on machines where
+// the GPU can dereference host addresses, quietly work on the wrong bytes).  The device address has to be asked
+// for, per device, with that device current: cudaGetSymbolAddress.  static_scratch_for() does that once per
+// device ordinal and remembers the answer.
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+
+static __device__ __align__(256) uint8_t g_static_blob[SSSGS_STATIC_SCRATCH_BYTES];
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+  bool ready = false;
+  uint8_t* blob = nullptr;  // device address of g_static_blob on this device
+  int num_sms = 0;
+};
+StaticDevice g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+// Must be called with `device` current.  First call per device: resolves the array's device address and reads
+// the SM count; later calls only read the cached values.
+int static_scratch_for(int device, StaticDevice* out) {
+  if (device < 0 || device >= kStaticMaxDevices)
+    return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: device ordinal %d outside [0, %d)", device, kStaticMaxDevices);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  StaticDevice& d = g_static_dev[device];
+  if (!d.ready) {
+    int major = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
+      return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: cannot query device %d (libsssgs has no CPU fallback)", device);
+    if (major != 10)
+      return fail(nullptr, SSSGS_EARCH, "sssgs_mlp_eval_static: device %d is sm_%dx; libsssgs is built for sm_100a only", device, major);
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_blob);
+    if (e != cudaSuccess || !p)
+      return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: cudaGetSymbolAddress failed on device %d: %s", device,
+                  cudaGetErrorString(e));
+    d.blob = static_cast<uint8_t*>(p);
+    d.num_sms = sms;
+    d.ready = true;
+  }
+  *out = d;
+  return SSSGS_OK;
+}
+
+}  // namespace
+
+extern "C" int sssgs_mlp_eval_static(int device, const sssgs_gaussians* g, const sssgs_mlp* mlp,
+                                     const sssgs_camera* cam, const sssgs_light* lights, int n_light,
+                                     float* mlp_out, void* cuda_stream) {
+  if (!g || !mlp || !cam || (n_light > 0 && !lights)) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: NULL argument");
+  if (n_light < 0) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: negative light count");
+  if (n_light > SSSGS_STATIC_MAX_LIGHTS)
+    return fail(nullptr, SSSGS_ECAPACITY, "sssgs_mlp_eval_static: n_light %d > SSSGS_STATIC_MAX_LIGHTS (%d); call once per batch of lights",
+                n_light, SSSGS_STATIC_MAX_LIGHTS);
+  if (g->n < 0) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: n < 0");
+  if (g->n > (int64_t)1 << 30) return fail(nullptr, SSSGS_ECAPACITY, "sssgs_mlp_eval_static: n %lld > 2^30", (long long)g->n);
+  if (g->vis_sh_degree < 0 || g->vis_sh_degree > 1) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: vis_sh_degree must be 0 or 1");
+  if (g->feat_dim < 0 || g->feat_dim > 88 || g->feat_dim % 4)
+    return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: feat_dim must be a multiple of 4 in [0,88]");
+  if (g->n > 0) {
+    // the arrays the MLP's input row is assembled from (Eq. 6); the others are not read
+    const void* req[] = {g->means, g->scales, g->rotations, g->normals, g->vis_sh};
+    for (const void* p : req)
+      if (!p || !aligned16(p))
+        return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: means / scales / rotations / normals / vis_sh is NULL or not 16-byte aligned");
+    if (g->feat_dim > 0 && (!g->feat || !aligned16(g->feat))) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: feat is NULL or misaligned");
+    if (n_light > 0 && (!mlp_out || !aligned16(mlp_out))) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: mlp_out is NULL or misaligned");
+  }
+  if (mlp->precomputed_out) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: mlp.precomputed_out must be NULL");
+  if (!mlp->params || !aligned16(mlp->params)) return fail(nullptr, SSSGS_EINVAL, "sssgs_mlp_eval_static: mlp.params is NULL or misaligned");
+  MlpPlan plan;
+  const int rc = build_plan(nullptr, *mlp, g->feat_dim, &plan);
+  if (rc != SSSGS_OK) return rc;
+  if ((size_t)plan.blob_bytes > (size_t)SSSGS_STATIC_SCRATCH_BYTES)
+    return fail(nullptr, SSSGS_ECAPACITY,
+                "sssgs_mlp_eval_static: the packed weights of this MLP take %d bytes, the static scratch holds %d "
+                "(SSSGS_STATIC_SCRATCH_BYTES); use sssgs_render with a context for larger networks",
+                plan.blob_bytes, (int)SSSGS_STATIC_SCRATCH_BYTES);
+  if (g->n == 0 || n_light == 0) return SSSGS_OK;
+
+  DeviceGuard guard(device);
+  if (!guard.ok) return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: cudaSetDevice(%d) failed", device);
+  StaticDevice dev;
+  const int rs = static_scratch_for(device, &dev);
+  if (rs != SSSGS_OK) return rs;
+
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const CamParams cp = make_cam(*cam);  // only the camera position (w_out) enters the MLP
+  LightBatch lb;
+  memset(&lb, 0, sizeof lb);
+  for (int l = 0; l < n_light; ++l) {
+    memcpy(lb.l[l].pos, lights[l].position, 12);
+    memcpy(lb.l[l].intensity, lights[l].intensity, 12);
+  }
+  // Nothing in the block has to start at zero: the pack kernel rewrites every byte of the operand and bias
+  // tiles of THIS plan (zero padding included), and the bytes between / behind them, which may still hold the
+  // previous call's network, are copied to shared memory but never addressed by an MMA descriptor.
+  launch_mlp_pack(*mlp, plan, dev.blob, s);
+  const int k = launch_mlp(*g, plan, dev.blob, cp, lb, n_light, reinterpret_cast<float4*>(mlp_out), nullptr, 0,
+                           dev.num_sms, nullptr, nullptr, nullptr, s);
+  if (k < 0) return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: MLP kernel configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: CUDA error: %s", cudaGetErrorString(e));
+  return SSSGS_OK;
+}
