@@ -362,3 +362,34 @@ def test_render_backward_through_the_inputs_equals_finite_differences():
             num = (loss(dataclasses.replace(s, **{field: hi})) - loss(dataclasses.replace(s, **{field: lo}))) \
                 / (float(hi[i, k]) - float(lo[i, k]))
             assert abs(num - grad[i, k]) <= 2e-3 * abs(grad[i, k]) + 1e-6, (field, i, k, num, grad[i, k])
+
+
+def test_shading_backward_of_the_back_projection_at_an_off_centre_pixel():
+    # The pixel term ((px - cx) / fx) z of the back-projection enters the shading backward through
+    # d(world point) / d(depth) = f + a r + b d.  Pin: the restatement's value at pixel (41, 17) of a 64 x 48 frame
+    # equals the closed form built from the camera's basis vectors (tests/test_oracle_shading.py), and its reverse-mode
+    # gradient w.r.t. the accumulated depth channel equals the central difference of that closed form in z.
+    import test_oracle_shading as tos
+    cam, light, basis, eye = tos._off_centre_setup()
+    px, py, z, A = 41, 17, 3.3, 0.8
+    n = tos._unit((0.3, -0.8, 0.4))
+    b = np.array([0.8, 0.4, 0.1])
+    g = torch.tensor(tos._gbuf_with_pixel(cam, px, py, z, n, b, 1.7, A=A), dtype=torch.float64, requires_grad=True)
+    rgb = ob.shade_torch(cam, light.position, light.intensity, g)
+    want = tos._lambert_at(cam, light, basis, eye, px, py, z, n, b, 1.7, A=A)
+    np.testing.assert_allclose(rgb[py, px].detach().numpy(), want, rtol=1e-9)
+    w = np.array([0.7, -1.3, 0.45])
+    (rgb[py, px] * torch.tensor(w)).sum().backward()
+    h = 1e-5
+    fd = (tos._lambert_at(cam, light, basis, eye, px, py, z + h, n, b, 1.7, A=A) -
+          tos._lambert_at(cam, light, basis, eye, px, py, z - h, n, b, 1.7, A=A)) @ w / (2 * h)
+    got = float(g.grad[py, px, 0]) * A            # channel 0 holds A z: d/dz = A d/d(channel)
+    assert abs(fd) > 1e-3 and abs(got - fd) <= 1e-7 * abs(fd) + 1e-10, (got, fd)
+    # teeth: with px and py swapped the derivative is a different number
+    fd_swapped = (tos._lambert_at(cam, light, basis, eye, py, px, z + h, n, b, 1.7, A=A) -
+                  tos._lambert_at(cam, light, basis, eye, py, px, z - h, n, b, 1.7, A=A)) @ w / (2 * h)
+    assert abs(fd_swapped - fd) > 1e-2 * abs(fd)
+    # no other pixel's G-buffer received a gradient
+    gg = g.grad.clone()
+    gg[py, px] = 0
+    assert float(gg.abs().max()) == 0.0

@@ -158,3 +158,128 @@ def test_fp32_shading_tracks_double():
         a = shade_point(n, l, v, **kw)[0]
         b = shade_point(n, l, v, f32=True, **kw)[0]
         np.testing.assert_allclose(a, b, rtol=2e-4, atol=2e-5)
+
+
+# ---- the pixel -> world back-projection ("The image space surface position is projected back to
+# the 3D space") at a pixel that is NOT the image centre.  Every pin above shades a 1x1 image (px = py = 0), where
+# the pixel term ((px - cx) / fx) z of the back-projection is a constant; here it is pinned against a world point
+# built from the camera's basis vectors alone. -----------------------------------------------------------------
+def _off_centre_setup():
+    from paper_2408_12282_b200.scenes import Camera, Light
+    W, H = 64, 48
+    eye = np.array([0.7, -3.1, 0.4])
+    f = _unit(np.array([0.1, 0.3, -0.2]) - eye)             # forward (+z of the camera)
+    r = _unit(np.cross(f, (0.0, 0.0, 1.0)))                 # right   (+x)
+    d = np.cross(f, r)                                      # down    (+y)
+    R = np.stack([r, d, f]).astype(np.float32)              # p_c = R p + t   (include/sssgs.h, sssgs_camera)
+    t = (-(R.astype(np.float64) @ eye)).astype(np.float32)
+    # anisotropic focal lengths and a principal point off the image centre: fx/fy, cx/cy mix-ups change the answer
+    cam = Camera(R=R, t=t, fx=61.0, fy=47.0, cx=29.25, cy=25.5, tan_half_fovx=W / 2 / 61.0, tan_half_fovy=H / 2 / 47.0,
+                 width=W, height=H, znear=0.2, bg=np.array([0.05, 0.1, 0.2], np.float32), position=eye.astype(np.float32))
+    light = Light(np.array([0.9, -1.2, 1.1], np.float32), np.array([1.0, 0.8, 0.6], np.float32))  # close: directions vary over the image
+    return cam, light, (r, d, f), eye
+
+
+def _world_point(cam, basis, eye, px, py, z):
+    """The point whose camera coordinates are (a z, b z, z), written with the basis vectors -- no R^T, no t."""
+    r, d, f = basis
+    # the camera the shader sees holds float32 R and t: use the same rounded basis / eye so that the comparison
+    # is at rounding level (the convention, not the rounding, is what is pinned)
+    Rm = cam.R.astype(np.float64)
+    r, d, f = Rm[0], Rm[1], Rm[2]
+    eye = -(Rm.T @ cam.t.astype(np.float64))
+    a, b = (px - cam.cx) / cam.fx, (py - cam.cy) / cam.fy
+    return eye + z * (f + a * r + b * d), eye
+
+
+def _lambert_at(cam, light, basis, eye, px, py, z, n, b, lin, A=1.0):
+    """Closed form of test_lambertian_closed_form (sss = 0, m = 0, r = 1) at the world point of pixel (px, py)."""
+    X, eye = _world_point(cam, basis, eye, px, py, z)
+    l = _unit(light.position.astype(np.float64) - X)
+    v = _unit(eye - X)
+    nl, nv = max(0.0, n @ l), max(1e-4, n @ v)
+    h = _unit(l + v)
+    F = 0.04 + 0.96 * (1 - v @ h) ** 5
+    # alpha_r = 1: D = 1 / (pi (nh^2 + |n x h|^2)^2) = 1 / pi, except where the viewer is behind the surface and
+    # n.h < 0 is clamped to 0 (then only |n x h|^2 = 1 - (n.h)^2 is left)
+    nh = n @ h
+    D = 1.0 / (np.pi * (max(0.0, nh) ** 2 + 1.0 - nh * nh) ** 2)
+    lout = (b / np.pi + D * F / ((1 + nl) * (1 + nv))) * lin * nl
+    return light.intensity.astype(np.float64) * A * lout + (1 - A) * cam.bg.astype(np.float64)
+
+
+def _gbuf_with_pixel(cam, px, py, z, n, b, lin, A=1.0):
+    g = np.zeros((cam.height, cam.width, 16))
+    g[..., 15] = 1.0
+    q = np.zeros(16)
+    q[0], q[1:4], q[4:7], q[7], q[8], q[9], q[13] = z, n, b, 1.0, 0.0, 0.0, lin
+    q[:14] *= A
+    q[14], q[15] = A, 1 - A
+    g[py, px] = q
+    return g
+
+
+def test_back_projection_off_centre_pixel():
+    cam, light, basis, eye = _off_centre_setup()
+    px, py, z = 41, 17, 3.3
+    n = _unit((0.3, -0.8, 0.4))
+    b = np.array([0.8, 0.4, 0.1])
+    g = _gbuf_with_pixel(cam, px, py, z, n, b, 1.7, A=0.8)
+    rgb = oracle.shade(cam, light, g)[0]
+    want = _lambert_at(cam, light, basis, eye, px, py, z, n, b, 1.7, A=0.8)
+    np.testing.assert_allclose(rgb[py, px], want, rtol=1e-9)
+    # every other pixel is background
+    mask = np.ones((cam.height, cam.width), bool)
+    mask[py, px] = False
+    np.testing.assert_allclose(rgb[mask], np.broadcast_to(cam.bg.astype(np.float64), (mask.sum(), 3)), atol=0)
+    # the pin has teeth: each plausible slip of the pixel term moves the closed form far beyond the tolerance
+    X, e = _world_point(cam, basis, eye, px, py, z)
+    slips = {
+        "px <-> py": _lambert_at(cam, light, basis, eye, py, px, z, n, b, 1.7, A=0.8),
+        "x sign": _lambert_at(cam, light, basis, eye, 2 * cam.cx - px, py, z, n, b, 1.7, A=0.8),
+        "y sign": _lambert_at(cam, light, basis, eye, px, 2 * cam.cy - py, z, n, b, 1.7, A=0.8),
+        "no pixel term": _lambert_at(cam, light, basis, eye, cam.cx, cam.cy, z, n, b, 1.7, A=0.8),
+        "fx <-> fy": _lambert_at(cam, light, basis, eye, cam.cx + (px - cam.cx) * cam.fx / cam.fy,
+                                 cam.cy + (py - cam.cy) * cam.fy / cam.fx, z, n, b, 1.7, A=0.8),
+        "cx <-> cy": _lambert_at(cam, light, basis, eye, px + cam.cx - cam.cy, py + cam.cy - cam.cx, z, n, b, 1.7, A=0.8),
+        "pixel term not scaled by z": _lambert_at(cam, light, basis, eye, cam.cx + (px - cam.cx) / z,
+                                                  cam.cy + (py - cam.cy) / z, z, n, b, 1.7, A=0.8),
+    }
+    for name, val in slips.items():
+        assert np.abs(val - want).max() > 1e-3 * np.abs(want).max(), name
+    # the fp32 evaluation of the same text (the calibration arm of S9) follows
+    np.testing.assert_allclose(oracle.shade(cam, light, g, f32=True)[0][py, px], want, rtol=2e-5)
+
+
+def test_back_projection_inverts_the_projection():
+    # the world point of pixel (px, py) at depth z, pushed through the (separately pinned) EWA projection of
+    # step 3, lands on (px, py) with depth z: the two halves of the path use one pixel convention
+    cam, light, basis, eye = _off_centre_setup()
+    pts = [(41, 17, 3.3), (5, 40, 2.1), (60, 3, 4.0)]
+    X = np.stack([_world_point(cam, basis, eye, px, py, z)[0] for px, py, z in pts])
+    from types import SimpleNamespace
+    sc = SimpleNamespace(n=len(pts), means=X.astype(np.float32), scales=np.full((len(pts), 3), 0.05, np.float32),
+                         rotations=np.tile(np.array([1, 0, 0, 0], np.float32), (len(pts), 1)))
+    proj = oracle.project(sc, cam)
+    assert proj.visible.all()
+    for k, (px, py, z) in enumerate(pts):
+        np.testing.assert_allclose(proj.pix[k], (px, py), atol=2e-4)
+        np.testing.assert_allclose(proj.depth[k], z, rtol=1e-6)
+
+
+def test_shading_every_pixel_of_a_frame_against_the_closed_form():
+    # all pixels of a 64 x 48 frame at varying depth / normal: no pixel-dependent term escapes
+    cam, light, basis, eye = _off_centre_setup()
+    rng = np.random.default_rng(3)
+    H, W = cam.height, cam.width
+    g = np.zeros((H, W, 16))
+    want = np.zeros((H, W, 3))
+    b = np.array([0.6, 0.5, 0.3])
+    for py in range(H):
+        for px in range(W):
+            z = 2.0 + 2.0 * rng.random()
+            n = _unit(rng.standard_normal(3))
+            g[py, px] = _gbuf_with_pixel(cam, px, py, z, n, b, 1.0)[py, px]
+            want[py, px] = _lambert_at(cam, light, basis, eye, px, py, z, n, b, 1.0)
+    rgb = oracle.shade(cam, light, g)[0]
+    np.testing.assert_allclose(rgb, want, rtol=1e-8, atol=1e-12)
