@@ -265,8 +265,11 @@ def shade_torch(cam, light_pos, light_intensity, gbuf: torch.Tensor) -> torch.Te
 # ---------------------------------------------------------------------------------------------------
 def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int = 0, lights=None, tile=16,
                     given_mlp_out=None, mlp_mode: int = 0, through_projection: bool = False,
-                    through_inputs: bool = False):
-    """Gradients of L = sum_l <grad_rgb[l], rgb_l> for one view.
+                    through_inputs: bool = False, grad_gbuf=None):
+    """Gradients of L = sum_l <grad_rgb[l], rgb_l> (+ sum_l <grad_gbuf[l], gbuf_l> when grad_gbuf [L, H, W, 16] is
+    given: the losses of PAPER.md L343-349 that act on the rasterised property images directly -- normal / depth
+    consistency, mask entropy on A, smoothness of roughness / metalness / sss / base colour, the incident-light
+    term) for one view.
 
     proj / vals / ranges: the oracle's projection and tile lists of the view (oracle.project / build_lists);
     mlp_inputs: [L][n, in_dim] float64 (oracle.mlp_inputs per light); grad_rgb [L, H, W, 3].
@@ -280,7 +283,7 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
     the walks: d_params is then zero).
     Returns a namespace of numpy float64 arrays:
       rgb [L,H,W,3], gbuf [L,H,W,16]              forward values of the restatement
-      d_gbuf [L,H,W,16]                           step a8 backward (per light)
+      d_gbuf [L,H,W,16]                           step a8 backward (per light), plus grad_gbuf where given
       d_mlp_out [L,n,4]                           what a7 hands to a2
       d_params [P]                                MLP weights and biases, packing of scenes.MlpSpec
       d_opacity [n], d_pix [n,2], d_conic [n,3], d_depth [n]   (depth = G-buffer channel 0's per-Gaussian value)
@@ -333,6 +336,8 @@ def render_backward(scene, proj, vals, ranges, mlp_inputs, grad_rgb, view: int =
         gb.retain_grad()
         rgb = shade_torch(cam, lt.position, lt.intensity, gb)
         loss = loss + (rgb * _t(grad_rgb[li])).sum()
+        if grad_gbuf is not None:
+            loss = loss + (gb * _t(grad_gbuf[li])).sum()
         rgbs.append(rgb)
         gbufs.append(gb)
         mlp_outs.append(mo)

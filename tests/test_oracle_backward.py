@@ -393,3 +393,65 @@ def test_shading_backward_of_the_back_projection_at_an_off_centre_pixel():
     gg = g.grad.clone()
     gg[py, px] = 0
     assert float(gg.abs().max()) == 0.0
+
+
+def test_upstream_gradient_on_the_gbuffer_equals_finite_differences():
+    # L = sum_l <G_rgb, rgb_l> + <G_gb, gbuf_l>: the losses on the rasterised property images
+    # reach the Gaussians through the compositing alone.  All 16 channels carry a gradient, the final
+    # transmittance (15) included.  Reference: central differences of the C++ forward oracle.
+    s = _scene()
+    cam, proj, vals, ranges, xs = _setup(s)
+    rng = np.random.default_rng(23)
+    G = 0.3 * rng.standard_normal((2, cam.height, cam.width, 3))
+    Gg = rng.standard_normal((2, cam.height, cam.width, 16))
+
+    def cpp_loss(scene, pr):
+        tot = 0.0
+        for li, lt in enumerate(scene.lights[0]):
+            mo = oracle.mlp_forward(xs[li], scene.mlp, 0)
+            comp = oracle.composite(scene, cam, pr, oracle.channels(scene, pr, mo), vals, ranges)
+            tot += float((oracle.shade(cam, lt, comp.gbuf)[0] * G[li]).sum() + (comp.gbuf * Gg[li]).sum())
+        return tot
+
+    r = ob.render_backward(s, proj, vals, ranges, xs, G, grad_gbuf=Gg)
+    np.testing.assert_allclose(r.loss, cpp_loss(s, proj), rtol=1e-11)
+    r0 = ob.render_backward(s, proj, vals, ranges, xs, G)
+    np.testing.assert_allclose(r.d_gbuf, r0.d_gbuf + Gg, rtol=1e-12, atol=1e-13)     # a8 backward + the upstream term
+    assert np.abs(r.d_opacity - r0.d_opacity).max() > 1e-2                          # and it reaches the Gaussians
+
+    def pick(g):
+        flat = np.abs(g).ravel()
+        return sorted(set(np.argsort(-flat)[:3].tolist() + rng.choice(flat.size, 2, replace=False).tolist()))
+
+    def check(name, got, ref):
+        assert abs(got - ref) <= 2e-5 * max(1.0, abs(ref)) + 1e-7, (name, got, ref)
+
+    for name, field, h in [("d_opacity", "opacities", 1e-4), ("d_normals", "normals", 1e-4), ("d_rough", "roughness", 1e-4),
+                           ("d_sss", "subsurface", 1e-4)]:
+        g = getattr(r, name)
+        for k in pick(g):
+            a = getattr(s, field)
+            ap, am = a.copy(), a.copy()
+            ap.ravel()[k] = np.float32(a.ravel()[k] + h)
+            am.ravel()[k] = np.float32(a.ravel()[k] - h)
+            fd = (cpp_loss(dataclasses.replace(s, **{field: ap}), proj) - cpp_loss(dataclasses.replace(s, **{field: am}), proj)) \
+                / (float(ap.ravel()[k]) - float(am.ravel()[k]))
+            check((name, k), g.ravel()[k], fd)
+    for name, field, h in [("d_pix", "pix", 2e-4), ("d_conic", "conic", 1e-5), ("d_depth", "depth", 1e-4)]:
+        g = getattr(r, name)
+        for k in pick(g):
+            vals_pm = []
+            for sgn in (+1, -1):
+                p2 = type(proj)(**vars(proj))
+                a = getattr(proj, field).copy()
+                a.ravel()[k] = np.float32(a.ravel()[k] + sgn * h)
+                setattr(p2, field, a)
+                vals_pm.append((cpp_loss(s, p2), float(a.ravel()[k])))
+            fd = (vals_pm[0][0] - vals_pm[1][0]) / (vals_pm[0][1] - vals_pm[1][1])
+            check((name, k), g.ravel()[k], fd)
+    # a loss on the final transmittance alone: dL/d opacity of a Gaussian = -sum_p dT(p) T(p) alpha_i(p) / (o_i (1 - alpha_i(p)))
+    # has the sign of -dT: more opacity, less transmittance
+    Gt = np.zeros_like(Gg)
+    Gt[..., 15] = 1.0
+    rt = ob.render_backward(s, proj, vals, ranges, xs, np.zeros_like(G), grad_gbuf=Gt)
+    assert (rt.d_opacity <= 1e-15).all() and rt.d_opacity.min() < -1e-2
