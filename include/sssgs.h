@@ -256,11 +256,12 @@ typedef struct {
 } sssgs_bake;
 int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_bake* bake, void* stream);
 
-/* Backward pass of the render path's steps a8 (deferred shading), a7 (compositing) and a2 (the MLP)
+/* Backward pass of the render path: steps a8 (deferred shading), a7 (compositing), a2 (the MLP) and, with the
+ * optional outputs below, a3 (the projection) and a1 (the MLP's input assembly)
  * ("optimize all parameters jointly via raytraced differentiable
  * rendering", L112, L343-349: the training losses are functions of the rendered image and of the
  * rasterised property images).  For ONE camera and its n_light lights, with
- *   L = sum_l < grad_rgb[l], rgb_l >
+ *   L = sum_l < grad_rgb[l], rgb_l >  ( + sum_l < grad_gbuffer_in[l], gbuffer_l >  when grad_gbuffer_in is given )
  * it computes dL/d of: the G-buffer of every light; the MLP outputs per (light, Gaussian); the MLP
  * parameters Theta; and per Gaussian the opacity, the 2-D mean, the conic (inverse 2-D covariance,
  * entries a, b, c of  power = -(a dx^2 + c dy^2) / 2 - b dx dy), the depth, the normal, the base
@@ -274,11 +275,12 @@ int sssgs_bake_visibility(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_
  * grad_params is then left zero).  Shading and compositing backward are fp32.  The MLP backward runs on the
  * tensor cores (binary16 operands, fp32 accumulation: the forward pass of the listed rows is re-evaluated with
  * the forward kernel's arithmetic; dL/d(mlp_out) is scaled by a power of two so that the deltas fit binary16)
- * when the MLP has no incident-head hidden layers and at most 4 trunk layers; otherwise, or with
- * SSSGS_BACKWARD_FP32, in fp32 on the CUDA cores (forward re-evaluated in fp32).  Per-Gaussian sums use float atomics: results are
+ * when mlp.compute is SSSGS_COMPUTE_FP16 and the MLP has no incident-head hidden layers and at most 4 trunk layers;
+ * otherwise (bf16 forward operands included: the binary16 re-evaluation would not reproduce that forward pass), or
+ * with SSSGS_BACKWARD_FP32, in fp32 on the CUDA cores (forward re-evaluated in fp32).  Per-Gaussian sums use float atomics: results are
  * reproducible to rounding, not bit for bit.  Enqueues on the stream, never synchronises.
- * With n_light = 0 (or n = 0) the per-Gaussian and parameter gradients are zeroed and the per-light
- * pointers are not read.  Errors: SSSGS_EINVAL (NULL / misaligned / dtype), SSSGS_ECAPACITY (n, image size). */
+ * With n_light = 0 the per-Gaussian and parameter gradients are zeroed and the per-light pointers are not read;
+ * with n = 0 grad_gbuffer is zeroed too (grad_gbuffer_in is not added: nothing is composited).  Errors: SSSGS_EINVAL (NULL / misaligned / dtype), SSSGS_ECAPACITY (n, image size). */
 typedef struct {
   const float* grad_rgb;     /* [n_light][H][W][3]  dL / d rgb                         (in)          */
   const float* gbuffer;      /* [n_light][H][W][16] the forward call's G-buffer        (in)          */
@@ -291,7 +293,8 @@ typedef struct {
   float* grad_depth;         /* [n]                                                    (out, required) */
   float* grad_attr;          /* [n][9]  normal (3), base colour (3), roughness, metalness, sss (out, required) */
   /* step a3 differentiated (Eq. 2): the three above pushed through the EWA projection.  All
-     three or none (NULL).  The dependence of the MLP INPUTS on these (step a1) is not differentiated.          */
+     three or none (NULL).  The dependence of the MLP INPUTS on them (step a1) is only included when grad_feat /
+     grad_vis_sh below are given.                                                                                  */
   float* grad_means;         /* [n][3]  dL / d mu                                      (out, may be NULL)  */
   float* grad_scales;        /* [n][3]  dL / d s (activated scales, as given)          (out, may be NULL)  */
   float* grad_rotations;     /* [n][4]  dL / d q (r, x, y, z), the quaternion as given (out, may be NULL)  */
@@ -301,6 +304,19 @@ typedef struct {
      clamp of the visibility to [0, 1] and the sign of the canonical quaternion are constants.                   */
   float* grad_feat;          /* [n][feat_dim]            dL / d feat                   (out, may be NULL)  */
   float* grad_vis_sh;        /* [n][(vis_sh_degree+1)^2] dL / d vis_sh                 (out, may be NULL)  */
+  /* Upstream gradient on the G-buffer itself: the losses of PAPER.md L343-349 that act on the rasterised property
+     images rather than on rgb (normal vs. depth consistency, mask entropy on A = channel 14, smoothness of
+     roughness / metalness / sss / base colour, the incident-light term on channel 13).  Layout and channel order of
+     sssgs_out.gbuffer (un-normalised accumulations; channel 15 = final transmittance).  It is added to what reaches
+     the G-buffer through rgb -- grad_gbuffer then holds the sum -- and is propagated through the compositing to
+     every per-Gaussian gradient, also where grad_rgb is zero.  Must not alias grad_gbuffer.                       */
+  const float* grad_gbuffer_in; /* [n_light][H][W][16]                                 (in, may be NULL)   */
+  /* The backward pass rebuilds the camera's tile lists with the context's max_instances.  If the instance count
+     exceeds it, the lists are truncated and EVERY gradient is undefined: counters (layout of sssgs_out.counters, one
+     camera; SSSGS_CNT_MLP_ROWS is 0) reports SSSGS_CNT_OVERFLOW / SSSGS_CNT_SORT_ERROR exactly as the forward call
+     does.  Check it after synchronising whenever the forward call's counters were not checked for the same scene,
+     camera and list mode (SSSGS_TIGHT_LISTS).                                                                    */
+  int64_t* counters;          /* [SSSGS_NCOUNTERS]                                     (out, may be NULL)  */
 } sssgs_grads;
 int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_mlp* mlp,
                           const sssgs_camera* cam, const sssgs_light* lights, int n_light,

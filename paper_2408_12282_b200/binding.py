@@ -87,7 +87,8 @@ class sssgs_out(ctypes.Structure):
 class sssgs_grads(ctypes.Structure):
     _fields_ = [(k, _vp) for k in ("grad_rgb", "gbuffer", "grad_gbuffer", "grad_mlp_out", "grad_params",
                                    "grad_opacity", "grad_mean2d", "grad_conic", "grad_depth", "grad_attr",
-                                   "grad_means", "grad_scales", "grad_rotations", "grad_feat", "grad_vis_sh")]
+                                   "grad_means", "grad_scales", "grad_rotations", "grad_feat", "grad_vis_sh",
+                                   "grad_gbuffer_in", "counters")]
 
 
 class sssgs_bake(ctypes.Structure):
@@ -361,9 +362,11 @@ class Renderer:
         return outputs
 
     def render_backward(self, cam, lights, grad_rgb, gbuffer, tight=False, stream=None, precomputed=None, fp32=False,
-                        through_inputs=False):
+                        through_inputs=False, grad_gbuffer_in=None):
         """Enqueue one sssgs_render_backward: cam one scene camera, lights its lights, grad_rgb [L,H,W,3] and
-        gbuffer [L,H,W,16] device tensors (the forward call's G-buffer).  Returns the dict of gradient tensors."""
+        gbuffer [L,H,W,16] device tensors (the forward call's G-buffer); grad_gbuffer_in [L,H,W,16]: optional
+        upstream gradient on the G-buffer.  Returns the dict of gradient tensors (+ "counters": the list counters of
+        the rebuilt tile lists, check SSSGS_CNT_OVERFLOW)."""
         torch = self.torch
         L, n, W, H = len(lights), max(self.n, 1), cam.width, cam.height
         z = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)  # noqa: E731
@@ -373,9 +376,12 @@ class Renderer:
         if through_inputs:   # step a1: the gradients through the MLP's inputs (added to means / scales / rotations / normal)
             out["grad_feat"] = z(n, max(self.feat_dim, 1))
             out["grad_vis_sh"] = z(n, (self.scene.vis_sh_degree + 1) ** 2)
+        out["counters"] = torch.zeros(SSSGS_NCOUNTERS, dtype=torch.int64, device=self.device)
         gr = sssgs_grads()
-        self._bwd_in = (grad_rgb.contiguous(), gbuffer.contiguous())
+        self._bwd_in = (grad_rgb.contiguous(), gbuffer.contiguous(),
+                        None if grad_gbuffer_in is None else grad_gbuffer_in.contiguous())
         gr.grad_rgb, gr.gbuffer = self._bwd_in[0].data_ptr(), self._bwd_in[1].data_ptr()
+        gr.grad_gbuffer_in = None if self._bwd_in[2] is None else self._bwd_in[2].data_ptr()
         for k, v in out.items():
             setattr(gr, k, v.data_ptr())
         larr = (sssgs_light * max(L, 1))(*[make_light(l) for l in lights])

@@ -303,7 +303,7 @@ int launch_zero(float* p, int64_t n, cudaStream_t s);
 int launch_project_backward(const sssgs_gaussians& g, const CamParams& cam, const float* g_mean2d, const float* g_conic,
                             const float* g_depth, float* d_means, float* d_scales, float* d_rot, cudaStream_t s);
 int launch_shade_backward(const CamParams& cam, const LightBatch& lights, int n_lights, const float* gbuf,
-                          const float* grad_rgb, float* grad_gbuf, cudaStream_t s);
+                          const float* grad_rgb, const float* grad_gbuf_in, float* grad_gbuf, cudaStream_t s);
 int launch_composite_backward(const CamParams& cam, int n_lights, const GeomBuffers& gb, const uint32_t* sorted_vals,
                               const float4* attr, const float4* mlp_out, int mlp_stride, const float* grad_gbuf,
                               float* g_opacity, float* g_mean2d, float* g_conic, float* g_depth, float* g_attr,

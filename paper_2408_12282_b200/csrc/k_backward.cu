@@ -45,7 +45,7 @@ __device__ __forceinline__ void normalize_bwd(const float* x, float inv_len, con
 __global__ void __launch_bounds__(256)
 shade_backward_kernel(CamParams cam, LightBatch lights, int n_lights, int64_t npix,
                       const float* __restrict__ gbuf, const float* __restrict__ grad_rgb,
-                      float* __restrict__ grad_gbuf) {
+                      const float* __restrict__ grad_gbuf_in, float* __restrict__ grad_gbuf) {
   const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
   if (i >= npix * n_lights) return;
   const int l_idx = (int)(i / npix);
@@ -191,6 +191,15 @@ shade_backward_kernel(CamParams cam, LightBatch lights, int n_lights, int64_t np
     }
     dG[14] = dA;
   }
+  // upstream gradient on the G-buffer itself (losses on the rasterised property images):
+  // added to what reaches the G-buffer through rgb, on covered and uncovered pixels alike
+  if (grad_gbuf_in != nullptr) {
+    const float4* ip = reinterpret_cast<const float4*>(grad_gbuf_in + i * 16);
+    for (int q = 0; q < 4; ++q) {
+      const float4 v = ip[q];
+      dG[4 * q] += v.x; dG[4 * q + 1] += v.y; dG[4 * q + 2] += v.z; dG[4 * q + 3] += v.w;
+    }
+  }
   float4* op = reinterpret_cast<float4*>(grad_gbuf + i * 16);
   for (int q = 0; q < 4; ++q) op[q] = make_float4(dG[4 * q], dG[4 * q + 1], dG[4 * q + 2], dG[4 * q + 3]);
 }
@@ -235,6 +244,7 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
   // upstream gradients of this pixel: light-independent channels summed over the lights, MLP channels per light
   float dGs[11];   // depth, n3, b3, rough, metal, sss, A
   float dGl[LB][4];
+  float dGT = 0.f;  // final transmittance (channel 15): non-zero only with an upstream gradient on the G-buffer
   for (int c = 0; c < 11; ++c) dGs[c] = 0.f;
   for (int l = 0; l < LB; ++l)
     for (int c = 0; c < 4; ++c) dGl[l][c] = 0.f;
@@ -244,6 +254,7 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
       const float* gp = grad_gbuf + ((int64_t)l * npix + pidx) * 16;
       for (int c = 0; c < 10; ++c) dGs[c] += gp[c];
       dGs[10] += gp[14];
+      dGT += gp[15];
       for (int c = 0; c < 4; ++c) dGl[l][c] = gp[10 + c];
     }
   }
@@ -314,7 +325,9 @@ composite_backward_kernel(CamParams cam, int n_lights, const uint2* __restrict__
     }
   }
   // ---- phase B: back to front ---------------------------------------------------------------------
-  float R = 0.f;   // sum_{j > i} w_j Phi_j
+  // R = sum_{j > i} w_j Phi_j, started at dGT T_final: the final transmittance T_final = prod_j (1 - alpha_j) has
+  // d T_final / d alpha_i = -T_final / (1 - alpha_i), the form of the suffix term below
+  float R = dGT * T;
   for (int b1 = max_last; b1 > 0; b1 -= kBwdBatch) {
     const int b0 = max(0, b1 - kBwdBatch), cnt = b1 - b0;
     __syncthreads();
@@ -1516,11 +1529,11 @@ int launch_project_backward(const sssgs_gaussians& g, const CamParams& cam, cons
 }
 
 int launch_shade_backward(const CamParams& cam, const LightBatch& lights, int n_lights, const float* gbuf,
-                          const float* grad_rgb, float* grad_gbuf, cudaStream_t s) {
+                          const float* grad_rgb, const float* grad_gbuf_in, float* grad_gbuf, cudaStream_t s) {
   const int64_t npix = (int64_t)cam.width * cam.height;
   const int64_t total = npix * n_lights;
   if (total == 0) return 0;
-  shade_backward_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(cam, lights, n_lights, npix, gbuf, grad_rgb, grad_gbuf);
+  shade_backward_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(cam, lights, n_lights, npix, gbuf, grad_rgb, grad_gbuf_in, grad_gbuf);
   return 1;
 }
 
@@ -1558,7 +1571,10 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
   ++launches;
 
   // ---- tensor-core path: a chain of <= 4 trunk layers and the two heads -------------------------------------
-  bool use_tc = !force_fp32 && mlp.n_inc_hidden == 0 && mlp.n_trunk >= 1 && mlp.n_trunk <= 4 && mlp.in_dim <= 128;
+  // The tensor-core path re-evaluates the forward pass with binary16 operands: it only matches a forward pass that
+  // ran with binary16 operands too.  A bf16 forward (sssgs_mlp.compute) is differentiated on the fp32 path.
+  bool use_tc = !force_fp32 && mlp.compute == SSSGS_COMPUTE_FP16 && mlp.n_inc_hidden == 0 && mlp.n_trunk >= 1 &&
+                mlp.n_trunk <= 4 && mlp.in_dim <= 128;
   for (int l = 0; l < mlp.n_trunk && use_tc; ++l)
     use_tc = mlp.trunk_width[l] % 16 == 0 && mlp.trunk_width[l] >= 16 && mlp.trunk_width[l] <= 128;
   if (use_tc) {

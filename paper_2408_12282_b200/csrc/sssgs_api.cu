@@ -697,6 +697,10 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   for (const void* p : per_light)   // per-light arrays are empty without lights
     if (n_light > 0 && (!p || !aligned16(p))) return fail(c, SSSGS_EINVAL, "a per-light gradient pointer is NULL or not 16-byte aligned");
   if (gr->grad_params && !aligned16(gr->grad_params)) return fail(c, SSSGS_EINVAL, "grad_params misaligned");
+  if (gr->grad_gbuffer_in && !aligned16(gr->grad_gbuffer_in)) return fail(c, SSSGS_EINVAL, "grad_gbuffer_in misaligned");
+  if (gr->grad_gbuffer_in && gr->grad_gbuffer_in == gr->grad_gbuffer)
+    return fail(c, SSSGS_EINVAL, "grad_gbuffer_in must not alias grad_gbuffer");
+  if (gr->counters && !aligned16(gr->counters)) return fail(c, SSSGS_EINVAL, "counters misaligned");
   const int n_geo = (gr->grad_means ? 1 : 0) + (gr->grad_scales ? 1 : 0) + (gr->grad_rotations ? 1 : 0);
   if (n_geo != 0 && n_geo != 3) return fail(c, SSSGS_EINVAL, "grad_means, grad_scales and grad_rotations: all three or none");
   if (n_geo == 3 && (!aligned16(gr->grad_means) || !aligned16(gr->grad_scales) || !aligned16(gr->grad_rotations)))
@@ -746,7 +750,9 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   launches += launch_zero(gr->grad_depth, n, s);
   launches += launch_zero(gr->grad_attr, n * 9, s);
   if (gr->grad_params) launches += launch_zero(gr->grad_params, (int64_t)(mlp->params_bytes / 4), s);
-  launches += launch_zero(gr->grad_gbuffer, (int64_t)n_light * npix * 16, s);
+  // grad_gbuffer is written in full by the shading backward of every light batch; only the degenerate call
+  // (no Gaussians: nothing below runs) has to clear it here
+  if (n == 0) launches += launch_zero(gr->grad_gbuffer, (int64_t)n_light * npix * 16, s);
   if (n_geo == 3) {   // the a1 backward accumulates into these, the projection backward adds to them
     launches += launch_zero(gr->grad_means, n * 3, s);
     launches += launch_zero(gr->grad_scales, n * 3, s);
@@ -757,7 +763,12 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
     launches += launch_zero(gr->grad_feat, n * g->feat_dim, s);
     launches += launch_zero(gr->grad_vis_sh, n * ncoef, s);
   }
-  if (n == 0 || n_light == 0) { c->launches = launches; return SSSGS_OK; }
+  if (n == 0 || n_light == 0) {
+    if (gr->counters && cudaMemsetAsync(gr->counters, 0, SSSGS_NCOUNTERS * sizeof(int64_t), s) != cudaSuccess)
+      return fail(c, SSSGS_ECUDA, "memset failed");
+    c->launches = launches;
+    return SSSGS_OK;
+  }
   // ---- forward state: attributes, geometry of the camera (as sssgs_render) -------------------------
   launches += launch_pack_attr(*g, c->attr, s);
   if (run_mlp) launches += launch_mlp_pack(*mlp, plan, c->mlp_blob, s);
@@ -782,7 +793,7 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
   const int fi = npass & 1;
   const uint32_t* sorted_tiles = c->gb.ikeys[fi];
   const uint32_t* sorted_vals = c->gb.ivals[fi];
-  launches += launch_ranges(sorted_tiles, cam, c->gb, cap, nullptr, nullptr, 0, s);
+  launches += launch_ranges(sorted_tiles, cam, c->gb, cap, nullptr, gr->counters, 0, s);
   float* const input_grads[6] = {gr->grad_means, gr->grad_scales, gr->grad_rotations, gr->grad_attr,
                                  n_in == 2 ? gr->grad_feat : nullptr, n_in == 2 ? gr->grad_vis_sh : nullptr};
   // ---- per light batch -----------------------------------------------------------------------------
@@ -803,6 +814,7 @@ int sssgs_render_backward(sssgs_ctx* c, const sssgs_gaussians* g, const sssgs_ml
       launches += launch_gather_precomputed(mlp->precomputed_out + (int64_t)l0 * n * 4, n, nl, n * 4, mlp_buf, s);
     }
     launches += launch_shade_backward(cam, lb, nl, gr->gbuffer + (int64_t)l0 * npix * 16, gr->grad_rgb + (int64_t)l0 * npix * 3,
+                                      gr->grad_gbuffer_in ? gr->grad_gbuffer_in + (int64_t)l0 * npix * 16 : nullptr,
                                       gr->grad_gbuffer + (int64_t)l0 * npix * 16, s);
     launches += launch_composite_backward(cam, nl, c->gb, sorted_vals, c->attr, mlp_buf, nl,
                                           gr->grad_gbuffer + (int64_t)l0 * npix * 16, gr->grad_opacity, gr->grad_mean2d,

@@ -45,16 +45,20 @@ def _rel(got, ref):
     return float(np.abs(np.asarray(got, np.float64) - ref).max() / max(np.abs(ref).max(), 1e-30))
 
 
-def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False, through_inputs=False):
+def _gpu(s, G, view=0, precomputed=None, tight=False, fp32=False, through_inputs=False, grad_gbuf=None, bf16=False,
+         max_instances=None):
     import torch
     from paper_2408_12282_b200 import binding
-    R = binding.Renderer(s)
+    R = binding.Renderer(s, compute=binding.SSSGS_COMPUTE_BF16 if bf16 else binding.SSSGS_COMPUTE_FP16,
+                         max_instances=max_instances)
     try:
         cam, lights = s.cameras[view], s.lights[view]
         pre = None if precomputed is None else torch.from_numpy(np.ascontiguousarray(precomputed, np.float32)).cuda()
         fwd = R.render(cams=[cam], lights=lights, want=("rgb", "gbuffer", "mlp_out"), precomputed=pre, tight=tight)
         g = R.render_backward(cam, lights, torch.from_numpy(np.ascontiguousarray(G, np.float32)).cuda(), fwd["gbuffer"],
-                              tight=tight, precomputed=pre, fp32=fp32, through_inputs=through_inputs)
+                              tight=tight, precomputed=pre, fp32=fp32, through_inputs=through_inputs,
+                              grad_gbuffer_in=None if grad_gbuf is None else
+                              torch.from_numpy(np.ascontiguousarray(grad_gbuf, np.float32)).cuda())
         torch.cuda.synchronize()
         launches = R.launch_count()
         out = {k: v.cpu().numpy() for k, v in g.items()}
@@ -356,3 +360,51 @@ def test_backward_rejects_bad_arguments():
         assert not out["grad_opacity"].any()
     finally:
         R.close()
+
+
+@pytest.mark.parametrize("n,w,h,lights,tight", [(400, 40, 32, 2, False), (3000, 96, 80, 9, True)])
+def test_upstream_gradient_on_the_gbuffer(n, w, h, lights, tight):
+    # sssgs_grads.grad_gbuffer_in: L = sum_l <G, rgb_l> + <Gg, gbuffer_l> (losses on the rasterised property images,
+    # PAPER.md L343-349); all 16 channels carry a gradient, the final transmittance included.  Same set-up and bar
+    # as test_walks_backward_given_mlp_outputs; a second call with grad_rgb = 0 shows the term is honoured alone.
+    s = _scene(n, w, h, lights)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    rng = np.random.default_rng(31 + n)
+    G = rng.standard_normal((lights, cam.height, cam.width, 3))
+    Gg = rng.standard_normal((lights, cam.height, cam.width, 16))
+    G[:, comp.unstable] = 0.0
+    Gg[:, comp.unstable] = 0.0
+    mo32 = mo.astype(np.float32)
+    for label, g_rgb in (("rgb + gbuffer", G), ("gbuffer only", np.zeros_like(G))):
+        r = ob.render_backward(s, proj, vals, ranges, xs, g_rgb, given_mlp_out=mo32.astype(np.float64), grad_gbuf=Gg)
+        out = _gpu(s, g_rgb, precomputed=mo32, tight=tight, grad_gbuf=Gg)
+        _check_all(out, r, s, 5e-5, f"upstream gbuffer gradient ({label}) n={n} L={lights}:")
+        assert out["counters"][2] == 0 and out["counters"][3] == 0 and out["counters"][1] > 0
+
+
+def test_backward_reports_list_overflow():
+    # the backward pass rebuilds the tile lists: with a too-small max_instances they are truncated and the
+    # gradients are undefined -- sssgs_grads.counters says so, as the forward call's counters do
+    s = _scene(3000, 96, 80, 1)
+    cam = s.cameras[0]
+    G = np.ones((1, cam.height, cam.width, 3))
+    ok = _gpu(s, G)
+    assert ok["counters"][2] == 0 and ok["counters"][1] > 1000
+    small = _gpu(s, G, max_instances=int(ok["counters"][1]) // 2)
+    assert small["counters"][2] == 1 and small["counters"][1] == ok["counters"][1]
+    assert all(np.isfinite(small[k]).all() for k in ("grad_opacity", "grad_mean2d", "grad_attr"))
+
+
+def test_mlp_backward_after_a_bf16_forward_runs_in_fp32():
+    # sssgs_mlp.compute = bf16: the tensor-core backward (binary16 re-evaluation) would not reproduce that forward
+    # pass, so the library differentiates on the fp32 path: dL/dTheta meets the fp32 bar against the float64 network
+    s = _scene(3000, 96, 80, 2)
+    cam, proj, vals, ranges, xs, mo, comp = _oracle_side(s)
+    G = np.random.default_rng(17).standard_normal((2, cam.height, cam.width, 3))
+    out = _gpu(s, G, bf16=True)
+    gm = out["grad_mlp_out"][:, :s.n].astype(np.float64)
+    params = ob._t(s.mlp.params).requires_grad_(True)
+    sum((ob.mlp_torch(ob._t(xs[l]), s.mlp, params, mode=0) * ob._t(gm[l])).sum() for l in range(2)).backward()
+    e = _rel(out["grad_params"], params.grad.numpy())
+    print(f"MLP backward after a bf16 forward: {e:.2e}")
+    assert e <= 5e-5
