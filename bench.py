@@ -42,13 +42,18 @@ from paper_2408_12282_b200 import multi, scenes  # noqa: E402
 
 METRIC = "Mpix/s (MLP + G-buffer splat + deferred shading)"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of a stage's heaviest kernel, from the `ncu --set full`
-# captures summarised in profiles/r02_ncu_full.md (tight lists, one view x all lights): (config, stage) -> bytes
+# captures summarised in profiles/r03_ncu_full.md (configs[4]) and profiles/r02_ncu_full.md (configs[1], [2]); tight
+# lists, one view x all lights: (config, stage) -> bytes.  Constants: a kernel change needs a new capture.
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    ("5", "prepass"): 378.9e6 + 617.3e6,   # raster_shade_kernel<1,1,4,4,1,0>: lists + rows in, weight cache + T out
-    ("5", "raster"): 796.0e6 + 98.0e6,     # raster_cached_kernel<8,0>: weight cache + rows in, 8 frames out
-    ("5", "mlp"): 190.6e6 + 29.4e6,        # mlp_kernel<8,1,1>: kept rows' inputs in, 8 x 16 B per kept row out
+    ("5", "prepass"): 375.5e6 + 617.1e6,   # raster_shade_kernel<1,1,4,4,1,0>: lists + rows in, weight cache + T out
+    ("5", "raster"): 795.4e6 + 98.1e6,     # raster_cached_kernel<8,0>: weight cache + rows in, 8 frames out
+    ("5", "mlp"): 190.6e6 + 30.0e6,        # mlp_kernel<8,1,1>: kept rows' inputs in, 8 x 16 B per kept row out
     ("3", "raster"): 148.3e6 + 61.6e6,     # raster_cached_kernel<8,1> (cfg 3, one of the 7 later batches)
     ("2", "raster"): 13.5e6 + 17.9e6,      # raster_shade_kernel<1,4,8,2,0,0> (cfg 2)
+}
+# the same two ncu metrics summed over EVERY kernel launch of one default step (tight lists, one view x all lights)
+NCU_DRAM_BYTES_PER_STEP = {
+    "5": 4.603e9,   # profiles/r03_ncu_full.md: the 19 launches of the step
 }
 FP32_LANES_PER_SM = 128
 HBM_NOMINAL_GBS = 8000.0   # BASELINE.json north_star: "~8 TB/s"
@@ -148,41 +153,38 @@ def config_dict(cfg, scene, fps):
 # ---------------------------------------------------------------------------------------------------
 # CPU oracle legs (cpu_baseline, --impl reference): the only places bench.py executes oracle/
 # ---------------------------------------------------------------------------------------------------
-def oracle_sample(scene, mlp_rows_budget=1_000_000):
-    """One whole-path render of the first (view, light) frame by the CPU oracle, as it stands.  A BOUNDED sample:
-    projection, lists, compositing and shading run in full; the MLP (plain loops, ~60 us per row and core) runs
-    on a seeded sample of at most `mlp_rows_budget` rows and its time is extrapolated linearly to all rows (a
-    row's cost does not depend on the row)."""
+def oracle_sample(scene, count_on=None):
+    """count_on = (vals, ranges) of another tile list of the same view (the device's tight list): the oracle's
+    compositor also counts the evaluated pairs of THAT list (outside the timed seconds) -> "p_eval_counted".
+
+    One whole-path render of the first (view, light) frame by the CPU oracle, as it stands: projection, lists,
+    the fp16-emulating MLP on ALL rows, compositing and shading of the whole frame.  Every second reported was
+    spent; nothing is extrapolated.  Bounded by construction: ONE frame (the GPU step renders `frames_per_step`)."""
     import oracle
     cam, lt = scene.cameras[0], scene.lights[0][0]
     t0 = time.perf_counter()
     proj = oracle.project(scene, cam)
     keys, vals, ranges = oracle.build_lists(proj)
     t_geo = time.perf_counter() - t0
-    n = int(scene.n)
-    if n > mlp_rows_budget:
-        rows = np.sort(np.random.default_rng(0).choice(n, size=mlp_rows_budget, replace=False))
-        sub = scenes.subset(scene, rows)
-    else:
-        rows, sub = np.arange(n), scene
     t0 = time.perf_counter()
-    x = oracle.mlp_inputs(sub, cam, lt.position)
-    y = oracle.mlp_forward(x, scene.mlp, 2)
-    t_mlp_sample = time.perf_counter() - t0
-    t_mlp = t_mlp_sample * n / max(len(rows), 1)
-    mlp_out = np.zeros((n, 4))
-    mlp_out[rows] = y
+    x = oracle.mlp_inputs(scene, cam, lt.position)
+    mlp_out = oracle.mlp_forward(x, scene.mlp, 2)
+    t_mlp = time.perf_counter() - t0
     t0 = time.perf_counter()
     comp = oracle.composite(scene, cam, proj, oracle.channels(scene, proj, mlp_out), vals, ranges)
     oracle.shade(cam, lt, comp.gbuf)
     t_img = time.perf_counter() - t0
     total = t_geo + t_mlp + t_img
-    return dict(seconds=total, cpu_seconds_spent=t_geo + t_mlp_sample + t_img, frames=1,
-                mpix_s=cam.width * cam.height / total / 1e6, cores=oracle.num_threads(),
-                mlp_rows_timed=int(len(rows)), p_eval=comp.p_eval, p_blend=comp.p_blend,
-                sample=(f"one whole-path render of the first (view, light) frame of {scene.name}: projection, lists, "
-                        f"compositing, shading in full ({t_geo + t_img:.1f} s); fp16-emulating MLP timed on "
-                        f"{len(rows)} of {n} rows ({t_mlp_sample:.1f} s) and scaled to all rows ({t_mlp:.1f} s)"))
+    counted = None
+    if count_on is not None:
+        c2 = oracle.composite(scene, cam, proj, oracle.channels(scene, proj, mlp_out), count_on[0], count_on[1])
+        assert c2.p_blend == comp.p_blend, "the device's tight list does not blend the pairs the canonical list blends"
+        counted = c2.p_eval
+    return dict(seconds=total, frames=1, p_eval_counted=counted, mpix_s=cam.width * cam.height / total / 1e6, cores=oracle.num_threads(),
+                p_eval=comp.p_eval, p_blend=comp.p_blend,
+                sample=(f"one whole-path render of the first (view, light) frame of {scene.name}, all measured: "
+                        f"projection + lists {t_geo:.1f} s, fp16-emulating MLP on all {int(scene.n)} rows {t_mlp:.1f} s, "
+                        f"compositing + shading of the whole frame {t_img:.1f} s"))
 
 
 def run_reference(args, rank):
@@ -191,7 +193,9 @@ def run_reference(args, rank):
         return
     scene, cams, lights, fps = workload(args.config)
     cam = cams[0]
-    steps = min(args.steps, 6 if scene.n > 200_000 else 30)      # bounded: a step is seconds of CPU work
+    # bounded: a step (one frame) is up to ~20 s of CPU work on the largest config; the whole run ends within
+    # a few minutes and `steps` / `ms_per_step` are what was really run and timed
+    steps = max(1, min(args.steps, 3 if scene.n > 200_000 else 30))
     warm = min(args.warmup, 1 if scene.n > 200_000 else 3)
     for _ in range(warm):
         oracle_sample(scene)
@@ -201,11 +205,14 @@ def run_reference(args, rank):
         t += r["seconds"]
         cores, sample = r["cores"], r["sample"]
     val = steps * cam.width * cam.height / t / 1e6
+    cfg_d = config_dict(args.config, scene, 1)     # this arm renders ONE (view, light) frame per step
+    cfg_d["gpu_arm_frames_per_step"] = int(fps)
+    cfg_d["l2"] = cfg_d["launch"] = "n/a (CPU)"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": "Mpix/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": t / steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": config_dict(args.config, scene, fps),
+        "config": cfg_d,
         "cpu_baseline": {"value": val, "unit": "Mpix/s", "cores": cores, "kind": "oracle",
                          "sample": sample + "; one frame per step (the oracle has no light batching)"},
         "e2e": {"value": val, "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -228,7 +235,11 @@ def mlp_flops_per_row(mlp):
     return fl + 2 * di
 
 
-def stage_models(scene, nl, n_vis, inst, ocnt, peaks, num_sms, mlp_rows, swept):
+def stage_models(scene, nl, n_vis, inst, ocnt, peaks, num_sms, mlp_rows, swept, tight):
+    """-> (work model per stage for the list mode being timed, the same with the canonical-list counters where that
+    differs, peaks).  With tight lists the evaluated-pair count is the oracle's count on the MINIMAL S5 list
+    (oracle/workload_counters.json p_eval_min): the device's tight list is a superset of it, so the figure is a lower
+    bound of the pairs the walk evaluated and the fraction is conservative."""
     n = scene.n
     alu_peak = num_sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s
     m = {
@@ -240,15 +251,22 @@ def stage_models(scene, nl, n_vis, inst, ocnt, peaks, num_sms, mlp_rows, swept):
         # rows the MLP actually evaluated (in a sweep: the Gaussians blended at some pixel of the view)
         "mlp": ("tensor", float(mlp_flops_per_row(scene.mlp)) * mlp_rows * nl),
     }
+    alt = {}
     if ocnt:
-        pe, pb = float(ocnt["p_eval"]), float(ocnt["p_blend"])
-        if swept:   # pre-pass: alpha + transmittance chain once per view; walks: blends only
-            m["prepass"] = ("alu", 10.0 * pe + 3.0 * pb)
-            m["raster"] = ("alu", 2.0 * (11.0 + 4.0 * nl) * pb)
+        def walks(pe, pb, out):
+            if swept:   # pre-pass: alpha + transmittance chain once per view; walks: blends only
+                out["prepass"] = ("alu", 10.0 * pe + 3.0 * pb)
+                out["raster"] = ("alu", 2.0 * (11.0 + 4.0 * nl) * pb)
+            else:
+                out["raster"] = ("alu", 10.0 * pe + (17.0 + 8.0 * (nl - 1)) * pb)
+        pb = float(ocnt["p_blend"])
+        if tight and "p_eval_min" in ocnt:
+            walks(float(ocnt["p_eval_min"]), pb, m)
+            walks(float(ocnt["p_eval"]), pb, alt)
         else:
-            m["raster"] = ("alu", 10.0 * pe + (17.0 + 8.0 * (nl - 1)) * pb)
+            walks(float(ocnt["p_eval"]), pb, m)
     pk = {"hbm": (peaks["hbm"], "GB/s"), "tensor": (peaks["bf16_burst"], "TFLOP/s"), "alu": (alu_peak, "TFLOP/s")}
-    return m, pk
+    return m, alt, pk
 
 
 class ConfigRun:
@@ -323,7 +341,8 @@ class ConfigRun:
         mlp_rows = self.cnt[b.CNT_MLP_ROWS] or self.scene.n
         swept = nlaunch.get("prepass", 0) > 0
         inst = min(self.cnt[b.CNT_INSTANCES], MAX_INSTANCES_PER_GAUSSIAN * self.scene.n)
-        models, pk = stage_models(self.scene, nl, self.cnt[b.CNT_NVIS], inst, ocnt, peaks, num_sms, mlp_rows, swept)
+        models, alt, pk = stage_models(self.scene, nl, self.cnt[b.CNT_NVIS], inst, ocnt, peaks, num_sms, mlp_rows, swept,
+                                       self.kw["tight"])
         out = {}
         for k, ms in stage_ms.items():
             if nlaunch[k] == 0:
@@ -335,6 +354,9 @@ class ConfigRun:
                 e.update(bound=bound, achieved=round(ach, 3), unit=pk[bound][1], frac=round(ach / pk[bound][0], 4))
                 if bound == "hbm":
                     e["frac_of_nominal_8TBs"] = round(ach / HBM_NOMINAL_GBS, 4)
+                if k in alt and alt[k][1] != work:
+                    e["counters"] = "minimal S5 list (p_eval_min): lower bound of the pairs a tight-list walk evaluates"
+                    e["frac_with_canonical_list_counters"] = round(alt[k][1] / (ms * 1e-3) / 1e12 / pk[bound][0], 4)
             out[k] = e
         return out, pk
 
@@ -446,6 +468,21 @@ def run_gpu(args, rank, world, local_rank):
                 "share_of_step": round(stage_ms[dom] / sum(stage_ms.values()), 3)}
         if sd.get("bound") == "hbm":
             roof["frac_of_nominal_8TBs"] = sd.get("frac_of_nominal_8TBs")
+        for extra in ("counters", "frac_with_canonical_list_counters"):
+            if extra in sd:
+                roof[extra] = sd[extra]
+        roof["traffic_source"] = ("constant from one `ncu --set full` capture of this kernel (profiles/r03_ncu_full.md), "
+                                  "not measured by this run" if roof["traffic"] else None)
+        # BASELINE.json's metric asks for the pipeline's share of the HBM roofline: DRAM bytes of ALL kernels of one
+        # step (same capture) over the measured step time.  The path is instruction-issue-bound, not HBM-bound.
+        step_bytes = NCU_DRAM_BYTES_PER_STEP.get(str(args.config)) if not args.canonical_lists else None
+        if step_bytes:
+            roof["hbm_frac_of_step"] = round(step_bytes / (med_ms * 1e-3) / 1e9 / peaks["hbm"], 4)
+            roof["hbm_bytes_per_step"] = step_bytes
+            roof["hbm_frac_of_step_source"] = ("sum of dram__bytes_read + dram__bytes_write over every kernel of one step "
+                                               "(profiles/r03_ncu_full.md) / median step time / measured HBM peak")
+        roof["pipeline_bound"] = "instruction issue (fp32 / integer ALU work of the list walks) + tensor pipe (MLP); not HBM"
+
         row = dict(ms_per_step_median=round(med_ms, 5), ms_per_step_min=round(min_ms, 5), frames_per_step=fps,
                    mpix_s=round(fps * npix / med_ms / 1e3, 1), gaussians_per_s=round(fps * scene.n / (med_ms * 1e-3), 0),
                    dominant_stage=dom, dominant_frac=sd.get("frac"), dominant_bound=sd.get("bound"),
@@ -457,6 +494,15 @@ def run_gpu(args, rank, world, local_rank):
             backward[key] = run.backward_ms()
         launches_per_step = run.launches
         cnt_head, mlp_rows_head = run.cnt, (run.cnt[binding.CNT_MLP_ROWS] or scene.n)
+        dev_list = None
+        if world == 1 and not args.no_cpu_baseline and not args.canonical_lists and not args.forward and not args.sum_lights:
+            # the tight list the timed step walked (geometry-only call), for the oracle to count its evaluated pairs
+            o = run.R.render(cams=run.cams, lights=run.lights[:1], want=("sorted_vals", "tile_ranges", "counters"),
+                             tight=True, precomputed=torch.zeros((1, max(scene.n, 1), 4), device=dev))
+            torch.cuda.synchronize()
+            n_inst = int(o["counters"][0][binding.CNT_INSTANCES])
+            dev_list = (o["sorted_vals"][0][:n_inst].cpu().numpy().view(np.uint32), o["tile_ranges"][0].cpu().numpy().view(np.uint32))
+            del o
         run.close()
         del run
         torch.cuda.empty_cache()
@@ -485,9 +531,19 @@ def run_gpu(args, rank, world, local_rank):
                 torch.cuda.empty_cache()
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            r = oracle_sample(scene)
+            r = oracle_sample(scene, count_on=dev_list)
             cpu = {"value": r["mpix_s"], "unit": "Mpix/s", "cores": r["cores"], "kind": "oracle",
-                   "sample": r["sample"] + f"; {r['cpu_seconds_spent']:.1f} s of CPU work"}
+                   "sample": r["sample"] + f"; {r['seconds']:.1f} s of CPU work"}
+            if r["p_eval_counted"] is not None and roof.get("bound") == "alu" and dom in ("prepass", "raster"):
+                # the dominant walk's fraction on the pairs of the list it really walked (counted by the oracle's
+                # compositor on the device's exported tight list; not part of the timed seconds)
+                pe, pb = float(r["p_eval_counted"]), float(r["p_blend"])
+                nl_ = len(scene.lights[0])
+                work = (10.0 * pe + 3.0 * pb) if dom == "prepass" else \
+                    (10.0 * pe + (17.0 + 8.0 * (nl_ - 1)) * pb if "prepass" not in stages else None)
+                if work:
+                    roof["p_eval_device_tight_list"] = int(pe)
+                    roof["frac_on_device_tight_list"] = round(work / (stage_ms[dom] * 1e-3) / 1e12 / roof["peak"], 4)
         cfg_d = config_dict(args.config, scene, fps)
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
