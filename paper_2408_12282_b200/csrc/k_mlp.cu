@@ -29,7 +29,7 @@
 //     mbarrier.  The whole warp runs the issue code with warp-uniform operands and the tcgen05
 //     instructions are predicated on one elected lane, so that the operands live in uniform
 //     registers: inside a divergent `if (lane == 0)` every operand of every MMA goes through R2UR
-//     and one MMA is issued per ~100-115 clocks instead of one per ~70 (csrc/bench_tmem_ld.cu).
+//     and one MMA is issued per ~100-115 clocks instead of one per ~70 (profiles/r02_tmem_ld_microbench.md).
 //
 // Output: float4 (L_SSS rgb, L_in) per (Gaussian, light), 16 B per row.
 #include <cuda_bf16.h>
