@@ -359,3 +359,21 @@ def bake_visibility(scene, dirs, weights, t_min: float, sh_degree: int = 1, rows
                               _p(dirs), _p(weights), ctypes.c_float(t_min), ctypes.c_int(sh_degree),
                               ctypes.c_int(1 if positions else 0), ctypes.c_int64(m), _p(rows_arr), _p(sh), _p(vis), _p(unstable))
     return sh, vis, unstable
+
+
+def relight(frames, weights) -> np.ndarray:
+    """Relighting from a precomputed reflectance field ("To speed up generation we can precompute a
+    reflectance field assuming white light.  We compute the relit view as the sum over the reflectance field scaled by
+    the environment illumination."):  out[p, c] = sum_l weights[l, c] * frames[l, p, c].
+    frames [L, H, W, 3]: the OLAT renders of one view under white unit-intensity point lights (on the black background
+    of a light stage; with another background every frame carries its (1 - A) bg term and the sum carries it L times
+    scaled -- the definition does not remove it); weights [L, 3]: RGB radiance of the environment towards light l.
+    Float64, lights added in order.  Pins: tests/test_oracle_forward.py (one-hot weights, brute force, equality with
+    shading under coloured lights -- Eq. 7 is linear in the light's intensity, S16)."""
+    frames = np.asarray(frames, np.float64)
+    weights = np.asarray(weights, np.float64)
+    assert frames.ndim == 4 and frames.shape[3] == 3 and weights.shape == (frames.shape[0], 3)
+    out = np.zeros(frames.shape[1:], np.float64)
+    for l in range(frames.shape[0]):
+        out += frames[l] * weights[l][None, None, :]
+    return out

@@ -67,3 +67,52 @@ def test_forward_frame_of_one_gaussian():
     r = oracle.forward_frame(s, mlp_out=mo)
     np.testing.assert_allclose(r.rgb[32, 32], 0.6 * mo[0, :3] + 0.4 * np.float64([0.1, 0.2, 0.3]), rtol=1e-6)
     assert np.allclose(r.rgb[0, 0], [0.1, 0.2, 0.3])
+
+
+# ---- oracle.relight: the reflectance-field sum of PAPER.md L301 ----------------------------------------------------
+def test_relight_one_hot_and_brute_force():
+    rng = np.random.default_rng(4)
+    L, H, W = 5, 3, 7
+    frames = rng.uniform(0.0, 2.0, (L, H, W, 3))
+    w = rng.uniform(0.0, 3.0, (L, 3))
+    for l in range(L):       # a single white light of the field switched on: that frame, exactly
+        e = np.zeros((L, 3))
+        e[l] = 1.0
+        np.testing.assert_array_equal(oracle.relight(frames, e), frames[l])
+    e = np.zeros((L, 3))
+    e[2, 1] = 0.5            # only the green channel of light 2
+    want = np.zeros((H, W, 3))
+    want[..., 1] = 0.5 * frames[2, ..., 1]
+    np.testing.assert_array_equal(oracle.relight(frames, e), want)
+    got = oracle.relight(frames, w)
+    for y in range(H):       # brute force, element by element
+        for x in range(W):
+            for c in range(3):
+                s = 0.0
+                for l in range(L):
+                    s += w[l, c] * frames[l, y, x, c]
+                assert abs(got[y, x, c] - s) <= 1e-14 * max(1.0, abs(s))
+    assert oracle.relight(np.zeros((0, H, W, 3)), np.zeros((0, 3))).shape == (H, W, 3)
+
+
+def test_relight_equals_shading_under_coloured_lights():
+    # Eq. 7 (L104-106) is linear in the light's RGB intensity (S16) and a point-light sum is a sum of frames
+    # (L301, App. D): on a black background, relighting the white-light OLAT frames with weights w_l equals the sum of
+    # the frames shaded under lights of intensity w_l -- a statement about the separately pinned shader.
+    import dataclasses
+    s = scenes.make_scene(3, n=300, width=24, height=20, lights=4)
+    cam = s.cameras[0]
+    assert not np.any(cam.bg)
+    r0 = oracle.render_frame(s, 0, 0)
+    rng = np.random.default_rng(9)
+    w = rng.uniform(0.1, 2.0, (4, 3))
+    white, coloured = [], np.zeros((cam.height, cam.width, 3))
+    for l, lt in enumerate(s.lights[0]):
+        r = oracle.render_frame(s, 0, l, geometry=r0)
+        assert np.all(lt.intensity == 1.0)
+        white.append(r.rgb)
+        lc = dataclasses.replace(lt, intensity=w[l].astype(np.float32))
+        coloured += oracle.shade(cam, lc, r.comp.gbuf)[0]
+    got = oracle.relight(np.stack(white), w.astype(np.float32))
+    assert np.abs(coloured).max() > 1e-2
+    np.testing.assert_allclose(got, coloured, rtol=1e-12, atol=1e-15)
