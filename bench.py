@@ -584,6 +584,49 @@ def fibonacci_dirs(K):
     return np.stack([r * np.cos(phi), r * np.sin(phi), z], 1).astype(np.float32), np.full(K, 4 * np.pi / K, np.float32)
 
 
+def run_relight(args, local_rank):
+    """--relight: times sssgs_relight on an OLAT stack of the config's frame shape
+    (frames_per_step lights), resident in HBM.  A side measurement with its own metric; HBM roofline: 12 (L + 1) P
+    bytes per call over the measured copy bandwidth."""
+    import torch
+    from paper_2408_12282_b200 import binding
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    scene, cams, lights, fps = workload(args.config)
+    cam, L = cams[0], max(len(lights), 1)
+    P = cam.width * cam.height
+    gen = torch.Generator(device=dev).manual_seed(1)
+    frames = torch.rand((L, cam.height, cam.width, 3), generator=gen, device=dev)
+    w = torch.rand((L, 3), generator=gen, device=dev)
+    out = torch.empty((cam.height, cam.width, 3), device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    call = lambda: binding.sssgs_relight(local_rank, frames.data_ptr(), L, P, w.data_ptr(), out.data_ptr(), stream.cuda_stream)  # noqa: E731
+    for _ in range(max(args.warmup, 3)):
+        call()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        call()
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.median([a.elapsed_time(b) for a, b in ev]))
+    peaks = load_peaks()
+    nbytes = 12.0 * (L + 1) * P
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    print(json.dumps({
+        "metric": "relit Mpix/s (sssgs_relight: sum over a precomputed reflectance field, PAPER.md L301)",
+        "value": P / (ms * 1e-3) / 1e6, "unit": "Mpix/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"OLAT stack of {L} frames {cam.width}x{cam.height} (frame shape of configs[{args.config - 1}])",
+                   "l2": "flushed between timed calls (256 MiB memset)"},
+        "gpu_launches": args.steps,
+        "roofline": {"kernel": "relight_vec_kernel", "bound": "hbm", "achieved": round(gbs, 1), "peak": peaks["hbm"],
+                     "unit": "GB/s", "frac": round(gbs / peaks["hbm"], 4), "traffic": None,
+                     "algorithmic_bytes": nbytes, "peak_source": peaks["source"]}}))
+
+
 def run_bake(args, local_rank):
     """--bake K: times sssgs_bake_visibility on the config's Gaussians, K Fibonacci directions.
     A side measurement: its JSON line has its own metric (rays/s) and is not the headline."""
@@ -637,6 +680,7 @@ def main():
                     help="BASELINE.json configs[C-1]; default 5 = the largest single-GPU configuration")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--relight", action="store_true", help="time sssgs_relight on an OLAT stack of the config's frame shape")
     ap.add_argument("--no-table", action="store_true", help="skip the per-config table (`configs`)")
     ap.add_argument("--canonical-lists", action="store_true",
                     help="render from the canonical tile lists instead of the tight ones (SSSGS_TIGHT_LISTS)")
@@ -657,6 +701,10 @@ def main():
     if args.bake:
         if rank == 0:
             run_bake(args, local_rank)
+        return
+    if args.relight:
+        if rank == 0:
+            run_relight(args, local_rank)
         return
     run_gpu(args, rank, world, local_rank)
 

@@ -372,6 +372,22 @@ int sssgs_render_backward(sssgs_ctx* ctx, const sssgs_gaussians* g, const sssgs_
 int sssgs_mlp_eval_static(int device, const sssgs_gaussians* g, const sssgs_mlp* mlp, const sssgs_camera* cam,
                           const sssgs_light* lights, int n_light, float* mlp_out, void* cuda_stream);
 
+/* Relighting from a precomputed reflectance field ("To speed up generation we can
+ * precompute a reflectance field assuming white light.  We compute the relit view as the sum over the reflectance
+ * field scaled by the environment illumination."):
+ *     out[p][c] = sum_{l < n_light} weights[l][c] * frames[l][p][c],      p < n_pixels, c = r, g, b
+ * frames  [n_light][n_pixels][3]: the OLAT frames of one view (sssgs_out.rgb of a render with white unit-intensity
+ *         lights; render them on a black background -- every frame carries its own (1 - A) bg term and the sum does
+ *         not remove it), DEVICE, 16-byte aligned;
+ * weights [n_light][3]: RGB radiance the environment sends from light l's direction, DEVICE;
+ * out     [n_pixels][3], DEVICE, 16-byte aligned, must not overlap frames.
+ * fp32, lights accumulated in order with fused multiply-adds.  One streaming kernel (12 (n_light + 1) n_pixels
+ * bytes of HBM traffic), no context, no scratch, no allocation; enqueues on the stream, never synchronises.  With
+ * n_light = 0 out is zeroed.  Errors (text via sssgs_last_error(NULL)): SSSGS_EINVAL, SSSGS_ECAPACITY (n_pixels >
+ * 2^40 / 12), SSSGS_EARCH, SSSGS_ECUDA.                                                                          */
+int sssgs_relight(int device, const float* frames, int n_light, int64_t n_pixels, const float* weights, float* out,
+                  void* cuda_stream);
+
 /* Per-stage device timing (measurement aid, off by default).  When enabled, sssgs_render
  * records CUDA events around each stage on the caller's stream (not capture-safe while on);
  * sssgs_profile_read synchronises those events and writes the milliseconds each stage of the

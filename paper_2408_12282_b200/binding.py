@@ -36,7 +36,7 @@ CNT_NVIS, CNT_INSTANCES, CNT_OVERFLOW, CNT_SORT_ERROR, CNT_MLP_ROWS = 0, 1, 2, 3
 EXPORTS = ["sssgs_workspace_bytes", "sssgs_create", "sssgs_destroy", "sssgs_render",
            "sssgs_render_host", "sssgs_last_launch_count", "sssgs_last_error",
            "sssgs_profile_enable", "sssgs_profile_read", "sssgs_bake_visibility", "sssgs_render_backward",
-           "sssgs_mlp_eval_static"]
+           "sssgs_mlp_eval_static", "sssgs_relight"]
 SSSGS_STATIC_SCRATCH_BYTES = 192 * 1024
 SSSGS_STATIC_MAX_LIGHTS = 8
 STAGES = ["pack", "project", "depth_sort", "emit", "tile_sort", "ranges", "mlp", "raster", "prepass"]
@@ -142,6 +142,8 @@ def lib() -> ctypes.CDLL:
         L.sssgs_mlp_eval_static.argtypes = [ctypes.c_int, ctypes.POINTER(sssgs_gaussians), ctypes.POINTER(sssgs_mlp),
                                             ctypes.POINTER(sssgs_camera), ctypes.POINTER(sssgs_light), ctypes.c_int,
                                             _vp, _vp]
+        L.sssgs_relight.restype = ctypes.c_int
+        L.sssgs_relight.argtypes = [ctypes.c_int, _vp, ctypes.c_int, ctypes.c_int64, _vp, _vp, _vp]
         L.sssgs_last_error.restype = ctypes.c_char_p
         L.sssgs_last_error.argtypes = [_vp]
         _lib = L
@@ -198,6 +200,14 @@ def sssgs_mlp_eval_static(device, g, mlp, cam, lights, n_light, mlp_out_ptr, str
     race on it.  Errors are reported through sssgs_last_error(NULL)."""
     rc = lib().sssgs_mlp_eval_static(int(device), ctypes.byref(g), ctypes.byref(mlp), ctypes.byref(cam), lights,
                                      int(n_light), _vp(mlp_out_ptr or 0), _vp(stream or 0))
+    if rc != SSSGS_OK:
+        raise SssgsError(rc, (lib().sssgs_last_error(None) or b"").decode())
+
+
+def sssgs_relight(device, frames_ptr, n_light, n_pixels, weights_ptr, out_ptr, stream=None) -> None:
+    """out[p][c] = sum_l weights[l][c] * frames[l][p][c]; device pointers, see include/sssgs.h."""
+    rc = lib().sssgs_relight(int(device), _vp(frames_ptr or 0), int(n_light), int(n_pixels), _vp(weights_ptr or 0),
+                             _vp(out_ptr or 0), _vp(stream or 0))
     if rc != SSSGS_OK:
         raise SssgsError(rc, (lib().sssgs_last_error(None) or b"").decode())
 

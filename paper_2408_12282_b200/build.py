@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsssgs.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["sssgs_api.cu", "k_project.cu", "k_sort.cu", "k_bin.cu", "k_raster.cu", "k_mlp.cu", "k_bvh.cu", "k_backward.cu"]
+SOURCES = ["sssgs_api.cu", "k_project.cu", "k_sort.cu", "k_bin.cu", "k_raster.cu", "k_mlp.cu", "k_bvh.cu", "k_backward.cu", "k_relight.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

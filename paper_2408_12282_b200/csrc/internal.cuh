@@ -316,4 +316,8 @@ int launch_mlp_backward(const sssgs_gaussians& g, const sssgs_mlp& mlp, const Ca
 
 int mlp_smem_bytes(const MlpPlan& plan);
 
+// reflectance-field relighting (k_relight.cu): out[p][c] = sum_l weights[l][c] frames[l][p][c]
+int launch_relight(const float* frames, int n_light, int64_t n_pixels, const float* weights, float* out, int num_sms,
+                   cudaStream_t s);
+
 }  // namespace sssgs

@@ -1106,3 +1106,32 @@ extern "C" int sssgs_mlp_eval_static(int device, const sssgs_gaussians* g, const
   if (e != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "sssgs_mlp_eval_static: CUDA error: %s", cudaGetErrorString(e));
   return SSSGS_OK;
 }
+
+// SURVEY 8(f).1, second half: relighting from a precomputed reflectance field.  Needs no context
+// and no scratch: a streaming sum over the OLAT stack.
+extern "C" int sssgs_relight(int device, const float* frames, int n_light, int64_t n_pixels, const float* weights,
+                             float* out, void* cuda_stream) {
+  if (n_light < 0 || n_pixels < 0) return fail(nullptr, SSSGS_EINVAL, "sssgs_relight: negative count");
+  if (n_pixels > ((int64_t)1 << 40) / 12) return fail(nullptr, SSSGS_ECAPACITY, "sssgs_relight: n_pixels too large");
+  if (n_pixels == 0) return SSSGS_OK;
+  if (!out || !aligned16(out)) return fail(nullptr, SSSGS_EINVAL, "sssgs_relight: out is NULL or not 16-byte aligned");
+  if (n_light > 0 && (!frames || !weights || !aligned16(frames)))
+    return fail(nullptr, SSSGS_EINVAL, "sssgs_relight: frames / weights NULL or frames not 16-byte aligned");
+  if (n_light > 0) {   // out must not overlap the stack it is computed from
+    const char* f0 = (const char*)frames;
+    const char* f1 = f0 + (size_t)n_light * n_pixels * 12;
+    const char* o0 = (const char*)out;
+    if (o0 < f1 && o0 + (size_t)n_pixels * 12 > f0) return fail(nullptr, SSSGS_EINVAL, "sssgs_relight: out overlaps frames");
+  }
+  DeviceGuard guard(device);
+  if (!guard.ok) return fail(nullptr, SSSGS_ECUDA, "sssgs_relight: cudaSetDevice(%d) failed", device);
+  int major = 0, sms = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess ||
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess)
+    return fail(nullptr, SSSGS_ECUDA, "sssgs_relight: cannot query device %d (libsssgs has no CPU fallback)", device);
+  if (major != 10) return fail(nullptr, SSSGS_EARCH, "sssgs_relight: device %d is sm_%dx; libsssgs is built for sm_100a only", device, major);
+  launch_relight(frames, n_light, n_pixels, weights, out, sms, (cudaStream_t)cuda_stream);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(nullptr, SSSGS_ECUDA, "sssgs_relight: CUDA error: %s", cudaGetErrorString(e));
+  return SSSGS_OK;
+}
